@@ -1,0 +1,233 @@
+/*
+ * ppl_oracle.c -- CPU oracle for the CCSD particle-particle ladder with Cholesky-decomposed ERIs.
+ *
+ * TEST INFRASTRUCTURE ONLY.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may build, load or call this file.  It shares no code with the CUDA path
+ * (paper_2603_20912_b200/) and neither includes nor is included by it.  Plain C, FP64, loops in
+ * the paper's order; no blocking, fusion or reordering beyond what the definition states.
+ *
+ * What it computes (the method reaches this definition exactly, up to FP64 summation order):
+ *
+ *     R[i,j,a,b] += sum_{c,d} ( sum_P L[P,a,c] * L[P,b,d] ) * t2[i,j,c,d]
+ *
+ *   - eq. (4)  PAPER.md:58   the pp-ladder term  sum_cd <ab|cd> t_ij^cd
+ *   - eq. (5)  PAPER.md:63   <ab|cd> ~= sum_x L^x_ac L^x_bd   (a pairs with c, b pairs with d;
+ *                            the printed summation index "r" is a garble for x -- reading A1/A2)
+ *   - eq. (6)  PAPER.md:68   t~_ij^ab = ... + sum_{x c d} L^x_ac L^x_bd t_ij^cd + ...
+ *   - einsum   PAPER.md:75   'xac,xbd,icjd->iajb'  (here stored as L[x,a,c], t2[i,j,c,d],
+ *                            R[i,j,a,b] -- BASELINE.json's layout, reading A3)
+ *   - route    PAPER.md:71-73, 118-120: the v^4-intermediate route, step 0 'xac,xbd->acbd'
+ *                            then step 1 'acbd,ecfd->efab', cost O(x v^4) + O(o^2 v^4)
+ *   - "+="     PAPER.md:177, 331 ("add to view of final result array"); coefficient 1 (A4, A5)
+ *
+ * Layouts: dense row-major, L[nchol][nvirt][nvirt], t2[nocc][nocc][nvirt][nvirt], R like t2.
+ * The oracle does NOT assume L[P,a,c] = L[P,c,a] nor t2 pair symmetry: it indexes exactly as
+ * written, so it stays valid for non-symmetric test inputs (reading A7).
+ *
+ * Pins (tests/test_oracle_pins.py, -m "not gpu"): brute force two ways on tiny sizes, a hand-worked
+ * 2x2 example (tests/golden/), nchol=1 triple product, identity-L and rank-1-L closed forms, unit
+ * impulse (index pairing), linearity / zero / accumulate, output pair symmetry with a negative
+ * control, exact-integer inputs against int64 arithmetic, numpy einsum, projection identity.
+ * Every entry point below is pinned; none is "parity unpinned".
+ */
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+int ppl_oracle_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* One (a,b) column of the two-step route:
+ *   step 0:  Wab[c][d] = sum_P L[P][a][c] * L[P][b][d]          (P ascending)
+ *   step 1:  out[ij]  += sum_{c,d} Wab[c][d] * t2[ij][c][d]      ((c,d) ascending)
+ * Wab is a caller-provided scratch of v*v doubles; out has stride out_stride between (i,j). */
+static void ladder_column(int o, int v, int x, const double *L, const double *t2, int a, int b,
+                          double *Wab, double *out, int64_t out_stride) {
+    const int64_t vv = (int64_t)v * v;
+    memset(Wab, 0, sizeof(double) * (size_t)vv);
+    for (int P = 0; P < x; ++P) {
+        const double *La = L + (int64_t)P * vv + (int64_t)a * v; /* L[P][a][:] */
+        const double *Lb = L + (int64_t)P * vv + (int64_t)b * v; /* L[P][b][:] */
+        for (int c = 0; c < v; ++c) {
+            const double lac = La[c];
+            double *Wc = Wab + (int64_t)c * v;
+            for (int d = 0; d < v; ++d) Wc[d] += lac * Lb[d];
+        }
+    }
+    const int64_t oo = (int64_t)o * o;
+    for (int64_t ij = 0; ij < oo; ++ij) {
+        const double *t = t2 + ij * vv;
+        double s = 0.0;
+        /* a fixed set of interleaved partial sums (the compiler's SIMD lanes): still one fixed
+         * summation order; any order is a valid evaluation of the definition (reading A13) */
+#pragma omp simd reduction(+ : s)
+        for (int64_t cd = 0; cd < vv; ++cd) s += Wab[cd] * t[cd];
+        out[ij * out_stride] += s;
+    }
+}
+
+/* R[i,j,a,b] += ladder term, every (a,b) column.  Columns write disjoint entries of R, so the
+ * OpenMP loop over (a,b) has no races. */
+int ppl_oracle_full(int nocc, int nvirt, int nchol, const double *L, const double *t2, double *R) {
+    if (nocc < 1 || nvirt < 1 || nchol < 1 || !L || !t2 || !R) return 1;
+    const int64_t vv = (int64_t)nvirt * nvirt;
+    int fail = 0;
+#pragma omp parallel
+    {
+        double *Wab = (double *)malloc(sizeof(double) * (size_t)vv);
+        if (!Wab) {
+#pragma omp atomic write
+            fail = 1;
+        }
+#pragma omp barrier
+        if (!fail) {
+#pragma omp for schedule(dynamic, 1)
+            for (int64_t ab = 0; ab < vv; ++ab) {
+                const int a = (int)(ab / nvirt), b = (int)(ab % nvirt);
+                ladder_column(nocc, nvirt, nchol, L, t2, a, b, Wab, R + ab, vv);
+            }
+        }
+        free(Wab);
+    }
+    return fail ? 3 : 0;
+}
+
+/* Rcols[p][ij] = ladder term at (a,b) = pairs[p] (bare term: Rcols is overwritten, not
+ * accumulated).  Used where the full oracle is unaffordable (large / XL configs). */
+int ppl_oracle_columns(int nocc, int nvirt, int nchol, const double *L, const double *t2,
+                       int64_t npairs, const int32_t *pairs, double *Rcols) {
+    if (nocc < 1 || nvirt < 1 || nchol < 1 || !L || !t2 || npairs < 0) return 1;
+    const int64_t vv = (int64_t)nvirt * nvirt, oo = (int64_t)nocc * nocc;
+    for (int64_t p = 0; p < npairs; ++p)
+        if (pairs[2 * p] < 0 || pairs[2 * p] >= nvirt || pairs[2 * p + 1] < 0 || pairs[2 * p + 1] >= nvirt)
+            return 1;
+    int fail = 0;
+#pragma omp parallel
+    {
+        double *Wab = (double *)malloc(sizeof(double) * (size_t)vv);
+        if (!Wab) {
+#pragma omp atomic write
+            fail = 1;
+        }
+#pragma omp barrier
+        if (!fail) {
+#pragma omp for schedule(dynamic, 1)
+            for (int64_t p = 0; p < npairs; ++p) {
+                double *out = Rcols + p * oo;
+                memset(out, 0, sizeof(double) * (size_t)oo);
+                ladder_column(nocc, nvirt, nchol, L, t2, pairs[2 * p], pairs[2 * p + 1], Wab, out, 1);
+            }
+        }
+        free(Wab);
+    }
+    return fail ? 3 : 0;
+}
+
+/* Brute force (i): materialise the whole W[a][c][b][d] = (ac|bd) (eq. 5) and contract it
+ * explicitly with t2 (eq. 4), six nested loops.  Tiny sizes only: v^4 doubles of memory. */
+int ppl_oracle_bruteforce_w(int nocc, int nvirt, int nchol, const double *L, const double *t2, double *R) {
+    const int64_t o = nocc, v = nvirt, x = nchol;
+    double *W = (double *)calloc((size_t)(v * v * v * v), sizeof(double));
+    if (!W) return 3;
+    for (int64_t a = 0; a < v; ++a)
+        for (int64_t c = 0; c < v; ++c)
+            for (int64_t b = 0; b < v; ++b)
+                for (int64_t d = 0; d < v; ++d) {
+                    double s = 0.0;
+                    for (int64_t P = 0; P < x; ++P) s += L[(P * v + a) * v + c] * L[(P * v + b) * v + d];
+                    W[((a * v + c) * v + b) * v + d] = s;
+                }
+    for (int64_t i = 0; i < o; ++i)
+        for (int64_t j = 0; j < o; ++j)
+            for (int64_t a = 0; a < v; ++a)
+                for (int64_t b = 0; b < v; ++b) {
+                    double s = 0.0;
+                    for (int64_t c = 0; c < v; ++c)
+                        for (int64_t d = 0; d < v; ++d)
+                            s += W[((a * v + c) * v + b) * v + d] * t2[((i * o + j) * v + c) * v + d];
+                    R[((i * o + j) * v + a) * v + b] += s;
+                }
+    free(W);
+    return 0;
+}
+
+/* Brute force (ii): the direct seven-index sum of eq. (6), no intermediate at all, accumulated in
+ * long double (x87 80-bit on x86-64): an independent, more accurate value that also bounds the
+ * oracle's own rounding error.  Cost O(x o^2 v^4): tiny sizes only. */
+int ppl_oracle_bruteforce_direct(int nocc, int nvirt, int nchol, const double *L, const double *t2, double *R) {
+    const int64_t o = nocc, v = nvirt, x = nchol;
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int64_t i = 0; i < o; ++i)
+        for (int64_t j = 0; j < o; ++j)
+            for (int64_t a = 0; a < v; ++a)
+                for (int64_t b = 0; b < v; ++b) {
+                    long double s = 0.0L;
+                    for (int64_t P = 0; P < x; ++P)
+                        for (int64_t c = 0; c < v; ++c)
+                            for (int64_t d = 0; d < v; ++d)
+                                s += (long double)L[(P * v + a) * v + c] * (long double)L[(P * v + b) * v + d] *
+                                     (long double)t2[((i * o + j) * v + c) * v + d];
+                    R[((i * o + j) * v + a) * v + b] += (double)s;
+                }
+    return 0;
+}
+
+/* Projection (Freivalds-style) of the definition, for full-coverage checks at sizes where the
+ * full oracle is unaffordable:
+ *     sum_{a,b} u[a] w[b] R[i,j,a,b] = sum_{c,d} M[c,d] t2[i,j,c,d],
+ *     M[c,d] = sum_P (sum_a u[a] L[P,a,c]) (sum_b w[b] L[P,b,d])
+ * which follows from eq. (6) by linearity.  out[ij] is overwritten.  Also returns
+ * absout[ij] = sum_cd |M[c,d]| |t2[ij,c,d]| if absout != NULL (a scale for error bounds).
+ * long double throughout; cost O(x v^2 + o^2 v^2). */
+int ppl_oracle_project(int nocc, int nvirt, int nchol, const double *L, const double *t2, const double *u,
+                       const double *w, double *out, double *absout) {
+    const int64_t o = nocc, v = nvirt, x = nchol, vv = v * v, oo = o * o;
+    long double *M = (long double *)calloc((size_t)vv, sizeof(long double));
+    if (!M) return 3;
+#pragma omp parallel
+    {
+        long double *Ml = (long double *)calloc((size_t)vv, sizeof(long double));
+        long double *uL = (long double *)malloc(sizeof(long double) * (size_t)v);
+        long double *wL = (long double *)malloc(sizeof(long double) * (size_t)v);
+#pragma omp for schedule(static)
+        for (int64_t P = 0; P < x; ++P) {
+            for (int64_t c = 0; c < v; ++c) {
+                long double su = 0.0L, sw = 0.0L;
+                for (int64_t a = 0; a < v; ++a) {
+                    su += (long double)u[a] * (long double)L[(P * v + a) * v + c];
+                    sw += (long double)w[a] * (long double)L[(P * v + a) * v + c];
+                }
+                uL[c] = su;
+                wL[c] = sw;
+            }
+            for (int64_t c = 0; c < v; ++c)
+                for (int64_t d = 0; d < v; ++d) Ml[c * v + d] += uL[c] * wL[d];
+        }
+#pragma omp critical
+        for (int64_t k = 0; k < vv; ++k) M[k] += Ml[k];
+        free(Ml);
+        free(uL);
+        free(wL);
+    }
+#pragma omp parallel for schedule(static)
+    for (int64_t ij = 0; ij < oo; ++ij) {
+        long double s = 0.0L, sa = 0.0L;
+        for (int64_t k = 0; k < vv; ++k) {
+            long double p = M[k] * (long double)t2[ij * vv + k];
+            s += p;
+            sa += p < 0 ? -p : p;
+        }
+        out[ij] = (double)s;
+        if (absout) absout[ij] = (double)sa;
+    }
+    free(M);
+    return 0;
+}

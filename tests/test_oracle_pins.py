@@ -1,0 +1,268 @@
+"""Pins for the CPU oracle (oracle/ppl_oracle.c) -- CPU only, no GPU, no CUDA path.
+
+The paper prints no worked numerical example of the ladder term, so the oracle is pinned to what
+the paper's equations and the mathematics fix:
+
+  hand-worked 2x2 example of eq. (6)                    tests/golden/hand_2x2.txt
+  brute force, two ways (explicit W; 7-index long double)   P1   (north_star i)
+  nchol = 1  ->  R_ij = L0 T_ij L0^T (library matmul)        P2   (north_star v)
+  identity L ->  R = (sum s_P^2) t2                          P3
+  rank-1 L   ->  closed form                                 P4
+  unit impulse -> R[i0,j0,a,b] = sum_P L[P,a,c0] L[P,b,d0]   P5   (pairing a-c, b-d: reading A2)
+  linearity, zero, accumulate semantics                      P6   (north_star ii, iii)
+  output pair symmetry + negative control                    P7   (north_star iv)
+  projection identity (oracle.project vs oracle.full)        P8
+  exact integers vs int64 arithmetic, bit for bit            P9
+  numpy einsum 'Pac,Pbd,ijcd->ijab' and the paper's two-step tensordot  P10
+
+Each pin is chosen so that a plausible mistake (dropped term, wrong sign or index, transposed
+operand, wrong pairing, overwrite instead of accumulate) fails at least one of them.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import ppl_inputs as I
+
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+RTOL = 1e-13  # oracle vs another FP64 evaluation order: ~1e-15 expected, 1e-13 asserted
+
+ODD_SHAPES = [(1, 1, 1), (2, 1, 3), (1, 5, 1), (3, 7, 5), (2, 9, 4), (3, 6, 7)]
+
+
+def rel(a, b):
+    m = np.abs(b).max()
+    return np.abs(a - b).max() / (m if m > 0 else 1.0)
+
+
+def rand_inputs(o, v, x, seed=1, symmetric=False, integer=False):
+    return I.make_L(v, x, seed, symmetric, integer), I.make_t2(o, v, seed, symmetric, integer)
+
+
+# ----------------------------------------------------------------------------- golden fixtures
+def _read_hand():
+    d = {}
+    for line in open(os.path.join(GOLD, "hand_2x2.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        k, *vals = line.split()
+        d[k] = np.array([float(s) for s in vals])
+    return d
+
+
+@pytest.mark.parametrize("fn", ["full", "bruteforce_w", "bruteforce_direct", "columns", "project"])
+def test_hand_worked_2x2(fn):
+    """eq. (6), by hand; non-symmetric L and t so the pairing and operand order matter."""
+    d = _read_hand()
+    L = d["L"].reshape(1, 2, 2).copy()
+    t2 = d["t2"].reshape(1, 1, 2, 2).copy()
+    want, bad = d["R"].reshape(2, 2), d["Rbad"].reshape(2, 2)
+    if fn == "columns":
+        pairs = [(0, 0), (0, 1), (1, 0), (1, 1)]
+        got = oracle.columns(L, t2, pairs).reshape(2, 2)
+    elif fn == "project":
+        got = np.empty((2, 2))
+        for a in range(2):
+            for b in range(2):
+                got[a, b] = oracle.project(L, t2, np.eye(2)[a], np.eye(2)[b])[0][0, 0]
+    else:
+        got = getattr(oracle, fn)(L, t2)[0, 0]
+    assert np.array_equal(got, want)  # small integers: exact
+    assert not np.array_equal(got, bad)
+
+
+def test_golden_tiny_samples():
+    """Regression anchor: entries of config 0 written by tests/golden/make_golden.py (oracle only)."""
+    L, t2 = I.make_config("tiny", seed=0)
+    R = oracle.full(L, t2)
+    n = 0
+    for line in open(os.path.join(GOLD, "oracle_tiny_samples.txt")):
+        if line.startswith("#"):
+            continue
+        i, j, a, b, hx, _ = line.split()
+        want = float.fromhex(hx)
+        assert abs(R[int(i), int(j), int(a), int(b)] - want) <= 1e-12 * 21.65
+        n += 1
+    assert n == 7
+
+
+# ----------------------------------------------------------------------------- P1 brute force
+@pytest.mark.parametrize("shape", [(5, 20, 60)] + ODD_SHAPES)
+@pytest.mark.parametrize("symmetric", [True, False])
+def test_P1_bruteforce(shape, symmetric):
+    o, v, x = shape
+    L, t2 = rand_inputs(o, v, x, seed=3, symmetric=symmetric)
+    R = oracle.full(L, t2)
+    assert rel(R, oracle.bruteforce_w(L, t2)) <= RTOL
+    assert rel(R, oracle.bruteforce_direct(L, t2)) <= RTOL
+
+
+def test_P1_columns_equal_full():
+    L, t2 = rand_inputs(3, 11, 9, seed=5)
+    R = oracle.full(L, t2)
+    pairs = [(a, b) for a in range(11) for b in range(11)]
+    C = oracle.columns(L, t2, pairs)  # [121, 3, 3]
+    assert np.array_equal(C.reshape(11, 11, 3, 3).transpose(2, 3, 0, 1), R)  # same code path, same order
+
+
+# ----------------------------------------------------------------------------- P2 nchol = 1
+@pytest.mark.parametrize("shape", [(5, 20, 1), (5, 53, 1), (2, 7, 1)])
+def test_P2_nchol1_triple_product(shape):
+    o, v, _ = shape
+    L, t2 = rand_inputs(o, v, 1, seed=7, symmetric=False)
+    R = oracle.full(L, t2)
+    want = np.matmul(np.matmul(L[0], t2), L[0].T)  # R_ij = L0 T_ij L0^T  (textbook triple product)
+    assert rel(R, want) <= RTOL
+    # transposed operand must fail (the test has power)
+    assert rel(R, np.matmul(np.matmul(L[0].T, t2), L[0])) > 1e-3
+
+
+# ----------------------------------------------------------------------------- P3 identity L
+def test_P3_identity_L():
+    o, v, x = 4, 13, 6
+    s = np.arange(1, x + 1, dtype=np.float64) * 0.5
+    L = np.ascontiguousarray(s[:, None, None] * np.eye(v)[None])
+    t2 = I.make_t2(o, v, 11, symmetric=False)
+    R = oracle.full(L, t2)
+    assert rel(R, (s**2).sum() * t2) <= RTOL
+
+
+# ----------------------------------------------------------------------------- P4 rank-1 L
+def test_P4_rank1_L():
+    o, v, x = 3, 17, 5
+    al = I.make_vec(x, 1, 20)
+    u = I.make_vec(v, 1, 21)
+    L = np.ascontiguousarray(al[:, None, None] * u[None, :, None] * u[None, None, :])
+    t2 = I.make_t2(o, v, 13, symmetric=False)
+    R = oracle.full(L, t2)
+    utu = np.einsum("c,ijcd,d->ij", u, t2, u)
+    want = (al**2).sum() * utu[:, :, None, None] * u[None, None, :, None] * u[None, None, None, :]
+    assert rel(R, want) <= RTOL
+
+
+# ----------------------------------------------------------------------------- P5 unit impulse
+def test_P5_impulse_pins_index_pairing():
+    o, v, x = 3, 8, 6
+    L = I.make_L(v, x, 17, symmetric=False)
+    i0, j0, c0, d0 = 1, 2, 3, 5
+    t2 = np.zeros((o, o, v, v))
+    t2[i0, j0, c0, d0] = 1.0
+    R = oracle.full(L, t2)
+    want = np.einsum("Pa,Pb->ab", L[:, :, c0], L[:, :, d0])  # sum_P L[P,a,c0] L[P,b,d0]
+    assert rel(R[i0, j0], want) <= RTOL
+    wrong = np.einsum("Pa,Pb->ab", L[:, :, d0], L[:, :, c0])  # (ad|bc) pairing
+    assert rel(R[i0, j0], wrong) > 1e-3
+    mask = np.ones((o, o), bool)
+    mask[i0, j0] = False
+    assert np.all(R[mask] == 0.0)  # no cross-talk between (i,j) blocks
+
+
+# ----------------------------------------------------------------------------- P6 linearity / zero / accumulate
+def test_P6_linearity_zero_accumulate():
+    o, v, x = 3, 9, 7
+    L = I.make_L(v, x, 19, symmetric=False)
+    t = I.make_t2(o, v, 19, symmetric=False)
+    tp = I.make_t2(o, v, 23, symmetric=False)
+    al, be = 0.75, -1.5
+    lhs = oracle.full(L, al * t + be * tp)
+    rhs = al * oracle.full(L, t) + be * oracle.full(L, tp)
+    assert rel(lhs, rhs) <= RTOL
+    # zero t2 leaves R bitwise unchanged
+    R0 = I.make_t2(o, v, 29, symmetric=False)
+    R = R0.copy()
+    oracle.full(L, np.zeros_like(t), R)
+    assert np.array_equal(R, R0)
+    # accumulate (+=, coefficient 1): R_in + term, and calling twice adds twice
+    R = R0.copy()
+    oracle.full(L, t, R)
+    term = oracle.full(L, t)
+    assert rel(R - R0, term) <= 1e-12
+    oracle.full(L, t, R)
+    assert rel(R - R0, 2 * term) <= 1e-12
+
+
+# ----------------------------------------------------------------------------- P7 output symmetry
+def test_P7_pair_symmetry_and_negative_control():
+    o, v, x = 4, 10, 8
+    L = I.make_L(v, x, 31, symmetric=False)  # holds for ANY L
+    ts = I.make_t2(o, v, 31, symmetric=True)
+    assert np.array_equal(ts, ts.transpose(1, 0, 3, 2))
+    R = oracle.full(L, ts)
+    assert rel(R, R.transpose(1, 0, 3, 2)) <= RTOL
+    tn = I.make_t2(o, v, 31, symmetric=False)
+    Rn = oracle.full(L, tn)
+    assert rel(Rn, Rn.transpose(1, 0, 3, 2)) > 1e-3  # non-symmetric t2 breaks it
+
+
+# ----------------------------------------------------------------------------- P8 projection
+@pytest.mark.parametrize("shape", [(5, 20, 60), (3, 7, 5)])
+def test_P8_projection_matches_full(shape):
+    o, v, x = shape
+    L, t2 = rand_inputs(o, v, x, seed=37, symmetric=False)
+    R = oracle.full(L, t2)
+    for k in range(4):
+        u, w = I.make_vec(v, 37, 40 + 2 * k), I.make_vec(v, 37, 41 + 2 * k)
+        got, scale = oracle.project(L, t2, u, w)
+        want = np.einsum("a,ijab,b->ij", u, R, w)
+        assert np.abs(got - want).max() <= 1e-13 * scale.max()
+    # and against an independent numpy evaluation of the identity's right-hand side
+    u, w = I.make_vec(v, 37, 50), I.make_vec(v, 37, 51)
+    M = np.einsum("Pc,Pd->cd", np.einsum("a,Pac->Pc", u, L), np.einsum("b,Pbd->Pd", w, L))
+    got, _ = oracle.project(L, t2, u, w)
+    assert rel(got, np.einsum("cd,ijcd->ij", M, t2)) <= RTOL
+
+
+# ----------------------------------------------------------------------------- P9 exact integers
+@pytest.mark.parametrize("shape", [(5, 20, 60), (3, 7, 5), (5, 53, 16)])
+def test_P9_exact_integers(shape):
+    o, v, x = shape
+    L, t2 = rand_inputs(o, v, x, seed=41, symmetric=True, integer=True)
+    Li, ti = L.astype(np.int64), t2.astype(np.int64)
+    W = np.einsum("Pac,Pbd->abcd", Li, Li)
+    want = np.einsum("abcd,ijcd->ijab", W, ti)  # int64: exact
+    for fn in (oracle.full, oracle.bruteforce_direct):
+        if fn is oracle.bruteforce_direct and v > 20:
+            continue
+        got = fn(L, t2)
+        assert np.array_equal(got, want.astype(np.float64))  # bit for bit, any summation order
+
+
+# ----------------------------------------------------------------------------- P10 other opinions
+@pytest.mark.parametrize("name", ["tiny", "small"])
+def test_P10_numpy_einsum_and_paper_tensordot(name):
+    L, t2 = I.make_config(name, seed=0)
+    R = oracle.full(L, t2)
+    if name == "tiny":  # numpy's einsum path is slow (no BLAS) beyond tiny sizes
+        assert rel(R, np.einsum("Pac,Pbd,ijcd->ijab", L, L, t2, optimize=True)) <= RTOL
+    # the paper's two steps with its axes: tensordot over x, then over (c,d)
+    W = np.tensordot(L, L, axes=(0, 0))  # [a,c,b,d]
+    out = np.tensordot(W, t2, axes=([1, 3], [2, 3]))  # [a,b,i,j]
+    assert rel(R, out.transpose(2, 3, 0, 1)) <= RTOL
+
+
+def test_oracle_self_error_bound():
+    """The FP64 oracle vs the long-double 7-index sum on config 0: its own rounding error, which
+    the 1e-11 GPU tolerance must dominate by orders of magnitude (reading A13)."""
+    L, t2 = I.make_config("tiny", seed=0)
+    assert rel(oracle.full(L, t2), oracle.bruteforce_direct(L, t2)) <= 1e-14
+
+
+# ----------------------------------------------------------------------------- input recipe
+def test_input_recipe():
+    """BASELINE.json configs: symmetric L with exp(-3P/nchol) decay, t2 ~ N(0,1e-2) pair-symmetric."""
+    o, v, x = 5, 53, 232
+    L, t2 = I.make_config("small", seed=0)
+    assert L.shape == (x, v, v) and t2.shape == (o, o, v, v)
+    assert np.array_equal(L, L.transpose(0, 2, 1))
+    assert np.array_equal(t2, t2.transpose(1, 0, 3, 2))
+    assert abs(t2.std() - 0.1) < 0.003 and abs(t2.mean()) < 0.003
+    sd = L.reshape(x, -1).std(axis=1)
+    want = np.exp(-3.0 * np.arange(x) / x)
+    assert np.all(np.abs(sd / want - 1.0) < 0.08)
+    # seeded and reproducible; different seeds differ
+    assert np.array_equal(L, I.make_L(v, x, 0))
+    assert not np.array_equal(L, I.make_L(v, x, 1))
+    p = I.sample_pairs(400, 64, seed=0)
+    assert p.min() >= 0 and p.max() < 400 and len({tuple(r) for r in p}) == len(p)
