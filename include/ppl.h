@@ -1,0 +1,158 @@
+/*
+ * ppl.h -- C ABI of libppl: the CCSD particle-particle ladder contraction with
+ * Cholesky-decomposed ERIs on one NVIDIA B200 (sm_100a), FP64.
+ *
+ *     R[i,j,a,b] += sum_{c,d} (ac|bd) * t2[i,j,c,d],      (ac|bd) = sum_P L[P,a,c] * L[P,b,d]
+ *
+ * Source of the operation (arxiv/paper_2603_20912, line numbers in /root/reference/PAPER.md):
+ *   eq. (4) l.58   pp-ladder term  sum_cd <ab|cd> t_ij^cd, the O(o^2 v^4) bottleneck of CCD/CCSD
+ *   eq. (5) l.63   <ab|cd> ~= sum_x L^x_ac L^x_bd  (one L array serves both factors, l.66)
+ *   eq. (6) l.68   t~_ij^ab = ... + sum_{x,c,d} L^x_ac L^x_bd t_ij^cd + ...
+ *   l.71-73, 118-120   evaluated through the v^4 intermediate in two steps:
+ *                      step 0 'xac,xbd->acbd'   (GEMM over the Cholesky index x = P)
+ *                      step 1 'acbd,ecfd->efab' (GEMM over (c,d)), result ACCUMULATED (l.177, 331)
+ * The v^4 intermediate W = (ac|bd) is never stored whole: it is produced one (a-block x b-block
+ * x all c,d) tile at a time into a ring in the plan's workspace and consumed at once.
+ *
+ * Conventions
+ *   - All arrays are dense, row-major FP64 (IEEE binary64) with no strides:
+ *         L [nchol][nvirt][nvirt]            Cholesky vectors, L[P][a][c]
+ *         t2[nocc][nocc][nvirt][nvirt]       amplitudes,       t2[i][j][c][d]
+ *         R [nocc][nocc][nvirt][nvirt]       result,           R[i][j][a][b]   (in/out)
+ *   - Semantics: accumulate, coefficient exactly 1 (eq. 6 has no prefactor).  The caller zeroes R
+ *     if it wants the bare term.  R must not alias L or t2.
+ *   - Ownership: the plan owns its workspace, internal stream and events.  L, t2, R are borrowed.
+ *   - Errors: every entry point returns a PPL_* code (ppl_plan returns NULL and records the code
+ *     for ppl_last_error()).  No exceptions, no exit(), NO CPU FALLBACK: on anything but a
+ *     compute-capability 10.x device the library refuses (PPL_ERR_UNSUPPORTED_DEVICE).
+ *   - Threading: one in-flight ppl_apply per plan (the workspace is shared); distinct plans are
+ *     independent.  ppl_last_error() is per thread.
+ */
+#ifndef PPL_H
+#define PPL_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ppl_plan_s ppl_plan_t; /* opaque */
+
+enum {
+    PPL_OK = 0,
+    PPL_ERR_INVALID_ARG = 1,         /* NULL / non-positive dimension / misaligned pointer */
+    PPL_ERR_WORKSPACE_TOO_SMALL = 2, /* workspace_bytes below the minimum plan */
+    PPL_ERR_ALLOC = 3,               /* cudaMalloc / host allocation failed */
+    PPL_ERR_CUDA = 4,                /* a CUDA runtime call or kernel launch failed */
+    PPL_ERR_UNSUPPORTED_DEVICE = 5,  /* no CUDA device, or not compute capability 10.x */
+    PPL_ERR_PRECONDITION = 6         /* ppl_check_inputs: a symmetry the plan relies on is violated */
+};
+
+/* Symmetry modes (ppl_plan_set_symmetry). */
+enum {
+    PPL_SYM_NONE = 0, /* general t2: every (a-block, b-block) tile is computed */
+    PPL_SYM_PAIR = 1  /* t2[i,j,c,d] == t2[j,i,d,c] (holds for CC amplitudes): then
+                         R_term[i,j,a,b] == R_term[j,i,b,a] for ANY L, so only tiles with
+                         a-block <= b-block are computed and the result is also accumulated into
+                         the mirrored entries.  Default.  Result undefined if t2 is not
+                         pair-symmetric (ppl_check_inputs detects that). */
+};
+
+/* What the planner chose; filled by ppl_plan_info.  Flop counts follow BASELINE.json:
+ * F_nom = 2*nchol*nvirt^4 + 2*nocc^2*nvirt^4; F_exec counts the tiles actually executed. */
+typedef struct ppl_info_s {
+    int32_t nocc, nvirt, nchol;
+    int32_t symmetry;          /* PPL_SYM_* */
+    int32_t ta, tb;            /* tile edge lengths along a and b (virtual indices per block) */
+    int32_t n_ablocks, n_bblocks;
+    int32_t n_tiles;           /* tiles executed per apply */
+    int32_t ring;              /* W-tile ring depth */
+    int32_t splitk;            /* split-K factor of step 1 (the (c,d) contraction) */
+    int32_t vec16;             /* 1: 16-byte async copies (nvirt even); 0: 8-byte path */
+    int32_t launches_per_apply;/* kernels launched by one ppl_apply */
+    int32_t reserved;
+    uint64_t workspace_bytes;  /* device bytes owned by the plan */
+    double flops_nominal;      /* F_nom */
+    double flops_executed;     /* F_exec: step 0 + step 1 over executed tiles (incl. tile padding: none) */
+    double flops_step0;        /* executed flops of step 0 ('xac,xbd->acbd') */
+    double flops_step1;        /* executed flops of step 1 ('acbd,ecfd->efab') */
+} ppl_info_t;
+
+/* Per-stage device times of the most recent profiled apply (ppl_apply_profiled), milliseconds. */
+typedef struct ppl_times_s {
+    float total_ms;
+    float step0_ms;  /* sum over tiles of the W-tile generation kernel */
+    float step1_ms;  /* sum over tiles of the (c,d) contraction kernel */
+    float reduce_ms; /* sum over tiles of the split-K reduction + accumulate + mirror kernel */
+    int32_t n_step0, n_step1, n_reduce; /* launches */
+} ppl_times_t;
+
+/* ppl_plan: choose tile shape, ring depth and split-K for (nocc, nvirt, nchol) and allocate the
+ * device workspace once (the analogue of the paper's memory functions, Table 1 l.99-116, and of
+ * its "avoid cudaMalloc per batch" remark l.340-342).
+ *   nocc, nvirt, nchol >= 1.
+ *   workspace_bytes: CAP on device memory the plan may allocate. 0 = automatic (what the
+ *     preferred plan needs, at most 90 % of currently free device memory -- cf. the paper's
+ *     avail*0.98*0.9, l.107).  If the cap is below the minimum plan (one (a,b) column of W plus
+ *     reduction scratch) -> NULL with PPL_ERR_WORKSPACE_TOO_SMALL.
+ * Uses the current CUDA device.  Returns NULL on failure (see ppl_last_error). */
+ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes);
+
+/* ppl_apply: enqueue  R += ladder(L, t2)  on `stream` (a cudaStream_t passed as void*; NULL =
+ * the legacy default stream).  Asynchronous: returns once the work is queued.  All effects are
+ * ordered after prior work on `stream` and complete before later work on `stream` (an internal
+ * producer stream is forked and joined with events).
+ *   L, t2, R: DEVICE pointers, layouts above, 8-byte aligned (16-byte aligned enables the fast
+ *   copy path when nvirt is even; torch allocations are 512-byte aligned).  They must stay valid
+ *   until the queued work completes. */
+int ppl_apply(ppl_plan_t *plan, const double *L, const double *t2, double *R, void *stream);
+
+/* ppl_apply_host: the same operation on HOST buffers (pageable or pinned): copies L and t2 to
+ * plan-owned device buffers, R in, runs ppl_apply, copies R back, and synchronises before
+ * returning.  Device staging buffers are allocated on first use and kept by the plan (they are
+ * not counted against workspace_bytes).  h2d/d2h byte counts are returned if non-NULL. */
+int ppl_apply_host(ppl_plan_t *plan, const double *L_host, const double *t2_host, double *R_host,
+                   uint64_t *h2d_bytes, uint64_t *d2h_bytes);
+
+/* ppl_apply_profiled: like ppl_apply but serialises the stages on `stream`, brackets every
+ * kernel with CUDA events, synchronises, and fills *times.  For measurement only. */
+int ppl_apply_profiled(ppl_plan_t *plan, const double *L, const double *t2, double *R, void *stream,
+                       ppl_times_t *times);
+
+/* ppl_destroy: free the workspace, stream and events.  NULL is a no-op returning PPL_OK.
+ * Synchronises the plan's internal stream first. */
+int ppl_destroy(ppl_plan_t *plan);
+
+/* ---- small extras ------------------------------------------------------------------------- */
+
+int ppl_last_error(void);                /* code of the last failure on this thread */
+const char *ppl_error_string(int code);  /* static string, never NULL */
+
+/* Set PPL_SYM_NONE / PPL_SYM_PAIR (default PPL_SYM_PAIR).  Re-plans the tile list; must not be
+ * called while an apply is in flight. */
+int ppl_plan_set_symmetry(ppl_plan_t *plan, int mode);
+
+int ppl_plan_info(const ppl_plan_t *plan, ppl_info_t *out);
+
+/* Debug: verify on the device that L[P,a,c]==L[P,c,a] (reported, not required) and, in
+ * PPL_SYM_PAIR mode, that t2[i,j,c,d]==t2[j,i,d,c] (required).  Synchronises `stream`.
+ * Returns PPL_OK, or PPL_ERR_PRECONDITION if t2 violates the symmetry the plan relies on.
+ * If flags != NULL: bit 0 = L not symmetric, bit 1 = t2 not pair-symmetric. */
+int ppl_check_inputs(ppl_plan_t *plan, const double *L, const double *t2, void *stream, int *flags);
+
+/* Measure the FP64 tensor (DMMA, mma.sync.m8n8k4.f64) issue-rate peak of the current device
+ * with a register-only kernel: the roofline denominator used by bench.py.  Writes TFLOP/s
+ * (best of `reps` launches of about `ms_target` milliseconds each).  Synchronises. */
+int ppl_probe_fp64_peak(double *tflops, int reps, double ms_target);
+
+/* Test hook: C(8x8) = A(8x4, row-major) * B(4x8, row-major) through ONE mma.sync.m8n8k4.f64 using
+ * the fragment layout the kernels assume (lane = 4g+q: a=A[g][q], b=B[q][g], c={C[g][2q],
+ * C[g][2q+1]}).  All three are DEVICE pointers.  Synchronises the device. */
+int ppl_debug_dmma_layout(const double *A_dev, const double *B_dev, double *C_dev);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PPL_H */

@@ -1,0 +1,232 @@
+"""Thin ctypes binding of libppl (include/ppl.h): argument marshalling only.
+
+Every step of the path (W-tile generation, (c,d) contraction, reduction/mirror) runs in the CUDA
+kernels behind the C ABI.  PyTorch is used for FP64 device buffers and streams, nothing else.
+There is no CPU fallback: if the library is missing or the device is not a B200-class GPU the
+calls raise.  Function names mirror the C ABI (ppl_plan, ppl_apply, ppl_destroy, ...).
+"""
+from __future__ import annotations
+
+import ctypes
+from ctypes import POINTER, c_char_p, c_double, c_float, c_int, c_int32, c_size_t, c_uint64, c_void_p
+
+from . import _build
+
+PPL_OK = 0
+PPL_ERR_INVALID_ARG = 1
+PPL_ERR_WORKSPACE_TOO_SMALL = 2
+PPL_ERR_ALLOC = 3
+PPL_ERR_CUDA = 4
+PPL_ERR_UNSUPPORTED_DEVICE = 5
+PPL_ERR_PRECONDITION = 6
+PPL_SYM_NONE = 0
+PPL_SYM_PAIR = 1
+
+
+class ppl_info_t(ctypes.Structure):
+    _fields_ = [
+        ("nocc", c_int32), ("nvirt", c_int32), ("nchol", c_int32), ("symmetry", c_int32),
+        ("ta", c_int32), ("tb", c_int32), ("n_ablocks", c_int32), ("n_bblocks", c_int32),
+        ("n_tiles", c_int32), ("ring", c_int32), ("splitk", c_int32), ("vec16", c_int32),
+        ("launches_per_apply", c_int32), ("reserved", c_int32),
+        ("workspace_bytes", c_uint64),
+        ("flops_nominal", c_double), ("flops_executed", c_double),
+        ("flops_step0", c_double), ("flops_step1", c_double),
+    ]
+
+    def asdict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_ if k != "reserved"}
+
+
+class ppl_times_t(ctypes.Structure):
+    _fields_ = [
+        ("total_ms", c_float), ("step0_ms", c_float), ("step1_ms", c_float), ("reduce_ms", c_float),
+        ("n_step0", c_int32), ("n_step1", c_int32), ("n_reduce", c_int32),
+    ]
+
+    def asdict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class PplError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: {error_string(code)} (PPL error {code})")
+
+
+# Every symbol include/ppl.h declares: (restype, argtypes)
+SYMBOLS = {
+    "ppl_plan": (c_void_p, [c_int, c_int, c_int, c_size_t]),
+    "ppl_apply": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "ppl_apply_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, POINTER(c_uint64), POINTER(c_uint64)]),
+    "ppl_apply_profiled": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, POINTER(ppl_times_t)]),
+    "ppl_destroy": (c_int, [c_void_p]),
+    "ppl_last_error": (c_int, []),
+    "ppl_error_string": (c_char_p, [c_int]),
+    "ppl_plan_set_symmetry": (c_int, [c_void_p, c_int]),
+    "ppl_plan_info": (c_int, [c_void_p, POINTER(ppl_info_t)]),
+    "ppl_check_inputs": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, POINTER(c_int)]),
+    "ppl_probe_fp64_peak": (c_int, [POINTER(c_double), c_int, c_double]),
+    "ppl_debug_dmma_layout": (c_int, [c_void_p, c_void_p, c_void_p]),
+}
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libppl.so (building it in-tree with nvcc if stale).  Raises if that is impossible."""
+    global _lib
+    if _lib is None:
+        so = _build.build()
+        L = ctypes.CDLL(so)
+        for name, (res, args) in SYMBOLS.items():
+            fn = getattr(L, name)  # AttributeError if the ABI is incomplete
+            fn.restype = res
+            fn.argtypes = args
+        _lib = L
+    return _lib
+
+
+def library_path() -> str:
+    return _build.SO
+
+
+def error_string(code: int) -> str:
+    return lib().ppl_error_string(code).decode()
+
+
+def ppl_last_error() -> int:
+    return int(lib().ppl_last_error())
+
+
+def _check(rc: int, where: str):
+    if rc != PPL_OK:
+        raise PplError(rc, where)
+
+
+def _dev_ptr(t, name: str, shape=None):
+    import torch
+
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
+        raise TypeError(f"{name}: need a contiguous CUDA float64 tensor")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise ValueError(f"{name}: shape {tuple(t.shape)} != {tuple(shape)}")
+    return c_void_p(t.data_ptr())
+
+
+def _stream_ptr(stream):
+    import torch
+
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+
+
+class Plan:
+    """Owner of an opaque ppl_plan_t* (workspace, internal stream, events)."""
+
+    def __init__(self, nocc: int, nvirt: int, nchol: int, workspace_bytes: int = 0):
+        h = lib().ppl_plan(int(nocc), int(nvirt), int(nchol), int(workspace_bytes))
+        if not h:
+            raise PplError(ppl_last_error(), "ppl_plan")
+        self._h = c_void_p(h)
+        self.nocc, self.nvirt, self.nchol = int(nocc), int(nvirt), int(nchol)
+
+    # -- C ABI mirrors -------------------------------------------------------------------------
+    def apply(self, L, t2, R, stream=None):
+        """R += ladder(L, t2), asynchronously on `stream` (default: torch's current stream)."""
+        o, v, x = self.nocc, self.nvirt, self.nchol
+        _check(lib().ppl_apply(self._h, _dev_ptr(L, "L", (x, v, v)), _dev_ptr(t2, "t2", (o, o, v, v)),
+                               _dev_ptr(R, "R", (o, o, v, v)), _stream_ptr(stream)), "ppl_apply")
+        return R
+
+    def apply_profiled(self, L, t2, R, stream=None) -> dict:
+        o, v, x = self.nocc, self.nvirt, self.nchol
+        t = ppl_times_t()
+        _check(lib().ppl_apply_profiled(self._h, _dev_ptr(L, "L", (x, v, v)), _dev_ptr(t2, "t2", (o, o, v, v)),
+                                        _dev_ptr(R, "R", (o, o, v, v)), _stream_ptr(stream), ctypes.byref(t)),
+               "ppl_apply_profiled")
+        return t.asdict()
+
+    def apply_host(self, L, t2, R):
+        """Host (numpy float64 / CPU torch) buffers; copies are part of the call. Returns (h2d, d2h) bytes."""
+        o, v, x = self.nocc, self.nvirt, self.nchol
+
+        def hp(a, name, shape):
+            import numpy as np
+
+            if hasattr(a, "data_ptr"):  # CPU torch tensor (e.g. pinned)
+                import torch
+
+                if a.is_cuda or a.dtype != torch.float64 or not a.is_contiguous() or tuple(a.shape) != shape:
+                    raise TypeError(f"{name}: need a contiguous CPU float64 tensor of shape {shape}")
+                return c_void_p(a.data_ptr())
+            if not isinstance(a, np.ndarray) or a.dtype != np.float64 or not a.flags.c_contiguous or a.shape != shape:
+                raise TypeError(f"{name}: need a C-contiguous float64 array of shape {shape}")
+            return c_void_p(a.ctypes.data)
+
+        h2d, d2h = c_uint64(0), c_uint64(0)
+        _check(lib().ppl_apply_host(self._h, hp(L, "L", (x, v, v)), hp(t2, "t2", (o, o, v, v)),
+                                    hp(R, "R", (o, o, v, v)), ctypes.byref(h2d), ctypes.byref(d2h)), "ppl_apply_host")
+        return int(h2d.value), int(d2h.value)
+
+    def set_symmetry(self, mode: int):
+        _check(lib().ppl_plan_set_symmetry(self._h, int(mode)), "ppl_plan_set_symmetry")
+
+    def info(self) -> dict:
+        out = ppl_info_t()
+        _check(lib().ppl_plan_info(self._h, ctypes.byref(out)), "ppl_plan_info")
+        return out.asdict()
+
+    def check_inputs(self, L, t2, stream=None) -> int:
+        """Returns flags (bit 0: L not symmetric, bit 1: t2 not pair-symmetric); raises on a violated precondition."""
+        flags = c_int(0)
+        rc = lib().ppl_check_inputs(self._h, _dev_ptr(L, "L"), _dev_ptr(t2, "t2"), _stream_ptr(stream), ctypes.byref(flags))
+        if rc not in (PPL_OK, PPL_ERR_PRECONDITION):
+            raise PplError(rc, "ppl_check_inputs")
+        if rc == PPL_ERR_PRECONDITION:
+            raise PplError(rc, "ppl_check_inputs")
+        return int(flags.value)
+
+    def destroy(self):
+        if self._h:
+            rc = lib().ppl_destroy(self._h)
+            self._h = c_void_p(None)
+            _check(rc, "ppl_destroy")
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+# function-style mirrors of the three north_star entry points
+def ppl_plan(nocc: int, nvirt: int, nchol: int, workspace_bytes: int = 0) -> Plan:
+    return Plan(nocc, nvirt, nchol, workspace_bytes)
+
+
+def ppl_apply(plan: Plan, L, t2, R, stream=None):
+    return plan.apply(L, t2, R, stream)
+
+
+def ppl_destroy(plan: Plan):
+    plan.destroy()
+
+
+def ppl_probe_fp64_peak(reps: int = 3, ms_target: float = 20.0) -> float:
+    out = c_double(0.0)
+    _check(lib().ppl_probe_fp64_peak(ctypes.byref(out), int(reps), float(ms_target)), "ppl_probe_fp64_peak")
+    return float(out.value)
+
+
+def ppl_debug_dmma_layout(A, B, C):
+    _check(lib().ppl_debug_dmma_layout(_dev_ptr(A, "A", (8, 4)), _dev_ptr(B, "B", (4, 8)), _dev_ptr(C, "C", (8, 8))),
+           "ppl_debug_dmma_layout")
+    return C
