@@ -1,0 +1,325 @@
+#!/usr/bin/env python
+"""bench.py -- the pp-ladder hot path on B200: seconds per ppl_apply call and FP64 TFLOP/s.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config large|xl|medium|small|tiny]
+                  [--impl ours|reference]
+
+A "step" is one ppl_apply: the whole hot path (step 0 W-tile generation, step 1
+(c,d) contraction, reduce/accumulate/mirror, ring/streams) over one seeded synthetic batch shaped
+like BASELINE.json's configs.  Default workload: 'large' (configs[3], one of the two configs the
+north_star target is quoted on; 'xl' is the other: --config xl).
+
+value  = executed FP64 TFLOP/s (flops of the tiles actually computed / time; pair symmetry halves
+         the nominal 2*nchol*nvirt^4 + 2*nocc^2*nvirt^4, and the line says so), inputs resident
+         in HBM.
+e2e    = the same through ppl_apply_host with pinned HOST buffers (H2D of L, t2, R and D2H of R
+         inside the timed region).
+roofline = the dominant kernel against the FP64 tensor (DMMA) pipe peak measured live by
+         ppl_probe_fp64_peak (MEASURED_PEAKS.json carries no FP64 figure).
+cpu_baseline = the oracle (oracle/ppl_oracle.c, as it stands) on the host cores, on a bounded
+         sample of (a,b) columns of the same workload; the same sample is compared with the GPU
+         result ("parity" key).
+Multi-GPU: the path does not shard (north_star: one GPU, no collectives) -> "replicas only": under
+torchrun every rank runs an independent replica; value is the aggregate, time the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "pp_ladder_fp64_tflops_executed"
+UNIT = "TFLOP/s"
+NOMINAL_FP64_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 * 1e-12  # 148 SM x 4 SMSP x 16 FMA/clk x 2 x 1.965 GHz = 37.23
+
+
+def col_flops(o, v, x):
+    """flops of one (a,b) column of the two-step route: step 0 (2 x v^2) + step 1 (2 o^2 v^2)."""
+    return 2.0 * x * v * v + 2.0 * o * o * v * v
+
+
+# ------------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.path = index, None, None
+
+    def start(self):
+        try:
+            f = tempfile.NamedTemporaryFile("w", suffix=".csv", delete=False)
+            self.path = f.name
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self) -> dict:
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if not self.proc:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        try:
+            rows = [r.split(",") for r in open(self.path).read().strip().splitlines() if r.strip()]
+            os.unlink(self.path)
+        except Exception:
+            return out
+        sm, reasons = [], set()
+        for r in rows:
+            try:
+                sm.append(float(r[0]))
+                out["sm_max_mhz"] = float(r[1])
+                for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                    if "Active" in val and "Not" not in val:
+                        reasons.add(name)
+            except Exception:
+                continue
+        if sm:
+            sm.sort()
+            out["sm_mhz"] = sm[len(sm) // 2]
+            out["power_w_max"] = max(float(r[2]) for r in rows if len(r) > 2)
+        out["samples"] = len(sm)
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+# --------------------------------------------------------------------------------------- reference
+def oracle_sample(L, t2, o, v, x, target_s=15.0, seed=0):
+    """Time oracle.columns on a bounded sample of (a,b) columns (~target_s of CPU work)."""
+    import oracle
+    import ppl_inputs as I
+
+    pilot = I.sample_pairs(v, 4, seed=seed + 1)[:8]
+    t0 = time.perf_counter()
+    oracle.columns(L, t2, pilot)
+    dt = max(time.perf_counter() - t0, 1e-4)
+    per_col = dt / len(pilot)
+    k = int(max(8, min(v * v, target_s / per_col)))
+    pairs = I.sample_pairs(v, k, seed=seed)[:k]
+    t0 = time.perf_counter()
+    cols = oracle.columns(L, t2, pairs)
+    dt = time.perf_counter() - t0
+    return pairs, cols, dt, oracle.num_threads()
+
+
+def run_reference(args, o, v, x):
+    """--impl reference: the oracle as it stands on the host cores; each step = a bounded sample."""
+    import ppl_inputs as I
+
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    L, t2 = I.make_L(v, x, 0), I.make_t2(o, v, 0)
+    import oracle
+
+    per_step_s = 8.0
+    pilot = I.sample_pairs(v, 4, seed=1)[:8]
+    t0 = time.perf_counter()
+    oracle.columns(L, t2, pilot)
+    per_col = max(time.perf_counter() - t0, 1e-4) / len(pilot)
+    k = int(max(4, min(v * v, per_step_s / per_col)))
+    pairs = I.sample_pairs(v, k, seed=0)[:k]
+    for _ in range(args.warmup):
+        oracle.columns(L, t2, pairs[: max(4, k // 8)])
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.columns(L, t2, pairs)
+    dt = time.perf_counter() - t0
+    tflops = args.steps * len(pairs) * col_flops(o, v, x) / dt * 1e-12
+    line = {
+        "impl": "reference", "metric": METRIC, "value": tflops, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.config, "nocc": o, "nvirt": v, "nchol": x, "seed": 0},
+        "cpu_baseline": {"value": tflops, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                         "sample": f"{len(pairs)} of {v*v} (a,b) columns per step (oracle.columns), all i,j"},
+        "e2e": {"value": tflops, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# -------------------------------------------------------------------------------------------- ours
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="large")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workspace-gb", type=float, default=0.0, help="workspace cap (0 = auto)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+
+    import ppl_inputs as I
+
+    o, v, x = I.CONFIGS[args.config]
+    if args.impl == "reference":
+        run_reference(args, o, v, x)
+        return
+
+    import numpy as np
+    import torch
+
+    import paper_2603_20912_b200 as P
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU path)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+
+        dist = dist_mod
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    # ---- seeded synthetic inputs in pinned host memory (shared bit-for-bit with the oracle) ----
+    t_gen = time.perf_counter()
+    Lh = torch.empty((x, v, v), dtype=torch.float64, pin_memory=True)
+    th = torch.empty((o, o, v, v), dtype=torch.float64, pin_memory=True)
+    Rh = torch.zeros((o, o, v, v), dtype=torch.float64, pin_memory=True)
+    I.make_L(v, x, 0, out=Lh.numpy())
+    I.make_t2(o, v, 0, out=th.numpy())
+    t_gen = time.perf_counter() - t_gen
+    Ld, td = Lh.to(dev, non_blocking=True), th.to(dev, non_blocking=True)
+    Rd = torch.zeros((o, o, v, v), dtype=torch.float64, device=dev)
+    torch.cuda.synchronize()
+
+    peak = P.ppl_probe_fp64_peak(3, 20.0)
+    t0 = time.perf_counter()
+    plan = P.Plan(o, v, x, int(args.workspace_gb * (1 << 30)))
+    plan_s = time.perf_counter() - t0
+    info = plan.info()
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 0)):
+        plan.apply(Ld, td, Rd)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    barrier()
+    evs[0].record(stream)
+    for k in range(args.steps):
+        plan.apply(Ld, td, Rd)  # R accumulates (+=) across steps; no work is skipped
+        evs[k + 1].record(stream)
+    barrier()
+    clocks = sampler.stop()
+    step_ms = [evs[k].elapsed_time(evs[k + 1]) for k in range(args.steps)]
+    total_ms = evs[0].elapsed_time(evs[-1])
+    if dist is not None:
+        tt = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        total_ms = float(tt.item())
+    ms_per_step = total_ms / args.steps
+    f_exec, f_nom = info["flops_executed"], info["flops_nominal"]
+    value = world * f_exec / (ms_per_step * 1e-3) * 1e-12
+
+    # ---- dominant kernel, timed live with CUDA events on the launching stream (serialised pass) ----
+    Rd.zero_()
+    prof = plan.apply_profiled(Ld, td, Rd)  # Rd now holds exactly one application of the term
+    torch.cuda.synchronize()
+    dom = "step0" if prof["step0_ms"] >= prof["step1_ms"] else "step1"
+    dom_flops = info["flops_" + dom] / prof["n_" + dom]
+    dom_ms = prof[dom + "_ms"] / prof["n_" + dom]
+    achieved = dom_flops / (dom_ms * 1e-3) * 1e-12
+    # per-launch DRAM traffic of the dominant kernel from the committed ncu --set full capture, if any
+    traffic = None
+    try:
+        tr = json.load(open(os.path.join(ROOT, "profiles", "dram_traffic.json")))
+        traffic = tr.get(args.config, {}).get(dom)
+    except Exception:
+        pass
+    roofline = {
+        "bound": "tensor", "kernel": "k_" + dom, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+        "frac": achieved / peak, "traffic": traffic,
+        "peak_source": "measured live: ppl_probe_fp64_peak (register-only DMMA m8n8k4 stream); "
+                       f"nominal {NOMINAL_FP64_TFLOPS:.2f} = 148 SM x 4 SMSP x 16 FMA/clk x 2 x 1.965 GHz",
+        "flops_per_launch": dom_flops, "ms_per_launch": dom_ms,
+        "how": "ppl_apply_profiled: one serialised apply after the timed steps, a CUDA event pair around every launch",
+        "step0_tflops": info["flops_step0"] / (prof["step0_ms"] * 1e-3) * 1e-12,
+        "step1_tflops": info["flops_step1"] / (prof["step1_ms"] * 1e-3) * 1e-12,
+        "share": {"step0": prof["step0_ms"] / prof["total_ms"], "step1": prof["step1_ms"] / prof["total_ms"],
+                  "reduce": prof["reduce_ms"] / prof["total_ms"]},
+    }
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.config, "nocc": o, "nvirt": v, "nchol": x, "seed": 0,
+                   "symmetry": "pair (tiles a-block<=b-block, mirrored)", "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "l2": "inputs larger than L2 (L, t2, W tiles >> 126 MB); no flush needed",
+                   "plan": {k: info[k] for k in ("ta", "tb", "n_tiles", "ring", "splitk", "vec16", "workspace_bytes")}},
+        "seconds_per_call": ms_per_step * 1e-3,
+        "tflops_executed": f_exec / (ms_per_step * 1e-3) * 1e-12,
+        "tflops_nominal_effective": f_nom / (ms_per_step * 1e-3) * 1e-12,
+        "flops_executed": f_exec, "flops_nominal": f_nom,
+        "frac_of_fp64_peak_measured": f_exec / (ms_per_step * 1e-3) * 1e-12 / peak,
+        "frac_of_fp64_peak_nominal": f_exec / (ms_per_step * 1e-3) * 1e-12 / NOMINAL_FP64_TFLOPS,
+        "step_ms": step_ms, "plan_seconds": plan_s, "input_gen_seconds": t_gen,
+        "clocks": clocks, "roofline": roofline,
+        "gpu_launches": info["launches_per_apply"] * args.steps,
+    }
+
+    if rank == 0 and not args.no_e2e:
+        # ---- end to end through the host entry point: H2D(L, t2, R) + apply + D2H(R) per step ----
+        n_e2e = max(1, min(args.steps, 3))
+        Rh.zero_()
+        h2d, d2h = plan.apply_host(Lh, th, Rh)  # warm-up (allocates the staging buffers)
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            h2d, d2h = plan.apply_host(Lh, th, Rh)
+        dt = (time.perf_counter() - t0) / n_e2e
+        line["e2e"] = {"value": world * f_exec / dt * 1e-12, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                       "d2h_bytes_per_step": d2h, "seconds_per_call": dt, "steps": n_e2e,
+                       "how": "ppl_apply_host on pinned host buffers; wall clock around the synchronous call"}
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        # ---- the oracle on the host cores, bounded sample; the same sample checks the GPU result ----
+        pairs, cols, dt, cores = oracle_sample(Lh.numpy(), th.numpy(), o, v, x)
+        line["cpu_baseline"] = {
+            "value": len(pairs) * col_flops(o, v, x) / dt * 1e-12, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{len(pairs)} of {v*v} (a,b) columns (oracle.columns), all i,j; {dt:.1f} s",
+            "extrapolated_seconds_per_call": dt / len(pairs) * v * v,
+        }
+        Rg = Rd.cpu().numpy()
+        got = Rg[:, :, pairs[:, 0], pairs[:, 1]].transpose(2, 0, 1)
+        err = float(np.abs(got - cols).max() / np.abs(cols).max())
+        line["parity"] = {"max_rel_err_vs_oracle": err, "tolerance": 1e-11, "columns": int(len(pairs)), "ok": bool(err <= 1e-11)}
+
+    plan.destroy()
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line))
+
+
+if __name__ == "__main__":
+    main()
