@@ -2,6 +2,7 @@
 // Everything on the data path runs in the kernels of ppl_kernels.cuh; there is no CPU fallback.
 #include "../../include/ppl.h"
 #include "ppl_kernels.cuh"
+#include "ppl_kernels_tma.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -62,6 +63,8 @@ struct ppl_plan_s {
     // host-path staging buffers (ppl_apply_host)
     double *dL = nullptr, *dT = nullptr, *dR = nullptr;
     double f_step0 = 0, f_step1 = 0;
+    int use_tma = 0;                 // 1: persistent TMA/mbarrier kernels (nvirt even); 0: cp.async kernels
+    CUtensorMap mapW[MAX_RING];      // W slots as {inner nvirt^2, outer T*T}, built at plan time
 };
 
 namespace {
@@ -200,6 +203,8 @@ int set_kernel_attrs() {
     PPL_CUDA(cudaFuncSetAttribute(ppl::k_step0<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_MN));
     PPL_CUDA(cudaFuncSetAttribute(ppl::k_step1<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_K));
     PPL_CUDA(cudaFuncSetAttribute(ppl::k_step1<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_K));
+    PPL_CUDA(cudaFuncSetAttribute(ppl::k_step0_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_TMA));
+    PPL_CUDA(cudaFuncSetAttribute(ppl::k_step1_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_TMA));
     g_attr_set = true;
     return PPL_OK;
 }
@@ -263,6 +268,80 @@ int launch_reduce(const ppl_plan_s *p, const Tile &t, double *R, cudaStream_t s)
     ppl::k_reduce<<<grid, 256, 0, s>>>(a);
     PPL_CUDA(cudaGetLastError());
     return PPL_OK;
+}
+
+
+// ---- TMA tensor maps (driver entry point fetched through the runtime: no libcuda link) ----
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn get_encode() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void *ptr = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(ptr);
+        else
+            (void)cudaGetLastError();
+    }
+    return fn;
+}
+// 2-D FP64 tensor {inner (contiguous), outer} with row stride `row_bytes`, box {box_inner, box_outer}, 128B swizzle
+int make_map_2d(CUtensorMap *map, const void *base, uint64_t inner, uint64_t outer, uint64_t row_bytes, uint32_t box_inner,
+                uint32_t box_outer) {
+    EncodeTiledFn enc = get_encode();
+    if (!enc) return PPL_ERR_CUDA;
+    const cuuint64_t gdim[2] = {inner, outer};
+    const cuuint64_t gstride[1] = {row_bytes};
+    const cuuint32_t box[2] = {box_inner, box_outer};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void *>(base), gdim, gstride, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? PPL_OK : PPL_ERR_CUDA;
+}
+
+int launch_step0_tma(const ppl_plan_s *p, const Tile &t, const CUtensorMap &mapL, double *W, cudaStream_t s) {
+    ppl::Step0TmaArgs a;
+    a.a0v = t.a0 * p->v;
+    a.b0v = t.b0 * p->v;
+    a.M = t.ta * p->v;
+    a.N = t.tb * p->v;
+    a.K = p->x;
+    a.v = p->v;
+    a.tb = t.tb;
+    a.W = W;
+    a.ldw = p->ldw;
+    const int items = ((a.M + ppl::BM - 1) / ppl::BM) * ((a.N + ppl::BN - 1) / ppl::BN);
+    ppl::k_step0_tma<<<std::min(items, p->num_sms), ppl::TMA_THREADS, ppl::SMEM_TMA, s>>>(mapL, a);
+    PPL_CUDA(cudaGetLastError());
+    return PPL_OK;
+}
+
+int launch_step1_tma(const ppl_plan_s *p, const Tile &t, const CUtensorMap &mapT, const CUtensorMap &mapW, cudaStream_t s) {
+    ppl::Step1TmaArgs a;
+    a.M = p->o * p->o;
+    a.N = t.ta * t.tb;
+    a.K = p->v * p->v;
+    a.k_per_split = t.k_per_split;
+    a.splitk = t.splitk;
+    a.part = p->part;
+    const int items = ((a.M + ppl::BM - 1) / ppl::BM) * ((a.N + ppl::BN - 1) / ppl::BN) * t.splitk;
+    ppl::k_step1_tma<<<std::min(items, p->num_sms), ppl::TMA_THREADS, ppl::SMEM_TMA, s>>>(mapT, mapW, a);
+    PPL_CUDA(cudaGetLastError());
+    return PPL_OK;
+}
+
+struct ApplyMaps {
+    CUtensorMap L, T;
+};
+int make_apply_maps(const ppl_plan_s *p, const double *L, const double *t2, ApplyMaps *m) {
+    const uint64_t vv = (uint64_t)p->v * p->v;
+    int rc = make_map_2d(&m->L, L, vv, (uint64_t)p->x, vv * 8, 16, ppl::BK);
+    if (rc == PPL_OK) rc = make_map_2d(&m->T, t2, vv, (uint64_t)p->o * p->o, vv * 8, ppl::BK, ppl::BM);
+    return rc;
 }
 
 int check_ptrs(const ppl_plan_s *p, const double *L, const double *t2, const double *R, bool *vec16) {
@@ -397,6 +476,16 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
         fail(PPL_ERR_CUDA);
         return nullptr;
     }
+    const char *envk = getenv("PPL_KERNELS");  // debug override: "cpasync" forces the non-TMA kernels
+    p->use_tma = p->vec16 && !(envk && strcmp(envk, "cpasync") == 0) && get_encode() != nullptr;
+    if (p->use_tma) {
+        const uint64_t vv = (uint64_t)nvirt * nvirt;
+        for (int i = 0; i < p->ring; ++i)
+            if (make_map_2d(&p->mapW[i], p->Wslot[i], vv, (uint64_t)p->T * p->T, (uint64_t)p->ldw * 8, ppl::BK, ppl::BN) != PPL_OK) {
+                p->use_tma = 0;
+                break;
+            }
+    }
     p->sym = PPL_SYM_PAIR;
     const int rc = build_tiles(p);
     if (rc != PPL_OK) {
@@ -443,6 +532,9 @@ int ppl_apply(ppl_plan_t *p, const double *L, const double *t2, double *R, void 
     if (rc != PPL_OK) return fail(rc);
     cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
     const int ntiles = (int)p->tiles.size();
+    const bool tma = p->use_tma && vec16;
+    ApplyMaps maps;
+    if (tma && (rc = make_apply_maps(p, L, t2, &maps)) != PPL_OK) return fail(rc);
     const bool two_streams = p->ring >= 2 && ntiles >= 2;
     cudaStream_t gen = two_streams ? p->gen : stream;
 
@@ -454,12 +546,14 @@ int ppl_apply(ppl_plan_t *p, const double *L, const double *t2, double *R, void 
         const Tile &t = p->tiles[k];
         const int slot = k % p->ring;
         if (two_streams && k >= p->ring) PPL_CUDA(cudaStreamWaitEvent(gen, p->ev_free[slot], 0));
-        if ((rc = launch_step0(p, t, L, p->Wslot[slot], vec16, gen)) != PPL_OK) return rc;
+        rc = tma ? launch_step0_tma(p, t, maps.L, p->Wslot[slot], gen) : launch_step0(p, t, L, p->Wslot[slot], vec16, gen);
+        if (rc != PPL_OK) return rc;
         if (two_streams) {
             PPL_CUDA(cudaEventRecord(p->ev_ready[slot], gen));
             PPL_CUDA(cudaStreamWaitEvent(stream, p->ev_ready[slot], 0));
         }
-        if ((rc = launch_step1(p, t, t2, p->Wslot[slot], vec16, stream)) != PPL_OK) return rc;
+        rc = tma ? launch_step1_tma(p, t, maps.T, p->mapW[slot], stream) : launch_step1(p, t, t2, p->Wslot[slot], vec16, stream);
+        if (rc != PPL_OK) return rc;
         if (two_streams) PPL_CUDA(cudaEventRecord(p->ev_free[slot], stream));
         if ((rc = launch_reduce(p, t, R, stream)) != PPL_OK) return rc;
     }
@@ -475,14 +569,18 @@ int ppl_apply_profiled(ppl_plan_t *p, const double *L, const double *t2, double 
     cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
     memset(times, 0, sizeof(*times));
     const int ntiles = (int)p->tiles.size();
+    const bool tma = p->use_tma && vec16;
+    ApplyMaps maps;
+    if (tma && (rc = make_apply_maps(p, L, t2, &maps)) != PPL_OK) return fail(rc);
     std::vector<cudaEvent_t> ev(3 * (size_t)ntiles + 1);
     for (auto &e : ev) PPL_CUDA(cudaEventCreate(&e));
     PPL_CUDA(cudaEventRecord(ev[0], stream));
     for (int k = 0; k < ntiles && rc == PPL_OK; ++k) {
         const Tile &t = p->tiles[k];
-        rc = launch_step0(p, t, L, p->Wslot[0], vec16, stream);
+        rc = tma ? launch_step0_tma(p, t, maps.L, p->Wslot[0], stream) : launch_step0(p, t, L, p->Wslot[0], vec16, stream);
         cudaEventRecord(ev[3 * k + 1], stream);
-        if (rc == PPL_OK) rc = launch_step1(p, t, t2, p->Wslot[0], vec16, stream);
+        if (rc == PPL_OK)
+            rc = tma ? launch_step1_tma(p, t, maps.T, p->mapW[0], stream) : launch_step1(p, t, t2, p->Wslot[0], vec16, stream);
         cudaEventRecord(ev[3 * k + 2], stream);
         if (rc == PPL_OK) rc = launch_reduce(p, t, R, stream);
         cudaEventRecord(ev[3 * k + 3], stream);

@@ -1,0 +1,349 @@
+// ppl_kernels_tma.cuh -- persistent, warp-specialised sm_100a GEMM kernels for both steps.
+//
+//   warps 8..11 (warpgroup 2)  : producer warpgroup; gives its registers away (setmaxnreg.dec) and one
+//                                elected lane of warp 8 is the TMA producer.  cp.async.bulk.tensor.2d loads 128B-swizzled boxes of
+//                                the operands into a TSTAGES-deep shared-memory ring and signals
+//                                full[stage] (mbarrier, complete_tx::bytes).
+//   warps 0..7                 : consumers.  Wait full[stage], read fragments with conflict-free
+//                                LDS.128, issue DMMA m8n8k4 (FP64 tensor pipe), arrive on empty[stage].
+//   grid = #SMs, each CTA strides over work items (output tile [, k-split]); the producer runs
+//   ahead across item boundaries, so the ring never drains between tiles and the epilogue of one
+//   item overlaps the loads of the next.  There is no __syncthreads in the main loop.
+//
+// Why this shape: ncu on the first (cp.async + __syncthreads) kernels showed the DMMA pipe 86 %
+// active; the rest was the per-k-tile address/LDGSTS section executed by all warps in lock step
+// behind the barrier and the per-CTA prologue/epilogue at 1 CTA/SM (profiles/r01_*.md).
+//
+// Shared-memory layouts (TMA SWIZZLE_128B: 16-byte chunk index ^= (128-byte row index & 7)):
+//   step 0, operand tile 128 (m) x 16 (k):  8 boxes [mchunk][k=16 rows][16 doubles of m]
+//   step 1, operand tile 128 (m) x 16 (k):  1 box   [m=128 rows][16 doubles of k]
+// Fragment rows are permuted so that the 8 lanes of a quarter warp hit 8 distinct 16-byte bank
+// groups: lane = 4g+q uses row/chunk index c(g) = (g>>1) + 4*(g&1).  The epilogues undo it.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "ppl_kernels.cuh"
+
+namespace ppl {
+
+constexpr int TSTAGES = 6;
+constexpr int CONSUMER_WARPS = 8;
+constexpr int TMA_THREADS = 32 * (CONSUMER_WARPS + 4);  // 2 consumer warpgroups + 1 producer warpgroup
+constexpr int CONSUMER_REGS = 232, PRODUCER_REGS = 40;  // setmaxnreg: 8*32*232 + 4*32*40 = 64512 <= 65536
+constexpr uint32_t TILE_BYTES = BM * BK * sizeof(double);          // one operand tile: 16 KB
+constexpr uint32_t STAGE_BYTES = 2 * TILE_BYTES;                   // A + B
+constexpr size_t SMEM_TMA = (size_t)TSTAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/;
+
+// ---- mbarrier / TMA primitives (PTX; SASS: SYNCS.*, UTMALDG) ----
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(void *dst, const CUtensorMap *map, int c0, int c1, uint64_t *bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n" ::"r"(
+            smem_u32(dst)),
+        "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar))
+        : "memory");
+}
+template <int N>
+__device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(N)); }
+template <int N>
+__device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(N)); }
+__device__ __forceinline__ void prefetch_tmap(const CUtensorMap *map) {
+    asm volatile("prefetch.tensormap [%0];\n" ::"l"(map) : "memory");
+}
+
+struct TmaSmem {
+    double *a, *b;           // [TSTAGES][BM*BK]
+    uint64_t *full, *empty;  // [TSTAGES]
+};
+__device__ __forceinline__ TmaSmem carve_smem(unsigned char *raw) {
+    const uint32_t base = smem_u32(raw);
+    unsigned char *al = raw + ((1024u - (base & 1023u)) & 1023u);
+    TmaSmem s;
+    s.a = reinterpret_cast<double *>(al);
+    s.b = reinterpret_cast<double *>(al + (size_t)TSTAGES * TILE_BYTES);
+    s.full = reinterpret_cast<uint64_t *>(al + (size_t)TSTAGES * STAGE_BYTES);
+    s.empty = s.full + TSTAGES;
+    return s;
+}
+__device__ __forceinline__ void init_barriers(const TmaSmem &s, int tid) {
+    if (tid == 0) {
+#pragma unroll
+        for (int i = 0; i < TSTAGES; ++i) {
+            mbar_init(&s.full[i], 1);
+            mbar_init(&s.empty[i], CONSUMER_WARPS);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+}
+
+// ---------------------------------------------------------------------------------------------
+// step 0 (TMA):  W[(a,b)][(c,d)] = sum_P L[P,a,c] L[P,b,d]      (eq. 5)
+// mapL: 2-D tensor {inner = nvirt^2 (a,c flattened), outer = nchol}, box {16, BK}, SWIZZLE_128B.
+// ---------------------------------------------------------------------------------------------
+struct Step0TmaArgs {
+    int a0v, b0v;   // a0*v, b0*v: first flattened (a,c) / (b,d) column of the panels
+    int M, N, K;    // ta*v, tb*v, nchol
+    int v, tb;
+    double *W;
+    int64_t ldw;
+};
+
+__global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_tma(const __grid_constant__ CUtensorMap mapL, const Step0TmaArgs p) {
+    extern __shared__ unsigned char smem_raw[];
+    const TmaSmem sm = carve_smem(smem_raw);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    init_barriers(sm, tid);
+
+    const int tiles_m = (p.M + BM - 1) / BM, tiles_n = (p.N + BN - 1) / BN;
+    const int num_items = tiles_m * tiles_n;
+    const int nkt = (p.K + BK - 1) / BK;
+
+    if (warp >= CONSUMER_WARPS) {
+        // ================================ producer warpgroup ================================
+        setmaxnreg_dec<PRODUCER_REGS>();
+        if (warp == CONSUMER_WARPS && lane == 0) {
+            prefetch_tmap(&mapL);
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int item = blockIdx.x; item < num_items; item += gridDim.x) {
+                int tm, tn;
+                raster(item, tiles_m, tiles_n, tm, tn);
+                const int xa = p.a0v + tm * BM, xb = p.b0v + tn * BN;
+                for (int kt = 0; kt < nkt; ++kt) {
+                    mbar_wait(&sm.empty[stage], phase ^ 1);
+                    mbar_expect_tx(&sm.full[stage], STAGE_BYTES);
+                    double *da = sm.a + (size_t)stage * BM * BK, *db = sm.b + (size_t)stage * BN * BK;
+#pragma unroll
+                    for (int i = 0; i < BM / 16; ++i) tma_load_2d(da + i * BK * 16, &mapL, xa + 16 * i, kt * BK, &sm.full[stage]);
+#pragma unroll
+                    for (int i = 0; i < BN / 16; ++i) tma_load_2d(db + i * BK * 16, &mapL, xb + 16 * i, kt * BK, &sm.full[stage]);
+                    if (++stage == TSTAGES) {
+                        stage = 0;
+                        phase ^= 1;
+                    }
+                }
+            }
+        }
+        return;
+    }
+    // ================================ consumers ================================
+    setmaxnreg_inc<CONSUMER_REGS>();
+    const int g = lane >> 2, q = lane & 3;
+    const int c = (g >> 1) + 4 * (g & 1);  // permuted row/chunk index of this lane's fragment row
+    const int wm = warp / WARPS_N, wn = warp % WARPS_N;
+    // fragment offsets (doubles) inside an operand tile for k4 even / odd: row k = 4*k4 + q
+    const int offk_even = q * 16 + ((c ^ q) << 1);
+    const int offk_odd = (q + 4) * 16 + ((c ^ (q + 4)) << 1);
+    int stage = 0;
+    uint32_t phase = 0;
+    for (int item = blockIdx.x; item < num_items; item += gridDim.x) {
+        int tm, tn;
+        raster(item, tiles_m, tiles_n, tm, tn);
+        const int m0 = tm * BM, n0 = tn * BN;
+        double acc[8][4][2];
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+        for (int kt = 0; kt < nkt; ++kt) {
+            mbar_wait(&sm.full[stage], phase);
+            const double *as = sm.a + (size_t)stage * BM * BK + (wm * 4) * (BK * 16);
+            const double *bs = sm.b + (size_t)stage * BN * BK + (wn * 2) * (BK * 16);
+#pragma unroll
+            for (int k4 = 0; k4 < BK / 4; ++k4) {
+                const int off = (k4 >> 1) * 128 + ((k4 & 1) ? offk_odd : offk_even);
+                double2 a[4], b[2];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) a[i] = *reinterpret_cast<const double2 *>(as + i * (BK * 16) + off);
+#pragma unroll
+                for (int j = 0; j < 2; ++j) b[j] = *reinterpret_cast<const double2 *>(bs + j * (BK * 16) + off);
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+#pragma unroll
+                    for (int j = 0; j < 2; ++j) {
+                        dmma(acc[2 * i][2 * j][0], acc[2 * i][2 * j][1], a[i].x, b[j].x);
+                        dmma(acc[2 * i][2 * j + 1][0], acc[2 * i][2 * j + 1][1], a[i].x, b[j].y);
+                        dmma(acc[2 * i + 1][2 * j][0], acc[2 * i + 1][2 * j][1], a[i].y, b[j].x);
+                        dmma(acc[2 * i + 1][2 * j + 1][0], acc[2 * i + 1][2 * j + 1][1], a[i].y, b[j].y);
+                    }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&sm.empty[stage]);
+            if (++stage == TSTAGES) {
+                stage = 0;
+                phase ^= 1;
+            }
+        }
+        // epilogue.  block (2i+e, 2j+f): frag row g <-> m = mw + 16i + 2c(g) + e;
+        //   c0 <-> n = nw + 16j + 2q + f,   c1 <-> n = nw + 16j + 2q + 8 + f
+        const int v = p.v;
+        const bool pair_ok = (v & 1) == 0;  // n even & v even: (n, n+1) share one b and are 16-byte aligned
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int m = m0 + wm * WTM + 16 * i + 2 * c + e;
+                if (m >= p.M) continue;
+                const int al = m / v, cc = m - al * v;
+                double *wrow = p.W + (int64_t)al * p.tb * p.ldw + (int64_t)cc * v;
+#pragma unroll
+                for (int j = 0; j < 2; ++j)
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {  // h = 0: c0 values, h = 1: c1 values
+                        const int n = n0 + wn * WTN + 16 * j + 2 * q + 8 * h;
+                        const double v0 = acc[2 * i + e][2 * j][h], v1 = acc[2 * i + e][2 * j + 1][h];
+                        const int bl = n / v, d = n - bl * v;
+                        if (pair_ok && n + 1 < p.N) {
+                            *reinterpret_cast<double2 *>(wrow + (int64_t)bl * p.ldw + d) = make_double2(v0, v1);
+                        } else {
+                            if (n < p.N) wrow[(int64_t)bl * p.ldw + d] = v0;
+                            if (n + 1 < p.N) {
+                                const int bl1 = (n + 1) / v, d1 = (n + 1) - bl1 * v;
+                                wrow[(int64_t)bl1 * p.ldw + d1] = v1;
+                            }
+                        }
+                    }
+            }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// step 1 (TMA):  part[z][(i,j)][(a,b)] = sum_{(c,d) in split z} t2[(i,j)][(c,d)] W[(a,b)][(c,d)]
+// mapA: t2 as {inner = nvirt^2, outer = nocc^2};  mapB: W slot as {inner = nvirt^2, outer = T*T};
+// box {16, 128}, SWIZZLE_128B.
+// ---------------------------------------------------------------------------------------------
+struct Step1TmaArgs {
+    int M, N, K;      // nocc^2, ta*tb, nvirt^2
+    int k_per_split;  // multiple of BK
+    int splitk;
+    double *part;     // [splitk][M][N]
+};
+
+__global__ void __launch_bounds__(TMA_THREADS, 1)
+    k_step1_tma(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, const Step1TmaArgs p) {
+    extern __shared__ unsigned char smem_raw[];
+    const TmaSmem sm = carve_smem(smem_raw);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    init_barriers(sm, tid);
+
+    const int tiles_m = (p.M + BM - 1) / BM, tiles_n = (p.N + BN - 1) / BN;
+    const int tiles_mn = tiles_m * tiles_n;
+    const int num_items = tiles_mn * p.splitk;
+
+    if (warp >= CONSUMER_WARPS) {
+        setmaxnreg_dec<PRODUCER_REGS>();
+        if (warp == CONSUMER_WARPS && lane == 0) {
+            prefetch_tmap(&mapA);
+            prefetch_tmap(&mapB);
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int item = blockIdx.x; item < num_items; item += gridDim.x) {
+                const int z = item / tiles_mn, r = item - z * tiles_mn;
+                const int tm = r % tiles_m, tn = r / tiles_m;
+                const int kbeg = z * p.k_per_split, kend = min(p.K, kbeg + p.k_per_split);
+                for (int k = kbeg; k < kend; k += BK) {
+                    mbar_wait(&sm.empty[stage], phase ^ 1);
+                    mbar_expect_tx(&sm.full[stage], STAGE_BYTES);
+                    tma_load_2d(sm.a + (size_t)stage * BM * BK, &mapA, k, tm * BM, &sm.full[stage]);
+                    tma_load_2d(sm.b + (size_t)stage * BN * BK, &mapB, k, tn * BN, &sm.full[stage]);
+                    if (++stage == TSTAGES) {
+                        stage = 0;
+                        phase ^= 1;
+                    }
+                }
+            }
+        }
+        return;
+    }
+    setmaxnreg_inc<CONSUMER_REGS>();
+    const int g = lane >> 2, q = lane & 3;
+    const int c = (g >> 1) + 4 * (g & 1);
+    const int wm = warp / WARPS_N, wn = warp % WARPS_N;
+    // row r = 8i + c, 16-byte chunk (k8*4 + q) ^ c
+    const int off0 = c * 16 + ((q ^ c) << 1);
+    const int off1 = c * 16 + (((4 + q) ^ c) << 1);
+    int stage = 0;
+    uint32_t phase = 0;
+    for (int item = blockIdx.x; item < num_items; item += gridDim.x) {
+        const int z = item / tiles_mn, r = item - z * tiles_mn;
+        const int tm = r % tiles_m, tn = r / tiles_m;
+        const int m0 = tm * BM, n0 = tn * BN;
+        const int kbeg = z * p.k_per_split, kend = min(p.K, kbeg + p.k_per_split);
+        double acc[8][4][2];
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+        for (int k = kbeg; k < kend; k += BK) {
+            mbar_wait(&sm.full[stage], phase);
+            const double *as = sm.a + (size_t)stage * BM * BK + (wm * WTM) * BK;
+            const double *bs = sm.b + (size_t)stage * BN * BK + (wn * WTN) * BK;
+#pragma unroll
+            for (int k8 = 0; k8 < BK / 8; ++k8) {
+                const int off = k8 ? off1 : off0;
+                double2 a[8], b[4];
+#pragma unroll
+                for (int i = 0; i < 8; ++i) a[i] = *reinterpret_cast<const double2 *>(as + i * 8 * BK + off);
+#pragma unroll
+                for (int j = 0; j < 4; ++j) b[j] = *reinterpret_cast<const double2 *>(bs + j * 8 * BK + off);
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i].x, b[j].x);
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i].y, b[j].y);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&sm.empty[stage]);
+            if (++stage == TSTAGES) {
+                stage = 0;
+                phase ^= 1;
+            }
+        }
+        // epilogue: block (i,j): frag row g <-> m = mw + 8i + c(g); c0 <-> n = nw + 8j + q, c1 <-> n + 4
+        double *part = p.part + (int64_t)z * p.M * p.N;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const int m = m0 + wm * WTM + 8 * i + c;
+            if (m >= p.M) continue;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int n = n0 + wn * WTN + 8 * j + q;
+                double *dst = part + (int64_t)m * p.N + n;
+                if (n < p.N) dst[0] = acc[i][j][0];
+                if (n + 4 < p.N) dst[4] = acc[i][j][1];
+            }
+        }
+    }
+}
+
+}  // namespace ppl
