@@ -9,7 +9,15 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(_HERE, "libppl.so")
 SOURCES = ["ppl_api.cu"]
-DEPS = ["ppl_api.cu", "ppl_kernels.cuh", os.path.join("..", "..", "include", "ppl.h")]
+
+
+def _deps():
+    """Every source the library is built from: all of csrc/ plus the public header."""
+    files = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh", ".h"))]
+    files.append(os.path.join(_HERE, "..", "include", "ppl.h"))
+    files.append(os.path.abspath(__file__))
+    return files
+
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-lineinfo", "-O3", "-std=c++17",
@@ -28,7 +36,7 @@ def stale() -> bool:
     if not os.path.exists(SO):
         return True
     t = os.path.getmtime(SO)
-    return any(os.path.getmtime(os.path.join(CSRC, d)) > t for d in DEPS)
+    return any(os.path.getmtime(d) > t for d in _deps())
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

@@ -101,6 +101,18 @@ __device__ __forceinline__ void init_barriers(const TmaSmem &s, int tid) {
     __syncthreads();
 }
 
+// Consumer-side release of a ring slot.  The slot read in iteration t is handed back to the producer
+// only after the try_wait loop of iteration t+1: warps issue in order, a DMMA cannot issue before the
+// LDS that feed it have returned, and every DMMA of iteration t precedes that loop -- so all shared
+// loads of the slot are complete when the arrive issues.  (Arriving at the end of iteration t is NOT
+// safe: ptxas hoists the arrive above the trailing DMMAs, right behind the last LDS *issue*; with the
+// LSU backed up by other warps' epilogue stores the TMA refill then overtook those loads -- caught by
+// tests/test_gpu_fullsize.py and reproduced by tests/test_gpu_parity.py::test_persistent_ring_*.)
+// The slot of the very last iteration is never released: the producer has nothing left to load.
+__device__ __forceinline__ void release_previous(const TmaSmem &sm, int rel_stage, int lane) {
+    if (rel_stage >= 0 && lane == 0) mbar_arrive(&sm.empty[rel_stage]);
+}
+
 // ---------------------------------------------------------------------------------------------
 // step 0 (TMA):  W[(a,b)][(c,d)] = sum_P L[P,a,c] L[P,b,d]      (eq. 5)
 // mapL: 2-D tensor {inner = nvirt^2 (a,c flattened), outer = nchol}, box {16, BK}, SWIZZLE_128B.
@@ -159,7 +171,7 @@ __global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_tma(const __grid_const
     // fragment offsets (doubles) inside an operand tile for k4 even / odd: row k = 4*k4 + q
     const int offk_even = q * 16 + ((c ^ q) << 1);
     const int offk_odd = (q + 4) * 16 + ((c ^ (q + 4)) << 1);
-    int stage = 0;
+    int stage = 0, rel_stage = -1;
     uint32_t phase = 0;
     for (int item = blockIdx.x; item < num_items; item += gridDim.x) {
         int tm, tn;
@@ -173,6 +185,7 @@ __global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_tma(const __grid_const
 
         for (int kt = 0; kt < nkt; ++kt) {
             mbar_wait(&sm.full[stage], phase);
+            release_previous(sm, rel_stage, lane);
             const double *as = sm.a + (size_t)stage * BM * BK + (wm * 4) * (BK * 16);
             const double *bs = sm.b + (size_t)stage * BN * BK + (wn * 2) * (BK * 16);
 #pragma unroll
@@ -193,8 +206,7 @@ __global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_tma(const __grid_const
                         dmma(acc[2 * i + 1][2 * j + 1][0], acc[2 * i + 1][2 * j + 1][1], a[i].y, b[j].y);
                     }
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&sm.empty[stage]);
+            rel_stage = stage;  // released after the NEXT stage's wait (see release_previous)
             if (++stage == TSTAGES) {
                 stage = 0;
                 phase ^= 1;
@@ -288,7 +300,7 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
     // row r = 8i + c, 16-byte chunk (k8*4 + q) ^ c
     const int off0 = c * 16 + ((q ^ c) << 1);
     const int off1 = c * 16 + (((4 + q) ^ c) << 1);
-    int stage = 0;
+    int stage = 0, rel_stage = -1;
     uint32_t phase = 0;
     for (int item = blockIdx.x; item < num_items; item += gridDim.x) {
         const int z = item / tiles_mn, r = item - z * tiles_mn;
@@ -303,6 +315,7 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
 
         for (int k = kbeg; k < kend; k += BK) {
             mbar_wait(&sm.full[stage], phase);
+            release_previous(sm, rel_stage, lane);
             const double *as = sm.a + (size_t)stage * BM * BK + (wm * WTM) * BK;
             const double *bs = sm.b + (size_t)stage * BN * BK + (wn * WTN) * BK;
 #pragma unroll
@@ -322,8 +335,7 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
 #pragma unroll
                     for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i].y, b[j].y);
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&sm.empty[stage]);
+            rel_stage = stage;  // released after the NEXT stage's wait (see release_previous)
             if (++stage == TSTAGES) {
                 stage = 0;
                 phase ^= 1;

@@ -108,6 +108,34 @@ def test_medium_exact_integers_sampled():
     _check_columns(L, t2, Rd, 128, exact=True)
 
 
+def test_medium_closed_form_tagged_tiles_repeated():
+    """Closed form at medium size, bit for bit, no oracle needed: L == 1 gives (ac|bd) == nchol for
+    every entry, so R[i,j,a,b] = nchol * sum_cd t2[i,j,c,d] (eq. 6 with a constant integral).  t2
+    tags every (row, 16-wide k-tile) pair -- t2[m][k] = k//16 + 1000*m, m = i*nocc+j -- so a fragment
+    read from a stale or a too-early pipeline slot, a neighbouring row or another work item changes
+    the integer result.  This exact pattern exposed a shared-memory WAR race in the persistent TMA
+    kernels (slot released before its loads had completed) in 12 of 12 runs; repeated here."""
+    import torch
+
+    o, v, x = I.CONFIGS["medium"]
+    vv = v * v
+    L = torch.ones((x, v, v), dtype=torch.float64, device="cuda")
+    m_idx = torch.arange(o * o, device="cuda", dtype=torch.float64).reshape(o * o, 1)
+    ktag = (torch.arange(vv, device="cuda") // 16).to(torch.float64)
+    t2 = (ktag.reshape(1, vv) + 1000.0 * m_idx).reshape(o, o, v, v).contiguous()
+    want = (x * (ktag.sum() + 1000.0 * m_idx * vv)).reshape(o, o, 1, 1)  # exact integers < 2^53
+    for sym in (P.PPL_SYM_NONE, P.PPL_SYM_NONE, P.PPL_SYM_NONE, P.PPL_SYM_NONE):
+        R = torch.zeros((o, o, v, v), dtype=torch.float64, device="cuda")
+        with P.Plan(o, v, x) as plan:
+            plan.set_symmetry(sym)
+            plan.apply(L, t2, R)
+            torch.cuda.synchronize()
+            assert int((R != want).sum().item()) == 0
+            R.zero_()
+            plan.apply_profiled(L, t2, R)  # the serialised launch order bench.py's roofline pass uses
+            assert int((R != want).sum().item()) == 0
+
+
 def test_large_sampled_columns_and_projections():
     if _host_gb() < 16:
         pytest.skip("not enough host memory for the large config")

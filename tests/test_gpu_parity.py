@@ -109,6 +109,21 @@ def test_exact_integers_bit_for_bit(shape, cap_cols, sym):
     assert np.array_equal(got, oracle.full(L, t2))
 
 
+@pytest.mark.parametrize("shape", [(24, 64, 128), (16, 72, 200), (30, 48, 260)])
+def test_persistent_ring_many_items_per_cta(shape):
+    """Regression for a shared-memory WAR race in the persistent TMA kernels: every CTA runs several
+    work items back to back and every item has more k-tiles than the ring has stages, so slots are
+    refilled across item boundaries while other warps are in their epilogue.  Exact-integer inputs:
+    any stale or early fragment changes the bits.  Repeated, because the race was timing dependent."""
+    o, v, x = shape
+    L = I.make_L(v, x, 43, integer=True)
+    t2 = I.make_t2(o, v, 43, integer=True)
+    want = oracle.full(L, t2)
+    for rep in range(6):
+        got, info = gpu_ladder(L, t2, return_info=True)
+        assert np.array_equal(got, want), (rep, info)
+
+
 def test_check_inputs_flags():
     import torch
 
