@@ -72,7 +72,7 @@ typedef struct ppl_info_s {
     int32_t splitk;            /* split-K factor of step 1 (the (c,d) contraction) */
     int32_t vec16;             /* 1: 16-byte async copies (nvirt even); 0: 8-byte path */
     int32_t launches_per_apply;/* kernels launched by one ppl_apply */
-    int32_t reserved;
+    int32_t step1_tile_m;      /* CTA tile rows of step 1 (16*NI chosen to tile nocc^2 with least padding) */
     uint64_t workspace_bytes;  /* device bytes owned by the plan */
     double flops_nominal;      /* F_nom */
     double flops_executed;     /* F_exec: step 0 + step 1 over executed tiles (incl. tile padding: none) */

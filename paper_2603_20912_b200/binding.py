@@ -28,14 +28,14 @@ class ppl_info_t(ctypes.Structure):
         ("nocc", c_int32), ("nvirt", c_int32), ("nchol", c_int32), ("symmetry", c_int32),
         ("ta", c_int32), ("tb", c_int32), ("n_ablocks", c_int32), ("n_bblocks", c_int32),
         ("n_tiles", c_int32), ("ring", c_int32), ("splitk", c_int32), ("vec16", c_int32),
-        ("launches_per_apply", c_int32), ("reserved", c_int32),
+        ("launches_per_apply", c_int32), ("step1_tile_m", c_int32),
         ("workspace_bytes", c_uint64),
         ("flops_nominal", c_double), ("flops_executed", c_double),
         ("flops_step0", c_double), ("flops_step1", c_double),
     ]
 
     def asdict(self):
-        return {k: getattr(self, k) for k, _ in self._fields_ if k != "reserved"}
+        return {k: getattr(self, k) for k, _ in self._fields_}
 
 
 class ppl_times_t(ctypes.Structure):

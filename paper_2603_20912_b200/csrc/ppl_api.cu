@@ -63,6 +63,7 @@ struct ppl_plan_s {
     // host-path staging buffers (ppl_apply_host)
     double *dL = nullptr, *dT = nullptr, *dR = nullptr;
     double f_step0 = 0, f_step1 = 0;
+    int ni1 = 8, bm1 = 128;          // step-1 CTA tile rows = 16*ni1 on the TMA path (128 on the cp.async path)
     int use_tma = 0;                 // 1: persistent TMA/mbarrier kernels (nvirt even); 0: cp.async kernels
     CUtensorMap mapW[MAX_RING];      // W slots as {inner nvirt^2, outer T*T}, built at plan time
 };
@@ -80,10 +81,24 @@ struct SplitChoice {
     double seconds;
 };
 
-SplitChoice choose_split(int M, int N, int K, int sms) {
-    const int tiles = ((M + ppl::BM - 1) / ppl::BM) * ((N + ppl::BN - 1) / ppl::BN);
+// CTA tile rows of step 1: 16*NI with NI in 5..10 chosen to pad nocc^2 the least (ties: larger tile)
+int choose_ni(int M) {
+    int best = 8;
+    long best_pad = -1;
+    for (int ni = 10; ni >= 5; --ni) {
+        const long bm = 16 * ni, pad = ((M + bm - 1) / bm) * bm;
+        if (best_pad < 0 || pad < best_pad) {
+            best_pad = pad;
+            best = ni;
+        }
+    }
+    return best;
+}
+
+SplitChoice choose_split(int M, int N, int K, int sms, int bm) {
+    const int tiles = ((M + bm - 1) / bm) * ((N + ppl::BN - 1) / ppl::BN);
     const int nkt = (K + ppl::BK - 1) / ppl::BK;
-    const double tau = 2.0 * ppl::BM * ppl::BN * ppl::BK / (PEAK_FLOPS / sms);  // one k-tile on one SM
+    const double tau = 2.0 * bm * ppl::BN * ppl::BK / (PEAK_FLOPS / sms);  // one k-tile on one SM
     SplitChoice best{1, nkt * ppl::BK, 1e300};
     const int smax = std::max(1, std::min(nkt / 8 + 1, 64));
     for (int s = 1; s <= smax; ++s) {
@@ -110,7 +125,7 @@ struct PlanEval {
     size_t slot_bytes = 0, part_bytes = 0;
 };
 
-PlanEval evaluate(int o, int v, int x, int T, int sym, int sms) {
+PlanEval evaluate(int o, int v, int x, int T, int sym, int sms, int bm1) {
     PlanEval ev;
     const int nblk = (v + T - 1) / T;
     const int64_t vv = (int64_t)v * v;
@@ -136,7 +151,7 @@ PlanEval evaluate(int o, int v, int x, int T, int sym, int sms) {
             if (cnt == 0) continue;
             const int ta = ae ? r : T, tb = be ? r : T;
             const int N = ta * tb;
-            const SplitChoice sc = choose_split(M, N, (int)std::min<int64_t>(vv, INT32_MAX), sms);
+            const SplitChoice sc = choose_split(M, N, (int)std::min<int64_t>(vv, INT32_MAX), sms, bm1);
             const double compute = step0_seconds(ta, tb, v, x, sms) + sc.seconds;
             const double dram = (t2_bytes + 2.0 * N * vv * 8.0) / HBM_BPS;
             total += cnt * (std::max(compute, dram) + 3 * LAUNCH_S);
@@ -161,7 +176,7 @@ int build_tiles(ppl_plan_s *p) {
             t.b0 = bb * T;
             t.tb = std::min(T, v - t.b0);
             t.mirror = (p->sym == PPL_SYM_PAIR && ab != bb) ? 1 : 0;
-            const SplitChoice sc = choose_split(p->o * p->o, t.ta * t.tb, (int)vv, p->num_sms);
+            const SplitChoice sc = choose_split(p->o * p->o, t.ta * t.tb, (int)vv, p->num_sms, p->bm1);
             t.splitk = sc.splitk;
             t.k_per_split = sc.k_per_split;
             if ((size_t)t.splitk * p->o * p->o * t.ta * t.tb * 8 > p->part_bytes) return PPL_ERR_WORKSPACE_TOO_SMALL;
@@ -204,7 +219,10 @@ int set_kernel_attrs() {
     PPL_CUDA(cudaFuncSetAttribute(ppl::k_step1<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_K));
     PPL_CUDA(cudaFuncSetAttribute(ppl::k_step1<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_K));
     PPL_CUDA(cudaFuncSetAttribute(ppl::k_step0_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_TMA));
-    PPL_CUDA(cudaFuncSetAttribute(ppl::k_step1_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_TMA));
+#define PPL_ATTR_NI(NI) \
+    PPL_CUDA(cudaFuncSetAttribute(ppl::k_step1_tma<NI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::Step1Cfg<NI>::SMEM));
+    PPL_ATTR_NI(5) PPL_ATTR_NI(6) PPL_ATTR_NI(7) PPL_ATTR_NI(8) PPL_ATTR_NI(9) PPL_ATTR_NI(10)
+#undef PPL_ATTR_NI
     g_attr_set = true;
     return PPL_OK;
 }
@@ -328,8 +346,17 @@ int launch_step1_tma(const ppl_plan_s *p, const Tile &t, const CUtensorMap &mapT
     a.k_per_split = t.k_per_split;
     a.splitk = t.splitk;
     a.part = p->part;
-    const int items = ((a.M + ppl::BM - 1) / ppl::BM) * ((a.N + ppl::BN - 1) / ppl::BN) * t.splitk;
-    ppl::k_step1_tma<<<std::min(items, p->num_sms), ppl::TMA_THREADS, ppl::SMEM_TMA, s>>>(mapT, mapW, a);
+    const int items = ((a.M + p->bm1 - 1) / p->bm1) * ((a.N + ppl::BN - 1) / ppl::BN) * t.splitk;
+    const int grid = std::min(items, p->num_sms);
+    switch (p->ni1) {
+#define PPL_LAUNCH_NI(NI)                                                                                        \
+    case NI:                                                                                                     \
+        ppl::k_step1_tma<NI><<<grid, ppl::TMA_THREADS, ppl::Step1Cfg<NI>::SMEM, s>>>(mapT, mapW, a);           \
+        break;
+        PPL_LAUNCH_NI(5) PPL_LAUNCH_NI(6) PPL_LAUNCH_NI(7) PPL_LAUNCH_NI(8) PPL_LAUNCH_NI(9) PPL_LAUNCH_NI(10)
+#undef PPL_LAUNCH_NI
+        default: return fail(PPL_ERR_INVALID_ARG);
+    }
     PPL_CUDA(cudaGetLastError());
     return PPL_OK;
 }
@@ -340,7 +367,7 @@ struct ApplyMaps {
 int make_apply_maps(const ppl_plan_s *p, const double *L, const double *t2, ApplyMaps *m) {
     const uint64_t vv = (uint64_t)p->v * p->v;
     int rc = make_map_2d(&m->L, L, vv, (uint64_t)p->x, vv * 8, 16, ppl::BK);
-    if (rc == PPL_OK) rc = make_map_2d(&m->T, t2, vv, (uint64_t)p->o * p->o, vv * 8, ppl::BK, ppl::BM);
+    if (rc == PPL_OK) rc = make_map_2d(&m->T, t2, vv, (uint64_t)p->o * p->o, vv * 8, ppl::BK, (uint32_t)p->bm1);
     return rc;
 }
 
@@ -412,6 +439,13 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
     const size_t auto_cap = (size_t)(0.9 * (double)free_b);
     const size_t cap = workspace_bytes ? std::min(workspace_bytes, auto_cap) : auto_cap;
 
+    const char *envk = getenv("PPL_KERNELS");  // debug override: "cpasync" forces the non-TMA kernels
+    p->use_tma = p->vec16 && !(envk && strcmp(envk, "cpasync") == 0) && get_encode() != nullptr;
+    if (p->use_tma) {
+        const char *envni = getenv("PPL_NI");  // debug override of the step-1 tile height
+        p->ni1 = (envni && atoi(envni) >= 5 && atoi(envni) <= 10) ? atoi(envni) : choose_ni(nocc * nocc);
+        p->bm1 = 16 * p->ni1;
+    }
     // choose the tile edge T (and ring depth) that minimises the estimated apply time under the cap
     const char *envT = getenv("PPL_TILE");  // debug override
     double best_t = 1e300;
@@ -423,7 +457,7 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
         const int nblk = (nvirt + T - 1) / T;
         const int r = nvirt - (nblk - 1) * T;
         if (!envT && nblk > 1 && 2 * r < T) continue;
-        const PlanEval ev = evaluate(nocc, nvirt, nchol, T, PPL_SYM_PAIR, p->num_sms);
+        const PlanEval ev = evaluate(nocc, nvirt, nchol, T, PPL_SYM_PAIR, p->num_sms, p->bm1);
         // the same plan must also serve PPL_SYM_NONE (same shapes), so part/slot sizes are identical
         int ring = 0;
         for (int rg = std::min(3, MAX_RING); rg >= 1; --rg)
@@ -476,8 +510,6 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
         fail(PPL_ERR_CUDA);
         return nullptr;
     }
-    const char *envk = getenv("PPL_KERNELS");  // debug override: "cpasync" forces the non-TMA kernels
-    p->use_tma = p->vec16 && !(envk && strcmp(envk, "cpasync") == 0) && get_encode() != nullptr;
     if (p->use_tma) {
         const uint64_t vv = (uint64_t)nvirt * nvirt;
         for (int i = 0; i < p->ring; ++i)
@@ -517,6 +549,7 @@ int ppl_plan_info(const ppl_plan_t *p, ppl_info_t *out) {
     out->splitk = p->tiles.empty() ? 0 : p->tiles[0].splitk;
     out->vec16 = p->vec16;
     out->launches_per_apply = 3 * (int)p->tiles.size();
+    out->step1_tile_m = p->bm1;
     out->workspace_bytes = p->ws_bytes;
     const double v4 = std::pow((double)p->v, 4);
     out->flops_nominal = 2.0 * p->x * v4 + 2.0 * p->o * p->o * v4;

@@ -247,8 +247,11 @@ __global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_tma(const __grid_const
 
 // ---------------------------------------------------------------------------------------------
 // step 1 (TMA):  part[z][(i,j)][(a,b)] = sum_{(c,d) in split z} t2[(i,j)][(c,d)] W[(a,b)][(c,d)]
-// mapA: t2 as {inner = nvirt^2, outer = nocc^2};  mapB: W slot as {inner = nvirt^2, outer = T*T};
-// box {16, 128}, SWIZZLE_128B.
+// mapA: t2 as {inner = nvirt^2, outer = nocc^2}, box {16, 16*NI};  mapB: W slot as {inner = nvirt^2,
+// outer = T*T}, box {16, 128}; SWIZZLE_128B.
+// NI = 8-row blocks per warp along M: CTA tile (16*NI) x 128.  nocc^2 is rarely a multiple of 128
+// (1600, 3600, 400), and rows padded up to a tile are DMMA work that counts for nothing; the host
+// picks NI in 5..10 that tiles nocc^2 with the least padding (160 | 1600, 144 | 3600, 80 | 400).
 // ---------------------------------------------------------------------------------------------
 struct Step1TmaArgs {
     int M, N, K;      // nocc^2, ta*tb, nvirt^2
@@ -257,14 +260,33 @@ struct Step1TmaArgs {
     double *part;     // [splitk][M][N]
 };
 
+template <int NI>
+struct Step1Cfg {
+    static constexpr int BM1 = 16 * NI;                                   // CTA tile rows
+    static constexpr int WTM1 = 8 * NI;                                   // warp tile rows
+    static constexpr uint32_t A_BYTES = BM1 * BK * sizeof(double);
+    static constexpr uint32_t STAGE = A_BYTES + TILE_BYTES;               // A + B(128 x 16)
+    static constexpr size_t SMEM = (size_t)TSTAGES * STAGE + 1024 + 256;
+};
+
+template <int NI>
 __global__ void __launch_bounds__(TMA_THREADS, 1)
     k_step1_tma(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, const Step1TmaArgs p) {
+    using Cfg = Step1Cfg<NI>;
+    constexpr int BM1 = Cfg::BM1, WTM1 = Cfg::WTM1;
     extern __shared__ unsigned char smem_raw[];
-    const TmaSmem sm = carve_smem(smem_raw);
+    // ring: [TSTAGES] A tiles, then [TSTAGES] B tiles, then the barriers
+    const uint32_t base = smem_u32(smem_raw);
+    unsigned char *al = smem_raw + ((1024u - (base & 1023u)) & 1023u);
+    TmaSmem sm;
+    sm.a = reinterpret_cast<double *>(al);
+    sm.b = reinterpret_cast<double *>(al + (size_t)TSTAGES * Cfg::A_BYTES);
+    sm.full = reinterpret_cast<uint64_t *>(al + (size_t)TSTAGES * Cfg::STAGE);
+    sm.empty = sm.full + TSTAGES;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     init_barriers(sm, tid);
 
-    const int tiles_m = (p.M + BM - 1) / BM, tiles_n = (p.N + BN - 1) / BN;
+    const int tiles_m = (p.M + BM1 - 1) / BM1, tiles_n = (p.N + BN - 1) / BN;
     const int tiles_mn = tiles_m * tiles_n;
     const int num_items = tiles_mn * p.splitk;
 
@@ -281,8 +303,8 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
                 const int kbeg = z * p.k_per_split, kend = min(p.K, kbeg + p.k_per_split);
                 for (int k = kbeg; k < kend; k += BK) {
                     mbar_wait(&sm.empty[stage], phase ^ 1);
-                    mbar_expect_tx(&sm.full[stage], STAGE_BYTES);
-                    tma_load_2d(sm.a + (size_t)stage * BM * BK, &mapA, k, tm * BM, &sm.full[stage]);
+                    mbar_expect_tx(&sm.full[stage], Cfg::STAGE);
+                    tma_load_2d(sm.a + (size_t)stage * BM1 * BK, &mapA, k, tm * BM1, &sm.full[stage]);
                     tma_load_2d(sm.b + (size_t)stage * BN * BK, &mapB, k, tn * BN, &sm.full[stage]);
                     if (++stage == TSTAGES) {
                         stage = 0;
@@ -305,33 +327,33 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
     for (int item = blockIdx.x; item < num_items; item += gridDim.x) {
         const int z = item / tiles_mn, r = item - z * tiles_mn;
         const int tm = r % tiles_m, tn = r / tiles_m;
-        const int m0 = tm * BM, n0 = tn * BN;
+        const int m0 = tm * BM1, n0 = tn * BN;
         const int kbeg = z * p.k_per_split, kend = min(p.K, kbeg + p.k_per_split);
-        double acc[8][4][2];
+        double acc[NI][4][2];
 #pragma unroll
-        for (int i = 0; i < 8; ++i)
+        for (int i = 0; i < NI; ++i)
 #pragma unroll
             for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
         for (int k = kbeg; k < kend; k += BK) {
             mbar_wait(&sm.full[stage], phase);
             release_previous(sm, rel_stage, lane);
-            const double *as = sm.a + (size_t)stage * BM * BK + (wm * WTM) * BK;
+            const double *as = sm.a + (size_t)stage * BM1 * BK + (wm * WTM1) * BK;
             const double *bs = sm.b + (size_t)stage * BN * BK + (wn * WTN) * BK;
 #pragma unroll
             for (int k8 = 0; k8 < BK / 8; ++k8) {
                 const int off = k8 ? off1 : off0;
-                double2 a[8], b[4];
+                double2 a[NI], b[4];
 #pragma unroll
-                for (int i = 0; i < 8; ++i) a[i] = *reinterpret_cast<const double2 *>(as + i * 8 * BK + off);
+                for (int i = 0; i < NI; ++i) a[i] = *reinterpret_cast<const double2 *>(as + i * 8 * BK + off);
 #pragma unroll
                 for (int j = 0; j < 4; ++j) b[j] = *reinterpret_cast<const double2 *>(bs + j * 8 * BK + off);
 #pragma unroll
-                for (int i = 0; i < 8; ++i)
+                for (int i = 0; i < NI; ++i)
 #pragma unroll
                     for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i].x, b[j].x);
 #pragma unroll
-                for (int i = 0; i < 8; ++i)
+                for (int i = 0; i < NI; ++i)
 #pragma unroll
                     for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i].y, b[j].y);
             }
@@ -344,8 +366,8 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
         // epilogue: block (i,j): frag row g <-> m = mw + 8i + c(g); c0 <-> n = nw + 8j + q, c1 <-> n + 4
         double *part = p.part + (int64_t)z * p.M * p.N;
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            const int m = m0 + wm * WTM + 8 * i + c;
+        for (int i = 0; i < NI; ++i) {
+            const int m = m0 + wm * WTM1 + 8 * i + c;
             if (m >= p.M) continue;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
