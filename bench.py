@@ -38,6 +38,7 @@ if ROOT not in sys.path:
 
 METRIC = "pp_ladder_fp64_tflops_executed"
 UNIT = "TFLOP/s"
+SYM_NAMES = {0: "none", 1: "pair", 2: "pair_sa"}
 NOMINAL_FP64_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 * 1e-12  # 148 SM x 4 SMSP x 16 FMA/clk x 2 x 1.965 GHz = 37.23
 
 
@@ -251,8 +252,11 @@ def main():
     # per-launch DRAM traffic of the dominant kernel from the committed ncu --set full capture, if any
     traffic = None
     try:
-        tr = json.load(open(os.path.join(ROOT, "profiles", "dram_traffic.json")))
-        traffic = tr.get(args.config, {}).get(dom)
+        import csv
+
+        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "dram_traffic.csv"))):
+            if row["config"] == args.config and row["symmetry"] == SYM_NAMES[info["symmetry"]] and row["kernel"] == dom:
+                traffic = float(row["dram_bytes_per_launch"])
     except Exception:
         pass
     roofline = {

@@ -45,6 +45,8 @@ def _load():
         lib.ppl_oracle_columns.restype = i
         lib.ppl_oracle_project.argtypes = [i, i, i, _dp, _dp, _dp, _dp, _dp, _dp]
         lib.ppl_oracle_project.restype = i
+        lib.ppl_oracle_full_ex.argtypes = [i, i, i, _dp, _dp, _dp, i, i, ctypes.c_double, ctypes.c_double]
+        lib.ppl_oracle_full_ex.restype = i
         _lib = lib
     return _lib
 
@@ -116,3 +118,22 @@ def project(L, t2, u, w):
     if rc:
         raise RuntimeError(f"oracle error {rc}")
     return out, absout
+
+
+LAYOUTS = {"ijab": 0, "iajb": 1}
+
+
+def full_ex(L, t2, R=None, t2_layout="ijab", r_layout="ijab", alpha=1.0, beta=1.0):
+    """R = beta*R + alpha*term with t2 / R stored 'ijab' ([i,j,c,d]) or 'iajb' ([i,c,j,d], the paper's
+    'icjd' -> 'iajb').  Shapes follow the layouts; R=None starts from zeros."""
+    x, v, _ = L.shape
+    o = t2.shape[0]
+    shp = {"ijab": (o, o, v, v), "iajb": (o, v, o, v)}
+    _chk(L, (x, v, v))
+    _chk(t2, shp[t2_layout])
+    R = np.zeros(shp[r_layout]) if R is None else _chk(R, shp[r_layout])
+    rc = _load().ppl_oracle_full_ex(o, v, x, _p(L), _p(t2), _p(R), LAYOUTS[t2_layout], LAYOUTS[r_layout],
+                                    float(alpha), float(beta))
+    if rc:
+        raise RuntimeError(f"oracle error {rc}")
+    return R

@@ -231,3 +231,60 @@ int ppl_oracle_project(int nocc, int nvirt, int nchol, const double *L, const do
     free(M);
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * Paper-layout / scaled variant.  The paper stores the amplitudes as
+ * 'icjd' and the result as 'iajb' (einsum 'xac,xbd,icjd->iajb'; also written
+ * '->efab') and pays a transpose to get there.
+ * This entry point evaluates the same definition with either storage order on either side:
+ *
+ *     R = beta * R + alpha * sum_{c,d} ( sum_P L[P,a,c] L[P,b,d] ) t[i,j,c,d]
+ *
+ *   layout 0 ("ijab"): element (i,j,p,q) at ((i*o + j)*v + p)*v + q     -- BASELINE.json / 'efab'
+ *   layout 1 ("iajb"): element (i,j,p,q) at ((i*v + p)*o + j)*v + q     -- the paper's 'icjd' / 'iajb'
+ * beta == 0 means overwrite: R is not read (it may hold NaN).  Same two steps per (a,b) column as
+ * ladder_column above, written out again with the index maps so it can be checked by eye.
+ * ------------------------------------------------------------------------------------------------ */
+static int64_t idx4(int layout, int64_t o, int64_t v, int64_t i, int64_t j, int64_t p, int64_t q) {
+    return layout == 0 ? ((i * o + j) * v + p) * v + q : ((i * v + p) * o + j) * v + q;
+}
+
+int ppl_oracle_full_ex(int nocc, int nvirt, int nchol, const double *L, const double *t2, double *R,
+                       int t2_layout, int r_layout, double alpha, double beta) {
+    if (nocc < 1 || nvirt < 1 || nchol < 1 || !L || !t2 || !R) return 1;
+    if ((t2_layout != 0 && t2_layout != 1) || (r_layout != 0 && r_layout != 1)) return 1;
+    const int64_t o = nocc, v = nvirt, x = nchol, vv = v * v;
+    int fail = 0;
+#pragma omp parallel
+    {
+        double *Wab = (double *)malloc(sizeof(double) * (size_t)vv);
+        if (!Wab) {
+#pragma omp atomic write
+            fail = 1;
+        }
+#pragma omp barrier
+        if (!fail) {
+#pragma omp for schedule(dynamic, 1)
+            for (int64_t ab = 0; ab < vv; ++ab) {
+                const int64_t a = ab / v, b = ab % v;
+                /* step 0: Wab[c][d] = sum_P L[P][a][c] L[P][b][d] */
+                memset(Wab, 0, sizeof(double) * (size_t)vv);
+                for (int64_t P = 0; P < x; ++P)
+                    for (int64_t c = 0; c < v; ++c)
+                        for (int64_t d = 0; d < v; ++d)
+                            Wab[c * v + d] += L[(P * v + a) * v + c] * L[(P * v + b) * v + d];
+                /* step 1: one dot product over (c,d) per (i,j) */
+                for (int64_t i = 0; i < o; ++i)
+                    for (int64_t j = 0; j < o; ++j) {
+                        double s = 0.0;
+                        for (int64_t c = 0; c < v; ++c)
+                            for (int64_t d = 0; d < v; ++d) s += Wab[c * v + d] * t2[idx4(t2_layout, o, v, i, j, c, d)];
+                        double *r = R + idx4(r_layout, o, v, i, j, a, b);
+                        *r = (beta == 0.0) ? alpha * s : beta * (*r) + alpha * s;
+                    }
+            }
+        }
+        free(Wab);
+    }
+    return fail ? 3 : 0;
+}

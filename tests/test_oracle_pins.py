@@ -266,3 +266,87 @@ def test_input_recipe():
     assert not np.array_equal(L, I.make_L(v, x, 1))
     p = I.sample_pairs(400, 64, seed=0)
     assert p.min() >= 0 and p.max() < 400 and len({tuple(r) for r in p}) == len(p)
+
+
+# ------------------------------------------------------------------ NEXT-1: paper layouts, alpha/beta
+@pytest.mark.parametrize("shape", [(3, 4, 5), (2, 7, 3), (1, 1, 1), (4, 3, 2)])
+def test_full_ex_is_the_papers_einsum_string(shape):
+    """PAPER.md:75 prints the contraction as 'xac,xbd,icjd->iajb': evaluate exactly that string with
+    numpy on arrays stored the paper's way and compare with oracle.full_ex in every layout combination."""
+    o, v, x = shape
+    L = I.make_L(v, x, 3, symmetric=False)
+    t_ijcd = I.make_t2(o, v, 3, symmetric=False)
+    t_icjd = np.ascontiguousarray(t_ijcd.transpose(0, 2, 1, 3))
+    want_iajb = np.einsum("xac,xbd,icjd->iajb", L, L, t_icjd)
+    want_ijab = np.ascontiguousarray(want_iajb.transpose(0, 2, 1, 3))
+    for tl, t in (("ijab", t_ijcd), ("iajb", t_icjd)):
+        for rl, want in (("ijab", want_ijab), ("iajb", want_iajb)):
+            assert rel(oracle.full_ex(L, t, None, tl, rl), want) <= RTOL
+    # the 'ijab'/'ijab' case is oracle.full itself
+    assert rel(oracle.full_ex(L, t_ijcd), oracle.full(L, t_ijcd)) <= RTOL
+
+
+def test_full_ex_alpha_beta_and_overwrite():
+    o, v, x = 3, 5, 4
+    L, t = rand_inputs(o, v, x, seed=5)
+    term = oracle.full(L, t)
+    R0 = I.make_vec(o * o * v * v, 5, 40).reshape(o, o, v, v)
+    got = oracle.full_ex(L, t, R0.copy(), alpha=-0.5, beta=2.0)
+    assert rel(got, 2.0 * R0 - 0.5 * term) <= RTOL
+    # beta = 0 overwrites and never reads R (NaN on entry must not propagate)
+    got = oracle.full_ex(L, t, np.full((o, o, v, v), np.nan), alpha=3.0, beta=0.0)
+    assert np.isfinite(got).all() and rel(got, 3.0 * term) <= RTOL
+    # wrong-layout negative control: reading 'icjd' storage as 'ijcd' gives a different answer
+    o, v, x = 3, 3, 2  # o == v so the shapes coincide and only the index meaning differs
+    L, t = rand_inputs(o, v, x, seed=6)
+    a = oracle.full_ex(L, t, None, "ijab", "ijab")
+    b = oracle.full_ex(L, t.reshape(o, v, o, v), None, "iajb", "ijab")
+    assert rel(a, b) > 1e-3
+
+
+# ------------------------------------------------ NEXT-4: symmetric / antisymmetric repacking identity
+@pytest.mark.parametrize("shape", [(3, 5, 4), (4, 6, 3), (1, 4, 2), (2, 1, 3)])
+def test_symmetric_antisymmetric_packing_identity(shape):
+    """For pair-symmetric t2 (t[i,j,c,d] = t[j,i,d,c]) and ANY L the term splits as
+         R[i,j,a,b] = R+ + R-,  R[j,i,a,b] = R+ - R-   (i <= j),
+         R+-[ij,ab] = sum_{c<=d} W+-[ab,cd] tau+-[ij,cd],
+         W+-[ab,cd] = (ac|bd) +- (ad|bc)  (c<d; W+[ab,cc] = (ac|bc)),
+         tau+-[ij,cd] = (t[ij,cd] +- t[ij,dc]) / 2  (c<d; tau+[ij,cc] = t[ij,cc])
+    -- the packing the CUDA path's PPL_SYM_PAIR_SA mode uses.  Built here with numpy from
+    the definitions and checked against the oracle, so the identity itself is pinned on the CPU."""
+    o, v, x = shape
+    L = I.make_L(v, x, 9, symmetric=False)
+    t = I.make_t2(o, v, 9, symmetric=True)
+    want = oracle.full(L, t)
+    X = np.einsum("Pac,Pbd->abcd", L, L)
+    cu, du = np.triu_indices(v)
+    cs, ds = np.triu_indices(v, 1)
+    off = (cu != du).astype(np.float64)
+    Wp = X[:, :, cu, du] + off * X[:, :, du, cu]
+    Wm = X[:, :, cs, ds] - X[:, :, ds, cs]
+    tp = np.where(cu == du, 1.0, 0.5) * (t[:, :, cu, du] + off * t[:, :, du, cu])
+    tm = 0.5 * (t[:, :, cs, ds] - t[:, :, ds, cs])
+    Rp = np.einsum("abk,ijk->ijab", Wp, tp)
+    Rm = np.einsum("abk,ijk->ijab", Wm, tm)
+    got = np.zeros_like(want)
+    for i in range(o):
+        for j in range(i, o):
+            got[i, j] = Rp[i, j] + Rm[i, j]
+            if i != j:
+                got[j, i] = Rp[i, j] - Rm[i, j]
+    assert rel(got, want) <= RTOL
+    # negative control: without pair symmetry the reconstruction from i <= j fails
+    if o > 1 and v > 1:
+        tn = I.make_t2(o, v, 9, symmetric=False)
+        wantn = oracle.full(L, tn)
+        tpn = np.where(cu == du, 1.0, 0.5) * (tn[:, :, cu, du] + off * tn[:, :, du, cu])
+        tmn = 0.5 * (tn[:, :, cs, ds] - tn[:, :, ds, cs])
+        Rpn = np.einsum("abk,ijk->ijab", Wp, tpn)
+        Rmn = np.einsum("abk,ijk->ijab", Wm, tmn)
+        gotn = np.zeros_like(wantn)
+        for i in range(o):
+            for j in range(i, o):
+                gotn[i, j] = Rpn[i, j] + Rmn[i, j]
+                if i != j:
+                    gotn[j, i] = Rpn[i, j] - Rmn[i, j]
+        assert rel(gotn, wantn) > 1e-3
