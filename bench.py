@@ -39,6 +39,9 @@ if ROOT not in sys.path:
 METRIC = "pp_ladder_fp64_tflops_executed"
 UNIT = "TFLOP/s"
 SYM_NAMES = {0: "none", 1: "pair", 2: "pair_sa"}
+SYM_DESC = {0: "none (every tile)", 1: "pair (tiles a-block<=b-block, mirrored)",
+            2: "pair_sa (tiles a-block<=b-block, mirrored; step 1 on symmetric/antisymmetric packed (i<=j),(c<=d) operands: "
+               "step-0 flops x~1/2, step-1 flops x~1/4 of nominal)"}
 NOMINAL_FP64_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 * 1e-12  # 148 SM x 4 SMSP x 16 FMA/clk x 2 x 1.965 GHz = 37.23
 
 
@@ -164,6 +167,8 @@ def main():
     ap.add_argument("--config", default="large")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workspace-gb", type=float, default=0.0, help="workspace cap (0 = auto)")
+    ap.add_argument("--symmetry", default="default", choices=["default", "pair_sa", "pair", "none"],
+                    help="default = the plan's own choice (pair_sa: A<=B tiles + symmetric/antisymmetric packed step 1)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -210,6 +215,8 @@ def main():
     t0 = time.perf_counter()
     plan = P.Plan(o, v, x, int(args.workspace_gb * (1 << 30)))
     plan_s = time.perf_counter() - t0
+    if args.symmetry != "default":
+        plan.set_symmetry({v_: k_ for k_, v_ in SYM_NAMES.items()}[args.symmetry])
     info = plan.info()
     stream = torch.cuda.current_stream()
 
@@ -269,7 +276,9 @@ def main():
         "step0_tflops": info["flops_step0"] / (prof["step0_ms"] * 1e-3) * 1e-12,
         "step1_tflops": info["flops_step1"] / (prof["step1_ms"] * 1e-3) * 1e-12,
         "share": {"step0": prof["step0_ms"] / prof["total_ms"], "step1": prof["step1_ms"] / prof["total_ms"],
-                  "reduce": prof["reduce_ms"] / prof["total_ms"]},
+                  "reduce": prof["reduce_ms"] / prof["total_ms"], "fold": prof["fold_ms"] / prof["total_ms"],
+                  "pack": prof["pack_ms"] / prof["total_ms"]},
+        "launches": {k: prof["n_" + k] for k in ("step0", "step1", "reduce", "fold", "pack")},
     }
 
     line = {
@@ -277,7 +286,7 @@ def main():
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": args.config, "nocc": o, "nvirt": v, "nchol": x, "seed": 0,
-                   "symmetry": "pair (tiles a-block<=b-block, mirrored)", "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "symmetry": SYM_DESC[info["symmetry"]], "parallelism": "replicas only" if world > 1 else "1 gpu",
                    "l2": "inputs larger than L2 (L, t2, W tiles >> 126 MB); no flush needed",
                    "plan": {k: info[k] for k in ("ta", "tb", "n_tiles", "ring", "splitk", "vec16", "workspace_bytes")}},
         "seconds_per_call": ms_per_step * 1e-3,

@@ -53,12 +53,34 @@ enum {
 /* Symmetry modes (ppl_plan_set_symmetry). */
 enum {
     PPL_SYM_NONE = 0, /* general t2: every (a-block, b-block) tile is computed */
-    PPL_SYM_PAIR = 1  /* t2[i,j,c,d] == t2[j,i,d,c] (holds for CC amplitudes): then
+    PPL_SYM_PAIR = 1, /* t2[i,j,c,d] == t2[j,i,d,c] (holds for CC amplitudes): then
                          R_term[i,j,a,b] == R_term[j,i,b,a] for ANY L, so only tiles with
-                         a-block <= b-block are computed and the result is also accumulated into
-                         the mirrored entries.  Default.  Result undefined if t2 is not
-                         pair-symmetric (ppl_check_inputs detects that). */
+                         a-block <= b-block are computed and the result is also written into
+                         the mirrored entries.  Result undefined if t2 is not pair-symmetric
+                         (ppl_check_inputs detects that). */
+    PPL_SYM_PAIR_SA = 2 /* same precondition as PPL_SYM_PAIR, and the same tiles; in addition step 1
+                         runs on symmetric / antisymmetric packed operands
+                             W+-[(ab)][(c<=d)] = (ac|bd) +- (ad|bc),  tau+-[(i<=j)][(c<=d)] = (t2[ij,cd] +- t2[ij,dc])/2,
+                             R[i,j,a,b] = R+ + R-,  R[j,i,a,b] = R+ - R-,
+                         which halves the flops of step 1 again (an identity for ANY L; SURVEY.md 8(f)
+                         NEXT-4, pinned on the CPU by tests/test_oracle_pins.py).  Default. */
 };
+
+/* Storage orders of the 4-index arrays t2 and R. */
+enum {
+    PPL_LAYOUT_IJAB = 0, /* [i][j][c][d] / [i][j][a][b]: BASELINE.json's layout, the paper's 'efab' */
+    PPL_LAYOUT_IAJB = 1  /* [i][c][j][d] / [i][a][j][b]: the paper's 'icjd' and 'iajb' */
+};
+
+/* Options of ppl_apply_ex.  R = beta * R + alpha * term.  beta == 0 overwrites: R is not read and
+ * may be uninitialised.  The permutations are folded into the packing / reduction kernels'
+ * addressing (the paper pays a transpose for them). */
+typedef struct ppl_opts_s {
+    int32_t t2_layout; /* PPL_LAYOUT_* of t2 */
+    int32_t r_layout;  /* PPL_LAYOUT_* of R  */
+    double alpha;      /* 1.0 in ppl_apply */
+    double beta;       /* 1.0 in ppl_apply (accumulate) */
+} ppl_opts_t;
 
 /* What the planner chose; filled by ppl_plan_info.  Flop counts follow BASELINE.json:
  * F_nom = 2*nchol*nvirt^4 + 2*nocc^2*nvirt^4; F_exec counts the tiles actually executed. */
@@ -78,6 +100,10 @@ typedef struct ppl_info_s {
     double flops_executed;     /* F_exec: step 0 + step 1 over executed tiles (incl. tile padding: none) */
     double flops_step0;        /* executed flops of step 0 ('xac,xbd->acbd') */
     double flops_step1;        /* executed flops of step 1 ('acbd,ecfd->efab') */
+    int32_t sa_splitk_plus, sa_splitk_minus; /* PPL_SYM_PAIR_SA: split-K of the + / - GEMMs (first tile) */
+    int32_t sa_tile_m_plus, sa_tile_m_minus; /* PPL_SYM_PAIR_SA: CTA tile rows of the + / - GEMMs */
+    int32_t sa_rows_plus, sa_rows_minus;     /* nocc(nocc+1)/2, nocc(nocc-1)/2 */
+    int32_t sa_k_plus, sa_k_minus;           /* nvirt(nvirt+1)/2, nvirt(nvirt-1)/2 */
 } ppl_info_t;
 
 /* Per-stage device times of the most recent profiled apply (ppl_apply_profiled), milliseconds. */
@@ -87,6 +113,9 @@ typedef struct ppl_times_s {
     float step1_ms;  /* sum over tiles of the (c,d) contraction kernel */
     float reduce_ms; /* sum over tiles of the split-K reduction + accumulate + mirror kernel */
     int32_t n_step0, n_step1, n_reduce; /* launches */
+    float fold_ms;   /* PPL_SYM_PAIR_SA: sum over tiles of the W -> W+- fold kernel */
+    float pack_ms;   /* PPL_SYM_PAIR_SA: t2 -> tau+- packing (once per apply); other modes: t2 permute if any */
+    int32_t n_fold, n_pack;
 } ppl_times_t;
 
 /* ppl_plan: choose tile shape, ring depth and split-K for (nocc, nvirt, nchol) and allocate the
@@ -109,6 +138,23 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes);
  *   until the queued work completes. */
 int ppl_apply(ppl_plan_t *plan, const double *L, const double *t2, double *R, void *stream);
 
+/* ppl_apply_ex: ppl_apply with options (storage orders of t2 and R, alpha, beta); opts == NULL
+ * means the defaults of ppl_apply.  Same stream semantics.  In the un-packed modes
+ * (PPL_SYM_NONE / PPL_SYM_PAIR) a t2 given as PPL_LAYOUT_IAJB is first permuted into a plan-owned
+ * buffer (allocated on first use, nocc^2 nvirt^2 doubles); in PPL_SYM_PAIR_SA the packing kernel
+ * reads either order in place. */
+int ppl_apply_ex(ppl_plan_t *plan, const double *L, const double *t2, double *R, const ppl_opts_t *opts,
+                 void *stream);
+
+/* ppl_apply_dense: step 1 alone on caller-supplied dense integrals (the
+ * paper's 'abcd,ecfd->efab'):
+ *     R[i,j,a,b] = beta*R[i,j,a,b] + alpha * sum_{c,d} eri[a-a0][b][c][d] * t2[i,j,c,d],   a0 <= a < a0+na, all b
+ * eri is a DEVICE slab [na][nvirt][nvirt][nvirt] of <ab|cd> (physicist order, as the paper's
+ * 'abcd'), i.e. exactly the [(a,b)][(c,d)] matrix step 1 consumes.  No symmetry is assumed or
+ * used.  nchol of the plan is ignored.  Only R entries with a in the slab are touched. */
+int ppl_apply_dense(ppl_plan_t *plan, const double *eri, int a0, int na, const double *t2, double *R,
+                    const ppl_opts_t *opts, void *stream);
+
 /* ppl_apply_host: the same operation on HOST buffers (pageable or pinned): copies L and t2 to
  * plan-owned device buffers, R in, runs ppl_apply, copies R back, and synchronises before
  * returning.  Device staging buffers are allocated on first use and kept by the plan (they are
@@ -130,7 +176,8 @@ int ppl_destroy(ppl_plan_t *plan);
 int ppl_last_error(void);                /* code of the last failure on this thread */
 const char *ppl_error_string(int code);  /* static string, never NULL */
 
-/* Set PPL_SYM_NONE / PPL_SYM_PAIR (default PPL_SYM_PAIR).  Re-plans the tile list; must not be
+/* Set PPL_SYM_NONE / PPL_SYM_PAIR / PPL_SYM_PAIR_SA (default PPL_SYM_PAIR_SA; PPL_SYM_PAIR if the
+ * workspace cap was too small for the packed operands).  Re-plans the tile list; must not be
  * called while an apply is in flight. */
 int ppl_plan_set_symmetry(ppl_plan_t *plan, int mode);
 

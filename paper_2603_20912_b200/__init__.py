@@ -14,7 +14,10 @@ from .binding import (  # noqa: F401
     PPL_ERR_WORKSPACE_TOO_SMALL,
     PPL_OK,
     PPL_SYM_NONE,
+    PPL_LAYOUT_IAJB,
+    PPL_LAYOUT_IJAB,
     PPL_SYM_PAIR,
+    PPL_SYM_PAIR_SA,
     SYMBOLS,
     Plan,
     PplError,

@@ -21,6 +21,10 @@ PPL_ERR_UNSUPPORTED_DEVICE = 5
 PPL_ERR_PRECONDITION = 6
 PPL_SYM_NONE = 0
 PPL_SYM_PAIR = 1
+PPL_SYM_PAIR_SA = 2
+PPL_LAYOUT_IJAB = 0
+PPL_LAYOUT_IAJB = 1
+LAYOUTS = {"ijab": PPL_LAYOUT_IJAB, "iajb": PPL_LAYOUT_IAJB}
 
 
 class ppl_info_t(ctypes.Structure):
@@ -32,6 +36,10 @@ class ppl_info_t(ctypes.Structure):
         ("workspace_bytes", c_uint64),
         ("flops_nominal", c_double), ("flops_executed", c_double),
         ("flops_step0", c_double), ("flops_step1", c_double),
+        ("sa_splitk_plus", c_int32), ("sa_splitk_minus", c_int32),
+        ("sa_tile_m_plus", c_int32), ("sa_tile_m_minus", c_int32),
+        ("sa_rows_plus", c_int32), ("sa_rows_minus", c_int32),
+        ("sa_k_plus", c_int32), ("sa_k_minus", c_int32),
     ]
 
     def asdict(self):
@@ -42,10 +50,15 @@ class ppl_times_t(ctypes.Structure):
     _fields_ = [
         ("total_ms", c_float), ("step0_ms", c_float), ("step1_ms", c_float), ("reduce_ms", c_float),
         ("n_step0", c_int32), ("n_step1", c_int32), ("n_reduce", c_int32),
+        ("fold_ms", c_float), ("pack_ms", c_float), ("n_fold", c_int32), ("n_pack", c_int32),
     ]
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class ppl_opts_t(ctypes.Structure):
+    _fields_ = [("t2_layout", c_int32), ("r_layout", c_int32), ("alpha", c_double), ("beta", c_double)]
 
 
 class PplError(RuntimeError):
@@ -58,6 +71,8 @@ class PplError(RuntimeError):
 SYMBOLS = {
     "ppl_plan": (c_void_p, [c_int, c_int, c_int, c_size_t]),
     "ppl_apply": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "ppl_apply_ex": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, POINTER(ppl_opts_t), c_void_p]),
+    "ppl_apply_dense": (c_int, [c_void_p, c_void_p, c_int, c_int, c_void_p, c_void_p, POINTER(ppl_opts_t), c_void_p]),
     "ppl_apply_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, POINTER(c_uint64), POINTER(c_uint64)]),
     "ppl_apply_profiled": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, POINTER(ppl_times_t)]),
     "ppl_destroy": (c_int, [c_void_p]),
@@ -138,6 +153,29 @@ class Plan:
         o, v, x = self.nocc, self.nvirt, self.nchol
         _check(lib().ppl_apply(self._h, _dev_ptr(L, "L", (x, v, v)), _dev_ptr(t2, "t2", (o, o, v, v)),
                                _dev_ptr(R, "R", (o, o, v, v)), _stream_ptr(stream)), "ppl_apply")
+        return R
+
+    def _shape4(self, layout: str):
+        o, v = self.nocc, self.nvirt
+        return (o, o, v, v) if layout == "ijab" else (o, v, o, v)
+
+    def apply_ex(self, L, t2, R, t2_layout="ijab", r_layout="ijab", alpha=1.0, beta=1.0, stream=None):
+        """R = beta*R + alpha*ladder(L, t2); t2 / R stored 'ijab' ([i,j,c,d]) or 'iajb' ([i,c,j,d])."""
+        v, x = self.nvirt, self.nchol
+        opts = ppl_opts_t(LAYOUTS[t2_layout], LAYOUTS[r_layout], float(alpha), float(beta))
+        _check(lib().ppl_apply_ex(self._h, _dev_ptr(L, "L", (x, v, v)), _dev_ptr(t2, "t2", self._shape4(t2_layout)),
+                                  _dev_ptr(R, "R", self._shape4(r_layout)), ctypes.byref(opts), _stream_ptr(stream)),
+               "ppl_apply_ex")
+        return R
+
+    def apply_dense(self, eri, a0, t2, R, t2_layout="ijab", r_layout="ijab", alpha=1.0, beta=1.0, stream=None):
+        """Step 1 alone on a dense slab eri[na][v][v][v] of <ab|cd>, a0 <= a < a0+na (the paper's 'abcd,ecfd->efab')."""
+        v = self.nvirt
+        na = int(eri.shape[0])
+        opts = ppl_opts_t(LAYOUTS[t2_layout], LAYOUTS[r_layout], float(alpha), float(beta))
+        _check(lib().ppl_apply_dense(self._h, _dev_ptr(eri, "eri", (na, v, v, v)), int(a0), na,
+                                     _dev_ptr(t2, "t2", self._shape4(t2_layout)), _dev_ptr(R, "R", self._shape4(r_layout)),
+                                     ctypes.byref(opts), _stream_ptr(stream)), "ppl_apply_dense")
         return R
 
     def apply_profiled(self, L, t2, R, stream=None) -> dict:

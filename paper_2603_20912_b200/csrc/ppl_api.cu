@@ -1,5 +1,6 @@
 // ppl_api.cu -- C ABI of libppl (include/ppl.h): planner, W-tile ring, stream orchestration.
-// Everything on the data path runs in the kernels of ppl_kernels.cuh; there is no CPU fallback.
+// Everything on the data path runs in the kernels of ppl_kernels.cuh / ppl_kernels_tma.cuh; there
+// is no CPU fallback.
 #include "../../include/ppl.h"
 #include "ppl_kernels.cuh"
 #include "ppl_kernels_tma.cuh"
@@ -29,10 +30,16 @@ int fail(int code) {
         }                                              \
     } while (0)
 
+struct SplitChoice {
+    int splitk = 1, k_per_split = ppl::BK;
+    double seconds = 0;
+};
+
 struct Tile {
     int a0, ta, b0, tb;
     int mirror;
-    int splitk, k_per_split;
+    SplitChoice full;    // step 1 over K = nvirt^2                (PPL_SYM_NONE / PPL_SYM_PAIR)
+    SplitChoice sp, sm;  // step 1 over the packed K+ / K- ranges  (PPL_SYM_PAIR_SA)
 };
 
 constexpr int MAX_RING = 4;
@@ -40,32 +47,41 @@ constexpr double PEAK_FLOPS = 37.2e12;  // nominal FP64 (148 SM x 64 FMA/clk x 2
 constexpr double HBM_BPS = 6.0e12;      // planner cost model only
 constexpr double LAUNCH_S = 4e-6;
 
+size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
+
 }  // namespace
 
 struct ppl_plan_s {
     int o = 0, v = 0, x = 0;
-    int sym = PPL_SYM_PAIR;
+    int sym = PPL_SYM_PAIR_SA;
+    int sa_ok = 0;        // the workspace holds the packed operands of PPL_SYM_PAIR_SA
     int T = 0;            // tile edge (ta = tb = T except at the ragged edge)
     int nblk = 0;
     int ring = 1;
     int vec16 = 0;
     int num_sms = 148;
-    int64_t ldw = 0;      // row stride of a W tile (doubles)
-    size_t cap = 0;       // workspace cap given by the caller (0 = auto)
-    size_t slot_bytes = 0, part_bytes = 0, ws_bytes = 0;
+    int use_tma = 0;      // 1: persistent TMA/mbarrier kernels; 0: cp.async kernels
+    int64_t vv = 0;       // nvirt^2 = row length of an un-packed W tile / of t2
+    // packed geometry (PPL_SYM_PAIR_SA)
+    int Mp = 0, Mm = 0;   // rows (i<=j), (i<j)
+    int Kp = 0, Km = 0;   // columns (c<=d), (c<d)
+    int64_t ldp = 0, ldm = 0;
+    int ni_full = 8, bm_full = 128, ni_p = 8, bm_p = 128, ni_m = 8, bm_m = 128;  // step-1 CTA tile rows (16*NI)
+    size_t cap = 0;
+    size_t x_bytes = 0, slot_bytes = 0, part_bytes = 0, tau_bytes = 0, ws_bytes = 0;
     unsigned char *ws = nullptr;
-    double *Wslot[MAX_RING] = {nullptr, nullptr, nullptr, nullptr};
+    double *X = nullptr;                   // SA: step-0 output tile [T*T][vv], folded into a ring slot
+    double *slot[MAX_RING] = {nullptr, nullptr, nullptr, nullptr};  // W tile, or W+ [T*T][ldp] followed by W- [T*T][ldm]
     double *part = nullptr;
-    int *flags = nullptr;  // device word for ppl_check_inputs
+    double *taup = nullptr, *taum = nullptr;
+    double *tperm = nullptr;               // un-packed modes with PPL_LAYOUT_IAJB input: t2 permuted (lazy)
+    int *flags = nullptr;                  // device word for ppl_check_inputs
     std::vector<Tile> tiles;
     cudaStream_t gen = nullptr, host_stream = nullptr;
-    cudaEvent_t ev_in = nullptr, ev_ready[MAX_RING] = {}, ev_free[MAX_RING] = {}, ev_gen_done = nullptr;
-    // host-path staging buffers (ppl_apply_host)
-    double *dL = nullptr, *dT = nullptr, *dR = nullptr;
+    cudaEvent_t ev_in = nullptr, ev_ready[MAX_RING] = {}, ev_free[MAX_RING] = {};
+    double *dL = nullptr, *dT = nullptr, *dR = nullptr;  // ppl_apply_host staging
     double f_step0 = 0, f_step1 = 0;
-    int ni1 = 8, bm1 = 128;          // step-1 CTA tile rows = 16*ni1 on the TMA path (128 on the cp.async path)
-    int use_tma = 0;                 // 1: persistent TMA/mbarrier kernels (nvirt even); 0: cp.async kernels
-    CUtensorMap mapW[MAX_RING];      // W slots as {inner nvirt^2, outer T*T}, built at plan time
+    CUtensorMap mapW[MAX_RING], mapWp[MAX_RING], mapWm[MAX_RING], mapTp, mapTm;  // plan-owned operands
 };
 
 namespace {
@@ -73,15 +89,11 @@ namespace {
 // ------------------------------------------------------------------------------------------
 // Planner: the analogue of the paper's memory functions (Table 1) -- but what
 // is being sized is the W-tile ring in HBM, not host->device batches.  For a candidate tile edge
-// T it estimates the time of one apply from CTA-wave counts of both GEMMs (tile 128x128x16 on
-// `sms` SMs), the best split-K per tile shape, and the t2/W streaming traffic.
+// T it estimates the time of one apply from CTA-wave counts of both GEMMs (CTA tile 128x128x16 on
+// `sms` SMs), the best split-K per tile shape, and the streaming traffic.
 // ------------------------------------------------------------------------------------------
-struct SplitChoice {
-    int splitk, k_per_split;
-    double seconds;
-};
 
-// CTA tile rows of step 1: 16*NI with NI in 5..10 chosen to pad nocc^2 the least (ties: larger tile)
+// CTA tile rows of step 1: 16*NI with NI in 5..10 chosen to pad M the least (ties: larger tile)
 int choose_ni(int M) {
     int best = 8;
     long best_pad = -1;
@@ -95,19 +107,22 @@ int choose_ni(int M) {
     return best;
 }
 
-SplitChoice choose_split(int M, int N, int K, int sms, int bm) {
+SplitChoice choose_split(int M, int N, int64_t K, int sms, int bm, size_t part_cap = ~(size_t)0) {
+    SplitChoice best;
+    if (M <= 0 || N <= 0 || K <= 0) return best;
     const int tiles = ((M + bm - 1) / bm) * ((N + ppl::BN - 1) / ppl::BN);
-    const int nkt = (K + ppl::BK - 1) / ppl::BK;
+    const int nkt = (int)((K + ppl::BK - 1) / ppl::BK);
     const double tau = 2.0 * bm * ppl::BN * ppl::BK / (PEAK_FLOPS / sms);  // one k-tile on one SM
-    SplitChoice best{1, nkt * ppl::BK, 1e300};
+    best = SplitChoice{1, nkt * ppl::BK, 1e300};
     const int smax = std::max(1, std::min(nkt / 8 + 1, 64));
     for (int s = 1; s <= smax; ++s) {
         const int kt_per = (nkt + s - 1) / s;
         const int s_eff = (nkt + kt_per - 1) / kt_per;  // no empty splits
         if (s_eff != s) continue;
+        if ((size_t)s * M * N * 8 > part_cap && s > 1) continue;
         const double waves = std::ceil((double)tiles * s / sms);
-        const double t = waves * (kt_per + 6) * tau            // +6: pipeline fill / epilogue
-                         + (double)(s + 2) * M * N * 8.0 / HBM_BPS;  // partials written + read by the reduce
+        const double t = waves * (kt_per + 6) * tau                      // +6: pipeline fill / epilogue
+                         + (double)(s + 2) * M * N * 8.0 / HBM_BPS;      // partials written + read by the reduce
         if (t < best.seconds) best = SplitChoice{s, kt_per * ppl::BK, t};
     }
     return best;
@@ -120,30 +135,30 @@ double step0_seconds(int ta, int tb, int v, int x, int sms) {
     return std::ceil((double)tiles / sms) * (nkt + 6) * tau;
 }
 
-struct PlanEval {
-    double seconds = 1e300;
-    size_t slot_bytes = 0, part_bytes = 0;
+struct Geometry {  // what depends on (o, v) only
+    int64_t vv;
+    int M, Mp, Mm, Kp, Km;
+    int64_t ldp, ldm;
+    int bm_full, bm_p, bm_m;
 };
 
-PlanEval evaluate(int o, int v, int x, int T, int sym, int sms, int bm1) {
+struct PlanEval {
+    double seconds = 1e300;
+    size_t x_bytes = 0, slot_bytes = 0, part_bytes = 0;
+};
+
+// estimated seconds of one apply with tile edge T in PPL_SYM_PAIR_SA (sa = true) or PPL_SYM_PAIR
+PlanEval evaluate(const Geometry &g, int o, int v, int x, int T, bool sa, int sms) {
     PlanEval ev;
     const int nblk = (v + T - 1) / T;
-    const int64_t vv = (int64_t)v * v;
-    const int M = o * o;
-    const double t2_bytes = (double)M * vv * 8.0;
+    const int r = v - (nblk - 1) * T;  // ragged edge
     double total = 0;
     size_t part_max = 0;
-    // distinct tile shapes: (T,T), (T,r), (r,T), (r,r) with r = ragged edge
-    const int r = v - (nblk - 1) * T;
-    auto count = [&](bool a_edge, bool b_edge) -> int64_t {
-        // number of executed tiles with the given edge flags
-        const int na = a_edge ? 1 : nblk - 1, nb = b_edge ? 1 : nblk - 1;
-        if (!sym) return (int64_t)na * nb;
-        // tiles with ablock <= bblock
+    auto count = [&](bool a_edge, bool b_edge) -> int64_t {  // executed tiles (a-block <= b-block) per shape
         if (a_edge && b_edge) return 1;
-        if (a_edge && !b_edge) return 0;                  // a = last block, b < last: a > b
-        if (!a_edge && b_edge) return nblk - 1;           // every a-block below the last pairs with the last
-        return (int64_t)(nblk - 1) * nblk / 2;            // interior a<=b
+        if (a_edge && !b_edge) return 0;
+        if (!a_edge && b_edge) return nblk - 1;
+        return (int64_t)(nblk - 1) * nblk / 2;
     };
     for (int ae = 0; ae < 2; ++ae)
         for (int be = 0; be < 2; ++be) {
@@ -151,38 +166,57 @@ PlanEval evaluate(int o, int v, int x, int T, int sym, int sms, int bm1) {
             if (cnt == 0) continue;
             const int ta = ae ? r : T, tb = be ? r : T;
             const int N = ta * tb;
-            const SplitChoice sc = choose_split(M, N, (int)std::min<int64_t>(vv, INT32_MAX), sms, bm1);
-            const double compute = step0_seconds(ta, tb, v, x, sms) + sc.seconds;
-            const double dram = (t2_bytes + 2.0 * N * vv * 8.0) / HBM_BPS;
-            total += cnt * (std::max(compute, dram) + 3 * LAUNCH_S);
-            part_max = std::max(part_max, (size_t)sc.splitk * M * N * 8);
+            const SplitChoice full = choose_split(g.M, N, g.vv, sms, g.bm_full);
+            size_t part = (size_t)full.splitk * g.M * N * 8;
+            double compute, dram;
+            if (sa) {
+                const SplitChoice sp = choose_split(g.Mp, N, g.Kp, sms, g.bm_p), sm = choose_split(g.Mm, N, g.Km, sms, g.bm_m);
+                const double fold = 2.0 * N * g.vv * 8.0 / HBM_BPS + LAUNCH_S;
+                compute = step0_seconds(ta, tb, v, x, sms) + fold + sp.seconds + sm.seconds;
+                dram = (((double)g.Mp * g.ldp + (double)g.Mm * g.ldm) * 8.0 + 4.0 * N * g.vv * 8.0) / HBM_BPS;
+                part = std::max(part, ((size_t)sp.splitk * g.Mp + (size_t)sm.splitk * g.Mm) * N * 8);
+                total += cnt * (std::max(compute, dram) + 5 * LAUNCH_S);
+            } else {
+                compute = step0_seconds(ta, tb, v, x, sms) + full.seconds;
+                dram = ((double)g.M * g.vv * 8.0 + 2.0 * N * g.vv * 8.0) / HBM_BPS;
+                total += cnt * (std::max(compute, dram) + 3 * LAUNCH_S);
+            }
+            part_max = std::max(part_max, part);
         }
     ev.seconds = total;
-    ev.slot_bytes = (size_t)T * T * vv * 8;
-    ev.part_bytes = part_max;
+    ev.x_bytes = sa ? align256((size_t)T * T * g.vv * 8) : 0;
+    ev.slot_bytes = align256(sa ? (size_t)T * T * (g.ldp + g.ldm) * 8 : (size_t)T * T * g.vv * 8);
+    ev.part_bytes = align256(part_max);
     return ev;
 }
 
 int build_tiles(ppl_plan_s *p) {
     p->tiles.clear();
     p->f_step0 = p->f_step1 = 0;
-    const int T = p->T, v = p->v;
-    const int64_t vv = (int64_t)v * v;
+    const int T = p->T, v = p->v, M = p->o * p->o;
+    const bool pair = p->sym != PPL_SYM_NONE, sa = p->sym == PPL_SYM_PAIR_SA;
     for (int ab = 0; ab < p->nblk; ++ab)
-        for (int bb = (p->sym == PPL_SYM_PAIR ? ab : 0); bb < p->nblk; ++bb) {
+        for (int bb = (pair ? ab : 0); bb < p->nblk; ++bb) {
             Tile t;
             t.a0 = ab * T;
             t.ta = std::min(T, v - t.a0);
             t.b0 = bb * T;
             t.tb = std::min(T, v - t.b0);
-            t.mirror = (p->sym == PPL_SYM_PAIR && ab != bb) ? 1 : 0;
-            const SplitChoice sc = choose_split(p->o * p->o, t.ta * t.tb, (int)vv, p->num_sms, p->bm1);
-            t.splitk = sc.splitk;
-            t.k_per_split = sc.k_per_split;
-            if ((size_t)t.splitk * p->o * p->o * t.ta * t.tb * 8 > p->part_bytes) return PPL_ERR_WORKSPACE_TOO_SMALL;
+            t.mirror = (pair && ab != bb) ? 1 : 0;
+            const int N = t.ta * t.tb;
+            if (sa) {
+                t.sp = choose_split(p->Mp, N, p->Kp, p->num_sms, p->bm_p);
+                t.sm = choose_split(p->Mm, N, p->Km, p->num_sms, p->bm_m);
+                if (((size_t)t.sp.splitk * p->Mp + (size_t)t.sm.splitk * p->Mm) * N * 8 > p->part_bytes)
+                    return PPL_ERR_WORKSPACE_TOO_SMALL;
+                p->f_step1 += 2.0 * N * ((double)p->Mp * p->Kp + (double)p->Mm * p->Km);
+            } else {
+                t.full = choose_split(M, N, p->vv, p->num_sms, p->bm_full, p->part_bytes);
+                if ((size_t)t.full.splitk * M * N * 8 > p->part_bytes) return PPL_ERR_WORKSPACE_TOO_SMALL;
+                p->f_step1 += 2.0 * M * (double)N * (double)p->vv;
+            }
             p->tiles.push_back(t);
-            p->f_step0 += 2.0 * p->x * (double)t.ta * t.tb * (double)vv;
-            p->f_step1 += 2.0 * p->o * p->o * (double)t.ta * t.tb * (double)vv;
+            p->f_step0 += 2.0 * p->x * (double)N * (double)p->vv;
         }
     return PPL_OK;
 }
@@ -198,13 +232,13 @@ void free_plan(ppl_plan_s *p) {
         cudaStreamDestroy(p->host_stream);
     }
     if (p->ev_in) cudaEventDestroy(p->ev_in);
-    if (p->ev_gen_done) cudaEventDestroy(p->ev_gen_done);
     for (int i = 0; i < MAX_RING; ++i) {
         if (p->ev_ready[i]) cudaEventDestroy(p->ev_ready[i]);
         if (p->ev_free[i]) cudaEventDestroy(p->ev_free[i]);
     }
     if (p->ws) cudaFree(p->ws);
     if (p->flags) cudaFree(p->flags);
+    if (p->tperm) cudaFree(p->tperm);
     if (p->dL) cudaFree(p->dL);
     if (p->dT) cudaFree(p->dT);
     if (p->dR) cudaFree(p->dR);
@@ -227,68 +261,6 @@ int set_kernel_attrs() {
     return PPL_OK;
 }
 
-int launch_step0(const ppl_plan_s *p, const Tile &t, const double *L, double *W, bool vec16, cudaStream_t s) {
-    ppl::Step0Args a;
-    a.A = L + (int64_t)t.a0 * p->v;
-    a.B = L + (int64_t)t.b0 * p->v;
-    a.ld = (int64_t)p->v * p->v;
-    a.M = t.ta * p->v;
-    a.N = t.tb * p->v;
-    a.K = p->x;
-    a.v = p->v;
-    a.tb = t.tb;
-    a.W = W;
-    a.ldw = p->ldw;
-    const int grid = ((a.M + ppl::BM - 1) / ppl::BM) * ((a.N + ppl::BN - 1) / ppl::BN);
-    if (vec16)
-        ppl::k_step0<2><<<grid, ppl::NTHREADS, ppl::SMEM_MN, s>>>(a);
-    else
-        ppl::k_step0<1><<<grid, ppl::NTHREADS, ppl::SMEM_MN, s>>>(a);
-    PPL_CUDA(cudaGetLastError());
-    return PPL_OK;
-}
-
-int launch_step1(const ppl_plan_s *p, const Tile &t, const double *t2, const double *W, bool vec16, cudaStream_t s) {
-    ppl::Step1Args a;
-    a.A = t2;
-    a.B = W;
-    a.lda = (int64_t)p->v * p->v;
-    a.ldb = p->ldw;
-    a.M = p->o * p->o;
-    a.N = t.ta * t.tb;
-    a.K = p->v * p->v;
-    a.k_per_split = t.k_per_split;
-    a.part = p->part;
-    dim3 grid(((a.M + ppl::BM - 1) / ppl::BM) * ((a.N + ppl::BN - 1) / ppl::BN), t.splitk);
-    if (vec16)
-        ppl::k_step1<2><<<grid, ppl::NTHREADS, ppl::SMEM_K, s>>>(a);
-    else
-        ppl::k_step1<1><<<grid, ppl::NTHREADS, ppl::SMEM_K, s>>>(a);
-    PPL_CUDA(cudaGetLastError());
-    return PPL_OK;
-}
-
-int launch_reduce(const ppl_plan_s *p, const Tile &t, double *R, cudaStream_t s) {
-    ppl::ReduceArgs a;
-    a.part = p->part;
-    a.splitk = t.splitk;
-    a.M = p->o * p->o;
-    a.N = t.ta * t.tb;
-    a.o = p->o;
-    a.v = p->v;
-    a.tb = t.tb;
-    a.a0 = t.a0;
-    a.b0 = t.b0;
-    a.mirror = t.mirror;
-    a.R = R;
-    const int64_t MN = (int64_t)a.M * a.N;
-    const int grid = (int)std::min<int64_t>((MN + 255) / 256, (int64_t)p->num_sms * 8);
-    ppl::k_reduce<<<grid, 256, 0, s>>>(a);
-    PPL_CUDA(cudaGetLastError());
-    return PPL_OK;
-}
-
-
 // ---- TMA tensor maps (driver entry point fetched through the runtime: no libcuda link) ----
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                                   const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -306,11 +278,12 @@ EncodeTiledFn get_encode() {
     }
     return fn;
 }
-// 2-D FP64 tensor {inner (contiguous), outer} with row stride `row_bytes`, box {box_inner, box_outer}, 128B swizzle
+// 2-D FP64 tensor {inner (contiguous), outer} with row stride `row_bytes`, box {box_inner, box_outer}, 128B swizzle;
+// out-of-bounds elements of a box are filled with zeros (tile edges, k tails)
 int make_map_2d(CUtensorMap *map, const void *base, uint64_t inner, uint64_t outer, uint64_t row_bytes, uint32_t box_inner,
                 uint32_t box_outer) {
     EncodeTiledFn enc = get_encode();
-    if (!enc) return PPL_ERR_CUDA;
+    if (!enc || inner == 0 || outer == 0) return PPL_ERR_CUDA;
     const cuuint64_t gdim[2] = {inner, outer};
     const cuuint64_t gstride[1] = {row_bytes};
     const cuuint32_t box[2] = {box_inner, box_outer};
@@ -321,54 +294,205 @@ int make_map_2d(CUtensorMap *map, const void *base, uint64_t inner, uint64_t out
     return r == CUDA_SUCCESS ? PPL_OK : PPL_ERR_CUDA;
 }
 
-int launch_step0_tma(const ppl_plan_s *p, const Tile &t, const CUtensorMap &mapL, double *W, cudaStream_t s) {
-    ppl::Step0TmaArgs a;
-    a.a0v = t.a0 * p->v;
-    a.b0v = t.b0 * p->v;
-    a.M = t.ta * p->v;
-    a.N = t.tb * p->v;
-    a.K = p->x;
-    a.v = p->v;
-    a.tb = t.tb;
-    a.W = W;
-    a.ldw = p->ldw;
-    const int items = ((a.M + ppl::BM - 1) / ppl::BM) * ((a.N + ppl::BN - 1) / ppl::BN);
-    ppl::k_step0_tma<<<std::min(items, p->num_sms), ppl::TMA_THREADS, ppl::SMEM_TMA, s>>>(mapL, a);
-    PPL_CUDA(cudaGetLastError());
-    return PPL_OK;
-}
-
-int launch_step1_tma(const ppl_plan_s *p, const Tile &t, const CUtensorMap &mapT, const CUtensorMap &mapW, cudaStream_t s) {
-    ppl::Step1TmaArgs a;
-    a.M = p->o * p->o;
-    a.N = t.ta * t.tb;
-    a.K = p->v * p->v;
-    a.k_per_split = t.k_per_split;
-    a.splitk = t.splitk;
-    a.part = p->part;
-    const int items = ((a.M + p->bm1 - 1) / p->bm1) * ((a.N + ppl::BN - 1) / ppl::BN) * t.splitk;
-    const int grid = std::min(items, p->num_sms);
-    switch (p->ni1) {
-#define PPL_LAUNCH_NI(NI)                                                                                        \
-    case NI:                                                                                                     \
-        ppl::k_step1_tma<NI><<<grid, ppl::TMA_THREADS, ppl::Step1Cfg<NI>::SMEM, s>>>(mapT, mapW, a);           \
-        break;
-        PPL_LAUNCH_NI(5) PPL_LAUNCH_NI(6) PPL_LAUNCH_NI(7) PPL_LAUNCH_NI(8) PPL_LAUNCH_NI(9) PPL_LAUNCH_NI(10)
-#undef PPL_LAUNCH_NI
-        default: return fail(PPL_ERR_INVALID_ARG);
+// ---- launches ----
+int launch_step0(const ppl_plan_s *p, const Tile &t, const double *L, const CUtensorMap *mapL, double *W, bool vec16,
+                 cudaStream_t s) {
+    const int M = t.ta * p->v, N = t.tb * p->v;
+    const int items = ((M + ppl::BM - 1) / ppl::BM) * ((N + ppl::BN - 1) / ppl::BN);
+    if (mapL) {
+        ppl::Step0TmaArgs a;
+        a.a0v = t.a0 * p->v;
+        a.b0v = t.b0 * p->v;
+        a.M = M;
+        a.N = N;
+        a.K = p->x;
+        a.v = p->v;
+        a.tb = t.tb;
+        a.W = W;
+        a.ldw = p->vv;
+        ppl::k_step0_tma<<<std::min(items, p->num_sms), ppl::TMA_THREADS, ppl::SMEM_TMA, s>>>(*mapL, a);
+    } else {
+        ppl::Step0Args a;
+        a.A = L + (int64_t)t.a0 * p->v;
+        a.B = L + (int64_t)t.b0 * p->v;
+        a.ld = p->vv;
+        a.M = M;
+        a.N = N;
+        a.K = p->x;
+        a.v = p->v;
+        a.tb = t.tb;
+        a.W = W;
+        a.ldw = p->vv;
+        if (vec16)
+            ppl::k_step0<2><<<items, ppl::NTHREADS, ppl::SMEM_MN, s>>>(a);
+        else
+            ppl::k_step0<1><<<items, ppl::NTHREADS, ppl::SMEM_MN, s>>>(a);
     }
     PPL_CUDA(cudaGetLastError());
     return PPL_OK;
 }
 
-struct ApplyMaps {
-    CUtensorMap L, T;
-};
-int make_apply_maps(const ppl_plan_s *p, const double *L, const double *t2, ApplyMaps *m) {
-    const uint64_t vv = (uint64_t)p->v * p->v;
-    int rc = make_map_2d(&m->L, L, vv, (uint64_t)p->x, vv * 8, 16, ppl::BK);
-    if (rc == PPL_OK) rc = make_map_2d(&m->T, t2, vv, (uint64_t)p->o * p->o, vv * 8, ppl::BK, (uint32_t)p->bm1);
-    return rc;
+// One step-1 GEMM: part[z][M][N] = sum_{k in split z} A[m][k] B[n][k]; A is lda-strided, B ldb-strided.
+// With maps: the persistent TMA kernel with CTA tile (16*ni) x 128; without: the cp.async kernel.
+int launch_step1(const ppl_plan_s *p, const CUtensorMap *mapA, const CUtensorMap *mapB, int ni, const double *A, int64_t lda,
+                 const double *B, int64_t ldb, int M, int N, int64_t K, const SplitChoice &sc, double *part, bool vec16,
+                 cudaStream_t s) {
+    if (M <= 0 || N <= 0 || K <= 0) return PPL_OK;
+    if (mapA && mapB) {
+        ppl::Step1TmaArgs a;
+        a.M = M;
+        a.N = N;
+        a.K = (int)K;
+        a.k_per_split = sc.k_per_split;
+        a.splitk = sc.splitk;
+        a.part = part;
+        const int bm = 16 * ni;
+        const int items = ((M + bm - 1) / bm) * ((N + ppl::BN - 1) / ppl::BN) * sc.splitk;
+        const int grid = std::min(items, p->num_sms);
+        switch (ni) {
+#define PPL_LAUNCH_NI(NI)                                                                                   \
+    case NI:                                                                                                \
+        ppl::k_step1_tma<NI><<<grid, ppl::TMA_THREADS, ppl::Step1Cfg<NI>::SMEM, s>>>(*mapA, *mapB, a);    \
+        break;
+            PPL_LAUNCH_NI(5) PPL_LAUNCH_NI(6) PPL_LAUNCH_NI(7) PPL_LAUNCH_NI(8) PPL_LAUNCH_NI(9) PPL_LAUNCH_NI(10)
+#undef PPL_LAUNCH_NI
+            default: return fail(PPL_ERR_INVALID_ARG);
+        }
+    } else {
+        ppl::Step1Args a;
+        a.A = A;
+        a.B = B;
+        a.lda = lda;
+        a.ldb = ldb;
+        a.M = M;
+        a.N = N;
+        a.K = (int)K;
+        a.k_per_split = sc.k_per_split;
+        a.part = part;
+        dim3 grid(((M + ppl::BM - 1) / ppl::BM) * ((N + ppl::BN - 1) / ppl::BN), sc.splitk);
+        if (vec16)
+            ppl::k_step1<2><<<grid, ppl::NTHREADS, ppl::SMEM_K, s>>>(a);
+        else
+            ppl::k_step1<1><<<grid, ppl::NTHREADS, ppl::SMEM_K, s>>>(a);
+    }
+    PPL_CUDA(cudaGetLastError());
+    return PPL_OK;
+}
+
+ppl::RStrides r_strides(int o, int v, int layout) {
+    ppl::RStrides s;
+    if (layout == PPL_LAYOUT_IAJB) {  // [i][a][j][b]
+        s.i = (int64_t)v * o * v;
+        s.a = (int64_t)o * v;
+        s.j = v;
+        s.b = 1;
+    } else {  // [i][j][a][b]
+        s.i = (int64_t)o * v * v;
+        s.j = (int64_t)v * v;
+        s.a = v;
+        s.b = 1;
+    }
+    return s;
+}
+
+int launch_reduce(const ppl_plan_s *p, const Tile &t, int splitk, int n_rows, int n_off, int tb, double *R,
+                  const ppl_opts_t &o, cudaStream_t s) {
+    ppl::ReduceArgs a;
+    a.part = p->part;
+    a.splitk = splitk;
+    a.M = p->o * p->o;
+    a.N = n_rows;
+    a.o = p->o;
+    a.v = p->v;
+    a.tb = tb;
+    a.a0 = t.a0;
+    a.b0 = t.b0;
+    a.n_off = n_off;
+    a.mirror = t.mirror;
+    a.alpha = o.alpha;
+    a.beta = o.beta;
+    a.rs = r_strides(p->o, p->v, o.r_layout);
+    a.R = R;
+    const int64_t MN = (int64_t)a.M * a.N;
+    const int grid = (int)std::min<int64_t>((MN + 255) / 256, (int64_t)p->num_sms * 8);
+    ppl::k_reduce<<<grid, 256, 0, s>>>(a);
+    PPL_CUDA(cudaGetLastError());
+    return PPL_OK;
+}
+
+int launch_reduce_sa(const ppl_plan_s *p, const Tile &t, const double *partp, const double *partm, double *R,
+                     const ppl_opts_t &o, cudaStream_t s) {
+    ppl::ReduceSaArgs a;
+    a.partp = partp;
+    a.partm = partm;
+    a.sp = t.sp.splitk;
+    a.sm = (p->Mm > 0 && p->Km > 0) ? t.sm.splitk : 0;
+    a.Mp = p->Mp;
+    a.Mm = p->Mm;
+    a.N = t.ta * t.tb;
+    a.o = p->o;
+    a.v = p->v;
+    a.tb = t.tb;
+    a.a0 = t.a0;
+    a.b0 = t.b0;
+    a.mirror = t.mirror;
+    a.alpha = o.alpha;
+    a.beta = o.beta;
+    a.rs = r_strides(p->o, p->v, o.r_layout);
+    a.R = R;
+    const int64_t MN = (int64_t)a.Mp * a.N;
+    const int grid = (int)std::min<int64_t>((MN + 255) / 256, (int64_t)p->num_sms * 8);
+    ppl::k_reduce_sa<<<grid, 256, 0, s>>>(a);
+    PPL_CUDA(cudaGetLastError());
+    return PPL_OK;
+}
+
+// W tile X [rows][vv] -> W+ [rows][ldp], W- [rows][ldm]
+int launch_fold(const ppl_plan_s *p, const double *X, int rows, double *Wp, double *Wm, cudaStream_t s) {
+    ppl::FoldArgs a;
+    a.src = X;
+    a.sc = p->v;
+    a.s_row = p->vv;
+    a.s_i = a.s_j = 0;
+    a.mode = 0;
+    a.rows = rows;
+    a.o = p->o;
+    a.v = p->v;
+    a.scale = 1.0;
+    a.dp = Wp;
+    a.dm = Wm;
+    a.ldp = p->ldp;
+    a.ldm = p->ldm;
+    const int nbv = (p->v + ppl::FT - 1) / ppl::FT;
+    dim3 grid(nbv * (nbv + 1) / 2, std::min(rows, 8192));
+    ppl::k_symfold<<<grid, 256, 0, s>>>(a);
+    PPL_CUDA(cudaGetLastError());
+    return PPL_OK;
+}
+
+// t2 (either storage order) -> tau+ [Mp][ldp], tau- [Mm][ldm]
+int launch_pack(const ppl_plan_s *p, const double *t2, int layout, cudaStream_t s) {
+    ppl::FoldArgs a;
+    a.src = t2;
+    const ppl::RStrides ts = r_strides(p->o, p->v, layout);  // t2[i,j,c,d] has the strides of R[i,j,a,b]
+    a.sc = ts.a;
+    a.s_row = 0;
+    a.s_i = ts.i;
+    a.s_j = ts.j;
+    a.mode = 1;
+    a.rows = p->o * p->o;
+    a.o = p->o;
+    a.v = p->v;
+    a.scale = 0.5;
+    a.dp = p->taup;
+    a.dm = p->taum;
+    a.ldp = p->ldp;
+    a.ldm = p->ldm;
+    const int nbv = (p->v + ppl::FT - 1) / ppl::FT;
+    dim3 grid(nbv * (nbv + 1) / 2, std::min(a.rows, 8192));
+    ppl::k_symfold<<<grid, 256, 0, s>>>(a);
+    PPL_CUDA(cudaGetLastError());
+    return PPL_OK;
 }
 
 int check_ptrs(const ppl_plan_s *p, const double *L, const double *t2, const double *R, bool *vec16) {
@@ -376,6 +500,137 @@ int check_ptrs(const ppl_plan_s *p, const double *L, const double *t2, const dou
     const uintptr_t all = (uintptr_t)L | (uintptr_t)t2 | (uintptr_t)R;
     if (all & 7) return PPL_ERR_INVALID_ARG;
     *vec16 = p->vec16 && ((all & 15) == 0);
+    return PPL_OK;
+}
+
+int check_opts(const ppl_opts_t *in, ppl_opts_t *out) {
+    out->t2_layout = PPL_LAYOUT_IJAB;
+    out->r_layout = PPL_LAYOUT_IJAB;
+    out->alpha = 1.0;
+    out->beta = 1.0;
+    if (!in) return PPL_OK;
+    if ((in->t2_layout != PPL_LAYOUT_IJAB && in->t2_layout != PPL_LAYOUT_IAJB) ||
+        (in->r_layout != PPL_LAYOUT_IJAB && in->r_layout != PPL_LAYOUT_IAJB))
+        return PPL_ERR_INVALID_ARG;
+    *out = *in;
+    return PPL_OK;
+}
+
+// un-packed modes: t2 as the [(i,j)][(c,d)] matrix step 1 reads; a 'iajb'-stored t2 is permuted into tperm
+int t2_matrix(ppl_plan_s *p, const double *t2, int layout, cudaStream_t s, const double **out) {
+    *out = t2;
+    if (layout == PPL_LAYOUT_IJAB) return PPL_OK;
+    const size_t bytes = (size_t)p->o * p->o * p->vv * 8;
+    if (!p->tperm && cudaMalloc(&p->tperm, bytes) != cudaSuccess) {
+        (void)cudaGetLastError();
+        p->tperm = nullptr;
+        return fail(PPL_ERR_ALLOC);
+    }
+    ppl::k_permute_t2<<<p->num_sms * 8, 256, 0, s>>>(t2, p->tperm, p->o, p->v);
+    PPL_CUDA(cudaGetLastError());
+    *out = p->tperm;
+    return PPL_OK;
+}
+
+// per-launch event log of ppl_apply_profiled
+enum Kind { K_PACK = 0, K_STEP0, K_FOLD, K_STEP1, K_REDUCE, K_KINDS };
+struct Prof {
+    std::vector<cudaEvent_t> ev;
+    std::vector<int> kind;
+    int launches[K_KINDS] = {0, 0, 0, 0, 0};
+    int mark(int k, int n_launches, cudaStream_t s) {
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) return PPL_ERR_CUDA;
+        ev.push_back(e);
+        kind.push_back(k);
+        if (k >= 0) launches[k] += n_launches;
+        return cudaEventRecord(e, s) == cudaSuccess ? PPL_OK : PPL_ERR_CUDA;
+    }
+};
+
+// The whole path.  prof == nullptr: two streams, W-tile ring (the product path).  prof != nullptr: one
+// stream, one slot, an event after every stage (measurement only).
+int run_apply(ppl_plan_s *p, const double *L, const double *t2, double *R, const ppl_opts_t *opts_in, cudaStream_t stream,
+              Prof *prof) {
+    bool vec16 = false;
+    int rc = check_ptrs(p, L, t2, R, &vec16);
+    ppl_opts_t opts;
+    if (rc == PPL_OK) rc = check_opts(opts_in, &opts);
+    if (rc != PPL_OK) return fail(rc);
+    const int ntiles = (int)p->tiles.size();
+    const bool sa = p->sym == PPL_SYM_PAIR_SA;
+    const bool tma0 = p->use_tma && vec16;             // step 0 reads the caller's L: needs 16-byte rows
+    const bool tma1 = sa ? p->use_tma != 0 : tma0;     // SA step 1 reads plan-owned, padded operands
+    const bool two_streams = !prof && p->ring >= 2 && ntiles >= 2;
+    cudaStream_t gen = two_streams ? p->gen : stream;
+#define PPL_MARK(k, n)                                                         \
+    do {                                                                       \
+        if (prof && prof->mark(k, n, stream) != PPL_OK) return fail(PPL_ERR_CUDA); \
+    } while (0)
+
+    if (two_streams) {  // fork: the producer stream starts after prior work on `stream`
+        PPL_CUDA(cudaEventRecord(p->ev_in, stream));
+        PPL_CUDA(cudaStreamWaitEvent(gen, p->ev_in, 0));
+    }
+    PPL_MARK(-1, 0);
+    const double *t2m = t2;
+    if (sa) {
+        if ((rc = launch_pack(p, t2, opts.t2_layout, stream)) != PPL_OK) return rc;
+        PPL_MARK(K_PACK, 1);
+    } else if (opts.t2_layout != PPL_LAYOUT_IJAB) {
+        if ((rc = t2_matrix(p, t2, opts.t2_layout, stream, &t2m)) != PPL_OK) return rc;
+        PPL_MARK(K_PACK, 1);
+    }
+    CUtensorMap mapL, mapT;
+    if (tma0 && make_map_2d(&mapL, L, (uint64_t)p->vv, (uint64_t)p->x, (uint64_t)p->vv * 8, 16, ppl::BK) != PPL_OK)
+        return fail(PPL_ERR_CUDA);
+    if (!sa && tma1 &&
+        make_map_2d(&mapT, t2m, (uint64_t)p->vv, (uint64_t)p->o * p->o, (uint64_t)p->vv * 8, ppl::BK, (uint32_t)p->bm_full) != PPL_OK)
+        return fail(PPL_ERR_CUDA);
+    const bool minus = sa && p->Mm > 0 && p->Km > 0;
+
+    for (int k = 0; k < ntiles; ++k) {
+        const Tile &t = p->tiles[k];
+        const int slot = prof ? 0 : k % p->ring;
+        const int N = t.ta * t.tb;
+        double *Wp = p->slot[slot], *Wm = p->slot[slot] + (size_t)p->T * p->T * p->ldp;
+        if (two_streams && k >= p->ring) PPL_CUDA(cudaStreamWaitEvent(gen, p->ev_free[slot], 0));
+        // ---- producer: step 0 (and the +- fold) ----
+        if ((rc = launch_step0(p, t, L, tma0 ? &mapL : nullptr, sa ? p->X : p->slot[slot], vec16, gen)) != PPL_OK) return rc;
+        PPL_MARK(K_STEP0, 1);
+        if (sa) {
+            if ((rc = launch_fold(p, p->X, N, Wp, Wm, gen)) != PPL_OK) return rc;
+            PPL_MARK(K_FOLD, 1);
+        }
+        if (two_streams) {
+            PPL_CUDA(cudaEventRecord(p->ev_ready[slot], gen));
+            PPL_CUDA(cudaStreamWaitEvent(stream, p->ev_ready[slot], 0));
+        }
+        // ---- consumer: step 1, reduce ----
+        if (sa) {
+            double *partp = p->part, *partm = p->part + (size_t)t.sp.splitk * p->Mp * N;
+            rc = launch_step1(p, tma1 ? &p->mapTp : nullptr, tma1 ? &p->mapWp[slot] : nullptr, p->ni_p, p->taup, p->ldp, Wp,
+                              p->ldp, p->Mp, N, p->Kp, t.sp, partp, true, stream);
+            if (rc == PPL_OK && minus)
+                rc = launch_step1(p, tma1 ? &p->mapTm : nullptr, tma1 ? &p->mapWm[slot] : nullptr, p->ni_m, p->taum, p->ldm,
+                                  Wm, p->ldm, p->Mm, N, p->Km, t.sm, partm, true, stream);
+            if (rc != PPL_OK) return rc;
+            PPL_MARK(K_STEP1, minus ? 2 : 1);
+            if (two_streams) PPL_CUDA(cudaEventRecord(p->ev_free[slot], stream));
+            if ((rc = launch_reduce_sa(p, t, partp, partm, R, opts, stream)) != PPL_OK) return rc;
+        } else {
+            rc = launch_step1(p, tma1 ? &mapT : nullptr, tma1 ? &p->mapW[slot] : nullptr, p->ni_full, t2m, p->vv, p->slot[slot],
+                              p->vv, p->o * p->o, N, p->vv, t.full, p->part, vec16, stream);
+            if (rc != PPL_OK) return rc;
+            PPL_MARK(K_STEP1, 1);
+            if (two_streams) PPL_CUDA(cudaEventRecord(p->ev_free[slot], stream));
+            if ((rc = launch_reduce(p, t, t.full.splitk, N, 0, t.tb, R, opts, stream)) != PPL_OK) return rc;
+        }
+        PPL_MARK(K_REDUCE, 1);
+    }
+#undef PPL_MARK
+    // join: every producer launch is followed by a consumer wait on `stream`, so `stream` already
+    // depends on all work of `gen`.
     return PPL_OK;
 }
 
@@ -426,8 +681,14 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
     p->x = nchol;
     p->num_sms = prop.multiProcessorCount;
     p->vec16 = (nvirt % 2 == 0) ? 1 : 0;
-    p->ldw = (int64_t)nvirt * nvirt;
+    p->vv = (int64_t)nvirt * nvirt;
     p->cap = workspace_bytes;
+    p->Mp = nocc * (nocc + 1) / 2;
+    p->Mm = nocc * (nocc - 1) / 2;
+    p->Kp = nvirt * (nvirt + 1) / 2;
+    p->Km = nvirt * (nvirt - 1) / 2;
+    p->ldp = ((int64_t)p->Kp + 15) / 16 * 16;  // rows of the packed operands are 128-byte aligned: TMA-legal for any nvirt
+    p->ldm = ((int64_t)std::max(p->Km, 1) + 15) / 16 * 16;
 
     size_t free_b = 0, total_b = 0;
     if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) {
@@ -440,42 +701,52 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
     const size_t cap = workspace_bytes ? std::min(workspace_bytes, auto_cap) : auto_cap;
 
     const char *envk = getenv("PPL_KERNELS");  // debug override: "cpasync" forces the non-TMA kernels
-    p->use_tma = p->vec16 && !(envk && strcmp(envk, "cpasync") == 0) && get_encode() != nullptr;
-    if (p->use_tma) {
-        const char *envni = getenv("PPL_NI");  // debug override of the step-1 tile height
-        p->ni1 = (envni && atoi(envni) >= 5 && atoi(envni) <= 10) ? atoi(envni) : choose_ni(nocc * nocc);
-        p->bm1 = 16 * p->ni1;
-    }
-    // choose the tile edge T (and ring depth) that minimises the estimated apply time under the cap
+    p->use_tma = !(envk && strcmp(envk, "cpasync") == 0) && get_encode() != nullptr;
+    const char *envni = getenv("PPL_NI");  // debug override of the step-1 tile height
+    const int ni_env = (envni && atoi(envni) >= 5 && atoi(envni) <= 10) ? atoi(envni) : 0;
+    p->ni_full = ni_env ? ni_env : choose_ni(nocc * nocc);
+    p->ni_p = ni_env ? ni_env : choose_ni(p->Mp);
+    p->ni_m = ni_env ? ni_env : choose_ni(std::max(p->Mm, 1));
+    const bool tma_full = p->use_tma && p->vec16;
+    p->bm_full = tma_full ? 16 * p->ni_full : ppl::BM;
+    p->bm_p = p->use_tma ? 16 * p->ni_p : ppl::BM;
+    p->bm_m = p->use_tma ? 16 * p->ni_m : ppl::BM;
+    Geometry g{p->vv, nocc * nocc, p->Mp, p->Mm, p->Kp, p->Km, p->ldp, p->ldm, p->bm_full, p->bm_p, p->bm_m};
+    p->tau_bytes = align256((size_t)p->Mp * p->ldp * 8) + align256((size_t)std::max(p->Mm, 1) * p->ldm * 8);
+
+    // choose the tile edge T (and ring depth) that minimises the estimated apply time under the cap:
+    // first with the packed operands of PPL_SYM_PAIR_SA, and if they do not fit, without them
     const char *envT = getenv("PPL_TILE");  // debug override
     double best_t = 1e300;
-    int best_T = 0, best_ring = 1;
+    int best_T = 0, best_ring = 1, best_sa = 0;
     PlanEval best_ev;
-    for (int T = nvirt; T >= 1; --T) {
-        if (envT && atoi(envT) > 0 && T != std::min(atoi(envT), nvirt)) continue;
-        // only edges that tile v evenly or nearly so (ragged edge at least T/2), to keep edge tiles efficient
-        const int nblk = (nvirt + T - 1) / T;
-        const int r = nvirt - (nblk - 1) * T;
-        if (!envT && nblk > 1 && 2 * r < T) continue;
-        const PlanEval ev = evaluate(nocc, nvirt, nchol, T, PPL_SYM_PAIR, p->num_sms, p->bm1);
-        // the same plan must also serve PPL_SYM_NONE (same shapes), so part/slot sizes are identical
-        int ring = 0;
-        for (int rg = std::min(3, MAX_RING); rg >= 1; --rg)
-            if (rg * ev.slot_bytes + ev.part_bytes + 256 <= cap) {
-                ring = rg;
-                break;
+    for (int sa = 1; sa >= 0 && best_T == 0; --sa)
+        for (int T = nvirt; T >= 1; --T) {
+            if (envT && atoi(envT) > 0 && T != std::min(atoi(envT), nvirt)) continue;
+            // only edges that tile v evenly or nearly so (ragged edge at least T/2), to keep edge tiles efficient
+            const int nblk = (nvirt + T - 1) / T;
+            const int r = nvirt - (nblk - 1) * T;
+            if (!envT && nblk > 1 && 2 * r < T) continue;
+            const PlanEval ev = evaluate(g, nocc, nvirt, nchol, T, sa != 0, p->num_sms);
+            const size_t fixed = ev.x_bytes + ev.part_bytes + (sa ? p->tau_bytes : 0) + 256;
+            int ring = 0;
+            for (int rg = std::min(3, MAX_RING); rg >= 1; --rg)
+                if (rg * ev.slot_bytes + fixed <= cap) {
+                    ring = rg;
+                    break;
+                }
+            if (ring == 0) continue;
+            const int ntiles = nblk * (nblk + 1) / 2;
+            ring = std::min(ring, std::max(1, ntiles));
+            const double t = ev.seconds * (ring >= 2 ? 1.0 : 1.03);
+            if (t < best_t) {
+                best_t = t;
+                best_T = T;
+                best_ring = ring;
+                best_ev = ev;
+                best_sa = sa;
             }
-        if (ring == 0) continue;
-        const int ntiles = nblk * (nblk + 1) / 2;
-        ring = std::min(ring, std::max(1, ntiles));
-        const double t = ev.seconds * (ring >= 2 ? 1.0 : 1.03);
-        if (t < best_t) {
-            best_t = t;
-            best_T = T;
-            best_ring = ring;
-            best_ev = ev;
         }
-    }
     if (best_T == 0) {
         free_plan(p);
         fail(PPL_ERR_WORKSPACE_TOO_SMALL);
@@ -484,22 +755,33 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
     p->T = best_T;
     p->nblk = (nvirt + best_T - 1) / best_T;
     p->ring = best_ring;
-    p->slot_bytes = (best_ev.slot_bytes + 255) & ~(size_t)255;
-    p->part_bytes = (best_ev.part_bytes + 255) & ~(size_t)255;
-    p->ws_bytes = p->ring * p->slot_bytes + p->part_bytes;
+    p->sa_ok = best_sa;
+    p->x_bytes = best_ev.x_bytes;
+    p->slot_bytes = best_ev.slot_bytes;
+    p->part_bytes = best_ev.part_bytes;
+    p->ws_bytes = p->x_bytes + p->ring * p->slot_bytes + p->part_bytes + (p->sa_ok ? p->tau_bytes : 0);
     if (cudaMalloc(&p->ws, p->ws_bytes) != cudaSuccess || cudaMalloc(&p->flags, sizeof(int)) != cudaSuccess) {
         (void)cudaGetLastError();
         free_plan(p);
         fail(PPL_ERR_ALLOC);
         return nullptr;
     }
-    for (int i = 0; i < p->ring; ++i) p->Wslot[i] = reinterpret_cast<double *>(p->ws + (size_t)i * p->slot_bytes);
-    p->part = reinterpret_cast<double *>(p->ws + (size_t)p->ring * p->slot_bytes);
+    {
+        unsigned char *q = p->ws;
+        p->X = reinterpret_cast<double *>(q);
+        q += p->x_bytes;
+        for (int i = 0; i < p->ring; ++i, q += p->slot_bytes) p->slot[i] = reinterpret_cast<double *>(q);
+        p->part = reinterpret_cast<double *>(q);
+        q += p->part_bytes;
+        if (p->sa_ok) {
+            p->taup = reinterpret_cast<double *>(q);
+            p->taum = reinterpret_cast<double *>(q + align256((size_t)p->Mp * p->ldp * 8));
+        }
+    }
 
     bool ok = cudaStreamCreateWithFlags(&p->gen, cudaStreamNonBlocking) == cudaSuccess;
     ok = ok && cudaStreamCreateWithFlags(&p->host_stream, cudaStreamNonBlocking) == cudaSuccess;
     ok = ok && cudaEventCreateWithFlags(&p->ev_in, cudaEventDisableTiming) == cudaSuccess;
-    ok = ok && cudaEventCreateWithFlags(&p->ev_gen_done, cudaEventDisableTiming) == cudaSuccess;
     for (int i = 0; i < MAX_RING && ok; ++i) {
         ok = ok && cudaEventCreateWithFlags(&p->ev_ready[i], cudaEventDisableTiming) == cudaSuccess;
         ok = ok && cudaEventCreateWithFlags(&p->ev_free[i], cudaEventDisableTiming) == cudaSuccess;
@@ -511,14 +793,31 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
         return nullptr;
     }
     if (p->use_tma) {
-        const uint64_t vv = (uint64_t)nvirt * nvirt;
-        for (int i = 0; i < p->ring; ++i)
-            if (make_map_2d(&p->mapW[i], p->Wslot[i], vv, (uint64_t)p->T * p->T, (uint64_t)p->ldw * 8, ppl::BK, ppl::BN) != PPL_OK) {
-                p->use_tma = 0;
-                break;
+        const uint64_t TT = (uint64_t)p->T * p->T;
+        bool m = true;
+        for (int i = 0; i < p->ring && m; ++i) {
+            if (p->vec16) m = m && make_map_2d(&p->mapW[i], p->slot[i], (uint64_t)p->vv, TT, (uint64_t)p->vv * 8, ppl::BK, ppl::BN) == PPL_OK;
+            if (p->sa_ok) {
+                m = m && make_map_2d(&p->mapWp[i], p->slot[i], (uint64_t)p->Kp, TT, (uint64_t)p->ldp * 8, ppl::BK, ppl::BN) == PPL_OK;
+                if (p->Km > 0)
+                    m = m && make_map_2d(&p->mapWm[i], p->slot[i] + TT * p->ldp, (uint64_t)p->Km, TT, (uint64_t)p->ldm * 8, ppl::BK,
+                                         ppl::BN) == PPL_OK;
             }
+        }
+        if (p->sa_ok && m) {
+            m = m && make_map_2d(&p->mapTp, p->taup, (uint64_t)p->Kp, (uint64_t)p->Mp, (uint64_t)p->ldp * 8, ppl::BK, (uint32_t)p->bm_p) == PPL_OK;
+            if (p->Km > 0 && p->Mm > 0)
+                m = m && make_map_2d(&p->mapTm, p->taum, (uint64_t)p->Km, (uint64_t)p->Mm, (uint64_t)p->ldm * 8, ppl::BK,
+                                     (uint32_t)p->bm_m) == PPL_OK;
+        }
+        if (!m) {
+            (void)cudaGetLastError();
+            free_plan(p);
+            fail(PPL_ERR_CUDA);
+            return nullptr;
+        }
     }
-    p->sym = PPL_SYM_PAIR;
+    p->sym = p->sa_ok ? PPL_SYM_PAIR_SA : PPL_SYM_PAIR;
     const int rc = build_tiles(p);
     if (rc != PPL_OK) {
         free_plan(p);
@@ -529,15 +828,23 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
 }
 
 int ppl_plan_set_symmetry(ppl_plan_t *p, int mode) {
-    if (!p || (mode != PPL_SYM_NONE && mode != PPL_SYM_PAIR)) return fail(PPL_ERR_INVALID_ARG);
+    if (!p || (mode != PPL_SYM_NONE && mode != PPL_SYM_PAIR && mode != PPL_SYM_PAIR_SA)) return fail(PPL_ERR_INVALID_ARG);
+    if (mode == PPL_SYM_PAIR_SA && !p->sa_ok) return fail(PPL_ERR_WORKSPACE_TOO_SMALL);
+    const int old = p->sym;
     p->sym = mode;
     const int rc = build_tiles(p);
-    return rc == PPL_OK ? PPL_OK : fail(rc);
+    if (rc != PPL_OK) {
+        p->sym = old;
+        build_tiles(p);
+        return fail(rc);
+    }
+    return PPL_OK;
 }
 
 int ppl_plan_info(const ppl_plan_t *p, ppl_info_t *out) {
     if (!p || !out) return fail(PPL_ERR_INVALID_ARG);
     memset(out, 0, sizeof(*out));
+    const bool sa = p->sym == PPL_SYM_PAIR_SA;
     out->nocc = p->o;
     out->nvirt = p->v;
     out->nchol = p->x;
@@ -546,98 +853,111 @@ int ppl_plan_info(const ppl_plan_t *p, ppl_info_t *out) {
     out->n_ablocks = out->n_bblocks = p->nblk;
     out->n_tiles = (int)p->tiles.size();
     out->ring = p->ring;
-    out->splitk = p->tiles.empty() ? 0 : p->tiles[0].splitk;
+    out->splitk = p->tiles.empty() ? 0 : (sa ? p->tiles[0].sp.splitk : p->tiles[0].full.splitk);
     out->vec16 = p->vec16;
-    out->launches_per_apply = 3 * (int)p->tiles.size();
-    out->step1_tile_m = p->bm1;
+    const bool minus = p->Mm > 0 && p->Km > 0;
+    out->launches_per_apply = sa ? 1 + (minus ? 5 : 4) * (int)p->tiles.size() : 3 * (int)p->tiles.size();
+    out->step1_tile_m = sa ? p->bm_p : p->bm_full;
     out->workspace_bytes = p->ws_bytes;
     const double v4 = std::pow((double)p->v, 4);
     out->flops_nominal = 2.0 * p->x * v4 + 2.0 * p->o * p->o * v4;
     out->flops_step0 = p->f_step0;
     out->flops_step1 = p->f_step1;
     out->flops_executed = p->f_step0 + p->f_step1;
+    out->sa_splitk_plus = p->tiles.empty() ? 0 : p->tiles[0].sp.splitk;
+    out->sa_splitk_minus = p->tiles.empty() ? 0 : p->tiles[0].sm.splitk;
+    out->sa_tile_m_plus = p->bm_p;
+    out->sa_tile_m_minus = p->bm_m;
+    out->sa_rows_plus = p->Mp;
+    out->sa_rows_minus = p->Mm;
+    out->sa_k_plus = p->Kp;
+    out->sa_k_minus = p->Km;
     return PPL_OK;
 }
 
-int ppl_apply(ppl_plan_t *p, const double *L, const double *t2, double *R, void *stream_) {
-    bool vec16 = false;
-    int rc = check_ptrs(p, L, t2, R, &vec16);
-    if (rc != PPL_OK) return fail(rc);
-    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
-    const int ntiles = (int)p->tiles.size();
-    const bool tma = p->use_tma && vec16;
-    ApplyMaps maps;
-    if (tma && (rc = make_apply_maps(p, L, t2, &maps)) != PPL_OK) return fail(rc);
-    const bool two_streams = p->ring >= 2 && ntiles >= 2;
-    cudaStream_t gen = two_streams ? p->gen : stream;
+int ppl_apply(ppl_plan_t *p, const double *L, const double *t2, double *R, void *stream) {
+    return run_apply(p, L, t2, R, nullptr, reinterpret_cast<cudaStream_t>(stream), nullptr);
+}
 
-    if (two_streams) {  // fork: the producer stream starts after prior work on `stream`
-        PPL_CUDA(cudaEventRecord(p->ev_in, stream));
-        PPL_CUDA(cudaStreamWaitEvent(gen, p->ev_in, 0));
-    }
-    for (int k = 0; k < ntiles; ++k) {
-        const Tile &t = p->tiles[k];
-        const int slot = k % p->ring;
-        if (two_streams && k >= p->ring) PPL_CUDA(cudaStreamWaitEvent(gen, p->ev_free[slot], 0));
-        rc = tma ? launch_step0_tma(p, t, maps.L, p->Wslot[slot], gen) : launch_step0(p, t, L, p->Wslot[slot], vec16, gen);
-        if (rc != PPL_OK) return rc;
-        if (two_streams) {
-            PPL_CUDA(cudaEventRecord(p->ev_ready[slot], gen));
-            PPL_CUDA(cudaStreamWaitEvent(stream, p->ev_ready[slot], 0));
-        }
-        rc = tma ? launch_step1_tma(p, t, maps.T, p->mapW[slot], stream) : launch_step1(p, t, t2, p->Wslot[slot], vec16, stream);
-        if (rc != PPL_OK) return rc;
-        if (two_streams) PPL_CUDA(cudaEventRecord(p->ev_free[slot], stream));
-        if ((rc = launch_reduce(p, t, R, stream)) != PPL_OK) return rc;
-    }
-    // join: every producer launch is followed by a consumer wait on `stream`, so `stream` already
-    // depends on all work of `gen`.
-    return PPL_OK;
+int ppl_apply_ex(ppl_plan_t *p, const double *L, const double *t2, double *R, const ppl_opts_t *opts, void *stream) {
+    return run_apply(p, L, t2, R, opts, reinterpret_cast<cudaStream_t>(stream), nullptr);
 }
 
 int ppl_apply_profiled(ppl_plan_t *p, const double *L, const double *t2, double *R, void *stream_, ppl_times_t *times) {
-    bool vec16 = false;
-    int rc = check_ptrs(p, L, t2, R, &vec16);
-    if (rc != PPL_OK || !times) return fail(rc != PPL_OK ? rc : PPL_ERR_INVALID_ARG);
+    if (!times) return fail(PPL_ERR_INVALID_ARG);
     cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
     memset(times, 0, sizeof(*times));
-    const int ntiles = (int)p->tiles.size();
-    const bool tma = p->use_tma && vec16;
-    ApplyMaps maps;
-    if (tma && (rc = make_apply_maps(p, L, t2, &maps)) != PPL_OK) return fail(rc);
-    std::vector<cudaEvent_t> ev(3 * (size_t)ntiles + 1);
-    for (auto &e : ev) PPL_CUDA(cudaEventCreate(&e));
-    PPL_CUDA(cudaEventRecord(ev[0], stream));
-    for (int k = 0; k < ntiles && rc == PPL_OK; ++k) {
-        const Tile &t = p->tiles[k];
-        rc = tma ? launch_step0_tma(p, t, maps.L, p->Wslot[0], stream) : launch_step0(p, t, L, p->Wslot[0], vec16, stream);
-        cudaEventRecord(ev[3 * k + 1], stream);
-        if (rc == PPL_OK)
-            rc = tma ? launch_step1_tma(p, t, maps.T, p->mapW[0], stream) : launch_step1(p, t, t2, p->Wslot[0], vec16, stream);
-        cudaEventRecord(ev[3 * k + 2], stream);
-        if (rc == PPL_OK) rc = launch_reduce(p, t, R, stream);
-        cudaEventRecord(ev[3 * k + 3], stream);
-    }
-    cudaError_t e = cudaStreamSynchronize(stream);
-    if (rc == PPL_OK && e == cudaSuccess) {
-        for (int k = 0; k < ntiles; ++k) {
-            float a = 0, b = 0, c = 0;
-            cudaEventElapsedTime(&a, ev[3 * k], ev[3 * k + 1]);
-            cudaEventElapsedTime(&b, ev[3 * k + 1], ev[3 * k + 2]);
-            cudaEventElapsedTime(&c, ev[3 * k + 2], ev[3 * k + 3]);
-            times->step0_ms += a;
-            times->step1_ms += b;
-            times->reduce_ms += c;
+    Prof prof;
+    int rc = run_apply(p, L, t2, R, nullptr, stream, &prof);
+    const cudaError_t e = cudaStreamSynchronize(stream);
+    if (rc == PPL_OK && e == cudaSuccess && prof.ev.size() >= 2) {
+        float acc[K_KINDS] = {0, 0, 0, 0, 0};
+        for (size_t k = 1; k < prof.ev.size(); ++k) {
+            float ms = 0;
+            cudaEventElapsedTime(&ms, prof.ev[k - 1], prof.ev[k]);
+            if (prof.kind[k] >= 0) acc[prof.kind[k]] += ms;
         }
-        cudaEventElapsedTime(&times->total_ms, ev[0], ev[3 * (size_t)ntiles]);
-        times->n_step0 = times->n_step1 = times->n_reduce = ntiles;
+        cudaEventElapsedTime(&times->total_ms, prof.ev.front(), prof.ev.back());
+        times->pack_ms = acc[K_PACK];
+        times->step0_ms = acc[K_STEP0];
+        times->fold_ms = acc[K_FOLD];
+        times->step1_ms = acc[K_STEP1];
+        times->reduce_ms = acc[K_REDUCE];
+        times->n_pack = prof.launches[K_PACK];
+        times->n_step0 = prof.launches[K_STEP0];
+        times->n_fold = prof.launches[K_FOLD];
+        times->n_step1 = prof.launches[K_STEP1];
+        times->n_reduce = prof.launches[K_REDUCE];
     }
-    for (auto &x : ev) cudaEventDestroy(x);
+    for (auto &x : prof.ev) cudaEventDestroy(x);
     if (e != cudaSuccess) {
         (void)cudaGetLastError();
         return fail(PPL_ERR_CUDA);
     }
     return rc;
+}
+
+int ppl_apply_dense(ppl_plan_t *p, const double *eri, int a0, int na, const double *t2, double *R, const ppl_opts_t *opts_in,
+                    void *stream_) {
+    bool vec16 = false;
+    int rc = check_ptrs(p, eri, t2, R, &vec16);
+    ppl_opts_t opts;
+    if (rc == PPL_OK) rc = check_opts(opts_in, &opts);
+    if (rc == PPL_OK && (a0 < 0 || na < 1 || a0 + na > p->v)) rc = PPL_ERR_INVALID_ARG;
+    if (rc != PPL_OK) return fail(rc);
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+    const double *t2m = t2;
+    if ((rc = t2_matrix(p, t2, opts.t2_layout, stream, &t2m)) != PPL_OK) return rc;
+    const bool tma = p->use_tma && vec16;
+    const int M = p->o * p->o;
+    const int64_t rows = (int64_t)na * p->v;
+    CUtensorMap mapT, mapE;
+    if (tma && (make_map_2d(&mapT, t2m, (uint64_t)p->vv, (uint64_t)M, (uint64_t)p->vv * 8, ppl::BK, (uint32_t)p->bm_full) != PPL_OK ||
+                make_map_2d(&mapE, eri, (uint64_t)p->vv, (uint64_t)rows, (uint64_t)p->vv * 8, ppl::BK, ppl::BN) != PPL_OK))
+        return fail(PPL_ERR_CUDA);
+    // rows of the slab matrix [(a,b)][(c,d)] in chunks the partials buffer can hold
+    const int chunk = (int)std::min<int64_t>(rows, std::max<int64_t>(ppl::BN, (int64_t)p->T * p->T / ppl::BN * ppl::BN));
+    Tile t;
+    t.a0 = a0;
+    t.b0 = 0;
+    t.ta = na;
+    t.tb = p->v;
+    t.mirror = 0;
+    for (int64_t n0 = 0; n0 < rows; n0 += chunk) {
+        const int N = (int)std::min<int64_t>(chunk, rows - n0);
+        const SplitChoice sc = choose_split(M, N, p->vv, p->num_sms, p->bm_full, p->part_bytes);
+        if ((size_t)sc.splitk * M * N * 8 > p->part_bytes) return fail(PPL_ERR_WORKSPACE_TOO_SMALL);
+        const double *B = eri + n0 * p->vv;
+        CUtensorMap mapB;  // the chunk's rows as their own tensor so that tile-edge rows beyond it read as zero
+        if (tma && make_map_2d(&mapB, B, (uint64_t)p->vv, (uint64_t)N, (uint64_t)p->vv * 8, ppl::BK, ppl::BN) != PPL_OK)
+            return fail(PPL_ERR_CUDA);
+        rc = launch_step1(p, tma ? &mapT : nullptr, tma ? &mapB : nullptr, p->ni_full, t2m, p->vv, B, p->vv, M, N, p->vv, sc,
+                          p->part, vec16, stream);
+        if (rc == PPL_OK) rc = launch_reduce(p, t, sc.splitk, N, (int)n0, p->v, R, opts, stream);
+        if (rc != PPL_OK) return rc;
+    }
+    (void)mapE;
+    return PPL_OK;
 }
 
 int ppl_apply_host(ppl_plan_t *p, const double *Lh, const double *t2h, double *Rh, uint64_t *h2d, uint64_t *d2h) {
@@ -682,7 +1002,7 @@ int ppl_check_inputs(ppl_plan_t *p, const double *L, const double *t2, void *str
     PPL_CUDA(cudaMemcpyAsync(&h, p->flags, sizeof(int), cudaMemcpyDeviceToHost, stream));
     PPL_CUDA(cudaStreamSynchronize(stream));
     if (flags) *flags = h;
-    if ((h & 2) && p->sym == PPL_SYM_PAIR) return fail(PPL_ERR_PRECONDITION);
+    if ((h & 2) && p->sym != PPL_SYM_NONE) return fail(PPL_ERR_PRECONDITION);
     return PPL_OK;
 }
 

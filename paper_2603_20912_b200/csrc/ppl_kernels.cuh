@@ -314,31 +314,177 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_step1(const Step1Args p) {
 
 // ---------------------------------------------------------------------------------------------
 // reduce + accumulate + mirror (fixed summation order over z: bit-reproducible)
+//   R = beta*R + alpha*sum_z part[z]   (beta == 0: overwrite, R is not read)
+// R is addressed through four element strides so that both storage orders of SURVEY 8(f) NEXT-1
+// ('ijab' = BASELINE.json / the paper's 'efab', and 'iajb' = the paper's 'iajb') are
+// written in place -- the paper's transpose step folds into this addressing.
+// Every R entry is touched exactly once per apply (tiles partition (a,b); the mirror covers the
+// other triangle), so beta scaling here is exact.
 // ---------------------------------------------------------------------------------------------
+struct RStrides {
+    int64_t i, j, a, b;  // element strides of R[i,j,a,b]
+};
 struct ReduceArgs {
     const double *part;  // [splitk][M][N]
     int splitk;
-    int M, N;            // nocc^2, ta*tb
+    int M, N;            // nocc^2, rows of this W tile
     int o, v, tb;        // nocc, nvirt, b count of this tile
     int a0, b0;          // first virtual index of the a / b block
-    int mirror;          // 1: also accumulate into R[j,i,b,a]
+    int n_off;           // row offset added to n before the (a,b) decode (dense-ERI slabs)
+    int mirror;          // 1: also write R[j,i,b,a]
+    double alpha, beta;
+    RStrides rs;
     double *R;
 };
 
+__device__ __forceinline__ void r_update(double *r, double val, double alpha, double beta) {
+    *r = (beta == 0.0) ? alpha * val : beta * (*r) + alpha * val;
+}
+
 __global__ void __launch_bounds__(256) k_reduce(const ReduceArgs p) {
     const int64_t MN = (int64_t)p.M * p.N;
-    const int64_t vv = (int64_t)p.v * p.v;
     for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < MN; idx += (int64_t)gridDim.x * blockDim.x) {
         double s = 0.0;
         for (int z = 0; z < p.splitk; ++z) s += p.part[(int64_t)z * MN + idx];
-        const int m = (int)(idx / p.N), n = (int)(idx - (int64_t)m * p.N);
+        const int m = (int)(idx / p.N), n = (int)(idx - (int64_t)m * p.N) + p.n_off;
         const int al = n / p.tb, bl = n - al * p.tb;
         const int a = p.a0 + al, b = p.b0 + bl;
-        p.R[(int64_t)m * vv + (int64_t)a * p.v + b] += s;
-        if (p.mirror) {
-            const int i = m / p.o, j = m - i * p.o;
-            p.R[(int64_t)(j * p.o + i) * vv + (int64_t)b * p.v + a] += s;
+        const int i = m / p.o, j = m - i * p.o;
+        r_update(p.R + i * p.rs.i + j * p.rs.j + a * p.rs.a + b * p.rs.b, s, p.alpha, p.beta);
+        if (p.mirror) r_update(p.R + j * p.rs.i + i * p.rs.j + b * p.rs.a + a * p.rs.b, s, p.alpha, p.beta);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// PPL_SYM_PAIR_SA: symmetric / antisymmetric packing.
+// For pair-symmetric t2 and ANY L, with (c,d) packed over c <= d (k+) and c < d (k-):
+//   W+-[(ab)][k]  = X[(ab)][c,d] +- X[(ab)][d,c]          (X = step-0 tile (ac|bd); W+ diag = X[c,c])
+//   tau+-[(ij)][k] = (t2[ij][c,d] +- t2[ij][d,c]) / 2      (i <= j rows only;   tau+ diag = t2[c,c])
+//   R+- = tau+- W+-^T ;  R[i,j,a,b] = R+ + R- ;  R[j,i,a,b] = R+ - R-
+// Both packings are the same gather: k_symfold does either (scale 1 for W, 1/2 for tau).
+// ---------------------------------------------------------------------------------------------
+__host__ __device__ __forceinline__ int64_t kplus(int c, int d, int v) { return (int64_t)c * v - (int64_t)c * (c - 1) / 2 + (d - c); }
+__host__ __device__ __forceinline__ int64_t kminus(int c, int d, int v) { return (int64_t)c * (2 * v - c - 1) / 2 + (d - c - 1); }
+
+struct FoldArgs {
+    const double *src;   // row r, element (c,d) at src + roff(r) + c*sc + d   (d contiguous)
+    int64_t sc;          // stride of c
+    int64_t s_row;       // mode 0: row r at r*s_row
+    int64_t s_i, s_j;    // mode 1: row (i,j) at i*s_i + j*s_j
+    int mode;            // 0: fold W tile rows (every row has + and -); 1: pack amplitudes, rows (i<=j) of an o x o grid
+    int rows;            // mode 0: number of rows; mode 1: o*o (rows with i > j are skipped)
+    int o, v;
+    double scale;        // factor of the off-diagonal (c<d) entries: 1 (W) or 1/2 (tau)
+    double *dp, *dm;     // packed outputs, row strides ldp / ldm
+    int64_t ldp, ldm;
+};
+
+constexpr int FT = 32;  // (c,d) block edge of the fold
+
+__global__ void __launch_bounds__(256) k_symfold(const FoldArgs p) {
+    __shared__ double sa[FT][FT + 1], sb[FT][FT + 1];
+    const int nbv = (p.v + FT - 1) / FT;
+    // blockIdx.x -> block pair (cb <= db); blockIdx.y strides over rows
+    int cb = 0, rem = blockIdx.x;
+    while (rem >= nbv - cb) {
+        rem -= nbv - cb;
+        ++cb;
+    }
+    const int db = cb + rem;
+    const int c0 = cb * FT, d0 = db * FT;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;  // 32 x 8
+    for (int r = blockIdx.y; r < p.rows; r += gridDim.y) {
+        int64_t roff, rowp, rowm;
+        if (p.mode == 0) {
+            roff = (int64_t)r * p.s_row;
+            rowp = rowm = r;
+        } else {
+            const int i = r / p.o, j = r - i * p.o;
+            if (i > j) continue;
+            roff = i * p.s_i + j * p.s_j;
+            rowp = (int64_t)i * p.o - (int64_t)i * (i - 1) / 2 + (j - i);
+            rowm = (i < j) ? (int64_t)i * (2 * p.o - i - 1) / 2 + (j - i - 1) : -1;
         }
+        const double *s = p.src + roff;
+        __syncthreads();  // previous row's reads of sa/sb are done
+#pragma unroll
+        for (int y = ty; y < FT; y += 8) {
+            const int c = c0 + y, d = d0 + tx;
+            sa[y][tx] = (c < p.v && d < p.v) ? s[(int64_t)c * p.sc + d] : 0.0;
+            if (cb != db) {
+                const int c2 = d0 + y, d2 = c0 + tx;  // the transposed block: element (c2,d2), c2 in db, d2 in cb
+                sb[y][tx] = (c2 < p.v && d2 < p.v) ? s[(int64_t)c2 * p.sc + d2] : 0.0;
+            }
+        }
+        __syncthreads();
+        double *op = p.dp + rowp * p.ldp;
+        double *om = rowm >= 0 ? p.dm + rowm * p.ldm : nullptr;
+#pragma unroll
+        for (int y = ty; y < FT; y += 8) {
+            const int c = c0 + y, d = d0 + tx;
+            if (c >= p.v || d >= p.v || d < c) continue;
+            const double xcd = sa[y][tx];
+            if (c == d) {
+                op[kplus(c, d, p.v)] = xcd;
+            } else {
+                const double xdc = (cb != db) ? sb[tx][y] : sa[tx][y];
+                op[kplus(c, d, p.v)] = p.scale * (xcd + xdc);
+                if (om) om[kminus(c, d, p.v)] = p.scale * (xcd - xdc);
+            }
+        }
+    }
+}
+
+struct ReduceSaArgs {
+    const double *partp, *partm;  // [sp][Mp][N], [sm][Mm][N]
+    int sp, sm;
+    int Mp, Mm, N;
+    int o, v, tb, a0, b0;
+    int mirror;                   // off-diagonal tile: also write the (b,a) entries
+    double alpha, beta;
+    RStrides rs;
+    double *R;
+};
+
+__global__ void __launch_bounds__(256) k_reduce_sa(const ReduceSaArgs p) {
+    const int64_t total = (int64_t)p.Mp * p.N;
+    const int64_t MpN = total, MmN = (int64_t)p.Mm * p.N;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int mp = (int)(idx / p.N), n = (int)(idx - (int64_t)mp * p.N);
+        // packed row mp -> (i <= j): i = largest with i*o - i(i-1)/2 <= mp
+        int i = (int)((2.0 * p.o + 1.0 - sqrt((2.0 * p.o + 1.0) * (2.0 * p.o + 1.0) - 8.0 * mp)) * 0.5);
+        while (i > 0 && (int64_t)i * p.o - (int64_t)i * (i - 1) / 2 > mp) --i;
+        while ((int64_t)(i + 1) * p.o - (int64_t)(i + 1) * i / 2 <= mp) ++i;
+        const int j = i + (mp - (int)((int64_t)i * p.o - (int64_t)i * (i - 1) / 2));
+        double rp = 0.0, rm = 0.0;
+        for (int z = 0; z < p.sp; ++z) rp += p.partp[(int64_t)z * MpN + idx];
+        if (i < j) {
+            const int64_t mm = (int64_t)i * (2 * p.o - i - 1) / 2 + (j - i - 1);
+            const int64_t im = mm * p.N + n;
+            for (int z = 0; z < p.sm; ++z) rm += p.partm[(int64_t)z * MmN + im];
+        }
+        const int al = n / p.tb, bl = n - al * p.tb;
+        const int a = p.a0 + al, b = p.b0 + bl;
+        const double v1 = rp + rm, v2 = rp - rm;  // R[i,j,a,b], R[j,i,a,b]
+        r_update(p.R + i * p.rs.i + j * p.rs.j + a * p.rs.a + b * p.rs.b, v1, p.alpha, p.beta);
+        if (i < j) r_update(p.R + j * p.rs.i + i * p.rs.j + a * p.rs.a + b * p.rs.b, v2, p.alpha, p.beta);
+        if (p.mirror) {
+            r_update(p.R + j * p.rs.i + i * p.rs.j + b * p.rs.a + a * p.rs.b, v1, p.alpha, p.beta);
+            if (i < j) r_update(p.R + i * p.rs.i + j * p.rs.j + b * p.rs.a + a * p.rs.b, v2, p.alpha, p.beta);
+        }
+    }
+}
+
+// t2 stored 'iajb' ([i][c][j][d], the paper's 'icjd') -> [i][j][c][d] for the un-packed modes
+__global__ void __launch_bounds__(256) k_permute_t2(const double *src, double *dst, int o, int v) {
+    const int64_t total = (int64_t)o * o * v * v;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int d = (int)(idx % v);
+        int64_t r = idx / v;
+        const int c = (int)(r % v);
+        r /= v;
+        const int j = (int)(r % o), i = (int)(r / o);
+        dst[idx] = src[(((int64_t)i * v + c) * o + j) * v + d];
     }
 }
 

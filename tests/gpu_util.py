@@ -4,7 +4,8 @@ import numpy as np
 import paper_2603_20912_b200 as P
 
 
-def gpu_ladder(L, t2, R0=None, sym=P.PPL_SYM_PAIR, workspace_bytes=0, return_info=False, stream=None):
+def gpu_ladder(L, t2, R0=None, sym=None, workspace_bytes=0, return_info=False, stream=None):
+    """sym=None: the plan's default (PPL_SYM_PAIR_SA when the workspace holds the packed operands, else PPL_SYM_PAIR)."""
     import torch
 
     x, v, _ = L.shape
@@ -14,7 +15,7 @@ def gpu_ladder(L, t2, R0=None, sym=P.PPL_SYM_PAIR, workspace_bytes=0, return_inf
     td = torch.from_numpy(t2).to(dev)
     Rd = torch.zeros((o, o, v, v), dtype=torch.float64, device=dev) if R0 is None else torch.from_numpy(R0).to(dev)
     with P.Plan(o, v, x, workspace_bytes) as plan:
-        if sym != P.PPL_SYM_PAIR:
+        if sym is not None:
             plan.set_symmetry(sym)
         info = plan.info()
         plan.apply(Ld, td, Rd, stream)

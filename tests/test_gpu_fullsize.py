@@ -34,7 +34,8 @@ def _host_gb():
     return 0.0
 
 
-def _run(name, integer=False):
+def _run(name, integer=False, sym=None):
+    """sym=None: the plan's default, which is what bench.py times (PPL_SYM_PAIR_SA)."""
     import torch
 
     o, v, x = I.CONFIGS[name]
@@ -42,8 +43,14 @@ def _run(name, integer=False):
     t2 = I.make_t2(o, v, 0, integer=integer)
     Ld, td = torch.from_numpy(L).cuda(), torch.from_numpy(t2).cuda()
     Rd = torch.zeros((o, o, v, v), dtype=torch.float64, device="cuda")
+    if integer:
+        td *= 2.0  # (t2[cd] +- t2[dc]) / 2 stays an integer in the packed mode
+        t2 *= 2.0
     with P.Plan(o, v, x) as plan:
+        if sym is not None:
+            plan.set_symmetry(sym)
         info = plan.info()
+        assert info["symmetry"] == (P.PPL_SYM_PAIR_SA if sym is None else sym)
         assert plan.check_inputs(Ld, td) == 0
         plan.apply(Ld, td, Rd)
         torch.cuda.synchronize()
@@ -90,8 +97,9 @@ def _check_projections(L, t2, Rd, rmax, nrand=2):
         assert np.abs(got - want).max() <= bound, (np.abs(got - want).max(), bound)
 
 
-def test_medium_sampled_columns_and_projections():
-    L, t2, Rd, info = _run("medium")
+@pytest.mark.parametrize("sym", [None, P.PPL_SYM_PAIR])
+def test_medium_sampled_columns_and_projections(sym):
+    L, t2, Rd, info = _run("medium", sym=sym)
     assert info["n_tiles"] > 1
     rmax = float(Rd.abs().max().item())
     _check_columns(L, t2, Rd, 256)
@@ -103,8 +111,9 @@ def test_medium_sampled_columns_and_projections():
         assert np.abs(Rd.cpu().numpy() - want).max() <= TOL * np.abs(want).max()
 
 
-def test_medium_exact_integers_sampled():
-    L, t2, Rd, _ = _run("medium", integer=True)
+@pytest.mark.parametrize("sym", [None, P.PPL_SYM_PAIR])
+def test_medium_exact_integers_sampled(sym):
+    L, t2, Rd, _ = _run("medium", integer=True, sym=sym)
     _check_columns(L, t2, Rd, 128, exact=True)
 
 
@@ -136,10 +145,11 @@ def test_medium_closed_form_tagged_tiles_repeated():
             assert int((R != want).sum().item()) == 0
 
 
-def test_large_sampled_columns_and_projections():
+@pytest.mark.parametrize("sym", [None, P.PPL_SYM_PAIR])
+def test_large_sampled_columns_and_projections(sym):
     if _host_gb() < 16:
         pytest.skip("not enough host memory for the large config")
-    L, t2, Rd, info = _run("large")
+    L, t2, Rd, info = _run("large", sym=sym)
     rmax = float(Rd.abs().max().item())
     _check_columns(L, t2, Rd, 96)
     _check_projections(L, t2, Rd, rmax, nrand=1)

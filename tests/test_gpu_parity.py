@@ -37,7 +37,7 @@ def test_dmma_fragment_layout():
 
 
 @pytest.mark.parametrize("name", ["tiny", "small"])
-@pytest.mark.parametrize("sym", [P.PPL_SYM_PAIR, P.PPL_SYM_NONE])
+@pytest.mark.parametrize("sym", [P.PPL_SYM_PAIR_SA, P.PPL_SYM_PAIR, P.PPL_SYM_NONE])
 def test_configs_0_1_full_parity(name, sym):
     L, t2 = I.make_config(name, seed=0)
     want = oracle.full(L, t2)
@@ -53,22 +53,35 @@ SHAPES = [
 ]
 
 
+def _cap(o, v, cap_cols, sym):
+    """workspace cap in units of W columns (v*v*8 bytes each) + room for partials (+ the packed
+    amplitudes and the un-folded step-0 tile in PPL_SYM_PAIR_SA): forces small tiles"""
+    if cap_cols == 0:
+        return 0
+    cap = cap_cols * v * v * 8 + 64 * o * o * cap_cols * 8 + 4096
+    if sym == P.PPL_SYM_PAIR_SA:
+        cap += (o * o + cap_cols) * (v * v + 64) * 8 + 4096
+    return cap
+
+
 @pytest.mark.parametrize("shape", SHAPES)
-@pytest.mark.parametrize("sym", [P.PPL_SYM_PAIR, P.PPL_SYM_NONE])
+@pytest.mark.parametrize("sym", [P.PPL_SYM_PAIR_SA, P.PPL_SYM_PAIR, P.PPL_SYM_NONE])
 @pytest.mark.parametrize("cap_cols", [0, 40, 7])
 def test_shapes_full_parity(shape, sym, cap_cols):
     o, v, x = shape
-    symmetric = sym == P.PPL_SYM_PAIR
+    symmetric = sym != P.PPL_SYM_NONE
     L = I.make_L(v, x, seed=5, symmetric=symmetric)  # non-symmetric L in general mode
     t2 = I.make_t2(o, v, seed=5, symmetric=symmetric)
+    if sym != P.PPL_SYM_NONE:  # the pair modes need pair-symmetric t2 only: L stays non-symmetric
+        L = I.make_L(v, x, seed=5, symmetric=False)
     want = oracle.full(L, t2)
-    # workspace cap in units of W columns (v*v*8 bytes each) + room for partials: forces small tiles
-    cap = 0 if cap_cols == 0 else cap_cols * v * v * 8 + 64 * o * o * cap_cols * 8 + 4096
+    cap = _cap(o, v, cap_cols, sym)
     try:
         got, info = gpu_ladder(L, t2, sym=sym, workspace_bytes=cap, return_info=True)
     except P.PplError as e:
         assert e.code == P.PPL_ERR_WORKSPACE_TOO_SMALL and cap_cols == 7
         pytest.skip("cap below the minimum plan for this shape")
+    assert info["symmetry"] == sym
     assert relerr(got, want) <= TOL, info
     if cap_cols and cap < v**4 * 8:  # the cap cannot hold the whole W: the plan must have tiled it
         assert info["n_tiles"] > 1 and info["workspace_bytes"] <= cap, info
@@ -96,31 +109,33 @@ def test_accumulate_semantics_and_zero_t2():
 
 
 @pytest.mark.parametrize("shape,cap_cols", [((5, 20, 60), 0), ((5, 53, 40), 0), ((4, 37, 19), 40), ((12, 18, 9), 7)])
-@pytest.mark.parametrize("sym", [P.PPL_SYM_PAIR, P.PPL_SYM_NONE])
+@pytest.mark.parametrize("sym", [P.PPL_SYM_PAIR_SA, P.PPL_SYM_PAIR, P.PPL_SYM_NONE])
 def test_exact_integers_bit_for_bit(shape, cap_cols, sym):
     """Small-integer inputs: every product and partial sum is exact in binary64, so any summation
     order gives the same bits -> separates logic bugs (tile edges, mirror, split-K) from rounding."""
     o, v, x = shape
-    symmetric = sym == P.PPL_SYM_PAIR
+    symmetric = sym != P.PPL_SYM_NONE
     L = I.make_L(v, x, 41, symmetric=symmetric, integer=True)
     t2 = I.make_t2(o, v, 41, symmetric=symmetric, integer=True)
-    cap = 0 if cap_cols == 0 else cap_cols * v * v * 8 + 64 * o * o * cap_cols * 8 + 4096
-    got = gpu_ladder(L, t2, sym=sym, workspace_bytes=cap)
+    if sym == P.PPL_SYM_PAIR_SA:
+        t2 *= 2.0  # tau+- = (t2[cd] +- t2[dc]) / 2 stays an exact integer
+    got = gpu_ladder(L, t2, sym=sym, workspace_bytes=_cap(o, v, cap_cols, sym))
     assert np.array_equal(got, oracle.full(L, t2))
 
 
 @pytest.mark.parametrize("shape", [(24, 64, 128), (16, 72, 200), (30, 48, 260)])
-def test_persistent_ring_many_items_per_cta(shape):
+@pytest.mark.parametrize("sym", [P.PPL_SYM_PAIR_SA, P.PPL_SYM_PAIR])
+def test_persistent_ring_many_items_per_cta(shape, sym):
     """Regression for a shared-memory WAR race in the persistent TMA kernels: every CTA runs several
     work items back to back and every item has more k-tiles than the ring has stages, so slots are
     refilled across item boundaries while other warps are in their epilogue.  Exact-integer inputs:
     any stale or early fragment changes the bits.  Repeated, because the race was timing dependent."""
     o, v, x = shape
     L = I.make_L(v, x, 43, integer=True)
-    t2 = I.make_t2(o, v, 43, integer=True)
+    t2 = 2.0 * I.make_t2(o, v, 43, integer=True)
     want = oracle.full(L, t2)
     for rep in range(6):
-        got, info = gpu_ladder(L, t2, return_info=True)
+        got, info = gpu_ladder(L, t2, sym=sym, return_info=True)
         assert np.array_equal(got, want), (rep, info)
 
 
