@@ -38,10 +38,12 @@ if ROOT not in sys.path:
 
 METRIC = "pp_ladder_fp64_tflops_executed"
 UNIT = "TFLOP/s"
-SYM_NAMES = {0: "none", 1: "pair", 2: "pair_sa"}
+SYM_NAMES = {0: "none", 1: "pair", 2: "pair_sa", 3: "full"}
 SYM_DESC = {0: "none (every tile)", 1: "pair (tiles a-block<=b-block, mirrored)",
             2: "pair_sa (tiles a-block<=b-block, mirrored; step 1 on symmetric/antisymmetric packed (i<=j),(c<=d) operands: "
-               "step-0 flops x~1/2, step-1 flops x~1/4 of nominal)"}
+               "step-0 flops x~1/2, step-1 flops x~1/4 of nominal)",
+            3: "full (8-fold ERI symmetry L[P,a,c]=L[P,c,a] + pair symmetry of t2: slabs of 16 a's, symmetric packed "
+               "S+-[(a<=b)][(c<=d)] blocks generated once and used twice: step-0 flops x~1/8, step-1 flops x~1/4 of nominal)"}
 NOMINAL_FP64_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 * 1e-12  # 148 SM x 4 SMSP x 16 FMA/clk x 2 x 1.965 GHz = 37.23
 
 
@@ -167,8 +169,8 @@ def main():
     ap.add_argument("--config", default="large")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workspace-gb", type=float, default=0.0, help="workspace cap (0 = auto)")
-    ap.add_argument("--symmetry", default="default", choices=["default", "pair_sa", "pair", "none"],
-                    help="default = the plan's own choice (pair_sa: A<=B tiles + symmetric/antisymmetric packed step 1)")
+    ap.add_argument("--symmetry", default="default", choices=["default", "full", "pair_sa", "pair", "none"],
+                    help="default = the plan's own choice (full: 8-fold ERI symmetry + pair symmetry, from nvirt = 96 up)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -58,12 +58,23 @@ enum {
                          a-block <= b-block are computed and the result is also written into
                          the mirrored entries.  Result undefined if t2 is not pair-symmetric
                          (ppl_check_inputs detects that). */
-    PPL_SYM_PAIR_SA = 2 /* same precondition as PPL_SYM_PAIR, and the same tiles; in addition step 1
+    PPL_SYM_PAIR_SA = 2,/* same precondition as PPL_SYM_PAIR, and the same tiles; in addition step 1
                          runs on symmetric / antisymmetric packed operands
                              W+-[(ab)][(c<=d)] = (ac|bd) +- (ad|bc),  tau+-[(i<=j)][(c<=d)] = (t2[ij,cd] +- t2[ij,dc])/2,
                              R[i,j,a,b] = R+ + R-,  R[j,i,a,b] = R+ - R-,
                          which halves the flops of step 1 again (an identity for ANY L; SURVEY.md 8(f)
-                         NEXT-4, pinned on the CPU by tests/test_oracle_pins.py).  Default. */
+                         NEXT-4, pinned on the CPU by tests/test_oracle_pins.py). */
+    PPL_SYM_FULL = 3    /* preconditions: t2 pair-symmetric AND L[P,a,c] == L[P,c,a] (real orbitals, PAPER.md:66;
+                         both named by north_star).  Then (ac|bd) has the full 8-fold symmetry and
+                             S+-[(a<=b)][(c<=d)] = (ac|bd) +- (ad|bc)
+                         is a SYMMETRIC matrix in its two pair indices: only its blocks on or above the diagonal
+                         are generated (a-blocks of 16; for slab A all of b, c, d >= A), each used twice
+                         (R+-[.][(ab)] += tau+-[.][(cd)] S[(ab)][(cd)] and R+-[.][(cd)] += tau+-[.][(ab)] S[(ab)][(cd)]),
+                         and step 0 computes only (ac|bd) with d-block >= b-block.  Executed flops: step 0 ~ 1/8,
+                         step 1 ~ 1/4 of nominal.  Result undefined if a precondition is violated
+                         (ppl_check_inputs detects both).  Needs even nvirt and 16-byte aligned pointers; its
+                         buffers (a 16 x nvirt^3 strip and the R+- accumulators) are allocated by ppl_plan when
+                         they fit under the workspace cap.  Default when available and nvirt >= 96. */
 };
 
 /* Storage orders of the 4-index arrays t2 and R. */
@@ -104,6 +115,11 @@ typedef struct ppl_info_s {
     int32_t sa_tile_m_plus, sa_tile_m_minus; /* PPL_SYM_PAIR_SA: CTA tile rows of the + / - GEMMs */
     int32_t sa_rows_plus, sa_rows_minus;     /* nocc(nocc+1)/2, nocc(nocc-1)/2 */
     int32_t sa_k_plus, sa_k_minus;           /* nvirt(nvirt+1)/2, nvirt(nvirt-1)/2 */
+    int32_t full_available;                  /* 1: ppl_plan allocated the PPL_SYM_FULL buffers */
+    int32_t full_tbg;                        /* PPL_SYM_FULL: b-group width (tile = 16 a's x full_tbg b's) */
+    int32_t full_slabs;                      /* PPL_SYM_FULL: number of a-blocks of 16 (one step-0 launch each) */
+    int32_t reserved_;
+    uint64_t full_workspace_bytes;           /* part of workspace_bytes that belongs to PPL_SYM_FULL */
 } ppl_info_t;
 
 /* Per-stage device times of the most recent profiled apply (ppl_apply_profiled), milliseconds. */
@@ -176,16 +192,17 @@ int ppl_destroy(ppl_plan_t *plan);
 int ppl_last_error(void);                /* code of the last failure on this thread */
 const char *ppl_error_string(int code);  /* static string, never NULL */
 
-/* Set PPL_SYM_NONE / PPL_SYM_PAIR / PPL_SYM_PAIR_SA (default PPL_SYM_PAIR_SA; PPL_SYM_PAIR if the
- * workspace cap was too small for the packed operands).  Re-plans the tile list; must not be
- * called while an apply is in flight. */
+/* Set PPL_SYM_NONE / PPL_SYM_PAIR / PPL_SYM_PAIR_SA / PPL_SYM_FULL.  Default: PPL_SYM_FULL when its
+ * buffers fit and nvirt >= 96 (even nvirt), else PPL_SYM_PAIR_SA, else PPL_SYM_PAIR if the workspace cap
+ * was too small for the packed operands.  PPL_ERR_WORKSPACE_TOO_SMALL if the plan holds no buffers for
+ * the requested mode.  Re-plans the tile list; must not be called while an apply is in flight. */
 int ppl_plan_set_symmetry(ppl_plan_t *plan, int mode);
 
 int ppl_plan_info(const ppl_plan_t *plan, ppl_info_t *out);
 
-/* Debug: verify on the device that L[P,a,c]==L[P,c,a] (reported, not required) and, in
- * PPL_SYM_PAIR mode, that t2[i,j,c,d]==t2[j,i,d,c] (required).  Synchronises `stream`.
- * Returns PPL_OK, or PPL_ERR_PRECONDITION if t2 violates the symmetry the plan relies on.
+/* Debug: verify on the device that L[P,a,c]==L[P,c,a] (required in PPL_SYM_FULL, else only reported)
+ * and, in every mode but PPL_SYM_NONE, that t2[i,j,c,d]==t2[j,i,d,c] (required).  Synchronises `stream`.
+ * Returns PPL_OK, or PPL_ERR_PRECONDITION if an input violates a symmetry the plan relies on.
  * If flags != NULL: bit 0 = L not symmetric, bit 1 = t2 not pair-symmetric. */
 int ppl_check_inputs(ppl_plan_t *plan, const double *L, const double *t2, void *stream, int *flags);
 

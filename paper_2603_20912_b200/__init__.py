@@ -18,6 +18,7 @@ from .binding import (  # noqa: F401
     PPL_LAYOUT_IJAB,
     PPL_SYM_PAIR,
     PPL_SYM_PAIR_SA,
+    PPL_SYM_FULL,
     SYMBOLS,
     Plan,
     PplError,

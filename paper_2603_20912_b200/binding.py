@@ -22,6 +22,7 @@ PPL_ERR_PRECONDITION = 6
 PPL_SYM_NONE = 0
 PPL_SYM_PAIR = 1
 PPL_SYM_PAIR_SA = 2
+PPL_SYM_FULL = 3
 PPL_LAYOUT_IJAB = 0
 PPL_LAYOUT_IAJB = 1
 LAYOUTS = {"ijab": PPL_LAYOUT_IJAB, "iajb": PPL_LAYOUT_IAJB}
@@ -40,6 +41,8 @@ class ppl_info_t(ctypes.Structure):
         ("sa_tile_m_plus", c_int32), ("sa_tile_m_minus", c_int32),
         ("sa_rows_plus", c_int32), ("sa_rows_minus", c_int32),
         ("sa_k_plus", c_int32), ("sa_k_minus", c_int32),
+        ("full_available", c_int32), ("full_tbg", c_int32), ("full_slabs", c_int32), ("reserved_", c_int32),
+        ("full_workspace_bytes", c_uint64),
     ]
 
     def asdict(self):

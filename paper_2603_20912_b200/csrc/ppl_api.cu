@@ -4,6 +4,7 @@
 #include "../../include/ppl.h"
 #include "ppl_kernels.cuh"
 #include "ppl_kernels_tma.cuh"
+#include "ppl_kernels_full.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -42,6 +43,23 @@ struct Tile {
     SplitChoice sp, sm;  // step 1 over the packed K+ / K- ranges  (PPL_SYM_PAIR_SA)
 };
 
+// PPL_SYM_FULL: one tile = (a-block A of 16) x (a group of b's), one slab = all tiles of one A
+struct FullTile {
+    int A0, ta;      // a-block
+    int bg0, nb;     // first b of the group, number of b's in it
+    int tbp;         // nb rounded up to a multiple of 16: W-tile rows are a_l*tbp + b_l
+    int k0p, k0m;    // first packed (c<=d) / (c<d) index with c >= A0: start of the use-1 contraction range
+    int k1p, k1m;    // first packed index with c >= A0+16: start of the use-2 output range
+    SplitChoice sp, sm;
+};
+struct FullSlab {
+    int A0, ta;
+    int tiles_m, tiles_n;  // step-0 CTA tiles: 128 rows (c, a_l), 128 columns (8 chunks of 16 d's)
+    size_t chunk_off;      // first entry of this slab in the chunk table
+    int tile_begin, tile_end;
+    double flops0;
+};
+
 constexpr int MAX_RING = 4;
 constexpr double PEAK_FLOPS = 37.2e12;  // nominal FP64 (148 SM x 64 FMA/clk x 2 x 1.965 GHz); planner cost model only
 constexpr double HBM_BPS = 6.0e12;      // planner cost model only
@@ -64,7 +82,8 @@ struct ppl_plan_s {
     int64_t vv = 0;       // nvirt^2 = row length of an un-packed W tile / of t2
     // packed geometry (PPL_SYM_PAIR_SA)
     int Mp = 0, Mm = 0;   // rows (i<=j), (i<j)
-    int Kp = 0, Km = 0;   // columns (c<=d), (c<d)
+    int Kp = 0, Km = 0;   // extents of the packed column indices of (c<=d), (c<d), holes included
+    int KpT = 0, KmT = 0; // number of pairs (c<=d), (c<d)
     int64_t ldp = 0, ldm = 0;
     int ni_full = 8, bm_full = 128, ni_p = 8, bm_p = 128, ni_m = 8, bm_m = 128;  // step-1 CTA tile rows (16*NI)
     size_t cap = 0;
@@ -82,6 +101,21 @@ struct ppl_plan_s {
     double *dL = nullptr, *dT = nullptr, *dR = nullptr;  // ppl_apply_host staging
     double f_step0 = 0, f_step1 = 0;
     CUtensorMap mapW[MAX_RING], mapWp[MAX_RING], mapWm[MAX_RING], mapTp, mapTm;  // plan-owned operands
+    // ---- PPL_SYM_FULL (own allocation `fws`; shares taup/taum with PPL_SYM_PAIR_SA) ----
+    int full_ok = 0;
+    int tbg = 0;                               // b-group width (multiple of 16)
+    size_t fws_bytes = 0;
+    unsigned char *fws = nullptr;
+    double *fX = nullptr;                      // strip [16*v rows (a_l*v + b)][vv]
+    double *fWp = nullptr, *fWm = nullptr;     // W+- tile [16*tbg][ldp], [16*tbg][ldm]
+    double *fpart = nullptr;
+    double *raccp = nullptr, *raccm = nullptr; // R+- accumulators [Mp][ldp], [Mm][ldm]
+    int2 *fchunks = nullptr;
+    size_t fpart_bytes = 0;
+    std::vector<FullSlab> slabs;
+    std::vector<FullTile> ftiles;
+    double ff_step0 = 0, ff_step1 = 0;
+    CUtensorMap mapFWp, mapFWm, mapFWpT, mapFWmT;  // the W+- tile as the B operand of use 1 (box 16 x 128 rows) / use 2 (box 16 x 16 rows)
 };
 
 namespace {
@@ -209,7 +243,7 @@ int build_tiles(ppl_plan_s *p) {
                 t.sm = choose_split(p->Mm, N, p->Km, p->num_sms, p->bm_m);
                 if (((size_t)t.sp.splitk * p->Mp + (size_t)t.sm.splitk * p->Mm) * N * 8 > p->part_bytes)
                     return PPL_ERR_WORKSPACE_TOO_SMALL;
-                p->f_step1 += 2.0 * N * ((double)p->Mp * p->Kp + (double)p->Mm * p->Km);
+                p->f_step1 += 2.0 * N * ((double)p->Mp * p->KpT + (double)p->Mm * p->KmT);
             } else {
                 t.full = choose_split(M, N, p->vv, p->num_sms, p->bm_full, p->part_bytes);
                 if ((size_t)t.full.splitk * M * N * 8 > p->part_bytes) return PPL_ERR_WORKSPACE_TOO_SMALL;
@@ -237,6 +271,7 @@ void free_plan(ppl_plan_s *p) {
         if (p->ev_free[i]) cudaEventDestroy(p->ev_free[i]);
     }
     if (p->ws) cudaFree(p->ws);
+    if (p->fws) cudaFree(p->fws);
     if (p->flags) cudaFree(p->flags);
     if (p->tperm) cudaFree(p->tperm);
     if (p->dL) cudaFree(p->dL);
@@ -253,8 +288,10 @@ int set_kernel_attrs() {
     PPL_CUDA(cudaFuncSetAttribute(ppl::k_step1<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_K));
     PPL_CUDA(cudaFuncSetAttribute(ppl::k_step1<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_K));
     PPL_CUDA(cudaFuncSetAttribute(ppl::k_step0_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_TMA));
-#define PPL_ATTR_NI(NI) \
-    PPL_CUDA(cudaFuncSetAttribute(ppl::k_step1_tma<NI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::Step1Cfg<NI>::SMEM));
+    PPL_CUDA(cudaFuncSetAttribute(ppl::k_step0_slab, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_TMA));
+#define PPL_ATTR_NI(NI)                                                                                                                \
+    PPL_CUDA(cudaFuncSetAttribute(ppl::k_step1_tma<NI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::Step1Cfg<NI>::SMEM)); \
+    PPL_CUDA(cudaFuncSetAttribute(ppl::k_step1t_tma<NI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::Step1Cfg<NI>::SMEM));
     PPL_ATTR_NI(5) PPL_ATTR_NI(6) PPL_ATTR_NI(7) PPL_ATTR_NI(8) PPL_ATTR_NI(9) PPL_ATTR_NI(10)
 #undef PPL_ATTR_NI
     g_attr_set = true;
@@ -336,13 +373,15 @@ int launch_step0(const ppl_plan_s *p, const Tile &t, const double *L, const CUte
 // With maps: the persistent TMA kernel with CTA tile (16*ni) x 128; without: the cp.async kernel.
 int launch_step1(const ppl_plan_s *p, const CUtensorMap *mapA, const CUtensorMap *mapB, int ni, const double *A, int64_t lda,
                  const double *B, int64_t ldb, int M, int N, int64_t K, const SplitChoice &sc, double *part, bool vec16,
-                 cudaStream_t s) {
-    if (M <= 0 || N <= 0 || K <= 0) return PPL_OK;
+                 cudaStream_t s, int k0 = 0) {
+    if (M <= 0 || N <= 0 || K - k0 <= 0) return PPL_OK;
+    if (k0 != 0 && !(mapA && mapB)) return fail(PPL_ERR_INVALID_ARG);
     if (mapA && mapB) {
         ppl::Step1TmaArgs a;
         a.M = M;
         a.N = N;
         a.K = (int)K;
+        a.k0 = k0;
         a.k_per_split = sc.k_per_split;
         a.splitk = sc.splitk;
         a.part = part;
@@ -459,6 +498,9 @@ int launch_fold(const ppl_plan_s *p, const double *X, int rows, double *Wp, doub
     a.o = p->o;
     a.v = p->v;
     a.scale = 1.0;
+    a.diag = 1.0;
+    a.tbp = a.bg0 = a.A0 = a.ta = 0;
+    a.cb_min = 0;
     a.dp = Wp;
     a.dm = Wm;
     a.ldp = p->ldp;
@@ -471,7 +513,7 @@ int launch_fold(const ppl_plan_s *p, const double *X, int rows, double *Wp, doub
 }
 
 // t2 (either storage order) -> tau+ [Mp][ldp], tau- [Mm][ldm]
-int launch_pack(const ppl_plan_s *p, const double *t2, int layout, cudaStream_t s) {
+int launch_pack(const ppl_plan_s *p, const double *t2, int layout, double diag, cudaStream_t s) {
     ppl::FoldArgs a;
     a.src = t2;
     const ppl::RStrides ts = r_strides(p->o, p->v, layout);  // t2[i,j,c,d] has the strides of R[i,j,a,b]
@@ -484,6 +526,9 @@ int launch_pack(const ppl_plan_s *p, const double *t2, int layout, cudaStream_t 
     a.o = p->o;
     a.v = p->v;
     a.scale = 0.5;
+    a.diag = diag;
+    a.tbp = a.bg0 = a.A0 = a.ta = 0;
+    a.cb_min = 0;
     a.dp = p->taup;
     a.dm = p->taum;
     a.ldp = p->ldp;
@@ -575,7 +620,7 @@ int run_apply(ppl_plan_s *p, const double *L, const double *t2, double *R, const
     PPL_MARK(-1, 0);
     const double *t2m = t2;
     if (sa) {
-        if ((rc = launch_pack(p, t2, opts.t2_layout, stream)) != PPL_OK) return rc;
+        if ((rc = launch_pack(p, t2, opts.t2_layout, 1.0, stream)) != PPL_OK) return rc;
         PPL_MARK(K_PACK, 1);
     } else if (opts.t2_layout != PPL_LAYOUT_IJAB) {
         if ((rc = t2_matrix(p, t2, opts.t2_layout, stream, &t2m)) != PPL_OK) return rc;
@@ -634,6 +679,316 @@ int run_apply(ppl_plan_s *p, const double *L, const double *t2, double *R, const
     return PPL_OK;
 }
 
+
+// ------------------------------------------------------------------------------------------
+// PPL_SYM_FULL (ppl_kernels_full.cuh): slabs of 16 a's, tiles (A; b-group), chunk table of step 0.
+// ------------------------------------------------------------------------------------------
+int full_geometry(ppl_plan_s *p, int tbg, size_t part_cap, std::vector<int2> *chunks_out) {
+    const int v = p->v, TA = ppl::TA_FULL;
+    p->slabs.clear();
+    p->ftiles.clear();
+    p->ff_step0 = p->ff_step1 = 0;
+    p->fpart_bytes = 0;
+    std::vector<int2> chunks;
+    for (int A0 = 0; A0 < v; A0 += TA) {
+        FullSlab sl;
+        sl.A0 = A0;
+        sl.ta = std::min(TA, v - A0);
+        sl.tiles_m = ((v - A0) + 7) / 8;  // 8 c's x 16 a_l per 128-row CTA tile
+        sl.chunk_off = chunks.size();
+        for (int b = A0; b < v; ++b)
+            for (int d0 = A0 + ((b - A0) & ~15); d0 < v; d0 += 16) chunks.push_back(make_int2(b, d0));
+        while ((chunks.size() - sl.chunk_off) % 8) chunks.push_back(make_int2(-1, 0));
+        sl.tiles_n = (int)((chunks.size() - sl.chunk_off) / 8);
+        sl.flops0 = 2.0 * p->x * (128.0 * sl.tiles_m) * (128.0 * sl.tiles_n);
+        p->ff_step0 += sl.flops0;
+        sl.tile_begin = (int)p->ftiles.size();
+        // b-groups: the 16-blocks of [A0, v) dealt into groups of at most tbg/16 blocks, as evenly as possible
+        const int nblk = (v - A0 + 15) / 16, per = tbg / 16, ng = (nblk + per - 1) / per;
+        int blk = 0;
+        for (int gi = 0; gi < ng; ++gi) {
+            const int cnt = nblk / ng + (gi < nblk % ng ? 1 : 0);
+            FullTile t;
+            t.A0 = A0;
+            t.ta = sl.ta;
+            t.bg0 = A0 + 16 * blk;
+            t.nb = std::min(16 * cnt, v - t.bg0);
+            t.tbp = 16 * cnt;
+            blk += cnt;
+            const int c1 = std::min(A0 + TA, v);
+            // range starts are even (TMA alignment): (A0,A0) sits at an even index, and the element before
+            // (A0, A0+1) in the minus triangle is a hole (A0 even)
+            t.k0p = (int)ppl::kplus(A0, A0, v);
+            t.k0m = A0 + 1 < v ? (int)ppl::kminus(A0, A0 + 1, v) - 1 : p->Km;
+            t.k1p = c1 < v ? (int)ppl::kplus(c1, c1, v) : p->Kp;
+            t.k1m = c1 + 1 < v ? (int)ppl::kminus(c1, c1 + 1, v) - 1 : p->Km;
+            const int N = TA * t.tbp;
+            t.sp = choose_split(p->Mp, N, p->Kp - t.k0p, p->num_sms, p->bm_p, part_cap / 2);
+            t.sm = choose_split(p->Mm, N, p->Km - t.k0m, p->num_sms, p->bm_m, part_cap / 2);
+            p->fpart_bytes = std::max(p->fpart_bytes, ((size_t)t.sp.splitk * p->Mp + (size_t)t.sm.splitk * p->Mm) * N * 8);
+            // executed flops: use 1 (contraction over J >= (A0,A0)) + use 2 (outputs J >= (A0+16,A0+16))
+            const double r0 = v - A0, r1 = v - c1;  // pairs with c >= A0 / c >= A0+16
+            p->ff_step1 += 2.0 * N * ((double)p->Mp * r0 * (r0 + 1) / 2 + (double)p->Mm * r0 * (r0 - 1) / 2);
+            p->ff_step1 += 2.0 * N * ((double)p->Mp * r1 * (r1 + 1) / 2 + (double)p->Mm * std::max(0.0, r1 * (r1 - 1) / 2));
+            p->ftiles.push_back(t);
+        }
+        sl.tile_end = (int)p->ftiles.size();
+        p->slabs.push_back(sl);
+    }
+    if (chunks_out) chunks_out->swap(chunks);
+    return PPL_OK;
+}
+
+// Allocate the PPL_SYM_FULL buffers if they fit into `room` bytes.  Returns PPL_OK and sets full_ok, or leaves it 0.
+int full_setup(ppl_plan_s *p, size_t room) {
+    p->full_ok = 0;
+    if (!p->use_tma || !p->vec16 || !p->sa_ok || p->v < 2) return PPL_OK;
+    const int v = p->v, TA = ppl::TA_FULL;
+    const char *envg = getenv("PPL_TBG");  // debug override of the b-group width
+    int tbg = (envg && atoi(envg) >= 16) ? atoi(envg) / 16 * 16 : 128;
+    tbg = std::min(tbg, (v + 15) / 16 * 16);
+    const size_t x_bytes = align256((size_t)TA * v * p->vv * 8);
+    const size_t racc_bytes = p->tau_bytes;  // same shapes as tau+-
+    std::vector<int2> chunks;
+    for (;; tbg = std::max(16, tbg / 2 / 16 * 16)) {
+        const size_t slot = align256((size_t)TA * tbg * p->ldp * 8) + align256((size_t)TA * tbg * p->ldm * 8);
+        const size_t part_cap = std::max<size_t>((size_t)64 << 20, slot / 8);
+        full_geometry(p, tbg, part_cap, &chunks);
+        const size_t chunk_bytes = align256(chunks.size() * sizeof(int2));
+        const size_t total = x_bytes + slot + align256(p->fpart_bytes) + racc_bytes + chunk_bytes + 256;
+        if (total <= room) {
+            p->tbg = tbg;
+            p->fws_bytes = total;
+            break;
+        }
+        if (tbg == 16) return PPL_OK;  // does not fit: the plan stays without PPL_SYM_FULL
+    }
+    if (cudaMalloc(&p->fws, p->fws_bytes) != cudaSuccess) {
+        (void)cudaGetLastError();
+        p->fws = nullptr;
+        return PPL_OK;
+    }
+    if (cudaMemset(p->fws, 0, p->fws_bytes) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return PPL_OK;
+    }
+    unsigned char *q = p->fws;
+    p->fX = reinterpret_cast<double *>(q);
+    q += x_bytes;
+    p->fWp = reinterpret_cast<double *>(q);
+    q += align256((size_t)TA * p->tbg * p->ldp * 8);
+    p->fWm = reinterpret_cast<double *>(q);
+    q += align256((size_t)TA * p->tbg * p->ldm * 8);
+    p->fpart = reinterpret_cast<double *>(q);
+    q += align256(p->fpart_bytes);
+    p->raccp = reinterpret_cast<double *>(q);
+    p->raccm = reinterpret_cast<double *>(q + align256((size_t)p->Mp * p->ldp * 8));
+    q += racc_bytes;
+    p->fchunks = reinterpret_cast<int2 *>(q);
+    if (cudaMemcpy(p->fchunks, chunks.data(), chunks.size() * sizeof(int2), cudaMemcpyHostToDevice) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return PPL_OK;
+    }
+    const uint64_t rows = (uint64_t)TA * p->tbg;
+    bool m = make_map_2d(&p->mapFWp, p->fWp, (uint64_t)p->Kp, rows, (uint64_t)p->ldp * 8, ppl::BK, ppl::BN) == PPL_OK;
+    m = m && make_map_2d(&p->mapFWpT, p->fWp, (uint64_t)p->Kp, rows, (uint64_t)p->ldp * 8, 16, ppl::BK) == PPL_OK;
+    if (p->Km > 0) {
+        m = m && make_map_2d(&p->mapFWm, p->fWm, (uint64_t)p->Km, rows, (uint64_t)p->ldm * 8, ppl::BK, ppl::BN) == PPL_OK;
+        m = m && make_map_2d(&p->mapFWmT, p->fWm, (uint64_t)p->Km, rows, (uint64_t)p->ldm * 8, 16, ppl::BK) == PPL_OK;
+    }
+    if (!m) return PPL_OK;
+    p->full_ok = 1;
+    return PPL_OK;
+}
+
+int launch_step1t(const ppl_plan_s *p, const CUtensorMap *mapA, const CUtensorMap *mapB, int ni, int M, const FullTile &t,
+                  bool minus, double *acc, int64_t ld, cudaStream_t s) {
+    ppl::Step1TArgs a;
+    a.M = M;
+    a.n_begin = minus ? t.k1m : t.k1p;
+    a.n_end = minus ? p->Km : p->Kp;
+    a.n_base = a.n_begin & ~15;
+    if (M <= 0 || a.n_end - a.n_begin <= 0) return PPL_OK;
+    a.kt_per_a = t.tbp / 16;
+    a.nkt = ppl::TA_FULL * a.kt_per_a;
+    a.A0 = t.A0;
+    a.bg0 = t.bg0;
+    a.v = p->v;
+    a.minus = minus ? 1 : 0;
+    a.acc = acc;
+    a.ld = ld;
+    const int bm = 16 * ni;
+    const int items = ((M + bm - 1) / bm) * ((a.n_end - a.n_base + ppl::BN - 1) / ppl::BN);
+    const int grid = std::min(items, p->num_sms);
+    switch (ni) {
+#define PPL_LAUNCH_NI(NI)                                                                                  \
+    case NI:                                                                                               \
+        ppl::k_step1t_tma<NI><<<grid, ppl::TMA_THREADS, ppl::Step1Cfg<NI>::SMEM, s>>>(*mapA, *mapB, a);  \
+        break;
+        PPL_LAUNCH_NI(5) PPL_LAUNCH_NI(6) PPL_LAUNCH_NI(7) PPL_LAUNCH_NI(8) PPL_LAUNCH_NI(9) PPL_LAUNCH_NI(10)
+#undef PPL_LAUNCH_NI
+        default: return fail(PPL_ERR_INVALID_ARG);
+    }
+    PPL_CUDA(cudaGetLastError());
+    return PPL_OK;
+}
+
+int launch_reduce_acc(const ppl_plan_s *p, const FullTile &t, const double *part, int splitk, int M, bool minus, double *acc,
+                      int64_t ld, cudaStream_t s) {
+    if (M <= 0 || splitk <= 0) return PPL_OK;
+    ppl::ReduceAccArgs a;
+    a.part = part;
+    a.splitk = splitk;
+    a.M = M;
+    a.N = ppl::TA_FULL * t.tbp;
+    a.tbp = t.tbp;
+    a.A0 = t.A0;
+    a.ta = t.ta;
+    a.bg0 = t.bg0;
+    a.v = p->v;
+    a.minus = minus ? 1 : 0;
+    a.acc = acc;
+    a.ld = ld;
+    const int64_t MN = (int64_t)a.M * a.N;
+    const int grid = (int)std::min<int64_t>((MN + 255) / 256, (int64_t)p->num_sms * 8);
+    ppl::k_reduce_acc<<<grid, 256, 0, s>>>(a);
+    PPL_CUDA(cudaGetLastError());
+    return PPL_OK;
+}
+
+// The whole path in PPL_SYM_FULL: everything on the caller's stream (every kernel fills the GPU; the
+// strip is single-buffered), prof as in run_apply.
+int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, const ppl_opts_t *opts_in, cudaStream_t stream,
+                   Prof *prof) {
+    bool vec16 = false;
+    int rc = check_ptrs(p, L, t2, R, &vec16);
+    ppl_opts_t opts;
+    if (rc == PPL_OK) rc = check_opts(opts_in, &opts);
+    if (rc == PPL_OK && (!p->full_ok || !vec16)) rc = PPL_ERR_INVALID_ARG;  // the TMA path needs 16-byte aligned L
+    if (rc != PPL_OK) return fail(rc);
+#define PPL_MARK(k, n)                                                             \
+    do {                                                                           \
+        if (prof && prof->mark(k, n, stream) != PPL_OK) return fail(PPL_ERR_CUDA); \
+    } while (0)
+    PPL_MARK(-1, 0);
+    static const bool dbg = getenv("PPL_DEBUG_SYNC") != nullptr;  // debug: synchronise and report after every launch
+#define PPL_DBG(label, k)                                                                              \
+    do {                                                                                               \
+        if (dbg) {                                                                                     \
+            const cudaError_t e__ = cudaStreamSynchronize(stream);                                     \
+            if (e__ != cudaSuccess) {                                                                  \
+                fprintf(stderr, "libppl: %s (tile/slab %d) failed: %s\n", label, (int)(k), cudaGetErrorString(e__)); \
+                return fail(PPL_ERR_CUDA);                                                             \
+            }                                                                                          \
+        }                                                                                              \
+    } while (0)
+    const bool minus = p->Mm > 0 && p->Km > 0;
+    if ((rc = launch_pack(p, t2, opts.t2_layout, 0.5, stream)) != PPL_OK) return rc;
+    PPL_CUDA(cudaMemsetAsync(p->raccp, 0, (size_t)p->Mp * p->ldp * 8, stream));
+    if (minus) PPL_CUDA(cudaMemsetAsync(p->raccm, 0, (size_t)p->Mm * p->ldm * 8, stream));
+    PPL_MARK(K_PACK, 1);
+    CUtensorMap mapL;
+    if (make_map_2d(&mapL, L, (uint64_t)p->vv, (uint64_t)p->x, (uint64_t)p->vv * 8, 16, ppl::BK) != PPL_OK) return fail(PPL_ERR_CUDA);
+    const int TA = ppl::TA_FULL;
+    for (const FullSlab &sl : p->slabs) {
+        ppl::Step0SlabArgs a0;
+        a0.A0 = sl.A0;
+        a0.ta = sl.ta;
+        a0.v = p->v;
+        a0.K = p->x;
+        a0.tiles_m = sl.tiles_m;
+        a0.tiles_n = sl.tiles_n;
+        a0.chunks = p->fchunks + sl.chunk_off;
+        a0.X = p->fX;
+        const int items = sl.tiles_m * sl.tiles_n;
+        ppl::k_step0_slab<<<std::min(items, p->num_sms), ppl::TMA_THREADS, ppl::SMEM_TMA, stream>>>(mapL, a0);
+        PPL_CUDA(cudaGetLastError());
+        PPL_DBG("k_step0_slab", sl.A0);
+        PPL_MARK(K_STEP0, 1);
+        for (int k = sl.tile_begin; k < sl.tile_end; ++k) {
+            const FullTile &t = p->ftiles[k];
+            const int N = TA * t.tbp;
+            {   // fold: strip rows -> W+- tile
+                ppl::FoldArgs f;
+                f.src = p->fX;
+                f.sc = p->v;
+                f.s_row = p->vv;
+                f.s_i = f.s_j = 0;
+                f.mode = 2;
+                f.rows = N;
+                f.o = p->o;
+                f.v = p->v;
+                f.scale = 1.0;
+                f.diag = 2.0;
+                f.tbp = t.tbp;
+                f.bg0 = t.bg0;
+                f.A0 = t.A0;
+                f.ta = t.ta;
+                f.cb_min = t.A0 / ppl::FT;
+                f.dp = p->fWp;
+                f.dm = p->fWm;
+                f.ldp = p->ldp;
+                f.ldm = p->ldm;
+                const int nb = (p->v + ppl::FT - 1) / ppl::FT - f.cb_min;
+                dim3 grid(nb * (nb + 1) / 2, std::min(N, 8192));
+                ppl::k_symfold<<<grid, 256, 0, stream>>>(f);
+                PPL_CUDA(cudaGetLastError());
+                PPL_DBG("k_symfold", k);
+                PPL_MARK(K_FOLD, 1);
+            }
+            // use 1: R+-acc[.][(a,b)] += tau+-[.][J >= (A0,A0)] W+-[(a,b)][J]^T
+            double *partp = p->fpart, *partm = p->fpart + (size_t)t.sp.splitk * p->Mp * N;
+            rc = launch_step1(p, &p->mapTp, &p->mapFWp, p->ni_p, nullptr, 0, nullptr, 0, p->Mp, N, p->Kp, t.sp, partp, true, stream,
+                              t.k0p);
+            const bool m1 = minus && p->Km - t.k0m > 0;
+            if (rc == PPL_OK && m1)
+                rc = launch_step1(p, &p->mapTm, &p->mapFWm, p->ni_m, nullptr, 0, nullptr, 0, p->Mm, N, p->Km, t.sm, partm, true,
+                                  stream, t.k0m);
+            if (rc != PPL_OK) return rc;
+            PPL_DBG("use 1 (k_step1_tma)", k);
+            PPL_MARK(K_STEP1, m1 ? 2 : 1);
+            rc = launch_reduce_acc(p, t, partp, t.sp.splitk, p->Mp, false, p->raccp, p->ldp, stream);
+            if (rc == PPL_OK && m1) rc = launch_reduce_acc(p, t, partm, t.sm.splitk, p->Mm, true, p->raccm, p->ldm, stream);
+            if (rc != PPL_OK) return rc;
+            PPL_DBG("k_reduce_acc", k);
+            PPL_MARK(K_REDUCE, m1 ? 2 : 1);
+            // use 2: R+-acc[.][J >= (A0+16,A0+16)] += tau+-[.][(a,b) in tile] W+-[(a,b)][J]
+            int n2 = 0;
+            if (p->Kp - t.k1p > 0) {
+                if ((rc = launch_step1t(p, &p->mapTp, &p->mapFWpT, p->ni_p, p->Mp, t, false, p->raccp, p->ldp, stream)) != PPL_OK) return rc;
+                PPL_DBG("use 2 plus (k_step1t_tma)", k);
+                ++n2;
+            }
+            if (minus && p->Km - t.k1m > 0) {
+                if ((rc = launch_step1t(p, &p->mapTm, &p->mapFWmT, p->ni_m, p->Mm, t, true, p->raccm, p->ldm, stream)) != PPL_OK) return rc;
+                PPL_DBG("use 2 minus (k_step1t_tma)", k);
+                ++n2;
+            }
+            if (n2) PPL_MARK(K_STEP1, n2);
+        }
+    }
+    {
+        ppl::UnpackArgs u;
+        u.rp = p->raccp;
+        u.rm = p->raccm;
+        u.ldp = p->ldp;
+        u.ldm = p->ldm;
+        u.o = p->o;
+        u.v = p->v;
+        u.alpha = opts.alpha;
+        u.beta = opts.beta;
+        u.rs = r_strides(p->o, p->v, opts.r_layout);
+        u.R = R;
+        ppl::k_unpack_full<<<p->num_sms * 8, 256, 0, stream>>>(u);
+        PPL_CUDA(cudaGetLastError());
+        PPL_DBG("k_unpack_full", 0);
+        PPL_MARK(K_REDUCE, 1);
+    }
+#undef PPL_MARK
+#undef PPL_DBG
+    return PPL_OK;
+}
+
 }  // namespace
 
 // =============================================================================================
@@ -685,8 +1040,10 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
     p->cap = workspace_bytes;
     p->Mp = nocc * (nocc + 1) / 2;
     p->Mm = nocc * (nocc - 1) / 2;
-    p->Kp = nvirt * (nvirt + 1) / 2;
-    p->Km = nvirt * (nvirt - 1) / 2;
+    p->KpT = nvirt * (nvirt + 1) / 2;
+    p->KmT = nvirt * (nvirt - 1) / 2;
+    p->Kp = (int)ppl::kplus_extent(nvirt);   // extents of the packed index ranges, holes included (ppl_kernels.cuh)
+    p->Km = (int)ppl::kminus_extent(nvirt);
     p->ldp = ((int64_t)p->Kp + 15) / 16 * 16;  // rows of the packed operands are 128-byte aligned: TMA-legal for any nvirt
     p->ldm = ((int64_t)std::max(p->Km, 1) + 15) / 16 * 16;
 
@@ -766,6 +1123,12 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
         fail(PPL_ERR_ALLOC);
         return nullptr;
     }
+    if (cudaMemset(p->ws, 0, p->ws_bytes) != cudaSuccess) {  // the holes of the packed layouts stay zero for good
+        (void)cudaGetLastError();
+        free_plan(p);
+        fail(PPL_ERR_CUDA);
+        return nullptr;
+    }
     {
         unsigned char *q = p->ws;
         p->X = reinterpret_cast<double *>(q);
@@ -824,12 +1187,24 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
         fail(rc);
         return nullptr;
     }
+    // PPL_SYM_FULL: its buffers are allocated when they fit under the cap; it is the default from nvirt = 96 up
+    // (below that the extra launches per slab cost more than the flops they save)
+    full_setup(p, cap > p->ws_bytes ? cap - p->ws_bytes : 0);
+    const char *envf = getenv("PPL_FULL_MIN_V");  // debug override
+    const int full_min_v = envf ? atoi(envf) : 96;
+    if (p->full_ok && nvirt >= full_min_v) p->sym = PPL_SYM_FULL;
     return p;
 }
 
 int ppl_plan_set_symmetry(ppl_plan_t *p, int mode) {
-    if (!p || (mode != PPL_SYM_NONE && mode != PPL_SYM_PAIR && mode != PPL_SYM_PAIR_SA)) return fail(PPL_ERR_INVALID_ARG);
+    if (!p || (mode != PPL_SYM_NONE && mode != PPL_SYM_PAIR && mode != PPL_SYM_PAIR_SA && mode != PPL_SYM_FULL))
+        return fail(PPL_ERR_INVALID_ARG);
     if (mode == PPL_SYM_PAIR_SA && !p->sa_ok) return fail(PPL_ERR_WORKSPACE_TOO_SMALL);
+    if (mode == PPL_SYM_FULL) {
+        if (!p->full_ok) return fail(PPL_ERR_WORKSPACE_TOO_SMALL);
+        p->sym = mode;  // the slab / tile lists were built by ppl_plan
+        return PPL_OK;
+    }
     const int old = p->sym;
     p->sym = mode;
     const int rc = build_tiles(p);
@@ -870,16 +1245,43 @@ int ppl_plan_info(const ppl_plan_t *p, ppl_info_t *out) {
     out->sa_tile_m_minus = p->bm_m;
     out->sa_rows_plus = p->Mp;
     out->sa_rows_minus = p->Mm;
-    out->sa_k_plus = p->Kp;
-    out->sa_k_minus = p->Km;
+    out->sa_k_plus = p->KpT;
+    out->sa_k_minus = p->KmT;
+    out->full_available = p->full_ok;
+    out->full_tbg = p->tbg;
+    out->full_slabs = (int)p->slabs.size();
+    out->full_workspace_bytes = p->fws_bytes;
+    out->workspace_bytes = p->ws_bytes + p->fws_bytes;
+    if (p->sym == PPL_SYM_FULL) {
+        out->ta = ppl::TA_FULL;
+        out->tb = p->tbg;
+        out->n_ablocks = (int)p->slabs.size();
+        out->n_bblocks = p->slabs.empty() ? 0 : p->slabs[0].tile_end - p->slabs[0].tile_begin;
+        out->n_tiles = (int)p->ftiles.size();
+        out->ring = 1;
+        out->splitk = p->ftiles.empty() ? 0 : p->ftiles[0].sp.splitk;
+        int launches = 2 + (int)p->slabs.size();  // pack, unpack, one step 0 per slab
+        for (const FullTile &t : p->ftiles) {
+            const bool m1 = minus && p->Km - t.k0m > 0;
+            launches += 1 + (m1 ? 4 : 2) + (p->Kp - t.k1p > 0 ? 1 : 0) + (minus && p->Km - t.k1m > 0 ? 1 : 0);
+        }
+        out->launches_per_apply = launches;
+        out->step1_tile_m = p->bm_p;
+        out->flops_step0 = p->ff_step0;
+        out->flops_step1 = p->ff_step1;
+        out->flops_executed = p->ff_step0 + p->ff_step1;
+        out->sa_splitk_plus = p->ftiles.empty() ? 0 : p->ftiles[0].sp.splitk;
+        out->sa_splitk_minus = p->ftiles.empty() ? 0 : p->ftiles[0].sm.splitk;
+    }
     return PPL_OK;
 }
 
 int ppl_apply(ppl_plan_t *p, const double *L, const double *t2, double *R, void *stream) {
-    return run_apply(p, L, t2, R, nullptr, reinterpret_cast<cudaStream_t>(stream), nullptr);
+    return ppl_apply_ex(p, L, t2, R, nullptr, stream);
 }
 
 int ppl_apply_ex(ppl_plan_t *p, const double *L, const double *t2, double *R, const ppl_opts_t *opts, void *stream) {
+    if (p && p->sym == PPL_SYM_FULL) return run_apply_full(p, L, t2, R, opts, reinterpret_cast<cudaStream_t>(stream), nullptr);
     return run_apply(p, L, t2, R, opts, reinterpret_cast<cudaStream_t>(stream), nullptr);
 }
 
@@ -888,7 +1290,8 @@ int ppl_apply_profiled(ppl_plan_t *p, const double *L, const double *t2, double 
     cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
     memset(times, 0, sizeof(*times));
     Prof prof;
-    int rc = run_apply(p, L, t2, R, nullptr, stream, &prof);
+    int rc = (p && p->sym == PPL_SYM_FULL) ? run_apply_full(p, L, t2, R, nullptr, stream, &prof)
+                                           : run_apply(p, L, t2, R, nullptr, stream, &prof);
     const cudaError_t e = cudaStreamSynchronize(stream);
     if (rc == PPL_OK && e == cudaSuccess && prof.ev.size() >= 2) {
         float acc[K_KINDS] = {0, 0, 0, 0, 0};
@@ -1003,6 +1406,7 @@ int ppl_check_inputs(ppl_plan_t *p, const double *L, const double *t2, void *str
     PPL_CUDA(cudaStreamSynchronize(stream));
     if (flags) *flags = h;
     if ((h & 2) && p->sym != PPL_SYM_NONE) return fail(PPL_ERR_PRECONDITION);
+    if ((h & 1) && p->sym == PPL_SYM_FULL) return fail(PPL_ERR_PRECONDITION);
     return PPL_OK;
 }
 

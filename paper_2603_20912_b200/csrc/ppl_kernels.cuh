@@ -363,18 +363,39 @@ __global__ void __launch_bounds__(256) k_reduce(const ReduceArgs p) {
 //   R+- = tau+- W+-^T ;  R[i,j,a,b] = R+ + R- ;  R[j,i,a,b] = R+ - R-
 // Both packings are the same gather: k_symfold does either (scale 1 for W, 1/2 for tau).
 // ---------------------------------------------------------------------------------------------
-__host__ __device__ __forceinline__ int64_t kplus(int c, int d, int v) { return (int64_t)c * v - (int64_t)c * (c - 1) / 2 + (d - c); }
-__host__ __device__ __forceinline__ int64_t kminus(int c, int d, int v) { return (int64_t)c * (2 * v - c - 1) / 2 + (d - c - 1); }
+// Packed column index of the pair (c <= d) / (c < d).  Row c of the triangle is placed so that the index of
+// (c,d) has the parity of d (one unused "hole" element every other row; holes are zero in tau+- for good:
+// the buffers are cleared once at plan time and no kernel writes a hole).  This makes every run
+// (c, d0..d0+15) with d0 even start at an even index, i.e. at a 16-byte aligned address: TMA boxes must
+// start 16-byte aligned (an odd FP64 coordinate raises an illegal-instruction error), and PPL_SYM_FULL reads
+// such runs of tau+- as k-tiles.  In the minus triangle the element before (c, c+1), c even, is a hole.
+__host__ __device__ __forceinline__ int64_t kplus(int c, int d, int v) {
+    return (int64_t)c * v - (int64_t)c * (c + 1) / 2 + (c + 1) / 2 + d;
+}
+__host__ __device__ __forceinline__ int64_t kminus(int c, int d, int v) {
+    return (int64_t)c * (2 * v - c - 1) / 2 - c + c / 2 + d;
+}
+__host__ __device__ __forceinline__ int64_t kplus_extent(int v) { return kplus(v - 1, v - 1, v) + 1; }
+__host__ __device__ __forceinline__ int64_t kminus_extent(int v) { return v >= 2 ? kminus(v - 2, v - 1, v) + 1 : 0; }
+// packed row index of the occupied pair (i <= j) / (i < j): dense, no holes
+__host__ __device__ __forceinline__ int64_t rowplus(int i, int j, int o) { return (int64_t)i * o - (int64_t)i * (i - 1) / 2 + (j - i); }
+__host__ __device__ __forceinline__ int64_t rowminus(int i, int j, int o) { return (int64_t)i * (2 * o - i - 1) / 2 + (j - i - 1); }
 
 struct FoldArgs {
     const double *src;   // row r, element (c,d) at src + roff(r) + c*sc + d   (d contiguous)
     int64_t sc;          // stride of c
-    int64_t s_row;       // mode 0: row r at r*s_row
+    int64_t s_row;       // mode 0: row r at r*s_row;  mode 2: row (a_l, b) at (a_l*v + b)*s_row
     int64_t s_i, s_j;    // mode 1: row (i,j) at i*s_i + j*s_j
-    int mode;            // 0: fold W tile rows (every row has + and -); 1: pack amplitudes, rows (i<=j) of an o x o grid
-    int rows;            // mode 0: number of rows; mode 1: o*o (rows with i > j are skipped)
+    int mode;            // 0: fold W tile rows (every row has + and -); 1: pack amplitudes, rows (i<=j) of an o x o grid;
+                         // 2: PPL_SYM_FULL: rows r = a_l*tbp + b_l of the tile (A; b-group) taken from the slab's strip;
+                         //    rows with a > b, b >= v or a_l >= ta are written as zeros; only c >= A0 is touched
+    int rows;            // mode 0/2: number of rows; mode 1: o*o (rows with i > j are skipped)
     int o, v;
     double scale;        // factor of the off-diagonal (c<d) entries: 1 (W) or 1/2 (tau)
+    double diag;         // factor of the diagonal (c==d) entries of the + part: PPL_SYM_PAIR_SA 1 (W), 1 (tau);
+                         // PPL_SYM_FULL 2 (W), 1/2 (tau) -- same products, but W+ becomes a symmetric matrix
+    int tbp, bg0, A0, ta;  // mode 2
+    int cb_min;          // first FT-block of c that is processed (mode 2: A0 / FT; else 0)
     double *dp, *dm;     // packed outputs, row strides ldp / ldm
     int64_t ldp, ldm;
 };
@@ -384,19 +405,27 @@ constexpr int FT = 32;  // (c,d) block edge of the fold
 __global__ void __launch_bounds__(256) k_symfold(const FoldArgs p) {
     __shared__ double sa[FT][FT + 1], sb[FT][FT + 1];
     const int nbv = (p.v + FT - 1) / FT;
-    // blockIdx.x -> block pair (cb <= db); blockIdx.y strides over rows
-    int cb = 0, rem = blockIdx.x;
+    // blockIdx.x -> block pair (cb <= db) among the blocks cb_min..nbv-1; blockIdx.y strides over rows
+    int cb = p.cb_min, rem = blockIdx.x;
     while (rem >= nbv - cb) {
         rem -= nbv - cb;
         ++cb;
     }
     const int db = cb + rem;
     const int c0 = cb * FT, d0 = db * FT;
+    const int cmin = p.mode == 2 ? p.A0 : 0;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;  // 32 x 8
     for (int r = blockIdx.y; r < p.rows; r += gridDim.y) {
         int64_t roff, rowp, rowm;
+        bool zero = false;
         if (p.mode == 0) {
             roff = (int64_t)r * p.s_row;
+            rowp = rowm = r;
+        } else if (p.mode == 2) {
+            const int al = r / p.tbp, bl = r - al * p.tbp;
+            const int a = p.A0 + al, b = p.bg0 + bl;
+            zero = al >= p.ta || b >= p.v || a > b;
+            roff = zero ? 0 : ((int64_t)al * p.v + b) * p.s_row;
             rowp = rowm = r;
         } else {
             const int i = r / p.o, j = r - i * p.o;
@@ -410,10 +439,10 @@ __global__ void __launch_bounds__(256) k_symfold(const FoldArgs p) {
 #pragma unroll
         for (int y = ty; y < FT; y += 8) {
             const int c = c0 + y, d = d0 + tx;
-            sa[y][tx] = (c < p.v && d < p.v) ? s[(int64_t)c * p.sc + d] : 0.0;
+            sa[y][tx] = (!zero && c < p.v && d < p.v && c >= cmin) ? s[(int64_t)c * p.sc + d] : 0.0;
             if (cb != db) {
                 const int c2 = d0 + y, d2 = c0 + tx;  // the transposed block: element (c2,d2), c2 in db, d2 in cb
-                sb[y][tx] = (c2 < p.v && d2 < p.v) ? s[(int64_t)c2 * p.sc + d2] : 0.0;
+                sb[y][tx] = (!zero && c2 < p.v && d2 < p.v && d2 >= cmin) ? s[(int64_t)c2 * p.sc + d2] : 0.0;
             }
         }
         __syncthreads();
@@ -422,10 +451,10 @@ __global__ void __launch_bounds__(256) k_symfold(const FoldArgs p) {
 #pragma unroll
         for (int y = ty; y < FT; y += 8) {
             const int c = c0 + y, d = d0 + tx;
-            if (c >= p.v || d >= p.v || d < c) continue;
+            if (c >= p.v || d >= p.v || d < c || c < cmin) continue;
             const double xcd = sa[y][tx];
             if (c == d) {
-                op[kplus(c, d, p.v)] = xcd;
+                op[kplus(c, d, p.v)] = p.diag * xcd;
             } else {
                 const double xdc = (cb != db) ? sb[tx][y] : sa[tx][y];
                 op[kplus(c, d, p.v)] = p.scale * (xcd + xdc);

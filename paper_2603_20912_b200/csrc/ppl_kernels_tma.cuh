@@ -254,7 +254,8 @@ __global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_tma(const __grid_const
 // picks NI in 5..10 that tiles nocc^2 with the least padding (160 | 1600, 144 | 3600, 80 | 400).
 // ---------------------------------------------------------------------------------------------
 struct Step1TmaArgs {
-    int M, N, K;      // nocc^2, ta*tb, nvirt^2
+    int M, N, K;      // nocc^2, ta*tb, nvirt^2 (K = END of the contraction range)
+    int k0;           // first k of the contraction range (0 except in PPL_SYM_FULL; any value: TMA boxes may start anywhere)
     int k_per_split;  // multiple of BK
     int splitk;
     double *part;     // [splitk][M][N]
@@ -300,7 +301,7 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
             for (int item = blockIdx.x; item < num_items; item += gridDim.x) {
                 const int z = item / tiles_mn, r = item - z * tiles_mn;
                 const int tm = r % tiles_m, tn = r / tiles_m;
-                const int kbeg = z * p.k_per_split, kend = min(p.K, kbeg + p.k_per_split);
+                const int kbeg = p.k0 + z * p.k_per_split, kend = min(p.K, kbeg + p.k_per_split);
                 for (int k = kbeg; k < kend; k += BK) {
                     mbar_wait(&sm.empty[stage], phase ^ 1);
                     mbar_expect_tx(&sm.full[stage], Cfg::STAGE);
@@ -328,7 +329,7 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
         const int z = item / tiles_mn, r = item - z * tiles_mn;
         const int tm = r % tiles_m, tn = r / tiles_m;
         const int m0 = tm * BM1, n0 = tn * BN;
-        const int kbeg = z * p.k_per_split, kend = min(p.K, kbeg + p.k_per_split);
+        const int kbeg = p.k0 + z * p.k_per_split, kend = min(p.K, kbeg + p.k_per_split);
         double acc[NI][4][2];
 #pragma unroll
         for (int i = 0; i < NI; ++i)

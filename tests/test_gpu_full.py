@@ -1,0 +1,150 @@
+"""-m gpu: PPL_SYM_FULL (full 8-fold ERI symmetry: slabs of 16 a's, symmetric S+- used twice, step 0
+restricted to d-block >= b-block; include/ppl.h) against the CPU oracle.  The mode needs symmetric L,
+pair-symmetric t2 and even nvirt.  Same tolerance as everywhere (1e-11 relative, exact integers bit
+for bit).  The identity behind it is pinned on the CPU (test_oracle_pins.py::test_full_symmetry_hook_identity)."""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_2603_20912_b200 as P
+import ppl_inputs as I
+from gpu_util import gpu_ladder, relerr
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-11
+
+# even nvirt; one slab (v <= 16), several slabs, ragged last slab (v % 16 != 0), nocc^2 > 128, one/two-element edges
+SHAPES = [(1, 2, 1), (2, 16, 4), (12, 18, 9), (3, 24, 17), (5, 20, 60), (3, 40, 33), (13, 22, 40), (6, 50, 70),
+          (4, 66, 30), (9, 100, 24), (24, 64, 128), (2, 130, 20)]
+
+
+@pytest.fixture
+def tbg_env():
+    old = os.environ.get("PPL_TBG")
+    yield lambda val: os.environ.__setitem__("PPL_TBG", str(val))
+    if old is None:
+        os.environ.pop("PPL_TBG", None)
+    else:
+        os.environ["PPL_TBG"] = old
+
+
+@pytest.mark.parametrize("shape", SHAPES)
+@pytest.mark.parametrize("tbg", [128, 32, 16])
+def test_full_mode_parity(shape, tbg, tbg_env):
+    o, v, x = shape
+    tbg_env(tbg)
+    L = I.make_L(v, x, seed=21, symmetric=True)
+    t2 = I.make_t2(o, v, seed=21, symmetric=True)
+    want = oracle.full(L, t2)
+    got, info = gpu_ladder(L, t2, sym=P.PPL_SYM_FULL, return_info=True)
+    assert info["symmetry"] == P.PPL_SYM_FULL and info["full_available"] == 1
+    assert info["full_tbg"] == min(tbg, (v + 15) // 16 * 16)
+    assert relerr(got, want) <= TOL, info
+
+
+@pytest.mark.parametrize("shape", [(5, 20, 60), (4, 38, 19), (12, 18, 9), (24, 64, 128), (7, 82, 33)])
+@pytest.mark.parametrize("tbg", [128, 16])
+def test_full_mode_exact_integers_bit_for_bit(shape, tbg, tbg_env):
+    o, v, x = shape
+    tbg_env(tbg)
+    L = I.make_L(v, x, 41, symmetric=True, integer=True)
+    t2 = 2.0 * I.make_t2(o, v, 41, symmetric=True, integer=True)  # tau+- (and t2[cc]/2) stay exact integers
+    want = oracle.full(L, t2)
+    for rep in range(3):
+        got = gpu_ladder(L, t2, sym=P.PPL_SYM_FULL)
+        assert np.array_equal(got, want), rep
+
+
+def test_full_mode_accumulates_and_handles_layouts_alpha_beta():
+    import torch
+
+    o, v, x = 4, 36, 19
+    L = I.make_L(v, x, 11, symmetric=True)
+    t2 = I.make_t2(o, v, 11, symmetric=True)
+    R0 = I.make_t2(o, v, 12, symmetric=False)
+    got = gpu_ladder(L, t2, R0=R0.copy(), sym=P.PPL_SYM_FULL)
+    assert relerr(got, oracle.full(L, t2, R0.copy())) <= TOL
+    for t2_layout, r_layout in (("iajb", "iajb"), ("ijab", "iajb"), ("iajb", "ijab")):
+        to = lambda a, lay: np.ascontiguousarray(a if lay == "ijab" else a.transpose(0, 2, 1, 3))
+        alpha, beta = -0.75, 0.5
+        want = oracle.full_ex(L, to(t2, t2_layout), to(R0, r_layout).copy(), t2_layout, r_layout, alpha, beta)
+        Ld, td, Rd = torch.from_numpy(L).cuda(), torch.from_numpy(to(t2, t2_layout)).cuda(), torch.from_numpy(to(R0, r_layout)).cuda()
+        with P.Plan(o, v, x) as plan:
+            plan.set_symmetry(P.PPL_SYM_FULL)
+            plan.apply_ex(Ld, td, Rd, t2_layout=t2_layout, r_layout=r_layout, alpha=alpha, beta=beta)
+            torch.cuda.synchronize()
+        assert relerr(Rd.cpu().numpy(), want) <= TOL, (t2_layout, r_layout)
+    # beta == 0 overwrites without reading R (NaN on entry must not leak)
+    Rn = torch.full((o, o, v, v), float("nan"), dtype=torch.float64, device="cuda")
+    with P.Plan(o, v, x) as plan:
+        plan.set_symmetry(P.PPL_SYM_FULL)
+        plan.apply_ex(torch.from_numpy(L).cuda(), torch.from_numpy(t2).cuda(), Rn, alpha=1.0, beta=0.0)
+        torch.cuda.synchronize()
+    assert relerr(Rn.cpu().numpy(), oracle.full(L, t2)) <= TOL
+
+
+def test_full_mode_preconditions_default_and_availability():
+    import torch
+
+    # default: PPL_SYM_FULL from nvirt = 96 up (even nvirt), PPL_SYM_PAIR_SA below; odd nvirt has no PPL_SYM_FULL
+    with P.Plan(3, 96, 8) as plan:
+        assert plan.info()["symmetry"] == P.PPL_SYM_FULL
+    with P.Plan(3, 40, 8) as plan:
+        info = plan.info()
+        assert info["symmetry"] == P.PPL_SYM_PAIR_SA and info["full_available"] == 1
+    with P.Plan(3, 97, 8) as plan:
+        info = plan.info()
+        assert info["symmetry"] == P.PPL_SYM_PAIR_SA and info["full_available"] == 0
+        with pytest.raises(P.PplError) as e:
+            plan.set_symmetry(P.PPL_SYM_FULL)
+        assert e.value.code == P.PPL_ERR_WORKSPACE_TOO_SMALL
+    # a cap that holds the PPL_SYM_PAIR_SA plan but not the 16 x nvirt^3 strip: the plan falls back
+    o, v, x = 3, 96, 8
+    with P.Plan(o, v, x, 40 << 20) as plan:
+        info = plan.info()
+        assert info["full_available"] == 0 and info["symmetry"] == P.PPL_SYM_PAIR_SA and info["workspace_bytes"] <= 40 << 20
+    # ppl_check_inputs: a non-symmetric L violates the precondition of PPL_SYM_FULL only
+    Ln = torch.from_numpy(I.make_L(v, x, 3, symmetric=False)).cuda()
+    Ls = torch.from_numpy(I.make_L(v, x, 3, symmetric=True)).cuda()
+    t2 = torch.from_numpy(I.make_t2(o, v, 3, symmetric=True)).cuda()
+    with P.Plan(o, v, x) as plan:
+        assert plan.check_inputs(Ls, t2) == 0
+        with pytest.raises(P.PplError) as e:
+            plan.check_inputs(Ln, t2)
+        assert e.value.code == P.PPL_ERR_PRECONDITION
+        plan.set_symmetry(P.PPL_SYM_PAIR_SA)
+        assert plan.check_inputs(Ln, t2) == 1  # reported, not required
+
+
+def test_full_mode_flop_accounting():
+    """Executed flops: step 0 about 1/8 and step 1 about 1/4 of nominal (plus block-edge overheads)."""
+    o, v, x = 20, 200, 800
+    with P.Plan(o, v, x) as plan:
+        info = plan.info()
+    assert info["symmetry"] == P.PPL_SYM_FULL
+    nom0, nom1 = 2.0 * x * v**4, 2.0 * o * o * v**4
+    # the 16-blocks on the diagonals (d-block == b-block, c-block == a-block) are computed whole: + O(16/nvirt)
+    assert 0.125 <= info["flops_step0"] / nom0 <= 0.19, info
+    assert 0.25 <= info["flops_step1"] / nom1 <= 0.32, info
+
+
+def test_full_mode_repeated_apply_and_stream_ordering():
+    import torch
+
+    o, v, x = 6, 48, 20
+    L = I.make_L(v, x, 5, symmetric=True, integer=True)
+    t2 = 2.0 * I.make_t2(o, v, 5, symmetric=True, integer=True)
+    want = oracle.full(L, t2)
+    Ld, td = torch.from_numpy(L).cuda(), torch.from_numpy(t2).cuda()
+    Rd = torch.zeros((o, o, v, v), dtype=torch.float64, device="cuda")
+    s = torch.cuda.Stream()
+    with P.Plan(o, v, x) as plan:
+        plan.set_symmetry(P.PPL_SYM_FULL)
+        with torch.cuda.stream(s):
+            for _ in range(3):
+                plan.apply(Ld, td, Rd, s)
+            Rd.mul_(0.5)  # ordered after the applies on the same stream
+        s.synchronize()
+    assert np.array_equal(Rd.cpu().numpy(), 1.5 * want)

@@ -35,7 +35,7 @@ def _host_gb():
 
 
 def _run(name, integer=False, sym=None):
-    """sym=None: the plan's default, which is what bench.py times (PPL_SYM_PAIR_SA)."""
+    """sym=None: the plan's default, which is what bench.py times (PPL_SYM_FULL from nvirt = 96 up)."""
     import torch
 
     o, v, x = I.CONFIGS[name]
@@ -50,7 +50,7 @@ def _run(name, integer=False, sym=None):
         if sym is not None:
             plan.set_symmetry(sym)
         info = plan.info()
-        assert info["symmetry"] == (P.PPL_SYM_PAIR_SA if sym is None else sym)
+        assert info["symmetry"] == (P.PPL_SYM_FULL if sym is None else sym)
         assert plan.check_inputs(Ld, td) == 0
         plan.apply(Ld, td, Rd)
         torch.cuda.synchronize()
@@ -97,7 +97,7 @@ def _check_projections(L, t2, Rd, rmax, nrand=2):
         assert np.abs(got - want).max() <= bound, (np.abs(got - want).max(), bound)
 
 
-@pytest.mark.parametrize("sym", [None, P.PPL_SYM_PAIR])
+@pytest.mark.parametrize("sym", [None, P.PPL_SYM_PAIR_SA, P.PPL_SYM_PAIR])
 def test_medium_sampled_columns_and_projections(sym):
     L, t2, Rd, info = _run("medium", sym=sym)
     assert info["n_tiles"] > 1
@@ -111,7 +111,7 @@ def test_medium_sampled_columns_and_projections(sym):
         assert np.abs(Rd.cpu().numpy() - want).max() <= TOL * np.abs(want).max()
 
 
-@pytest.mark.parametrize("sym", [None, P.PPL_SYM_PAIR])
+@pytest.mark.parametrize("sym", [None, P.PPL_SYM_PAIR_SA, P.PPL_SYM_PAIR])
 def test_medium_exact_integers_sampled(sym):
     L, t2, Rd, _ = _run("medium", integer=True, sym=sym)
     _check_columns(L, t2, Rd, 128, exact=True)
@@ -145,7 +145,7 @@ def test_medium_closed_form_tagged_tiles_repeated():
             assert int((R != want).sum().item()) == 0
 
 
-@pytest.mark.parametrize("sym", [None, P.PPL_SYM_PAIR])
+@pytest.mark.parametrize("sym", [None, P.PPL_SYM_PAIR_SA, P.PPL_SYM_PAIR])
 def test_large_sampled_columns_and_projections(sym):
     if _host_gb() < 16:
         pytest.skip("not enough host memory for the large config")

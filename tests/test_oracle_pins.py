@@ -350,3 +350,81 @@ def test_symmetric_antisymmetric_packing_identity(shape):
                 if i != j:
                     gotn[j, i] = Rpn[i, j] - Rmn[i, j]
         assert rel(gotn, wantn) > 1e-3
+
+
+# ------------------------------------------------ full 8-fold symmetry: the "hook" decomposition of PPL_SYM_FULL
+def _kp(c, d, v):
+    return c * v - c * (c - 1) // 2 + (d - c)
+
+
+def _km(c, d, v):
+    return c * (2 * v - c - 1) // 2 + (d - c - 1)
+
+
+def _full_symmetry_emulation(L, t2, T):
+    """The data flow of the CUDA path's PPL_SYM_FULL mode (include/ppl.h), step by step in numpy:
+    a-blocks of T; for slab A only integrals with all four indices >= A0 are formed; the packed
+    S+-[(a<=b)][(c<=d)] = (ac|bd) +- (ad|bc) rows of the slab are used once as rows (contraction over
+    (c,d) with c >= A0) and once as columns (outputs (c,d) with c >= A0+T)."""
+    x, v, _ = L.shape
+    o = t2.shape[0]
+    Kp, Km, Mp, Mm = v * (v + 1) // 2, v * (v - 1) // 2, o * (o + 1) // 2, o * (o - 1) // 2
+    taup, taum = np.zeros((Mp, Kp)), np.zeros((max(Mm, 1), max(Km, 1)))
+    for i in range(o):
+        for j in range(i, o):
+            for c in range(v):
+                taup[_kp(i, j, o), _kp(c, c, v)] = 0.5 * t2[i, j, c, c]
+                for d in range(c + 1, v):
+                    taup[_kp(i, j, o), _kp(c, d, v)] = 0.5 * (t2[i, j, c, d] + t2[i, j, d, c])
+                    if i < j:
+                        taum[_km(i, j, o), _km(c, d, v)] = 0.5 * (t2[i, j, c, d] - t2[i, j, d, c])
+    Rp, Rm = np.zeros((Mp, Kp)), np.zeros((max(Mm, 1), max(Km, 1)))
+    for A0 in range(0, v, T):
+        ta = min(T, v - A0)
+        c1 = A0 + ta
+        X = np.einsum("Pac,Pbd->abcd", L[:, A0:c1, A0:], L[:, A0:, A0:])  # (ac|bd), b, c, d >= A0 only
+        k0p, k1p = _kp(A0, A0, v), _kp(c1, c1, v)
+        k0m, k1m = A0 * (2 * v - A0 - 1) // 2, c1 * (2 * v - c1 - 1) // 2
+        for al in range(ta):
+            a = A0 + al
+            for b in range(a, v):
+                Xab = X[al, b - A0]
+                wp, wm = np.zeros(Kp), np.zeros(max(Km, 1))
+                for c in range(A0, v):
+                    for d in range(c, v):
+                        wp[_kp(c, d, v)] = Xab[c - A0, d - A0] + Xab[d - A0, c - A0]
+                        if c < d:
+                            wm[_km(c, d, v)] = Xab[c - A0, d - A0] - Xab[d - A0, c - A0]
+                Rp[:, _kp(a, b, v)] += taup[:, k0p:] @ wp[k0p:]             # use 1
+                Rp[:, k1p:] += np.outer(taup[:, _kp(a, b, v)], wp[k1p:])    # use 2
+                if a < b and Mm > 0:
+                    Rm[:, _km(a, b, v)] += taum[:, k0m:Km] @ wm[k0m:Km]
+                    Rm[:, k1m:Km] += np.outer(taum[:, _km(a, b, v)], wm[k1m:Km])
+    R = np.zeros_like(t2)
+    for i in range(o):
+        for j in range(i, o):
+            for a in range(v):
+                for b in range(a, v):
+                    rp = Rp[_kp(i, j, o), _kp(a, b, v)]
+                    rm = Rm[_km(i, j, o), _km(a, b, v)] if (i < j and a < b) else 0.0
+                    R[i, j, a, b] = R[j, i, b, a] = rp + rm
+                    R[j, i, a, b] = R[i, j, b, a] = rp - rm
+    return R
+
+
+@pytest.mark.parametrize("shape,T", [((3, 7, 5), 3), ((2, 5, 4), 2), ((4, 9, 6), 4), ((1, 4, 3), 2), ((3, 6, 2), 6), ((2, 1, 3), 1)])
+def test_full_symmetry_hook_identity(shape, T):
+    """With L[P,a,c] = L[P,c,a] AND pair-symmetric t2 the whole term follows from the integrals
+    (ac|bd) with a in block A and b, c, d >= A0 alone (1/8 of the v^4 tensor), because
+    S+-[(ab)][(cd)] = (ac|bd) +- (ad|bc) is symmetric in its two pair indices.  Pinned against the oracle;
+    negative controls: a non-symmetric L, or a non-pair-symmetric t2, breaks it."""
+    o, v, x = shape
+    L = I.make_L(v, x, 13, symmetric=True)
+    t = I.make_t2(o, v, 13, symmetric=True)
+    assert rel(_full_symmetry_emulation(L, t, T), oracle.full(L, t)) <= RTOL
+    if v > 2 and T < v:
+        Ln = I.make_L(v, x, 13, symmetric=False)
+        assert rel(_full_symmetry_emulation(Ln, t, T), oracle.full(Ln, t)) > 1e-3
+    if o > 1 and v > 1:
+        tn = I.make_t2(o, v, 13, symmetric=False)
+        assert rel(_full_symmetry_emulation(L, tn, T), oracle.full(L, tn)) > 1e-3
