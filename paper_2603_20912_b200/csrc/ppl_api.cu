@@ -506,7 +506,7 @@ int launch_fold(const ppl_plan_s *p, const double *X, int rows, double *Wp, doub
     a.ldp = p->ldp;
     a.ldm = p->ldm;
     const int nbv = (p->v + ppl::FT - 1) / ppl::FT;
-    dim3 grid(nbv * (nbv + 1) / 2, std::min(rows, 8192));
+    dim3 grid(nbv * (nbv + 1) / 2, ppl::fold_grid_y(nbv * (nbv + 1) / 2, rows, p->num_sms));
     ppl::k_symfold<<<grid, 256, 0, s>>>(a);
     PPL_CUDA(cudaGetLastError());
     return PPL_OK;
@@ -534,7 +534,7 @@ int launch_pack(const ppl_plan_s *p, const double *t2, int layout, double diag, 
     a.ldp = p->ldp;
     a.ldm = p->ldm;
     const int nbv = (p->v + ppl::FT - 1) / ppl::FT;
-    dim3 grid(nbv * (nbv + 1) / 2, std::min(a.rows, 8192));
+    dim3 grid(nbv * (nbv + 1) / 2, ppl::fold_grid_y(nbv * (nbv + 1) / 2, a.rows, p->num_sms));
     ppl::k_symfold<<<grid, 256, 0, s>>>(a);
     PPL_CUDA(cudaGetLastError());
     return PPL_OK;
@@ -745,7 +745,7 @@ int full_setup(ppl_plan_s *p, size_t room) {
     if (!p->use_tma || !p->vec16 || !p->sa_ok || p->v < 2) return PPL_OK;
     const int v = p->v, TA = ppl::TA_FULL;
     const char *envg = getenv("PPL_TBG");  // debug override of the b-group width
-    int tbg = (envg && atoi(envg) >= 16) ? atoi(envg) / 16 * 16 : 128;
+    int tbg = (envg && atoi(envg) >= 16) ? atoi(envg) / 16 * 16 : 256;
     tbg = std::min(tbg, (v + 15) / 16 * 16);
     const size_t x_bytes = align256((size_t)TA * v * p->vv * 8);
     const size_t racc_bytes = p->tau_bytes;  // same shapes as tau+-
@@ -930,7 +930,7 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
                 f.ldp = p->ldp;
                 f.ldm = p->ldm;
                 const int nb = (p->v + ppl::FT - 1) / ppl::FT - f.cb_min;
-                dim3 grid(nb * (nb + 1) / 2, std::min(N, 8192));
+                dim3 grid(nb * (nb + 1) / 2, ppl::fold_grid_y(nb * (nb + 1) / 2, N, p->num_sms));
                 ppl::k_symfold<<<grid, 256, 0, stream>>>(f);
                 PPL_CUDA(cudaGetLastError());
                 PPL_DBG("k_symfold", k);

@@ -402,7 +402,39 @@ struct FoldArgs {
 
 constexpr int FT = 32;  // (c,d) block edge of the fold
 
-__global__ void __launch_bounds__(256) k_symfold(const FoldArgs p) {
+// Row bookkeeping of k_symfold: where row r of the launch reads from and which packed rows it writes.
+struct FoldRow {
+    int64_t roff, rowp, rowm;
+    bool zero;  // write zeros (PPL_SYM_FULL rows with a > b or beyond the ragged edge)
+    bool skip;  // nothing to do (amplitude rows with i > j)
+};
+
+__device__ __forceinline__ FoldRow fold_row(const FoldArgs &p, int r) {
+    FoldRow f;
+    f.zero = f.skip = false;
+    if (p.mode == 0) {
+        f.roff = (int64_t)r * p.s_row;
+        f.rowp = f.rowm = r;
+    } else if (p.mode == 2) {
+        const int al = r / p.tbp, bl = r - al * p.tbp;
+        const int a = p.A0 + al, b = p.bg0 + bl;
+        f.zero = al >= p.ta || b >= p.v || a > b;
+        f.roff = f.zero ? 0 : ((int64_t)al * p.v + b) * p.s_row;
+        f.rowp = f.rowm = r;
+    } else {
+        const int i = r / p.o, j = r - i * p.o;
+        f.skip = i > j;
+        f.roff = i * p.s_i + j * p.s_j;
+        f.rowp = (int64_t)i * p.o - (int64_t)i * (i - 1) / 2 + (j - i);
+        f.rowm = (i < j) ? (int64_t)i * (2 * p.o - i - 1) / 2 + (j - i - 1) : -1;
+    }
+    return f;
+}
+
+// One CTA owns one (c-block <= d-block) pair of 32 x 32 blocks and strides over the rows; the two source
+// blocks of the NEXT row are fetched into registers while the current row goes through shared memory
+// (transpose) and out, so that every thread keeps 8 global loads in flight across the barriers.
+__global__ void __launch_bounds__(256, 4) k_symfold(const FoldArgs p) {
     __shared__ double sa[FT][FT + 1], sb[FT][FT + 1];
     const int nbv = (p.v + FT - 1) / FT;
     // blockIdx.x -> block pair (cb <= db) among the blocks cb_min..nbv-1; blockIdx.y strides over rows
@@ -415,53 +447,66 @@ __global__ void __launch_bounds__(256) k_symfold(const FoldArgs p) {
     const int c0 = cb * FT, d0 = db * FT;
     const int cmin = p.mode == 2 ? p.A0 : 0;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;  // 32 x 8
-    for (int r = blockIdx.y; r < p.rows; r += gridDim.y) {
-        int64_t roff, rowp, rowm;
-        bool zero = false;
-        if (p.mode == 0) {
-            roff = (int64_t)r * p.s_row;
-            rowp = rowm = r;
-        } else if (p.mode == 2) {
-            const int al = r / p.tbp, bl = r - al * p.tbp;
-            const int a = p.A0 + al, b = p.bg0 + bl;
-            zero = al >= p.ta || b >= p.v || a > b;
-            roff = zero ? 0 : ((int64_t)al * p.v + b) * p.s_row;
-            rowp = rowm = r;
-        } else {
-            const int i = r / p.o, j = r - i * p.o;
-            if (i > j) continue;
-            roff = i * p.s_i + j * p.s_j;
-            rowp = (int64_t)i * p.o - (int64_t)i * (i - 1) / 2 + (j - i);
-            rowm = (i < j) ? (int64_t)i * (2 * p.o - i - 1) / 2 + (j - i - 1) : -1;
+    const bool offdiag = cb != db;
+    double va[FT / 8], vb[FT / 8];
+    auto fetch = [&](const FoldRow &f) {
+        const double *s = p.src + f.roff;
+        const bool live = !f.zero && !f.skip;
+#pragma unroll
+        for (int k = 0; k < FT / 8; ++k) {
+            const int y = ty + 8 * k;
+            const int c = c0 + y, d = d0 + tx;
+            va[k] = (live && c < p.v && d < p.v && c >= cmin) ? __ldg(s + (int64_t)c * p.sc + d) : 0.0;
+            const int c2 = d0 + y, d2 = c0 + tx;  // the transposed block: element (c2,d2), c2 in db, d2 in cb
+            vb[k] = (live && offdiag && c2 < p.v && d2 < p.v && d2 >= cmin) ? __ldg(s + (int64_t)c2 * p.sc + d2) : 0.0;
         }
-        const double *s = p.src + roff;
+    };
+    int r = blockIdx.y;
+    if (r >= p.rows) return;
+    FoldRow cur = fold_row(p, r);
+    fetch(cur);
+    for (; r < p.rows; r += gridDim.y) {
         __syncthreads();  // previous row's reads of sa/sb are done
 #pragma unroll
-        for (int y = ty; y < FT; y += 8) {
-            const int c = c0 + y, d = d0 + tx;
-            sa[y][tx] = (!zero && c < p.v && d < p.v && c >= cmin) ? s[(int64_t)c * p.sc + d] : 0.0;
-            if (cb != db) {
-                const int c2 = d0 + y, d2 = c0 + tx;  // the transposed block: element (c2,d2), c2 in db, d2 in cb
-                sb[y][tx] = (!zero && c2 < p.v && d2 < p.v && d2 >= cmin) ? s[(int64_t)c2 * p.sc + d2] : 0.0;
-            }
+        for (int k = 0; k < FT / 8; ++k) {
+            sa[ty + 8 * k][tx] = va[k];
+            if (offdiag) sb[ty + 8 * k][tx] = vb[k];
+        }
+        const FoldRow now = cur;
+        const int rn = r + gridDim.y;
+        if (rn < p.rows) {
+            cur = fold_row(p, rn);
+            fetch(cur);
         }
         __syncthreads();
-        double *op = p.dp + rowp * p.ldp;
-        double *om = rowm >= 0 ? p.dm + rowm * p.ldm : nullptr;
+        if (now.skip) continue;
+        double *op = p.dp + now.rowp * p.ldp;
+        double *om = now.rowm >= 0 ? p.dm + now.rowm * p.ldm : nullptr;
 #pragma unroll
-        for (int y = ty; y < FT; y += 8) {
+        for (int k = 0; k < FT / 8; ++k) {
+            const int y = ty + 8 * k;
             const int c = c0 + y, d = d0 + tx;
             if (c >= p.v || d >= p.v || d < c || c < cmin) continue;
             const double xcd = sa[y][tx];
             if (c == d) {
                 op[kplus(c, d, p.v)] = p.diag * xcd;
             } else {
-                const double xdc = (cb != db) ? sb[tx][y] : sa[tx][y];
+                const double xdc = offdiag ? sb[tx][y] : sa[tx][y];
                 op[kplus(c, d, p.v)] = p.scale * (xcd + xdc);
                 if (om) om[kminus(c, d, p.v)] = p.scale * (xcd - xdc);
             }
         }
     }
+}
+
+// grid.y of a k_symfold launch: about four resident waves of CTAs (4 per SM), each CTA striding over rows
+static inline int fold_grid_y(int pairs, int rows, int sms) {
+    const long want = (long)sms * 4 * 4;
+    long y = (want + pairs - 1) / pairs;
+    if (y < 1) y = 1;
+    if (y > rows) y = rows;
+    if (y > 65535) y = 65535;
+    return (int)y;
 }
 
 struct ReduceSaArgs {

@@ -293,7 +293,9 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
                 phase ^= 1;
             }
         }
-        // epilogue: read-modify-write of the accumulator matrix; every element belongs to exactly one item
+        // epilogue: accumulate into the R+- matrix.  Every element belongs to exactly one item of this launch and
+        // launches are ordered on the stream, so the sequence of additions per element is fixed (bit-reproducible);
+        // the adds are issued as reductions (RED.ADD.F64, no return value): no load latency in the epilogue.
 #pragma unroll
         for (int i = 0; i < NI; ++i) {
             const int m = m0 + wm * WTM1 + 8 * i + c;
@@ -303,19 +305,9 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
                 const int n = n0 + wn * WTN + 16 * j + 4 * q;  // multiple of 4; rows are 128-byte aligned
                 double *dst = p.acc + (int64_t)m * p.ld + n;
                 const double vals[4] = {acc[i][j][0][0], acc[i][j][1][0], acc[i][j][0][1], acc[i][j][1][1]};
-                if (n >= p.n_begin && n + 3 < p.n_end) {
-                    double2 r0 = *reinterpret_cast<double2 *>(dst), r1 = *reinterpret_cast<double2 *>(dst + 2);
-                    r0.x += vals[0];
-                    r0.y += vals[1];
-                    r1.x += vals[2];
-                    r1.y += vals[3];
-                    *reinterpret_cast<double2 *>(dst) = r0;
-                    *reinterpret_cast<double2 *>(dst + 2) = r1;
-                } else {
 #pragma unroll
-                    for (int t = 0; t < 4; ++t)
-                        if (n + t >= p.n_begin && n + t < p.n_end) dst[t] += vals[t];
-                }
+                for (int t = 0; t < 4; ++t)
+                    if (n + t >= p.n_begin && n + t < p.n_end) atomicAdd(dst + t, vals[t]);
             }
         }
     }
