@@ -160,6 +160,90 @@ def run_reference(args, o, v, x):
     print(json.dumps(line))
 
 
+# ------------------------------------------------------------- the paper's own Table 3 shapes (host-resident)
+# Seconds per contraction printed in Table 3 for these shapes:
+# operands in HOST memory, time includes batching, transfers and DGEMMs -- the same boundary as ppl_apply_host.
+TABLE3_PAPER_SECONDS = {
+    "table3_n800_o100": {"GH200 PyTorch C-split": 355.9, "GH200 CuPy C-split": 306.6, "H100 PyTorch C-split": 330.5,
+                         "H100 CuPy C-split": 461.5, "GH200 PyTorch X-split": 574.7, "H100 PyTorch X-split": 789.4},
+    "table3_n800_o150": {"GH200 PyTorch C-split": 475.3, "GH200 CuPy C-split": 532.8, "H100 PyTorch C-split": 651.2,
+                         "H100 CuPy C-split": 940.9, "GH200 PyTorch X-split": 637.4, "H100 PyTorch X-split": 1128.1},
+}
+
+
+def run_table3(args, o, v, x):
+    """--config table3_*: one of the paper's own benchmark shapes with HOST-resident operands.
+    t2 and R (39 GB each at N=800, nocc=100) do not fit in HBM next to the workspace: ppl_apply_host streams them
+    through staging buffers (PPL_SYM_FULL).  The only number is end to end: wall clock around ppl_apply_host."""
+    import numpy as np
+    import torch
+
+    import paper_2603_20912_b200 as P
+    import ppl_inputs as I
+
+    if args.impl == "reference":
+        print(json.dumps({"impl": "reference", "unavailable": "table3_* shapes are an e2e-only context workload; "
+                          "the reference arm runs on the BASELINE.json configs"}))
+        return
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU path)")
+    torch.cuda.set_device(0)
+    t0 = time.perf_counter()
+    plan = P.Plan(o, v, x, 0)  # before anything else is allocated: the plan sizes itself to 90 % of free memory
+    plan_s = time.perf_counter() - t0
+    info = plan.info()
+    t_gen = time.perf_counter()
+    Lh = torch.empty((x, v, v), dtype=torch.float64, pin_memory=True)
+    th = torch.empty((o, o, v, v), dtype=torch.float64, pin_memory=True)
+    Rh = torch.zeros((o, o, v, v), dtype=torch.float64, pin_memory=True)
+    I.make_L(v, x, 0, out=Lh.numpy())
+    I.make_t2(o, v, 0, out=th.numpy())
+    t_gen = time.perf_counter() - t_gen
+    sampler = ClockSampler(0)
+    for _ in range(max(args.warmup, 0)):
+        plan.apply_host(Lh, th, Rh)
+    Rh.zero_()
+    sampler.start()
+    secs = []
+    for _ in range(args.steps):
+        t0 = time.perf_counter()
+        h2d, d2h = plan.apply_host(Lh, th, Rh)
+        secs.append(time.perf_counter() - t0)
+    clocks = sampler.stop()
+    dt = sum(secs) / len(secs)
+    f_exec, f_nom = info["flops_executed"], info["flops_nominal"]
+    paper = TABLE3_PAPER_SECONDS.get(args.config, {})
+    best = min(paper.values()) if paper else None
+    line = {
+        "metric": "pp_ladder_seconds_per_call_host_resident", "value": dt, "unit": "s", "n_gpus": 1, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": False, "scaling": "weak",
+        "vs_baseline": (dt / best) if best else None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.config, "nocc": o, "nvirt": v, "nchol": x, "seed": 0,
+                   "note": "shape of the paper's Table 3 row (PAPER.md:417-451); operands in pinned HOST memory; "
+                           "symmetric L and pair-symmetric t2 (the paper used unstructured random arrays and no symmetry)",
+                   "symmetry": SYM_DESC[info["symmetry"]],
+                   "plan": {k: info[k] for k in ("ta", "tb", "n_tiles", "workspace_bytes")}},
+        "step_seconds": secs, "plan_seconds": plan_s, "input_gen_seconds": t_gen,
+        "tflops_executed": f_exec / dt * 1e-12, "tflops_nominal_effective": f_nom / dt * 1e-12,
+        "flops_executed": f_exec, "flops_nominal": f_nom,
+        "e2e": {"value": dt, "unit": "s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "how": "ppl_apply_host on pinned host buffers; wall clock around the synchronous call"},
+        "paper_seconds_other_hardware": paper, "clocks": clocks,
+        "gpu_launches": info["launches_per_apply"] * args.steps,
+    }
+    if not args.no_cpu_baseline:
+        Rh.zero_()
+        plan.apply_host(Lh, th, Rh)  # exactly one application of the term for the comparison
+        pairs, cols, dto, cores = oracle_sample(Lh.numpy(), th.numpy(), o, v, x, target_s=20.0)
+        got = Rh.numpy()[:, :, pairs[:, 0], pairs[:, 1]].transpose(2, 0, 1)
+        err = float(np.abs(got - cols).max() / np.abs(cols).max())
+        line["cpu_baseline"] = {"value": dto / len(pairs) * v * v, "unit": "s (extrapolated from the sample)", "cores": cores,
+                                "kind": "oracle", "sample": f"{len(pairs)} of {v*v} (a,b) columns (oracle.columns), all i,j; {dto:.1f} s"}
+        line["parity"] = {"max_rel_err_vs_oracle": err, "tolerance": 1e-11, "columns": int(len(pairs)), "ok": bool(err <= 1e-11)}
+    plan.destroy()
+    print(json.dumps(line))
+
+
 # -------------------------------------------------------------------------------------------- ours
 def main():
     ap = argparse.ArgumentParser()
@@ -177,6 +261,9 @@ def main():
 
     import ppl_inputs as I
 
+    if args.config in I.TABLE3_SHAPES:
+        run_table3(args, *I.TABLE3_SHAPES[args.config])
+        return
     o, v, x = I.CONFIGS[args.config]
     if args.impl == "reference":
         run_reference(args, o, v, x)

@@ -171,10 +171,15 @@ int ppl_apply_ex(ppl_plan_t *plan, const double *L, const double *t2, double *R,
 int ppl_apply_dense(ppl_plan_t *plan, const double *eri, int a0, int na, const double *t2, double *R,
                     const ppl_opts_t *opts, void *stream);
 
-/* ppl_apply_host: the same operation on HOST buffers (pageable or pinned): copies L and t2 to
- * plan-owned device buffers, R in, runs ppl_apply, copies R back, and synchronises before
- * returning.  Device staging buffers are allocated on first use and kept by the plan (they are
- * not counted against workspace_bytes).  h2d/d2h byte counts are returned if non-NULL. */
+/* ppl_apply_host: the same operation on HOST buffers (pageable or pinned), the paper's own setting (operands in
+ * host memory).  Synchronises before returning.  Device buffers are
+ * allocated on first use and kept by the plan (they are not counted against workspace_bytes).
+ *   PPL_SYM_FULL: L is copied whole; t2 and R never sit on the device whole -- t2 is streamed through two staging
+ *     buffers (1 GiB each) and packed chunk by chunk into tau+-, the slabs run on the packed operands, and the result
+ *     is unpacked chunk by chunk (R chunk in, R += term, R chunk out), copies of one chunk overlapping the kernels of
+ *     the other.  Device residency is about half of L + t2 + R: shapes of the paper's Table 3 fit on one 180 GB GPU.
+ *   other modes: L, t2 and R are copied whole, ppl_apply runs, R is copied back (PPL_ERR_ALLOC if they do not fit).
+ * h2d/d2h byte counts are returned if non-NULL.  R accumulates (+=) as in ppl_apply. */
 int ppl_apply_host(ppl_plan_t *plan, const double *L_host, const double *t2_host, double *R_host,
                    uint64_t *h2d_bytes, uint64_t *d2h_bytes);
 

@@ -99,6 +99,8 @@ struct ppl_plan_s {
     cudaStream_t gen = nullptr, host_stream = nullptr;
     cudaEvent_t ev_in = nullptr, ev_ready[MAX_RING] = {}, ev_free[MAX_RING] = {};
     double *dL = nullptr, *dT = nullptr, *dR = nullptr;  // ppl_apply_host staging
+    double *hstage[2] = {nullptr, nullptr};              // ppl_apply_host in PPL_SYM_FULL: two chunk buffers for t2 / R
+    int hchunk_rows = 0;                                 // (i,j) rows per chunk
     double f_step0 = 0, f_step1 = 0;
     CUtensorMap mapW[MAX_RING], mapWp[MAX_RING], mapWm[MAX_RING], mapTp, mapTm;  // plan-owned operands
     // ---- PPL_SYM_FULL (own allocation `fws`; shares taup/taum with PPL_SYM_PAIR_SA) ----
@@ -277,6 +279,8 @@ void free_plan(ppl_plan_s *p) {
     if (p->dL) cudaFree(p->dL);
     if (p->dT) cudaFree(p->dT);
     if (p->dR) cudaFree(p->dR);
+    for (int i = 0; i < 2; ++i)
+        if (p->hstage[i]) cudaFree(p->hstage[i]);
     delete p;
 }
 
@@ -495,6 +499,7 @@ int launch_fold(const ppl_plan_s *p, const double *X, int rows, double *Wp, doub
     a.s_i = a.s_j = 0;
     a.mode = 0;
     a.rows = rows;
+    a.row0 = 0;
     a.o = p->o;
     a.v = p->v;
     a.scale = 1.0;
@@ -513,7 +518,9 @@ int launch_fold(const ppl_plan_s *p, const double *X, int rows, double *Wp, doub
 }
 
 // t2 (either storage order) -> tau+ [Mp][ldp], tau- [Mm][ldm]
-int launch_pack(const ppl_plan_s *p, const double *t2, int layout, double diag, cudaStream_t s) {
+// rows [row0, row1) of the flattened (i,j) index (default: all); t2 is the address of element (0,0,0,0) -- when the
+// amplitudes are packed chunk by chunk (ppl_apply_host) only the rows of the chunk are dereferenced
+int launch_pack(const ppl_plan_s *p, const double *t2, int layout, double diag, cudaStream_t s, int row0 = 0, int row1 = -1) {
     ppl::FoldArgs a;
     a.src = t2;
     const ppl::RStrides ts = r_strides(p->o, p->v, layout);  // t2[i,j,c,d] has the strides of R[i,j,a,b]
@@ -522,7 +529,8 @@ int launch_pack(const ppl_plan_s *p, const double *t2, int layout, double diag, 
     a.s_i = ts.i;
     a.s_j = ts.j;
     a.mode = 1;
-    a.rows = p->o * p->o;
+    a.rows = row1 >= 0 ? row1 : p->o * p->o;
+    a.row0 = row0;
     a.o = p->o;
     a.v = p->v;
     a.scale = 0.5;
@@ -534,7 +542,7 @@ int launch_pack(const ppl_plan_s *p, const double *t2, int layout, double diag, 
     a.ldp = p->ldp;
     a.ldm = p->ldm;
     const int nbv = (p->v + ppl::FT - 1) / ppl::FT;
-    dim3 grid(nbv * (nbv + 1) / 2, ppl::fold_grid_y(nbv * (nbv + 1) / 2, a.rows, p->num_sms));
+    dim3 grid(nbv * (nbv + 1) / 2, ppl::fold_grid_y(nbv * (nbv + 1) / 2, a.rows - a.row0, p->num_sms));
     ppl::k_symfold<<<grid, 256, 0, s>>>(a);
     PPL_CUDA(cudaGetLastError());
     return PPL_OK;
@@ -858,10 +866,15 @@ int launch_reduce_acc(const ppl_plan_s *p, const FullTile &t, const double *part
 
 // The whole path in PPL_SYM_FULL: everything on the caller's stream (every kernel fills the GPU; the
 // strip is single-buffered), prof as in run_apply.
+enum { FULL_PACK = 1, FULL_COMPUTE = 2, FULL_UNPACK = 4, FULL_ALL = 7 };
+int launch_unpack_full(const ppl_plan_s *p, const ppl_opts_t &opts, double *R, int64_t idx0, int64_t idx1, cudaStream_t stream);
+
+// phases: FULL_PACK (t2 -> tau+-, clear R+-acc), FULL_COMPUTE (all slabs), FULL_UNPACK (R+-acc -> R).  ppl_apply runs all
+// three; ppl_apply_host packs and unpacks chunk by chunk itself and calls this with FULL_COMPUTE only (t2, R unused).
 int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, const ppl_opts_t *opts_in, cudaStream_t stream,
-                   Prof *prof) {
+                   Prof *prof, int phases = FULL_ALL) {
     bool vec16 = false;
-    int rc = check_ptrs(p, L, t2, R, &vec16);
+    int rc = check_ptrs(p, L, (phases & FULL_PACK) ? t2 : L, (phases & FULL_UNPACK) ? R : L, &vec16);
     ppl_opts_t opts;
     if (rc == PPL_OK) rc = check_opts(opts_in, &opts);
     if (rc == PPL_OK && (!p->full_ok || !vec16)) rc = PPL_ERR_INVALID_ARG;  // the TMA path needs 16-byte aligned L
@@ -883,10 +896,13 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
         }                                                                                              \
     } while (0)
     const bool minus = p->Mm > 0 && p->Km > 0;
-    if ((rc = launch_pack(p, t2, opts.t2_layout, 0.5, stream)) != PPL_OK) return rc;
-    PPL_CUDA(cudaMemsetAsync(p->raccp, 0, (size_t)p->Mp * p->ldp * 8, stream));
-    if (minus) PPL_CUDA(cudaMemsetAsync(p->raccm, 0, (size_t)p->Mm * p->ldm * 8, stream));
-    PPL_MARK(K_PACK, 1);
+    if (phases & FULL_PACK) {
+        if ((rc = launch_pack(p, t2, opts.t2_layout, 0.5, stream)) != PPL_OK) return rc;
+        PPL_CUDA(cudaMemsetAsync(p->raccp, 0, (size_t)p->Mp * p->ldp * 8, stream));
+        if (minus) PPL_CUDA(cudaMemsetAsync(p->raccm, 0, (size_t)p->Mm * p->ldm * 8, stream));
+        PPL_MARK(K_PACK, 1);
+    }
+    if (!(phases & FULL_COMPUTE)) return PPL_OK;
     CUtensorMap mapL;
     if (make_map_2d(&mapL, L, (uint64_t)p->vv, (uint64_t)p->x, (uint64_t)p->vv * 8, 16, ppl::BK) != PPL_OK) return fail(PPL_ERR_CUDA);
     const int TA = ppl::TA_FULL;
@@ -916,6 +932,7 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
                 f.s_i = f.s_j = 0;
                 f.mode = 2;
                 f.rows = N;
+                f.row0 = 0;
                 f.o = p->o;
                 f.v = p->v;
                 f.scale = 1.0;
@@ -967,25 +984,34 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
             if (n2) PPL_MARK(K_STEP1, n2);
         }
     }
-    {
-        ppl::UnpackArgs u;
-        u.rp = p->raccp;
-        u.rm = p->raccm;
-        u.ldp = p->ldp;
-        u.ldm = p->ldm;
-        u.o = p->o;
-        u.v = p->v;
-        u.alpha = opts.alpha;
-        u.beta = opts.beta;
-        u.rs = r_strides(p->o, p->v, opts.r_layout);
-        u.R = R;
-        ppl::k_unpack_full<<<p->num_sms * 8, 256, 0, stream>>>(u);
-        PPL_CUDA(cudaGetLastError());
+    if (phases & FULL_UNPACK) {
+        if ((rc = launch_unpack_full(p, opts, R, 0, (int64_t)p->o * p->o * p->vv, stream)) != PPL_OK) return rc;
         PPL_DBG("k_unpack_full", 0);
         PPL_MARK(K_REDUCE, 1);
     }
 #undef PPL_MARK
 #undef PPL_DBG
+    return PPL_OK;
+}
+
+// R[idx] = beta R + alpha (R+ +- R-) for the flattened (i,j,a,b) indices [idx0, idx1); R is the address of element (0,0,0,0)
+int launch_unpack_full(const ppl_plan_s *p, const ppl_opts_t &opts, double *R, int64_t idx0, int64_t idx1, cudaStream_t stream) {
+    ppl::UnpackArgs u;
+    u.rp = p->raccp;
+    u.rm = p->raccm;
+    u.ldp = p->ldp;
+    u.ldm = p->ldm;
+    u.o = p->o;
+    u.v = p->v;
+    u.alpha = opts.alpha;
+    u.beta = opts.beta;
+    u.rs = r_strides(p->o, p->v, opts.r_layout);
+    u.R = R;
+    u.idx0 = idx0;
+    u.idx1 = idx1;
+    const int64_t blocks = (idx1 - idx0 + 255) / 256;
+    ppl::k_unpack_full<<<(int)std::min<int64_t>(std::max<int64_t>(blocks, 1), (int64_t)p->num_sms * 8), 256, 0, stream>>>(u);
+    PPL_CUDA(cudaGetLastError());
     return PPL_OK;
 }
 
@@ -1363,17 +1389,93 @@ int ppl_apply_dense(ppl_plan_t *p, const double *eri, int a0, int na, const doub
     return PPL_OK;
 }
 
+// PPL_SYM_FULL on host operands: the device never holds t2 or R.  t2 is streamed through two staging buffers and
+// packed chunk by chunk into tau+- (rows (i,j) of a chunk are contiguous in the [i][j][c][d] order), the slabs run on
+// the packed operands, and R+-acc is unpacked chunk by chunk into the staging buffers (R chunk in, result out).
+// Device residency: L + tau+- + R+-acc + the PPL_SYM_FULL workspace -- about half of L + t2 + R + workspace, which
+// is what lets the paper's Table 3 shapes (t2 and R of 39 GB each at N = 800) run on one 180 GB GPU.
+static int apply_host_full(ppl_plan_s *p, const double *Lh, const double *t2h, double *Rh, uint64_t *h2d, uint64_t *d2h) {
+    const size_t nL = (size_t)p->x * p->vv * 8;
+    const int64_t rows = (int64_t)p->o * p->o;
+    const size_t row_bytes = (size_t)p->vv * 8;
+    if (!p->dL && cudaMalloc(&p->dL, nL) != cudaSuccess) {
+        (void)cudaGetLastError();
+        p->dL = nullptr;
+        return fail(PPL_ERR_ALLOC);
+    }
+    if (!p->hstage[0]) {
+        const char *envc = getenv("PPL_HOST_CHUNK_MB");  // debug override of the staging-buffer size
+        const size_t want = (envc && atol(envc) > 0) ? (size_t)atol(envc) << 20 : (size_t)1 << 30;
+        p->hchunk_rows = (int)std::max<int64_t>(1, std::min<int64_t>(rows, (int64_t)(want / row_bytes)));
+        for (int i = 0; i < 2; ++i)
+            if (cudaMalloc(&p->hstage[i], (size_t)p->hchunk_rows * row_bytes) != cudaSuccess) {
+                (void)cudaGetLastError();
+                for (int k = 0; k < 2; ++k) {
+                    if (p->hstage[k]) cudaFree(p->hstage[k]);
+                    p->hstage[k] = nullptr;
+                }
+                return fail(PPL_ERR_ALLOC);
+            }
+    }
+    cudaStream_t st[2] = {p->host_stream, p->gen};
+    const bool minus = p->Mm > 0 && p->Km > 0;
+    ppl_opts_t opts;
+    check_opts(nullptr, &opts);
+    // phase A: L in; t2 chunks in -> tau+- (chunk k on stream k % 2, each stream owns one staging buffer)
+    PPL_CUDA(cudaMemsetAsync(p->raccp, 0, (size_t)p->Mp * p->ldp * 8, st[1]));
+    if (minus) PPL_CUDA(cudaMemsetAsync(p->raccm, 0, (size_t)p->Mm * p->ldm * 8, st[1]));
+    int k = 0;
+    for (int64_t r0 = 0; r0 < rows; r0 += p->hchunk_rows, ++k) {
+        const int64_t r1 = std::min<int64_t>(rows, r0 + p->hchunk_rows);
+        cudaStream_t s = st[k & 1];
+        double *buf = p->hstage[k & 1];
+        PPL_CUDA(cudaMemcpyAsync(buf, t2h + r0 * p->vv, (size_t)(r1 - r0) * row_bytes, cudaMemcpyHostToDevice, s));
+        const int rc = launch_pack(p, buf - r0 * p->vv, PPL_LAYOUT_IJAB, 0.5, s, (int)r0, (int)r1);
+        if (rc != PPL_OK) return rc;
+    }
+    PPL_CUDA(cudaMemcpyAsync(p->dL, Lh, nL, cudaMemcpyHostToDevice, st[0]));
+    PPL_CUDA(cudaEventRecord(p->ev_in, st[1]));
+    PPL_CUDA(cudaStreamWaitEvent(st[0], p->ev_in, 0));
+    // phase B: all slabs on the packed operands
+    int rc = run_apply_full(p, p->dL, nullptr, nullptr, nullptr, st[0], nullptr, FULL_COMPUTE);
+    if (rc != PPL_OK) return rc;
+    PPL_CUDA(cudaEventRecord(p->ev_in, st[0]));
+    PPL_CUDA(cudaStreamWaitEvent(st[1], p->ev_in, 0));
+    // phase C: R chunk in, R += term, R chunk out
+    k = 0;
+    for (int64_t r0 = 0; r0 < rows; r0 += p->hchunk_rows, ++k) {
+        const int64_t r1 = std::min<int64_t>(rows, r0 + p->hchunk_rows);
+        cudaStream_t s = st[k & 1];
+        double *buf = p->hstage[k & 1];
+        const size_t bytes = (size_t)(r1 - r0) * row_bytes;
+        PPL_CUDA(cudaMemcpyAsync(buf, Rh + r0 * p->vv, bytes, cudaMemcpyHostToDevice, s));
+        if ((rc = launch_unpack_full(p, opts, buf - r0 * p->vv, r0 * p->vv, r1 * p->vv, s)) != PPL_OK) return rc;
+        PPL_CUDA(cudaMemcpyAsync(Rh + r0 * p->vv, buf, bytes, cudaMemcpyDeviceToHost, s));
+    }
+    PPL_CUDA(cudaStreamSynchronize(st[0]));
+    PPL_CUDA(cudaStreamSynchronize(st[1]));
+    const uint64_t nT = (uint64_t)rows * row_bytes;
+    if (h2d) *h2d = (uint64_t)nL + 2 * nT;
+    if (d2h) *d2h = nT;
+    return PPL_OK;
+}
+
 int ppl_apply_host(ppl_plan_t *p, const double *Lh, const double *t2h, double *Rh, uint64_t *h2d, uint64_t *d2h) {
     if (!p || !Lh || !t2h || !Rh) return fail(PPL_ERR_INVALID_ARG);
+    if (p->sym == PPL_SYM_FULL && p->full_ok && (((uintptr_t)Lh | (uintptr_t)t2h | (uintptr_t)Rh) & 7) == 0)
+        return apply_host_full(p, Lh, t2h, Rh, h2d, d2h);
     const size_t nL = (size_t)p->x * p->v * p->v * 8, nT = (size_t)p->o * p->o * p->v * p->v * 8;
-    if (!p->dL) {
-        if (cudaMalloc(&p->dL, nL) != cudaSuccess || cudaMalloc(&p->dT, nT) != cudaSuccess ||
-            cudaMalloc(&p->dR, nT) != cudaSuccess) {
+    if (!p->dL && cudaMalloc(&p->dL, nL) != cudaSuccess) {
+        (void)cudaGetLastError();
+        p->dL = nullptr;
+        return fail(PPL_ERR_ALLOC);
+    }
+    if (!p->dT) {
+        if (cudaMalloc(&p->dT, nT) != cudaSuccess || cudaMalloc(&p->dR, nT) != cudaSuccess) {
             (void)cudaGetLastError();
-            if (p->dL) cudaFree(p->dL);
             if (p->dT) cudaFree(p->dT);
             if (p->dR) cudaFree(p->dR);
-            p->dL = p->dT = p->dR = nullptr;
+            p->dT = p->dR = nullptr;
             return fail(PPL_ERR_ALLOC);
         }
     }

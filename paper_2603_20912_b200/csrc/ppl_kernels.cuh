@@ -390,6 +390,7 @@ struct FoldArgs {
                          // 2: PPL_SYM_FULL: rows r = a_l*tbp + b_l of the tile (A; b-group) taken from the slab's strip;
                          //    rows with a > b, b >= v or a_l >= ta are written as zeros; only c >= A0 is touched
     int rows;            // mode 0/2: number of rows; mode 1: o*o (rows with i > j are skipped)
+    int row0;            // first row processed (0 except when amplitudes are packed chunk by chunk: rows [row0, rows))
     int o, v;
     double scale;        // factor of the off-diagonal (c<d) entries: 1 (W) or 1/2 (tau)
     double diag;         // factor of the diagonal (c==d) entries of the + part: PPL_SYM_PAIR_SA 1 (W), 1 (tau);
@@ -461,7 +462,7 @@ __global__ void __launch_bounds__(256, 4) k_symfold(const FoldArgs p) {
             vb[k] = (live && offdiag && c2 < p.v && d2 < p.v && d2 >= cmin) ? __ldg(s + (int64_t)c2 * p.sc + d2) : 0.0;
         }
     };
-    int r = blockIdx.y;
+    int r = p.row0 + blockIdx.y;
     if (r >= p.rows) return;
     FoldRow cur = fold_row(p, r);
     fetch(cur);

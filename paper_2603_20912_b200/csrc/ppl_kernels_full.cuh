@@ -350,11 +350,11 @@ struct UnpackArgs {
     double alpha, beta;
     RStrides rs;
     double *R;
+    int64_t idx0, idx1;  // range of the flattened (i,j,a,b) index that is written (all: 0, o^2 v^2)
 };
 
 __global__ void __launch_bounds__(256) k_unpack_full(const UnpackArgs p) {
-    const int64_t total = (int64_t)p.o * p.o * p.v * p.v;
-    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+    for (int64_t idx = p.idx0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < p.idx1; idx += (int64_t)gridDim.x * blockDim.x) {
         const int b = (int)(idx % p.v);
         int64_t r = idx / p.v;
         const int a = (int)(r % p.v);

@@ -25,6 +25,12 @@ CONFIGS = {
     "xl": (60, 600, 2400),
 }
 CONFIG_ORDER = ["tiny", "small", "medium", "large", "xl"]
+# Shapes of the paper's own synthetic ladder benchmark (Table 3; N = nocc + nvirt basis functions,
+# nchol = 5N): host-resident operands, a second workload.  Not BASELINE.json configs.
+TABLE3_SHAPES = {
+    "table3_n800_o100": (100, 700, 4000),
+    "table3_n800_o150": (150, 650, 4000),
+}
 
 
 def build(force: bool = False) -> str:

@@ -148,3 +148,43 @@ def test_full_mode_repeated_apply_and_stream_ordering():
             Rd.mul_(0.5)  # ordered after the applies on the same stream
         s.synchronize()
     assert np.array_equal(Rd.cpu().numpy(), 1.5 * want)
+
+
+@pytest.fixture
+def chunk_env():
+    old = os.environ.get("PPL_HOST_CHUNK_MB")
+    yield lambda val: os.environ.__setitem__("PPL_HOST_CHUNK_MB", str(val))
+    if old is None:
+        os.environ.pop("PPL_HOST_CHUNK_MB", None)
+    else:
+        os.environ["PPL_HOST_CHUNK_MB"] = old
+
+
+@pytest.mark.parametrize("shape,chunk_mb", [((6, 96, 40), 1), ((9, 100, 24), 1), ((5, 130, 20), 1), ((4, 98, 30), 1024)])
+def test_host_entry_point_streams_t2_and_R_in_chunks(shape, chunk_mb, chunk_env):
+    """ppl_apply_host in PPL_SYM_FULL: t2 and R never sit on the device whole; they pass through
+    two staging buffers of `chunk_mb` (several chunks, ragged last one, odd chunk counts) and R accumulates (+=)."""
+    o, v, x = shape
+    chunk_env(chunk_mb)
+    L = I.make_L(v, x, seed=61, symmetric=True)
+    t2 = I.make_t2(o, v, seed=61, symmetric=True)
+    R0 = I.make_vec(o * o * v * v, 61, 40).reshape(o, o, v, v)
+    want = oracle.full(L, t2)
+    R = R0.copy()
+    with P.Plan(o, v, x) as plan:
+        assert plan.info()["symmetry"] == P.PPL_SYM_FULL
+        for rep in range(2):  # the staging buffers are reused; the second call adds the term again
+            h2d, d2h = plan.apply_host(L, t2, R)
+            assert h2d == L.nbytes + t2.nbytes + R.nbytes and d2h == R.nbytes
+            assert relerr(R - R0, (rep + 1) * want) <= TOL, rep
+
+
+def test_host_entry_point_exact_integers_chunked(chunk_env):
+    o, v, x = 7, 98, 12
+    chunk_env(1)
+    L = I.make_L(v, x, 43, symmetric=True, integer=True)
+    t2 = 2.0 * I.make_t2(o, v, 43, symmetric=True, integer=True)
+    R = np.zeros((o, o, v, v))
+    with P.Plan(o, v, x) as plan:
+        plan.apply_host(L, t2, R)
+    assert np.array_equal(R, oracle.full(L, t2))
