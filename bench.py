@@ -244,6 +244,23 @@ def run_table3(args, o, v, x):
     print(json.dumps(line))
 
 
+# ------------------------------------------------------------------------------ N > 1: replicas only
+def max_over_ranks(ms: float, dist, device) -> float:
+    """Device time of the slowest rank (one scalar all-reduce: plumbing, not data path). dist=None: one process."""
+    if dist is None:
+        return ms
+    import torch
+
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replicas_value(flops_per_replica: float, ms_per_step: float, world: int) -> float:
+    """Whole-job TFLOP/s of `world` independent replicas that all finished within ms_per_step (the max over ranks)."""
+    return world * flops_per_replica / (ms_per_step * 1e-3) * 1e-12
+
+
 # -------------------------------------------------------------------------------------------- ours
 def main():
     ap = argparse.ArgumentParser()
@@ -329,13 +346,10 @@ def main():
     clocks = sampler.stop()
     step_ms = [evs[k].elapsed_time(evs[k + 1]) for k in range(args.steps)]
     total_ms = evs[0].elapsed_time(evs[-1])
-    if dist is not None:
-        tt = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_ms = float(tt.item())
+    total_ms = max_over_ranks(total_ms, dist, dev)
     ms_per_step = total_ms / args.steps
     f_exec, f_nom = info["flops_executed"], info["flops_nominal"]
-    value = world * f_exec / (ms_per_step * 1e-3) * 1e-12
+    value = replicas_value(f_exec, ms_per_step, world)
 
     # ---- dominant kernel, timed live with CUDA events on the launching stream (serialised pass) ----
     Rd.zero_()
