@@ -117,6 +117,8 @@ struct ppl_plan_s {
     std::vector<FullSlab> slabs;
     std::vector<FullTile> ftiles;
     double ff_step0 = 0, ff_step1 = 0;
+    cudaStream_t fs[4] = {nullptr, nullptr, nullptr, nullptr};  // side streams of the four step-1 GEMMs of a tile
+    cudaEvent_t ev_fold = nullptr, evg[4] = {nullptr, nullptr, nullptr, nullptr};
     CUtensorMap mapFWp, mapFWm, mapFWpT, mapFWmT;  // the W+- tile as the B operand of use 1 (box 16 x 128 rows) / use 2 (box 16 x 16 rows)
 };
 
@@ -268,6 +270,14 @@ void free_plan(ppl_plan_s *p) {
         cudaStreamDestroy(p->host_stream);
     }
     if (p->ev_in) cudaEventDestroy(p->ev_in);
+    if (p->ev_fold) cudaEventDestroy(p->ev_fold);
+    for (int i = 0; i < 4; ++i) {
+        if (p->fs[i]) {
+            cudaStreamSynchronize(p->fs[i]);
+            cudaStreamDestroy(p->fs[i]);
+        }
+        if (p->evg[i]) cudaEventDestroy(p->evg[i]);
+    }
     for (int i = 0; i < MAX_RING; ++i) {
         if (p->ev_ready[i]) cudaEventDestroy(p->ev_ready[i]);
         if (p->ev_free[i]) cudaEventDestroy(p->ev_free[i]);
@@ -805,6 +815,15 @@ int full_setup(ppl_plan_s *p, size_t room) {
         m = m && make_map_2d(&p->mapFWmT, p->fWm, (uint64_t)p->Km, rows, (uint64_t)p->ldm * 8, 16, ppl::BK) == PPL_OK;
     }
     if (!m) return PPL_OK;
+    bool ok = cudaEventCreateWithFlags(&p->ev_fold, cudaEventDisableTiming) == cudaSuccess;
+    for (int i = 0; i < 4 && ok; ++i) {
+        ok = ok && cudaStreamCreateWithFlags(&p->fs[i], cudaStreamNonBlocking) == cudaSuccess;
+        ok = ok && cudaEventCreateWithFlags(&p->evg[i], cudaEventDisableTiming) == cudaSuccess;
+    }
+    if (!ok) {
+        (void)cudaGetLastError();
+        return PPL_OK;
+    }
     p->full_ok = 1;
     return PPL_OK;
 }
@@ -906,6 +925,9 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
     CUtensorMap mapL;
     if (make_map_2d(&mapL, L, (uint64_t)p->vv, (uint64_t)p->x, (uint64_t)p->vv * 8, 16, ppl::BK) != PPL_OK) return fail(PPL_ERR_CUDA);
     const int TA = ppl::TA_FULL;
+    static const bool serial = getenv("PPL_FULL_SERIAL") != nullptr;  // debug: everything on the caller's stream
+    const bool conc = !prof && !dbg && !serial;
+    bool gemms_pending = false;
     for (const FullSlab &sl : p->slabs) {
         ppl::Step0SlabArgs a0;
         a0.A0 = sl.A0;
@@ -924,6 +946,8 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
         for (int k = sl.tile_begin; k < sl.tile_end; ++k) {
             const FullTile &t = p->ftiles[k];
             const int N = TA * t.tbp;
+            if (conc && gemms_pending)  // the previous tile's GEMMs still read the W+- slot
+                for (int i = 0; i < 4; ++i) PPL_CUDA(cudaStreamWaitEvent(stream, p->evg[i], 0));
             {   // fold: strip rows -> W+- tile
                 ppl::FoldArgs f;
                 f.src = p->fX;
@@ -953,37 +977,53 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
                 PPL_DBG("k_symfold", k);
                 PPL_MARK(K_FOLD, 1);
             }
+            // The four GEMMs of the tile are independent given the fold (use 1 writes the R+-acc columns of the slab,
+            // use 2 those above it; + and - are different matrices): outside the profiled pass each runs on a side
+            // stream of its own, so that the tail of one persistent kernel is filled by the CTAs of the next, and the
+            // next slab's step 0 (ordered only behind this slab's last fold: it overwrites the strip) fills theirs.
+            cudaStream_t g0 = conc ? p->fs[0] : stream, g1 = conc ? p->fs[1] : stream, g2 = conc ? p->fs[2] : stream,
+                         g3 = conc ? p->fs[3] : stream;
+            if (conc) {
+                PPL_CUDA(cudaEventRecord(p->ev_fold, stream));
+                for (int i = 0; i < 4; ++i) PPL_CUDA(cudaStreamWaitEvent(p->fs[i], p->ev_fold, 0));
+            }
             // use 1: R+-acc[.][(a,b)] += tau+-[.][J >= (A0,A0)] W+-[(a,b)][J]^T
             double *partp = p->fpart, *partm = p->fpart + (size_t)t.sp.splitk * p->Mp * N;
-            rc = launch_step1(p, &p->mapTp, &p->mapFWp, p->ni_p, nullptr, 0, nullptr, 0, p->Mp, N, p->Kp, t.sp, partp, true, stream,
+            rc = launch_step1(p, &p->mapTp, &p->mapFWp, p->ni_p, nullptr, 0, nullptr, 0, p->Mp, N, p->Kp, t.sp, partp, true, g0,
                               t.k0p);
             const bool m1 = minus && p->Km - t.k0m > 0;
             if (rc == PPL_OK && m1)
                 rc = launch_step1(p, &p->mapTm, &p->mapFWm, p->ni_m, nullptr, 0, nullptr, 0, p->Mm, N, p->Km, t.sm, partm, true,
-                                  stream, t.k0m);
+                                  g1, t.k0m);
             if (rc != PPL_OK) return rc;
             PPL_DBG("use 1 (k_step1_tma)", k);
             PPL_MARK(K_STEP1, m1 ? 2 : 1);
-            rc = launch_reduce_acc(p, t, partp, t.sp.splitk, p->Mp, false, p->raccp, p->ldp, stream);
-            if (rc == PPL_OK && m1) rc = launch_reduce_acc(p, t, partm, t.sm.splitk, p->Mm, true, p->raccm, p->ldm, stream);
+            rc = launch_reduce_acc(p, t, partp, t.sp.splitk, p->Mp, false, p->raccp, p->ldp, g0);
+            if (rc == PPL_OK && m1) rc = launch_reduce_acc(p, t, partm, t.sm.splitk, p->Mm, true, p->raccm, p->ldm, g1);
             if (rc != PPL_OK) return rc;
             PPL_DBG("k_reduce_acc", k);
             PPL_MARK(K_REDUCE, m1 ? 2 : 1);
             // use 2: R+-acc[.][J >= (A0+16,A0+16)] += tau+-[.][(a,b) in tile] W+-[(a,b)][J]
             int n2 = 0;
             if (p->Kp - t.k1p > 0) {
-                if ((rc = launch_step1t(p, &p->mapTp, &p->mapFWpT, p->ni_p, p->Mp, t, false, p->raccp, p->ldp, stream)) != PPL_OK) return rc;
+                if ((rc = launch_step1t(p, &p->mapTp, &p->mapFWpT, p->ni_p, p->Mp, t, false, p->raccp, p->ldp, g2)) != PPL_OK) return rc;
                 PPL_DBG("use 2 plus (k_step1t_tma)", k);
                 ++n2;
             }
             if (minus && p->Km - t.k1m > 0) {
-                if ((rc = launch_step1t(p, &p->mapTm, &p->mapFWmT, p->ni_m, p->Mm, t, true, p->raccm, p->ldm, stream)) != PPL_OK) return rc;
+                if ((rc = launch_step1t(p, &p->mapTm, &p->mapFWmT, p->ni_m, p->Mm, t, true, p->raccm, p->ldm, g3)) != PPL_OK) return rc;
                 PPL_DBG("use 2 minus (k_step1t_tma)", k);
                 ++n2;
             }
             if (n2) PPL_MARK(K_STEP1, n2);
+            if (conc) {
+                for (int i = 0; i < 4; ++i) PPL_CUDA(cudaEventRecord(p->evg[i], p->fs[i]));
+                gemms_pending = true;
+            }
         }
     }
+    if (conc && gemms_pending)
+        for (int i = 0; i < 4; ++i) PPL_CUDA(cudaStreamWaitEvent(stream, p->evg[i], 0));
     if (phases & FULL_UNPACK) {
         if ((rc = launch_unpack_full(p, opts, R, 0, (int64_t)p->o * p->o * p->vv, stream)) != PPL_OK) return rc;
         PPL_DBG("k_unpack_full", 0);
