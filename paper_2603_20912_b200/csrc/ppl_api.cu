@@ -109,17 +109,19 @@ struct ppl_plan_s {
     size_t fws_bytes = 0;
     unsigned char *fws = nullptr;
     double *fX = nullptr;                      // strip [16*v rows (a_l*v + b)][vv]
-    double *fWp = nullptr, *fWm = nullptr;     // W+- tile [16*tbg][ldp], [16*tbg][ldm]
+    int fslots = 1;                            // W+- slots (2 when they fit: the fold of tile k+1 overlaps the GEMMs of tile k)
+    double *fWp[2] = {nullptr, nullptr}, *fWm[2] = {nullptr, nullptr};  // W+- tile [16*tbg][ldp], [16*tbg][ldm]
     double *fpart = nullptr;
     double *raccp = nullptr, *raccm = nullptr; // R+- accumulators [Mp][ldp], [Mm][ldm]
     int2 *fchunks = nullptr;
     size_t fpart_bytes = 0;
+    size_t fpart_m_off = 0;                    // doubles: the minus partials start here (fixed: + and - run on different streams)
     std::vector<FullSlab> slabs;
     std::vector<FullTile> ftiles;
     double ff_step0 = 0, ff_step1 = 0;
     cudaStream_t fs[4] = {nullptr, nullptr, nullptr, nullptr};  // side streams of the four step-1 GEMMs of a tile
-    cudaEvent_t ev_fold = nullptr, evg[4] = {nullptr, nullptr, nullptr, nullptr};
-    CUtensorMap mapFWp, mapFWm, mapFWpT, mapFWmT;  // the W+- tile as the B operand of use 1 (box 16 x 128 rows) / use 2 (box 16 x 16 rows)
+    cudaEvent_t ev_fold[2] = {nullptr, nullptr}, evg[2][4] = {};
+    CUtensorMap mapFWp[2], mapFWm[2], mapFWpT[2], mapFWmT[2];  // the W+- tile as the B operand of use 1 (box 16 x 128 rows) / use 2 (box 16 x 16 rows)
 };
 
 namespace {
@@ -270,13 +272,15 @@ void free_plan(ppl_plan_s *p) {
         cudaStreamDestroy(p->host_stream);
     }
     if (p->ev_in) cudaEventDestroy(p->ev_in);
-    if (p->ev_fold) cudaEventDestroy(p->ev_fold);
-    for (int i = 0; i < 4; ++i) {
+    for (int i = 0; i < 4; ++i)
         if (p->fs[i]) {
             cudaStreamSynchronize(p->fs[i]);
             cudaStreamDestroy(p->fs[i]);
         }
-        if (p->evg[i]) cudaEventDestroy(p->evg[i]);
+    for (int s = 0; s < 2; ++s) {
+        if (p->ev_fold[s]) cudaEventDestroy(p->ev_fold[s]);
+        for (int i = 0; i < 4; ++i)
+            if (p->evg[s][i]) cudaEventDestroy(p->evg[s][i]);
     }
     for (int i = 0; i < MAX_RING; ++i) {
         if (p->ev_ready[i]) cudaEventDestroy(p->ev_ready[i]);
@@ -707,6 +711,7 @@ int full_geometry(ppl_plan_s *p, int tbg, size_t part_cap, std::vector<int2> *ch
     p->ftiles.clear();
     p->ff_step0 = p->ff_step1 = 0;
     p->fpart_bytes = 0;
+    size_t part_p = 0, part_m = 0;
     std::vector<int2> chunks;
     for (int A0 = 0; A0 < v; A0 += TA) {
         FullSlab sl;
@@ -743,7 +748,10 @@ int full_geometry(ppl_plan_s *p, int tbg, size_t part_cap, std::vector<int2> *ch
             const int N = TA * t.tbp;
             t.sp = choose_split(p->Mp, N, p->Kp - t.k0p, p->num_sms, p->bm_p, part_cap / 2);
             t.sm = choose_split(p->Mm, N, p->Km - t.k0m, p->num_sms, p->bm_m, part_cap / 2);
-            p->fpart_bytes = std::max(p->fpart_bytes, ((size_t)t.sp.splitk * p->Mp + (size_t)t.sm.splitk * p->Mm) * N * 8);
+            part_p = std::max(part_p, (size_t)t.sp.splitk * p->Mp * N);
+            part_m = std::max(part_m, (size_t)t.sm.splitk * p->Mm * N);
+            p->fpart_m_off = (part_p + 31) / 32 * 32;
+            p->fpart_bytes = (p->fpart_m_off + part_m) * 8;
             // executed flops: use 1 (contraction over J >= (A0,A0)) + use 2 (outputs J >= (A0+16,A0+16))
             const double r0 = v - A0, r1 = v - c1;  // pairs with c >= A0 / c >= A0+16
             p->ff_step1 += 2.0 * N * ((double)p->Mp * r0 * (r0 + 1) / 2 + (double)p->Mm * r0 * (r0 - 1) / 2);
@@ -768,15 +776,21 @@ int full_setup(ppl_plan_s *p, size_t room) {
     const size_t x_bytes = align256((size_t)TA * v * p->vv * 8);
     const size_t racc_bytes = p->tau_bytes;  // same shapes as tau+-
     std::vector<int2> chunks;
+    const char *envs = getenv("PPL_FULL_SLOTS");  // debug override: 1 = single W+- slot
+    const int want_slots = (envs && atoi(envs) == 1) ? 1 : 2;
     for (;; tbg = std::max(16, tbg / 2 / 16 * 16)) {
         const size_t slot = align256((size_t)TA * tbg * p->ldp * 8) + align256((size_t)TA * tbg * p->ldm * 8);
         const size_t part_cap = std::max<size_t>((size_t)64 << 20, slot / 8);
         full_geometry(p, tbg, part_cap, &chunks);
         const size_t chunk_bytes = align256(chunks.size() * sizeof(int2));
-        const size_t total = x_bytes + slot + align256(p->fpart_bytes) + racc_bytes + chunk_bytes + 256;
-        if (total <= room) {
+        const size_t base = x_bytes + align256(p->fpart_bytes) + racc_bytes + chunk_bytes + 256;
+        int ns = 0;
+        for (int s = want_slots; s >= 1 && !ns; --s)
+            if (base + s * slot <= room) ns = s;
+        if (ns) {
             p->tbg = tbg;
-            p->fws_bytes = total;
+            p->fslots = ns;
+            p->fws_bytes = base + ns * slot;
             break;
         }
         if (tbg == 16) return PPL_OK;  // does not fit: the plan stays without PPL_SYM_FULL
@@ -793,10 +807,12 @@ int full_setup(ppl_plan_s *p, size_t room) {
     unsigned char *q = p->fws;
     p->fX = reinterpret_cast<double *>(q);
     q += x_bytes;
-    p->fWp = reinterpret_cast<double *>(q);
-    q += align256((size_t)TA * p->tbg * p->ldp * 8);
-    p->fWm = reinterpret_cast<double *>(q);
-    q += align256((size_t)TA * p->tbg * p->ldm * 8);
+    for (int s = 0; s < p->fslots; ++s) {
+        p->fWp[s] = reinterpret_cast<double *>(q);
+        q += align256((size_t)TA * p->tbg * p->ldp * 8);
+        p->fWm[s] = reinterpret_cast<double *>(q);
+        q += align256((size_t)TA * p->tbg * p->ldm * 8);
+    }
     p->fpart = reinterpret_cast<double *>(q);
     q += align256(p->fpart_bytes);
     p->raccp = reinterpret_cast<double *>(q);
@@ -808,17 +824,21 @@ int full_setup(ppl_plan_s *p, size_t room) {
         return PPL_OK;
     }
     const uint64_t rows = (uint64_t)TA * p->tbg;
-    bool m = make_map_2d(&p->mapFWp, p->fWp, (uint64_t)p->Kp, rows, (uint64_t)p->ldp * 8, ppl::BK, ppl::BN) == PPL_OK;
-    m = m && make_map_2d(&p->mapFWpT, p->fWp, (uint64_t)p->Kp, rows, (uint64_t)p->ldp * 8, 16, ppl::BK) == PPL_OK;
-    if (p->Km > 0) {
-        m = m && make_map_2d(&p->mapFWm, p->fWm, (uint64_t)p->Km, rows, (uint64_t)p->ldm * 8, ppl::BK, ppl::BN) == PPL_OK;
-        m = m && make_map_2d(&p->mapFWmT, p->fWm, (uint64_t)p->Km, rows, (uint64_t)p->ldm * 8, 16, ppl::BK) == PPL_OK;
+    bool m = true;
+    for (int s = 0; s < p->fslots; ++s) {
+        m = m && make_map_2d(&p->mapFWp[s], p->fWp[s], (uint64_t)p->Kp, rows, (uint64_t)p->ldp * 8, ppl::BK, ppl::BN) == PPL_OK;
+        m = m && make_map_2d(&p->mapFWpT[s], p->fWp[s], (uint64_t)p->Kp, rows, (uint64_t)p->ldp * 8, 16, ppl::BK) == PPL_OK;
+        if (p->Km > 0) {
+            m = m && make_map_2d(&p->mapFWm[s], p->fWm[s], (uint64_t)p->Km, rows, (uint64_t)p->ldm * 8, ppl::BK, ppl::BN) == PPL_OK;
+            m = m && make_map_2d(&p->mapFWmT[s], p->fWm[s], (uint64_t)p->Km, rows, (uint64_t)p->ldm * 8, 16, ppl::BK) == PPL_OK;
+        }
     }
     if (!m) return PPL_OK;
-    bool ok = cudaEventCreateWithFlags(&p->ev_fold, cudaEventDisableTiming) == cudaSuccess;
-    for (int i = 0; i < 4 && ok; ++i) {
-        ok = ok && cudaStreamCreateWithFlags(&p->fs[i], cudaStreamNonBlocking) == cudaSuccess;
-        ok = ok && cudaEventCreateWithFlags(&p->evg[i], cudaEventDisableTiming) == cudaSuccess;
+    bool ok = true;
+    for (int i = 0; i < 4 && ok; ++i) ok = ok && cudaStreamCreateWithFlags(&p->fs[i], cudaStreamNonBlocking) == cudaSuccess;
+    for (int s = 0; s < 2 && ok; ++s) {
+        ok = ok && cudaEventCreateWithFlags(&p->ev_fold[s], cudaEventDisableTiming) == cudaSuccess;
+        for (int i = 0; i < 4 && ok; ++i) ok = ok && cudaEventCreateWithFlags(&p->evg[s][i], cudaEventDisableTiming) == cudaSuccess;
     }
     if (!ok) {
         (void)cudaGetLastError();
@@ -927,7 +947,7 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
     const int TA = ppl::TA_FULL;
     static const bool serial = getenv("PPL_FULL_SERIAL") != nullptr;  // debug: everything on the caller's stream
     const bool conc = !prof && !dbg && !serial;
-    bool gemms_pending = false;
+    int tile_no = 0;
     for (const FullSlab &sl : p->slabs) {
         ppl::Step0SlabArgs a0;
         a0.A0 = sl.A0;
@@ -946,8 +966,9 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
         for (int k = sl.tile_begin; k < sl.tile_end; ++k) {
             const FullTile &t = p->ftiles[k];
             const int N = TA * t.tbp;
-            if (conc && gemms_pending)  // the previous tile's GEMMs still read the W+- slot
-                for (int i = 0; i < 4; ++i) PPL_CUDA(cudaStreamWaitEvent(stream, p->evg[i], 0));
+            const int sl_w = conc ? (tile_no % p->fslots) : 0;  // W+- slot of this tile
+            if (conc && tile_no >= p->fslots)  // the GEMMs of the tile that used this slot last still read it
+                for (int i = 0; i < 4; ++i) PPL_CUDA(cudaStreamWaitEvent(stream, p->evg[sl_w][i], 0));
             {   // fold: strip rows -> W+- tile
                 ppl::FoldArgs f;
                 f.src = p->fX;
@@ -966,8 +987,8 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
                 f.A0 = t.A0;
                 f.ta = t.ta;
                 f.cb_min = t.A0 / ppl::FT;
-                f.dp = p->fWp;
-                f.dm = p->fWm;
+                f.dp = p->fWp[sl_w];
+                f.dm = p->fWm[sl_w];
                 f.ldp = p->ldp;
                 f.ldm = p->ldm;
                 const int nb = (p->v + ppl::FT - 1) / ppl::FT - f.cb_min;
@@ -984,20 +1005,27 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
             cudaStream_t g0 = conc ? p->fs[0] : stream, g1 = conc ? p->fs[1] : stream, g2 = conc ? p->fs[2] : stream,
                          g3 = conc ? p->fs[3] : stream;
             if (conc) {
-                PPL_CUDA(cudaEventRecord(p->ev_fold, stream));
-                for (int i = 0; i < 4; ++i) PPL_CUDA(cudaStreamWaitEvent(p->fs[i], p->ev_fold, 0));
+                PPL_CUDA(cudaEventRecord(p->ev_fold[sl_w], stream));
+                for (int i = 0; i < 4; ++i) PPL_CUDA(cudaStreamWaitEvent(p->fs[i], p->ev_fold[sl_w], 0));
             }
             // use 1: R+-acc[.][(a,b)] += tau+-[.][J >= (A0,A0)] W+-[(a,b)][J]^T
-            double *partp = p->fpart, *partm = p->fpart + (size_t)t.sp.splitk * p->Mp * N;
-            rc = launch_step1(p, &p->mapTp, &p->mapFWp, p->ni_p, nullptr, 0, nullptr, 0, p->Mp, N, p->Kp, t.sp, partp, true, g0,
+            double *partp = p->fpart, *partm = p->fpart + p->fpart_m_off;
+            rc = launch_step1(p, &p->mapTp, &p->mapFWp[sl_w], p->ni_p, nullptr, 0, nullptr, 0, p->Mp, N, p->Kp, t.sp, partp, true, g0,
                               t.k0p);
             const bool m1 = minus && p->Km - t.k0m > 0;
             if (rc == PPL_OK && m1)
-                rc = launch_step1(p, &p->mapTm, &p->mapFWm, p->ni_m, nullptr, 0, nullptr, 0, p->Mm, N, p->Km, t.sm, partm, true,
+                rc = launch_step1(p, &p->mapTm, &p->mapFWm[sl_w], p->ni_m, nullptr, 0, nullptr, 0, p->Mm, N, p->Km, t.sm, partm, true,
                                   g1, t.k0m);
             if (rc != PPL_OK) return rc;
             PPL_DBG("use 1 (k_step1_tma)", k);
             PPL_MARK(K_STEP1, m1 ? 2 : 1);
+            if (conc && tile_no >= 1) {
+                // use 2 of the previous tile (previous slab) adds into the R+-acc columns this reduction updates:
+                // order them (with two W+- slots the fold no longer separates consecutive tiles)
+                const int prev = (tile_no - 1) % p->fslots;
+                PPL_CUDA(cudaStreamWaitEvent(g0, p->evg[prev][2], 0));
+                PPL_CUDA(cudaStreamWaitEvent(g1, p->evg[prev][3], 0));
+            }
             rc = launch_reduce_acc(p, t, partp, t.sp.splitk, p->Mp, false, p->raccp, p->ldp, g0);
             if (rc == PPL_OK && m1) rc = launch_reduce_acc(p, t, partm, t.sm.splitk, p->Mm, true, p->raccm, p->ldm, g1);
             if (rc != PPL_OK) return rc;
@@ -1006,24 +1034,24 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
             // use 2: R+-acc[.][J >= (A0+16,A0+16)] += tau+-[.][(a,b) in tile] W+-[(a,b)][J]
             int n2 = 0;
             if (p->Kp - t.k1p > 0) {
-                if ((rc = launch_step1t(p, &p->mapTp, &p->mapFWpT, p->ni_p, p->Mp, t, false, p->raccp, p->ldp, g2)) != PPL_OK) return rc;
+                if ((rc = launch_step1t(p, &p->mapTp, &p->mapFWpT[sl_w], p->ni_p, p->Mp, t, false, p->raccp, p->ldp, g2)) != PPL_OK) return rc;
                 PPL_DBG("use 2 plus (k_step1t_tma)", k);
                 ++n2;
             }
             if (minus && p->Km - t.k1m > 0) {
-                if ((rc = launch_step1t(p, &p->mapTm, &p->mapFWmT, p->ni_m, p->Mm, t, true, p->raccm, p->ldm, g3)) != PPL_OK) return rc;
+                if ((rc = launch_step1t(p, &p->mapTm, &p->mapFWmT[sl_w], p->ni_m, p->Mm, t, true, p->raccm, p->ldm, g3)) != PPL_OK) return rc;
                 PPL_DBG("use 2 minus (k_step1t_tma)", k);
                 ++n2;
             }
             if (n2) PPL_MARK(K_STEP1, n2);
-            if (conc) {
-                for (int i = 0; i < 4; ++i) PPL_CUDA(cudaEventRecord(p->evg[i], p->fs[i]));
-                gemms_pending = true;
-            }
+            if (conc)
+                for (int i = 0; i < 4; ++i) PPL_CUDA(cudaEventRecord(p->evg[sl_w][i], p->fs[i]));
+            ++tile_no;
         }
     }
-    if (conc && gemms_pending)
-        for (int i = 0; i < 4; ++i) PPL_CUDA(cudaStreamWaitEvent(stream, p->evg[i], 0));
+    if (conc)  // join: the side streams run in order, so the events of the last min(tiles, slots) tiles cover all work
+        for (int s = 0; s < std::min(tile_no, p->fslots); ++s)
+            for (int i = 0; i < 4; ++i) PPL_CUDA(cudaStreamWaitEvent(stream, p->evg[s][i], 0));
     if (phases & FULL_UNPACK) {
         if ((rc = launch_unpack_full(p, opts, R, 0, (int64_t)p->o * p->o * p->vv, stream)) != PPL_OK) return rc;
         PPL_DBG("k_unpack_full", 0);

@@ -44,7 +44,7 @@ def test_full_mode_parity(shape, tbg, tbg_env):
     assert relerr(got, want) <= TOL, info
 
 
-@pytest.mark.parametrize("shape", [(5, 20, 60), (4, 38, 19), (12, 18, 9), (24, 64, 128), (7, 82, 33)])
+@pytest.mark.parametrize("shape", [(5, 20, 60), (4, 38, 19), (12, 18, 9), (24, 64, 128), (7, 82, 33), (3, 130, 12), (9, 100, 24)])
 @pytest.mark.parametrize("tbg", [128, 16])
 def test_full_mode_exact_integers_bit_for_bit(shape, tbg, tbg_env):
     o, v, x = shape
