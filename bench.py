@@ -161,13 +161,13 @@ def run_reference(args, o, v, x):
 
 
 # ------------------------------------------------------------- the paper's own Table 3 shapes (host-resident)
-# Seconds per contraction printed in Table 3 (PAPER.md:428-429, 440-441; BASELINE.md section 2) for these shapes:
+# Seconds per contraction printed in Table 3 (PAPER.md:428-431; BASELINE.md section 2) for these shapes:
 # operands in HOST memory, time includes batching, transfers and DGEMMs -- the same boundary as ppl_apply_host.
 TABLE3_PAPER_SECONDS = {
     "table3_n800_o100": {"GH200 PyTorch C-split": 355.9, "GH200 CuPy C-split": 306.6, "H100 PyTorch C-split": 330.5,
                          "H100 CuPy C-split": 461.5, "GH200 PyTorch X-split": 574.7, "H100 PyTorch X-split": 789.4},
-    "table3_n800_o150": {"GH200 PyTorch C-split": 475.3, "GH200 CuPy C-split": 532.8, "H100 PyTorch C-split": 651.2,
-                         "H100 CuPy C-split": 940.9, "GH200 PyTorch X-split": 637.4, "H100 PyTorch X-split": 1128.1},
+    "table3_n900_o100": {"GH200 PyTorch C-split": 587.1, "GH200 CuPy C-split": 495.0, "H100 PyTorch C-split": 496.2,
+                         "H100 CuPy C-split": 809.7, "GH200 PyTorch X-split": 1265.7, "H100 PyTorch X-split": 1753.3},
 }
 
 
@@ -189,7 +189,11 @@ def run_table3(args, o, v, x):
         raise SystemExit("bench.py: no CUDA device (there is no CPU path)")
     torch.cuda.set_device(0)
     t0 = time.perf_counter()
-    plan = P.Plan(o, v, x, 0)  # before anything else is allocated: the plan sizes itself to 90 % of free memory
+    # before anything else is allocated; the cap leaves room for what ppl_apply_host allocates on first use
+    # (L whole + two 1-GiB staging buffers)
+    free_b = torch.cuda.mem_get_info()[0]
+    cap = int(free_b * 0.98) - x * v * v * 8 - (3 << 30)
+    plan = P.Plan(o, v, x, cap)
     plan_s = time.perf_counter() - t0
     info = plan.info()
     t_gen = time.perf_counter()

@@ -29,7 +29,7 @@ CONFIG_ORDER = ["tiny", "small", "medium", "large", "xl"]
 # nchol = 5N): host-resident operands, a second workload.  Not BASELINE.json configs.
 TABLE3_SHAPES = {
     "table3_n800_o100": (100, 700, 4000),
-    "table3_n800_o150": (150, 650, 4000),
+    "table3_n900_o100": (100, 800, 4500),
 }
 
 
