@@ -719,8 +719,10 @@ int full_geometry(ppl_plan_s *p, int tbg, size_t part_cap, std::vector<int2> *ch
         sl.ta = std::min(TA, v - A0);
         sl.tiles_m = ((v - A0) + 7) / 8;  // 8 c's x 16 a_l per 128-row CTA tile
         sl.chunk_off = chunks.size();
-        for (int b = A0; b < v; ++b)
-            for (int d0 = A0 + ((b - A0) & ~15); d0 < v; d0 += 16) chunks.push_back(make_int2(b, d0));
+        // d-block major: the 8 chunks of a CTA tile are 8 consecutive b's of one d-block, so that the b<->d image
+        // X[a,d,c,b] is written as runs of 8 b's (two full 32-byte sectors, merged in L2) instead of lone doubles
+        for (int d0 = A0; d0 < v; d0 += 16)
+            for (int b = A0; b < std::min(d0 + 16, v); ++b) chunks.push_back(make_int2(b, d0));
         while ((chunks.size() - sl.chunk_off) % 8) chunks.push_back(make_int2(-1, 0));
         sl.tiles_n = (int)((chunks.size() - sl.chunk_off) / 8);
         sl.flops0 = 2.0 * p->x * (128.0 * sl.tiles_m) * (128.0 * sl.tiles_n);

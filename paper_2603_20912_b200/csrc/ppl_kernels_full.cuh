@@ -133,6 +133,9 @@ __global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_slab(const __grid_cons
         int2 ch[2];
 #pragma unroll
         for (int j = 0; j < 2; ++j) ch[j] = p.chunks[8 * tn + 2 * wn + j];
+        // the chunk table is d-block major with b ascending: a thread's two chunks are normally (b, d0), (b+1, d0) with b
+        // even, and then the b<->d image of both is ONE 16-byte store per d (X[a,d,c,b..b+1])
+        const bool pair = ch[0].x >= 0 && ch[1].x == ch[0].x + 1 && ch[1].y == ch[0].y && (ch[0].x & 1) == 0;
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const int cc = p.A0 + 8 * tm + 4 * wm + i;
@@ -153,14 +156,28 @@ __global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_slab(const __grid_cons
                         const double v0 = acc[2 * i + e][2 * j][h], v1 = acc[2 * i + e][2 * j + 1][h];
                         if (d + 1 < v) {  // v even (TMA path), d even: 16-byte aligned
                             *reinterpret_cast<double2 *>(xa + (int64_t)b * vv + d) = make_double2(v0, v1);
-                            if (offdiag) {
+                            if (offdiag && !pair) {
                                 xa[(int64_t)d * vv + b] = v0;
                                 xa[(int64_t)(d + 1) * vv + b] = v1;
                             }
                         } else if (d < v) {
                             xa[(int64_t)b * vv + d] = v0;
-                            if (offdiag) xa[(int64_t)d * vv + b] = v0;
+                            if (offdiag && !pair) xa[(int64_t)d * vv + b] = v0;
                         }
+                    }
+                }
+                if (pair) {
+                    const int b = ch[0].x, d0 = ch[0].y;
+                    if (d0 != p.A0 + ((b - p.A0) & ~15)) {  // b, b+1 share a 16-block (b even)
+#pragma unroll
+                        for (int h = 0; h < 2; ++h)
+#pragma unroll
+                            for (int f = 0; f < 2; ++f) {
+                                const int d = d0 + 2 * q + 8 * h + f;
+                                if (d < v)
+                                    *reinterpret_cast<double2 *>(xa + (int64_t)d * vv + b) =
+                                        make_double2(acc[2 * i + e][f][h], acc[2 * i + e][2 + f][h]);
+                            }
                     }
                 }
             }
