@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- the pp-ladder hot path on B200: seconds per ppl_apply call and FP64 TFLOP/s.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config large|xl|medium|small|tiny]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config large|xl|medium|small|tiny | --shape o,v,x]
                   [--impl ours|reference]
 
 A "step" is one ppl_apply: the whole hot path (step 0 W-tile generation, step 1
@@ -272,6 +272,7 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="large")
+    ap.add_argument("--shape", default=None, help="nocc,nvirt,nchol: a custom shape with the same generators (overrides --config)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workspace-gb", type=float, default=0.0, help="workspace cap (0 = auto)")
     ap.add_argument("--symmetry", default="default", choices=["default", "full", "pair_sa", "pair", "none"],
@@ -282,10 +283,14 @@ def main():
 
     import ppl_inputs as I
 
-    if args.config in I.TABLE3_SHAPES:
+    if args.shape:
+        o, v, x = (int(t) for t in args.shape.split(","))
+        args.config = f"custom_{o}_{v}_{x}"
+    elif args.config in I.TABLE3_SHAPES:
         run_table3(args, *I.TABLE3_SHAPES[args.config])
         return
-    o, v, x = I.CONFIGS[args.config]
+    else:
+        o, v, x = I.CONFIGS[args.config]
     if args.impl == "reference":
         run_reference(args, o, v, x)
         return

@@ -72,7 +72,10 @@ enum {
                          (R+-[.][(ab)] += tau+-[.][(cd)] S[(ab)][(cd)] and R+-[.][(cd)] += tau+-[.][(ab)] S[(ab)][(cd)]),
                          and step 0 computes only (ac|bd) with d-block >= b-block.  Executed flops: step 0 ~ 1/8,
                          step 1 ~ 1/4 of nominal.  Result undefined if a precondition is violated
-                         (ppl_check_inputs detects both).  Needs even nvirt and 16-byte aligned pointers; its
+                         (ppl_check_inputs detects both).  Even nvirt: L must be 16-byte aligned (TMA reads it in
+                         place).  Odd nvirt: the path runs in the geometry of nvirt + 1 -- L is copied per apply into
+                         a plan-owned [nchol][nvirt+1][nvirt+1] buffer with a zero pad row / column,
+                         the pad index of the packed operands carries exact zeros and never reaches R.  Its
                          buffers (a 16 x nvirt^3 strip and the R+- accumulators) are allocated by ppl_plan when
                          they fit under the workspace cap.  Default when available and nvirt >= 96. */
 };
@@ -114,7 +117,7 @@ typedef struct ppl_info_s {
     int32_t sa_splitk_plus, sa_splitk_minus; /* PPL_SYM_PAIR_SA: split-K of the + / - GEMMs (first tile) */
     int32_t sa_tile_m_plus, sa_tile_m_minus; /* PPL_SYM_PAIR_SA: CTA tile rows of the + / - GEMMs */
     int32_t sa_rows_plus, sa_rows_minus;     /* nocc(nocc+1)/2, nocc(nocc-1)/2 */
-    int32_t sa_k_plus, sa_k_minus;           /* nvirt(nvirt+1)/2, nvirt(nvirt-1)/2 */
+    int32_t sa_k_plus, sa_k_minus;           /* v'(v'+1)/2, v'(v'-1)/2, v' = nvirt rounded up to even */
     int32_t full_available;                  /* 1: ppl_plan allocated the PPL_SYM_FULL buffers */
     int32_t full_tbg;                        /* PPL_SYM_FULL: b-group width (tile = 16 a's x full_tbg b's) */
     int32_t full_slabs;                      /* PPL_SYM_FULL: number of a-blocks of 16 (one step-0 launch each) */
@@ -198,7 +201,7 @@ int ppl_last_error(void);                /* code of the last failure on this thr
 const char *ppl_error_string(int code);  /* static string, never NULL */
 
 /* Set PPL_SYM_NONE / PPL_SYM_PAIR / PPL_SYM_PAIR_SA / PPL_SYM_FULL.  Default: PPL_SYM_FULL when its
- * buffers fit and nvirt >= 96 (even nvirt), else PPL_SYM_PAIR_SA, else PPL_SYM_PAIR if the workspace cap
+ * buffers fit and nvirt >= 96, else PPL_SYM_PAIR_SA, else PPL_SYM_PAIR if the workspace cap
  * was too small for the packed operands.  PPL_ERR_WORKSPACE_TOO_SMALL if the plan holds no buffers for
  * the requested mode.  Re-plans the tile list; must not be called while an apply is in flight. */
 int ppl_plan_set_symmetry(ppl_plan_t *plan, int mode);

@@ -80,6 +80,9 @@ struct ppl_plan_s {
     int num_sms = 148;
     int use_tma = 0;      // 1: persistent TMA/mbarrier kernels; 0: cp.async kernels
     int64_t vv = 0;       // nvirt^2 = row length of an un-packed W tile / of t2
+    int vp = 0;           // nvirt rounded up to even: the geometry of every PACKED operand (tau+-, W+-, R+-acc) and of the
+    int64_t vvp = 0;      // whole PPL_SYM_FULL path; for odd nvirt the pad index carries exact zeros
+    double *Lpad = nullptr;  // PPL_SYM_FULL with odd nvirt: L copied into [x][vp][vp] (TMA needs 16-byte rows), inside fws
     // packed geometry (PPL_SYM_PAIR_SA)
     int Mp = 0, Mm = 0;   // rows (i<=j), (i<j)
     int Kp = 0, Km = 0;   // extents of the packed column indices of (c<=d), (c<d), holes included
@@ -515,7 +518,8 @@ int launch_fold(const ppl_plan_s *p, const double *X, int rows, double *Wp, doub
     a.rows = rows;
     a.row0 = 0;
     a.o = p->o;
-    a.v = p->v;
+    a.v = p->vp;
+    a.vs = p->v;
     a.scale = 1.0;
     a.diag = 1.0;
     a.tbp = a.bg0 = a.A0 = a.ta = 0;
@@ -524,7 +528,7 @@ int launch_fold(const ppl_plan_s *p, const double *X, int rows, double *Wp, doub
     a.dm = Wm;
     a.ldp = p->ldp;
     a.ldm = p->ldm;
-    const int nbv = (p->v + ppl::FT - 1) / ppl::FT;
+    const int nbv = (p->vp + ppl::FT - 1) / ppl::FT;
     dim3 grid(nbv * (nbv + 1) / 2, ppl::fold_grid_y(nbv * (nbv + 1) / 2, rows, p->num_sms));
     ppl::k_symfold<<<grid, 256, 0, s>>>(a);
     PPL_CUDA(cudaGetLastError());
@@ -546,7 +550,8 @@ int launch_pack(const ppl_plan_s *p, const double *t2, int layout, double diag, 
     a.rows = row1 >= 0 ? row1 : p->o * p->o;
     a.row0 = row0;
     a.o = p->o;
-    a.v = p->v;
+    a.v = p->vp;
+    a.vs = p->v;
     a.scale = 0.5;
     a.diag = diag;
     a.tbp = a.bg0 = a.A0 = a.ta = 0;
@@ -555,7 +560,7 @@ int launch_pack(const ppl_plan_s *p, const double *t2, int layout, double diag, 
     a.dm = p->taum;
     a.ldp = p->ldp;
     a.ldm = p->ldm;
-    const int nbv = (p->v + ppl::FT - 1) / ppl::FT;
+    const int nbv = (p->vp + ppl::FT - 1) / ppl::FT;
     dim3 grid(nbv * (nbv + 1) / 2, ppl::fold_grid_y(nbv * (nbv + 1) / 2, a.rows - a.row0, p->num_sms));
     ppl::k_symfold<<<grid, 256, 0, s>>>(a);
     PPL_CUDA(cudaGetLastError());
@@ -706,7 +711,7 @@ int run_apply(ppl_plan_s *p, const double *L, const double *t2, double *R, const
 // PPL_SYM_FULL (ppl_kernels_full.cuh): slabs of 16 a's, tiles (A; b-group), chunk table of step 0.
 // ------------------------------------------------------------------------------------------
 int full_geometry(ppl_plan_s *p, int tbg, size_t part_cap, std::vector<int2> *chunks_out) {
-    const int v = p->v, TA = ppl::TA_FULL;
+    const int v = p->vp, TA = ppl::TA_FULL;
     p->slabs.clear();
     p->ftiles.clear();
     p->ff_step0 = p->ff_step1 = 0;
@@ -770,12 +775,13 @@ int full_geometry(ppl_plan_s *p, int tbg, size_t part_cap, std::vector<int2> *ch
 // Allocate the PPL_SYM_FULL buffers if they fit into `room` bytes.  Returns PPL_OK and sets full_ok, or leaves it 0.
 int full_setup(ppl_plan_s *p, size_t room) {
     p->full_ok = 0;
-    if (!p->use_tma || !p->vec16 || !p->sa_ok || p->v < 2) return PPL_OK;
-    const int v = p->v, TA = ppl::TA_FULL;
+    if (!p->use_tma || !p->sa_ok || p->v < 2) return PPL_OK;
+    const int v = p->vp, TA = ppl::TA_FULL;
+    const size_t lpad_bytes = (p->v & 1) ? align256((size_t)p->x * p->vvp * 8) : 0;
     const char *envg = getenv("PPL_TBG");  // debug override of the b-group width
     int tbg = (envg && atoi(envg) >= 16) ? atoi(envg) / 16 * 16 : 256;
     tbg = std::min(tbg, (v + 15) / 16 * 16);
-    const size_t x_bytes = align256((size_t)TA * v * p->vv * 8);
+    const size_t x_bytes = align256((size_t)TA * v * p->vvp * 8);
     const size_t racc_bytes = p->tau_bytes;  // same shapes as tau+-
     std::vector<int2> chunks;
     const char *envs = getenv("PPL_FULL_SLOTS");  // debug override: 1 = single W+- slot
@@ -785,7 +791,7 @@ int full_setup(ppl_plan_s *p, size_t room) {
         const size_t part_cap = std::max<size_t>((size_t)64 << 20, slot / 8);
         full_geometry(p, tbg, part_cap, &chunks);
         const size_t chunk_bytes = align256(chunks.size() * sizeof(int2));
-        const size_t base = x_bytes + align256(p->fpart_bytes) + racc_bytes + chunk_bytes + 256;
+        const size_t base = x_bytes + align256(p->fpart_bytes) + racc_bytes + chunk_bytes + lpad_bytes + 256;
         int ns = 0;
         for (int s = want_slots; s >= 1 && !ns; --s)
             if (base + s * slot <= room) ns = s;
@@ -821,6 +827,8 @@ int full_setup(ppl_plan_s *p, size_t room) {
     p->raccm = reinterpret_cast<double *>(q + align256((size_t)p->Mp * p->ldp * 8));
     q += racc_bytes;
     p->fchunks = reinterpret_cast<int2 *>(q);
+    q += align256(chunks.size() * sizeof(int2));
+    p->Lpad = lpad_bytes ? reinterpret_cast<double *>(q) : nullptr;
     if (cudaMemcpy(p->fchunks, chunks.data(), chunks.size() * sizeof(int2), cudaMemcpyHostToDevice) != cudaSuccess) {
         (void)cudaGetLastError();
         return PPL_OK;
@@ -862,7 +870,7 @@ int launch_step1t(const ppl_plan_s *p, const CUtensorMap *mapA, const CUtensorMa
     a.nkt = ppl::TA_FULL * a.kt_per_a;
     a.A0 = t.A0;
     a.bg0 = t.bg0;
-    a.v = p->v;
+    a.v = p->vp;
     a.minus = minus ? 1 : 0;
     a.acc = acc;
     a.ld = ld;
@@ -894,7 +902,7 @@ int launch_reduce_acc(const ppl_plan_s *p, const FullTile &t, const double *part
     a.A0 = t.A0;
     a.ta = t.ta;
     a.bg0 = t.bg0;
-    a.v = p->v;
+    a.v = p->vp;
     a.minus = minus ? 1 : 0;
     a.acc = acc;
     a.ld = ld;
@@ -918,7 +926,7 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
     int rc = check_ptrs(p, L, (phases & FULL_PACK) ? t2 : L, (phases & FULL_UNPACK) ? R : L, &vec16);
     ppl_opts_t opts;
     if (rc == PPL_OK) rc = check_opts(opts_in, &opts);
-    if (rc == PPL_OK && (!p->full_ok || !vec16)) rc = PPL_ERR_INVALID_ARG;  // the TMA path needs 16-byte aligned L
+    if (rc == PPL_OK && (!p->full_ok || (!vec16 && !p->Lpad))) rc = PPL_ERR_INVALID_ARG;  // TMA reads L: 16-byte aligned rows, or the padded copy
     if (rc != PPL_OK) return fail(rc);
 #define PPL_MARK(k, n)                                                             \
     do {                                                                           \
@@ -944,8 +952,14 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
         PPL_MARK(K_PACK, 1);
     }
     if (!(phases & FULL_COMPUTE)) return PPL_OK;
+    if (p->Lpad) {  // odd nvirt: L -> [x][vp][vp] with a zero pad row / column (2 x |L| bytes of HBM traffic, << 1 % of an apply)
+        ppl::k_pad_L<<<p->num_sms * 8, 256, 0, stream>>>(L, p->Lpad, p->x, p->v, p->vp);
+        PPL_CUDA(cudaGetLastError());
+        PPL_MARK(K_PACK, 1);
+        L = p->Lpad;
+    }
     CUtensorMap mapL;
-    if (make_map_2d(&mapL, L, (uint64_t)p->vv, (uint64_t)p->x, (uint64_t)p->vv * 8, 16, ppl::BK) != PPL_OK) return fail(PPL_ERR_CUDA);
+    if (make_map_2d(&mapL, L, (uint64_t)p->vvp, (uint64_t)p->x, (uint64_t)p->vvp * 8, 16, ppl::BK) != PPL_OK) return fail(PPL_ERR_CUDA);
     const int TA = ppl::TA_FULL;
     static const bool serial = getenv("PPL_FULL_SERIAL") != nullptr;  // debug: everything on the caller's stream
     const bool conc = !prof && !dbg && !serial;
@@ -954,7 +968,7 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
         ppl::Step0SlabArgs a0;
         a0.A0 = sl.A0;
         a0.ta = sl.ta;
-        a0.v = p->v;
+        a0.v = p->vp;
         a0.K = p->x;
         a0.tiles_m = sl.tiles_m;
         a0.tiles_n = sl.tiles_n;
@@ -974,14 +988,14 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
             {   // fold: strip rows -> W+- tile
                 ppl::FoldArgs f;
                 f.src = p->fX;
-                f.sc = p->v;
-                f.s_row = p->vv;
+                f.sc = p->vp;
+                f.s_row = p->vvp;
                 f.s_i = f.s_j = 0;
                 f.mode = 2;
                 f.rows = N;
                 f.row0 = 0;
                 f.o = p->o;
-                f.v = p->v;
+                f.v = f.vs = p->vp;
                 f.scale = 1.0;
                 f.diag = 2.0;
                 f.tbp = t.tbp;
@@ -993,7 +1007,7 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
                 f.dm = p->fWm[sl_w];
                 f.ldp = p->ldp;
                 f.ldm = p->ldm;
-                const int nb = (p->v + ppl::FT - 1) / ppl::FT - f.cb_min;
+                const int nb = (p->vp + ppl::FT - 1) / ppl::FT - f.cb_min;
                 dim3 grid(nb * (nb + 1) / 2, ppl::fold_grid_y(nb * (nb + 1) / 2, N, p->num_sms));
                 ppl::k_symfold<<<grid, 256, 0, stream>>>(f);
                 PPL_CUDA(cudaGetLastError());
@@ -1073,6 +1087,7 @@ int launch_unpack_full(const ppl_plan_s *p, const ppl_opts_t &opts, double *R, i
     u.ldm = p->ldm;
     u.o = p->o;
     u.v = p->v;
+    u.vk = p->vp;
     u.alpha = opts.alpha;
     u.beta = opts.beta;
     u.rs = r_strides(p->o, p->v, opts.r_layout);
@@ -1133,13 +1148,15 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
     p->num_sms = prop.multiProcessorCount;
     p->vec16 = (nvirt % 2 == 0) ? 1 : 0;
     p->vv = (int64_t)nvirt * nvirt;
+    p->vp = nvirt + (nvirt & 1);
+    p->vvp = (int64_t)p->vp * p->vp;
     p->cap = workspace_bytes;
     p->Mp = nocc * (nocc + 1) / 2;
     p->Mm = nocc * (nocc - 1) / 2;
-    p->KpT = nvirt * (nvirt + 1) / 2;
-    p->KmT = nvirt * (nvirt - 1) / 2;
-    p->Kp = (int)ppl::kplus_extent(nvirt);   // extents of the packed index ranges, holes included (ppl_kernels.cuh)
-    p->Km = (int)ppl::kminus_extent(nvirt);
+    p->KpT = p->vp * (p->vp + 1) / 2;         // packed geometry: nvirt rounded up to even (the pad index carries zeros)
+    p->KmT = p->vp * (p->vp - 1) / 2;
+    p->Kp = (int)ppl::kplus_extent(p->vp);   // extents of the packed index ranges, holes included (ppl_kernels.cuh)
+    p->Km = (int)ppl::kminus_extent(p->vp);
     p->ldp = ((int64_t)p->Kp + 15) / 16 * 16;  // rows of the packed operands are 128-byte aligned: TMA-legal for any nvirt
     p->ldm = ((int64_t)std::max(p->Km, 1) + 15) / 16 * 16;
 
@@ -1356,7 +1373,7 @@ int ppl_plan_info(const ppl_plan_t *p, ppl_info_t *out) {
         out->n_tiles = (int)p->ftiles.size();
         out->ring = 1;
         out->splitk = p->ftiles.empty() ? 0 : p->ftiles[0].sp.splitk;
-        int launches = 2 + (int)p->slabs.size();  // pack, unpack, one step 0 per slab
+        int launches = 2 + (int)p->slabs.size() + (p->Lpad ? 1 : 0);  // pack, unpack, one step 0 per slab (+ the L pad copy for odd nvirt)
         for (const FullTile &t : p->ftiles) {
             const bool m1 = minus && p->Km - t.k0m > 0;
             launches += 1 + (m1 ? 4 : 2) + (p->Kp - t.k1p > 0 ? 1 : 0) + (minus && p->Km - t.k1m > 0 ? 1 : 0);

@@ -391,7 +391,8 @@ struct FoldArgs {
                          //    rows with a > b, b >= v or a_l >= ta are written as zeros; only c >= A0 is touched
     int rows;            // mode 0/2: number of rows; mode 1: o*o (rows with i > j are skipped)
     int row0;            // first row processed (0 except when amplitudes are packed chunk by chunk: rows [row0, rows))
-    int o, v;
+    int o, v;            // v: nvirt of the PACKED geometry (kplus/kminus, block grid): the caller's nvirt rounded up to even
+    int vs;              // nvirt of the source: entries with c >= vs or d >= vs are read as zeros (the pad index of odd nvirt)
     double scale;        // factor of the off-diagonal (c<d) entries: 1 (W) or 1/2 (tau)
     double diag;         // factor of the diagonal (c==d) entries of the + part: PPL_SYM_PAIR_SA 1 (W), 1 (tau);
                          // PPL_SYM_FULL 2 (W), 1/2 (tau) -- same products, but W+ becomes a symmetric matrix
@@ -457,9 +458,9 @@ __global__ void __launch_bounds__(256, 4) k_symfold(const FoldArgs p) {
         for (int k = 0; k < FT / 8; ++k) {
             const int y = ty + 8 * k;
             const int c = c0 + y, d = d0 + tx;
-            va[k] = (live && c < p.v && d < p.v && c >= cmin) ? __ldg(s + (int64_t)c * p.sc + d) : 0.0;
+            va[k] = (live && c < p.vs && d < p.vs && c >= cmin) ? __ldg(s + (int64_t)c * p.sc + d) : 0.0;
             const int c2 = d0 + y, d2 = c0 + tx;  // the transposed block: element (c2,d2), c2 in db, d2 in cb
-            vb[k] = (live && offdiag && c2 < p.v && d2 < p.v && d2 >= cmin) ? __ldg(s + (int64_t)c2 * p.sc + d2) : 0.0;
+            vb[k] = (live && offdiag && c2 < p.vs && d2 < p.vs && d2 >= cmin) ? __ldg(s + (int64_t)c2 * p.sc + d2) : 0.0;
         }
     };
     int r = p.row0 + blockIdx.y;

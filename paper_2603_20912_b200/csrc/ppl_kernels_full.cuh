@@ -363,7 +363,8 @@ __global__ void __launch_bounds__(256) k_reduce_acc(const ReduceAccArgs p) {
 struct UnpackArgs {
     const double *rp, *rm;
     int64_t ldp, ldm;
-    int o, v;
+    int o, v;            // v: the caller's nvirt (extent of a, b in R)
+    int vk;              // nvirt of the packed geometry (v rounded up to even)
     double alpha, beta;
     RStrides rs;
     double *R;
@@ -378,12 +379,27 @@ __global__ void __launch_bounds__(256) k_unpack_full(const UnpackArgs p) {
         r /= p.v;
         const int j = (int)(r % p.o), i = (int)(r / p.o);
         const int i1 = min(i, j), j1 = max(i, j), a1 = min(a, b), b1 = max(a, b);
-        double val = p.rp[rowplus(i1, j1, p.o) * p.ldp + kplus(a1, b1, p.v)];
+        double val = p.rp[rowplus(i1, j1, p.o) * p.ldp + kplus(a1, b1, p.vk)];
         if (i1 != j1 && a1 != b1) {
-            const double rm = p.rm[rowminus(i1, j1, p.o) * p.ldm + kminus(a1, b1, p.v)];
+            const double rm = p.rm[rowminus(i1, j1, p.o) * p.ldm + kminus(a1, b1, p.vk)];
             val += ((i > j) == (a > b)) ? rm : -rm;
         }
         r_update(p.R + i * p.rs.i + j * p.rs.j + a * p.rs.a + b * p.rs.b, val, p.alpha, p.beta);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// odd nvirt: L[x][v][v] -> Lpad[x][vp][vp], vp = v + 1, the pad row and column zero.  Rows of Lpad are 16-byte
+// aligned (TMA-legal) and the pad index contributes exact zeros everywhere downstream.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_pad_L(const double *__restrict__ L, double *__restrict__ Lpad, int x, int v, int vp) {
+    const int64_t total = (int64_t)x * vp * vp;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int c = (int)(idx % vp);
+        const int64_t r = idx / vp;
+        const int a = (int)(r % vp);
+        const int64_t P = r / vp;
+        Lpad[idx] = (a < v && c < v) ? __ldg(L + (P * v + a) * v + c) : 0.0;
     }
 }
 

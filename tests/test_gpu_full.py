@@ -1,6 +1,7 @@
 """-m gpu: PPL_SYM_FULL (full 8-fold ERI symmetry: slabs of 16 a's, symmetric S+- used twice, step 0
-restricted to d-block >= b-block; include/ppl.h) against the CPU oracle.  The mode needs symmetric L,
-pair-symmetric t2 and even nvirt.  Same tolerance as everywhere (1e-11 relative, exact integers bit
+restricted to d-block >= b-block; include/ppl.h) against the CPU oracle.  The mode needs symmetric L and
+pair-symmetric t2; odd nvirt runs in the geometry of nvirt + 1 with a zero pad index (L copied into 16-byte aligned
+rows for TMA).  Same tolerance as everywhere (1e-11 relative, exact integers bit
 for bit).  The identity behind it is pinned on the CPU (test_oracle_pins.py::test_full_symmetry_hook_identity)."""
 import os
 
@@ -15,9 +16,11 @@ from gpu_util import gpu_ladder, relerr
 pytestmark = pytest.mark.gpu
 TOL = 1e-11
 
-# even nvirt; one slab (v <= 16), several slabs, ragged last slab (v % 16 != 0), nocc^2 > 128, one/two-element edges
+# even nvirt; one slab (v <= 16), several slabs, ragged last slab (v % 16 != 0), nocc^2 > 128, one/two-element edges;
+# odd nvirt (padded to nvirt + 1): below / at / above a 16-block edge, the small config's 53, one-element edges
 SHAPES = [(1, 2, 1), (2, 16, 4), (12, 18, 9), (3, 24, 17), (5, 20, 60), (3, 40, 33), (13, 22, 40), (6, 50, 70),
-          (4, 66, 30), (9, 100, 24), (24, 64, 128), (2, 130, 20)]
+          (4, 66, 30), (9, 100, 24), (24, 64, 128), (2, 130, 20),
+          (2, 3, 2), (3, 15, 7), (4, 17, 9), (5, 31, 12), (3, 33, 20), (5, 53, 232), (7, 97, 30), (2, 129, 16), (1, 5, 1)]
 
 
 @pytest.fixture
@@ -44,7 +47,8 @@ def test_full_mode_parity(shape, tbg, tbg_env):
     assert relerr(got, want) <= TOL, info
 
 
-@pytest.mark.parametrize("shape", [(5, 20, 60), (4, 38, 19), (12, 18, 9), (24, 64, 128), (7, 82, 33), (3, 130, 12), (9, 100, 24)])
+@pytest.mark.parametrize("shape", [(5, 20, 60), (4, 38, 19), (12, 18, 9), (24, 64, 128), (7, 82, 33), (3, 130, 12), (9, 100, 24),
+                                   (4, 37, 19), (6, 81, 33), (3, 113, 12), (5, 53, 40)])
 @pytest.mark.parametrize("tbg", [128, 16])
 def test_full_mode_exact_integers_bit_for_bit(shape, tbg, tbg_env):
     o, v, x = shape
@@ -57,10 +61,11 @@ def test_full_mode_exact_integers_bit_for_bit(shape, tbg, tbg_env):
         assert np.array_equal(got, want), rep
 
 
-def test_full_mode_accumulates_and_handles_layouts_alpha_beta():
+@pytest.mark.parametrize("nvirt", [36, 35])
+def test_full_mode_accumulates_and_handles_layouts_alpha_beta(nvirt):
     import torch
 
-    o, v, x = 4, 36, 19
+    o, v, x = 4, nvirt, 19
     L = I.make_L(v, x, 11, symmetric=True)
     t2 = I.make_t2(o, v, 11, symmetric=True)
     R0 = I.make_t2(o, v, 12, symmetric=False)
@@ -88,7 +93,7 @@ def test_full_mode_accumulates_and_handles_layouts_alpha_beta():
 def test_full_mode_preconditions_default_and_availability():
     import torch
 
-    # default: PPL_SYM_FULL from nvirt = 96 up (even nvirt), PPL_SYM_PAIR_SA below; odd nvirt has no PPL_SYM_FULL
+    # default: PPL_SYM_FULL from nvirt = 96 up (odd nvirt included: padded geometry), PPL_SYM_PAIR_SA below
     with P.Plan(3, 96, 8) as plan:
         assert plan.info()["symmetry"] == P.PPL_SYM_FULL
     with P.Plan(3, 40, 8) as plan:
@@ -96,10 +101,10 @@ def test_full_mode_preconditions_default_and_availability():
         assert info["symmetry"] == P.PPL_SYM_PAIR_SA and info["full_available"] == 1
     with P.Plan(3, 97, 8) as plan:
         info = plan.info()
-        assert info["symmetry"] == P.PPL_SYM_PAIR_SA and info["full_available"] == 0
-        with pytest.raises(P.PplError) as e:
-            plan.set_symmetry(P.PPL_SYM_FULL)
-        assert e.value.code == P.PPL_ERR_WORKSPACE_TOO_SMALL
+        assert info["symmetry"] == P.PPL_SYM_FULL and info["full_available"] == 1 and info["nvirt"] == 97
+    with P.Plan(3, 53, 8) as plan:
+        info = plan.info()
+        assert info["symmetry"] == P.PPL_SYM_PAIR_SA and info["full_available"] == 1
     # a cap that holds the PPL_SYM_PAIR_SA plan but not the 16 x nvirt^3 strip: the plan falls back
     o, v, x = 3, 96, 8
     with P.Plan(o, v, x, 40 << 20) as plan:
@@ -160,7 +165,8 @@ def chunk_env():
         os.environ["PPL_HOST_CHUNK_MB"] = old
 
 
-@pytest.mark.parametrize("shape,chunk_mb", [((6, 96, 40), 1), ((9, 100, 24), 1), ((5, 130, 20), 1), ((4, 98, 30), 1024)])
+@pytest.mark.parametrize("shape,chunk_mb", [((6, 96, 40), 1), ((9, 100, 24), 1), ((5, 130, 20), 1), ((4, 98, 30), 1024),
+                                            ((6, 97, 40), 1), ((5, 131, 20), 1)])
 def test_host_entry_point_streams_t2_and_R_in_chunks(shape, chunk_mb, chunk_env):
     """ppl_apply_host in PPL_SYM_FULL: t2 and R never sit on the device whole; they pass through
     two staging buffers of `chunk_mb` (several chunks, ragged last one, odd chunk counts) and R accumulates (+=)."""
