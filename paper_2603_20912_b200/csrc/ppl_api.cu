@@ -36,6 +36,14 @@ struct SplitChoice {
     double seconds = 0;
 };
 
+// Row tiling of the M side of step 1.  TMA kernels: 8-row blocks dealt to 2*tiles_m half-tiles of `base` or `base+1`
+// blocks (ppl::MSplit); cp.async kernels: uniform tiles of 128 rows.
+struct MGeom {
+    int tiles_m = 1, base = 0, rem = 0;
+    int ni = 8;         // template instance (TMA box of the A operand: 16*ni rows)
+    double rows = 128;  // average rows computed per CTA tile (cost model)
+};
+
 struct Tile {
     int a0, ta, b0, tb;
     int mirror;
@@ -88,7 +96,8 @@ struct ppl_plan_s {
     int Kp = 0, Km = 0;   // extents of the packed column indices of (c<=d), (c<d), holes included
     int KpT = 0, KmT = 0; // number of pairs (c<=d), (c<d)
     int64_t ldp = 0, ldm = 0;
-    int ni_full = 8, bm_full = 128, ni_p = 8, bm_p = 128, ni_m = 8, bm_m = 128;  // step-1 CTA tile rows (16*NI)
+    int bm_full = 128, bm_p = 128, bm_m = 128;  // step-1 CTA tile rows (TMA box: 16*NI)
+    MGeom mg_full, mg_p, mg_m;                  // row tiling of nocc^2 / the packed (i<=j) / (i<j) rows
     size_t cap = 0;
     size_t x_bytes = 0, slot_bytes = 0, part_bytes = 0, tau_bytes = 0, ws_bytes = 0;
     unsigned char *ws = nullptr;
@@ -136,26 +145,31 @@ namespace {
 // `sms` SMs), the best split-K per tile shape, and the streaming traffic.
 // ------------------------------------------------------------------------------------------
 
-// CTA tile rows of step 1: 16*NI with NI in 5..10 chosen to pad M the least (ties: larger tile)
-int choose_ni(int M) {
-    int best = 8;
-    long best_pad = -1;
-    for (int ni = 10; ni >= 5; --ni) {
-        const long bm = 16 * ni, pad = ((M + bm - 1) / bm) * bm;
-        if (best_pad < 0 || pad < best_pad) {
-            best_pad = pad;
-            best = ni;
-        }
-    }
-    return best;
+// TMA kernels: the fewest CTA tiles of at most 16*10 rows, rows dealt in 8-row blocks as evenly as possible
+// (ppl_kernels_tma.cuh, MSplit): padding < 8 rows in all.  nmax: largest template instance to use (debug override).
+// Every warp row gets ni or ni - 1 blocks: the only two cases the kernels are compiled for.
+MGeom m_geom_tma(int M, int nmax) {
+    MGeom g;
+    const int blocks = (std::max(M, 1) + 7) / 8;
+    g.tiles_m = (blocks + 2 * nmax - 1) / (2 * nmax);
+    g.base = blocks / (2 * g.tiles_m);
+    g.rem = blocks % (2 * g.tiles_m);
+    g.ni = g.base + (g.rem > 0 ? 1 : 0);  // 1 .. nmax
+    g.rows = 8.0 * blocks / g.tiles_m;
+    return g;
+}
+MGeom m_geom_plain(int M) {
+    MGeom g;
+    g.tiles_m = (std::max(M, 1) + ppl::BM - 1) / ppl::BM;
+    return g;
 }
 
-SplitChoice choose_split(int M, int N, int64_t K, int sms, int bm, size_t part_cap = ~(size_t)0) {
+SplitChoice choose_split(int M, int N, int64_t K, int sms, const MGeom &mg, size_t part_cap = ~(size_t)0) {
     SplitChoice best;
     if (M <= 0 || N <= 0 || K <= 0) return best;
-    const int tiles = ((M + bm - 1) / bm) * ((N + ppl::BN - 1) / ppl::BN);
+    const int tiles = mg.tiles_m * ((N + ppl::BN - 1) / ppl::BN);
     const int nkt = (int)((K + ppl::BK - 1) / ppl::BK);
-    const double tau = 2.0 * bm * ppl::BN * ppl::BK / (PEAK_FLOPS / sms);  // one k-tile on one SM
+    const double tau = 2.0 * mg.rows * ppl::BN * ppl::BK / (PEAK_FLOPS / sms);  // one k-tile on one SM
     best = SplitChoice{1, nkt * ppl::BK, 1e300};
     const int smax = std::max(1, std::min(nkt / 8 + 1, 64));
     for (int s = 1; s <= smax; ++s) {
@@ -182,7 +196,7 @@ struct Geometry {  // what depends on (o, v) only
     int64_t vv;
     int M, Mp, Mm, Kp, Km;
     int64_t ldp, ldm;
-    int bm_full, bm_p, bm_m;
+    MGeom mg_full, mg_p, mg_m;
 };
 
 struct PlanEval {
@@ -209,11 +223,11 @@ PlanEval evaluate(const Geometry &g, int o, int v, int x, int T, bool sa, int sm
             if (cnt == 0) continue;
             const int ta = ae ? r : T, tb = be ? r : T;
             const int N = ta * tb;
-            const SplitChoice full = choose_split(g.M, N, g.vv, sms, g.bm_full);
+            const SplitChoice full = choose_split(g.M, N, g.vv, sms, g.mg_full);
             size_t part = (size_t)full.splitk * g.M * N * 8;
             double compute, dram;
             if (sa) {
-                const SplitChoice sp = choose_split(g.Mp, N, g.Kp, sms, g.bm_p), sm = choose_split(g.Mm, N, g.Km, sms, g.bm_m);
+                const SplitChoice sp = choose_split(g.Mp, N, g.Kp, sms, g.mg_p), sm = choose_split(g.Mm, N, g.Km, sms, g.mg_m);
                 const double fold = 2.0 * N * g.vv * 8.0 / HBM_BPS + LAUNCH_S;
                 compute = step0_seconds(ta, tb, v, x, sms) + fold + sp.seconds + sm.seconds;
                 dram = (((double)g.Mp * g.ldp + (double)g.Mm * g.ldm) * 8.0 + 4.0 * N * g.vv * 8.0) / HBM_BPS;
@@ -248,13 +262,13 @@ int build_tiles(ppl_plan_s *p) {
             t.mirror = (pair && ab != bb) ? 1 : 0;
             const int N = t.ta * t.tb;
             if (sa) {
-                t.sp = choose_split(p->Mp, N, p->Kp, p->num_sms, p->bm_p);
-                t.sm = choose_split(p->Mm, N, p->Km, p->num_sms, p->bm_m);
+                t.sp = choose_split(p->Mp, N, p->Kp, p->num_sms, p->mg_p);
+                t.sm = choose_split(p->Mm, N, p->Km, p->num_sms, p->mg_m);
                 if (((size_t)t.sp.splitk * p->Mp + (size_t)t.sm.splitk * p->Mm) * N * 8 > p->part_bytes)
                     return PPL_ERR_WORKSPACE_TOO_SMALL;
                 p->f_step1 += 2.0 * N * ((double)p->Mp * p->KpT + (double)p->Mm * p->KmT);
             } else {
-                t.full = choose_split(M, N, p->vv, p->num_sms, p->bm_full, p->part_bytes);
+                t.full = choose_split(M, N, p->vv, p->num_sms, p->mg_full, p->part_bytes);
                 if ((size_t)t.full.splitk * M * N * 8 > p->part_bytes) return PPL_ERR_WORKSPACE_TOO_SMALL;
                 p->f_step1 += 2.0 * M * (double)N * (double)p->vv;
             }
@@ -313,7 +327,7 @@ int set_kernel_attrs() {
 #define PPL_ATTR_NI(NI)                                                                                                                \
     PPL_CUDA(cudaFuncSetAttribute(ppl::k_step1_tma<NI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::Step1Cfg<NI>::SMEM)); \
     PPL_CUDA(cudaFuncSetAttribute(ppl::k_step1t_tma<NI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::Step1Cfg<NI>::SMEM));
-    PPL_ATTR_NI(5) PPL_ATTR_NI(6) PPL_ATTR_NI(7) PPL_ATTR_NI(8) PPL_ATTR_NI(9) PPL_ATTR_NI(10)
+    PPL_ATTR_NI(1) PPL_ATTR_NI(2) PPL_ATTR_NI(3) PPL_ATTR_NI(4) PPL_ATTR_NI(5) PPL_ATTR_NI(6) PPL_ATTR_NI(7) PPL_ATTR_NI(8) PPL_ATTR_NI(9) PPL_ATTR_NI(10)
 #undef PPL_ATTR_NI
     g_attr_set = true;
     return PPL_OK;
@@ -392,7 +406,7 @@ int launch_step0(const ppl_plan_s *p, const Tile &t, const double *L, const CUte
 
 // One step-1 GEMM: part[z][M][N] = sum_{k in split z} A[m][k] B[n][k]; A is lda-strided, B ldb-strided.
 // With maps: the persistent TMA kernel with CTA tile (16*ni) x 128; without: the cp.async kernel.
-int launch_step1(const ppl_plan_s *p, const CUtensorMap *mapA, const CUtensorMap *mapB, int ni, const double *A, int64_t lda,
+int launch_step1(const ppl_plan_s *p, const CUtensorMap *mapA, const CUtensorMap *mapB, const MGeom &mg, const double *A, int64_t lda,
                  const double *B, int64_t ldb, int M, int N, int64_t K, const SplitChoice &sc, double *part, bool vec16,
                  cudaStream_t s, int k0 = 0) {
     if (M <= 0 || N <= 0 || K - k0 <= 0) return PPL_OK;
@@ -406,15 +420,16 @@ int launch_step1(const ppl_plan_s *p, const CUtensorMap *mapA, const CUtensorMap
         a.k_per_split = sc.k_per_split;
         a.splitk = sc.splitk;
         a.part = part;
-        const int bm = 16 * ni;
-        const int items = ((M + bm - 1) / bm) * ((N + ppl::BN - 1) / ppl::BN) * sc.splitk;
+        a.ms = ppl::MSplit{mg.tiles_m, mg.base, mg.rem};
+        const int items = mg.tiles_m * ((N + ppl::BN - 1) / ppl::BN) * sc.splitk;
         const int grid = std::min(items, p->num_sms);
-        switch (ni) {
+        switch (mg.ni) {
 #define PPL_LAUNCH_NI(NI)                                                                                   \
     case NI:                                                                                                \
         ppl::k_step1_tma<NI><<<grid, ppl::TMA_THREADS, ppl::Step1Cfg<NI>::SMEM, s>>>(*mapA, *mapB, a);    \
         break;
-            PPL_LAUNCH_NI(5) PPL_LAUNCH_NI(6) PPL_LAUNCH_NI(7) PPL_LAUNCH_NI(8) PPL_LAUNCH_NI(9) PPL_LAUNCH_NI(10)
+            PPL_LAUNCH_NI(1) PPL_LAUNCH_NI(2) PPL_LAUNCH_NI(3) PPL_LAUNCH_NI(4) PPL_LAUNCH_NI(5) PPL_LAUNCH_NI(6) PPL_LAUNCH_NI(7)
+            PPL_LAUNCH_NI(8) PPL_LAUNCH_NI(9) PPL_LAUNCH_NI(10)
 #undef PPL_LAUNCH_NI
             default: return fail(PPL_ERR_INVALID_ARG);
         }
@@ -681,17 +696,17 @@ int run_apply(ppl_plan_s *p, const double *L, const double *t2, double *R, const
         // ---- consumer: step 1, reduce ----
         if (sa) {
             double *partp = p->part, *partm = p->part + (size_t)t.sp.splitk * p->Mp * N;
-            rc = launch_step1(p, tma1 ? &p->mapTp : nullptr, tma1 ? &p->mapWp[slot] : nullptr, p->ni_p, p->taup, p->ldp, Wp,
+            rc = launch_step1(p, tma1 ? &p->mapTp : nullptr, tma1 ? &p->mapWp[slot] : nullptr, p->mg_p, p->taup, p->ldp, Wp,
                               p->ldp, p->Mp, N, p->Kp, t.sp, partp, true, stream);
             if (rc == PPL_OK && minus)
-                rc = launch_step1(p, tma1 ? &p->mapTm : nullptr, tma1 ? &p->mapWm[slot] : nullptr, p->ni_m, p->taum, p->ldm,
+                rc = launch_step1(p, tma1 ? &p->mapTm : nullptr, tma1 ? &p->mapWm[slot] : nullptr, p->mg_m, p->taum, p->ldm,
                                   Wm, p->ldm, p->Mm, N, p->Km, t.sm, partm, true, stream);
             if (rc != PPL_OK) return rc;
             PPL_MARK(K_STEP1, minus ? 2 : 1);
             if (two_streams) PPL_CUDA(cudaEventRecord(p->ev_free[slot], stream));
             if ((rc = launch_reduce_sa(p, t, partp, partm, R, opts, stream)) != PPL_OK) return rc;
         } else {
-            rc = launch_step1(p, tma1 ? &mapT : nullptr, tma1 ? &p->mapW[slot] : nullptr, p->ni_full, t2m, p->vv, p->slot[slot],
+            rc = launch_step1(p, tma1 ? &mapT : nullptr, tma1 ? &p->mapW[slot] : nullptr, p->mg_full, t2m, p->vv, p->slot[slot],
                               p->vv, p->o * p->o, N, p->vv, t.full, p->part, vec16, stream);
             if (rc != PPL_OK) return rc;
             PPL_MARK(K_STEP1, 1);
@@ -753,8 +768,8 @@ int full_geometry(ppl_plan_s *p, int tbg, size_t part_cap, std::vector<int2> *ch
             t.k1p = c1 < v ? (int)ppl::kplus(c1, c1, v) : p->Kp;
             t.k1m = c1 + 1 < v ? (int)ppl::kminus(c1, c1 + 1, v) - 1 : p->Km;
             const int N = TA * t.tbp;
-            t.sp = choose_split(p->Mp, N, p->Kp - t.k0p, p->num_sms, p->bm_p, part_cap / 2);
-            t.sm = choose_split(p->Mm, N, p->Km - t.k0m, p->num_sms, p->bm_m, part_cap / 2);
+            t.sp = choose_split(p->Mp, N, p->Kp - t.k0p, p->num_sms, p->mg_p, part_cap / 2);
+            t.sm = choose_split(p->Mm, N, p->Km - t.k0m, p->num_sms, p->mg_m, part_cap / 2);
             part_p = std::max(part_p, (size_t)t.sp.splitk * p->Mp * N);
             part_m = std::max(part_m, (size_t)t.sm.splitk * p->Mm * N);
             p->fpart_m_off = (part_p + 31) / 32 * 32;
@@ -858,7 +873,7 @@ int full_setup(ppl_plan_s *p, size_t room) {
     return PPL_OK;
 }
 
-int launch_step1t(const ppl_plan_s *p, const CUtensorMap *mapA, const CUtensorMap *mapB, int ni, int M, const FullTile &t,
+int launch_step1t(const ppl_plan_s *p, const CUtensorMap *mapA, const CUtensorMap *mapB, const MGeom &mg, int M, const FullTile &t,
                   bool minus, double *acc, int64_t ld, cudaStream_t s) {
     ppl::Step1TArgs a;
     a.M = M;
@@ -874,15 +889,16 @@ int launch_step1t(const ppl_plan_s *p, const CUtensorMap *mapA, const CUtensorMa
     a.minus = minus ? 1 : 0;
     a.acc = acc;
     a.ld = ld;
-    const int bm = 16 * ni;
-    const int items = ((M + bm - 1) / bm) * ((a.n_end - a.n_base + ppl::BN - 1) / ppl::BN);
+    a.ms = ppl::MSplit{mg.tiles_m, mg.base, mg.rem};
+    const int items = mg.tiles_m * ((a.n_end - a.n_base + ppl::BN - 1) / ppl::BN);
     const int grid = std::min(items, p->num_sms);
-    switch (ni) {
+    switch (mg.ni) {
 #define PPL_LAUNCH_NI(NI)                                                                                  \
     case NI:                                                                                               \
         ppl::k_step1t_tma<NI><<<grid, ppl::TMA_THREADS, ppl::Step1Cfg<NI>::SMEM, s>>>(*mapA, *mapB, a);  \
         break;
-        PPL_LAUNCH_NI(5) PPL_LAUNCH_NI(6) PPL_LAUNCH_NI(7) PPL_LAUNCH_NI(8) PPL_LAUNCH_NI(9) PPL_LAUNCH_NI(10)
+        PPL_LAUNCH_NI(1) PPL_LAUNCH_NI(2) PPL_LAUNCH_NI(3) PPL_LAUNCH_NI(4) PPL_LAUNCH_NI(5) PPL_LAUNCH_NI(6) PPL_LAUNCH_NI(7)
+            PPL_LAUNCH_NI(8) PPL_LAUNCH_NI(9) PPL_LAUNCH_NI(10)
 #undef PPL_LAUNCH_NI
         default: return fail(PPL_ERR_INVALID_ARG);
     }
@@ -1026,11 +1042,11 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
             }
             // use 1: R+-acc[.][(a,b)] += tau+-[.][J >= (A0,A0)] W+-[(a,b)][J]^T
             double *partp = p->fpart, *partm = p->fpart + p->fpart_m_off;
-            rc = launch_step1(p, &p->mapTp, &p->mapFWp[sl_w], p->ni_p, nullptr, 0, nullptr, 0, p->Mp, N, p->Kp, t.sp, partp, true, g0,
+            rc = launch_step1(p, &p->mapTp, &p->mapFWp[sl_w], p->mg_p, nullptr, 0, nullptr, 0, p->Mp, N, p->Kp, t.sp, partp, true, g0,
                               t.k0p);
             const bool m1 = minus && p->Km - t.k0m > 0;
             if (rc == PPL_OK && m1)
-                rc = launch_step1(p, &p->mapTm, &p->mapFWm[sl_w], p->ni_m, nullptr, 0, nullptr, 0, p->Mm, N, p->Km, t.sm, partm, true,
+                rc = launch_step1(p, &p->mapTm, &p->mapFWm[sl_w], p->mg_m, nullptr, 0, nullptr, 0, p->Mm, N, p->Km, t.sm, partm, true,
                                   g1, t.k0m);
             if (rc != PPL_OK) return rc;
             PPL_DBG("use 1 (k_step1_tma)", k);
@@ -1050,12 +1066,12 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
             // use 2: R+-acc[.][J >= (A0+16,A0+16)] += tau+-[.][(a,b) in tile] W+-[(a,b)][J]
             int n2 = 0;
             if (p->Kp - t.k1p > 0) {
-                if ((rc = launch_step1t(p, &p->mapTp, &p->mapFWpT[sl_w], p->ni_p, p->Mp, t, false, p->raccp, p->ldp, g2)) != PPL_OK) return rc;
+                if ((rc = launch_step1t(p, &p->mapTp, &p->mapFWpT[sl_w], p->mg_p, p->Mp, t, false, p->raccp, p->ldp, g2)) != PPL_OK) return rc;
                 PPL_DBG("use 2 plus (k_step1t_tma)", k);
                 ++n2;
             }
             if (minus && p->Km - t.k1m > 0) {
-                if ((rc = launch_step1t(p, &p->mapTm, &p->mapFWmT[sl_w], p->ni_m, p->Mm, t, true, p->raccm, p->ldm, g3)) != PPL_OK) return rc;
+                if ((rc = launch_step1t(p, &p->mapTm, &p->mapFWmT[sl_w], p->mg_m, p->Mm, t, true, p->raccm, p->ldm, g3)) != PPL_OK) return rc;
                 PPL_DBG("use 2 minus (k_step1t_tma)", k);
                 ++n2;
             }
@@ -1173,15 +1189,15 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
     const char *envk = getenv("PPL_KERNELS");  // debug override: "cpasync" forces the non-TMA kernels
     p->use_tma = !(envk && strcmp(envk, "cpasync") == 0) && get_encode() != nullptr;
     const char *envni = getenv("PPL_NI");  // debug override of the step-1 tile height
-    const int ni_env = (envni && atoi(envni) >= 5 && atoi(envni) <= 10) ? atoi(envni) : 0;
-    p->ni_full = ni_env ? ni_env : choose_ni(nocc * nocc);
-    p->ni_p = ni_env ? ni_env : choose_ni(p->Mp);
-    p->ni_m = ni_env ? ni_env : choose_ni(std::max(p->Mm, 1));
+    const int ni_env = (envni && atoi(envni) >= 1 && atoi(envni) <= 10) ? atoi(envni) : 10;  // largest instance used
     const bool tma_full = p->use_tma && p->vec16;
-    p->bm_full = tma_full ? 16 * p->ni_full : ppl::BM;
-    p->bm_p = p->use_tma ? 16 * p->ni_p : ppl::BM;
-    p->bm_m = p->use_tma ? 16 * p->ni_m : ppl::BM;
-    Geometry g{p->vv, nocc * nocc, p->Mp, p->Mm, p->Kp, p->Km, p->ldp, p->ldm, p->bm_full, p->bm_p, p->bm_m};
+    p->mg_full = tma_full ? m_geom_tma(nocc * nocc, ni_env) : m_geom_plain(nocc * nocc);
+    p->mg_p = p->use_tma ? m_geom_tma(p->Mp, ni_env) : m_geom_plain(p->Mp);
+    p->mg_m = p->use_tma ? m_geom_tma(std::max(p->Mm, 1), ni_env) : m_geom_plain(std::max(p->Mm, 1));
+    p->bm_full = tma_full ? 16 * p->mg_full.ni : ppl::BM;
+    p->bm_p = p->use_tma ? 16 * p->mg_p.ni : ppl::BM;
+    p->bm_m = p->use_tma ? 16 * p->mg_m.ni : ppl::BM;
+    Geometry g{p->vv, nocc * nocc, p->Mp, p->Mm, p->Kp, p->Km, p->ldp, p->ldm, p->mg_full, p->mg_p, p->mg_m};
     p->tau_bytes = align256((size_t)p->Mp * p->ldp * 8) + align256((size_t)std::max(p->Mm, 1) * p->ldm * 8);
 
     // choose the tile edge T (and ring depth) that minimises the estimated apply time under the cap:
@@ -1461,13 +1477,13 @@ int ppl_apply_dense(ppl_plan_t *p, const double *eri, int a0, int na, const doub
     t.mirror = 0;
     for (int64_t n0 = 0; n0 < rows; n0 += chunk) {
         const int N = (int)std::min<int64_t>(chunk, rows - n0);
-        const SplitChoice sc = choose_split(M, N, p->vv, p->num_sms, p->bm_full, p->part_bytes);
+        const SplitChoice sc = choose_split(M, N, p->vv, p->num_sms, p->mg_full, p->part_bytes);
         if ((size_t)sc.splitk * M * N * 8 > p->part_bytes) return fail(PPL_ERR_WORKSPACE_TOO_SMALL);
         const double *B = eri + n0 * p->vv;
         CUtensorMap mapB;  // the chunk's rows as their own tensor so that tile-edge rows beyond it read as zero
         if (tma && make_map_2d(&mapB, B, (uint64_t)p->vv, (uint64_t)N, (uint64_t)p->vv * 8, ppl::BK, ppl::BN) != PPL_OK)
             return fail(PPL_ERR_CUDA);
-        rc = launch_step1(p, tma ? &mapT : nullptr, tma ? &mapB : nullptr, p->ni_full, t2m, p->vv, B, p->vv, M, N, p->vv, sc,
+        rc = launch_step1(p, tma ? &mapT : nullptr, tma ? &mapB : nullptr, p->mg_full, t2m, p->vv, B, p->vv, M, N, p->vv, sc,
                           p->part, vec16, stream);
         if (rc == PPL_OK) rc = launch_reduce(p, t, sc.splitk, N, (int)n0, p->v, R, opts, stream);
         if (rc != PPL_OK) return rc;

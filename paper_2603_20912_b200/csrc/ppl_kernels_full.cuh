@@ -201,15 +201,65 @@ struct Step1TArgs {
     int nkt, kt_per_a;
     int A0, bg0, v;
     int minus;
+    MSplit ms;           // row tiling of M (ppl_kernels_tma.cuh)
     double *acc;         // [M][ld]
     int64_t ld;
 };
+
+// k loop of one work item of use 2 for a warp that owns NA 8-row blocks (see step1_consume)
+template <int NI, int NA>
+__device__ __forceinline__ void step1t_consume(double (&acc)[NI][2][2][2], const TmaSmem &sm, int as_off, int bs_off, int offa0, int offa1,
+                                               int offb_e0, int offb_e1, int nkt, int nact, int &stage, uint32_t &phase, int &rel_stage,
+                                               int lane) {
+    constexpr int BM1 = Step1Cfg<NI>::BM1;
+    for (int kt = 0; kt < nkt; ++kt) {
+        mbar_wait(&sm.full[stage], phase);
+        release_previous(sm, rel_stage, lane);
+        const double *as = sm.a + (size_t)stage * BM1 * BK + as_off;
+        const double *bs = sm.b + (size_t)stage * BN * BK + bs_off;
+#pragma unroll
+        for (int k8 = 0; k8 < BK / 8; ++k8) {
+            double2 a[NA > 0 ? NA : 1], b0[2], b1[2];
+#pragma unroll
+            for (int i = 0; i < NA; ++i)
+                a[i] = *reinterpret_cast<const double2 *>(as + i * 8 * BK + (k8 ? offa1 : offa0));
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                b0[j] = *reinterpret_cast<const double2 *>(bs + j * (BK * 16) + k8 * 128 + offb_e0);
+                b1[j] = *reinterpret_cast<const double2 *>(bs + j * (BK * 16) + k8 * 128 + offb_e1);
+            }
+#pragma unroll
+            for (int i = 0; i < NA; ++i)
+                {
+#pragma unroll
+                    for (int j = 0; j < 2; ++j) {
+                        dmma(acc[i][j][0][0], acc[i][j][0][1], a[i].x, b0[j].x);
+                        dmma(acc[i][j][1][0], acc[i][j][1][1], a[i].x, b0[j].y);
+                    }
+                }
+#pragma unroll
+            for (int i = 0; i < NA; ++i)
+                {
+#pragma unroll
+                    for (int j = 0; j < 2; ++j) {
+                        dmma(acc[i][j][0][0], acc[i][j][0][1], a[i].y, b1[j].x);
+                        dmma(acc[i][j][1][0], acc[i][j][1][1], a[i].y, b1[j].y);
+                    }
+                }
+        }
+        rel_stage = stage;
+        if (++stage == TSTAGES) {
+            stage = 0;
+            phase ^= 1;
+        }
+    }
+}
 
 template <int NI>
 __global__ void __launch_bounds__(TMA_THREADS, 1)
     k_step1t_tma(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, const Step1TArgs p) {
     using Cfg = Step1Cfg<NI>;
-    constexpr int BM1 = Cfg::BM1, WTM1 = Cfg::WTM1;
+    constexpr int BM1 = Cfg::BM1;
     extern __shared__ unsigned char smem_raw[];
     const uint32_t base = smem_u32(smem_raw);
     unsigned char *al = smem_raw + ((1024u - (base & 1023u)) & 1023u);
@@ -221,7 +271,7 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     init_barriers(sm, tid);
 
-    const int tiles_m = (p.M + BM1 - 1) / BM1, tiles_n = (p.n_end - p.n_base + BN - 1) / BN;
+    const int tiles_m = p.ms.tiles_m, tiles_n = (p.n_end - p.n_base + BN - 1) / BN;
     const int num_items = tiles_m * tiles_n;
 
     if (warp >= CONSUMER_WARPS) {
@@ -234,12 +284,14 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
             for (int item = blockIdx.x; item < num_items; item += gridDim.x) {
                 const int tm = item % tiles_m, tn = item / tiles_m;
                 const int n0 = p.n_base + tn * BN;
+                int row0, ni0, ni1;
+                m_tile(p.ms, tm, row0, ni0, ni1);
                 for (int kt = 0; kt < p.nkt; ++kt) {
                     const int a = p.A0 + kt / p.kt_per_a, b1 = p.bg0 + 16 * (kt % p.kt_per_a);
                     const int64_t kap = p.minus ? kminus(a, b1, p.v) : kplus(a, b1, p.v);  // even: b1 is a multiple of 16
                     mbar_wait(&sm.empty[stage], phase ^ 1);
                     mbar_expect_tx(&sm.full[stage], Cfg::STAGE);
-                    tma_load_2d(sm.a + (size_t)stage * BM1 * BK, &mapA, (int)kap, tm * BM1, &sm.full[stage]);
+                    tma_load_2d(sm.a + (size_t)stage * BM1 * BK, &mapA, (int)kap, row0, &sm.full[stage]);
                     double *db = sm.b + (size_t)stage * BN * BK;
 #pragma unroll
                     for (int i = 0; i < 8; ++i) tma_load_2d(db + i * BK * 16, &mapB, n0 + 16 * i, kt * BK, &sm.full[stage]);
@@ -265,8 +317,11 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
     int stage = 0, rel_stage = -1;
     uint32_t phase = 0;
     for (int item = blockIdx.x; item < num_items; item += gridDim.x) {
-        const int tm = item % tiles_m, tn = item / tiles_m;
-        const int m0 = tm * BM1, n0 = p.n_base + tn * BN;
+        const int tm = item % tiles_m;
+        int row0, ni0, ni1;
+        m_tile(p.ms, tm, row0, ni0, ni1);
+        const int nact = wm ? ni1 : ni0;
+        const int wrow = wm ? 8 * ni0 : 0;
         // acc[i][j2][f][h]: row m = 8i + c(g); h = 0 <-> n = 16 j2 + 4q + f, h = 1 <-> n = 16 j2 + 4q + 2 + f
         double acc[NI][2][2][2];
 #pragma unroll
@@ -274,52 +329,28 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
 #pragma unroll
             for (int j = 0; j < 2; ++j) acc[i][j][0][0] = acc[i][j][0][1] = acc[i][j][1][0] = acc[i][j][1][1] = 0.0;
 
-        for (int kt = 0; kt < p.nkt; ++kt) {
-            mbar_wait(&sm.full[stage], phase);
-            release_previous(sm, rel_stage, lane);
-            const double *as = sm.a + (size_t)stage * BM1 * BK + (wm * WTM1) * BK;
-            const double *bs = sm.b + (size_t)stage * BN * BK + (wn * 2) * (BK * 16);
-#pragma unroll
-            for (int k8 = 0; k8 < BK / 8; ++k8) {
-                double2 a[NI], b0[2], b1[2];
-#pragma unroll
-                for (int i = 0; i < NI; ++i) a[i] = *reinterpret_cast<const double2 *>(as + i * 8 * BK + (k8 ? offa1 : offa0));
-#pragma unroll
-                for (int j = 0; j < 2; ++j) {
-                    b0[j] = *reinterpret_cast<const double2 *>(bs + j * (BK * 16) + k8 * 128 + offb_e0);
-                    b1[j] = *reinterpret_cast<const double2 *>(bs + j * (BK * 16) + k8 * 128 + offb_e1);
-                }
-#pragma unroll
-                for (int i = 0; i < NI; ++i)
-#pragma unroll
-                    for (int j = 0; j < 2; ++j) {
-                        dmma(acc[i][j][0][0], acc[i][j][0][1], a[i].x, b0[j].x);
-                        dmma(acc[i][j][1][0], acc[i][j][1][1], a[i].x, b0[j].y);
-                    }
-#pragma unroll
-                for (int i = 0; i < NI; ++i)
-#pragma unroll
-                    for (int j = 0; j < 2; ++j) {
-                        dmma(acc[i][j][0][0], acc[i][j][0][1], a[i].y, b1[j].x);
-                        dmma(acc[i][j][1][0], acc[i][j][1][1], a[i].y, b1[j].y);
-                    }
-            }
-            rel_stage = stage;
-            if (++stage == TSTAGES) {
-                stage = 0;
-                phase ^= 1;
-            }
-        }
+        if (nact == NI)
+            step1t_consume<NI, NI>(acc, sm, wrow * BK, (wn * 2) * (BK * 16), offa0, offa1, offb_e0, offb_e1, p.nkt, nact, stage,
+                                          phase, rel_stage, lane);
+        else  // nact == NI - 1: the host's row tiling hands a warp NI or NI - 1 blocks, nothing else (m_geom_tma)
+            step1t_consume<NI, NI - 1>(acc, sm, wrow * BK, (wn * 2) * (BK * 16), offa0, offa1, offb_e0, offb_e1, p.nkt, nact,
+                                              stage, phase, rel_stage, lane);
         // epilogue: accumulate into the R+- matrix.  Every element belongs to exactly one item of this launch and
         // launches are ordered on the stream, so the sequence of additions per element is fixed (bit-reproducible);
         // the adds are issued as reductions (RED.ADD.F64, no return value): no load latency in the epilogue.
+        int it2 = item;  // tile coordinates derived again behind an opaque move: nothing of them stays live across the k loop
+        asm volatile("" : "+r"(it2));
+        int erow0, eni0, eni1;
+        m_tile(p.ms, it2 % tiles_m, erow0, eni0, eni1);
+        const int enact = wm ? eni1 : eni0, en0 = p.n_base + (it2 / tiles_m) * BN;
+        erow0 += wm ? 8 * eni0 : 0;
 #pragma unroll
         for (int i = 0; i < NI; ++i) {
-            const int m = m0 + wm * WTM1 + 8 * i + c;
-            if (m >= p.M) continue;
+            const int m = erow0 + 8 * i + c;
+            if (i >= enact || m >= p.M) continue;
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
-                const int n = n0 + wn * WTN + 16 * j + 4 * q;  // multiple of 4; rows are 128-byte aligned
+                const int n = en0 + wn * WTN + 16 * j + 4 * q;  // multiple of 4; rows are 128-byte aligned
                 double *dst = p.acc + (int64_t)m * p.ld + n;
                 const double vals[4] = {acc[i][j][0][0], acc[i][j][1][0], acc[i][j][0][1], acc[i][j][1][1]};
 #pragma unroll

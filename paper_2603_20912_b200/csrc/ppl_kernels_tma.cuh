@@ -249,32 +249,86 @@ __global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_tma(const __grid_const
 // step 1 (TMA):  part[z][(i,j)][(a,b)] = sum_{(c,d) in split z} t2[(i,j)][(c,d)] W[(a,b)][(c,d)]
 // mapA: t2 as {inner = nvirt^2, outer = nocc^2}, box {16, 16*NI};  mapB: W slot as {inner = nvirt^2,
 // outer = T*T}, box {16, 128}; SWIZZLE_128B.
-// NI = 8-row blocks per warp along M: CTA tile (16*NI) x 128.  nocc^2 is rarely a multiple of 128
-// (1600, 3600, 400), and rows padded up to a tile are DMMA work that counts for nothing; the host
-// picks NI in 5..10 that tiles nocc^2 with the least padding (160 | 1600, 144 | 3600, 80 | 400).
+// NI = maximum number of 8-row blocks per warp along M (TMA box of A: 16*NI rows); see MSplit below.
 // ---------------------------------------------------------------------------------------------
+// Rows of the M side (nocc^2, or the packed (i<=j) / (i<j) rows) are cut into 8-row blocks and dealt to 2*tiles_m
+// "half-tiles" -- the two warp rows of a CTA tile -- of `base` or `base + 1` blocks (the first `rem` get the extra one).
+// nocc^2-like extents are rarely a multiple of a CTA tile height (820, 780, 1830, 210 ...): with uniform tiles of
+// 16*NI rows the padding was 3-5 % of the DMMA work of step 1; this way it is < 8 rows in all.  Each SMSP hosts one
+// warp of either warp row, so a CTA tile costs ni0 + ni1 blocks on every SMSP: tiles differ by at most 2 in 2*NI.
+struct MSplit {
+    int tiles_m, base, rem;
+};
+__device__ __forceinline__ void m_tile(const MSplit &g, int tm, int &row0, int &ni0, int &ni1) {
+    const int h = 2 * tm;
+    ni0 = g.base + (h < g.rem ? 1 : 0);
+    ni1 = g.base + (h + 1 < g.rem ? 1 : 0);
+    row0 = 8 * (h * g.base + min(h, g.rem));
+}
+
 struct Step1TmaArgs {
     int M, N, K;      // nocc^2, ta*tb, nvirt^2 (K = END of the contraction range)
     int k0;           // first k of the contraction range (0 except in PPL_SYM_FULL; any value: TMA boxes may start anywhere)
     int k_per_split;  // multiple of BK
     int splitk;
+    MSplit ms;
     double *part;     // [splitk][M][N]
 };
 
 template <int NI>
 struct Step1Cfg {
-    static constexpr int BM1 = 16 * NI;                                   // CTA tile rows
-    static constexpr int WTM1 = 8 * NI;                                   // warp tile rows
+    static constexpr int BM1 = 16 * NI;                                   // CTA tile rows (TMA box; a tile uses 8*(ni0+ni1) of them)
     static constexpr uint32_t A_BYTES = BM1 * BK * sizeof(double);
     static constexpr uint32_t STAGE = A_BYTES + TILE_BYTES;               // A + B(128 x 16)
     static constexpr size_t SMEM = (size_t)TSTAGES * STAGE + 1024 + 256;
 };
 
+// The k loop of one work item of step 1 for a warp that owns NA (= NI or NI - 1) 8-row blocks.
+// as_off / bs_off: the warp's first row inside the A / B stage tile.
+template <int NI, int NA>
+__device__ __forceinline__ void step1_consume(double (&acc)[NI][4][2], const TmaSmem &sm, int as_off, int bs_off, int off0, int off1,
+                                              int nkt, int nact, int &stage, uint32_t &phase, int &rel_stage, int lane) {
+    constexpr int BM1 = Step1Cfg<NI>::BM1;
+    for (int kt = 0; kt < nkt; ++kt) {
+        mbar_wait(&sm.full[stage], phase);
+        release_previous(sm, rel_stage, lane);
+        const double *as = sm.a + (size_t)stage * BM1 * BK + as_off;
+        const double *bs = sm.b + (size_t)stage * BN * BK + bs_off;
+#pragma unroll
+        for (int k8 = 0; k8 < BK / 8; ++k8) {
+            const int off = k8 ? off1 : off0;
+            double2 a[NA > 0 ? NA : 1], b[4];
+#pragma unroll
+            for (int i = 0; i < NA; ++i)
+                a[i] = *reinterpret_cast<const double2 *>(as + i * 8 * BK + off);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) b[j] = *reinterpret_cast<const double2 *>(bs + j * 8 * BK + off);
+#pragma unroll
+            for (int i = 0; i < NA; ++i)
+                {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i].x, b[j].x);
+                }
+#pragma unroll
+            for (int i = 0; i < NA; ++i)
+                {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i].y, b[j].y);
+                }
+        }
+        rel_stage = stage;  // released after the NEXT stage's wait (see release_previous)
+        if (++stage == TSTAGES) {
+            stage = 0;
+            phase ^= 1;
+        }
+    }
+}
+
 template <int NI>
 __global__ void __launch_bounds__(TMA_THREADS, 1)
     k_step1_tma(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, const Step1TmaArgs p) {
     using Cfg = Step1Cfg<NI>;
-    constexpr int BM1 = Cfg::BM1, WTM1 = Cfg::WTM1;
+    constexpr int BM1 = Cfg::BM1;
     extern __shared__ unsigned char smem_raw[];
     // ring: [TSTAGES] A tiles, then [TSTAGES] B tiles, then the barriers
     const uint32_t base = smem_u32(smem_raw);
@@ -287,7 +341,7 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     init_barriers(sm, tid);
 
-    const int tiles_m = (p.M + BM1 - 1) / BM1, tiles_n = (p.N + BN - 1) / BN;
+    const int tiles_m = p.ms.tiles_m, tiles_n = (p.N + BN - 1) / BN;
     const int tiles_mn = tiles_m * tiles_n;
     const int num_items = tiles_mn * p.splitk;
 
@@ -301,11 +355,13 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
             for (int item = blockIdx.x; item < num_items; item += gridDim.x) {
                 const int z = item / tiles_mn, r = item - z * tiles_mn;
                 const int tm = r % tiles_m, tn = r / tiles_m;
+                int row0, ni0, ni1;
+                m_tile(p.ms, tm, row0, ni0, ni1);
                 const int kbeg = p.k0 + z * p.k_per_split, kend = min(p.K, kbeg + p.k_per_split);
                 for (int k = kbeg; k < kend; k += BK) {
                     mbar_wait(&sm.empty[stage], phase ^ 1);
                     mbar_expect_tx(&sm.full[stage], Cfg::STAGE);
-                    tma_load_2d(sm.a + (size_t)stage * BM1 * BK, &mapA, k, tm * BM1, &sm.full[stage]);
+                    tma_load_2d(sm.a + (size_t)stage * BM1 * BK, &mapA, k, row0, &sm.full[stage]);
                     tma_load_2d(sm.b + (size_t)stage * BN * BK, &mapB, k, tn * BN, &sm.full[stage]);
                     if (++stage == TSTAGES) {
                         stage = 0;
@@ -327,52 +383,42 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
     uint32_t phase = 0;
     for (int item = blockIdx.x; item < num_items; item += gridDim.x) {
         const int z = item / tiles_mn, r = item - z * tiles_mn;
-        const int tm = r % tiles_m, tn = r / tiles_m;
-        const int m0 = tm * BM1, n0 = tn * BN;
+        const int tm = r % tiles_m;
+        int row0, ni0, ni1;
+        m_tile(p.ms, tm, row0, ni0, ni1);
+        const int nact = wm ? ni1 : ni0;          // 8-row blocks of this warp
+        const int wrow = wm ? 8 * ni0 : 0;        // its first row inside the CTA tile
         const int kbeg = p.k0 + z * p.k_per_split, kend = min(p.K, kbeg + p.k_per_split);
+        const int nkt = max(0, (kend - kbeg + BK - 1) / BK);
         double acc[NI][4][2];
 #pragma unroll
         for (int i = 0; i < NI; ++i)
 #pragma unroll
             for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-        for (int k = kbeg; k < kend; k += BK) {
-            mbar_wait(&sm.full[stage], phase);
-            release_previous(sm, rel_stage, lane);
-            const double *as = sm.a + (size_t)stage * BM1 * BK + (wm * WTM1) * BK;
-            const double *bs = sm.b + (size_t)stage * BN * BK + (wn * WTN) * BK;
-#pragma unroll
-            for (int k8 = 0; k8 < BK / 8; ++k8) {
-                const int off = k8 ? off1 : off0;
-                double2 a[NI], b[4];
-#pragma unroll
-                for (int i = 0; i < NI; ++i) a[i] = *reinterpret_cast<const double2 *>(as + i * 8 * BK + off);
-#pragma unroll
-                for (int j = 0; j < 4; ++j) b[j] = *reinterpret_cast<const double2 *>(bs + j * 8 * BK + off);
-#pragma unroll
-                for (int i = 0; i < NI; ++i)
-#pragma unroll
-                    for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i].x, b[j].x);
-#pragma unroll
-                for (int i = 0; i < NI; ++i)
-#pragma unroll
-                    for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i].y, b[j].y);
-            }
-            rel_stage = stage;  // released after the NEXT stage's wait (see release_previous)
-            if (++stage == TSTAGES) {
-                stage = 0;
-                phase ^= 1;
-            }
-        }
-        // epilogue: block (i,j): frag row g <-> m = mw + 8i + c(g); c0 <-> n = nw + 8j + q, c1 <-> n + 4
-        double *part = p.part + (int64_t)z * p.M * p.N;
+        if (nact == NI)
+            step1_consume<NI, NI>(acc, sm, wrow * BK, (wn * WTN) * BK, off0, off1, nkt, nact, stage, phase, rel_stage, lane);
+        else  // nact == NI - 1: the host's row tiling hands a warp NI or NI - 1 blocks, nothing else (m_geom_tma)
+            step1_consume<NI, NI - 1>(acc, sm, wrow * BK, (wn * WTN) * BK, off0, off1, nkt, nact, stage, phase, rel_stage, lane);
+
+        // epilogue: block (i,j): frag row g <-> m = row0 + wrow + 8i + c(g); c0 <-> n = nw + 8j + q, c1 <-> n + 4
+        // (the tile coordinates are derived again from the item number behind an opaque move, so that none of them
+        // stays live across the k loop: the NI = 10 instance has no register to spare)
+        int it2 = item;
+        asm volatile("" : "+r"(it2));
+        const int z2 = it2 / tiles_mn, r2 = it2 - z2 * tiles_mn;
+        int erow0, eni0, eni1;
+        m_tile(p.ms, r2 % tiles_m, erow0, eni0, eni1);
+        const int enact = wm ? eni1 : eni0, en0 = (r2 / tiles_m) * BN;
+        erow0 += wm ? 8 * eni0 : 0;
+        double *part = p.part + (int64_t)z2 * p.M * p.N;
 #pragma unroll
         for (int i = 0; i < NI; ++i) {
-            const int m = m0 + wm * WTM1 + 8 * i + c;
-            if (m >= p.M) continue;
+            const int m = erow0 + 8 * i + c;
+            if (i >= enact || m >= p.M) continue;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
-                const int n = n0 + wn * WTN + 8 * j + q;
+                const int n = en0 + wn * WTN + 8 * j + q;
                 double *dst = part + (int64_t)m * p.N + n;
                 if (n < p.N) dst[0] = acc[i][j][0];
                 if (n + 4 < p.N) dst[4] = acc[i][j][1];
