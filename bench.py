@@ -276,7 +276,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workspace-gb", type=float, default=0.0, help="workspace cap (0 = auto)")
     ap.add_argument("--symmetry", default="default", choices=["default", "full", "pair_sa", "pair", "none"],
-                    help="default = the plan's own choice (full: 8-fold ERI symmetry + pair symmetry, from nvirt = 96 up)")
+                    help="default = the plan's own choice (full: 8-fold ERI symmetry + pair symmetry, from nvirt = 52 up)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -77,7 +77,7 @@ enum {
                          a plan-owned [nchol][nvirt+1][nvirt+1] buffer with a zero pad row / column,
                          the pad index of the packed operands carries exact zeros and never reaches R.  Its
                          buffers (a 16 x nvirt^3 strip and the R+- accumulators) are allocated by ppl_plan when
-                         they fit under the workspace cap.  Default when available and nvirt >= 96. */
+                         they fit under the workspace cap.  Default when available and nvirt >= 52. */
 };
 
 /* Storage orders of the 4-index arrays t2 and R. */
@@ -201,7 +201,7 @@ int ppl_last_error(void);                /* code of the last failure on this thr
 const char *ppl_error_string(int code);  /* static string, never NULL */
 
 /* Set PPL_SYM_NONE / PPL_SYM_PAIR / PPL_SYM_PAIR_SA / PPL_SYM_FULL.  Default: PPL_SYM_FULL when its
- * buffers fit and nvirt >= 96, else PPL_SYM_PAIR_SA, else PPL_SYM_PAIR if the workspace cap
+ * buffers fit and nvirt >= 52, else PPL_SYM_PAIR_SA, else PPL_SYM_PAIR if the workspace cap
  * was too small for the packed operands.  PPL_ERR_WORKSPACE_TOO_SMALL if the plan holds no buffers for
  * the requested mode.  Re-plans the tile list; must not be called while an apply is in flight. */
 int ppl_plan_set_symmetry(ppl_plan_t *plan, int mode);

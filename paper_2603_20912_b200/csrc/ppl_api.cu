@@ -1316,11 +1316,13 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
         fail(rc);
         return nullptr;
     }
-    // PPL_SYM_FULL: its buffers are allocated when they fit under the cap; it is the default from nvirt = 96 up
-    // (below that the extra launches per slab cost more than the flops they save)
+    // PPL_SYM_FULL: its buffers are allocated when they fit under the cap; it is the default from nvirt = 52 up
+    // (below that the extra launches per slab cost more than the flops they save: measured crossover with
+    // PPL_SYM_PAIR_SA at nocc = 5..8, nchol = 4 nvirt: 0.157 vs 0.186 ms at nvirt = 48, 0.283 vs 0.274 ms at 53,
+    // 0.365 vs 0.328 ms at 64, 1.71 vs 0.97 ms at 96)
     full_setup(p, cap > p->ws_bytes ? cap - p->ws_bytes : 0);
     const char *envf = getenv("PPL_FULL_MIN_V");  // debug override
-    const int full_min_v = envf ? atoi(envf) : 96;
+    const int full_min_v = envf ? atoi(envf) : 52;
     if (p->full_ok && nvirt >= full_min_v) p->sym = PPL_SYM_FULL;
     return p;
 }

@@ -93,7 +93,7 @@ def test_full_mode_accumulates_and_handles_layouts_alpha_beta(nvirt):
 def test_full_mode_preconditions_default_and_availability():
     import torch
 
-    # default: PPL_SYM_FULL from nvirt = 96 up (odd nvirt included: padded geometry), PPL_SYM_PAIR_SA below
+    # default: PPL_SYM_FULL from nvirt = 52 up (odd nvirt included: padded geometry), PPL_SYM_PAIR_SA below
     with P.Plan(3, 96, 8) as plan:
         assert plan.info()["symmetry"] == P.PPL_SYM_FULL
     with P.Plan(3, 40, 8) as plan:
@@ -103,6 +103,9 @@ def test_full_mode_preconditions_default_and_availability():
         info = plan.info()
         assert info["symmetry"] == P.PPL_SYM_FULL and info["full_available"] == 1 and info["nvirt"] == 97
     with P.Plan(3, 53, 8) as plan:
+        info = plan.info()
+        assert info["symmetry"] == P.PPL_SYM_FULL and info["full_available"] == 1
+    with P.Plan(3, 51, 8) as plan:
         info = plan.info()
         assert info["symmetry"] == P.PPL_SYM_PAIR_SA and info["full_available"] == 1
     # a cap that holds the PPL_SYM_PAIR_SA plan but not the 16 x nvirt^3 strip: the plan falls back

@@ -35,7 +35,7 @@ def _host_gb():
 
 
 def _run(name, integer=False, sym=None):
-    """sym=None: the plan's default, which is what bench.py times (PPL_SYM_FULL from nvirt = 96 up)."""
+    """sym=None: the plan's default, which is what bench.py times (PPL_SYM_FULL from nvirt = 52 up)."""
     import torch
 
     o, v, x = I.CONFIGS[name]
