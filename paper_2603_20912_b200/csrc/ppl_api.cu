@@ -113,6 +113,8 @@ struct ppl_plan_s {
     double *dL = nullptr, *dT = nullptr, *dR = nullptr;  // ppl_apply_host staging
     double *hstage[2] = {nullptr, nullptr};              // ppl_apply_host in PPL_SYM_FULL: two chunk buffers for t2 / R
     int hchunk_rows = 0;                                 // (i,j) rows per chunk
+    cudaStream_t hs2 = nullptr;                          // second chunk stream of ppl_apply_host (the first is `gen`)
+    cudaEvent_t ev_tau = nullptr, ev_done = nullptr;     // tau+- complete / all slabs done
     double f_step0 = 0, f_step1 = 0;
     CUtensorMap mapW[MAX_RING], mapWp[MAX_RING], mapWm[MAX_RING], mapTp, mapTm;  // plan-owned operands
     // ---- PPL_SYM_FULL (own allocation `fws`; shares taup/taum with PPL_SYM_PAIR_SA) ----
@@ -289,6 +291,12 @@ void free_plan(ppl_plan_s *p) {
         cudaStreamDestroy(p->host_stream);
     }
     if (p->ev_in) cudaEventDestroy(p->ev_in);
+    if (p->hs2) {
+        cudaStreamSynchronize(p->hs2);
+        cudaStreamDestroy(p->hs2);
+    }
+    if (p->ev_tau) cudaEventDestroy(p->ev_tau);
+    if (p->ev_done) cudaEventDestroy(p->ev_done);
     for (int i = 0; i < 4; ++i)
         if (p->fs[i]) {
             cudaStreamSynchronize(p->fs[i]);
@@ -936,8 +944,10 @@ int launch_unpack_full(const ppl_plan_s *p, const ppl_opts_t &opts, double *R, i
 
 // phases: FULL_PACK (t2 -> tau+-, clear R+-acc), FULL_COMPUTE (all slabs), FULL_UNPACK (R+-acc -> R).  ppl_apply runs all
 // three; ppl_apply_host packs and unpacks chunk by chunk itself and calls this with FULL_COMPUTE only (t2, R unused).
+// tau_ready (ppl_apply_host): tau+- are being packed on other streams; step 0 of the first slab needs only L and starts at
+// once, the event is waited for behind it.
 int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, const ppl_opts_t *opts_in, cudaStream_t stream,
-                   Prof *prof, int phases = FULL_ALL) {
+                   Prof *prof, int phases = FULL_ALL, cudaEvent_t tau_ready = nullptr) {
     bool vec16 = false;
     int rc = check_ptrs(p, L, (phases & FULL_PACK) ? t2 : L, (phases & FULL_UNPACK) ? R : L, &vec16);
     ppl_opts_t opts;
@@ -995,6 +1005,7 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
         PPL_CUDA(cudaGetLastError());
         PPL_DBG("k_step0_slab", sl.A0);
         PPL_MARK(K_STEP0, 1);
+        if (tau_ready && sl.A0 == 0) PPL_CUDA(cudaStreamWaitEvent(stream, tau_ready, 0));
         for (int k = sl.tile_begin; k < sl.tile_end; ++k) {
             const FullTile &t = p->ftiles[k];
             const int N = TA * t.tbp;
@@ -1522,13 +1533,25 @@ static int apply_host_full(ppl_plan_s *p, const double *Lh, const double *t2h, d
                 return fail(PPL_ERR_ALLOC);
             }
     }
-    cudaStream_t st[2] = {p->host_stream, p->gen};
+    if (!p->hs2) {
+        bool ok = cudaStreamCreateWithFlags(&p->hs2, cudaStreamNonBlocking) == cudaSuccess;
+        ok = ok && cudaEventCreateWithFlags(&p->ev_tau, cudaEventDisableTiming) == cudaSuccess;
+        ok = ok && cudaEventCreateWithFlags(&p->ev_done, cudaEventDisableTiming) == cudaSuccess;
+        if (!ok) {
+            (void)cudaGetLastError();
+            return fail(PPL_ERR_CUDA);
+        }
+    }
+    cudaStream_t cs = p->host_stream;         // L in, all slabs
+    cudaStream_t st[2] = {p->gen, p->hs2};    // chunk k of t2 / R on stream k % 2; each stream owns one staging buffer
     const bool minus = p->Mm > 0 && p->Km > 0;
     ppl_opts_t opts;
     check_opts(nullptr, &opts);
-    // phase A: L in; t2 chunks in -> tau+- (chunk k on stream k % 2, each stream owns one staging buffer)
-    PPL_CUDA(cudaMemsetAsync(p->raccp, 0, (size_t)p->Mp * p->ldp * 8, st[1]));
-    if (minus) PPL_CUDA(cudaMemsetAsync(p->raccm, 0, (size_t)p->Mm * p->ldm * 8, st[1]));
+    const int64_t nchunks = (rows + p->hchunk_rows - 1) / p->hchunk_rows;
+    // phase A: L in on the compute stream; t2 chunks in -> tau+- on the chunk streams, overlapping L and step 0 of slab 0
+    PPL_CUDA(cudaMemcpyAsync(p->dL, Lh, nL, cudaMemcpyHostToDevice, cs));
+    PPL_CUDA(cudaMemsetAsync(p->raccp, 0, (size_t)p->Mp * p->ldp * 8, cs));
+    if (minus) PPL_CUDA(cudaMemsetAsync(p->raccm, 0, (size_t)p->Mm * p->ldm * 8, cs));
     int k = 0;
     for (int64_t r0 = 0; r0 < rows; r0 += p->hchunk_rows, ++k) {
         const int64_t r1 = std::min<int64_t>(rows, r0 + p->hchunk_rows);
@@ -1538,27 +1561,37 @@ static int apply_host_full(ppl_plan_s *p, const double *Lh, const double *t2h, d
         const int rc = launch_pack(p, buf - r0 * p->vv, PPL_LAYOUT_IJAB, 0.5, s, (int)r0, (int)r1);
         if (rc != PPL_OK) return rc;
     }
-    PPL_CUDA(cudaMemcpyAsync(p->dL, Lh, nL, cudaMemcpyHostToDevice, st[0]));
     PPL_CUDA(cudaEventRecord(p->ev_in, st[1]));
     PPL_CUDA(cudaStreamWaitEvent(st[0], p->ev_in, 0));
+    PPL_CUDA(cudaEventRecord(p->ev_tau, st[0]));
+    // the first two R chunks travel to the (now free) staging buffers while the slabs run
+    auto r_chunk_in = [&](int64_t kk) -> int {
+        const int64_t r0 = kk * p->hchunk_rows, r1 = std::min<int64_t>(rows, r0 + p->hchunk_rows);
+        PPL_CUDA(cudaMemcpyAsync(p->hstage[kk & 1], Rh + r0 * p->vv, (size_t)(r1 - r0) * row_bytes, cudaMemcpyHostToDevice, st[kk & 1]));
+        return PPL_OK;
+    };
+    int rc = PPL_OK;
+    for (int64_t kk = 0; kk < std::min<int64_t>(2, nchunks); ++kk)
+        if ((rc = r_chunk_in(kk)) != PPL_OK) return rc;
     // phase B: all slabs on the packed operands
-    int rc = run_apply_full(p, p->dL, nullptr, nullptr, nullptr, st[0], nullptr, FULL_COMPUTE);
+    rc = run_apply_full(p, p->dL, nullptr, nullptr, nullptr, cs, nullptr, FULL_COMPUTE, p->ev_tau);
     if (rc != PPL_OK) return rc;
-    PPL_CUDA(cudaEventRecord(p->ev_in, st[0]));
-    PPL_CUDA(cudaStreamWaitEvent(st[1], p->ev_in, 0));
-    // phase C: R chunk in, R += term, R chunk out
-    k = 0;
-    for (int64_t r0 = 0; r0 < rows; r0 += p->hchunk_rows, ++k) {
-        const int64_t r1 = std::min<int64_t>(rows, r0 + p->hchunk_rows);
-        cudaStream_t s = st[k & 1];
-        double *buf = p->hstage[k & 1];
+    PPL_CUDA(cudaEventRecord(p->ev_done, cs));
+    PPL_CUDA(cudaStreamWaitEvent(st[0], p->ev_done, 0));
+    PPL_CUDA(cudaStreamWaitEvent(st[1], p->ev_done, 0));
+    // phase C: R chunk in (the first two are there already), R += term, R chunk out
+    for (int64_t kk = 0; kk < nchunks; ++kk) {
+        const int64_t r0 = kk * p->hchunk_rows, r1 = std::min<int64_t>(rows, r0 + p->hchunk_rows);
+        cudaStream_t s = st[kk & 1];
+        double *buf = p->hstage[kk & 1];
         const size_t bytes = (size_t)(r1 - r0) * row_bytes;
-        PPL_CUDA(cudaMemcpyAsync(buf, Rh + r0 * p->vv, bytes, cudaMemcpyHostToDevice, s));
+        if (kk >= 2 && (rc = r_chunk_in(kk)) != PPL_OK) return rc;
         if ((rc = launch_unpack_full(p, opts, buf - r0 * p->vv, r0 * p->vv, r1 * p->vv, s)) != PPL_OK) return rc;
         PPL_CUDA(cudaMemcpyAsync(Rh + r0 * p->vv, buf, bytes, cudaMemcpyDeviceToHost, s));
     }
     PPL_CUDA(cudaStreamSynchronize(st[0]));
     PPL_CUDA(cudaStreamSynchronize(st[1]));
+    PPL_CUDA(cudaStreamSynchronize(cs));
     const uint64_t nT = (uint64_t)rows * row_bytes;
     if (h2d) *h2d = (uint64_t)nL + 2 * nT;
     if (d2h) *d2h = nT;
