@@ -277,6 +277,8 @@ def main():
     ap.add_argument("--workspace-gb", type=float, default=0.0, help="workspace cap (0 = auto)")
     ap.add_argument("--symmetry", default="default", choices=["default", "full", "pair_sa", "pair", "none"],
                     help="default = the plan's own choice (full: 8-fold ERI symmetry + pair symmetry, from nvirt = 52 up)")
+    ap.add_argument("--graph", default="auto", choices=["auto", "on", "off"],
+                    help="ppl_plan_set_graph: replay one CUDA graph per apply (auto: launch-bound shapes only)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -332,6 +334,7 @@ def main():
     plan_s = time.perf_counter() - t0
     if args.symmetry != "default":
         plan.set_symmetry({v_: k_ for k_, v_ in SYM_NAMES.items()}[args.symmetry])
+    plan.set_graph({"auto": -1, "off": 0, "on": 1}[args.graph])
     info = plan.info()
     stream = torch.cuda.current_stream()
 
@@ -400,7 +403,8 @@ def main():
         "config": {"workload": args.config, "nocc": o, "nvirt": v, "nchol": x, "seed": 0,
                    "symmetry": SYM_DESC[info["symmetry"]], "parallelism": "replicas only" if world > 1 else "1 gpu",
                    "l2": "inputs larger than L2 (L, t2, W tiles >> 126 MB); no flush needed",
-                   "plan": {k: info[k] for k in ("ta", "tb", "n_tiles", "ring", "splitk", "vec16", "workspace_bytes")}},
+                   "plan": {k: info[k] for k in ("ta", "tb", "n_tiles", "ring", "splitk", "vec16", "workspace_bytes")},
+                   "graph": args.graph},
         "seconds_per_call": ms_per_step * 1e-3,
         "tflops_executed": f_exec / (ms_per_step * 1e-3) * 1e-12,
         "tflops_nominal_effective": f_nom / (ms_per_step * 1e-3) * 1e-12,

@@ -206,6 +206,15 @@ const char *ppl_error_string(int code);  /* static string, never NULL */
  * the requested mode.  Re-plans the tile list; must not be called while an apply is in flight. */
 int ppl_plan_set_symmetry(ppl_plan_t *plan, int mode);
 
+/* CUDA graph of one apply.  mode 1: ppl_apply / ppl_apply_ex capture the whole apply (all kernels, the forks and
+ * joins of the plan's side streams) once into a CUDA graph and replay it with one cudaGraphLaunch on `stream`
+ * for as long as (L, t2, R, opts, symmetry mode) stay the same; any change re-captures.  mode 0: plain launches.
+ * mode -1 (default): graph when the plan's executed flops are below 5e9 (launch-bound shapes: tiny, small),
+ * plain launches above.  If the caller is itself capturing `stream`, the plain launches are issued (and land in
+ * the caller's graph) whatever the mode.  ppl_apply_dense, ppl_apply_host and ppl_apply_profiled never use it.
+ * Same results bit for bit: the graph holds the same kernels with the same arguments in the same order. */
+int ppl_plan_set_graph(ppl_plan_t *plan, int mode);
+
 int ppl_plan_info(const ppl_plan_t *plan, ppl_info_t *out);
 
 /* Debug: verify on the device that L[P,a,c]==L[P,c,a] (required in PPL_SYM_FULL, else only reported)

@@ -82,6 +82,7 @@ SYMBOLS = {
     "ppl_last_error": (c_int, []),
     "ppl_error_string": (c_char_p, [c_int]),
     "ppl_plan_set_symmetry": (c_int, [c_void_p, c_int]),
+    "ppl_plan_set_graph": (c_int, [c_void_p, c_int]),
     "ppl_plan_info": (c_int, [c_void_p, POINTER(ppl_info_t)]),
     "ppl_check_inputs": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, POINTER(c_int)]),
     "ppl_probe_fp64_peak": (c_int, [POINTER(c_double), c_int, c_double]),
@@ -213,6 +214,10 @@ class Plan:
 
     def set_symmetry(self, mode: int):
         _check(lib().ppl_plan_set_symmetry(self._h, int(mode)), "ppl_plan_set_symmetry")
+
+    def set_graph(self, mode: int):
+        """-1 auto (default), 0 plain launches, 1 replay one CUDA graph per (L, t2, R, opts) key."""
+        _check(lib().ppl_plan_set_graph(self._h, int(mode)), "ppl_plan_set_graph")
 
     def info(self) -> dict:
         out = ppl_info_t()

@@ -71,6 +71,7 @@ struct FullSlab {
 constexpr int MAX_RING = 4;
 constexpr double PEAK_FLOPS = 37.2e12;  // nominal FP64 (148 SM x 64 FMA/clk x 2 x 1.965 GHz); planner cost model only
 constexpr double HBM_BPS = 6.0e12;      // planner cost model only
+constexpr double GRAPH_AUTO_FLOPS = 5.0e9;   // ppl_plan_set_graph(-1): measured -- tiny 47.7 -> 37.9 us, small (1.7e9) 270 -> 231 us with the graph; (10,100,400) (2.8e10) 1.44 -> 1.51 ms, medium 26.1 -> 26.8 ms without
 constexpr double LAUNCH_S = 4e-6;
 
 size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
@@ -136,6 +137,16 @@ struct ppl_plan_s {
     cudaStream_t fs[4] = {nullptr, nullptr, nullptr, nullptr};  // side streams of the four step-1 GEMMs of a tile
     cudaEvent_t ev_fold[2] = {nullptr, nullptr}, evg[2][4] = {};
     CUtensorMap mapFWp[2], mapFWm[2], mapFWpT[2], mapFWmT[2];  // the W+- tile as the B operand of use 1 (box 16 x 128 rows) / use 2 (box 16 x 16 rows)
+    // ---- CUDA graph of one apply (launch-bound shapes; ppl_plan_set_graph) ----
+    int graph_mode = -1;                       // -1: auto (graph when the executed flops are below GRAPH_AUTO_FLOPS), 0: off, 1: on
+    cudaStream_t gcap = nullptr;               // capture origin (never the caller's stream: the legacy stream cannot capture)
+    cudaGraphExec_t gexec = nullptr;           // the instantiated apply for the key below
+    struct GraphKey {
+        const double *L = nullptr, *t2 = nullptr;
+        double *R = nullptr;
+        ppl_opts_t opts = {0, 0, 0.0, 0.0};
+        int sym = -1;
+    } gkey;
 };
 
 namespace {
@@ -291,6 +302,8 @@ void free_plan(ppl_plan_s *p) {
         cudaStreamDestroy(p->host_stream);
     }
     if (p->ev_in) cudaEventDestroy(p->ev_in);
+    if (p->gexec) cudaGraphExecDestroy(p->gexec);
+    if (p->gcap) cudaStreamDestroy(p->gcap);
     if (p->hs2) {
         cudaStreamSynchronize(p->hs2);
         cudaStreamDestroy(p->hs2);
@@ -1422,9 +1435,86 @@ int ppl_apply(ppl_plan_t *p, const double *L, const double *t2, double *R, void 
     return ppl_apply_ex(p, L, t2, R, nullptr, stream);
 }
 
-int ppl_apply_ex(ppl_plan_t *p, const double *L, const double *t2, double *R, const ppl_opts_t *opts, void *stream) {
-    if (p && p->sym == PPL_SYM_FULL) return run_apply_full(p, L, t2, R, opts, reinterpret_cast<cudaStream_t>(stream), nullptr);
-    return run_apply(p, L, t2, R, opts, reinterpret_cast<cudaStream_t>(stream), nullptr);
+namespace {
+
+int apply_direct(ppl_plan_s *p, const double *L, const double *t2, double *R, const ppl_opts_t *opts, cudaStream_t stream) {
+    if (p && p->sym == PPL_SYM_FULL) return run_apply_full(p, L, t2, R, opts, stream, nullptr);
+    return run_apply(p, L, t2, R, opts, stream, nullptr);
+}
+
+// Launch-bound shapes (tiny: 6 launches of a few microseconds; small: 33 launches, 4 side streams and
+// ~60 event operations for 46 us of DMMA work): the whole apply -- forks and joins of the side streams
+// included -- is captured once into a CUDA graph, keyed on the three pointers, the options and the
+// symmetry mode, and replayed with one cudaGraphLaunch while the key stays the same (a CCSD iteration
+// calls the ladder on the same buffers).  A new key re-captures (the TMA descriptors of L and t2 are
+// kernel parameters, so the nodes cannot simply be re-pointed).
+bool graph_wanted(const ppl_plan_s *p) {
+    if (p->graph_mode >= 0) return p->graph_mode == 1;
+    const double f = p->sym == PPL_SYM_FULL ? p->ff_step0 + p->ff_step1 : p->f_step0 + p->f_step1;
+    return f < GRAPH_AUTO_FLOPS;
+}
+
+int apply_graph(ppl_plan_s *p, const double *L, const double *t2, double *R, const ppl_opts_t *opts_in, cudaStream_t stream) {
+    ppl_opts_t opts;
+    bool vec16;
+    int rc = check_ptrs(p, L, t2, R, &vec16);
+    if (rc == PPL_OK) rc = check_opts(opts_in, &opts);
+    if (rc != PPL_OK) return fail(rc);
+    const ppl_plan_s::GraphKey &k = p->gkey;
+    const bool hit = p->gexec && k.L == L && k.t2 == t2 && k.R == R && k.sym == p->sym && k.opts.t2_layout == opts.t2_layout &&
+                     k.opts.r_layout == opts.r_layout && k.opts.alpha == opts.alpha && k.opts.beta == opts.beta;
+    if (!hit) {
+        if (p->gexec) {
+            cudaGraphExecDestroy(p->gexec);
+            p->gexec = nullptr;
+        }
+        if (!p->gcap) PPL_CUDA(cudaStreamCreateWithFlags(&p->gcap, cudaStreamNonBlocking));
+        PPL_CUDA(cudaStreamBeginCapture(p->gcap, cudaStreamCaptureModeRelaxed));
+        rc = apply_direct(p, L, t2, R, &opts, p->gcap);
+        cudaGraph_t g = nullptr;
+        const cudaError_t e = cudaStreamEndCapture(p->gcap, &g);  // also ends a capture that failed half way
+        if (rc != PPL_OK || e != cudaSuccess || !g) {
+            if (g) cudaGraphDestroy(g);
+            (void)cudaGetLastError();
+            return rc != PPL_OK ? rc : fail(PPL_ERR_CUDA);
+        }
+        const cudaError_t ei = cudaGraphInstantiate(&p->gexec, g, 0);
+        cudaGraphDestroy(g);
+        if (ei != cudaSuccess) {
+            (void)cudaGetLastError();
+            p->gexec = nullptr;
+            return fail(PPL_ERR_CUDA);
+        }
+        p->gkey.L = L;
+        p->gkey.t2 = t2;
+        p->gkey.R = R;
+        p->gkey.opts = opts;
+        p->gkey.sym = p->sym;
+    }
+    PPL_CUDA(cudaGraphLaunch(p->gexec, stream));
+    return PPL_OK;
+}
+
+}  // namespace
+
+int ppl_apply_ex(ppl_plan_t *p, const double *L, const double *t2, double *R, const ppl_opts_t *opts, void *stream_) {
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+    if (p && graph_wanted(p)) {
+        // a caller who is capturing `stream` gets the plain launches recorded into their own graph
+        cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(stream, &st) != cudaSuccess) {
+            (void)cudaGetLastError();
+            st = cudaStreamCaptureStatusActive;
+        }
+        if (st == cudaStreamCaptureStatusNone) return apply_graph(p, L, t2, R, opts, stream);
+    }
+    return apply_direct(p, L, t2, R, opts, stream);
+}
+
+int ppl_plan_set_graph(ppl_plan_t *p, int mode) {
+    if (!p || mode < -1 || mode > 1) return fail(PPL_ERR_INVALID_ARG);
+    p->graph_mode = mode;
+    return PPL_OK;
 }
 
 int ppl_apply_profiled(ppl_plan_t *p, const double *L, const double *t2, double *R, void *stream_, ppl_times_t *times) {
