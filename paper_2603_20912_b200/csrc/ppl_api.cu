@@ -6,6 +6,7 @@
 #include "ppl_kernels_tma.cuh"
 #include "ppl_kernels_full.cuh"
 
+#include <atomic>
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
@@ -336,9 +337,12 @@ void free_plan(ppl_plan_s *p) {
     delete p;
 }
 
-bool g_attr_set = false;
+std::atomic<bool> g_attr_set[64];  // per device: function attributes belong to the device's context
 int set_kernel_attrs() {
-    if (g_attr_set) return PPL_OK;
+    int dev = 0;
+    PPL_CUDA(cudaGetDevice(&dev));
+    const bool known = dev >= 0 && dev < 64;
+    if (known && g_attr_set[dev].load()) return PPL_OK;
     PPL_CUDA(cudaFuncSetAttribute(ppl::k_step0<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_MN));
     PPL_CUDA(cudaFuncSetAttribute(ppl::k_step0<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_MN));
     PPL_CUDA(cudaFuncSetAttribute(ppl::k_step1<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_K));
@@ -350,7 +354,7 @@ int set_kernel_attrs() {
     PPL_CUDA(cudaFuncSetAttribute(ppl::k_step1t_tma<NI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::Step1Cfg<NI>::SMEM));
     PPL_ATTR_NI(1) PPL_ATTR_NI(2) PPL_ATTR_NI(3) PPL_ATTR_NI(4) PPL_ATTR_NI(5) PPL_ATTR_NI(6) PPL_ATTR_NI(7) PPL_ATTR_NI(8) PPL_ATTR_NI(9) PPL_ATTR_NI(10)
 #undef PPL_ATTR_NI
-    g_attr_set = true;
+    if (known) g_attr_set[dev].store(true);
     return PPL_OK;
 }
 
