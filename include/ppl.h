@@ -191,8 +191,8 @@ int ppl_apply_host(ppl_plan_t *plan, const double *L_host, const double *t2_host
 int ppl_apply_profiled(ppl_plan_t *plan, const double *L, const double *t2, double *R, void *stream,
                        ppl_times_t *times);
 
-/* ppl_destroy: free the workspace, stream and events.  NULL is a no-op returning PPL_OK.
- * Synchronises the plan's internal stream first. */
+/* ppl_destroy: free the workspace, streams, events and the stored CUDA graph.  NULL is a no-op returning PPL_OK.
+ * Synchronises the device first (applies may still be in flight on the caller's streams). */
 int ppl_destroy(ppl_plan_t *plan);
 
 /* ---- small extras ------------------------------------------------------------------------- */

@@ -294,6 +294,9 @@ int build_tiles(ppl_plan_s *p) {
 
 void free_plan(ppl_plan_s *p) {
     if (!p) return;
+    // applies (plain launches on the caller's stream, or a graph launch) may still be in flight on streams the plan
+    // does not own: wait for the device before the workspace goes away
+    if (cudaDeviceSynchronize() != cudaSuccess) (void)cudaGetLastError();
     if (p->gen) {
         cudaStreamSynchronize(p->gen);
         cudaStreamDestroy(p->gen);

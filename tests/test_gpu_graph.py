@@ -125,3 +125,24 @@ def test_caller_captures_the_apply(sym):
         g.replay()
         torch.cuda.synchronize()
     assert relerr(Rd.cpu().numpy(), R0 + 3.0 * term) <= TOL
+
+
+@pytest.mark.parametrize("sym", SYMS)
+def test_graph_paper_layouts_alpha_beta(sym):
+    """'icjd' -> 'iajb' with alpha / beta under the graph: the un-packed modes allocate their permuted t2 lazily,
+    inside the (relaxed-mode) capture."""
+    o, v, x = 4, 38, 19
+    L, t2, R0 = _inputs(o, v, x, seed=13)
+    tl = np.ascontiguousarray(t2.transpose(0, 2, 1, 3))
+    Rl = np.ascontiguousarray(R0.transpose(0, 2, 1, 3))
+    want = oracle.full_ex(L, tl, Rl.copy(), "iajb", "iajb", -0.75, 0.5)
+    got = {}
+    for mode in (0, 1):
+        with P.Plan(o, v, x, 0) as plan:
+            if sym == P.PPL_SYM_FULL and not plan.info()["full_available"]:
+                pytest.skip("no PPL_SYM_FULL buffers for this shape")
+            plan.set_symmetry(sym)
+            plan.set_graph(mode)
+            got[mode] = _apply(plan, L, tl, Rl, t2_layout="iajb", r_layout="iajb", alpha=-0.75, beta=0.5)
+    assert relerr(got[1], want) <= TOL
+    assert np.array_equal(got[0], got[1])
