@@ -47,6 +47,8 @@ def _load():
         lib.ppl_oracle_project.restype = i
         lib.ppl_oracle_full_ex.argtypes = [i, i, i, _dp, _dp, _dp, i, i, ctypes.c_double, ctypes.c_double]
         lib.ppl_oracle_full_ex.restype = i
+        lib.ppl_oracle_eri_slab.argtypes = [i, i, _dp, i, i, _dp]
+        lib.ppl_oracle_eri_slab.restype = i
         _lib = lib
     return _lib
 
@@ -137,3 +139,15 @@ def full_ex(L, t2, R=None, t2_layout="ijab", r_layout="ijab", alpha=1.0, beta=1.
     if rc:
         raise RuntimeError(f"oracle error {rc}")
     return R
+
+
+def eri_slab(L, a0: int, na: int) -> np.ndarray:
+    """eri[al,b,c,d] = <ab|cd> = sum_P L[P,a0+al,c] L[P,b,d]: step 0 alone ('xac,xbd->acbd'),
+    stored in the order of the paper's dense variant 'abcd'."""
+    x, v, _ = L.shape
+    _chk(L, (x, v, v))
+    out = np.empty((na, v, v, v))
+    rc = _load().ppl_oracle_eri_slab(v, x, _p(L), int(a0), int(na), _p(out))
+    if rc:
+        raise RuntimeError(f"oracle error {rc}")
+    return out

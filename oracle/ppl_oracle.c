@@ -28,6 +28,8 @@
  * 2x2 example (tests/golden/), nchol=1 triple product, identity-L and rank-1-L closed forms, unit
  * impulse (index pairing), linearity / zero / accumulate, output pair symmetry with a negative
  * control, exact-integer inputs against int64 arithmetic, numpy einsum, projection identity.
+ * ppl_oracle_eri_slab (step 0 alone) is pinned by a hand-worked example, numpy einsum, the nchol = 1 outer
+ * product, the ERI symmetries and by reproducing ppl_oracle_full when contracted with t2.
  * Every entry point below is pinned; none is "parity unpinned".
  */
 #include <stdint.h>
@@ -287,4 +289,29 @@ int ppl_oracle_full_ex(int nocc, int nvirt, int nchol, const double *L, const do
         free(Wab);
     }
     return fail ? 3 : 0;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * Step 0 alone (PAPER.md:118-120 'xac,xbd->acbd'; eq. 5): a slab of the dense integrals
+ * in the order the paper's dense variant consumes them ('abcd,ecfd->efab'):
+ *
+ *     eri[al][b][c][d] = <ab|cd> = (ac|bd) = sum_P L[P][a0+al][c] * L[P][b][d],   0 <= al < na
+ *
+ * P ascending, plain double accumulation.  No symmetry of L is assumed.  eri is overwritten.
+ * Pinned by tests/test_oracle_pins.py (numpy einsum, nchol = 1 outer product bit for bit, the index
+ * pairing negative control, and: contracting it with t2 reproduces ppl_oracle_full). */
+int ppl_oracle_eri_slab(int nvirt, int nchol, const double *L, int a0, int na, double *eri) {
+    if (nvirt < 1 || nchol < 1 || !L || !eri || a0 < 0 || na < 1 || a0 + na > nvirt) return 1;
+    const int64_t v = nvirt, x = nchol, vv = v * v;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t ab = 0; ab < (int64_t)na * v; ++ab) {
+        const int64_t a = a0 + ab / v, b = ab % v;
+        double *Wab = eri + ab * vv;
+        memset(Wab, 0, sizeof(double) * (size_t)vv);
+        for (int64_t P = 0; P < x; ++P)
+            for (int64_t c = 0; c < v; ++c)
+                for (int64_t d = 0; d < v; ++d)
+                    Wab[c * v + d] += L[(P * v + a) * v + c] * L[(P * v + b) * v + d];
+    }
+    return 0;
 }

@@ -428,3 +428,56 @@ def test_full_symmetry_hook_identity(shape, T):
     if o > 1 and v > 1:
         tn = I.make_t2(o, v, 13, symmetric=False)
         assert rel(_full_symmetry_emulation(L, tn, T), oracle.full(L, tn)) > 1e-3
+
+
+# ----------------------------------------------------------------------------- step 0 alone: oracle.eri_slab
+def test_eri_slab_hand_worked_2x2():
+    """eq. (5), by hand with the L of tests/golden/hand_2x2.txt (nchol = 1): <ab|cd> = L[a,c] L[b,d].
+    L is not symmetric, so the other pairing L[a,d] L[b,c] gives a different tensor (negative control)."""
+    L = _read_hand()["L"].reshape(1, 2, 2).copy()
+    eri = oracle.eri_slab(L, 0, 2)
+    # a b c d -> L[a,c] L[b,d]; L = [[1,2],[3,4]]
+    want = np.array([[[[1, 2], [2, 4]], [[3, 4], [6, 8]]], [[[3, 6], [4, 8]], [[9, 12], [12, 16]]]], dtype=float)
+    assert np.array_equal(eri, want)
+    bad = np.einsum("ad,bc->abcd", L[0], L[0])
+    assert not np.array_equal(eri, bad)
+
+
+@pytest.mark.parametrize("shape", [(1, 1), (5, 1), (7, 5), (9, 4), (20, 60), (53, 17)])
+def test_eri_slab_against_einsum_and_outer_product(shape):
+    v, x = shape
+    L = I.make_L(v, x, 3, symmetric=False)
+    for a0, na in {(0, v), (v // 2, v - v // 2), (v - 1, 1), (0, 1)}:
+        eri = oracle.eri_slab(L, a0, na)
+        want = np.einsum("Pac,Pbd->abcd", L[:, a0:a0 + na, :], L, optimize=True)  # library contraction, own summation order
+        assert rel(eri, want) <= RTOL
+    # nchol = 1: a single product per entry, so the outer product is reproduced bit for bit
+    e1 = oracle.eri_slab(L[:1].copy(), 0, v)
+    assert np.array_equal(e1, np.einsum("ac,bd->abcd", L[0], L[0]))
+
+
+def test_eri_slab_contracted_with_t2_reproduces_the_ladder():
+    """'abcd,ijcd->ijab' on the slab is the ladder term (eq. 4): ties eri_slab to the pinned oracle.full."""
+    o, v, x = 3, 11, 6
+    L, t2 = rand_inputs(o, v, x, seed=4)
+    R = oracle.full(L, t2)
+    for a0, na in ((0, 4), (4, 7)):
+        eri = oracle.eri_slab(L, a0, na)
+        got = np.tensordot(t2, eri, axes=([2, 3], [2, 3]))  # [i,j,al,b]
+        assert rel(got, R[:, :, a0:a0 + na, :]) <= RTOL
+
+
+def test_eri_slab_symmetries_and_exact_integers():
+    v, x = 10, 7
+    Ls = I.make_L(v, x, 5, symmetric=True, integer=True)
+    e = oracle.eri_slab(Ls, 0, v)
+    want = np.einsum("Pac,Pbd->abcd", Ls.astype(np.int64), Ls.astype(np.int64))
+    assert np.array_equal(e, want.astype(float))  # exact integers: any summation order gives the same bits
+    # real orbitals (PAPER.md:66): the 8-fold symmetry of (ac|bd) in the <ab|cd> order
+    assert np.array_equal(e, e.transpose(2, 1, 0, 3))  # a <-> c
+    assert np.array_equal(e, e.transpose(0, 3, 2, 1))  # b <-> d
+    assert np.array_equal(e, e.transpose(1, 0, 3, 2))  # (ac) <-> (bd)
+    Ln = I.make_L(v, x, 5, symmetric=False, integer=True)
+    en = oracle.eri_slab(Ln, 0, v)
+    assert np.array_equal(en, en.transpose(1, 0, 3, 2))       # holds for any L
+    assert not np.array_equal(en, en.transpose(2, 1, 0, 3))   # needs L[P,a,c] = L[P,c,a]: negative control
