@@ -165,6 +165,15 @@ int ppl_apply(ppl_plan_t *plan, const double *L, const double *t2, double *R, vo
 int ppl_apply_ex(ppl_plan_t *plan, const double *L, const double *t2, double *R, const ppl_opts_t *opts,
                  void *stream);
 
+/* ppl_generate_eri: step 0 alone (the paper's 'xac,xbd->acbd'; eq. 5) -- the dense
+ * integrals of a slab of a's in the order the paper's dense variant consumes them ('abcd'):
+ *     eri[a-a0][b][c][d] = <ab|cd> = (ac|bd) = sum_P L[P,a,c] * L[P,b,d],   a0 <= a < a0+na, all b, c, d
+ * eri is a DEVICE buffer of na * nvirt^3 doubles, overwritten; L as in ppl_apply.  No symmetry of L is assumed or
+ * used; nocc of the plan is ignored.  ppl_generate_eri followed by ppl_apply_dense on the same slab equals the
+ * slab's share of ppl_apply (the dense / Cholesky duality of PAPER.md:75).  Asynchronous on `stream`.
+ * PPL_ERR_INVALID_ARG for a slab outside [0, nvirt) or misaligned pointers. */
+int ppl_generate_eri(ppl_plan_t *plan, const double *L, int a0, int na, double *eri, void *stream);
+
 /* ppl_apply_dense: step 1 alone on caller-supplied dense integrals (the
  * paper's 'abcd,ecfd->efab'):
  *     R[i,j,a,b] = beta*R[i,j,a,b] + alpha * sum_{c,d} eri[a-a0][b][c][d] * t2[i,j,c,d],   a0 <= a < a0+na, all b

@@ -76,6 +76,7 @@ SYMBOLS = {
     "ppl_apply": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
     "ppl_apply_ex": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, POINTER(ppl_opts_t), c_void_p]),
     "ppl_apply_dense": (c_int, [c_void_p, c_void_p, c_int, c_int, c_void_p, c_void_p, POINTER(ppl_opts_t), c_void_p]),
+    "ppl_generate_eri": (c_int, [c_void_p, c_void_p, c_int, c_int, c_void_p, c_void_p]),
     "ppl_apply_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, POINTER(c_uint64), POINTER(c_uint64)]),
     "ppl_apply_profiled": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, POINTER(ppl_times_t)]),
     "ppl_destroy": (c_int, [c_void_p]),
@@ -181,6 +182,13 @@ class Plan:
                                      _dev_ptr(t2, "t2", self._shape4(t2_layout)), _dev_ptr(R, "R", self._shape4(r_layout)),
                                      ctypes.byref(opts), _stream_ptr(stream)), "ppl_apply_dense")
         return R
+
+    def generate_eri(self, L, a0, na, eri, stream=None):
+        """Step 0 alone: eri[na][v][v][v] = <ab|cd> for a0 <= a < a0+na (the paper's 'xac,xbd->acbd' in 'abcd' order)."""
+        v, x = self.nvirt, self.nchol
+        _check(lib().ppl_generate_eri(self._h, _dev_ptr(L, "L", (x, v, v)), int(a0), int(na),
+                                      _dev_ptr(eri, "eri", (int(na), v, v, v)), _stream_ptr(stream)), "ppl_generate_eri")
+        return eri
 
     def apply_profiled(self, L, t2, R, stream=None) -> dict:
         o, v, x = self.nocc, self.nvirt, self.nchol

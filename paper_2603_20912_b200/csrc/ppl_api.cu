@@ -1602,6 +1602,32 @@ int ppl_apply_dense(ppl_plan_t *p, const double *eri, int a0, int na, const doub
     return PPL_OK;
 }
 
+// Step 0 alone: the dense slab eri[a - a0][b][c][d] = <ab|cd> = sum_P L[P,a,c] L[P,b,d] for a0 <= a < a0 + na, all b, c, d.
+// One W tile (A-block = the slab, B-block = all b) written straight into the caller's buffer: its [(a,b)][(c,d)] row
+// order IS the paper's 'abcd'.  Slabs are cut into pieces of at most 64 a's so that a piece is one grouped raster.
+int ppl_generate_eri(ppl_plan_t *p, const double *L, int a0, int na, double *eri, void *stream_) {
+    bool vec16 = false;
+    int rc = check_ptrs(p, L, L, eri, &vec16);
+    if (rc == PPL_OK && (a0 < 0 || na < 1 || a0 + na > p->v)) rc = PPL_ERR_INVALID_ARG;
+    if (rc != PPL_OK) return fail(rc);
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+    const bool tma = p->use_tma && vec16;
+    CUtensorMap mapL;
+    if (tma && make_map_2d(&mapL, L, (uint64_t)p->vv, (uint64_t)p->x, (uint64_t)p->vv * 8, 16, ppl::BK) != PPL_OK)
+        return fail(PPL_ERR_CUDA);
+    for (int a = a0; a < a0 + na; a += 64) {
+        Tile t;
+        t.a0 = a;
+        t.ta = std::min(64, a0 + na - a);
+        t.b0 = 0;
+        t.tb = p->v;
+        t.mirror = 0;
+        double *W = eri + (int64_t)(a - a0) * p->v * p->vv;
+        if ((rc = launch_step0(p, t, L, tma ? &mapL : nullptr, W, vec16, stream)) != PPL_OK) return rc;
+    }
+    return PPL_OK;
+}
+
 // PPL_SYM_FULL on host operands: the device never holds t2 or R.  t2 is streamed through two staging buffers and
 // packed chunk by chunk into tau+- (rows (i,j) of a chunk are contiguous in the [i][j][c][d] order), the slabs run on
 // the packed operands, and R+-acc is unpacked chunk by chunk into the staging buffers (R chunk in, result out).
