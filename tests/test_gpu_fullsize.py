@@ -8,7 +8,7 @@ The full oracle is unaffordable there (large: 164 TFLOP, XL: 1.56 PFLOP on CPU),
   P8   random and block-indicator projections sum_ab u_a w_b R[i,j,a,b] against oracle.project
        (long double): every entry of R takes part, so a missing, duplicated or mis-mirrored tile
        is caught; bound 1e-11 * max|R| * sum|u_a| sum|w_b|;
-  P9   exact small-integer inputs: sampled columns must match bit for bit (medium).
+  P9   exact small-integer inputs: sampled columns must match bit for bit (medium; large in the default mode).
 Medium can also be compared in full: PPL_FULL_ORACLE=1 (minutes of CPU).
 """
 import os
@@ -153,6 +153,15 @@ def test_large_sampled_columns_and_projections(sym):
     rmax = float(Rd.abs().max().item())
     _check_columns(L, t2, Rd, 96)
     _check_projections(L, t2, Rd, rmax, nrand=1)
+
+
+def test_large_exact_integers_sampled():
+    """P9 at large, default mode (the launch configuration bench.py times): |R| <= 4 * 1600 * 4 * 160000 << 2^53, every
+    partial sum is an exactly representable integer in any order, so the sampled columns must match bit for bit."""
+    if _host_gb() < 16:
+        pytest.skip("not enough host memory for the large config")
+    L, t2, Rd, _ = _run("large", integer=True)
+    _check_columns(L, t2, Rd, 64, exact=True)
 
 
 def test_xl_sampled_columns_and_projections():
