@@ -125,6 +125,9 @@ struct ppl_plan_s {
     size_t fws_bytes = 0;
     unsigned char *fws = nullptr;
     double *fX = nullptr;                      // strip [16*v rows (a_l*v + b)][vv]
+    double *fX2 = nullptr;                     // second strip (when it fits): step 0 of slab k+1 runs on `fs0` while slab k is folded
+    cudaStream_t fs0 = nullptr;                // producer stream of step 0 (two strips only)
+    cudaEvent_t ev_fork = nullptr, ev_s0[2] = {nullptr, nullptr}, ev_xfree[2] = {nullptr, nullptr};
     int fslots = 1;                            // W+- slots (2 when they fit: the fold of tile k+1 overlaps the GEMMs of tile k)
     double *fWp[2] = {nullptr, nullptr}, *fWm[2] = {nullptr, nullptr};  // W+- tile [16*tbg][ldp], [16*tbg][ldm]
     double *fpart = nullptr;
@@ -319,6 +322,15 @@ void free_plan(ppl_plan_s *p) {
             cudaStreamSynchronize(p->fs[i]);
             cudaStreamDestroy(p->fs[i]);
         }
+    if (p->fs0) {
+        cudaStreamSynchronize(p->fs0);
+        cudaStreamDestroy(p->fs0);
+    }
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+    for (int s = 0; s < 2; ++s) {
+        if (p->ev_s0[s]) cudaEventDestroy(p->ev_s0[s]);
+        if (p->ev_xfree[s]) cudaEventDestroy(p->ev_xfree[s]);
+    }
     for (int s = 0; s < 2; ++s) {
         if (p->ev_fold[s]) cudaEventDestroy(p->ev_fold[s]);
         for (int i = 0; i < 4; ++i)
@@ -829,6 +841,11 @@ int full_setup(ppl_plan_s *p, size_t room) {
     std::vector<int2> chunks;
     const char *envs = getenv("PPL_FULL_SLOTS");  // debug override: 1 = single W+- slot
     const int want_slots = (envs && atoi(envs) == 1) ? 1 : 2;
+    // A second strip pays where slabs are short (medium: 26.19 -> 25.82 ms for 1 GB); at large it buys 0.15 % for 8.2 GB
+    // and is not taken.  PPL_FULL_STRIPS: debug override (1 = never, 2 = whenever it fits).
+    const char *envx = getenv("PPL_FULL_STRIPS");
+    const int want_strips = envx ? (atoi(envx) == 1 ? 1 : 2) : (x_bytes <= ((size_t)2 << 30) ? 2 : 1);
+    bool two_strips = false;
     for (;; tbg = std::max(16, tbg / 2 / 16 * 16)) {
         const size_t slot = align256((size_t)TA * tbg * p->ldp * 8) + align256((size_t)TA * tbg * p->ldm * 8);
         const size_t part_cap = std::max<size_t>((size_t)64 << 20, slot / 8);
@@ -842,6 +859,8 @@ int full_setup(ppl_plan_s *p, size_t room) {
             p->tbg = tbg;
             p->fslots = ns;
             p->fws_bytes = base + ns * slot;
+            two_strips = want_strips == 2 && ns == want_slots && p->fws_bytes + x_bytes <= room;
+            if (two_strips) p->fws_bytes += x_bytes;
             break;
         }
         if (tbg == 16) return PPL_OK;  // does not fit: the plan stays without PPL_SYM_FULL
@@ -872,6 +891,8 @@ int full_setup(ppl_plan_s *p, size_t room) {
     p->fchunks = reinterpret_cast<int2 *>(q);
     q += align256(chunks.size() * sizeof(int2));
     p->Lpad = lpad_bytes ? reinterpret_cast<double *>(q) : nullptr;
+    q += lpad_bytes;
+    p->fX2 = two_strips ? reinterpret_cast<double *>(q) : nullptr;
     if (cudaMemcpy(p->fchunks, chunks.data(), chunks.size() * sizeof(int2), cudaMemcpyHostToDevice) != cudaSuccess) {
         (void)cudaGetLastError();
         return PPL_OK;
@@ -889,6 +910,14 @@ int full_setup(ppl_plan_s *p, size_t room) {
     if (!m) return PPL_OK;
     bool ok = true;
     for (int i = 0; i < 4 && ok; ++i) ok = ok && cudaStreamCreateWithFlags(&p->fs[i], cudaStreamNonBlocking) == cudaSuccess;
+    if (p->fX2) {
+        ok = ok && cudaStreamCreateWithFlags(&p->fs0, cudaStreamNonBlocking) == cudaSuccess;  // (stream priorities either way: no gain, measured)
+        ok = ok && cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming) == cudaSuccess;
+        for (int s = 0; s < 2 && ok; ++s) {
+            ok = ok && cudaEventCreateWithFlags(&p->ev_s0[s], cudaEventDisableTiming) == cudaSuccess;
+            ok = ok && cudaEventCreateWithFlags(&p->ev_xfree[s], cudaEventDisableTiming) == cudaSuccess;
+        }
+    }
     for (int s = 0; s < 2 && ok; ++s) {
         ok = ok && cudaEventCreateWithFlags(&p->ev_fold[s], cudaEventDisableTiming) == cudaSuccess;
         for (int i = 0; i < 4 && ok; ++i) ok = ok && cudaEventCreateWithFlags(&p->evg[s][i], cudaEventDisableTiming) == cudaSuccess;
@@ -1009,8 +1038,18 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
     const int TA = ppl::TA_FULL;
     static const bool serial = getenv("PPL_FULL_SERIAL") != nullptr;  // debug: everything on the caller's stream
     const bool conc = !prof && !dbg && !serial;
-    int tile_no = 0;
+    int tile_no = 0, slab_no = 0;
+    // Two strips: step 0 runs on its own stream, one slab ahead of the folds (strip k & 1), so that the HBM-bound fold of
+    // slab k and the tail of its GEMMs are filled by the DMMA work of slab k + 1 instead of standing between two slabs.
+    const bool dual = conc && p->fX2 != nullptr;
+    cudaStream_t s0 = dual ? p->fs0 : stream;
+    if (dual) {  // fork: step 0 starts behind everything queued on `stream` so far (the padded copy of L included)
+        PPL_CUDA(cudaEventRecord(p->ev_fork, stream));
+        PPL_CUDA(cudaStreamWaitEvent(s0, p->ev_fork, 0));
+    }
     for (const FullSlab &sl : p->slabs) {
+        const int xi = dual ? (slab_no & 1) : 0;
+        double *const X = xi ? p->fX2 : p->fX;
         ppl::Step0SlabArgs a0;
         a0.A0 = sl.A0;
         a0.ta = sl.ta;
@@ -1019,12 +1058,17 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
         a0.tiles_m = sl.tiles_m;
         a0.tiles_n = sl.tiles_n;
         a0.chunks = p->fchunks + sl.chunk_off;
-        a0.X = p->fX;
+        a0.X = X;
         const int items = sl.tiles_m * sl.tiles_n;
-        ppl::k_step0_slab<<<std::min(items, p->num_sms), ppl::TMA_THREADS, ppl::SMEM_TMA, stream>>>(mapL, a0);
+        if (dual && slab_no >= 2) PPL_CUDA(cudaStreamWaitEvent(s0, p->ev_xfree[xi], 0));  // the folds of slab k - 2 have read this strip
+        ppl::k_step0_slab<<<std::min(items, p->num_sms), ppl::TMA_THREADS, ppl::SMEM_TMA, s0>>>(mapL, a0);
         PPL_CUDA(cudaGetLastError());
         PPL_DBG("k_step0_slab", sl.A0);
         PPL_MARK(K_STEP0, 1);
+        if (dual) {
+            PPL_CUDA(cudaEventRecord(p->ev_s0[xi], s0));
+            PPL_CUDA(cudaStreamWaitEvent(stream, p->ev_s0[xi], 0));
+        }
         if (tau_ready && sl.A0 == 0) PPL_CUDA(cudaStreamWaitEvent(stream, tau_ready, 0));
         for (int k = sl.tile_begin; k < sl.tile_end; ++k) {
             const FullTile &t = p->ftiles[k];
@@ -1034,7 +1078,7 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
                 for (int i = 0; i < 4; ++i) PPL_CUDA(cudaStreamWaitEvent(stream, p->evg[sl_w][i], 0));
             {   // fold: strip rows -> W+- tile
                 ppl::FoldArgs f;
-                f.src = p->fX;
+                f.src = X;
                 f.sc = p->vp;
                 f.s_row = p->vvp;
                 f.s_i = f.s_j = 0;
@@ -1111,6 +1155,8 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
                 for (int i = 0; i < 4; ++i) PPL_CUDA(cudaEventRecord(p->evg[sl_w][i], p->fs[i]));
             ++tile_no;
         }
+        if (dual) PPL_CUDA(cudaEventRecord(p->ev_xfree[xi], stream));  // behind the last fold of this slab
+        ++slab_no;
     }
     if (conc)  // join: the side streams run in order, so the events of the last min(tiles, slots) tiles cover all work
         for (int s = 0; s < std::min(tile_no, p->fslots); ++s)

@@ -197,3 +197,37 @@ def test_host_entry_point_exact_integers_chunked(chunk_env):
     with P.Plan(o, v, x) as plan:
         plan.apply_host(L, t2, R)
     assert np.array_equal(R, oracle.full(L, t2))
+
+
+@pytest.mark.parametrize("shape", [(6, 96, 40), (4, 130, 12), (5, 53, 40)])
+def test_one_and_two_strips_agree_bit_for_bit(shape):
+    """Two strips (step 0 of slab k+1 on its own stream while slab k is folded; the default while a strip is <= 2 GiB)
+    and one strip (large, XL) run the same kernels on the same arguments in the same per-buffer order."""
+    import torch
+
+    o, v, x = shape
+    L = I.make_L(v, x, 71, symmetric=True)
+    t2 = I.make_t2(o, v, 71, symmetric=True)
+    want = oracle.full(L, t2)
+    Ld, td = torch.from_numpy(L).cuda(), torch.from_numpy(t2).cuda()
+    got = {}
+    old = os.environ.get("PPL_FULL_STRIPS")
+    try:
+        for strips in ("1", "2"):
+            os.environ["PPL_FULL_STRIPS"] = strips
+            with P.Plan(o, v, x, 0) as plan:
+                plan.set_symmetry(P.PPL_SYM_FULL)
+                plan.set_graph(0)
+                Rd = torch.zeros((o, o, v, v), dtype=torch.float64, device="cuda")
+                for _ in range(2):  # twice: events and strips are reused across applies
+                    plan.apply(Ld, td, Rd)
+                torch.cuda.synchronize()
+                got[strips] = (Rd.cpu().numpy(), plan.info()["workspace_bytes"])
+    finally:
+        if old is None:
+            os.environ.pop("PPL_FULL_STRIPS", None)
+        else:
+            os.environ["PPL_FULL_STRIPS"] = old
+    assert got["2"][1] > got["1"][1]  # the second strip was really allocated
+    assert np.abs(got["2"][0] - 2.0 * want).max() <= 1e-11 * np.abs(2.0 * want).max()
+    assert np.array_equal(got["1"][0], got["2"][0])
