@@ -1038,6 +1038,28 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
     const int TA = ppl::TA_FULL;
     static const bool serial = getenv("PPL_FULL_SERIAL") != nullptr;  // debug: everything on the caller's stream
     const bool conc = !prof && !dbg && !serial;
+    // PPL_TRACE (debug): a timed event pair around every launch ON ITS OWN STREAM -- the concurrency is kept -- and a
+    // timeline on stderr after a synchronise: "label index stream t_eligible_ms t_end_ms" (t_eligible: the stream has
+    // reached the launch, i.e. its predecessors and awaited events are complete).
+    static const bool trace_env = getenv("PPL_TRACE") != nullptr;
+    const bool trace = trace_env && conc;
+    struct TraceRec {
+        const char *label;
+        int k, sid;
+        cudaEvent_t b, e;
+    };
+    std::vector<TraceRec> tr;
+    auto tb = [&](const char *label, int k, int sid, cudaStream_t st) {
+        if (!trace) return;
+        TraceRec r{label, k, sid, nullptr, nullptr};
+        cudaEventCreate(&r.b);
+        cudaEventCreate(&r.e);
+        cudaEventRecord(r.b, st);
+        tr.push_back(r);
+    };
+    auto te = [&](cudaStream_t st) {
+        if (trace) cudaEventRecord(tr.back().e, st);
+    };
     int tile_no = 0, slab_no = 0;
     // Two strips: step 0 runs on its own stream, one slab ahead of the folds (strip k & 1), so that the HBM-bound fold of
     // slab k and the tail of its GEMMs are filled by the DMMA work of slab k + 1 instead of standing between two slabs.
@@ -1061,7 +1083,9 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
         a0.X = X;
         const int items = sl.tiles_m * sl.tiles_n;
         if (dual && slab_no >= 2) PPL_CUDA(cudaStreamWaitEvent(s0, p->ev_xfree[xi], 0));  // the folds of slab k - 2 have read this strip
+        tb("step0", sl.A0, 0, s0);
         ppl::k_step0_slab<<<std::min(items, p->num_sms), ppl::TMA_THREADS, ppl::SMEM_TMA, s0>>>(mapL, a0);
+        te(s0);
         PPL_CUDA(cudaGetLastError());
         PPL_DBG("k_step0_slab", sl.A0);
         PPL_MARK(K_STEP0, 1);
@@ -1100,7 +1124,9 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
                 f.ldm = p->ldm;
                 const int nb = (p->vp + ppl::FT - 1) / ppl::FT - f.cb_min;
                 dim3 grid(nb * (nb + 1) / 2, ppl::fold_grid_y(nb * (nb + 1) / 2, N, p->num_sms));
+                tb("fold", k, 1, stream);
                 ppl::k_symfold<<<grid, 256, 0, stream>>>(f);
+                te(stream);
                 PPL_CUDA(cudaGetLastError());
                 PPL_DBG("k_symfold", k);
                 PPL_MARK(K_FOLD, 1);
@@ -1117,12 +1143,17 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
             }
             // use 1: R+-acc[.][(a,b)] += tau+-[.][J >= (A0,A0)] W+-[(a,b)][J]^T
             double *partp = p->fpart, *partm = p->fpart + p->fpart_m_off;
+            tb("use1+", k, 2, g0);
             rc = launch_step1(p, &p->mapTp, &p->mapFWp[sl_w], p->mg_p, nullptr, 0, nullptr, 0, p->Mp, N, p->Kp, t.sp, partp, true, g0,
                               t.k0p);
+            te(g0);
             const bool m1 = minus && p->Km - t.k0m > 0;
-            if (rc == PPL_OK && m1)
+            if (rc == PPL_OK && m1) {
+                tb("use1-", k, 3, g1);
                 rc = launch_step1(p, &p->mapTm, &p->mapFWm[sl_w], p->mg_m, nullptr, 0, nullptr, 0, p->Mm, N, p->Km, t.sm, partm, true,
                                   g1, t.k0m);
+                te(g1);
+            }
             if (rc != PPL_OK) return rc;
             PPL_DBG("use 1 (k_step1_tma)", k);
             PPL_MARK(K_STEP1, m1 ? 2 : 1);
@@ -1133,20 +1164,30 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
                 PPL_CUDA(cudaStreamWaitEvent(g0, p->evg[prev][2], 0));
                 PPL_CUDA(cudaStreamWaitEvent(g1, p->evg[prev][3], 0));
             }
+            tb("red+", k, 2, g0);
             rc = launch_reduce_acc(p, t, partp, t.sp.splitk, p->Mp, false, p->raccp, p->ldp, g0);
-            if (rc == PPL_OK && m1) rc = launch_reduce_acc(p, t, partm, t.sm.splitk, p->Mm, true, p->raccm, p->ldm, g1);
+            te(g0);
+            if (rc == PPL_OK && m1) {
+                tb("red-", k, 3, g1);
+                rc = launch_reduce_acc(p, t, partm, t.sm.splitk, p->Mm, true, p->raccm, p->ldm, g1);
+                te(g1);
+            }
             if (rc != PPL_OK) return rc;
             PPL_DBG("k_reduce_acc", k);
             PPL_MARK(K_REDUCE, m1 ? 2 : 1);
             // use 2: R+-acc[.][J >= (A0+16,A0+16)] += tau+-[.][(a,b) in tile] W+-[(a,b)][J]
             int n2 = 0;
             if (p->Kp - t.k1p > 0) {
+                tb("use2+", k, 4, g2);
                 if ((rc = launch_step1t(p, &p->mapTp, &p->mapFWpT[sl_w], p->mg_p, p->Mp, t, false, p->raccp, p->ldp, g2)) != PPL_OK) return rc;
+                te(g2);
                 PPL_DBG("use 2 plus (k_step1t_tma)", k);
                 ++n2;
             }
             if (minus && p->Km - t.k1m > 0) {
+                tb("use2-", k, 5, g3);
                 if ((rc = launch_step1t(p, &p->mapTm, &p->mapFWmT[sl_w], p->mg_m, p->Mm, t, true, p->raccm, p->ldm, g3)) != PPL_OK) return rc;
+                te(g3);
                 PPL_DBG("use 2 minus (k_step1t_tma)", k);
                 ++n2;
             }
@@ -1162,9 +1203,24 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
         for (int s = 0; s < std::min(tile_no, p->fslots); ++s)
             for (int i = 0; i < 4; ++i) PPL_CUDA(cudaStreamWaitEvent(stream, p->evg[s][i], 0));
     if (phases & FULL_UNPACK) {
+        tb("unpack", 0, 1, stream);
         if ((rc = launch_unpack_full(p, opts, R, 0, (int64_t)p->o * p->o * p->vv, stream)) != PPL_OK) return rc;
+        te(stream);
         PPL_DBG("k_unpack_full", 0);
         PPL_MARK(K_REDUCE, 1);
+    }
+    if (trace && !tr.empty()) {
+        if (cudaStreamSynchronize(stream) == cudaSuccess)
+            for (const TraceRec &r : tr) {
+                float tb_ms = 0, te_ms = 0;
+                cudaEventElapsedTime(&tb_ms, tr.front().b, r.b);
+                cudaEventElapsedTime(&te_ms, tr.front().b, r.e);
+                fprintf(stderr, "PPL_TRACE %-6s %4d s%d %10.4f %10.4f\n", r.label, r.k, r.sid, tb_ms, te_ms);
+            }
+        for (const TraceRec &r : tr) {
+            cudaEventDestroy(r.b);
+            cudaEventDestroy(r.e);
+        }
     }
 #undef PPL_MARK
 #undef PPL_DBG
