@@ -226,6 +226,14 @@ int ppl_plan_set_graph(ppl_plan_t *plan, int mode);
 
 int ppl_plan_info(const ppl_plan_t *plan, ppl_info_t *out);
 
+/* ppl_plan_dry: the planner alone.  Runs exactly the host half of ppl_plan -- packed geometry, row tiling of step 1,
+ * tile edge, ring depth, split-K, slabs / b-groups / strips of PPL_SYM_FULL, buffer sizes, flop accounting -- for a
+ * STATED device (free bytes, SM count; the TMA kernel family is assumed) and fills *out as ppl_plan_info would.  No CUDA
+ * call, nothing allocated: usable (and tested) on a machine without a GPU.  mode: a PPL_SYM_* value, or -1 for the
+ * default ppl_plan would choose.  Errors as ppl_plan / ppl_plan_set_symmetry (PPL_ERR_WORKSPACE_TOO_SMALL ...). */
+int ppl_plan_dry(int nocc, int nvirt, int nchol, size_t workspace_bytes, size_t device_free_bytes, int num_sms, int mode,
+                 ppl_info_t *out);
+
 /* Debug: verify on the device that L[P,a,c]==L[P,c,a] (required in PPL_SYM_FULL, else only reported)
  * and, in every mode but PPL_SYM_NONE, that t2[i,j,c,d]==t2[j,i,d,c] (required).  Synchronises `stream`.
  * Returns PPL_OK, or PPL_ERR_PRECONDITION if an input violates a symmetry the plan relies on.

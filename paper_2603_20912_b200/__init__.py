@@ -30,6 +30,7 @@ from .binding import (  # noqa: F401
     ppl_destroy,
     ppl_last_error,
     ppl_plan,
+    ppl_plan_dry,
     ppl_probe_fp64_peak,
 )
 from ._build import build  # noqa: F401

@@ -85,6 +85,7 @@ SYMBOLS = {
     "ppl_plan_set_symmetry": (c_int, [c_void_p, c_int]),
     "ppl_plan_set_graph": (c_int, [c_void_p, c_int]),
     "ppl_plan_info": (c_int, [c_void_p, POINTER(ppl_info_t)]),
+    "ppl_plan_dry": (c_int, [c_int, c_int, c_int, c_size_t, c_size_t, c_int, c_int, POINTER(ppl_info_t)]),
     "ppl_check_inputs": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, POINTER(c_int)]),
     "ppl_probe_fp64_peak": (c_int, [POINTER(c_double), c_int, c_double]),
     "ppl_debug_dmma_layout": (c_int, [c_void_p, c_void_p, c_void_p]),
@@ -264,6 +265,15 @@ class Plan:
 # function-style mirrors of the three north_star entry points
 def ppl_plan(nocc: int, nvirt: int, nchol: int, workspace_bytes: int = 0) -> Plan:
     return Plan(nocc, nvirt, nchol, workspace_bytes)
+
+
+def ppl_plan_dry(nocc: int, nvirt: int, nchol: int, workspace_bytes: int = 0, device_free_bytes: int = 170 << 30,
+                 num_sms: int = 148, mode: int = -1) -> dict:
+    """The planner alone, for a stated device: no GPU needed.  Returns what Plan.info() would."""
+    out = ppl_info_t()
+    _check(lib().ppl_plan_dry(int(nocc), int(nvirt), int(nchol), int(workspace_bytes), int(device_free_bytes), int(num_sms),
+                              int(mode), ctypes.byref(out)), "ppl_plan_dry")
+    return out.asdict()
 
 
 def ppl_apply(plan: Plan, L, t2, R, stream=None):

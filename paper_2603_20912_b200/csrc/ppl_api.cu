@@ -142,6 +142,7 @@ struct ppl_plan_s {
     cudaEvent_t ev_fold[2] = {nullptr, nullptr}, evg[2][4] = {};
     CUtensorMap mapFWp[2], mapFWm[2], mapFWpT[2], mapFWmT[2];  // the W+- tile as the B operand of use 1 (box 16 x 128 rows) / use 2 (box 16 x 16 rows)
     // ---- CUDA graph of one apply (launch-bound shapes; ppl_plan_set_graph) ----
+    int dry = 0;                               // ppl_plan_dry: geometry only, the plan owns nothing on the device
     int graph_mode = -1;                       // -1: auto (graph when the executed flops are below GRAPH_AUTO_FLOPS), 0: off, 1: on
     cudaStream_t gcap = nullptr;               // capture origin (never the caller's stream: the legacy stream cannot capture)
     cudaGraphExec_t gexec = nullptr;           // the instantiated apply for the key below
@@ -299,7 +300,8 @@ void free_plan(ppl_plan_s *p) {
     if (!p) return;
     // applies (plain launches on the caller's stream, or a graph launch) may still be in flight on streams the plan
     // does not own: wait for the device before the workspace goes away
-    if (cudaDeviceSynchronize() != cudaSuccess) (void)cudaGetLastError();
+    const bool owns_device = p->ws || p->fws || p->flags || p->gen || p->gexec;  // not so for ppl_plan_dry or a plan that failed early
+    if (!p->dry && owns_device && cudaDeviceSynchronize() != cudaSuccess) (void)cudaGetLastError();
     if (p->gen) {
         cudaStreamSynchronize(p->gen);
         cudaStreamDestroy(p->gen);
@@ -828,7 +830,7 @@ int full_geometry(ppl_plan_s *p, int tbg, size_t part_cap, std::vector<int2> *ch
 }
 
 // Allocate the PPL_SYM_FULL buffers if they fit into `room` bytes.  Returns PPL_OK and sets full_ok, or leaves it 0.
-int full_setup(ppl_plan_s *p, size_t room) {
+int full_setup(ppl_plan_s *p, size_t room, bool dry = false) {
     p->full_ok = 0;
     if (!p->use_tma || !p->sa_ok || p->v < 2) return PPL_OK;
     const int v = p->vp, TA = ppl::TA_FULL;
@@ -864,6 +866,10 @@ int full_setup(ppl_plan_s *p, size_t room) {
             break;
         }
         if (tbg == 16) return PPL_OK;  // does not fit: the plan stays without PPL_SYM_FULL
+    }
+    if (dry) {  // geometry only (ppl_plan_dry): slabs, tiles, splits and byte counts are final at this point
+        p->full_ok = 1;
+        return PPL_OK;
     }
     if (cudaMalloc(&p->fws, p->fws_bytes) != cudaSuccess) {
         (void)cudaGetLastError();
@@ -1269,32 +1275,23 @@ const char *ppl_error_string(int code) {
     }
 }
 
-ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
-    if (nocc < 1 || nvirt < 1 || nchol < 1 || (int64_t)nvirt * nvirt > INT32_MAX / 2 ||
-        (int64_t)nocc * nocc > INT32_MAX / 2) {
-        fail(PPL_ERR_INVALID_ARG);
-        return nullptr;
-    }
-    int dev = 0;
-    cudaDeviceProp prop;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
-        (void)cudaGetLastError();
-        fail(PPL_ERR_UNSUPPORTED_DEVICE);
-        return nullptr;
-    }
-    if (prop.major != 10) {
-        fail(PPL_ERR_UNSUPPORTED_DEVICE);
-        return nullptr;
-    }
+}  // extern "C"
+
+namespace {
+
+// The host half of ppl_plan: everything that follows from (nocc, nvirt, nchol), the byte budget `cap`, the SM count and
+// the kernel family alone -- packed geometry, row tiling of step 1, tile edge T, ring depth, buffer sizes.  No CUDA call.
+ppl_plan_s *plan_host(int nocc, int nvirt, int nchol, size_t workspace_bytes, size_t cap, int num_sms, bool use_tma, int *rc_out) {
+    *rc_out = PPL_OK;
     ppl_plan_s *p = new (std::nothrow) ppl_plan_s();
     if (!p) {
-        fail(PPL_ERR_ALLOC);
+        *rc_out = PPL_ERR_ALLOC;
         return nullptr;
     }
     p->o = nocc;
     p->v = nvirt;
     p->x = nchol;
-    p->num_sms = prop.multiProcessorCount;
+    p->num_sms = num_sms;
     p->vec16 = (nvirt % 2 == 0) ? 1 : 0;
     p->vv = (int64_t)nvirt * nvirt;
     p->vp = nvirt + (nvirt & 1);
@@ -1308,19 +1305,7 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
     p->Km = (int)ppl::kminus_extent(p->vp);
     p->ldp = ((int64_t)p->Kp + 15) / 16 * 16;  // rows of the packed operands are 128-byte aligned: TMA-legal for any nvirt
     p->ldm = ((int64_t)std::max(p->Km, 1) + 15) / 16 * 16;
-
-    size_t free_b = 0, total_b = 0;
-    if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) {
-        (void)cudaGetLastError();
-        free_plan(p);
-        fail(PPL_ERR_CUDA);
-        return nullptr;
-    }
-    const size_t auto_cap = (size_t)(0.9 * (double)free_b);
-    const size_t cap = workspace_bytes ? std::min(workspace_bytes, auto_cap) : auto_cap;
-
-    const char *envk = getenv("PPL_KERNELS");  // debug override: "cpasync" forces the non-TMA kernels
-    p->use_tma = !(envk && strcmp(envk, "cpasync") == 0) && get_encode() != nullptr;
+    p->use_tma = use_tma ? 1 : 0;
     const char *envni = getenv("PPL_NI");  // debug override of the step-1 tile height
     const int ni_env = (envni && atoi(envni) >= 1 && atoi(envni) <= 10) ? atoi(envni) : 10;  // largest instance used
     const bool tma_full = p->use_tma && p->vec16;
@@ -1368,7 +1353,7 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
         }
     if (best_T == 0) {
         free_plan(p);
-        fail(PPL_ERR_WORKSPACE_TOO_SMALL);
+        *rc_out = PPL_ERR_WORKSPACE_TOO_SMALL;
         return nullptr;
     }
     p->T = best_T;
@@ -1379,6 +1364,54 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
     p->slot_bytes = best_ev.slot_bytes;
     p->part_bytes = best_ev.part_bytes;
     p->ws_bytes = p->x_bytes + p->ring * p->slot_bytes + p->part_bytes + (p->sa_ok ? p->tau_bytes : 0);
+    return p;
+}
+
+bool dims_ok(int nocc, int nvirt, int nchol) {
+    return nocc >= 1 && nvirt >= 1 && nchol >= 1 && (int64_t)nvirt * nvirt <= INT32_MAX / 2 && (int64_t)nocc * nocc <= INT32_MAX / 2;
+}
+
+int full_min_v() {
+    const char *envf = getenv("PPL_FULL_MIN_V");  // debug override
+    return envf ? atoi(envf) : 52;
+}
+
+}  // namespace
+
+extern "C" {
+
+ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
+    if (!dims_ok(nocc, nvirt, nchol)) {
+        fail(PPL_ERR_INVALID_ARG);
+        return nullptr;
+    }
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        fail(PPL_ERR_UNSUPPORTED_DEVICE);
+        return nullptr;
+    }
+    if (prop.major != 10) {
+        fail(PPL_ERR_UNSUPPORTED_DEVICE);
+        return nullptr;
+    }
+    size_t free_b = 0, total_b = 0;
+    if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) {
+        (void)cudaGetLastError();
+        fail(PPL_ERR_CUDA);
+        return nullptr;
+    }
+    const size_t auto_cap = (size_t)(0.9 * (double)free_b);
+    const size_t cap = workspace_bytes ? std::min(workspace_bytes, auto_cap) : auto_cap;
+    const char *envk = getenv("PPL_KERNELS");  // debug override: "cpasync" forces the non-TMA kernels
+    const bool use_tma = !(envk && strcmp(envk, "cpasync") == 0) && get_encode() != nullptr;
+    int rc_host = PPL_OK;
+    ppl_plan_s *p = plan_host(nocc, nvirt, nchol, workspace_bytes, cap, prop.multiProcessorCount, use_tma, &rc_host);
+    if (!p) {
+        fail(rc_host);
+        return nullptr;
+    }
     if (cudaMalloc(&p->ws, p->ws_bytes) != cudaSuccess || cudaMalloc(&p->flags, sizeof(int)) != cudaSuccess) {
         (void)cudaGetLastError();
         free_plan(p);
@@ -1454,10 +1487,30 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
     // PPL_SYM_PAIR_SA at nocc = 5..8, nchol = 4 nvirt: 0.157 vs 0.186 ms at nvirt = 48, 0.283 vs 0.274 ms at 53,
     // 0.365 vs 0.328 ms at 64, 1.71 vs 0.97 ms at 96)
     full_setup(p, cap > p->ws_bytes ? cap - p->ws_bytes : 0);
-    const char *envf = getenv("PPL_FULL_MIN_V");  // debug override
-    const int full_min_v = envf ? atoi(envf) : 52;
-    if (p->full_ok && nvirt >= full_min_v) p->sym = PPL_SYM_FULL;
+    if (p->full_ok && nvirt >= full_min_v()) p->sym = PPL_SYM_FULL;
     return p;
+}
+
+// ppl_plan_dry: the planner alone, for a stated device (free bytes, SM count): no CUDA call, nothing allocated.
+int ppl_plan_dry(int nocc, int nvirt, int nchol, size_t workspace_bytes, size_t device_free_bytes, int num_sms, int mode,
+                 ppl_info_t *out) {
+    if (!out || !dims_ok(nocc, nvirt, nchol) || num_sms < 1 || mode < -1 || mode > PPL_SYM_FULL) return fail(PPL_ERR_INVALID_ARG);
+    const size_t auto_cap = (size_t)(0.9 * (double)device_free_bytes);
+    const size_t cap = workspace_bytes ? std::min(workspace_bytes, auto_cap) : auto_cap;
+    int rc = PPL_OK;
+    ppl_plan_s *p = plan_host(nocc, nvirt, nchol, workspace_bytes, cap, num_sms, true, &rc);
+    if (!p) return fail(rc);
+    p->dry = 1;
+    p->sym = p->sa_ok ? PPL_SYM_PAIR_SA : PPL_SYM_PAIR;
+    rc = build_tiles(p);
+    if (rc == PPL_OK) {
+        full_setup(p, cap > p->ws_bytes ? cap - p->ws_bytes : 0, true);
+        if (p->full_ok && nvirt >= full_min_v()) p->sym = PPL_SYM_FULL;
+        if (mode >= 0) rc = ppl_plan_set_symmetry(p, mode);
+    }
+    if (rc == PPL_OK) rc = ppl_plan_info(p, out);
+    free_plan(p);
+    return rc == PPL_OK ? PPL_OK : fail(rc);
 }
 
 int ppl_plan_set_symmetry(ppl_plan_t *p, int mode) {
@@ -1524,7 +1577,7 @@ int ppl_plan_info(const ppl_plan_t *p, ppl_info_t *out) {
         out->n_tiles = (int)p->ftiles.size();
         out->ring = 1;
         out->splitk = p->ftiles.empty() ? 0 : p->ftiles[0].sp.splitk;
-        int launches = 2 + (int)p->slabs.size() + (p->Lpad ? 1 : 0);  // pack, unpack, one step 0 per slab (+ the L pad copy for odd nvirt)
+        int launches = 2 + (int)p->slabs.size() + ((p->v & 1) ? 1 : 0);  // pack, unpack, one step 0 per slab (+ the L pad copy for odd nvirt)
         for (const FullTile &t : p->ftiles) {
             const bool m1 = minus && p->Km - t.k0m > 0;
             launches += 1 + (m1 ? 4 : 2) + (p->Kp - t.k1p > 0 ? 1 : 0) + (minus && p->Km - t.k1m > 0 ? 1 : 0);

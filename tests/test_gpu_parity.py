@@ -189,3 +189,14 @@ def test_workspace_too_small_and_bad_pointers():
     assert ei.value.code == P.PPL_ERR_WORKSPACE_TOO_SMALL
     with P.Plan(5, 20, 60) as plan:
         assert P.lib().ppl_apply(plan._h, None, None, None, None) == P.PPL_ERR_INVALID_ARG
+
+
+@pytest.mark.parametrize("shape", [(5, 20, 60), (5, 53, 232), (7, 81, 300), (20, 200, 800), (12, 18, 9)])
+def test_dry_planner_equals_the_device_plan(shape):
+    """ppl_plan_dry (the planner alone, tests/test_planner_cpu.py) and ppl_plan on the device agree field by field."""
+    import torch
+
+    with P.Plan(*shape) as plan:
+        dev = plan.info()
+    dry = P.ppl_plan_dry(*shape, device_free_bytes=torch.cuda.mem_get_info()[0], num_sms=torch.cuda.get_device_properties(0).multi_processor_count)
+    assert dry == dev
