@@ -121,7 +121,8 @@ typedef struct ppl_info_s {
     int32_t full_available;                  /* 1: ppl_plan allocated the PPL_SYM_FULL buffers */
     int32_t full_tbg;                        /* PPL_SYM_FULL: b-group width (tile = 16 a's x full_tbg b's) */
     int32_t full_slabs;                      /* PPL_SYM_FULL: number of a-blocks of 16 (one step-0 launch each) */
-    int32_t reserved_;
+    int32_t full_tight;                      /* PPL_SYM_FULL buffers are the memory-tight kind: a strip of one (slab; b-group)
+                                                tile instead of the slab's 16 nvirt^3, step 0 per tile at 1/4 of nominal */
     uint64_t full_workspace_bytes;           /* part of workspace_bytes that belongs to PPL_SYM_FULL */
 } ppl_info_t;
 

@@ -41,7 +41,7 @@ class ppl_info_t(ctypes.Structure):
         ("sa_tile_m_plus", c_int32), ("sa_tile_m_minus", c_int32),
         ("sa_rows_plus", c_int32), ("sa_rows_minus", c_int32),
         ("sa_k_plus", c_int32), ("sa_k_minus", c_int32),
-        ("full_available", c_int32), ("full_tbg", c_int32), ("full_slabs", c_int32), ("reserved_", c_int32),
+        ("full_available", c_int32), ("full_tbg", c_int32), ("full_slabs", c_int32), ("full_tight", c_int32),
         ("full_workspace_bytes", c_uint64),
     ]
 

@@ -60,6 +60,9 @@ struct FullTile {
     int k0p, k0m;    // first packed (c<=d) / (c<d) index with c >= A0: start of the use-1 contraction range
     int k1p, k1m;    // first packed index with c >= A0+16: start of the use-2 output range
     SplitChoice sp, sm;
+    // memory-tight mode: step 0 runs per tile on the full (b in group, d >= A0) rectangle into a strip of the tile's rows
+    size_t chunk_off = 0;
+    int tiles_n = 0;
 };
 struct FullSlab {
     int A0, ta;
@@ -121,6 +124,7 @@ struct ppl_plan_s {
     CUtensorMap mapW[MAX_RING], mapWp[MAX_RING], mapWm[MAX_RING], mapTp, mapTm;  // plan-owned operands
     // ---- PPL_SYM_FULL (own allocation `fws`; shares taup/taum with PPL_SYM_PAIR_SA) ----
     int full_ok = 0;
+    int full_tight = 0;                        // 1: the strip holds one (slab; b-group) tile, step 0 runs per tile without the b<->d image
     int tbg = 0;                               // b-group width (multiple of 16)
     size_t fws_bytes = 0;
     unsigned char *fws = nullptr;
@@ -767,7 +771,7 @@ int run_apply(ppl_plan_s *p, const double *L, const double *t2, double *R, const
 // ------------------------------------------------------------------------------------------
 // PPL_SYM_FULL (ppl_kernels_full.cuh): slabs of 16 a's, tiles (A; b-group), chunk table of step 0.
 // ------------------------------------------------------------------------------------------
-int full_geometry(ppl_plan_s *p, int tbg, size_t part_cap, std::vector<int2> *chunks_out) {
+int full_geometry(ppl_plan_s *p, int tbg, size_t part_cap, std::vector<int2> *chunks_out, bool tight = false) {
     const int v = p->vp, TA = ppl::TA_FULL;
     p->slabs.clear();
     p->ftiles.clear();
@@ -783,9 +787,11 @@ int full_geometry(ppl_plan_s *p, int tbg, size_t part_cap, std::vector<int2> *ch
         sl.chunk_off = chunks.size();
         // d-block major: the 8 chunks of a CTA tile are 8 consecutive b's of one d-block, so that the b<->d image
         // X[a,d,c,b] is written as runs of 8 b's (two full 32-byte sectors, merged in L2) instead of lone doubles
-        for (int d0 = A0; d0 < v; d0 += 16)
-            for (int b = A0; b < std::min(d0 + 16, v); ++b) chunks.push_back(make_int2(b, d0));
-        while ((chunks.size() - sl.chunk_off) % 8) chunks.push_back(make_int2(-1, 0));
+        if (!tight) {
+            for (int d0 = A0; d0 < v; d0 += 16)
+                for (int b = A0; b < std::min(d0 + 16, v); ++b) chunks.push_back(make_int2(b, d0));
+            while ((chunks.size() - sl.chunk_off) % 8) chunks.push_back(make_int2(-1, 0));
+        }
         sl.tiles_n = (int)((chunks.size() - sl.chunk_off) / 8);
         sl.flops0 = 2.0 * p->x * (128.0 * sl.tiles_m) * (128.0 * sl.tiles_n);
         p->ff_step0 += sl.flops0;
@@ -820,6 +826,16 @@ int full_geometry(ppl_plan_s *p, int tbg, size_t part_cap, std::vector<int2> *ch
             const double r0 = v - A0, r1 = v - c1;  // pairs with c >= A0 / c >= A0+16
             p->ff_step1 += 2.0 * N * ((double)p->Mp * r0 * (r0 + 1) / 2 + (double)p->Mm * r0 * (r0 - 1) / 2);
             p->ff_step1 += 2.0 * N * ((double)p->Mp * r1 * (r1 + 1) / 2 + (double)p->Mm * std::max(0.0, r1 * (r1 - 1) / 2));
+            if (tight) {  // the full (b, d) rectangle of the group: no image, twice the step-0 flops, a strip of tbp rows per a
+                t.chunk_off = chunks.size();
+                for (int d0 = A0; d0 < v; d0 += 16)
+                    for (int b = t.bg0; b < t.bg0 + t.nb; ++b) chunks.push_back(make_int2(b, d0));
+                while ((chunks.size() - t.chunk_off) % 8) chunks.push_back(make_int2(-1, 0));
+                t.tiles_n = (int)((chunks.size() - t.chunk_off) / 8);
+                const double f0 = 2.0 * p->x * (128.0 * sl.tiles_m) * (128.0 * t.tiles_n);
+                sl.flops0 += f0;
+                p->ff_step0 += f0;
+            }
             p->ftiles.push_back(t);
         }
         sl.tile_end = (int)p->ftiles.size();
@@ -838,35 +854,45 @@ int full_setup(ppl_plan_s *p, size_t room, bool dry = false) {
     const char *envg = getenv("PPL_TBG");  // debug override of the b-group width
     int tbg = (envg && atoi(envg) >= 16) ? atoi(envg) / 16 * 16 : 256;
     tbg = std::min(tbg, (v + 15) / 16 * 16);
-    const size_t x_bytes = align256((size_t)TA * v * p->vvp * 8);
     const size_t racc_bytes = p->tau_bytes;  // same shapes as tau+-
     std::vector<int2> chunks;
     const char *envs = getenv("PPL_FULL_SLOTS");  // debug override: 1 = single W+- slot
     const int want_slots = (envs && atoi(envs) == 1) ? 1 : 2;
-    // A second strip pays where slabs are short (medium: 26.19 -> 25.82 ms for 1 GB); at large it buys 0.15 % for 8.2 GB
-    // and is not taken.  PPL_FULL_STRIPS: debug override (1 = never, 2 = whenever it fits).
-    const char *envx = getenv("PPL_FULL_STRIPS");
-    const int want_strips = envx ? (atoi(envx) == 1 ? 1 : 2) : (x_bytes <= ((size_t)2 << 30) ? 2 : 1);
-    bool two_strips = false;
-    for (;; tbg = std::max(16, tbg / 2 / 16 * 16)) {
-        const size_t slot = align256((size_t)TA * tbg * p->ldp * 8) + align256((size_t)TA * tbg * p->ldm * 8);
-        const size_t part_cap = std::max<size_t>((size_t)64 << 20, slot / 8);
-        full_geometry(p, tbg, part_cap, &chunks);
-        const size_t chunk_bytes = align256(chunks.size() * sizeof(int2));
-        const size_t base = x_bytes + align256(p->fpart_bytes) + racc_bytes + chunk_bytes + lpad_bytes + 256;
-        int ns = 0;
-        for (int s = want_slots; s >= 1 && !ns; --s)
-            if (base + s * slot <= room) ns = s;
-        if (ns) {
-            p->tbg = tbg;
-            p->fslots = ns;
-            p->fws_bytes = base + ns * slot;
-            two_strips = want_strips == 2 && ns == want_slots && p->fws_bytes + x_bytes <= room;
-            if (two_strips) p->fws_bytes += x_bytes;
-            break;
+    const char *envx = getenv("PPL_FULL_STRIPS");  // debug override: 1 = one strip, 2 = two whenever they fit
+    const char *envt = getenv("PPL_FULL_TIGHT");   // debug override: 1 = memory-tight mode even when the slab strip fits
+    const int tbg0 = tbg;
+    size_t x_bytes = 0;
+    bool two_strips = false, fits = false;
+    // First the slab strip (16 v^3 doubles: step 0 on d-block >= b-block only, 1/8 of nominal).  If it does not fit under
+    // the cap, the memory-tight mode: a strip of one (slab; b-group) tile (16 tbg v^2), step 0 per tile on the group's
+    // full (b, d) rectangle (1/4 of nominal), everything behind the fold unchanged.
+    for (int tight = (envt && atoi(envt) == 1) ? 1 : 0; tight <= 1 && !fits; ++tight)
+        for (tbg = tbg0;; tbg = std::max(16, tbg / 2 / 16 * 16)) {
+            x_bytes = align256((size_t)TA * (tight ? tbg : v) * p->vvp * 8);
+            // A second strip pays where slabs are short (medium: 26.19 -> 25.82 ms for 1 GB); at large it buys 0.15 % for
+            // 8.2 GB and is not taken.  In the tight mode it is what lets step 0 of tile k+1 overlap the GEMMs of tile k.
+            const int want_strips = envx ? (atoi(envx) == 1 ? 1 : 2) : ((tight || x_bytes <= ((size_t)2 << 30)) ? 2 : 1);
+            const size_t slot = align256((size_t)TA * tbg * p->ldp * 8) + align256((size_t)TA * tbg * p->ldm * 8);
+            const size_t part_cap = std::max<size_t>((size_t)64 << 20, slot / 8);
+            full_geometry(p, tbg, part_cap, &chunks, tight != 0);
+            const size_t chunk_bytes = align256(chunks.size() * sizeof(int2));
+            const size_t base = x_bytes + align256(p->fpart_bytes) + racc_bytes + chunk_bytes + lpad_bytes + 256;
+            int ns = 0;
+            for (int s = want_slots; s >= 1 && !ns; --s)
+                if (base + s * slot <= room) ns = s;
+            if (ns) {
+                p->tbg = tbg;
+                p->fslots = ns;
+                p->full_tight = tight;
+                p->fws_bytes = base + ns * slot;
+                two_strips = want_strips == 2 && ns == want_slots && p->fws_bytes + x_bytes <= room;
+                if (two_strips) p->fws_bytes += x_bytes;
+                fits = true;
+                break;
+            }
+            if (tbg == 16) break;
         }
-        if (tbg == 16) return PPL_OK;  // does not fit: the plan stays without PPL_SYM_FULL
-    }
+    if (!fits) return PPL_OK;  // the plan stays without PPL_SYM_FULL
     if (dry) {  // geometry only (ppl_plan_dry): slabs, tiles, splits and byte counts are final at this point
         p->full_ok = 1;
         return PPL_OK;
@@ -1066,7 +1092,7 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
     auto te = [&](cudaStream_t st) {
         if (trace) cudaEventRecord(tr.back().e, st);
     };
-    int tile_no = 0, slab_no = 0;
+    int tile_no = 0;
     // Two strips: step 0 runs on its own stream, one slab ahead of the folds (strip k & 1), so that the HBM-bound fold of
     // slab k and the tail of its GEMMs are filled by the DMMA work of slab k + 1 instead of standing between two slabs.
     const bool dual = conc && p->fX2 != nullptr;
@@ -1075,21 +1101,29 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
         PPL_CUDA(cudaEventRecord(p->ev_fork, stream));
         PPL_CUDA(cudaStreamWaitEvent(s0, p->ev_fork, 0));
     }
-    for (const FullSlab &sl : p->slabs) {
-        const int xi = dual ? (slab_no & 1) : 0;
-        double *const X = xi ? p->fX2 : p->fX;
+    // One unit of step 0: a slab (the whole strip: d-block >= b-block plus the b<->d image) or, in the memory-tight mode,
+    // one (slab; b-group) tile on its full (b, d) rectangle.  Unit u writes strip u & 1 when there are two.
+    const bool tight = p->full_tight != 0;
+    int unit_no = 0, xi = 0;
+    double *X = p->fX;
+    auto step0_unit = [&](const FullSlab &sl, const FullTile *t) -> int {
+        xi = dual ? (unit_no & 1) : 0;
+        X = xi ? p->fX2 : p->fX;
         ppl::Step0SlabArgs a0;
         a0.A0 = sl.A0;
         a0.ta = sl.ta;
         a0.v = p->vp;
         a0.K = p->x;
         a0.tiles_m = sl.tiles_m;
-        a0.tiles_n = sl.tiles_n;
-        a0.chunks = p->fchunks + sl.chunk_off;
+        a0.tiles_n = t ? t->tiles_n : sl.tiles_n;
+        a0.chunks = p->fchunks + (t ? t->chunk_off : sl.chunk_off);
         a0.X = X;
-        const int items = sl.tiles_m * sl.tiles_n;
-        if (dual && slab_no >= 2) PPL_CUDA(cudaStreamWaitEvent(s0, p->ev_xfree[xi], 0));  // the folds of slab k - 2 have read this strip
-        tb("step0", sl.A0, 0, s0);
+        a0.rows_per_a = t ? t->tbp : p->vp;
+        a0.b_base = t ? t->bg0 : 0;
+        a0.image = t ? 0 : 1;
+        const int items = a0.tiles_m * a0.tiles_n;
+        if (dual && unit_no >= 2) PPL_CUDA(cudaStreamWaitEvent(s0, p->ev_xfree[xi], 0));  // the folds of unit u - 2 have read this strip
+        tb("step0", t ? t->bg0 : sl.A0, 0, s0);
         ppl::k_step0_slab<<<std::min(items, p->num_sms), ppl::TMA_THREADS, ppl::SMEM_TMA, s0>>>(mapL, a0);
         te(s0);
         PPL_CUDA(cudaGetLastError());
@@ -1099,10 +1133,20 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
             PPL_CUDA(cudaEventRecord(p->ev_s0[xi], s0));
             PPL_CUDA(cudaStreamWaitEvent(stream, p->ev_s0[xi], 0));
         }
-        if (tau_ready && sl.A0 == 0) PPL_CUDA(cudaStreamWaitEvent(stream, tau_ready, 0));
+        if (tau_ready && unit_no == 0) PPL_CUDA(cudaStreamWaitEvent(stream, tau_ready, 0));
+        return PPL_OK;
+    };
+    auto unit_done = [&]() -> int {  // behind the last fold that reads the unit's strip
+        if (dual) PPL_CUDA(cudaEventRecord(p->ev_xfree[xi], stream));
+        ++unit_no;
+        return PPL_OK;
+    };
+    for (const FullSlab &sl : p->slabs) {
+        if (!tight && (rc = step0_unit(sl, nullptr)) != PPL_OK) return rc;
         for (int k = sl.tile_begin; k < sl.tile_end; ++k) {
             const FullTile &t = p->ftiles[k];
             const int N = TA * t.tbp;
+            if (tight && (rc = step0_unit(sl, &t)) != PPL_OK) return rc;
             const int sl_w = conc ? (tile_no % p->fslots) : 0;  // W+- slot of this tile
             if (conc && tile_no >= p->fslots)  // the GEMMs of the tile that used this slot last still read it
                 for (int i = 0; i < 4; ++i) PPL_CUDA(cudaStreamWaitEvent(stream, p->evg[sl_w][i], 0));
@@ -1120,6 +1164,8 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
                 f.scale = 1.0;
                 f.diag = 2.0;
                 f.tbp = t.tbp;
+                f.rows_per_a = tight ? t.tbp : p->vp;
+                f.b_base = tight ? t.bg0 : 0;
                 f.bg0 = t.bg0;
                 f.A0 = t.A0;
                 f.ta = t.ta;
@@ -1136,6 +1182,7 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
                 PPL_CUDA(cudaGetLastError());
                 PPL_DBG("k_symfold", k);
                 PPL_MARK(K_FOLD, 1);
+                if (tight && (rc = unit_done()) != PPL_OK) return rc;
             }
             // The four GEMMs of the tile are independent given the fold (use 1 writes the R+-acc columns of the slab,
             // use 2 those above it; + and - are different matrices): outside the profiled pass each runs on a side
@@ -1202,8 +1249,7 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
                 for (int i = 0; i < 4; ++i) PPL_CUDA(cudaEventRecord(p->evg[sl_w][i], p->fs[i]));
             ++tile_no;
         }
-        if (dual) PPL_CUDA(cudaEventRecord(p->ev_xfree[xi], stream));  // behind the last fold of this slab
-        ++slab_no;
+        if (!tight && (rc = unit_done()) != PPL_OK) return rc;
     }
     if (conc)  // join: the side streams run in order, so the events of the last min(tiles, slots) tiles cover all work
         for (int s = 0; s < std::min(tile_no, p->fslots); ++s)
@@ -1567,6 +1613,7 @@ int ppl_plan_info(const ppl_plan_t *p, ppl_info_t *out) {
     out->full_available = p->full_ok;
     out->full_tbg = p->tbg;
     out->full_slabs = (int)p->slabs.size();
+    out->full_tight = p->full_ok ? p->full_tight : 0;
     out->full_workspace_bytes = p->fws_bytes;
     out->workspace_bytes = p->ws_bytes + p->fws_bytes;
     if (p->sym == PPL_SYM_FULL) {
@@ -1577,7 +1624,8 @@ int ppl_plan_info(const ppl_plan_t *p, ppl_info_t *out) {
         out->n_tiles = (int)p->ftiles.size();
         out->ring = 1;
         out->splitk = p->ftiles.empty() ? 0 : p->ftiles[0].sp.splitk;
-        int launches = 2 + (int)p->slabs.size() + ((p->v & 1) ? 1 : 0);  // pack, unpack, one step 0 per slab (+ the L pad copy for odd nvirt)
+        // pack, unpack, one step 0 per slab -- per tile in the memory-tight mode -- (+ the L pad copy for odd nvirt)
+        int launches = 2 + (int)(p->full_tight ? p->ftiles.size() : p->slabs.size()) + ((p->v & 1) ? 1 : 0);
         for (const FullTile &t : p->ftiles) {
             const bool m1 = minus && p->Km - t.k0m > 0;
             launches += 1 + (m1 ? 4 : 2) + (p->Kp - t.k1p > 0 ? 1 : 0) + (minus && p->Km - t.k1m > 0 ? 1 : 0);

@@ -397,6 +397,7 @@ struct FoldArgs {
     double diag;         // factor of the diagonal (c==d) entries of the + part: PPL_SYM_PAIR_SA 1 (W), 1 (tau);
                          // PPL_SYM_FULL 2 (W), 1/2 (tau) -- same products, but W+ becomes a symmetric matrix
     int tbp, bg0, A0, ta;  // mode 2
+    int rows_per_a = 0, b_base = 0;  // mode 2: strip row of (a_l, b) is a_l * rows_per_a + b - b_base (v, 0: the slab's whole strip)
     int cb_min;          // first FT-block of c that is processed (mode 2: A0 / FT; else 0)
     double *dp, *dm;     // packed outputs, row strides ldp / ldm
     int64_t ldp, ldm;
@@ -421,7 +422,7 @@ __device__ __forceinline__ FoldRow fold_row(const FoldArgs &p, int r) {
         const int al = r / p.tbp, bl = r - al * p.tbp;
         const int a = p.A0 + al, b = p.bg0 + bl;
         f.zero = al >= p.ta || b >= p.v || a > b;
-        f.roff = f.zero ? 0 : ((int64_t)al * p.v + b) * p.s_row;
+        f.roff = f.zero ? 0 : ((int64_t)al * p.rows_per_a + b - p.b_base) * p.s_row;
         f.rowp = f.rowm = r;
     } else {
         const int i = r / p.o, j = r - i * p.o;

@@ -35,7 +35,11 @@ struct Step0SlabArgs {
     int v, K;            // nvirt, nchol
     int tiles_m, tiles_n;
     const int2 *chunks;  // [8 * tiles_n] (b, d0)
-    double *X;           // strip [(a_l * v + b)][c * v + d], row stride v*v
+    double *X;           // strip [(a_l * rows_per_a + b - b_base)][c * v + d], row stride v*v
+    int rows_per_a;      // strip rows per a_l: v (the slab's whole strip) or the b-group width (memory-tight mode)
+    int b_base;          // first b of the strip: 0, or the b-group's first b
+    int image;           // 1: chunks cover d-block >= b-block only and the epilogue stores the b<->d image too (rows of
+                         // every b >= A0 must be in the strip); 0: the chunks cover the full (b, d) rectangle of the group
 };
 
 __global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_slab(const __grid_constant__ CUtensorMap mapL, const Step0SlabArgs p) {
@@ -144,12 +148,12 @@ __global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_slab(const __grid_cons
             for (int e = 0; e < 2; ++e) {
                 const int al = 2 * c + e;
                 if (al >= p.ta) continue;
-                double *xa = p.X + (int64_t)al * v * vv + (int64_t)cc * v;  // + b*vv + d
+                double *xa = p.X + ((int64_t)al * p.rows_per_a - p.b_base) * vv + (int64_t)cc * v;  // + b*vv + d
 #pragma unroll
                 for (int j = 0; j < 2; ++j) {
                     const int b = ch[j].x, d0 = ch[j].y;
                     if (b < 0) continue;
-                    const bool offdiag = d0 != p.A0 + ((b - p.A0) & ~15);  // d-block above the b-block: store the b<->d image too
+                    const bool offdiag = p.image && d0 != p.A0 + ((b - p.A0) & ~15);  // d-block above the b-block: store the b<->d image too
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
                         const int d = d0 + 2 * q + 8 * h;
@@ -166,7 +170,7 @@ __global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_slab(const __grid_cons
                         }
                     }
                 }
-                if (pair) {
+                if (pair && p.image) {
                     const int b = ch[0].x, d0 = ch[0].y;
                     if (d0 != p.A0 + ((b - p.A0) & ~15)) {  // b, b+1 share a 16-block (b even)
 #pragma unroll

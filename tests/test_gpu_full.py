@@ -231,3 +231,75 @@ def test_one_and_two_strips_agree_bit_for_bit(shape):
     assert got["2"][1] > got["1"][1]  # the second strip was really allocated
     assert np.abs(got["2"][0] - 2.0 * want).max() <= 1e-11 * np.abs(2.0 * want).max()
     assert np.array_equal(got["1"][0], got["2"][0])
+
+
+@pytest.fixture
+def tight_env():
+    old = {k: os.environ.get(k) for k in ("PPL_FULL_TIGHT", "PPL_TBG", "PPL_FULL_STRIPS")}
+    yield lambda **kw: [os.environ.__setitem__(k, str(val)) for k, val in kw.items()]
+    for k, val in old.items():
+        if val is None:
+            os.environ.pop(k, None)
+        else:
+            os.environ[k] = val
+
+
+@pytest.mark.parametrize("shape", [(1, 2, 1), (2, 16, 4), (12, 18, 9), (5, 20, 60), (3, 40, 33), (6, 50, 70), (5, 53, 40), (4, 98, 30), (7, 130, 20)])
+@pytest.mark.parametrize("tbg,strips", [(16, 2), (32, 1), (256, 2)])
+def test_memory_tight_mode_parity(shape, tbg, strips, tight_env):
+    """PPL_SYM_FULL with a strip of one (slab; b-group) tile: step 0 per tile on the full (b, d) rectangle (no image),
+    the fold and the GEMMs unchanged.  Forced here (PPL_FULL_TIGHT=1); taken by the planner when 16 v^3 does not fit."""
+    o, v, x = shape
+    tight_env(PPL_FULL_TIGHT=1, PPL_TBG=tbg, PPL_FULL_STRIPS=strips)
+    L = I.make_L(v, x, 81, symmetric=True)
+    t2 = I.make_t2(o, v, 81, symmetric=True)
+    R0 = I.make_vec(o * o * v * v, 82, 40).reshape(o, o, v, v)
+    want = oracle.full(L, t2, R0.copy())
+    got, info = gpu_ladder(L, t2, R0=R0.copy(), sym=P.PPL_SYM_FULL, return_info=True)
+    assert info["full_tight"] == 1 and info["symmetry"] == P.PPL_SYM_FULL, info
+    assert relerr(got, want) <= 1e-11, info
+
+
+@pytest.mark.parametrize("shape", [(5, 20, 60), (4, 38, 19), (24, 64, 128), (7, 82, 33), (3, 130, 12), (5, 53, 40)])
+def test_memory_tight_mode_exact_integers_and_flops(shape, tight_env):
+    o, v, x = shape
+    L = I.make_L(v, x, 83, symmetric=True, integer=True)
+    t2 = 2.0 * I.make_t2(o, v, 83, symmetric=True, integer=True)
+    want = oracle.full(L, t2)
+    tight_env(PPL_FULL_TIGHT=0, PPL_TBG=32)
+    ref, info_ref = gpu_ladder(L, t2, sym=P.PPL_SYM_FULL, return_info=True)
+    tight_env(PPL_FULL_TIGHT=1, PPL_TBG=32)
+    got, info = gpu_ladder(L, t2, sym=P.PPL_SYM_FULL, return_info=True)
+    assert info["full_tight"] == 1 and info_ref["full_tight"] == 0
+    assert np.array_equal(got, want) and np.array_equal(ref, want)
+    # same step 1; step 0 on the full rectangle: more than the image mode, at most about twice it
+    assert info["flops_step1"] == info_ref["flops_step1"]
+    assert info_ref["flops_step0"] <= info["flops_step0"] <= 2.0 * info_ref["flops_step0"]  # equal when one CTA tile covers either
+    if v >= 64:
+        assert info["flops_step0"] > 1.2 * info_ref["flops_step0"]
+    assert info["full_workspace_bytes"] < info_ref["full_workspace_bytes"] or v <= 32
+
+
+def test_memory_tight_mode_is_what_a_small_cap_gets(tight_env):
+    """Under a cap that has no room for the 16 v^3 strip the planner keeps the 8-fold path in its memory-tight form."""
+    import torch
+
+    o, v, x = 6, 128, 40
+    L = I.make_L(v, x, 85, symmetric=True)
+    t2 = I.make_t2(o, v, 85, symmetric=True)
+    want = oracle.full(L, t2)
+    with P.Plan(o, v, x, 0) as plan:
+        roomy = plan.info()
+    assert roomy["full_available"] == 1 and roomy["full_tight"] == 0
+    free = torch.cuda.mem_get_info()[0]
+    cap = roomy["workspace_bytes"]
+    while True:  # shrink the cap until the planner (asked without the device) gives up the 16 v^3 strip (268 MB here)
+        cap -= 32 << 20
+        dry = P.ppl_plan_dry(o, v, x, workspace_bytes=cap, device_free_bytes=free)
+        assert dry["full_available"] == 1, "the tight mode should come before PPL_SYM_FULL is lost"
+        if dry["full_tight"]:
+            break
+    got, info = gpu_ladder(L, t2, sym=P.PPL_SYM_FULL, workspace_bytes=cap, return_info=True)
+    assert info["full_tight"] == 1 and info["workspace_bytes"] <= cap, info
+    assert relerr(got, want) <= 1e-11
+    assert dry["full_tbg"] == info["full_tbg"] and dry["n_tiles"] == info["n_tiles"]

@@ -118,9 +118,23 @@ def test_workspace_caps_and_fallbacks():
     # a device with little free memory behaves like a cap
     small_dev = P.ppl_plan_dry(o, v, x, device_free_bytes=4 << 30)
     assert small_dev["workspace_bytes"] <= 0.9 * (4 << 30) and small_dev["full_available"] == 0
-    # near the HBM limit (DESIGN 6.2): (80, 800, 3200) with 82 GB of inputs resident leaves no room for PPL_SYM_FULL
+    # near the HBM limit (DESIGN 6.2): (80, 800, 3200) with 82 GB of inputs resident leaves no room for the 65.5 GB strip
+    # of PPL_SYM_FULL: the plan keeps the 8-fold path in its memory-tight form (a strip of one (slab; b-group) tile)
     big = P.ppl_plan_dry(80, 800, 3200, device_free_bytes=(178 - 82) << 30)
-    assert big["full_available"] == 0 and big["symmetry"] == P.PPL_SYM_PAIR_SA and big["ta"] == 16
+    assert big["full_available"] == 1 and big["full_tight"] == 1 and big["symmetry"] == P.PPL_SYM_FULL
+    assert big["workspace_bytes"] <= 0.9 * ((178 - 82) << 30)
+    n0, n1 = 2.0 * 3200 * 800 ** 4, 2.0 * 6400 * 800 ** 4
+    assert 2.0 <= big["flops_step0"] / (n0 / 8) <= 2.3    # the full (b, d) rectangle: a quarter of nominal, not an eighth
+    assert 1.0 <= big["flops_step1"] / (n1 / 4) <= 1.04   # step 1 as in the roomy plan
+    # between "fits" and "PPL_SYM_FULL lost" there is always the tight form
+    seen_tight = False
+    for mb in range(22000, 2000, -500):
+        d = P.ppl_plan_dry(o, v, x, workspace_bytes=mb << 20)
+        seen_tight = seen_tight or d["full_tight"] == 1
+        if not d["full_available"]:
+            break
+        assert d["full_tight"] in (0, 1) and d["symmetry"] == P.PPL_SYM_FULL
+    assert seen_tight
 
 
 @pytest.mark.parametrize("sms", [1, 8, 132, 148, 160])
