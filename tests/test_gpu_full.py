@@ -303,3 +303,21 @@ def test_memory_tight_mode_is_what_a_small_cap_gets(tight_env):
     assert info["full_tight"] == 1 and info["workspace_bytes"] <= cap, info
     assert relerr(got, want) <= 1e-11
     assert dry["full_tbg"] == info["full_tbg"] and dry["n_tiles"] == info["n_tiles"]
+
+
+@pytest.mark.parametrize("shape", [(6, 96, 40), (5, 131, 20), (7, 98, 12)])
+def test_host_entry_point_in_the_memory_tight_form(shape, chunk_env, tight_env):
+    """ppl_apply_host (t2 and R streamed in chunks) on a plan whose PPL_SYM_FULL buffers are the one-tile-strip kind."""
+    o, v, x = shape
+    chunk_env(1)
+    tight_env(PPL_FULL_TIGHT=1, PPL_TBG=32)
+    L = I.make_L(v, x, 91, symmetric=True, integer=True)
+    t2 = 2.0 * I.make_t2(o, v, 91, symmetric=True, integer=True)
+    R0 = I.make_vec(o * o * v * v, 92, 40, integer=True).reshape(o, o, v, v)
+    want = oracle.full(L, t2, R0.copy())
+    R = R0.copy()
+    with P.Plan(o, v, x) as plan:
+        info = plan.info()
+        assert info["symmetry"] == P.PPL_SYM_FULL and info["full_tight"] == 1
+        plan.apply_host(L, t2, R)
+    assert np.array_equal(R, want)
