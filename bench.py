@@ -168,6 +168,8 @@ TABLE3_PAPER_SECONDS = {
                          "H100 CuPy C-split": 461.5, "GH200 PyTorch X-split": 574.7, "H100 PyTorch X-split": 789.4},
     "table3_n900_o100": {"GH200 PyTorch C-split": 587.1, "GH200 CuPy C-split": 495.0, "H100 PyTorch C-split": 496.2,
                          "H100 CuPy C-split": 809.7, "GH200 PyTorch X-split": 1265.7, "H100 PyTorch X-split": 1753.3},
+    "table3_n1000_o50": {"GH200 PyTorch C-split": 574.6, "GH200 CuPy C-split": 763.0, "H100 PyTorch C-split": 673.0,
+                         "H100 CuPy C-split": 1006.4, "GH200 PyTorch X-split": 5262.6},
 }
 
 
@@ -226,7 +228,7 @@ def run_table3(args, o, v, x):
                    "note": "shape of the paper's Table 3 row (PAPER.md:417-451); operands in pinned HOST memory; "
                            "symmetric L and pair-symmetric t2 (the paper used unstructured random arrays and no symmetry)",
                    "symmetry": SYM_DESC[info["symmetry"]],
-                   "plan": {k: info[k] for k in ("ta", "tb", "n_tiles", "workspace_bytes")}},
+                   "plan": {k: info[k] for k in ("ta", "tb", "n_tiles", "workspace_bytes", "full_tight")}},
         "step_seconds": secs, "plan_seconds": plan_s, "input_gen_seconds": t_gen,
         "tflops_executed": f_exec / dt * 1e-12, "tflops_nominal_effective": f_nom / dt * 1e-12,
         "flops_executed": f_exec, "flops_nominal": f_nom,
