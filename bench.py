@@ -168,6 +168,10 @@ TABLE3_PAPER_SECONDS = {
                          "H100 CuPy C-split": 461.5, "GH200 PyTorch X-split": 574.7, "H100 PyTorch X-split": 789.4},
     "table3_n900_o100": {"GH200 PyTorch C-split": 587.1, "GH200 CuPy C-split": 495.0, "H100 PyTorch C-split": 496.2,
                          "H100 CuPy C-split": 809.7, "GH200 PyTorch X-split": 1265.7, "H100 PyTorch X-split": 1753.3},
+    "table3_n800_o150": {"GH200 PyTorch C-split": 475.3, "GH200 CuPy C-split": 532.8, "H100 PyTorch C-split": 651.2,
+                         "H100 CuPy C-split": 940.9, "GH200 PyTorch X-split": 637.4},
+    "table3_n1000_o100": {"GH200 PyTorch C-split": 805.8, "GH200 CuPy C-split": 829.1, "H100 PyTorch C-split": 827.1,
+                          "H100 CuPy C-split": 1338.7, "GH200 PyTorch X-split": 2673.7},
     "table3_n1000_o50": {"GH200 PyTorch C-split": 574.6, "GH200 CuPy C-split": 763.0, "H100 PyTorch C-split": 673.0,
                          "H100 CuPy C-split": 1006.4, "GH200 PyTorch X-split": 5262.6},
 }
@@ -198,6 +202,15 @@ def run_table3(args, o, v, x):
     plan = P.Plan(o, v, x, cap)
     plan_s = time.perf_counter() - t0
     info = plan.info()
+    need = (x * v * v + 2 * o * o * v * v) * 8
+    avail = 0
+    for ln in open("/proc/meminfo"):
+        if ln.startswith("MemAvailable"):
+            avail = int(ln.split()[1]) * 1024
+    if need > 0.845 * avail:  # pinned pages cannot be swapped; 162 GB of 194 GB pins on this pool's hosts, 166 GB does not
+        plan.destroy()
+        print(json.dumps({"unavailable": f"{need / 1e9:.0f} GB of pinned host operands on a host with {avail / 1e9:.0f} GB available"}))
+        return
     t_gen = time.perf_counter()
     Lh = torch.empty((x, v, v), dtype=torch.float64, pin_memory=True)
     th = torch.empty((o, o, v, v), dtype=torch.float64, pin_memory=True)

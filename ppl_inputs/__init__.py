@@ -30,6 +30,8 @@ CONFIG_ORDER = ["tiny", "small", "medium", "large", "xl"]
 TABLE3_SHAPES = {
     "table3_n800_o100": (100, 700, 4000),
     "table3_n900_o100": (100, 800, 4500),
+    "table3_n800_o150": (150, 650, 4000),  # PAPER.md:440-441 (nvec = 5 N = 4000; 166 GB of host operands)
+    "table3_n1000_o100": (100, 900, 5000),  # PAPER.md:432-433 (162 GB of host operands)
     "table3_n1000_o50": (50, 950, 10000),   # PAPER.md:448-449 (nvec = 10 N: the row with the paper's best derived rate)
 }
 
