@@ -192,6 +192,10 @@ int ppl_apply_dense(ppl_plan_t *plan, const double *eri, int a0, int na, const d
  *     is unpacked chunk by chunk (R chunk in, R += term, R chunk out), copies of one chunk overlapping the kernels of
  *     the other.  Device residency is about half of L + t2 + R: shapes of the paper's Table 3 fit on one 180 GB GPU.
  *   other modes: L, t2 and R are copied whole, ppl_apply runs, R is copied back (PPL_ERR_ALLOC if they do not fit).
+ *   At shapes that fill the device, plan with workspace_bytes = free device bytes - |L| - 3 GiB (what bench.py's
+ *   table3_* configs do): the automatic cap of ppl_plan (90 % of the free bytes) leaves no room for L and the staging
+ *   buffers, and the call then returns PPL_ERR_ALLOC.  Under such a cap the plan takes the memory-tight form of
+ *   PPL_SYM_FULL (ppl_info_t.full_tight) when the 16 nvirt^3 strip does not fit.
  * h2d/d2h byte counts are returned if non-NULL.  R accumulates (+=) as in ppl_apply. */
 int ppl_apply_host(ppl_plan_t *plan, const double *L_host, const double *t2_host, double *R_host,
                    uint64_t *h2d_bytes, uint64_t *d2h_bytes);
