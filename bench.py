@@ -151,9 +151,12 @@ def run_reference(args, o, v, x):
         "impl": "reference", "metric": METRIC, "value": tflops, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.config, "nocc": o, "nvirt": v, "nchol": x, "seed": 0},
+        "config": workload_config(args.config, o, v, x),
+        "seconds_per_call": dt / args.steps / len(pairs) * v * v,
+        "seconds_per_call_how": "EXTRAPOLATED: measured seconds per sampled (a,b) column x nvirt^2 columns",
         "cpu_baseline": {"value": tflops, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-                         "sample": f"{len(pairs)} of {v*v} (a,b) columns per step (oracle.columns), all i,j"},
+                         "sample": f"{len(pairs)} of {v*v} (a,b) columns per step (oracle.columns), all i,j",
+                         "extrapolated_seconds_per_call": dt / args.steps / len(pairs) * v * v},
         "e2e": {"value": tflops, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -328,12 +331,216 @@ def replicas_value(flops_per_replica: float, ms_per_step: float, world: int) -> 
 
 
 # -------------------------------------------------------------------------------------------- ours
+L2_BYTES = 126 << 20
+
+
+def workload_config(name, o, v, x):
+    """The `config` object: identical in both arms (ours / reference) so that the lines are comparable."""
+    small = (x * v * v + 2 * o * o * v * v) * 8 < 2 * L2_BYTES
+    return {"workload": name, "nocc": o, "nvirt": v, "nchol": x, "seed": 0,
+            "l2": ("flushed between timed iterations (256 MiB memset outside the event pair): inputs smaller than L2"
+                   if small else "inputs larger than L2 (L, t2, W tiles >> 126 MB); no flush needed")}
+
+
+def probe_leg():
+    """--probe: the instruction streams the pipe choice was made between, cuBLAS DGEMM for context, clocks."""
+    import torch
+
+    import paper_2603_20912_b200 as P
+
+    torch.cuda.set_device(0)
+    sampler = ClockSampler(0)
+    sampler.start()
+    out = {k: P.ppl_probe_fp64_pipe(k, 3, 50.0) for k in ("dmma8", "dmma16", "dfma16", "mix8")}
+    n = 8192
+    a = torch.randn(n, n, dtype=torch.float64, device="cuda")
+    b = torch.randn(n, n, dtype=torch.float64, device="cuda")
+    for _ in range(2):
+        torch.matmul(a, b)
+    best = 0.0
+    for _ in range(10):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        torch.matmul(a, b)
+        e1.record()
+        torch.cuda.synchronize()
+        best = max(best, 2.0 * n ** 3 / (e0.elapsed_time(e1) * 1e-3) * 1e-12)
+    out["cublas_dgemm_8192"] = best
+    out["nominal"] = NOMINAL_FP64_TFLOPS
+    out["unit"] = UNIT
+    out["clocks"] = sampler.stop()
+    out["what"] = ("register-only loops, 16 warps/SM x 148 SMs: dmma8/dmma16 = mma.sync.m8n8k4.f64 with 8/16 independent "
+                   "accumulator chains per warp; dfma16 = DFMA, 16 chains per thread; mix8 = DMMA + DFMA interleaved "
+                   "(flops of both counted); cublas = torch.matmul FP64 8192^3 best of 10 (library bar, context)")
+    print(json.dumps(out))
+
+
+def run_ours(name, o, v, x, args, steps, warmup, dist, dev, rank, world, peak):
+    """One workload through ppl_apply (device-resident), ppl_apply_profiled (roofline), ppl_apply_host (e2e) and the
+    oracle sample (cpu_baseline + parity).  Returns the JSON record."""
+    import numpy as np
+    import torch
+
+    import paper_2603_20912_b200 as P
+    import ppl_inputs as I
+
+    # ---- seeded synthetic inputs in pinned host memory (shared bit-for-bit with the oracle) ----
+    t_gen = time.perf_counter()
+    Lh = torch.empty((x, v, v), dtype=torch.float64, pin_memory=True)
+    th = torch.empty((o, o, v, v), dtype=torch.float64, pin_memory=True)
+    Rh = torch.zeros((o, o, v, v), dtype=torch.float64, pin_memory=True)
+    I.make_L(v, x, 0, out=Lh.numpy())
+    I.make_t2(o, v, 0, out=th.numpy())
+    t_gen = time.perf_counter() - t_gen
+    Ld, td = Lh.to(dev, non_blocking=True), th.to(dev, non_blocking=True)
+    Rd = torch.zeros((o, o, v, v), dtype=torch.float64, device=dev)
+    torch.cuda.synchronize()
+
+    t0 = time.perf_counter()
+    plan = P.Plan(o, v, x, int(args.workspace_gb * (1 << 30)))
+    plan_s = time.perf_counter() - t0
+    if args.symmetry != "default":
+        plan.set_symmetry({v_: k_ for k_, v_ in SYM_NAMES.items()}[args.symmetry])
+    plan.set_graph({"auto": -1, "off": 0, "on": 1}[args.graph])
+    info = plan.info()
+    stream = torch.cuda.current_stream()
+    cfg = workload_config(name, o, v, x)
+    flush = cfg["l2"].startswith("flushed")
+    scratch = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if flush else None
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(warmup, 0)):
+        plan.apply(Ld, td, Rd)
+    barrier()
+    sampler = ClockSampler(dev.index or 0)
+    sampler.start()
+    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
+    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
+    barrier()
+    for k in range(steps):
+        if flush:
+            scratch.zero_()  # outside the event pair
+        ev0[k].record(stream)
+        plan.apply(Ld, td, Rd)  # R accumulates (+=) across steps; no work is skipped
+        ev1[k].record(stream)
+    barrier()
+    clocks = sampler.stop()
+    step_ms = [ev0[k].elapsed_time(ev1[k]) for k in range(steps)]
+    # without a flush the steps run back to back: the span first start -> last end is the timed region
+    total_ms = sum(step_ms) if flush else ev0[0].elapsed_time(ev1[-1])
+    total_ms = max_over_ranks(total_ms, dist, dev)
+    ms_per_step = total_ms / steps
+    sec = ms_per_step * 1e-3
+    f_exec, f_nom, f_use = info["flops_executed"], info["flops_nominal"], info["flops_useful"]
+    value = replicas_value(f_exec, ms_per_step, world)
+
+    # ---- dominant kernel, timed live with CUDA events on the launching stream (serialised pass) ----
+    Rd.zero_()
+    prof = plan.apply_profiled(Ld, td, Rd)  # Rd now holds exactly one application of the term
+    torch.cuda.synchronize()
+    dom = "step0" if prof["step0_ms"] >= prof["step1_ms"] else "step1"
+    dom_flops = info["flops_" + dom] / max(prof["n_" + dom], 1)
+    dom_ms = prof[dom + "_ms"] / max(prof["n_" + dom], 1)
+    achieved = dom_flops / (dom_ms * 1e-3) * 1e-12
+    dom_useful = info["flops_useful_" + dom] / (prof[dom + "_ms"] * 1e-3) * 1e-12
+    traffic = None
+    try:
+        import csv
+
+        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "dram_traffic.csv"))):
+            if row["config"] == name and row["symmetry"] == SYM_NAMES[info["symmetry"]] and row["kernel"] == dom:
+                traffic = float(row["dram_bytes_per_launch"])
+    except Exception:
+        pass
+    roofline = {
+        "bound": "tensor", "kernel": "k_" + dom, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+        "frac": achieved / peak, "traffic": traffic,
+        "achieved_useful": dom_useful, "frac_useful": dom_useful / peak,
+        "peak_source": "measured live: ppl_probe_fp64_peak (register-only DMMA m8n8k4 stream; profiles/r02_fp64_peaks.md); "
+                       f"nominal {NOMINAL_FP64_TFLOPS:.2f} = 148 SM x 4 SMSP x 16 FMA/clk x 2 x 1.965 GHz",
+        "flops_per_launch": dom_flops, "ms_per_launch": dom_ms,
+        "how": "ppl_apply_profiled: one serialised apply after the timed steps, a CUDA event pair around every launch; "
+               "achieved = flops of the GEMM extents launched / time, achieved_useful = the symmetry-unique flops of the "
+               "same launches / the same time",
+        "step0_tflops": info["flops_step0"] / (prof["step0_ms"] * 1e-3) * 1e-12,
+        "step1_tflops": info["flops_step1"] / (prof["step1_ms"] * 1e-3) * 1e-12,
+        "share": {"step0": prof["step0_ms"] / prof["total_ms"], "step1": prof["step1_ms"] / prof["total_ms"],
+                  "reduce": prof["reduce_ms"] / prof["total_ms"], "fold": prof["fold_ms"] / prof["total_ms"],
+                  "pack": prof["pack_ms"] / prof["total_ms"]},
+        "launches": {k: prof["n_" + k] for k in ("step0", "step1", "reduce", "fold", "pack")},
+    }
+
+    rec = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": cfg,
+        "run": {"symmetry": SYM_DESC[info["symmetry"]], "parallelism": "replicas only" if world > 1 else "1 gpu",
+                "plan": {k: info[k] for k in ("ta", "tb", "n_tiles", "ring", "splitk", "vec16", "workspace_bytes")},
+                "graph": args.graph},
+        "seconds_per_call": sec,
+        "tflops_executed": f_exec / sec * 1e-12,
+        "tflops_useful": f_use / sec * 1e-12,
+        "tflops_nominal_effective": f_nom / sec * 1e-12,
+        "flops_executed": f_exec, "flops_useful": f_use, "flops_nominal": f_nom,
+        "executed_over_useful": f_exec / f_use,
+        "frac_of_fp64_peak_measured": f_exec / sec * 1e-12 / peak,
+        "frac_of_fp64_peak_measured_useful": f_use / sec * 1e-12 / peak,
+        "frac_of_fp64_peak_nominal": f_exec / sec * 1e-12 / NOMINAL_FP64_TFLOPS,
+        "step_ms": step_ms, "plan_seconds": plan_s, "input_gen_seconds": t_gen,
+        "clocks": clocks, "roofline": roofline,
+        "gpu_launches": info["launches_per_apply"] * steps,
+    }
+
+    if rank == 0 and not args.no_e2e:
+        # ---- end to end through the host entry point: H2D(L, t2, R) + apply + D2H(R) per step ----
+        n_e2e = max(1, args.e2e_steps if args.e2e_steps > 0 else steps)
+        Rh.zero_()
+        h2d, d2h = plan.apply_host(Lh, th, Rh)  # warm-up (allocates the staging buffers)
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            h2d, d2h = plan.apply_host(Lh, th, Rh)
+        dt = (time.perf_counter() - t0) / n_e2e
+        rec["e2e"] = {"value": world * f_exec / dt * 1e-12, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                      "d2h_bytes_per_step": d2h, "seconds_per_call": dt, "steps": n_e2e,
+                      "tflops_useful": world * f_use / dt * 1e-12,
+                      "how": "ppl_apply_host on pinned host buffers; wall clock around the synchronous call"}
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        # ---- the oracle on the host cores, bounded sample; the same sample checks the GPU result ----
+        pairs, cols, dt, cores = oracle_sample(Lh.numpy(), th.numpy(), o, v, x)
+        rec["cpu_baseline"] = {
+            "value": len(pairs) * col_flops(o, v, x) / dt * 1e-12, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{len(pairs)} of {v*v} (a,b) columns (oracle.columns), all i,j; {dt:.1f} s",
+            "extrapolated_seconds_per_call": dt / len(pairs) * v * v,
+        }
+        Rg = Rd.cpu().numpy()
+        got = Rg[:, :, pairs[:, 0], pairs[:, 1]].transpose(2, 0, 1)
+        err = float(np.abs(got - cols).max() / np.abs(cols).max())
+        rec["parity"] = {"max_rel_err_vs_oracle": err, "tolerance": 1e-11, "columns": int(len(pairs)), "ok": bool(err <= 1e-11)}
+
+    if rank == 0 and world == 1 and args.paper_recipe > 0:
+        Rd.zero_()
+        plan.apply(Ld, td, Rd)
+        torch.cuda.synchronize()
+        rec["paper_recipe"] = paper_recipe_leg(Ld, td, Rd, args.paper_recipe)
+
+    plan.destroy()
+    del Ld, td, Rd, Lh, th, Rh, scratch
+    torch.cuda.empty_cache()
+    return rec
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="large")
+    ap.add_argument("--config", default="xl", help="xl (default: the largest single-GPU config of BASELINE.json; the line "
+                    "then also carries a complete 'large' record), large, medium, small, tiny, table3_*")
     ap.add_argument("--shape", default=None, help="nocc,nvirt,nchol: a custom shape with the same generators (overrides --config)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workspace-gb", type=float, default=0.0, help="workspace cap (0 = auto)")
@@ -342,13 +549,19 @@ def main():
     ap.add_argument("--graph", default="auto", choices=["auto", "on", "off"],
                     help="ppl_plan_set_graph: replay one CUDA graph per apply (auto: launch-bound shapes only)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=0, help="timed ppl_apply_host calls (0 = --steps)")
+    ap.add_argument("--no-secondary", action="store_true", help="with --config xl: skip the 'large' sub-record")
     ap.add_argument("--paper-recipe", type=int, default=0, metavar="STEPS",
                     help="context leg: time STEPS calls of the paper's tensordot recipe (cuBLAS) on the same inputs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--probe", action="store_true", help="only measure the FP64 instruction-stream peaks and print them")
     args = ap.parse_args()
 
     import ppl_inputs as I
 
+    if args.probe:
+        probe_leg()
+        return
     if args.shape:
         o, v, x = (int(t) for t in args.shape.split(","))
         args.config = f"custom_{o}_{v}_{x}"
@@ -361,7 +574,6 @@ def main():
         run_reference(args, o, v, x)
         return
 
-    import numpy as np
     import torch
 
     import paper_2603_20912_b200 as P
@@ -379,140 +591,13 @@ def main():
         dist = dist_mod
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
-
-    # ---- seeded synthetic inputs in pinned host memory (shared bit-for-bit with the oracle) ----
-    t_gen = time.perf_counter()
-    Lh = torch.empty((x, v, v), dtype=torch.float64, pin_memory=True)
-    th = torch.empty((o, o, v, v), dtype=torch.float64, pin_memory=True)
-    Rh = torch.zeros((o, o, v, v), dtype=torch.float64, pin_memory=True)
-    I.make_L(v, x, 0, out=Lh.numpy())
-    I.make_t2(o, v, 0, out=th.numpy())
-    t_gen = time.perf_counter() - t_gen
-    Ld, td = Lh.to(dev, non_blocking=True), th.to(dev, non_blocking=True)
-    Rd = torch.zeros((o, o, v, v), dtype=torch.float64, device=dev)
-    torch.cuda.synchronize()
-
     peak = P.ppl_probe_fp64_peak(3, 20.0)
-    t0 = time.perf_counter()
-    plan = P.Plan(o, v, x, int(args.workspace_gb * (1 << 30)))
-    plan_s = time.perf_counter() - t0
-    if args.symmetry != "default":
-        plan.set_symmetry({v_: k_ for k_, v_ in SYM_NAMES.items()}[args.symmetry])
-    plan.set_graph({"auto": -1, "off": 0, "on": 1}[args.graph])
-    info = plan.info()
-    stream = torch.cuda.current_stream()
 
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    for _ in range(max(args.warmup, 0)):
-        plan.apply(Ld, td, Rd)
-    barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
-    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-    barrier()
-    evs[0].record(stream)
-    for k in range(args.steps):
-        plan.apply(Ld, td, Rd)  # R accumulates (+=) across steps; no work is skipped
-        evs[k + 1].record(stream)
-    barrier()
-    clocks = sampler.stop()
-    step_ms = [evs[k].elapsed_time(evs[k + 1]) for k in range(args.steps)]
-    total_ms = evs[0].elapsed_time(evs[-1])
-    total_ms = max_over_ranks(total_ms, dist, dev)
-    ms_per_step = total_ms / args.steps
-    f_exec, f_nom = info["flops_executed"], info["flops_nominal"]
-    value = replicas_value(f_exec, ms_per_step, world)
-
-    # ---- dominant kernel, timed live with CUDA events on the launching stream (serialised pass) ----
-    Rd.zero_()
-    prof = plan.apply_profiled(Ld, td, Rd)  # Rd now holds exactly one application of the term
-    torch.cuda.synchronize()
-    dom = "step0" if prof["step0_ms"] >= prof["step1_ms"] else "step1"
-    dom_flops = info["flops_" + dom] / prof["n_" + dom]
-    dom_ms = prof[dom + "_ms"] / prof["n_" + dom]
-    achieved = dom_flops / (dom_ms * 1e-3) * 1e-12
-    # per-launch DRAM traffic of the dominant kernel from the committed ncu --set full capture, if any
-    traffic = None
-    try:
-        import csv
-
-        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "dram_traffic.csv"))):
-            if row["config"] == args.config and row["symmetry"] == SYM_NAMES[info["symmetry"]] and row["kernel"] == dom:
-                traffic = float(row["dram_bytes_per_launch"])
-    except Exception:
-        pass
-    roofline = {
-        "bound": "tensor", "kernel": "k_" + dom, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-        "frac": achieved / peak, "traffic": traffic,
-        "peak_source": "measured live: ppl_probe_fp64_peak (register-only DMMA m8n8k4 stream); "
-                       f"nominal {NOMINAL_FP64_TFLOPS:.2f} = 148 SM x 4 SMSP x 16 FMA/clk x 2 x 1.965 GHz",
-        "flops_per_launch": dom_flops, "ms_per_launch": dom_ms,
-        "how": "ppl_apply_profiled: one serialised apply after the timed steps, a CUDA event pair around every launch",
-        "step0_tflops": info["flops_step0"] / (prof["step0_ms"] * 1e-3) * 1e-12,
-        "step1_tflops": info["flops_step1"] / (prof["step1_ms"] * 1e-3) * 1e-12,
-        "share": {"step0": prof["step0_ms"] / prof["total_ms"], "step1": prof["step1_ms"] / prof["total_ms"],
-                  "reduce": prof["reduce_ms"] / prof["total_ms"], "fold": prof["fold_ms"] / prof["total_ms"],
-                  "pack": prof["pack_ms"] / prof["total_ms"]},
-        "launches": {k: prof["n_" + k] for k in ("step0", "step1", "reduce", "fold", "pack")},
-    }
-
-    line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.config, "nocc": o, "nvirt": v, "nchol": x, "seed": 0,
-                   "symmetry": SYM_DESC[info["symmetry"]], "parallelism": "replicas only" if world > 1 else "1 gpu",
-                   "l2": "inputs larger than L2 (L, t2, W tiles >> 126 MB); no flush needed",
-                   "plan": {k: info[k] for k in ("ta", "tb", "n_tiles", "ring", "splitk", "vec16", "workspace_bytes")},
-                   "graph": args.graph},
-        "seconds_per_call": ms_per_step * 1e-3,
-        "tflops_executed": f_exec / (ms_per_step * 1e-3) * 1e-12,
-        "tflops_nominal_effective": f_nom / (ms_per_step * 1e-3) * 1e-12,
-        "flops_executed": f_exec, "flops_nominal": f_nom,
-        "frac_of_fp64_peak_measured": f_exec / (ms_per_step * 1e-3) * 1e-12 / peak,
-        "frac_of_fp64_peak_nominal": f_exec / (ms_per_step * 1e-3) * 1e-12 / NOMINAL_FP64_TFLOPS,
-        "step_ms": step_ms, "plan_seconds": plan_s, "input_gen_seconds": t_gen,
-        "clocks": clocks, "roofline": roofline,
-        "gpu_launches": info["launches_per_apply"] * args.steps,
-    }
-
-    if rank == 0 and not args.no_e2e:
-        # ---- end to end through the host entry point: H2D(L, t2, R) + apply + D2H(R) per step ----
-        n_e2e = max(1, min(args.steps, 3))
-        Rh.zero_()
-        h2d, d2h = plan.apply_host(Lh, th, Rh)  # warm-up (allocates the staging buffers)
-        t0 = time.perf_counter()
-        for _ in range(n_e2e):
-            h2d, d2h = plan.apply_host(Lh, th, Rh)
-        dt = (time.perf_counter() - t0) / n_e2e
-        line["e2e"] = {"value": world * f_exec / dt * 1e-12, "unit": UNIT, "h2d_bytes_per_step": h2d,
-                       "d2h_bytes_per_step": d2h, "seconds_per_call": dt, "steps": n_e2e,
-                       "how": "ppl_apply_host on pinned host buffers; wall clock around the synchronous call"}
-
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        # ---- the oracle on the host cores, bounded sample; the same sample checks the GPU result ----
-        pairs, cols, dt, cores = oracle_sample(Lh.numpy(), th.numpy(), o, v, x)
-        line["cpu_baseline"] = {
-            "value": len(pairs) * col_flops(o, v, x) / dt * 1e-12, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"{len(pairs)} of {v*v} (a,b) columns (oracle.columns), all i,j; {dt:.1f} s",
-            "extrapolated_seconds_per_call": dt / len(pairs) * v * v,
-        }
-        Rg = Rd.cpu().numpy()
-        got = Rg[:, :, pairs[:, 0], pairs[:, 1]].transpose(2, 0, 1)
-        err = float(np.abs(got - cols).max() / np.abs(cols).max())
-        line["parity"] = {"max_rel_err_vs_oracle": err, "tolerance": 1e-11, "columns": int(len(pairs)), "ok": bool(err <= 1e-11)}
-
-    if rank == 0 and world == 1 and args.paper_recipe > 0:
-        Rd.zero_()
-        plan.apply(Ld, td, Rd)
-        torch.cuda.synchronize()
-        line["paper_recipe"] = paper_recipe_leg(Ld, td, Rd, args.paper_recipe)
-
-    plan.destroy()
+    line = run_ours(args.config, o, v, x, args, args.steps, args.warmup, dist, dev, rank, world, peak)
+    if args.config == "xl" and not args.no_secondary and not args.shape:
+        # BASELINE.json quotes the metric on "the two largest configs": the other one rides on the same line
+        lo, lv, lx = I.CONFIGS["large"]
+        line["large"] = run_ours("large", lo, lv, lx, args, args.steps, args.warmup, dist, dev, rank, world, peak)
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()

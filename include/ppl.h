@@ -111,7 +111,9 @@ typedef struct ppl_info_s {
     int32_t step1_tile_m;      /* CTA tile rows of step 1 (16*NI chosen to tile nocc^2 with least padding) */
     uint64_t workspace_bytes;  /* device bytes owned by the plan */
     double flops_nominal;      /* F_nom */
-    double flops_executed;     /* F_exec: step 0 + step 1 over executed tiles (incl. tile padding: none) */
+    double flops_executed;     /* F_exec: the GEMM extents actually launched, step 0 + step 1 -- INCLUDING what the launches spend
+                                  on CTA-tile padding, pad chunks, structurally zero rows and slab-granularity overshoot
+                                  (the hardware-rate numerator; compare with flops_useful below) */
     double flops_step0;        /* executed flops of step 0 ('xac,xbd->acbd') */
     double flops_step1;        /* executed flops of step 1 ('acbd,ecfd->efab') */
     int32_t sa_splitk_plus, sa_splitk_minus; /* PPL_SYM_PAIR_SA: split-K of the + / - GEMMs (first tile) */
@@ -124,6 +126,14 @@ typedef struct ppl_info_s {
     int32_t full_tight;                      /* PPL_SYM_FULL buffers are the memory-tight kind: a strip of one (slab; b-group)
                                                 tile instead of the slab's 16 nvirt^3, step 0 per tile at 1/4 of nominal */
     uint64_t full_workspace_bytes;           /* part of workspace_bytes that belongs to PPL_SYM_FULL */
+    /* Useful flops: what the symmetry the mode exploits leaves to compute, with no tile padding, no zero rows and no
+     * slab-granularity overshoot -- the figure flops_executed is to be compared with (bench.py prints both rates).
+     *   PPL_SYM_FULL:    step 0  2 nchol U, U = P (P + 1) / 2 unique (ac|bd) of the 8-fold symmetry, P = nvirt (nvirt + 1) / 2;
+     *                    step 1  2 (M+ K+^2 + M- K-^2): the whole symmetric S+- matrices applied once
+     *                    (M+- = nocc (nocc +- 1) / 2 rows, K+- = nvirt (nvirt +- 1) / 2 packed pairs)
+     *   PPL_SYM_PAIR_SA: step 0  2 nchol nvirt^2 P (W rows a <= b only);  step 1  2 (M+ K+ + M- K-) P
+     *   PPL_SYM_PAIR:    (2 nchol + 2 nocc^2) nvirt^2 P;   PPL_SYM_NONE: the nominal count. */
+    double flops_useful, flops_useful_step0, flops_useful_step1;
 } ppl_info_t;
 
 /* Per-stage device times of the most recent profiled apply (ppl_apply_profiled), milliseconds. */
@@ -249,6 +259,17 @@ int ppl_check_inputs(ppl_plan_t *plan, const double *L, const double *t2, void *
  * with a register-only kernel: the roofline denominator used by bench.py.  Writes TFLOP/s
  * (best of `reps` launches of about `ms_target` milliseconds each).  Synchronises. */
 int ppl_probe_fp64_peak(double *tflops, int reps, double ms_target);
+
+/* The same measurement for the instruction streams the pipe choice was made between (north_star: "FP64 DMMA or the
+ * FP64 FMA pipe, whichever ncu shows faster"; evidence in profiles/r02_fp64_peaks.md).  All are register-only loops of
+ * 16 warps per SM on every SM; flops counted: 512 per DMMA m8n8k4, 2 per lane per DFMA. */
+enum {
+    PPL_PROBE_DMMA8 = 0,  /* 8 independent DMMA accumulator chains per warp (ppl_probe_fp64_peak) */
+    PPL_PROBE_DMMA16 = 1, /* 16 chains per warp: shows that the 8-chain figure is not dependency-limited */
+    PPL_PROBE_DFMA16 = 2, /* plain DFMA, 16 independent chains per thread */
+    PPL_PROBE_MIX8 = 3    /* one DFMA per lane interleaved with every DMMA (8 + 8 chains) */
+};
+int ppl_probe_fp64_pipe(int kind, double *tflops, int reps, double ms_target);
 
 /* Test hook: C(8x8) = A(8x4, row-major) * B(4x8, row-major) through ONE mma.sync.m8n8k4.f64 using
  * the fragment layout the kernels assume (lane = 4g+q: a=A[g][q], b=B[q][g], c={C[g][2q],

@@ -32,5 +32,6 @@ from .binding import (  # noqa: F401
     ppl_plan,
     ppl_plan_dry,
     ppl_probe_fp64_peak,
+    ppl_probe_fp64_pipe,
 )
 from ._build import build  # noqa: F401

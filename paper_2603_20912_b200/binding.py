@@ -43,6 +43,7 @@ class ppl_info_t(ctypes.Structure):
         ("sa_k_plus", c_int32), ("sa_k_minus", c_int32),
         ("full_available", c_int32), ("full_tbg", c_int32), ("full_slabs", c_int32), ("full_tight", c_int32),
         ("full_workspace_bytes", c_uint64),
+        ("flops_useful", c_double), ("flops_useful_step0", c_double), ("flops_useful_step1", c_double),
     ]
 
     def asdict(self):
@@ -88,6 +89,7 @@ SYMBOLS = {
     "ppl_plan_dry": (c_int, [c_int, c_int, c_int, c_size_t, c_size_t, c_int, c_int, POINTER(ppl_info_t)]),
     "ppl_check_inputs": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, POINTER(c_int)]),
     "ppl_probe_fp64_peak": (c_int, [POINTER(c_double), c_int, c_double]),
+    "ppl_probe_fp64_pipe": (c_int, [c_int, POINTER(c_double), c_int, c_double]),
     "ppl_debug_dmma_layout": (c_int, [c_void_p, c_void_p, c_void_p]),
 }
 
@@ -287,6 +289,16 @@ def ppl_destroy(plan: Plan):
 def ppl_probe_fp64_peak(reps: int = 3, ms_target: float = 20.0) -> float:
     out = c_double(0.0)
     _check(lib().ppl_probe_fp64_peak(ctypes.byref(out), int(reps), float(ms_target)), "ppl_probe_fp64_peak")
+    return float(out.value)
+
+
+PROBE_KINDS = {"dmma8": 0, "dmma16": 1, "dfma16": 2, "mix8": 3}
+
+
+def ppl_probe_fp64_pipe(kind: str, reps: int = 3, ms_target: float = 20.0) -> float:
+    """TFLOP/s of a register-only instruction stream: 'dmma8' (the peak probe), 'dmma16', 'dfma16', 'mix8'."""
+    out = c_double(0.0)
+    _check(lib().ppl_probe_fp64_pipe(PROBE_KINDS[kind], ctypes.byref(out), int(reps), float(ms_target)), "ppl_probe_fp64_pipe")
     return float(out.value)
 
 

@@ -1610,6 +1610,28 @@ int ppl_plan_info(const ppl_plan_t *p, ppl_info_t *out) {
     out->sa_rows_minus = p->Mm;
     out->sa_k_plus = p->KpT;
     out->sa_k_minus = p->KmT;
+    {   // useful flops of the mode (include/ppl.h): exact pair counts, no padding, no zero rows, no overshoot
+        const double v = p->v, P2 = v * (v + 1) / 2, Q2 = v * (v - 1) / 2, M = (double)p->o * p->o;
+        const double Mp = p->Mp, Mm = p->Mm;
+        switch (p->sym) {
+            case PPL_SYM_FULL:
+                out->flops_useful_step0 = 2.0 * p->x * P2 * (P2 + 1) / 2;
+                out->flops_useful_step1 = 2.0 * (Mp * P2 * P2 + Mm * Q2 * Q2);
+                break;
+            case PPL_SYM_PAIR_SA:
+                out->flops_useful_step0 = 2.0 * p->x * v * v * P2;
+                out->flops_useful_step1 = 2.0 * (Mp * P2 + Mm * Q2) * P2;
+                break;
+            case PPL_SYM_PAIR:
+                out->flops_useful_step0 = 2.0 * p->x * v * v * P2;
+                out->flops_useful_step1 = 2.0 * M * v * v * P2;
+                break;
+            default:
+                out->flops_useful_step0 = 2.0 * p->x * v4;
+                out->flops_useful_step1 = 2.0 * M * v4;
+        }
+        out->flops_useful = out->flops_useful_step0 + out->flops_useful_step1;
+    }
     out->full_available = p->full_ok;
     out->full_tbg = p->tbg;
     out->full_slabs = (int)p->slabs.size();
@@ -1982,8 +2004,8 @@ int ppl_destroy(ppl_plan_t *p) {
     return PPL_OK;
 }
 
-int ppl_probe_fp64_peak(double *tflops, int reps, double ms_target) {
-    if (!tflops || reps < 1) return fail(PPL_ERR_INVALID_ARG);
+int ppl_probe_fp64_pipe(int kind, double *tflops, int reps, double ms_target) {
+    if (!tflops || reps < 1 || kind < PPL_PROBE_DMMA8 || kind > PPL_PROBE_MIX8) return fail(PPL_ERR_INVALID_ARG);
     int dev = 0;
     cudaDeviceProp prop;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess || prop.major != 10) {
@@ -1995,14 +2017,26 @@ int ppl_probe_fp64_peak(double *tflops, int reps, double ms_target) {
     cudaEvent_t e0, e1;
     PPL_CUDA(cudaEventCreate(&e0));
     PPL_CUDA(cudaEventCreate(&e1));
-    const int sms = prop.multiProcessorCount, threads = 512;
-    // 8 DMMA per iteration per warp, 512 flop each
-    const double flop_per_iter = 512.0 * 8 * (threads / 32) * sms;
-    int iters = (int)std::max(1024.0, ms_target * 1e-3 * PEAK_FLOPS / flop_per_iter);
+    const int sms = prop.multiProcessorCount, threads = 512, warps = threads / 32;
+    // flops per loop iteration of one warp: a DMMA m8n8k4 is 8*8*4*2 = 512, a DFMA 2 per lane
+    double per_warp = 0;
+    switch (kind) {
+        case PPL_PROBE_DMMA8: per_warp = 8 * 512.0; break;
+        case PPL_PROBE_DMMA16: per_warp = 16 * 512.0; break;
+        case PPL_PROBE_DFMA16: per_warp = 16 * 64.0; break;
+        case PPL_PROBE_MIX8: per_warp = 8 * (512.0 + 64.0); break;
+    }
+    const double flop_per_iter = per_warp * warps * sms;
+    const int iters = (int)std::max(1024.0, ms_target * 1e-3 * PEAK_FLOPS / flop_per_iter);
     double best = 0;
     for (int r = 0; r < reps + 1; ++r) {
         cudaEventRecord(e0, 0);
-        ppl::k_probe_dmma<<<sms, threads>>>(out, iters, 1.0000001, 1e-9);
+        switch (kind) {
+            case PPL_PROBE_DMMA8: ppl::k_probe_dmma<<<sms, threads>>>(out, iters, 1.0000001, 1e-9); break;
+            case PPL_PROBE_DMMA16: ppl::k_probe_dmma_n<16><<<sms, threads>>>(out, iters, 1.0000001, 1e-9); break;
+            case PPL_PROBE_DFMA16: ppl::k_probe_dfma<16><<<sms, threads>>>(out, iters, 1.0000001, 1e-9); break;
+            case PPL_PROBE_MIX8: ppl::k_probe_mix<8><<<sms, threads>>>(out, iters, 1.0000001, 1e-9); break;
+        }
         cudaEventRecord(e1, 0);
         if (cudaEventSynchronize(e1) != cudaSuccess) {
             (void)cudaGetLastError();
@@ -2018,6 +2052,10 @@ int ppl_probe_fp64_peak(double *tflops, int reps, double ms_target) {
     cudaFree(out);
     *tflops = best;
     return PPL_OK;
+}
+
+int ppl_probe_fp64_peak(double *tflops, int reps, double ms_target) {
+    return ppl_probe_fp64_pipe(PPL_PROBE_DMMA8, tflops, reps, ms_target);
 }
 
 // test hook: C(8x8) = A(8x4) B(4x8) through one DMMA with the fragment layout the kernels assume

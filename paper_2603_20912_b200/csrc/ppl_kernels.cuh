@@ -607,6 +607,65 @@ __global__ void __launch_bounds__(512, 1) k_probe_dmma(double *out, int iters, d
     if (s == 123.456) out[0] = s;  // never true; keeps the loop alive
 }
 
+// Variants of the probe that back the pipe choice (north_star: "DMMA or the FP64 FMA pipe, whichever is faster";
+// DESIGN.md section 6, profiles/r02_fp64_peaks.md).  ACC independent accumulator chains per warp (DMMA) or per
+// thread (DFMA); MIX interleaves one DFMA chain step per DMMA.  flops per iteration and warp:
+//   DMMA: ACC * 512;  DFMA: ACC * 2 * 32;  MIX: ACC * (512 + 64).
+template <int ACC>
+__global__ void __launch_bounds__(512, 1) k_probe_dmma_n(double *out, int iters, double a, double b) {
+    double d0[ACC], d1[ACC];
+#pragma unroll
+    for (int i = 0; i < ACC; ++i) {
+        d0[i] = threadIdx.x * 1e-3 + i;
+        d1[i] = i;
+    }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < ACC; ++i) dmma(d0[i], d1[i], a, b);
+    }
+    double s = 0;
+#pragma unroll
+    for (int i = 0; i < ACC; ++i) s += d0[i] + d1[i];
+    if (s == 123.456) out[0] = s;
+}
+
+template <int ACC>
+__global__ void __launch_bounds__(512, 1) k_probe_dfma(double *out, int iters, double a, double b) {
+    double f[ACC];
+#pragma unroll
+    for (int i = 0; i < ACC; ++i) f[i] = threadIdx.x * 1e-3 + i;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < ACC; ++i) f[i] = fma(f[i], a, b);
+    }
+    double s = 0;
+#pragma unroll
+    for (int i = 0; i < ACC; ++i) s += f[i];
+    if (s == 123.456) out[0] = s;
+}
+
+template <int ACC>
+__global__ void __launch_bounds__(512, 1) k_probe_mix(double *out, int iters, double a, double b) {
+    double d0[ACC], d1[ACC], f[ACC];
+#pragma unroll
+    for (int i = 0; i < ACC; ++i) {
+        d0[i] = threadIdx.x * 1e-3 + i;
+        d1[i] = i;
+        f[i] = 0.5 * i;
+    }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < ACC; ++i) {
+            dmma(d0[i], d1[i], a, b);
+            f[i] = fma(f[i], a, b);
+        }
+    }
+    double s = 0;
+#pragma unroll
+    for (int i = 0; i < ACC; ++i) s += d0[i] + d1[i] + f[i];
+    if (s == 123.456) out[0] = s;
+}
+
 // C(8x8) = A(8x4, row-major) * B(4x8, row-major) with one warp, using the layout stated above
 __global__ void k_dmma_layout(const double *A, const double *B, double *C) {
     const int lane = threadIdx.x, g = lane >> 2, q = lane & 3;
