@@ -49,6 +49,9 @@ def _load():
         lib.ppl_oracle_full_ex.restype = i
         lib.ppl_oracle_eri_slab.argtypes = [i, i, _dp, i, i, _dp]
         lib.ppl_oracle_eri_slab.restype = i
+        lib.ppl_oracle_contract_pair.argtypes = [ctypes.c_char_p, ctypes.POINTER(i64), ctypes.POINTER(i64), _dp, _dp, _dp,
+                                                 ctypes.c_double, ctypes.c_double]
+        lib.ppl_oracle_contract_pair.restype = i
         _lib = lib
     return _lib
 
@@ -151,3 +154,24 @@ def eri_slab(L, a0: int, na: int) -> np.ndarray:
     if rc:
         raise RuntimeError(f"oracle error {rc}")
     return out
+
+
+def contract_pair(subscripts: str, A: np.ndarray, B: np.ndarray, C: np.ndarray | None = None, alpha=1.0, beta=0.0) -> np.ndarray:
+    """C = beta*C + alpha * einsum(subscripts, A, B) from the definition ('op0,op1->out'); one loop
+    nest over every index letter, plain double accumulation.  C=None: a fresh output (beta is then 0)."""
+    ins, out = subscripts.replace(" ", "").split("->")
+    s0, s1 = ins.split(",")
+    assert A.dtype == np.float64 and B.dtype == np.float64 and A.flags.c_contiguous and B.flags.c_contiguous
+    assert A.ndim == len(s0) and B.ndim == len(s1)
+    ext = dict(zip(s0, A.shape))
+    ext.update(zip(s1, B.shape))
+    shape = tuple(ext[c] for c in out)
+    if C is None:
+        C, beta = np.zeros(shape), 0.0
+    _chk(C, shape)
+    d0 = (ctypes.c_int64 * max(A.ndim, 1))(*A.shape)
+    d1 = (ctypes.c_int64 * max(B.ndim, 1))(*B.shape)
+    rc = _load().ppl_oracle_contract_pair(subscripts.encode(), d0, d1, _p(A), _p(B), _p(C), float(alpha), float(beta))
+    if rc:
+        raise RuntimeError(f"oracle error {rc}: malformed contraction {subscripts!r}")
+    return C

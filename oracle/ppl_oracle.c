@@ -30,6 +30,10 @@
  * control, exact-integer inputs against int64 arithmetic, numpy einsum, projection identity.
  * ppl_oracle_eri_slab (step 0 alone) is pinned by a hand-worked example, numpy einsum, the nchol = 1 outer
  * product, the ERI symmetries and by reproducing ppl_oracle_full when contracted with t2.
+ * ppl_oracle_contract_pair (the generic two-operand contraction 'op0,op1->out' of PAPER.md:195-209) is the einsum
+ * definition written out -- one loop nest over every index letter -- pinned by a hand-worked 2x2x2 example
+ * (tests/golden/contract_pair_hand.txt), numpy einsum on the paper's strings and others, matmul / outer-product /
+ * trace-free special cases and exact integers.
  * Every entry point below is pinned; none is "parity unpinned".
  */
 #include <stdint.h>
@@ -312,6 +316,90 @@ int ppl_oracle_eri_slab(int nvirt, int nchol, const double *L, int a0, int na, d
             for (int64_t c = 0; c < v; ++c)
                 for (int64_t d = 0; d < v; ++d)
                     Wab[c * v + d] += L[(P * v + a) * v + c] * L[(P * v + b) * v + d];
+    }
+    return 0;
+}
+
+
+/* ---------------------------------------------------------------------------------------------
+ * Generic pair contraction  'op0,op1->out'  ("any tensor contraction ... translated into a sequence
+ * of two-array contractions ... op0,op1->out"; the ladder's own two steps are 'xac,xbd->acbd' and 'abcd,ecfd->efab',
+ * PAPER.md:118-120).  The einsum definition, nothing else:
+ *
+ *     C[out indices] = beta * C[out indices] + alpha * sum_{indices not in out} A[op0 indices] * B[op1 indices]
+ *
+ * subs: "op0,op1->out", one ASCII letter per axis, no repeated letter inside one operand, every out letter must occur
+ * in op0 or op1.  dims0 / dims1: extents of the axes of A / B in the order of op0 / op1 (a letter shared by both must
+ * have the same extent).  All arrays dense row-major in the order of their subscripts.  beta == 0 overwrites (C is
+ * not read).  One loop nest over the out letters (odometer, row-major), inside it one over the summed letters
+ * (odometer in order of first appearance), plain double accumulation.  Returns 0, or 1 on a malformed request.
+ * --------------------------------------------------------------------------------------------- */
+int ppl_oracle_contract_pair(const char *subs, const int64_t *dims0, const int64_t *dims1, const double *A, const double *B,
+                             double *C, double alpha, double beta) {
+    char op[3][16];
+    int n[3] = {0, 0, 0};
+    int which = 0;
+    for (const char *q = subs; *q; ++q) {
+        if (*q == ',') {
+            if (which != 0) return 1;
+            which = 1;
+        } else if (*q == '-' && q[1] == '>') {
+            if (which != 1) return 1;
+            which = 2;
+            ++q;
+        } else if ((*q >= 'a' && *q <= 'z') || (*q >= 'A' && *q <= 'Z')) {
+            if (n[which] >= 15) return 1;
+            for (int k = 0; k < n[which]; ++k)
+                if (op[which][k] == *q) return 1; /* repeated letter inside one operand */
+            op[which][n[which]++] = *q;
+        } else if (*q != ' ') {
+            return 1;
+        }
+    }
+    if (which != 2) return 1;
+    int64_t ext[128];
+    for (int k = 0; k < 128; ++k) ext[k] = -1;
+    for (int k = 0; k < n[0]; ++k) ext[(int)op[0][k]] = dims0[k];
+    for (int k = 0; k < n[1]; ++k) {
+        if (ext[(int)op[1][k]] >= 0 && ext[(int)op[1][k]] != dims1[k]) return 1;
+        ext[(int)op[1][k]] = dims1[k];
+    }
+    for (int k = 0; k < n[2]; ++k)
+        if (ext[(int)op[2][k]] < 0) return 1;
+    /* summed letters, in order of first appearance */
+    char sum[32];
+    int ns = 0;
+    for (int w = 0; w < 2; ++w)
+        for (int k = 0; k < n[w]; ++k) {
+            int seen = 0;
+            for (int j = 0; j < n[2]; ++j) seen |= op[2][j] == op[w][k];
+            for (int j = 0; j < ns; ++j) seen |= sum[j] == op[w][k];
+            if (!seen) sum[ns++] = op[w][k];
+        }
+    int64_t val[128]; /* current value of every letter */
+    for (int k = 0; k < 128; ++k) val[k] = 0;
+    int64_t nout = 1, nsum = 1;
+    for (int k = 0; k < n[2]; ++k) nout *= ext[(int)op[2][k]];
+    for (int k = 0; k < ns; ++k) nsum *= ext[(int)sum[k]];
+    for (int64_t io = 0; io < nout; ++io) {
+        int64_t r = io; /* row-major odometer of the out letters */
+        for (int k = n[2] - 1; k >= 0; --k) {
+            val[(int)op[2][k]] = r % ext[(int)op[2][k]];
+            r /= ext[(int)op[2][k]];
+        }
+        double acc = 0.0;
+        for (int64_t is = 0; is < nsum; ++is) {
+            int64_t q = is;
+            for (int k = ns - 1; k >= 0; --k) {
+                val[(int)sum[k]] = q % ext[(int)sum[k]];
+                q /= ext[(int)sum[k]];
+            }
+            int64_t ia = 0, ib = 0;
+            for (int k = 0; k < n[0]; ++k) ia = ia * dims0[k] + val[(int)op[0][k]];
+            for (int k = 0; k < n[1]; ++k) ib = ib * dims1[k] + val[(int)op[1][k]];
+            acc += A[ia] * B[ib];
+        }
+        C[io] = (beta == 0.0) ? alpha * acc : beta * C[io] + alpha * acc;
     }
     return 0;
 }
