@@ -159,6 +159,31 @@ typedef struct ppl_times_s {
  * Uses the current CUDA device.  Returns NULL on failure (see ppl_last_error). */
 ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes);
 
+/* Debug / experiment knobs of the planner and the orchestration, for tests and A/B measurements (they replace the
+ * environment variables of round 1; the library reads no environment variable except PPL_TRACE).  All zero = the
+ * product's defaults; ppl_plan(...) == ppl_plan_ex(..., NULL).  The struct is copied into the plan. */
+typedef struct ppl_debug_opts_s {
+    int32_t tile_edge;        /* un-packed modes: force the W-tile edge T (0 = the planner's choice) */
+    int32_t ni_max;           /* largest row-tile instance of step 1, 1..10 (0 = 10) */
+    int32_t cpasync_kernels;  /* 1 = the cp.async kernels instead of the TMA kernels */
+    int32_t full_min_v;       /* smallest nvirt at which PPL_SYM_FULL is the default (0 = 52) */
+    int32_t full_tbg;         /* PPL_SYM_FULL: largest W+- tile, in rows / 16 (0 = 256); a multiple of 16 */
+    int32_t full_slots;       /* PPL_SYM_FULL: 1 = a single W+- slot (0 = two when they fit) */
+    int32_t full_strips;      /* PPL_SYM_FULL: 1 = one strip, 2 = two whenever they fit (0 = the planner's choice) */
+    int32_t full_tight;       /* PPL_SYM_FULL: 1 = the memory-tight form even when the slab strip fits */
+    int32_t full_rect_tiles;  /* PPL_SYM_FULL: 1 = rectangular (slab; b-group) W+- tiles with their zero rows (the round-1 form;
+                                 always used by the memory-tight form) instead of runs of the packed pair index */
+    int32_t full_no_diag_pack;/* PPL_SYM_FULL: 1 = diagonal d-blocks of step 0 as 16 plain chunks instead of 9 packed ones */
+    int32_t full_serial;      /* PPL_SYM_FULL: 1 = every launch on the caller's stream */
+    int32_t debug_sync;       /* 1 = synchronise and report on stderr after every launch */
+    int32_t trace;            /* 1 = timeline of one apply on stderr (also: environment variable PPL_TRACE) */
+    int32_t host_chunk_mb;    /* ppl_apply_host: staging-buffer size in MiB (0 = 1024) */
+    int32_t reserved[18];     /* must be zero */
+} ppl_debug_opts_t;
+
+/* ppl_plan with debug options (NULL = defaults). */
+ppl_plan_t *ppl_plan_ex(int nocc, int nvirt, int nchol, size_t workspace_bytes, const ppl_debug_opts_t *dbg);
+
 /* ppl_apply: enqueue  R += ladder(L, t2)  on `stream` (a cudaStream_t passed as void*; NULL =
  * the legacy default stream).  Asynchronous: returns once the work is queued.  All effects are
  * ordered after prior work on `stream` and complete before later work on `stream` (an internal
@@ -193,6 +218,29 @@ int ppl_generate_eri(ppl_plan_t *plan, const double *L, int a0, int na, double *
  * used.  nchol of the plan is ignored.  Only R entries with a in the slab are touched. */
 int ppl_apply_dense(ppl_plan_t *plan, const double *eri, int a0, int na, const double *t2, double *R,
                     const ppl_opts_t *opts, void *stream);
+
+/* ppl_contract_pair: the generic pair contraction of the paper's generic recipe (pseudo-code 211-338;
+ * SURVEY.md 8(f) NEXT-3):
+ *     C[out] = beta * C[out] + alpha * sum_{summed letters} A[op0] * B[op1]
+ * subscripts: "op0,op1->out", one ASCII letter per axis (at most 12 per operand), no letter repeated inside an operand,
+ *   every letter in exactly TWO of op0, op1, out (a tensordot: surviving letters of op0, surviving letters of op1,
+ *   summed letters; `out` may order the surviving letters in any way).  Examples: the ladder's own steps
+ *   "xac,xbd->acbd" and "abcd,ecfd->efab", "xac,icjd->xajd", "ik,kj->ij".
+ * dims0 / dims1: extents of the axes of A / B in the order of op0 / op1 (a shared letter must agree).
+ * A, B, C: DEVICE pointers, dense row-major FP64 in the order of their subscripts, 8-byte aligned (16-byte aligned
+ *   operands with even extents along their unit-stride letter take the 16-byte copy path).  C must not alias A or B.
+ *   beta == 0 overwrites: C is not read.
+ * workspace: DEVICE memory, 256-byte aligned, at least the bytes ppl_contract_pair_workspace reports (offset tables of
+ *   8 (2 M + 2 N + 2 K) bytes plus room for split-K partials; with less than the report -- but at least the tables --
+ *   the call lowers its split-K factor instead of failing).  Borrowed until the queued work completes.
+ * Where the paper batches along the surviving axes to fit VRAM and calls tensordot (permuted copies + DGEMM) per batch,
+ * this is one in-place GEMM over offset tables on the FP64 tensor pipe; the summed axes (the Cholesky index among them)
+ * are split only inside the kernel, with a fixed-order reduction: results are bit-reproducible.  No symmetry is assumed.
+ * Asynchronous on `stream`.  Needs no plan.  PPL_ERR_INVALID_ARG for a malformed request,
+ * PPL_ERR_WORKSPACE_TOO_SMALL if the workspace cannot hold the tables, PPL_ERR_UNSUPPORTED_DEVICE off cc 10.x. */
+int ppl_contract_pair_workspace(const char *subscripts, const int64_t *dims0, const int64_t *dims1, size_t *bytes);
+int ppl_contract_pair(const char *subscripts, const int64_t *dims0, const int64_t *dims1, const double *A, const double *B,
+                      double *C, double alpha, double beta, void *workspace, size_t workspace_bytes, void *stream);
 
 /* ppl_apply_host: the same operation on HOST buffers (pageable or pinned), the paper's own setting (operands in
  * host memory).  Synchronises before returning.  Device buffers are
@@ -248,6 +296,8 @@ int ppl_plan_info(const ppl_plan_t *plan, ppl_info_t *out);
  * default ppl_plan would choose.  Errors as ppl_plan / ppl_plan_set_symmetry (PPL_ERR_WORKSPACE_TOO_SMALL ...). */
 int ppl_plan_dry(int nocc, int nvirt, int nchol, size_t workspace_bytes, size_t device_free_bytes, int num_sms, int mode,
                  ppl_info_t *out);
+int ppl_plan_dry_ex(int nocc, int nvirt, int nchol, size_t workspace_bytes, size_t device_free_bytes, int num_sms, int mode,
+                    const ppl_debug_opts_t *dbg, ppl_info_t *out);
 
 /* Debug: verify on the device that L[P,a,c]==L[P,c,a] (required in PPL_SYM_FULL, else only reported)
  * and, in every mode but PPL_SYM_NONE, that t2[i,j,c,d]==t2[j,i,d,c] (required).  Synchronises `stream`.

@@ -26,6 +26,7 @@ from .binding import (  # noqa: F401
     lib,
     library_path,
     ppl_apply,
+    ppl_contract_pair,
     ppl_debug_dmma_layout,
     ppl_destroy,
     ppl_last_error,

@@ -65,6 +65,25 @@ class ppl_opts_t(ctypes.Structure):
     _fields_ = [("t2_layout", c_int32), ("r_layout", c_int32), ("alpha", c_double), ("beta", c_double)]
 
 
+class ppl_debug_opts_t(ctypes.Structure):
+    """include/ppl.h ppl_debug_opts_t: planner / orchestration knobs for tests and A/B runs; all zero = the defaults."""
+    _fields_ = [(k, c_int32) for k in (
+        "tile_edge", "ni_max", "cpasync_kernels", "full_min_v", "full_tbg", "full_slots", "full_strips", "full_tight",
+        "full_rect_tiles", "full_no_diag_pack", "full_serial", "debug_sync", "trace", "host_chunk_mb")] + [("reserved", c_int32 * 18)]
+
+
+def _debug_opts(debug):
+    if not debug:
+        return None
+    d = ppl_debug_opts_t()
+    names = {k for k, _ in ppl_debug_opts_t._fields_} - {"reserved"}
+    for k, val in debug.items():
+        if k not in names:
+            raise KeyError(f"unknown debug option {k!r}; known: {sorted(names)}")
+        setattr(d, k, int(val))
+    return ctypes.byref(d)
+
+
 class PplError(RuntimeError):
     def __init__(self, code: int, where: str):
         self.code = code
@@ -74,10 +93,14 @@ class PplError(RuntimeError):
 # Every symbol include/ppl.h declares: (restype, argtypes)
 SYMBOLS = {
     "ppl_plan": (c_void_p, [c_int, c_int, c_int, c_size_t]),
+    "ppl_plan_ex": (c_void_p, [c_int, c_int, c_int, c_size_t, POINTER(ppl_debug_opts_t)]),
     "ppl_apply": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
     "ppl_apply_ex": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, POINTER(ppl_opts_t), c_void_p]),
     "ppl_apply_dense": (c_int, [c_void_p, c_void_p, c_int, c_int, c_void_p, c_void_p, POINTER(ppl_opts_t), c_void_p]),
     "ppl_generate_eri": (c_int, [c_void_p, c_void_p, c_int, c_int, c_void_p, c_void_p]),
+    "ppl_contract_pair_workspace": (c_int, [c_char_p, POINTER(ctypes.c_int64), POINTER(ctypes.c_int64), POINTER(c_size_t)]),
+    "ppl_contract_pair": (c_int, [c_char_p, POINTER(ctypes.c_int64), POINTER(ctypes.c_int64), c_void_p, c_void_p, c_void_p,
+                                  c_double, c_double, c_void_p, c_size_t, c_void_p]),
     "ppl_apply_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, POINTER(c_uint64), POINTER(c_uint64)]),
     "ppl_apply_profiled": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, POINTER(ppl_times_t)]),
     "ppl_destroy": (c_int, [c_void_p]),
@@ -87,6 +110,7 @@ SYMBOLS = {
     "ppl_plan_set_graph": (c_int, [c_void_p, c_int]),
     "ppl_plan_info": (c_int, [c_void_p, POINTER(ppl_info_t)]),
     "ppl_plan_dry": (c_int, [c_int, c_int, c_int, c_size_t, c_size_t, c_int, c_int, POINTER(ppl_info_t)]),
+    "ppl_plan_dry_ex": (c_int, [c_int, c_int, c_int, c_size_t, c_size_t, c_int, c_int, POINTER(ppl_debug_opts_t), POINTER(ppl_info_t)]),
     "ppl_check_inputs": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, POINTER(c_int)]),
     "ppl_probe_fp64_peak": (c_int, [POINTER(c_double), c_int, c_double]),
     "ppl_probe_fp64_pipe": (c_int, [c_int, POINTER(c_double), c_int, c_double]),
@@ -148,8 +172,12 @@ def _stream_ptr(stream):
 class Plan:
     """Owner of an opaque ppl_plan_t* (workspace, internal stream, events)."""
 
-    def __init__(self, nocc: int, nvirt: int, nchol: int, workspace_bytes: int = 0):
-        h = lib().ppl_plan(int(nocc), int(nvirt), int(nchol), int(workspace_bytes))
+    def __init__(self, nocc: int, nvirt: int, nchol: int, workspace_bytes: int = 0, debug: dict | None = None):
+        """debug: ppl_debug_opts_t fields by name (tests / A-B runs only); None = ppl_plan."""
+        if debug:
+            h = lib().ppl_plan_ex(int(nocc), int(nvirt), int(nchol), int(workspace_bytes), _debug_opts(debug))
+        else:
+            h = lib().ppl_plan(int(nocc), int(nvirt), int(nchol), int(workspace_bytes))
         if not h:
             raise PplError(ppl_last_error(), "ppl_plan")
         self._h = c_void_p(h)
@@ -270,11 +298,11 @@ def ppl_plan(nocc: int, nvirt: int, nchol: int, workspace_bytes: int = 0) -> Pla
 
 
 def ppl_plan_dry(nocc: int, nvirt: int, nchol: int, workspace_bytes: int = 0, device_free_bytes: int = 170 << 30,
-                 num_sms: int = 148, mode: int = -1) -> dict:
+                 num_sms: int = 148, mode: int = -1, debug: dict | None = None) -> dict:
     """The planner alone, for a stated device: no GPU needed.  Returns what Plan.info() would."""
     out = ppl_info_t()
-    _check(lib().ppl_plan_dry(int(nocc), int(nvirt), int(nchol), int(workspace_bytes), int(device_free_bytes), int(num_sms),
-                              int(mode), ctypes.byref(out)), "ppl_plan_dry")
+    _check(lib().ppl_plan_dry_ex(int(nocc), int(nvirt), int(nchol), int(workspace_bytes), int(device_free_bytes), int(num_sms),
+                                 int(mode), _debug_opts(debug), ctypes.byref(out)), "ppl_plan_dry")
     return out.asdict()
 
 
@@ -290,6 +318,35 @@ def ppl_probe_fp64_peak(reps: int = 3, ms_target: float = 20.0) -> float:
     out = c_double(0.0)
     _check(lib().ppl_probe_fp64_peak(ctypes.byref(out), int(reps), float(ms_target)), "ppl_probe_fp64_peak")
     return float(out.value)
+
+
+def ppl_contract_pair(subscripts: str, A, B, C=None, alpha: float = 1.0, beta: float = 0.0, stream=None, workspace=None):
+    """C = beta*C + alpha*einsum(subscripts, A, B) for a two-operand contraction of tensordot type (include/ppl.h).
+    A, B, C: contiguous CUDA float64 tensors; C=None allocates the output (beta is then 0).  The workspace (a torch
+    uint8 CUDA tensor) is allocated per call unless one is passed in; it must outlive the queued work."""
+    import torch
+
+    ins, out = subscripts.replace(" ", "").split("->")
+    s0, s1 = ins.split(",")
+    d0 = (ctypes.c_int64 * max(A.dim(), 1))(*A.shape)
+    d1 = (ctypes.c_int64 * max(B.dim(), 1))(*B.shape)
+    ext = dict(zip(s0, A.shape))
+    ext.update(zip(s1, B.shape))
+    shape = tuple(ext[c] for c in out)
+    if C is None:
+        C, beta = torch.empty(shape, dtype=torch.float64, device=A.device), 0.0
+    need = c_size_t(0)
+    _check(lib().ppl_contract_pair_workspace(subscripts.encode(), d0, d1, ctypes.byref(need)), "ppl_contract_pair_workspace")
+    if workspace is None:
+        workspace = torch.empty(int(need.value) + 256, dtype=torch.uint8, device=A.device)
+    base = workspace.data_ptr()
+    aligned = (base + 255) // 256 * 256
+    _check(lib().ppl_contract_pair(subscripts.encode(), d0, d1, _dev_ptr(A, "A"), _dev_ptr(B, "B"), _dev_ptr(C, "C", shape),
+                                   float(alpha), float(beta), c_void_p(aligned), workspace.numel() - (aligned - base),
+                                   _stream_ptr(stream)), "ppl_contract_pair")
+    if hasattr(workspace, "record_stream"):
+        workspace.record_stream(stream if stream is not None else torch.cuda.current_stream())
+    return C
 
 
 PROBE_KINDS = {"dmma8": 0, "dmma16": 1, "dfma16": 2, "mix8": 3}

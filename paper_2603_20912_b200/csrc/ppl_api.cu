@@ -23,6 +23,9 @@ int fail(int code) {
     g_last_error = code;
     return code;
 }
+}  // namespace
+int ppl_fail_code(int code) { return fail(code); }  // for the other translation units of the library (ppl_contract.cu)
+namespace {
 #define PPL_CUDA(expr)                                 \
     do {                                               \
         cudaError_t e__ = (expr);                      \
@@ -63,6 +66,12 @@ struct FullTile {
     // memory-tight mode: step 0 runs per tile on the full (b in group, d >= A0) rectangle into a strip of the tile's rows
     size_t chunk_off = 0;
     int tiles_n = 0;
+    // range tiles (the default outside the memory-tight form): the W+- rows are a run of the packed pair index of (a <= b),
+    // a in the slab -- no zero rows for a > b and no rounding of the b count, only the holes of the packed layout
+    int range = 0;
+    int kp0 = 0, np = 0, npr = 0;  // plus: first packed index, rows, rows rounded up to 16 (the k-tiles of use 2)
+    int km0 = 0, nm = 0, nmr = 0;  // minus rows of the same pairs
+    int nzm = 0, zrows_m[24] = {};  // minus rows no pair writes (holes, tail): zeroed by the fold
 };
 struct FullSlab {
     int A0, ta;
@@ -137,6 +146,12 @@ struct ppl_plan_s {
     double *fpart = nullptr;
     double *raccp = nullptr, *raccm = nullptr; // R+- accumulators [Mp][ldp], [Mm][ldm]
     int2 *fchunks = nullptr;
+    double *Lq = nullptr;                      // packed diagonal 16 x 16 blocks of L: [x][ldq] (ppl_kernels_full.cuh, k_pack_diag)
+    int nfull = 0;                             // full 16-blocks of the (padded) virtual index
+    int64_t ldq = 0;
+    int diag_pack = 0;
+    CUtensorMap mapLq;
+    ppl_debug_opts_t dbg = {};
     size_t fpart_bytes = 0;
     size_t fpart_m_off = 0;                    // doubles: the minus partials start here (fixed: + and - run on different streams)
     std::vector<FullSlab> slabs;
@@ -771,6 +786,14 @@ int run_apply(ppl_plan_s *p, const double *L, const double *t2, double *R, const
 // ------------------------------------------------------------------------------------------
 // PPL_SYM_FULL (ppl_kernels_full.cuh): slabs of 16 a's, tiles (A; b-group), chunk table of step 0.
 // ------------------------------------------------------------------------------------------
+// flops of one step-1 launch as the CTA tiles execute it: rows in 8-row blocks (MSplit), columns in tiles of 128, k in tiles of 16
+double gemm_flops_launched(const MGeom &mg, int M, int64_t ncols, int64_t krange) {
+    if (M <= 0 || ncols <= 0 || krange <= 0) return 0;
+    const double rows = 8.0 * ((M + 7) / 8);
+    (void)mg;
+    return 2.0 * rows * (128.0 * ((ncols + 127) / 128)) * (16.0 * ((krange + 15) / 16));
+}
+
 int full_geometry(ppl_plan_s *p, int tbg, size_t part_cap, std::vector<int2> *chunks_out, bool tight = false) {
     const int v = p->vp, TA = ppl::TA_FULL;
     p->slabs.clear();
@@ -779,6 +802,12 @@ int full_geometry(ppl_plan_s *p, int tbg, size_t part_cap, std::vector<int2> *ch
     p->fpart_bytes = 0;
     size_t part_p = 0, part_m = 0;
     std::vector<int2> chunks;
+    const bool range_tiles = !tight && !p->dbg.full_rect_tiles;
+    const bool diag_pack = !tight && !p->dbg.full_no_diag_pack && v >= 16;
+    p->diag_pack = diag_pack ? 1 : 0;
+    p->nfull = v / 16;
+    p->ldq = (int64_t)std::max(p->nfull, 1) * ppl::DIAG_PACKED;
+    std::vector<unsigned char> mark;
     for (int A0 = 0; A0 < v; A0 += TA) {
         FullSlab sl;
         sl.A0 = A0;
@@ -788,55 +817,137 @@ int full_geometry(ppl_plan_s *p, int tbg, size_t part_cap, std::vector<int2> *ch
         // d-block major: the 8 chunks of a CTA tile are 8 consecutive b's of one d-block, so that the b<->d image
         // X[a,d,c,b] is written as runs of 8 b's (two full 32-byte sectors, merged in L2) instead of lone doubles
         if (!tight) {
-            for (int d0 = A0; d0 < v; d0 += 16)
-                for (int b = A0; b < std::min(d0 + 16, v); ++b) chunks.push_back(make_int2(b, d0));
+            // A ragged last d-block [dL, v) of width w < 16 would cost a whole 16-wide chunk for every b >= A0.  It is
+            // covered from the other side instead: the w b's of that block against every d-block from A0 up (chunks with
+            // d-block BELOW the b-block; the epilogue stores their b<->d image like that of any off-diagonal chunk), which
+            // is w * ceil(r / 16) chunks instead of r (nvirt = 200, 600: w = 8, half as many).
+            const int dL = A0 + (v - 1 - A0) / 16 * 16, w = v - dL;
+            const bool reverse = w < 16 && (int64_t)w * ((v - A0 + 15) / 16) < (v - A0);
+            // Diagonal blocks (b-block == d-block, full 16 x 16): only b <= d is needed -- 9 chunks of the packed copy Lq
+            // (k_pack_diag) instead of 16 plain ones.  They go behind the plain chunks so that those keep their
+            // (b even, b + 1) pairing inside the column tiles (16-byte image stores).
+            for (int d0 = A0; d0 < v; d0 += 16) {
+                if (reverse && d0 == dL) break;
+                const bool packed = diag_pack && d0 + 16 <= v;
+                for (int b = A0; b < (packed ? d0 : std::min(d0 + 16, v)); ++b) chunks.push_back(make_int2(b, d0));
+            }
+            if (reverse)
+                for (int d0 = A0; d0 <= dL; d0 += 16)
+                    for (int b = dL; b < v; ++b) chunks.push_back(make_int2(b, d0));
+            if (diag_pack)
+                for (int d0 = A0; d0 + 16 <= v; d0 += 16)
+                    for (int j = 0; j < ppl::DIAG_PACKED / 16; ++j)
+                        chunks.push_back(make_int2(-2 - d0 / 16, d0 / 16 * ppl::DIAG_PACKED + 16 * j));
             while ((chunks.size() - sl.chunk_off) % 8) chunks.push_back(make_int2(-1, 0));
         }
         sl.tiles_n = (int)((chunks.size() - sl.chunk_off) / 8);
         sl.flops0 = 2.0 * p->x * (128.0 * sl.tiles_m) * (128.0 * sl.tiles_n);
         p->ff_step0 += sl.flops0;
         sl.tile_begin = (int)p->ftiles.size();
-        // b-groups: the 16-blocks of [A0, v) dealt into groups of at most tbg/16 blocks, as evenly as possible
-        const int nblk = (v - A0 + 15) / 16, per = tbg / 16, ng = (nblk + per - 1) / per;
-        int blk = 0;
-        for (int gi = 0; gi < ng; ++gi) {
-            const int cnt = nblk / ng + (gi < nblk % ng ? 1 : 0);
-            FullTile t;
-            t.A0 = A0;
-            t.ta = sl.ta;
-            t.bg0 = A0 + 16 * blk;
-            t.nb = std::min(16 * cnt, v - t.bg0);
-            t.tbp = 16 * cnt;
-            blk += cnt;
-            const int c1 = std::min(A0 + TA, v);
-            // range starts are even (TMA alignment): (A0,A0) sits at an even index, and the element before
-            // (A0, A0+1) in the minus triangle is a hole (A0 even)
-            t.k0p = (int)ppl::kplus(A0, A0, v);
-            t.k0m = A0 + 1 < v ? (int)ppl::kminus(A0, A0 + 1, v) - 1 : p->Km;
-            t.k1p = c1 < v ? (int)ppl::kplus(c1, c1, v) : p->Kp;
-            t.k1m = c1 + 1 < v ? (int)ppl::kminus(c1, c1 + 1, v) - 1 : p->Km;
-            const int N = TA * t.tbp;
-            t.sp = choose_split(p->Mp, N, p->Kp - t.k0p, p->num_sms, p->mg_p, part_cap / 2);
-            t.sm = choose_split(p->Mm, N, p->Km - t.k0m, p->num_sms, p->mg_m, part_cap / 2);
-            part_p = std::max(part_p, (size_t)t.sp.splitk * p->Mp * N);
-            part_m = std::max(part_m, (size_t)t.sm.splitk * p->Mm * N);
+        const int c1 = std::min(A0 + TA, v);
+        // range starts are even (TMA alignment): (A0,A0) sits at an even index, and the element before
+        // (A0, A0+1) in the minus triangle is a hole (A0 even)
+        const int k0p = (int)ppl::kplus(A0, A0, v);
+        const int k0m = A0 + 1 < v ? (int)ppl::kminus(A0, A0 + 1, v) - 1 : p->Km;
+        const int k1p = c1 < v ? (int)ppl::kplus(c1, c1, v) : p->Kp;
+        const int k1m = c1 + 1 < v ? (int)ppl::kminus(c1, c1 + 1, v) - 1 : p->Km;
+        auto finish_tile = [&](FullTile &t, int Np, int Nm, int Kup, int Kum) {
+            // Np / Nm: W+- rows contracted by use 1 (its GEMM N); Kup / Kum: W+- rows contracted by use 2 (its GEMM K)
+            t.k0p = k0p;
+            t.k0m = k0m;
+            t.k1p = k1p;
+            t.k1m = k1m;
+            t.sp = choose_split(p->Mp, Np, p->Kp - t.k0p, p->num_sms, p->mg_p, part_cap / 2);
+            t.sm = choose_split(p->Mm, Nm, p->Km - t.k0m, p->num_sms, p->mg_m, part_cap / 2);
+            part_p = std::max(part_p, (size_t)t.sp.splitk * p->Mp * Np);
+            part_m = std::max(part_m, (size_t)t.sm.splitk * p->Mm * std::max(Nm, 0));
             p->fpart_m_off = (part_p + 31) / 32 * 32;
             p->fpart_bytes = (p->fpart_m_off + part_m) * 8;
-            // executed flops: use 1 (contraction over J >= (A0,A0)) + use 2 (outputs J >= (A0+16,A0+16))
-            const double r0 = v - A0, r1 = v - c1;  // pairs with c >= A0 / c >= A0+16
-            p->ff_step1 += 2.0 * N * ((double)p->Mp * r0 * (r0 + 1) / 2 + (double)p->Mm * r0 * (r0 - 1) / 2);
-            p->ff_step1 += 2.0 * N * ((double)p->Mp * r1 * (r1 + 1) / 2 + (double)p->Mm * std::max(0.0, r1 * (r1 - 1) / 2));
-            if (tight) {  // the full (b, d) rectangle of the group: no image, twice the step-0 flops, a strip of tbp rows per a
-                t.chunk_off = chunks.size();
-                for (int d0 = A0; d0 < v; d0 += 16)
-                    for (int b = t.bg0; b < t.bg0 + t.nb; ++b) chunks.push_back(make_int2(b, d0));
-                while ((chunks.size() - t.chunk_off) % 8) chunks.push_back(make_int2(-1, 0));
-                t.tiles_n = (int)((chunks.size() - t.chunk_off) / 8);
-                const double f0 = 2.0 * p->x * (128.0 * sl.tiles_m) * (128.0 * t.tiles_n);
-                sl.flops0 += f0;
-                p->ff_step0 += f0;
+            // executed flops, as the CTA tiles run them: use 1 (contraction over J >= (A0,A0)) + use 2 (outputs J >= (A0+16,A0+16))
+            p->ff_step1 += gemm_flops_launched(p->mg_p, p->Mp, Np, p->Kp - t.k0p) + gemm_flops_launched(p->mg_m, p->Mm, Nm, p->Km - t.k0m);
+            p->ff_step1 += gemm_flops_launched(p->mg_p, p->Mp, p->Kp - (t.k1p & ~15), Kup) +
+                           gemm_flops_launched(p->mg_m, p->Mm, p->Km - (t.k1m & ~15), Kum);
+        };
+        if (range_tiles) {
+            // the slab's pairs (a <= b), a in the slab, are ONE run of the packed index; it is cut into tiles of at most 16 tbg
+            // rows at multiples of 128 (the column tile of use 1)
+            const int64_t lo = k0p, hi = ppl::kplus(A0 + sl.ta - 1, v - 1, v) + 1, Ls = hi - lo, NT = (int64_t)TA * tbg;
+            const int ng = (int)((Ls + NT - 1) / NT);
+            int64_t chunk = ((Ls + ng - 1) / ng + 127) / 128 * 128;
+            if (chunk > NT) chunk = NT;
+            int64_t prev_last_m = -1;
+            for (int64_t kp0 = lo; kp0 < hi; kp0 += chunk) {
+                FullTile t;
+                t.A0 = A0;
+                t.ta = sl.ta;
+                t.bg0 = A0;
+                t.nb = v - A0;
+                t.tbp = 0;
+                t.range = 1;
+                t.kp0 = (int)kp0;
+                t.np = (int)(std::min(kp0 + chunk, hi) - kp0);
+                t.npr = (t.np + 15) / 16 * 16;
+                // the minus rows of the tile's pairs
+                int64_t first_m = -1, last_m = -1;
+                int a = A0;
+                for (int64_t kap = kp0; kap < kp0 + t.np; ++kap) {
+                    while (a + 1 < A0 + sl.ta && ppl::kplus(a + 1, a + 1, v) <= kap) ++a;
+                    const int b = a + (int)(kap - ppl::kplus(a, a, v));
+                    if (b >= v || b <= a) continue;  // hole / diagonal pair
+                    const int64_t km = ppl::kminus(a, b, v);
+                    if (first_m < 0) first_m = km;
+                    last_m = km;
+                }
+                if (first_m >= 0) {
+                    t.km0 = (int)(first_m & ~(int64_t)1);
+                    if ((int64_t)t.km0 <= prev_last_m) return PPL_ERR_INVALID_ARG;  // never: cuts fall on even indices (kplus / kminus parity = parity of b)
+                    t.nm = (int)(last_m + 1 - t.km0);
+                    t.nmr = (t.nm + 15) / 16 * 16;
+                    prev_last_m = last_m;
+                    mark.assign(t.nmr, 0);
+                    a = A0;
+                    for (int64_t kap = kp0; kap < kp0 + t.np; ++kap) {
+                        while (a + 1 < A0 + sl.ta && ppl::kplus(a + 1, a + 1, v) <= kap) ++a;
+                        const int b = a + (int)(kap - ppl::kplus(a, a, v));
+                        if (b >= v || b <= a) continue;
+                        mark[ppl::kminus(a, b, v) - t.km0] = 1;
+                    }
+                    for (int r = 0; r < t.nmr; ++r)
+                        if (!mark[r]) {
+                            if (t.nzm >= 24) return PPL_ERR_INVALID_ARG;  // never: <= 8 holes (one per two a's) + 15 tail rows
+                            t.zrows_m[t.nzm++] = r;
+                        }
+                }
+                finish_tile(t, t.np, t.nm, t.npr, t.nmr);
+                p->ftiles.push_back(t);
             }
-            p->ftiles.push_back(t);
+        } else {
+            // b-groups: the 16-blocks of [A0, v) dealt into groups of at most tbg/16 blocks, as evenly as possible
+            const int nblk = (v - A0 + 15) / 16, per = tbg / 16, ng = (nblk + per - 1) / per;
+            int blk = 0;
+            for (int gi = 0; gi < ng; ++gi) {
+                const int cnt = nblk / ng + (gi < nblk % ng ? 1 : 0);
+                FullTile t;
+                t.A0 = A0;
+                t.ta = sl.ta;
+                t.bg0 = A0 + 16 * blk;
+                t.nb = std::min(16 * cnt, v - t.bg0);
+                t.tbp = 16 * cnt;
+                blk += cnt;
+                const int N = TA * t.tbp;
+                finish_tile(t, N, N, N, N);
+                if (tight) {  // the full (b, d) rectangle of the group: no image, twice the step-0 flops, a strip of tbp rows per a
+                    t.chunk_off = chunks.size();
+                    for (int d0 = A0; d0 < v; d0 += 16)
+                        for (int b = t.bg0; b < t.bg0 + t.nb; ++b) chunks.push_back(make_int2(b, d0));
+                    while ((chunks.size() - t.chunk_off) % 8) chunks.push_back(make_int2(-1, 0));
+                    t.tiles_n = (int)((chunks.size() - t.chunk_off) / 8);
+                    const double f0 = 2.0 * p->x * (128.0 * sl.tiles_m) * (128.0 * t.tiles_n);
+                    sl.flops0 += f0;
+                    p->ff_step0 += f0;
+                }
+                p->ftiles.push_back(t);
+            }
         }
         sl.tile_end = (int)p->ftiles.size();
         p->slabs.push_back(sl);
@@ -851,32 +962,33 @@ int full_setup(ppl_plan_s *p, size_t room, bool dry = false) {
     if (!p->use_tma || !p->sa_ok || p->v < 2) return PPL_OK;
     const int v = p->vp, TA = ppl::TA_FULL;
     const size_t lpad_bytes = (p->v & 1) ? align256((size_t)p->x * p->vvp * 8) : 0;
-    const char *envg = getenv("PPL_TBG");  // debug override of the b-group width
-    int tbg = (envg && atoi(envg) >= 16) ? atoi(envg) / 16 * 16 : 256;
+    int tbg = p->dbg.full_tbg >= 16 ? p->dbg.full_tbg / 16 * 16 : 256;  // debug override of the largest tile (rows / 16)
     tbg = std::min(tbg, (v + 15) / 16 * 16);
     const size_t racc_bytes = p->tau_bytes;  // same shapes as tau+-
     std::vector<int2> chunks;
-    const char *envs = getenv("PPL_FULL_SLOTS");  // debug override: 1 = single W+- slot
-    const int want_slots = (envs && atoi(envs) == 1) ? 1 : 2;
-    const char *envx = getenv("PPL_FULL_STRIPS");  // debug override: 1 = one strip, 2 = two whenever they fit
-    const char *envt = getenv("PPL_FULL_TIGHT");   // debug override: 1 = memory-tight mode even when the slab strip fits
+    const int want_slots = p->dbg.full_slots == 1 ? 1 : 2;
     const int tbg0 = tbg;
-    size_t x_bytes = 0;
+    size_t x_bytes = 0, lq_bytes = 0;
     bool two_strips = false, fits = false;
     // First the slab strip (16 v^3 doubles: step 0 on d-block >= b-block only, 1/8 of nominal).  If it does not fit under
     // the cap, the memory-tight mode: a strip of one (slab; b-group) tile (16 tbg v^2), step 0 per tile on the group's
     // full (b, d) rectangle (1/4 of nominal), everything behind the fold unchanged.
-    for (int tight = (envt && atoi(envt) == 1) ? 1 : 0; tight <= 1 && !fits; ++tight)
+    for (int tight = p->dbg.full_tight == 1 ? 1 : 0; tight <= 1 && !fits; ++tight)
         for (tbg = tbg0;; tbg = std::max(16, tbg / 2 / 16 * 16)) {
             x_bytes = align256((size_t)TA * (tight ? tbg : v) * p->vvp * 8);
             // A second strip pays where slabs are short (medium: 26.19 -> 25.82 ms for 1 GB); at large it buys 0.15 % for
             // 8.2 GB and is not taken.  In the tight mode it is what lets step 0 of tile k+1 overlap the GEMMs of tile k.
-            const int want_strips = envx ? (atoi(envx) == 1 ? 1 : 2) : ((tight || x_bytes <= ((size_t)2 << 30)) ? 2 : 1);
-            const size_t slot = align256((size_t)TA * tbg * p->ldp * 8) + align256((size_t)TA * tbg * p->ldm * 8);
+            const int want_strips = p->dbg.full_strips ? (p->dbg.full_strips == 1 ? 1 : 2) : ((tight || x_bytes <= ((size_t)2 << 30)) ? 2 : 1);
+            const size_t slot_rows = (size_t)TA * tbg + 16;  // + 16: the minus run of a range tile may be a few rows longer than the plus run
+            const size_t slot = align256(slot_rows * p->ldp * 8) + align256(slot_rows * p->ldm * 8);
             const size_t part_cap = std::max<size_t>((size_t)64 << 20, slot / 8);
-            full_geometry(p, tbg, part_cap, &chunks, tight != 0);
+            if (full_geometry(p, tbg, part_cap, &chunks, tight != 0) != PPL_OK) {
+                p->dbg.full_rect_tiles = 1;  // (never taken: the range tiling failed its own invariants)
+                full_geometry(p, tbg, part_cap, &chunks, tight != 0);
+            }
             const size_t chunk_bytes = align256(chunks.size() * sizeof(int2));
-            const size_t base = x_bytes + align256(p->fpart_bytes) + racc_bytes + chunk_bytes + lpad_bytes + 256;
+            lq_bytes = p->diag_pack ? align256((size_t)p->x * p->ldq * 8) : 0;
+            const size_t base = x_bytes + align256(p->fpart_bytes) + racc_bytes + chunk_bytes + lpad_bytes + lq_bytes + 256;
             int ns = 0;
             for (int s = want_slots; s >= 1 && !ns; --s)
                 if (base + s * slot <= room) ns = s;
@@ -906,14 +1018,15 @@ int full_setup(ppl_plan_s *p, size_t room, bool dry = false) {
         (void)cudaGetLastError();
         return PPL_OK;
     }
+    const size_t slot_rows = (size_t)TA * p->tbg + 16;
     unsigned char *q = p->fws;
     p->fX = reinterpret_cast<double *>(q);
     q += x_bytes;
     for (int s = 0; s < p->fslots; ++s) {
         p->fWp[s] = reinterpret_cast<double *>(q);
-        q += align256((size_t)TA * p->tbg * p->ldp * 8);
+        q += align256(slot_rows * p->ldp * 8);
         p->fWm[s] = reinterpret_cast<double *>(q);
-        q += align256((size_t)TA * p->tbg * p->ldm * 8);
+        q += align256(slot_rows * p->ldm * 8);
     }
     p->fpart = reinterpret_cast<double *>(q);
     q += align256(p->fpart_bytes);
@@ -924,12 +1037,14 @@ int full_setup(ppl_plan_s *p, size_t room, bool dry = false) {
     q += align256(chunks.size() * sizeof(int2));
     p->Lpad = lpad_bytes ? reinterpret_cast<double *>(q) : nullptr;
     q += lpad_bytes;
+    p->Lq = lq_bytes ? reinterpret_cast<double *>(q) : nullptr;
+    q += lq_bytes;
     p->fX2 = two_strips ? reinterpret_cast<double *>(q) : nullptr;
     if (cudaMemcpy(p->fchunks, chunks.data(), chunks.size() * sizeof(int2), cudaMemcpyHostToDevice) != cudaSuccess) {
         (void)cudaGetLastError();
         return PPL_OK;
     }
-    const uint64_t rows = (uint64_t)TA * p->tbg;
+    const uint64_t rows = slot_rows;
     bool m = true;
     for (int s = 0; s < p->fslots; ++s) {
         m = m && make_map_2d(&p->mapFWp[s], p->fWp[s], (uint64_t)p->Kp, rows, (uint64_t)p->ldp * 8, ppl::BK, ppl::BN) == PPL_OK;
@@ -939,6 +1054,7 @@ int full_setup(ppl_plan_s *p, size_t room, bool dry = false) {
             m = m && make_map_2d(&p->mapFWmT[s], p->fWm[s], (uint64_t)p->Km, rows, (uint64_t)p->ldm * 8, 16, ppl::BK) == PPL_OK;
         }
     }
+    if (p->Lq) m = m && make_map_2d(&p->mapLq, p->Lq, (uint64_t)p->ldq, (uint64_t)p->x, (uint64_t)p->ldq * 8, 16, ppl::BK) == PPL_OK;
     if (!m) return PPL_OK;
     bool ok = true;
     for (int i = 0; i < 4 && ok; ++i) ok = ok && cudaStreamCreateWithFlags(&p->fs[i], cudaStreamNonBlocking) == cudaSuccess;
@@ -970,8 +1086,11 @@ int launch_step1t(const ppl_plan_s *p, const CUtensorMap *mapA, const CUtensorMa
     a.n_end = minus ? p->Km : p->Kp;
     a.n_base = a.n_begin & ~15;
     if (M <= 0 || a.n_end - a.n_begin <= 0) return PPL_OK;
-    a.kt_per_a = t.tbp / 16;
-    a.nkt = ppl::TA_FULL * a.kt_per_a;
+    a.range = t.range;
+    a.kap0 = minus ? t.km0 : t.kp0;
+    a.kt_per_a = t.range ? 1 : t.tbp / 16;
+    a.nkt = t.range ? (minus ? t.nmr : t.npr) / 16 : ppl::TA_FULL * a.kt_per_a;
+    if (a.nkt <= 0) return PPL_OK;
     a.A0 = t.A0;
     a.bg0 = t.bg0;
     a.v = p->vp;
@@ -998,6 +1117,22 @@ int launch_step1t(const ppl_plan_s *p, const CUtensorMap *mapA, const CUtensorMa
 int launch_reduce_acc(const ppl_plan_s *p, const FullTile &t, const double *part, int splitk, int M, bool minus, double *acc,
                       int64_t ld, cudaStream_t s) {
     if (M <= 0 || splitk <= 0) return PPL_OK;
+    if (t.range) {
+        ppl::ReduceRangeArgs a;
+        a.part = part;
+        a.splitk = splitk;
+        a.M = M;
+        a.N = minus ? t.nm : t.np;
+        a.k0 = minus ? t.km0 : t.kp0;
+        a.acc = acc;
+        a.ld = ld;
+        if (a.N <= 0) return PPL_OK;
+        const int64_t MN = (int64_t)a.M * a.N;
+        const int grid = (int)std::min<int64_t>((MN + 255) / 256, (int64_t)p->num_sms * 8);
+        ppl::k_reduce_range<<<grid, 256, 0, s>>>(a);
+        PPL_CUDA(cudaGetLastError());
+        return PPL_OK;
+    }
     ppl::ReduceAccArgs a;
     a.part = part;
     a.splitk = splitk;
@@ -1033,14 +1168,15 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
     int rc = check_ptrs(p, L, (phases & FULL_PACK) ? t2 : L, (phases & FULL_UNPACK) ? R : L, &vec16);
     ppl_opts_t opts;
     if (rc == PPL_OK) rc = check_opts(opts_in, &opts);
-    if (rc == PPL_OK && (!p->full_ok || (!vec16 && !p->Lpad))) rc = PPL_ERR_INVALID_ARG;  // TMA reads L: 16-byte aligned rows, or the padded copy
+    // only L is read by TMA (16-byte aligned rows, or the padded copy); t2 and R are packed / unpacked with scalar accesses
+    if (rc == PPL_OK && (!p->full_ok || (((uintptr_t)L & 15) != 0 && !p->Lpad))) rc = PPL_ERR_INVALID_ARG;
     if (rc != PPL_OK) return fail(rc);
 #define PPL_MARK(k, n)                                                             \
     do {                                                                           \
         if (prof && prof->mark(k, n, stream) != PPL_OK) return fail(PPL_ERR_CUDA); \
     } while (0)
     PPL_MARK(-1, 0);
-    static const bool dbg = getenv("PPL_DEBUG_SYNC") != nullptr;  // debug: synchronise and report after every launch
+    const bool dbg = p->dbg.debug_sync != 0;  // debug: synchronise and report after every launch
 #define PPL_DBG(label, k)                                                                              \
     do {                                                                                               \
         if (dbg) {                                                                                     \
@@ -1067,14 +1203,21 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
     }
     CUtensorMap mapL;
     if (make_map_2d(&mapL, L, (uint64_t)p->vvp, (uint64_t)p->x, (uint64_t)p->vvp * 8, 16, ppl::BK) != PPL_OK) return fail(PPL_ERR_CUDA);
+    if (p->Lq && p->diag_pack && !p->full_tight) {  // the diagonal 16 x 16 blocks of L, pairs b <= d only (|L| / (nvirt / 16) bytes)
+        const int64_t total = (int64_t)p->x * p->nfull * ppl::DIAG_PACKED;
+        const int grid = (int)std::min<int64_t>((total + 255) / 256, (int64_t)p->num_sms * 8);
+        ppl::k_pack_diag<<<std::max(grid, 1), 256, 0, stream>>>(L, p->Lq, p->x, p->vp, p->nfull, p->ldq);
+        PPL_CUDA(cudaGetLastError());
+        PPL_MARK(K_PACK, 1);
+    }
     const int TA = ppl::TA_FULL;
-    static const bool serial = getenv("PPL_FULL_SERIAL") != nullptr;  // debug: everything on the caller's stream
+    const bool serial = p->dbg.full_serial != 0;  // debug: everything on the caller's stream
     const bool conc = !prof && !dbg && !serial;
     // PPL_TRACE (debug): a timed event pair around every launch ON ITS OWN STREAM -- the concurrency is kept -- and a
     // timeline on stderr after a synchronise: "label index stream t_eligible_ms t_end_ms" (t_eligible: the stream has
     // reached the launch, i.e. its predecessors and awaited events are complete).
     static const bool trace_env = getenv("PPL_TRACE") != nullptr;
-    const bool trace = trace_env && conc;
+    const bool trace = (trace_env || p->dbg.trace) && conc;
     struct TraceRec {
         const char *label;
         int k, sid;
@@ -1124,7 +1267,7 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
         const int items = a0.tiles_m * a0.tiles_n;
         if (dual && unit_no >= 2) PPL_CUDA(cudaStreamWaitEvent(s0, p->ev_xfree[xi], 0));  // the folds of unit u - 2 have read this strip
         tb("step0", t ? t->bg0 : sl.A0, 0, s0);
-        ppl::k_step0_slab<<<std::min(items, p->num_sms), ppl::TMA_THREADS, ppl::SMEM_TMA, s0>>>(mapL, a0);
+        ppl::k_step0_slab<<<std::min(items, p->num_sms), ppl::TMA_THREADS, ppl::SMEM_TMA, s0>>>(mapL, p->Lq ? p->mapLq : mapL, a0);
         te(s0);
         PPL_CUDA(cudaGetLastError());
         PPL_DBG("k_step0_slab", sl.A0);
@@ -1145,7 +1288,8 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
         if (!tight && (rc = step0_unit(sl, nullptr)) != PPL_OK) return rc;
         for (int k = sl.tile_begin; k < sl.tile_end; ++k) {
             const FullTile &t = p->ftiles[k];
-            const int N = TA * t.tbp;
+            const int N = t.range ? t.np : TA * t.tbp;   // W+ rows contracted by use 1
+            const int Nm = t.range ? t.nm : TA * t.tbp;  // W- rows
             if (tight && (rc = step0_unit(sl, &t)) != PPL_OK) return rc;
             const int sl_w = conc ? (tile_no % p->fslots) : 0;  // W+- slot of this tile
             if (conc && tile_no >= p->fslots)  // the GEMMs of the tile that used this slot last still read it
@@ -1156,9 +1300,14 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
                 f.sc = p->vp;
                 f.s_row = p->vvp;
                 f.s_i = f.s_j = 0;
-                f.mode = 2;
-                f.rows = N;
+                f.mode = t.range ? 3 : 2;
+                f.rows = t.range ? t.npr + t.nzm : N;
                 f.row0 = 0;
+                f.kp0 = t.kp0;
+                f.kp1 = t.kp0 + t.np;
+                f.km0 = t.km0;
+                f.nzm = t.nzm;
+                for (int z = 0; z < t.nzm; ++z) f.zrows_m[z] = t.zrows_m[z];
                 f.o = p->o;
                 f.v = f.vs = p->vp;
                 f.scale = 1.0;
@@ -1175,7 +1324,7 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
                 f.ldp = p->ldp;
                 f.ldm = p->ldm;
                 const int nb = (p->vp + ppl::FT - 1) / ppl::FT - f.cb_min;
-                dim3 grid(nb * (nb + 1) / 2, ppl::fold_grid_y(nb * (nb + 1) / 2, N, p->num_sms));
+                dim3 grid(nb * (nb + 1) / 2, ppl::fold_grid_y(nb * (nb + 1) / 2, f.rows, p->num_sms));
                 tb("fold", k, 1, stream);
                 ppl::k_symfold<<<grid, 256, 0, stream>>>(f);
                 te(stream);
@@ -1200,10 +1349,10 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
             rc = launch_step1(p, &p->mapTp, &p->mapFWp[sl_w], p->mg_p, nullptr, 0, nullptr, 0, p->Mp, N, p->Kp, t.sp, partp, true, g0,
                               t.k0p);
             te(g0);
-            const bool m1 = minus && p->Km - t.k0m > 0;
+            const bool m1 = minus && p->Km - t.k0m > 0 && Nm > 0;
             if (rc == PPL_OK && m1) {
                 tb("use1-", k, 3, g1);
-                rc = launch_step1(p, &p->mapTm, &p->mapFWm[sl_w], p->mg_m, nullptr, 0, nullptr, 0, p->Mm, N, p->Km, t.sm, partm, true,
+                rc = launch_step1(p, &p->mapTm, &p->mapFWm[sl_w], p->mg_m, nullptr, 0, nullptr, 0, p->Mm, Nm, p->Km, t.sm, partm, true,
                                   g1, t.k0m);
                 te(g1);
             }
@@ -1237,7 +1386,7 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
                 PPL_DBG("use 2 plus (k_step1t_tma)", k);
                 ++n2;
             }
-            if (minus && p->Km - t.k1m > 0) {
+            if (minus && p->Km - t.k1m > 0 && Nm > 0) {
                 tb("use2-", k, 5, g3);
                 if ((rc = launch_step1t(p, &p->mapTm, &p->mapFWmT[sl_w], p->mg_m, p->Mm, t, true, p->raccm, p->ldm, g3)) != PPL_OK) return rc;
                 te(g3);
@@ -1327,13 +1476,15 @@ namespace {
 
 // The host half of ppl_plan: everything that follows from (nocc, nvirt, nchol), the byte budget `cap`, the SM count and
 // the kernel family alone -- packed geometry, row tiling of step 1, tile edge T, ring depth, buffer sizes.  No CUDA call.
-ppl_plan_s *plan_host(int nocc, int nvirt, int nchol, size_t workspace_bytes, size_t cap, int num_sms, bool use_tma, int *rc_out) {
+ppl_plan_s *plan_host(int nocc, int nvirt, int nchol, size_t workspace_bytes, size_t cap, int num_sms, bool use_tma,
+                      const ppl_debug_opts_t *dbg, int *rc_out) {
     *rc_out = PPL_OK;
     ppl_plan_s *p = new (std::nothrow) ppl_plan_s();
     if (!p) {
         *rc_out = PPL_ERR_ALLOC;
         return nullptr;
     }
+    if (dbg) p->dbg = *dbg;
     p->o = nocc;
     p->v = nvirt;
     p->x = nchol;
@@ -1352,8 +1503,7 @@ ppl_plan_s *plan_host(int nocc, int nvirt, int nchol, size_t workspace_bytes, si
     p->ldp = ((int64_t)p->Kp + 15) / 16 * 16;  // rows of the packed operands are 128-byte aligned: TMA-legal for any nvirt
     p->ldm = ((int64_t)std::max(p->Km, 1) + 15) / 16 * 16;
     p->use_tma = use_tma ? 1 : 0;
-    const char *envni = getenv("PPL_NI");  // debug override of the step-1 tile height
-    const int ni_env = (envni && atoi(envni) >= 1 && atoi(envni) <= 10) ? atoi(envni) : 10;  // largest instance used
+    const int ni_env = (p->dbg.ni_max >= 1 && p->dbg.ni_max <= 10) ? p->dbg.ni_max : 10;  // largest row-tile instance used
     const bool tma_full = p->use_tma && p->vec16;
     p->mg_full = tma_full ? m_geom_tma(nocc * nocc, ni_env) : m_geom_plain(nocc * nocc);
     p->mg_p = p->use_tma ? m_geom_tma(p->Mp, ni_env) : m_geom_plain(p->Mp);
@@ -1366,17 +1516,17 @@ ppl_plan_s *plan_host(int nocc, int nvirt, int nchol, size_t workspace_bytes, si
 
     // choose the tile edge T (and ring depth) that minimises the estimated apply time under the cap:
     // first with the packed operands of PPL_SYM_PAIR_SA, and if they do not fit, without them
-    const char *envT = getenv("PPL_TILE");  // debug override
+    const int forced_T = p->dbg.tile_edge > 0 ? std::min(p->dbg.tile_edge, nvirt) : 0;  // debug override
     double best_t = 1e300;
     int best_T = 0, best_ring = 1, best_sa = 0;
     PlanEval best_ev;
     for (int sa = 1; sa >= 0 && best_T == 0; --sa)
         for (int T = nvirt; T >= 1; --T) {
-            if (envT && atoi(envT) > 0 && T != std::min(atoi(envT), nvirt)) continue;
+            if (forced_T && T != forced_T) continue;
             // only edges that tile v evenly or nearly so (ragged edge at least T/2), to keep edge tiles efficient
             const int nblk = (nvirt + T - 1) / T;
             const int r = nvirt - (nblk - 1) * T;
-            if (!envT && nblk > 1 && 2 * r < T) continue;
+            if (!forced_T && nblk > 1 && 2 * r < T) continue;
             const PlanEval ev = evaluate(g, nocc, nvirt, nchol, T, sa != 0, p->num_sms);
             const size_t fixed = ev.x_bytes + ev.part_bytes + (sa ? p->tau_bytes : 0) + 256;
             int ring = 0;
@@ -1417,16 +1567,17 @@ bool dims_ok(int nocc, int nvirt, int nchol) {
     return nocc >= 1 && nvirt >= 1 && nchol >= 1 && (int64_t)nvirt * nvirt <= INT32_MAX / 2 && (int64_t)nocc * nocc <= INT32_MAX / 2;
 }
 
-int full_min_v() {
-    const char *envf = getenv("PPL_FULL_MIN_V");  // debug override
-    return envf ? atoi(envf) : 52;
-}
+int full_min_v(const ppl_plan_s *p) { return p->dbg.full_min_v > 0 ? p->dbg.full_min_v : 52; }
 
 }  // namespace
 
 extern "C" {
 
 ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
+    return ppl_plan_ex(nocc, nvirt, nchol, workspace_bytes, nullptr);
+}
+
+ppl_plan_t *ppl_plan_ex(int nocc, int nvirt, int nchol, size_t workspace_bytes, const ppl_debug_opts_t *dbg) {
     if (!dims_ok(nocc, nvirt, nchol)) {
         fail(PPL_ERR_INVALID_ARG);
         return nullptr;
@@ -1450,10 +1601,9 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
     }
     const size_t auto_cap = (size_t)(0.9 * (double)free_b);
     const size_t cap = workspace_bytes ? std::min(workspace_bytes, auto_cap) : auto_cap;
-    const char *envk = getenv("PPL_KERNELS");  // debug override: "cpasync" forces the non-TMA kernels
-    const bool use_tma = !(envk && strcmp(envk, "cpasync") == 0) && get_encode() != nullptr;
+    const bool use_tma = !(dbg && dbg->cpasync_kernels) && get_encode() != nullptr;
     int rc_host = PPL_OK;
-    ppl_plan_s *p = plan_host(nocc, nvirt, nchol, workspace_bytes, cap, prop.multiProcessorCount, use_tma, &rc_host);
+    ppl_plan_s *p = plan_host(nocc, nvirt, nchol, workspace_bytes, cap, prop.multiProcessorCount, use_tma, dbg, &rc_host);
     if (!p) {
         fail(rc_host);
         return nullptr;
@@ -1533,25 +1683,30 @@ ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
     // PPL_SYM_PAIR_SA at nocc = 5..8, nchol = 4 nvirt: 0.157 vs 0.186 ms at nvirt = 48, 0.283 vs 0.274 ms at 53,
     // 0.365 vs 0.328 ms at 64, 1.71 vs 0.97 ms at 96)
     full_setup(p, cap > p->ws_bytes ? cap - p->ws_bytes : 0);
-    if (p->full_ok && nvirt >= full_min_v()) p->sym = PPL_SYM_FULL;
+    if (p->full_ok && nvirt >= full_min_v(p)) p->sym = PPL_SYM_FULL;
     return p;
 }
 
 // ppl_plan_dry: the planner alone, for a stated device (free bytes, SM count): no CUDA call, nothing allocated.
 int ppl_plan_dry(int nocc, int nvirt, int nchol, size_t workspace_bytes, size_t device_free_bytes, int num_sms, int mode,
                  ppl_info_t *out) {
+    return ppl_plan_dry_ex(nocc, nvirt, nchol, workspace_bytes, device_free_bytes, num_sms, mode, nullptr, out);
+}
+
+int ppl_plan_dry_ex(int nocc, int nvirt, int nchol, size_t workspace_bytes, size_t device_free_bytes, int num_sms, int mode,
+                    const ppl_debug_opts_t *dbg, ppl_info_t *out) {
     if (!out || !dims_ok(nocc, nvirt, nchol) || num_sms < 1 || mode < -1 || mode > PPL_SYM_FULL) return fail(PPL_ERR_INVALID_ARG);
     const size_t auto_cap = (size_t)(0.9 * (double)device_free_bytes);
     const size_t cap = workspace_bytes ? std::min(workspace_bytes, auto_cap) : auto_cap;
     int rc = PPL_OK;
-    ppl_plan_s *p = plan_host(nocc, nvirt, nchol, workspace_bytes, cap, num_sms, true, &rc);
+    ppl_plan_s *p = plan_host(nocc, nvirt, nchol, workspace_bytes, cap, num_sms, !(dbg && dbg->cpasync_kernels), dbg, &rc);
     if (!p) return fail(rc);
     p->dry = 1;
     p->sym = p->sa_ok ? PPL_SYM_PAIR_SA : PPL_SYM_PAIR;
     rc = build_tiles(p);
     if (rc == PPL_OK) {
         full_setup(p, cap > p->ws_bytes ? cap - p->ws_bytes : 0, true);
-        if (p->full_ok && nvirt >= full_min_v()) p->sym = PPL_SYM_FULL;
+        if (p->full_ok && nvirt >= full_min_v(p)) p->sym = PPL_SYM_FULL;
         if (mode >= 0) rc = ppl_plan_set_symmetry(p, mode);
     }
     if (rc == PPL_OK) rc = ppl_plan_info(p, out);
@@ -1647,10 +1802,12 @@ int ppl_plan_info(const ppl_plan_t *p, ppl_info_t *out) {
         out->ring = 1;
         out->splitk = p->ftiles.empty() ? 0 : p->ftiles[0].sp.splitk;
         // pack, unpack, one step 0 per slab -- per tile in the memory-tight mode -- (+ the L pad copy for odd nvirt)
-        int launches = 2 + (int)(p->full_tight ? p->ftiles.size() : p->slabs.size()) + ((p->v & 1) ? 1 : 0);
+        int launches = 2 + (int)(p->full_tight ? p->ftiles.size() : p->slabs.size()) + ((p->v & 1) ? 1 : 0) +
+                       ((p->diag_pack && !p->full_tight) ? 1 : 0);
         for (const FullTile &t : p->ftiles) {
-            const bool m1 = minus && p->Km - t.k0m > 0;
-            launches += 1 + (m1 ? 4 : 2) + (p->Kp - t.k1p > 0 ? 1 : 0) + (minus && p->Km - t.k1m > 0 ? 1 : 0);
+            const int Nm = t.range ? t.nm : ppl::TA_FULL * t.tbp;
+            const bool m1 = minus && p->Km - t.k0m > 0 && Nm > 0;
+            launches += 1 + (m1 ? 4 : 2) + (p->Kp - t.k1p > 0 ? 1 : 0) + (minus && p->Km - t.k1m > 0 && Nm > 0 ? 1 : 0);
         }
         out->launches_per_apply = launches;
         out->step1_tile_m = p->bm_p;
@@ -1803,7 +1960,10 @@ int ppl_apply_dense(ppl_plan_t *p, const double *eri, int a0, int na, const doub
                 make_map_2d(&mapE, eri, (uint64_t)p->vv, (uint64_t)rows, (uint64_t)p->vv * 8, ppl::BK, ppl::BN) != PPL_OK))
         return fail(PPL_ERR_CUDA);
     // rows of the slab matrix [(a,b)][(c,d)] in chunks the partials buffer can hold
-    const int chunk = (int)std::min<int64_t>(rows, std::max<int64_t>(ppl::BN, (int64_t)p->T * p->T / ppl::BN * ppl::BN));
+    // (the buffer was sized for N <= T*T rows at the planner's split: with split-K 1 it holds part_bytes / (8 M) rows)
+    int64_t chunk = std::min<int64_t>(rows, (int64_t)(p->part_bytes / ((size_t)8 * M)));
+    if (chunk >= ppl::BN) chunk = chunk / ppl::BN * ppl::BN;
+    if (chunk < 1) return fail(PPL_ERR_WORKSPACE_TOO_SMALL);
     Tile t;
     t.a0 = a0;
     t.b0 = 0;
@@ -1812,7 +1972,7 @@ int ppl_apply_dense(ppl_plan_t *p, const double *eri, int a0, int na, const doub
     t.mirror = 0;
     for (int64_t n0 = 0; n0 < rows; n0 += chunk) {
         const int N = (int)std::min<int64_t>(chunk, rows - n0);
-        const SplitChoice sc = choose_split(M, N, p->vv, p->num_sms, p->mg_full, p->part_bytes);
+        SplitChoice sc = choose_split(M, N, p->vv, p->num_sms, p->mg_full, p->part_bytes);
         if ((size_t)sc.splitk * M * N * 8 > p->part_bytes) return fail(PPL_ERR_WORKSPACE_TOO_SMALL);
         const double *B = eri + n0 * p->vv;
         CUtensorMap mapB;  // the chunk's rows as their own tensor so that tile-edge rows beyond it read as zero
@@ -1868,8 +2028,7 @@ static int apply_host_full(ppl_plan_s *p, const double *Lh, const double *t2h, d
         return fail(PPL_ERR_ALLOC);
     }
     if (!p->hstage[0]) {
-        const char *envc = getenv("PPL_HOST_CHUNK_MB");  // debug override of the staging-buffer size
-        const size_t want = (envc && atol(envc) > 0) ? (size_t)atol(envc) << 20 : (size_t)1 << 30;
+        const size_t want = p->dbg.host_chunk_mb > 0 ? (size_t)p->dbg.host_chunk_mb << 20 : (size_t)1 << 30;  // debug override of the staging-buffer size
         p->hchunk_rows = (int)std::max<int64_t>(1, std::min<int64_t>(rows, (int64_t)(want / row_bytes)));
         for (int i = 0; i < 2; ++i)
             if (cudaMalloc(&p->hstage[i], (size_t)p->hchunk_rows * row_bytes) != cudaSuccess) {

@@ -1,0 +1,415 @@
+// ppl_contract.cu -- the generic pair contraction 'op0,op1->out' of the paper's generic recipe:
+//
+//     C[out] = beta * C[out] + alpha * sum_{summed letters} A[op0] * B[op1]            (FP64, dense row-major operands)
+//
+// for any two-operand contraction of tensordot type (every letter occurs in exactly two of op0, op1, out; the paper's
+// "a...,b...->a..b.."), e.g. the ladder's own steps 'xac,xbd->acbd' and 'abcd,ecfd->efab'.
+//
+// The paper moves such a contraction through VRAM in host-driven batches along the surviving (non-summed) axes and calls
+// tensordot -- i.e. permuted copies plus a library DGEMM -- per batch (Table 1 mem(generic)).  Here the
+// operands are resident and nothing is permuted or copied: the contraction is ONE GEMM  C[m][n] = sum_k A[m][k] B[n][k]
+// whose rows m run over the surviving letters of op0, columns n over those of op1 and k over the summed letters, with
+// every operand addressed in place through offset tables ("block-scatter" addressing: element (m, k) of A sits at
+// offAm[m] + offAk[k]).  The batches of the paper are the CTA tiles (128 m x 128 n): always along surviving axes; the
+// summed axes (the Cholesky index x among them) are never split across launches -- only inside the kernel (split-K with
+// a fixed-order reduction, so results are bit-reproducible).  Tiles are staged global -> shared with cp.async (16-byte
+// where an operand's unit-stride letter allows, else 8-byte), a 4-stage ring, and multiplied on the FP64 tensor pipe
+// (DMMA m8n8k4) with the accumulators in registers.
+#include "../../include/ppl.h"
+#include "ppl_device.cuh"
+
+#include <algorithm>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+int ppl_fail_code(int code);  // ppl_api.cu: records the code for ppl_last_error() and returns it
+
+namespace ppl {
+
+constexpr int GLD_MN = BM + 4;  // row stride of a [k][m] tile (doubles): 16-byte aligned rows, conflict-free LDS.64
+constexpr int GLD_K = BK + 4;   // row stride of a [m][k] tile
+constexpr int GTILE = (BK * GLD_MN > BM * GLD_K) ? BK * GLD_MN : BM * GLD_K;  // doubles per operand tile per stage
+constexpr size_t SMEM_GATHER = (size_t)STAGES * 2 * GTILE * sizeof(double);
+
+struct ContractArgs {
+    const double *A, *B;
+    double *C;
+    const int64_t *offAm, *offAk, *offBn, *offBk, *offCm, *offCn;  // element offsets
+    int M, N, K;
+    int a_vec, b_vec;   // 1: pairs along the operand's unit-stride direction may be fetched with one 16-byte copy
+    int k_per_split;    // multiple of BK
+    int splitk;
+    double *part;       // splitk > 1: [splitk][M][N]
+    double alpha, beta;
+};
+
+// One operand tile: 128 rows (m or n) x 16 k.  KFAST: the operand's unit-stride letter is a summed one -> smem [row][k]
+// (stride GLD_K), threads run along k; else smem [k][row] (stride GLD_MN), threads run along the rows.
+template <bool KFAST>
+__device__ __forceinline__ void gather_tile(double *s, const double *g, const int64_t *offR, const int64_t *offK, int r0, int R,
+                                            int k0, int Kend, bool vec, int tid) {
+    if (KFAST) {
+        if (vec) {  // 8 pairs per row
+#pragma unroll
+            for (int c = 0; c < (BM * BK / 2) / NTHREADS; ++c) {
+                const int idx = tid + c * NTHREADS, row = idx >> 3, k = (idx & 7) << 1;
+                const bool ok = r0 + row < R && k0 + k < Kend;  // Kend and k0 + k even: the pair is in or out as one
+                const double *src = ok ? g + offR[r0 + row] + offK[k0 + k] : g;
+                cp_async16(s + row * GLD_K + k, src, ok ? 16 : 0);
+            }
+        } else {
+#pragma unroll
+            for (int c = 0; c < (BM * BK) / NTHREADS; ++c) {
+                const int idx = tid + c * NTHREADS, row = idx >> 4, k = idx & 15;
+                const bool ok = r0 + row < R && k0 + k < Kend;
+                const double *src = ok ? g + offR[r0 + row] + offK[k0 + k] : g;
+                cp_async8(s + row * GLD_K + k, src, ok ? 8 : 0);
+            }
+        }
+    } else {
+        if (vec) {  // 64 pairs per k
+#pragma unroll
+            for (int c = 0; c < (BM * BK / 2) / NTHREADS; ++c) {
+                const int idx = tid + c * NTHREADS, k = idx >> 6, row = (idx & 63) << 1;
+                const bool ok = r0 + row < R && k0 + k < Kend;  // R even when vec
+                const double *src = ok ? g + offR[r0 + row] + offK[k0 + k] : g;
+                cp_async16(s + k * GLD_MN + row, src, ok ? 16 : 0);
+            }
+        } else {
+#pragma unroll
+            for (int c = 0; c < (BM * BK) / NTHREADS; ++c) {
+                const int idx = tid + c * NTHREADS, k = idx >> 7, row = idx & 127;
+                const bool ok = r0 + row < R && k0 + k < Kend;
+                const double *src = ok ? g + offR[r0 + row] + offK[k0 + k] : g;
+                cp_async8(s + k * GLD_MN + row, src, ok ? 8 : 0);
+            }
+        }
+    }
+}
+
+template <bool AKF, bool BKF>
+__global__ void __launch_bounds__(NTHREADS, 1) k_contract_gather(const ContractArgs p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double *As = reinterpret_cast<double *>(smem_raw);
+    double *Bs = As + STAGES * GTILE;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int g = lane >> 2, q = lane & 3;
+    const int wm = warp / WARPS_N, wn = warp % WARPS_N;
+    const int tiles_m = (p.M + BM - 1) / BM, tiles_n = (p.N + BN - 1) / BN;
+    int tm, tn;
+    raster(blockIdx.x, tiles_m, tiles_n, tm, tn);
+    const int m0 = tm * BM, n0 = tn * BN;
+    const int z = blockIdx.y;
+    const int Kbeg = z * p.k_per_split, Kend = min(p.K, Kbeg + p.k_per_split);
+    const int nkt = max(0, (Kend - Kbeg + BK - 1) / BK);
+
+    double acc[8][4][2];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+#pragma unroll
+    for (int s = 0; s < STAGES - 1; ++s) {
+        if (s < nkt) {
+            gather_tile<AKF>(As + s * GTILE, p.A, p.offAm, p.offAk, m0, p.M, Kbeg + s * BK, Kend, p.a_vec != 0, tid);
+            gather_tile<BKF>(Bs + s * GTILE, p.B, p.offBn, p.offBk, n0, p.N, Kbeg + s * BK, Kend, p.b_vec != 0, tid);
+        }
+        cp_async_commit();
+    }
+    // element (row, kk) of a stage tile
+    constexpr int a_sr = AKF ? GLD_K : 1, a_sk = AKF ? 1 : GLD_MN;
+    constexpr int b_sr = BKF ? GLD_K : 1, b_sk = BKF ? 1 : GLD_MN;
+    for (int kt = 0; kt < nkt; ++kt) {
+        cp_async_wait<STAGES - 2>();
+        __syncthreads();
+        {
+            const int kn = kt + STAGES - 1;
+            if (kn < nkt) {
+                const int s = kn % STAGES;
+                gather_tile<AKF>(As + s * GTILE, p.A, p.offAm, p.offAk, m0, p.M, Kbeg + kn * BK, Kend, p.a_vec != 0, tid);
+                gather_tile<BKF>(Bs + s * GTILE, p.B, p.offBn, p.offBk, n0, p.N, Kbeg + kn * BK, Kend, p.b_vec != 0, tid);
+            }
+            cp_async_commit();
+        }
+        const double *as = As + (kt % STAGES) * GTILE + (wm * WTM + g) * a_sr;
+        const double *bs = Bs + (kt % STAGES) * GTILE + (wn * WTN + g) * b_sr;
+#pragma unroll
+        for (int k4 = 0; k4 < BK / 4; ++k4) {
+            const int kk = k4 * 4 + q;
+            double a[8], b[4];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) a[i] = as[i * 8 * a_sr + kk * a_sk];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) b[j] = bs[j * 8 * b_sr + kk * b_sk];
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        }
+    }
+    cp_async_wait<0>();
+
+    // epilogue: block (i,j): row g <-> m = mw + 8i + g; cols n = nw + 8j + 2q, +1
+    if (p.splitk > 1) {
+        double *part = p.part + (int64_t)z * p.M * p.N;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const int m = m0 + wm * WTM + 8 * i + g;
+            if (m >= p.M) continue;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int n = n0 + wn * WTN + 8 * j + 2 * q;
+                if (n < p.N) part[(int64_t)m * p.N + n] = acc[i][j][0];
+                if (n + 1 < p.N) part[(int64_t)m * p.N + n + 1] = acc[i][j][1];
+            }
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const int m = m0 + wm * WTM + 8 * i + g;
+            if (m >= p.M) continue;
+            double *crow = p.C + p.offCm[m];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int n = n0 + wn * WTN + 8 * j + 2 * q;
+                if (n < p.N) r_update(crow + p.offCn[n], acc[i][j][0], p.alpha, p.beta);
+                if (n + 1 < p.N) r_update(crow + p.offCn[n + 1], acc[i][j][1], p.alpha, p.beta);
+            }
+        }
+    }
+}
+
+// fixed-order sum of the split-K partials, then C = beta C + alpha sum
+__global__ void __launch_bounds__(256) k_contract_reduce(const ContractArgs p) {
+    const int64_t MN = (int64_t)p.M * p.N;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < MN; idx += (int64_t)gridDim.x * blockDim.x) {
+        double s = 0.0;
+        for (int zz = 0; zz < p.splitk; ++zz) s += p.part[(int64_t)zz * MN + idx];
+        const int m = (int)(idx / p.N), n = (int)(idx - (int64_t)m * p.N);
+        r_update(p.C + p.offCm[m] + p.offCn[n], s, p.alpha, p.beta);
+    }
+}
+
+}  // namespace ppl
+
+namespace {
+
+struct Parsed {
+    std::vector<char> op[3];
+    int64_t ext[128];
+    std::vector<char> Ml, Nl, Kl;  // surviving letters of op0 / op1 (in their operand's order), summed letters (in op0's order)
+    int64_t M = 1, N = 1, K = 1;
+};
+
+// "op0,op1->out": letters only, none repeated inside one operand, every letter in exactly two of the three
+int parse(const char *subs, const int64_t *dims0, const int64_t *dims1, Parsed *ps) {
+    if (!subs || !dims0 || !dims1) return PPL_ERR_INVALID_ARG;
+    int which = 0;
+    for (const char *q = subs; *q; ++q) {
+        const char ch = *q;
+        if (ch == ' ') continue;
+        if (ch == ',') {
+            if (which != 0) return PPL_ERR_INVALID_ARG;
+            which = 1;
+        } else if (ch == '-' && q[1] == '>') {
+            if (which != 1) return PPL_ERR_INVALID_ARG;
+            which = 2;
+            ++q;
+        } else if ((ch >= 'a' && ch <= 'z') || (ch >= 'A' && ch <= 'Z')) {
+            for (char c : ps->op[which])
+                if (c == ch) return PPL_ERR_INVALID_ARG;
+            if (ps->op[which].size() >= 12) return PPL_ERR_INVALID_ARG;
+            ps->op[which].push_back(ch);
+        } else {
+            return PPL_ERR_INVALID_ARG;
+        }
+    }
+    if (which != 2) return PPL_ERR_INVALID_ARG;
+    for (int k = 0; k < 128; ++k) ps->ext[k] = 0;
+    auto has = [&](int w, char c) { return std::find(ps->op[w].begin(), ps->op[w].end(), c) != ps->op[w].end(); };
+    for (size_t k = 0; k < ps->op[0].size(); ++k) {
+        if (dims0[k] < 1) return PPL_ERR_INVALID_ARG;
+        ps->ext[(int)ps->op[0][k]] = dims0[k];
+    }
+    for (size_t k = 0; k < ps->op[1].size(); ++k) {
+        const char c = ps->op[1][k];
+        if (dims1[k] < 1 || (has(0, c) && ps->ext[(int)c] != dims1[k])) return PPL_ERR_INVALID_ARG;
+        ps->ext[(int)c] = dims1[k];
+    }
+    for (char c : ps->op[0]) {
+        if (has(1, c) == has(2, c)) return PPL_ERR_INVALID_ARG;  // in all three (batch letter) or in op0 alone
+        (has(1, c) ? ps->Kl : ps->Ml).push_back(c);
+    }
+    for (char c : ps->op[1]) {
+        if (has(0, c) == has(2, c)) return PPL_ERR_INVALID_ARG;
+        if (!has(0, c)) ps->Nl.push_back(c);
+    }
+    for (char c : ps->op[2])
+        if (!has(0, c) && !has(1, c)) return PPL_ERR_INVALID_ARG;
+    if (ps->op[2].size() != ps->Ml.size() + ps->Nl.size()) return PPL_ERR_INVALID_ARG;
+    for (char c : ps->Ml) ps->M *= ps->ext[(int)c];
+    for (char c : ps->Nl) ps->N *= ps->ext[(int)c];
+    for (char c : ps->Kl) ps->K *= ps->ext[(int)c];
+    const int64_t lim = INT32_MAX / 2;
+    if (ps->M > lim || ps->N > lim || ps->K > lim) return PPL_ERR_INVALID_ARG;
+    return PPL_OK;
+}
+
+// element stride of letter c in a dense row-major array with subscripts `op`
+int64_t stride_of(const std::vector<char> &op, const int64_t *ext, char c) {
+    int64_t s = 1;
+    for (size_t k = op.size(); k-- > 0;) {
+        if (op[k] == c) return s;
+        s *= ext[(int)op[k]];
+    }
+    return 0;
+}
+
+// offsets of the flattened index over `letters` (last letter fastest) in the array with subscripts `op`
+void fill_offsets(const std::vector<char> &letters, const std::vector<char> &op, const int64_t *ext, int64_t count, int64_t *out) {
+    std::vector<int64_t> st(letters.size()), ex(letters.size()), dig(letters.size(), 0);
+    for (size_t k = 0; k < letters.size(); ++k) {
+        st[k] = stride_of(op, ext, letters[k]);
+        ex[k] = ext[(int)letters[k]];
+    }
+    int64_t off = 0;
+    for (int64_t i = 0; i < count; ++i) {
+        out[i] = off;
+        for (size_t k = letters.size(); k-- > 0;) {  // odometer
+            off += st[k];
+            if (++dig[k] < ex[k]) break;
+            off -= st[k] * ex[k];
+            dig[k] = 0;
+        }
+    }
+}
+
+// pairs (2i, 2i+1) along `run` adjacent in memory and every address of a pair 16-byte aligned?
+bool pairs_ok(const int64_t *run, int64_t nrun, const int64_t *other, int64_t nother, const void *base) {
+    if (((uintptr_t)base & 15) != 0 || (nrun & 1)) return false;
+    for (int64_t i = 0; i < nrun; i += 2)
+        if ((run[i] & 1) || run[i + 1] != run[i] + 1) return false;
+    for (int64_t i = 0; i < nother; ++i)
+        if (other[i] & 1) return false;
+    return true;
+}
+
+size_t table_bytes(const Parsed &ps) { return (size_t)(2 * ps.M + 2 * ps.N + 2 * ps.K) * sizeof(int64_t); }
+
+int pick_splitk(const Parsed &ps, int sms, size_t room) {
+    const int64_t tiles = ((ps.M + ppl::BM - 1) / ppl::BM) * ((ps.N + ppl::BN - 1) / ppl::BN);
+    const int64_t nkt = (ps.K + ppl::BK - 1) / ppl::BK;
+    int64_t s = std::min<int64_t>((2 * sms + tiles - 1) / tiles, nkt / 8);  // about two waves, at least 8 k-tiles per split
+    s = std::max<int64_t>(1, std::min<int64_t>(s, 64));
+    while (s > 1 && (size_t)s * ps.M * ps.N * 8 > room) --s;
+    return (int)s;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ppl_contract_pair_workspace(const char *subscripts, const int64_t *dims0, const int64_t *dims1, size_t *bytes) {
+    Parsed ps;
+    const int rc = parse(subscripts, dims0, dims1, &ps);
+    if (rc != PPL_OK || !bytes) return ppl_fail_code(rc != PPL_OK ? rc : PPL_ERR_INVALID_ARG);
+    const int s = pick_splitk(ps, 148, ~(size_t)0);
+    *bytes = ((table_bytes(ps) + 255) & ~(size_t)255) + (s > 1 ? (size_t)s * ps.M * ps.N * 8 : 0);
+    return PPL_OK;
+}
+
+int ppl_contract_pair(const char *subscripts, const int64_t *dims0, const int64_t *dims1, const double *A, const double *B, double *C,
+                      double alpha, double beta, void *workspace, size_t workspace_bytes, void *stream_) {
+    Parsed ps;
+    int rc = parse(subscripts, dims0, dims1, &ps);
+    if (rc != PPL_OK) return ppl_fail_code(rc);
+    if (!A || !B || !C || (((uintptr_t)A | (uintptr_t)B | (uintptr_t)C) & 7)) return ppl_fail_code(PPL_ERR_INVALID_ARG);
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess || prop.major != 10) {
+        (void)cudaGetLastError();
+        return ppl_fail_code(PPL_ERR_UNSUPPORTED_DEVICE);
+    }
+    const size_t tb = (table_bytes(ps) + 255) & ~(size_t)255;
+    if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < tb) return ppl_fail_code(PPL_ERR_WORKSPACE_TOO_SMALL);
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+
+    // offset tables: rows of A / C over the surviving letters of op0, columns of B / C over those of op1, k over the
+    // summed letters (in op0's order for both operands)
+    std::vector<int64_t> tab((size_t)(2 * ps.M + 2 * ps.N + 2 * ps.K));
+    int64_t *hAm = tab.data(), *hCm = hAm + ps.M, *hBn = hCm + ps.M, *hCn = hBn + ps.N, *hAk = hCn + ps.N, *hBk = hAk + ps.K;
+    fill_offsets(ps.Ml, ps.op[0], ps.ext, ps.M, hAm);
+    fill_offsets(ps.Ml, ps.op[2], ps.ext, ps.M, hCm);
+    fill_offsets(ps.Nl, ps.op[1], ps.ext, ps.N, hBn);
+    fill_offsets(ps.Nl, ps.op[2], ps.ext, ps.N, hCn);
+    fill_offsets(ps.Kl, ps.op[0], ps.ext, ps.K, hAk);
+    fill_offsets(ps.Kl, ps.op[1], ps.ext, ps.K, hBk);
+    // (a pageable source is staged by the runtime before the call returns: `tab` may go out of scope afterwards)
+    if (cudaMemcpyAsync(workspace, tab.data(), tab.size() * sizeof(int64_t), cudaMemcpyHostToDevice, stream) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return ppl_fail_code(PPL_ERR_CUDA);
+    }
+    const int64_t *d = reinterpret_cast<const int64_t *>(workspace);
+    ppl::ContractArgs a;
+    a.A = A;
+    a.B = B;
+    a.C = C;
+    a.offAm = d;
+    a.offCm = d + ps.M;
+    a.offBn = a.offCm + ps.M;
+    a.offCn = a.offBn + ps.N;
+    a.offAk = a.offCn + ps.N;
+    a.offBk = a.offAk + ps.K;
+    a.M = (int)ps.M;
+    a.N = (int)ps.N;
+    a.K = (int)ps.K;
+    // which way does each operand run in memory: along a summed letter (k-fast) or along a surviving one?
+    const bool a_kfast = !ps.op[0].empty() && std::find(ps.Kl.begin(), ps.Kl.end(), ps.op[0].back()) != ps.Kl.end();
+    const bool b_kfast = !ps.op[1].empty() && std::find(ps.Kl.begin(), ps.Kl.end(), ps.op[1].back()) != ps.Kl.end();
+    a.a_vec = a_kfast ? pairs_ok(hAk, ps.K, hAm, ps.M, A) : pairs_ok(hAm, ps.M, hAk, ps.K, A);
+    a.b_vec = b_kfast ? pairs_ok(hBk, ps.K, hBn, ps.N, B) : pairs_ok(hBn, ps.N, hBk, ps.K, B);
+    a.splitk = pick_splitk(ps, prop.multiProcessorCount, workspace_bytes - tb);
+    const int64_t nkt = (ps.K + ppl::BK - 1) / ppl::BK;
+    const int64_t kt_per = (nkt + a.splitk - 1) / a.splitk;
+    a.splitk = (int)((nkt + kt_per - 1) / kt_per);  // no empty splits
+    a.k_per_split = (int)(kt_per * ppl::BK);
+    a.part = a.splitk > 1 ? reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(workspace) + tb) : nullptr;
+    a.alpha = alpha;
+    a.beta = beta;
+
+    static bool attr_set[64] = {};
+    if (dev >= 0 && dev < 64 && !attr_set[dev]) {
+        bool ok = cudaFuncSetAttribute(ppl::k_contract_gather<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
+        ok = ok && cudaFuncSetAttribute(ppl::k_contract_gather<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
+        ok = ok && cudaFuncSetAttribute(ppl::k_contract_gather<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
+        ok = ok && cudaFuncSetAttribute(ppl::k_contract_gather<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
+        if (!ok) {
+            (void)cudaGetLastError();
+            return ppl_fail_code(PPL_ERR_CUDA);
+        }
+        attr_set[dev] = true;
+    }
+    const int64_t tiles = ((ps.M + ppl::BM - 1) / ppl::BM) * ((ps.N + ppl::BN - 1) / ppl::BN);
+    if (tiles > INT32_MAX) return ppl_fail_code(PPL_ERR_INVALID_ARG);
+    const dim3 grid((unsigned)tiles, (unsigned)a.splitk);
+    if (a_kfast && b_kfast)
+        ppl::k_contract_gather<true, true><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
+    else if (a_kfast)
+        ppl::k_contract_gather<true, false><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
+    else if (b_kfast)
+        ppl::k_contract_gather<false, true><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
+    else
+        ppl::k_contract_gather<false, false><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
+    if (cudaGetLastError() != cudaSuccess) return ppl_fail_code(PPL_ERR_CUDA);
+    if (a.splitk > 1) {
+        const int64_t MN = ps.M * ps.N;
+        const int g = (int)std::min<int64_t>((MN + 255) / 256, (int64_t)prop.multiProcessorCount * 8);
+        ppl::k_contract_reduce<<<g, 256, 0, stream>>>(a);
+        if (cudaGetLastError() != cudaSuccess) return ppl_fail_code(PPL_ERR_CUDA);
+    }
+    return PPL_OK;
+}
+
+}  // extern "C"

@@ -16,49 +16,9 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "ppl_device.cuh"
+
 namespace ppl {
-
-constexpr int BM = 128;      // CTA tile rows
-constexpr int BN = 128;      // CTA tile cols
-constexpr int BK = 16;       // k per pipeline stage
-constexpr int STAGES = 4;    // cp.async ring depth
-constexpr int NTHREADS = 256;
-constexpr int WARPS_N = 4;   // 2 (m) x 4 (n) warps, warp tile 64 x 32
-constexpr int WTM = 64, WTN = 32;
-constexpr int PADMN = 4;     // row padding (doubles) of the MN-contiguous smem layout
-constexpr int LDS_MN = BM + PADMN;
-constexpr int GROUP_M = 12;  // raster group: a wave of 148 CTAs covers ~12 x 12 tiles (L2 reuse)
-
-constexpr size_t SMEM_MN = (size_t)STAGES * BK * (LDS_MN + LDS_MN) * sizeof(double);
-constexpr size_t SMEM_K = (size_t)STAGES * (BM + BN) * BK * sizeof(double);
-
-__device__ __forceinline__ void dmma(double &d0, double &d1, double a, double b) {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-                 : "+d"(d0), "+d"(d1)
-                 : "d"(a), "d"(b));
-}
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-// zero-filling async copies: bytes beyond src_bytes are written as 0 (tile edges, k tail)
-__device__ __forceinline__ void cp_async16(void *dst, const void *src, int src_bytes) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(smem_u32(dst)), "l"(src), "r"(src_bytes));
-}
-__device__ __forceinline__ void cp_async8(void *dst, const void *src, int src_bytes) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(smem_u32(dst)), "l"(src), "r"(src_bytes));
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
-
-// tile index -> (tm, tn) with grouped rasterisation
-__device__ __forceinline__ void raster(int pid, int tiles_m, int tiles_n, int &tm, int &tn) {
-    const int per_group = GROUP_M * tiles_n;
-    const int gid = pid / per_group;
-    const int first_m = gid * GROUP_M;
-    const int gsize = min(tiles_m - first_m, GROUP_M);
-    const int r = pid - gid * per_group;
-    tm = first_m + r % gsize;
-    tn = r / gsize;
-}
 
 // ---------------------------------------------------------------------------------------------
 // step 0: both operands MN-contiguous ("k-outer"): A[k][m] = L[P=k][a0 + m/v][m%v], B likewise.
@@ -321,9 +281,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_step1(const Step1Args p) {
 // Every R entry is touched exactly once per apply (tiles partition (a,b); the mirror covers the
 // other triangle), so beta scaling here is exact.
 // ---------------------------------------------------------------------------------------------
-struct RStrides {
-    int64_t i, j, a, b;  // element strides of R[i,j,a,b]
-};
 struct ReduceArgs {
     const double *part;  // [splitk][M][N]
     int splitk;
@@ -336,10 +293,6 @@ struct ReduceArgs {
     RStrides rs;
     double *R;
 };
-
-__device__ __forceinline__ void r_update(double *r, double val, double alpha, double beta) {
-    *r = (beta == 0.0) ? alpha * val : beta * (*r) + alpha * val;
-}
 
 __global__ void __launch_bounds__(256) k_reduce(const ReduceArgs p) {
     const int64_t MN = (int64_t)p.M * p.N;
@@ -386,7 +339,7 @@ struct FoldArgs {
     int64_t sc;          // stride of c
     int64_t s_row;       // mode 0: row r at r*s_row;  mode 2: row (a_l, b) at (a_l*v + b)*s_row
     int64_t s_i, s_j;    // mode 1: row (i,j) at i*s_i + j*s_j
-    int mode;            // 0: fold W tile rows (every row has + and -); 1: pack amplitudes, rows (i<=j) of an o x o grid;
+    int mode;            // 0: fold W tile rows (every row has + and -); 1: pack amplitudes, rows (i<=j) of an o x o grid; 3: see below;
                          // 2: PPL_SYM_FULL: rows r = a_l*tbp + b_l of the tile (A; b-group) taken from the slab's strip;
                          //    rows with a > b, b >= v or a_l >= ta are written as zeros; only c >= A0 is touched
     int rows;            // mode 0/2: number of rows; mode 1: o*o (rows with i > j are skipped)
@@ -396,8 +349,14 @@ struct FoldArgs {
     double scale;        // factor of the off-diagonal (c<d) entries: 1 (W) or 1/2 (tau)
     double diag;         // factor of the diagonal (c==d) entries of the + part: PPL_SYM_PAIR_SA 1 (W), 1 (tau);
                          // PPL_SYM_FULL 2 (W), 1/2 (tau) -- same products, but W+ becomes a symmetric matrix
-    int tbp, bg0, A0, ta;  // mode 2
-    int rows_per_a = 0, b_base = 0;  // mode 2: strip row of (a_l, b) is a_l * rows_per_a + b - b_base (v, 0: the slab's whole strip)
+    int tbp, bg0, A0, ta;  // mode 2 (A0, ta also mode 3)
+    int rows_per_a = 0, b_base = 0;  // mode 2/3: strip row of (a_l, b) is a_l * rows_per_a + b - b_base (v, 0: the slab's whole strip)
+    // mode 3: PPL_SYM_FULL with W+- rows = a run of the packed pair index of (a <= b): plus row r <-> kplus index kp0 + r
+    // (kp1: end of the run; rows up to the next multiple of 16 and the holes of the packed layout are written as zeros),
+    // the minus row of the same pair is kminus(a,b) - km0; rows [rows - nzm, rows) of the launch zero the minus rows
+    // zrows_m[.] (holes and the tail up to a multiple of 16), which no pair writes.
+    int kp0 = 0, kp1 = 0, km0 = 0, nzm = 0;
+    int zrows_m[24] = {};
     int cb_min;          // first FT-block of c that is processed (mode 2: A0 / FT; else 0)
     double *dp, *dm;     // packed outputs, row strides ldp / ldm
     int64_t ldp, ldm;
@@ -424,6 +383,27 @@ __device__ __forceinline__ FoldRow fold_row(const FoldArgs &p, int r) {
         f.zero = al >= p.ta || b >= p.v || a > b;
         f.roff = f.zero ? 0 : ((int64_t)al * p.rows_per_a + b - p.b_base) * p.s_row;
         f.rowp = f.rowm = r;
+    } else if (p.mode == 3) {
+        const int nplus = p.rows - p.nzm;
+        f.zero = true;
+        f.roff = 0;
+        f.rowp = f.rowm = -1;
+        if (r >= nplus) {  // a minus row no pair owns
+            f.rowm = p.zrows_m[r - nplus];
+        } else {
+            f.rowp = r;
+            const int64_t kap = (int64_t)p.kp0 + r;
+            if (kap < p.kp1) {
+                int a = p.A0 + p.ta - 1;
+                while (a > p.A0 && kplus(a, a, p.v) > kap) --a;
+                const int b = a + (int)(kap - kplus(a, a, p.v));
+                if (b < p.v) {  // b == v: the hole in front of the next triangle row
+                    f.zero = false;
+                    f.roff = ((int64_t)(a - p.A0) * p.rows_per_a + b - p.b_base) * p.s_row;
+                    f.rowm = a < b ? kminus(a, b, p.v) - p.km0 : -1;
+                }
+            }
+        }
     } else {
         const int i = r / p.o, j = r - i * p.o;
         f.skip = i > j;
@@ -448,7 +428,7 @@ __global__ void __launch_bounds__(256, 4) k_symfold(const FoldArgs p) {
     }
     const int db = cb + rem;
     const int c0 = cb * FT, d0 = db * FT;
-    const int cmin = p.mode == 2 ? p.A0 : 0;
+    const int cmin = (p.mode == 2 || p.mode == 3) ? p.A0 : 0;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;  // 32 x 8
     const bool offdiag = cb != db;
     double va[FT / 8], vb[FT / 8];
@@ -483,7 +463,7 @@ __global__ void __launch_bounds__(256, 4) k_symfold(const FoldArgs p) {
         }
         __syncthreads();
         if (now.skip) continue;
-        double *op = p.dp + now.rowp * p.ldp;
+        double *op = now.rowp >= 0 ? p.dp + now.rowp * p.ldp : nullptr;
         double *om = now.rowm >= 0 ? p.dm + now.rowm * p.ldm : nullptr;
 #pragma unroll
         for (int k = 0; k < FT / 8; ++k) {
@@ -492,10 +472,10 @@ __global__ void __launch_bounds__(256, 4) k_symfold(const FoldArgs p) {
             if (c >= p.v || d >= p.v || d < c || c < cmin) continue;
             const double xcd = sa[y][tx];
             if (c == d) {
-                op[kplus(c, d, p.v)] = p.diag * xcd;
+                if (op) op[kplus(c, d, p.v)] = p.diag * xcd;
             } else {
                 const double xdc = offdiag ? sb[tx][y] : sa[tx][y];
-                op[kplus(c, d, p.v)] = p.scale * (xcd + xdc);
+                if (op) op[kplus(c, d, p.v)] = p.scale * (xcd + xdc);
                 if (om) om[kminus(c, d, p.v)] = p.scale * (xcd - xdc);
             }
         }

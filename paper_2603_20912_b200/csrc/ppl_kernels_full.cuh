@@ -30,6 +30,35 @@ constexpr int TA_FULL = 16;  // a-block edge of PPL_SYM_FULL: one TMA box row of
 // Column tile tn: 8 boxes, box j <-> chunk 8 tn + j of the slab's chunk table: (b, d0) -> coordinate
 // b*v + d0 (16 d's of L[P][b][.]); b < 0 marks padding.  Chunks of one b start at its own 16-block.
 // ---------------------------------------------------------------------------------------------
+// Diagonal (b-block == d-block) 16 x 16 blocks of L, packed: only the pairs b_l <= d_l are needed there (the rest is their
+// b<->d image), 136 of 256.  k_pack_diag copies them once per apply into Lq[P][blk * 144 + t], t = the row-major index of
+// (b_l <= d_l) in the triangle (row b_l holds 16 - b_l entries; t = 136..143 are zero padding): 9 TMA chunks of 16 columns
+// per block instead of 16.  Chunk-table entry of a packed chunk: x = -2 - blk, y = its inner coordinate in Lq.
+constexpr int DIAG_PACKED = 144, DIAG_PAIRS = 136;
+__host__ __device__ __forceinline__ bool diag_unpack(int t, int &bl, int &dl) {
+    if (t >= DIAG_PAIRS) return false;
+    bl = 0;
+    int off = 0;
+    while (t - off >= 16 - bl) {
+        off += 16 - bl;
+        ++bl;
+    }
+    dl = bl + (t - off);
+    return true;
+}
+__global__ void __launch_bounds__(256) k_pack_diag(const double *__restrict__ L, double *__restrict__ Lq, int x, int v, int nfull,
+                                                  int64_t ldq) {
+    const int64_t per_p = (int64_t)nfull * DIAG_PACKED, total = (int64_t)x * per_p;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t P = idx / per_p;
+        const int r = (int)(idx - P * per_p), blk = r / DIAG_PACKED, t = r - blk * DIAG_PACKED;
+        int bl, dl;
+        double val = 0.0;
+        if (diag_unpack(t, bl, dl)) val = __ldg(L + (P * v + 16 * blk + bl) * v + 16 * blk + dl);
+        Lq[P * ldq + r] = val;
+    }
+}
+
 struct Step0SlabArgs {
     int A0, ta;          // first a of the slab, number of a's (16 except in the last slab)
     int v, K;            // nvirt, nchol
@@ -42,7 +71,8 @@ struct Step0SlabArgs {
                          // every b >= A0 must be in the strip); 0: the chunks cover the full (b, d) rectangle of the group
 };
 
-__global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_slab(const __grid_constant__ CUtensorMap mapL, const Step0SlabArgs p) {
+__global__ void __launch_bounds__(TMA_THREADS, 1)
+    k_step0_slab(const __grid_constant__ CUtensorMap mapL, const __grid_constant__ CUtensorMap mapQ, const Step0SlabArgs p) {
     extern __shared__ unsigned char smem_raw[];
     const TmaSmem sm = carve_smem(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -56,18 +86,21 @@ __global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_slab(const __grid_cons
         setmaxnreg_dec<PRODUCER_REGS>();
         if (warp == CONSUMER_WARPS && lane == 0) {
             prefetch_tmap(&mapL);
+            prefetch_tmap(&mapQ);
             int stage = 0;
             uint32_t phase = 0;
             for (int item = blockIdx.x; item < num_items; item += gridDim.x) {
                 int tm, tn;
                 raster(item, p.tiles_m, p.tiles_n, tm, tn);
                 int xa[8], xb[8];
+                unsigned packed = 0;  // bit i: chunk i of the column tile comes from the packed diagonal blocks (mapQ)
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
                     const int c = p.A0 + 8 * tm + i;
                     xa[i] = c < v ? c * v + p.A0 : vv;  // beyond the tensor: the box is zero-filled
                     const int2 ch = p.chunks[8 * tn + i];
-                    xb[i] = ch.x >= 0 ? ch.x * v + ch.y : vv;
+                    xb[i] = ch.x >= 0 ? ch.x * v + ch.y : (ch.x == -1 ? vv : ch.y);
+                    packed |= (ch.x <= -2 ? 1u : 0u) << i;
                 }
                 for (int kt = 0; kt < nkt; ++kt) {
                     mbar_wait(&sm.empty[stage], phase ^ 1);
@@ -76,7 +109,8 @@ __global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_slab(const __grid_cons
 #pragma unroll
                     for (int i = 0; i < 8; ++i) tma_load_2d(da + i * BK * 16, &mapL, xa[i], kt * BK, &sm.full[stage]);
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) tma_load_2d(db + i * BK * 16, &mapL, xb[i], kt * BK, &sm.full[stage]);
+                    for (int i = 0; i < 8; ++i)
+                        tma_load_2d(db + i * BK * 16, ((packed >> i) & 1) ? &mapQ : &mapL, xb[i], kt * BK, &sm.full[stage]);
                     if (++stage == TSTAGES) {
                         stage = 0;
                         phase ^= 1;
@@ -152,7 +186,22 @@ __global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_slab(const __grid_cons
 #pragma unroll
                 for (int j = 0; j < 2; ++j) {
                     const int b = ch[j].x, d0 = ch[j].y;
-                    if (b < 0) continue;
+                    if (b == -1) continue;
+                    if (b <= -2) {  // packed diagonal block: column t of the triangle -> (b_l <= d_l), plus the b<->d image
+                        const int blk = -2 - b, t0 = d0 - blk * DIAG_PACKED + 2 * q;
+#pragma unroll
+                        for (int h = 0; h < 2; ++h)
+#pragma unroll
+                            for (int f = 0; f < 2; ++f) {
+                                int bl, dl;
+                                if (!diag_unpack(t0 + 8 * h + f, bl, dl)) continue;
+                                const double val = acc[2 * i + e][2 * j + f][h];
+                                const int bb = 16 * blk + bl, dd = 16 * blk + dl;
+                                xa[(int64_t)bb * vv + dd] = val;
+                                if (bl != dl) xa[(int64_t)dd * vv + bb] = val;
+                            }
+                        continue;
+                    }
                     const bool offdiag = p.image && d0 != p.A0 + ((b - p.A0) & ~15);  // d-block above the b-block: store the b<->d image too
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
@@ -200,6 +249,8 @@ __global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_slab(const __grid_cons
 // ---------------------------------------------------------------------------------------------
 struct Step1TArgs {
     int M;
+    int range;           // 1: the W rows are a run of the packed pair index: k-tile kt <-> tau columns kap0 + 16 kt (kt_per_a, A0, bg0 unused)
+    int kap0;
     int n_base;          // n_begin rounded down to a multiple of 16: the column of tile 0
     int n_begin, n_end;
     int nkt, kt_per_a;
@@ -291,8 +342,13 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
                 int row0, ni0, ni1;
                 m_tile(p.ms, tm, row0, ni0, ni1);
                 for (int kt = 0; kt < p.nkt; ++kt) {
-                    const int a = p.A0 + kt / p.kt_per_a, b1 = p.bg0 + 16 * (kt % p.kt_per_a);
-                    const int64_t kap = p.minus ? kminus(a, b1, p.v) : kplus(a, b1, p.v);  // even: b1 is a multiple of 16
+                    int64_t kap;
+                    if (p.range) {
+                        kap = (int64_t)p.kap0 + 16 * kt;  // even: the run starts at an even index
+                    } else {
+                        const int a = p.A0 + kt / p.kt_per_a, b1 = p.bg0 + 16 * (kt % p.kt_per_a);
+                        kap = p.minus ? kminus(a, b1, p.v) : kplus(a, b1, p.v);  // even: b1 is a multiple of 16
+                    }
                     mbar_wait(&sm.empty[stage], phase ^ 1);
                     mbar_expect_tx(&sm.full[stage], Cfg::STAGE);
                     tma_load_2d(sm.a + (size_t)stage * BM1 * BK, &mapA, (int)kap, row0, &sm.full[stage]);
@@ -388,6 +444,25 @@ __global__ void __launch_bounds__(256) k_reduce_acc(const ReduceAccArgs p) {
         for (int z = 0; z < p.splitk; ++z) s += p.part[(int64_t)z * MN + idx];
         const int64_t k = p.minus ? kminus(a, b, p.v) : kplus(a, b, p.v);
         p.acc[(int64_t)m * p.ld + k] += s;
+    }
+}
+
+// the same for W+- rows that are a run of the packed pair index: Racc[m][k0 + n] += sum_z part[z][m][n] (holes of the
+// packed layout are rows of zeros in W+-, so they receive += 0)
+struct ReduceRangeArgs {
+    const double *part;  // [splitk][M][N]
+    int splitk, M, N;
+    int k0;
+    double *acc;
+    int64_t ld;
+};
+__global__ void __launch_bounds__(256) k_reduce_range(const ReduceRangeArgs p) {
+    const int64_t MN = (int64_t)p.M * p.N;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < MN; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int m = (int)(idx / p.N), n = (int)(idx - (int64_t)m * p.N);
+        double s = 0.0;
+        for (int z = 0; z < p.splitk; ++z) s += p.part[(int64_t)z * MN + idx];
+        p.acc[(int64_t)m * p.ld + p.k0 + n] += s;
     }
 }
 

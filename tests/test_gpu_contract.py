@@ -1,0 +1,139 @@
+"""-m gpu: ppl_contract_pair -- the generic pair contraction 'op0,op1->out' --
+against oracle.contract_pair (the einsum definition, pinned in tests/test_oracle_contract_pins.py) on the same seeded
+inputs.  Tolerance as everywhere: max|dC| <= 1e-11 max|C|; exact-integer inputs bit for bit."""
+import numpy as np
+import pytest
+
+import oracle
+import paper_2603_20912_b200 as P
+import ppl_inputs as I
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-11
+
+
+def _rand(shape, seed, integer=False):
+    return I.make_vec(int(np.prod(shape)), seed, 60, integer=integer).reshape(shape)
+
+
+def gpu_contract(subs, A, B, C0=None, alpha=1.0, beta=0.0, offset=0, workspace_bytes=None):
+    """offset: element offset of the device buffers from their allocation (8-byte aligned only when odd)."""
+    import torch
+
+    def dev(a):
+        flat = torch.empty(a.size + offset, dtype=torch.float64, device="cuda")
+        view = flat[offset:].view(a.shape)
+        view.copy_(torch.from_numpy(a))
+        return view
+
+    Ad, Bd = dev(A), dev(B)
+    Cd = None if C0 is None else dev(C0)
+    ws = None if workspace_bytes is None else torch.empty(workspace_bytes + 256, dtype=torch.uint8, device="cuda")
+    out = P.ppl_contract_pair(subs, Ad, Bd, Cd, alpha=alpha, beta=beta, workspace=ws)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def relerr(got, want):
+    m = np.abs(want).max()
+    return float(np.abs(got - want).max() / (m if m > 0 else 1.0))
+
+
+CASES = [
+    # the paper's two ladder steps, several CTA tiles with ragged edges; even and odd extents
+    ("xac,xbd->acbd", (37, 9, 30), (37, 11, 26)),
+    ("xac,xbd->acbd", (20, 7, 19), (20, 5, 19)),
+    ("abcd,ecfd->efab", (6, 7, 20, 22), (5, 20, 5, 22)),
+    ("abcd,efcd->efab", (12, 13, 9, 10), (4, 6, 9, 10)),
+    ("acbd,efcd->efab", (5, 11, 6, 13), (3, 4, 11, 13)),
+    # a Cholesky factor against an amplitude; summed letter in the middle of op1
+    ("xac,icjd->xajd", (9, 8, 14), (6, 14, 7, 10)),
+    # plain matrix products in all four storage combinations (unit-stride letter summed or surviving, per operand)
+    ("ik,kj->ij", (150, 70), (70, 140)),
+    ("ki,kj->ij", (70, 150), (70, 140)),
+    ("ik,jk->ij", (150, 70), (140, 70)),
+    ("ki,jk->ij", (70, 150), (140, 70)),
+    ("ik,jk->ji", (131, 33), (67, 33)),
+    # degenerate: outer product (nothing summed), full inner product (nothing survives), matrix-vector
+    ("i,j->ji", (300,), (5,)),
+    ("abc,abc->", (6, 10, 8), (6, 10, 8)),
+    ("abcd,cd->ab", (9, 10, 12, 14), (12, 14)),
+    ("abc,dcb->ad", (130, 6, 8), (129, 8, 6)),
+    ("xab,xcd->dbca", (10, 12, 6), (10, 9, 14)),
+    # few tiles, long contraction: split-K with the fixed-order reduction
+    ("ik,jk->ij", (40, 6000), (30, 6000)),
+    ("ki,kj->ij", (5001, 40), (5001, 30)),
+]
+
+
+@pytest.mark.parametrize("subs,sa,sb", CASES)
+def test_parity_with_the_oracle(subs, sa, sb):
+    A, B = _rand(sa, 1), _rand(sb, 2)
+    want = oracle.contract_pair(subs, A, B)
+    assert relerr(gpu_contract(subs, A, B), want) <= TOL
+    # buffers that are only 8-byte aligned take the 8-byte copy path
+    assert relerr(gpu_contract(subs, A, B, offset=1), want) <= TOL
+
+
+@pytest.mark.parametrize("subs,sa,sb", CASES[:8] + CASES[-2:])
+def test_exact_integers_bit_for_bit(subs, sa, sb):
+    A, B = _rand(sa, 3, integer=True), _rand(sb, 4, integer=True)
+    want = oracle.contract_pair(subs, A, B)
+    for rep in range(2):
+        assert np.array_equal(gpu_contract(subs, A, B), want), rep
+
+
+def test_alpha_beta_and_overwrite():
+    subs, sa, sb = "xac,xbd->acbd", (21, 6, 17), (21, 5, 18)
+    A, B = _rand(sa, 5), _rand(sb, 6)
+    C0 = _rand((6, 17, 5, 18), 7)
+    want = oracle.contract_pair(subs, A, B, C0.copy(), alpha=-0.75, beta=0.5)
+    assert relerr(gpu_contract(subs, A, B, C0.copy(), alpha=-0.75, beta=0.5), want) <= TOL
+    nan = np.full(C0.shape, np.nan)
+    assert relerr(gpu_contract(subs, A, B, nan, alpha=1.0, beta=0.0), oracle.contract_pair(subs, A, B)) <= TOL
+    # split-K path
+    A, B = _rand((24, 4000), 8), _rand((17, 4000), 9)
+    C0 = _rand((24, 17), 10)
+    want = oracle.contract_pair("ik,jk->ij", A, B, C0.copy(), alpha=2.0, beta=-1.0)
+    assert relerr(gpu_contract("ik,jk->ij", A, B, C0.copy(), alpha=2.0, beta=-1.0), want) <= TOL
+
+
+def test_two_pair_contractions_are_the_ladder():
+    """PAPER.md:118-120 through the generic entry point: 'xac,xbd->acbd' then 'acbd,efcd->efab' == oracle.full."""
+    import torch
+
+    o, v, x = 4, 22, 30
+    L = I.make_L(v, x, 11, symmetric=False)
+    t2 = I.make_t2(o, v, 11, symmetric=False)
+    Ld, td = torch.from_numpy(L).cuda(), torch.from_numpy(t2).cuda()
+    W = P.ppl_contract_pair("xac,xbd->acbd", Ld, Ld)
+    R = P.ppl_contract_pair("acbd,efcd->efab", W, td)
+    torch.cuda.synchronize()
+    assert relerr(R.cpu().numpy(), oracle.full(L, t2)) <= TOL
+    # and equals ppl_apply in the mode that assumes nothing
+    Rd = torch.zeros((o, o, v, v), dtype=torch.float64, device="cuda")
+    with P.Plan(o, v, x) as plan:
+        plan.set_symmetry(P.PPL_SYM_NONE)
+        plan.apply(Ld, td, Rd)
+        torch.cuda.synchronize()
+    assert relerr(R.cpu().numpy(), Rd.cpu().numpy()) <= TOL
+
+
+def test_workspace_rules_and_malformed_requests():
+    import torch
+
+    A, B = _rand((24, 4000), 12), _rand((17, 4000), 13)
+    want = oracle.contract_pair("ik,jk->ij", A, B)
+    tables = 8 * (2 * 24 + 2 * 17 + 2 * 4000)
+    tables = (tables + 255) // 256 * 256
+    # with room for the tables only the call runs without split-K; same result within rounding
+    assert relerr(gpu_contract("ik,jk->ij", A, B, workspace_bytes=tables), want) <= TOL
+    with pytest.raises(P.PplError) as e:
+        gpu_contract("ik,jk->ij", A, B, workspace_bytes=tables - 256)
+    assert e.value.code == P.PPL_ERR_WORKSPACE_TOO_SMALL
+    Ad, Bd = torch.zeros((3, 3), dtype=torch.float64, device="cuda"), torch.zeros((3, 3), dtype=torch.float64, device="cuda")
+    for bad in ("ab,bc", "aa,ab->b", "ab,bc,cd->ad", "ab,bc->abc", "ab,ab->ab", "ab,cd->ac"):
+        with pytest.raises((P.PplError, KeyError, ValueError)):
+            P.ppl_contract_pair(bad, Ad, Bd)
+    with pytest.raises(P.PplError):  # extents of a shared letter disagree
+        P.ppl_contract_pair("ab,bc->ac", Ad, torch.zeros((4, 3), dtype=torch.float64, device="cuda"))

@@ -3,8 +3,6 @@ restricted to d-block >= b-block; include/ppl.h) against the CPU oracle.  The mo
 pair-symmetric t2; odd nvirt runs in the geometry of nvirt + 1 with a zero pad index (L copied into 16-byte aligned
 rows for TMA).  Same tolerance as everywhere (1e-11 relative, exact integers bit
 for bit).  The identity behind it is pinned on the CPU (test_oracle_pins.py::test_full_symmetry_hook_identity)."""
-import os
-
 import numpy as np
 import pytest
 
@@ -23,25 +21,22 @@ SHAPES = [(1, 2, 1), (2, 16, 4), (12, 18, 9), (3, 24, 17), (5, 20, 60), (3, 40, 
           (2, 3, 2), (3, 15, 7), (4, 17, 9), (5, 31, 12), (3, 33, 20), (5, 53, 232), (7, 97, 30), (2, 129, 16), (1, 5, 1)]
 
 
-@pytest.fixture
-def tbg_env():
-    old = os.environ.get("PPL_TBG")
-    yield lambda val: os.environ.__setitem__("PPL_TBG", str(val))
-    if old is None:
-        os.environ.pop("PPL_TBG", None)
-    else:
-        os.environ["PPL_TBG"] = old
+# the two forms of the W+- tiles and of the diagonal d-blocks of step 0 (include/ppl.h, ppl_debug_opts_t): the product's
+# (runs of the packed pair index; 9 packed chunks per diagonal block) and the round-1 form (rectangular tiles with zero
+# rows; 16 plain chunks), which the memory-tight form still uses
+FORMS = {"range+packed": {}, "rect+plain": {"full_rect_tiles": 1, "full_no_diag_pack": 1},
+         "range+plain": {"full_no_diag_pack": 1}, "rect+packed": {"full_rect_tiles": 1}}
 
 
 @pytest.mark.parametrize("shape", SHAPES)
 @pytest.mark.parametrize("tbg", [128, 32, 16])
-def test_full_mode_parity(shape, tbg, tbg_env):
+@pytest.mark.parametrize("form", ["range+packed", "rect+plain"])
+def test_full_mode_parity(shape, tbg, form):
     o, v, x = shape
-    tbg_env(tbg)
     L = I.make_L(v, x, seed=21, symmetric=True)
     t2 = I.make_t2(o, v, seed=21, symmetric=True)
     want = oracle.full(L, t2)
-    got, info = gpu_ladder(L, t2, sym=P.PPL_SYM_FULL, return_info=True)
+    got, info = gpu_ladder(L, t2, sym=P.PPL_SYM_FULL, return_info=True, debug=dict(FORMS[form], full_tbg=tbg))
     assert info["symmetry"] == P.PPL_SYM_FULL and info["full_available"] == 1
     assert info["full_tbg"] == min(tbg, (v + 15) // 16 * 16)
     assert relerr(got, want) <= TOL, info
@@ -50,14 +45,14 @@ def test_full_mode_parity(shape, tbg, tbg_env):
 @pytest.mark.parametrize("shape", [(5, 20, 60), (4, 38, 19), (12, 18, 9), (24, 64, 128), (7, 82, 33), (3, 130, 12), (9, 100, 24),
                                    (4, 37, 19), (6, 81, 33), (3, 113, 12), (5, 53, 40)])
 @pytest.mark.parametrize("tbg", [128, 16])
-def test_full_mode_exact_integers_bit_for_bit(shape, tbg, tbg_env):
+@pytest.mark.parametrize("form", sorted(FORMS))
+def test_full_mode_exact_integers_bit_for_bit(shape, tbg, form):
     o, v, x = shape
-    tbg_env(tbg)
     L = I.make_L(v, x, 41, symmetric=True, integer=True)
     t2 = 2.0 * I.make_t2(o, v, 41, symmetric=True, integer=True)  # tau+- (and t2[cc]/2) stay exact integers
     want = oracle.full(L, t2)
-    for rep in range(3):
-        got = gpu_ladder(L, t2, sym=P.PPL_SYM_FULL)
+    for rep in range(2):
+        got = gpu_ladder(L, t2, sym=P.PPL_SYM_FULL, debug=dict(FORMS[form], full_tbg=tbg))
         assert np.array_equal(got, want), rep
 
 
@@ -158,29 +153,18 @@ def test_full_mode_repeated_apply_and_stream_ordering():
     assert np.array_equal(Rd.cpu().numpy(), 1.5 * want)
 
 
-@pytest.fixture
-def chunk_env():
-    old = os.environ.get("PPL_HOST_CHUNK_MB")
-    yield lambda val: os.environ.__setitem__("PPL_HOST_CHUNK_MB", str(val))
-    if old is None:
-        os.environ.pop("PPL_HOST_CHUNK_MB", None)
-    else:
-        os.environ["PPL_HOST_CHUNK_MB"] = old
-
-
 @pytest.mark.parametrize("shape,chunk_mb", [((6, 96, 40), 1), ((9, 100, 24), 1), ((5, 130, 20), 1), ((4, 98, 30), 1024),
                                             ((6, 97, 40), 1), ((5, 131, 20), 1)])
-def test_host_entry_point_streams_t2_and_R_in_chunks(shape, chunk_mb, chunk_env):
+def test_host_entry_point_streams_t2_and_R_in_chunks(shape, chunk_mb):
     """ppl_apply_host in PPL_SYM_FULL: t2 and R never sit on the device whole; they pass through
     two staging buffers of `chunk_mb` (several chunks, ragged last one, odd chunk counts) and R accumulates (+=)."""
     o, v, x = shape
-    chunk_env(chunk_mb)
     L = I.make_L(v, x, seed=61, symmetric=True)
     t2 = I.make_t2(o, v, seed=61, symmetric=True)
     R0 = I.make_vec(o * o * v * v, 61, 40).reshape(o, o, v, v)
     want = oracle.full(L, t2)
     R = R0.copy()
-    with P.Plan(o, v, x) as plan:
+    with P.Plan(o, v, x, debug=dict(host_chunk_mb=chunk_mb)) as plan:
         assert plan.info()["symmetry"] == P.PPL_SYM_FULL
         for rep in range(2):  # the staging buffers are reused; the second call adds the term again
             h2d, d2h = plan.apply_host(L, t2, R)
@@ -188,13 +172,12 @@ def test_host_entry_point_streams_t2_and_R_in_chunks(shape, chunk_mb, chunk_env)
             assert relerr(R - R0, (rep + 1) * want) <= TOL, rep
 
 
-def test_host_entry_point_exact_integers_chunked(chunk_env):
+def test_host_entry_point_exact_integers_chunked():
     o, v, x = 7, 98, 12
-    chunk_env(1)
     L = I.make_L(v, x, 43, symmetric=True, integer=True)
     t2 = 2.0 * I.make_t2(o, v, 43, symmetric=True, integer=True)
     R = np.zeros((o, o, v, v))
-    with P.Plan(o, v, x) as plan:
+    with P.Plan(o, v, x, debug=dict(host_chunk_mb=1)) as plan:
         plan.apply_host(L, t2, R)
     assert np.array_equal(R, oracle.full(L, t2))
 
@@ -211,65 +194,46 @@ def test_one_and_two_strips_agree_bit_for_bit(shape):
     want = oracle.full(L, t2)
     Ld, td = torch.from_numpy(L).cuda(), torch.from_numpy(t2).cuda()
     got = {}
-    old = os.environ.get("PPL_FULL_STRIPS")
-    try:
-        for strips in ("1", "2"):
-            os.environ["PPL_FULL_STRIPS"] = strips
-            with P.Plan(o, v, x, 0) as plan:
-                plan.set_symmetry(P.PPL_SYM_FULL)
-                plan.set_graph(0)
-                Rd = torch.zeros((o, o, v, v), dtype=torch.float64, device="cuda")
-                for _ in range(2):  # twice: events and strips are reused across applies
-                    plan.apply(Ld, td, Rd)
-                torch.cuda.synchronize()
-                got[strips] = (Rd.cpu().numpy(), plan.info()["workspace_bytes"])
-    finally:
-        if old is None:
-            os.environ.pop("PPL_FULL_STRIPS", None)
-        else:
-            os.environ["PPL_FULL_STRIPS"] = old
+    for strips in ("1", "2"):
+        with P.Plan(o, v, x, 0, debug=dict(full_strips=int(strips))) as plan:
+            plan.set_symmetry(P.PPL_SYM_FULL)
+            plan.set_graph(0)
+            Rd = torch.zeros((o, o, v, v), dtype=torch.float64, device="cuda")
+            for _ in range(2):  # twice: events and strips are reused across applies
+                plan.apply(Ld, td, Rd)
+            torch.cuda.synchronize()
+            got[strips] = (Rd.cpu().numpy(), plan.info()["workspace_bytes"])
     assert got["2"][1] > got["1"][1]  # the second strip was really allocated
     assert np.abs(got["2"][0] - 2.0 * want).max() <= 1e-11 * np.abs(2.0 * want).max()
     assert np.array_equal(got["1"][0], got["2"][0])
 
 
-@pytest.fixture
-def tight_env():
-    old = {k: os.environ.get(k) for k in ("PPL_FULL_TIGHT", "PPL_TBG", "PPL_FULL_STRIPS")}
-    yield lambda **kw: [os.environ.__setitem__(k, str(val)) for k, val in kw.items()]
-    for k, val in old.items():
-        if val is None:
-            os.environ.pop(k, None)
-        else:
-            os.environ[k] = val
-
-
 @pytest.mark.parametrize("shape", [(1, 2, 1), (2, 16, 4), (12, 18, 9), (5, 20, 60), (3, 40, 33), (6, 50, 70), (5, 53, 40), (4, 98, 30), (7, 130, 20)])
 @pytest.mark.parametrize("tbg,strips", [(16, 2), (32, 1), (256, 2)])
-def test_memory_tight_mode_parity(shape, tbg, strips, tight_env):
+def test_memory_tight_mode_parity(shape, tbg, strips):
     """PPL_SYM_FULL with a strip of one (slab; b-group) tile: step 0 per tile on the full (b, d) rectangle (no image),
-    the fold and the GEMMs unchanged.  Forced here (PPL_FULL_TIGHT=1); taken by the planner when 16 v^3 does not fit."""
+    the fold and the GEMMs unchanged.  Forced here (debug option full_tight); taken by the planner when 16 v^3 does not fit."""
     o, v, x = shape
-    tight_env(PPL_FULL_TIGHT=1, PPL_TBG=tbg, PPL_FULL_STRIPS=strips)
     L = I.make_L(v, x, 81, symmetric=True)
     t2 = I.make_t2(o, v, 81, symmetric=True)
     R0 = I.make_vec(o * o * v * v, 82, 40).reshape(o, o, v, v)
     want = oracle.full(L, t2, R0.copy())
-    got, info = gpu_ladder(L, t2, R0=R0.copy(), sym=P.PPL_SYM_FULL, return_info=True)
+    got, info = gpu_ladder(L, t2, R0=R0.copy(), sym=P.PPL_SYM_FULL, return_info=True,
+                           debug=dict(full_tight=1, full_tbg=tbg, full_strips=strips))
     assert info["full_tight"] == 1 and info["symmetry"] == P.PPL_SYM_FULL, info
     assert relerr(got, want) <= 1e-11, info
 
 
 @pytest.mark.parametrize("shape", [(5, 20, 60), (4, 38, 19), (24, 64, 128), (7, 82, 33), (3, 130, 12), (5, 53, 40)])
-def test_memory_tight_mode_exact_integers_and_flops(shape, tight_env):
+def test_memory_tight_mode_exact_integers_and_flops(shape):
     o, v, x = shape
     L = I.make_L(v, x, 83, symmetric=True, integer=True)
     t2 = 2.0 * I.make_t2(o, v, 83, symmetric=True, integer=True)
     want = oracle.full(L, t2)
-    tight_env(PPL_FULL_TIGHT=0, PPL_TBG=32)
-    ref, info_ref = gpu_ladder(L, t2, sym=P.PPL_SYM_FULL, return_info=True)
-    tight_env(PPL_FULL_TIGHT=1, PPL_TBG=32)
-    got, info = gpu_ladder(L, t2, sym=P.PPL_SYM_FULL, return_info=True)
+    # the reference in the round-1 form (rectangular tiles, plain diagonal chunks): the tight form shares its step 1
+    ref, info_ref = gpu_ladder(L, t2, sym=P.PPL_SYM_FULL, return_info=True,
+                               debug=dict(full_tbg=32, full_rect_tiles=1, full_no_diag_pack=1))
+    got, info = gpu_ladder(L, t2, sym=P.PPL_SYM_FULL, return_info=True, debug=dict(full_tight=1, full_tbg=32))
     assert info["full_tight"] == 1 and info_ref["full_tight"] == 0
     assert np.array_equal(got, want) and np.array_equal(ref, want)
     # same step 1; step 0 on the full rectangle: more than the image mode, at most about twice it
@@ -280,7 +244,7 @@ def test_memory_tight_mode_exact_integers_and_flops(shape, tight_env):
     assert info["full_workspace_bytes"] < info_ref["full_workspace_bytes"] or v <= 32
 
 
-def test_memory_tight_mode_is_what_a_small_cap_gets(tight_env):
+def test_memory_tight_mode_is_what_a_small_cap_gets():
     """Under a cap that has no room for the 16 v^3 strip the planner keeps the 8-fold path in its memory-tight form."""
     import torch
 
@@ -306,17 +270,15 @@ def test_memory_tight_mode_is_what_a_small_cap_gets(tight_env):
 
 
 @pytest.mark.parametrize("shape", [(6, 96, 40), (5, 131, 20), (7, 98, 12)])
-def test_host_entry_point_in_the_memory_tight_form(shape, chunk_env, tight_env):
+def test_host_entry_point_in_the_memory_tight_form(shape):
     """ppl_apply_host (t2 and R streamed in chunks) on a plan whose PPL_SYM_FULL buffers are the one-tile-strip kind."""
     o, v, x = shape
-    chunk_env(1)
-    tight_env(PPL_FULL_TIGHT=1, PPL_TBG=32)
     L = I.make_L(v, x, 91, symmetric=True, integer=True)
     t2 = 2.0 * I.make_t2(o, v, 91, symmetric=True, integer=True)
     R0 = I.make_vec(o * o * v * v, 92, 40, integer=True).reshape(o, o, v, v)
     want = oracle.full(L, t2, R0.copy())
     R = R0.copy()
-    with P.Plan(o, v, x) as plan:
+    with P.Plan(o, v, x, debug=dict(host_chunk_mb=1, full_tight=1, full_tbg=32)) as plan:
         info = plan.info()
         assert info["symmetry"] == P.PPL_SYM_FULL and info["full_tight"] == 1
         plan.apply_host(L, t2, R)

@@ -63,6 +63,94 @@ def test_packed_geometry_and_pair_sa_accounting(shape):
         assert d[key] % 16 == 0 and 16 <= d[key] <= 160  # CTA tile rows 16*NI, NI = 1..10
 
 
+def kplus(c, d, v):
+    """Packed index of the pair (c <= d): restated from DESIGN.md 6.1 (row c starts so that the index has the parity of d)."""
+    return c * v - c * (c + 1) // 2 + (c + 1) // 2 + d
+
+
+def kminus(c, d, v):
+    return c * (2 * v - c - 1) // 2 - c + c // 2 + d
+
+
+def full_mode_flops_from_the_grid(o, v, x, tbg=256, rect=False, plain_diag=False):
+    """PPL_SYM_FULL's executed flops recomputed from the tile grid as DESIGN.md 6.2 describes it (even nvirt):
+    step 0: per slab of 16 a's a GEMM of (8 c x 16 a_l = 128)-row tiles x (8 chunks of 16 d = 128)-column tiles over nchol;
+    step 1: per W+- tile use 1 (rows of tau x tile rows x packed columns J >= (A0, A0)) and use 2 (rows of tau x packed
+    columns J >= (A0 + 16, A0 + 16) x tile rows), counted as the CTA tiles run them (rows in 8s, columns in 128s, k in 16s)."""
+    Mp, Mm = o * (o + 1) // 2, o * (o - 1) // 2
+    Kp, Km = kplus(v - 1, v - 1, v) + 1, (kminus(v - 2, v - 1, v) + 1 if v >= 2 else 0)
+    up = lambda a, b: (a + b - 1) // b * b
+    gemm = lambda M, ncols, kr: 0 if min(M, ncols, kr) <= 0 else 2.0 * up(M, 8) * up(ncols, 128) * up(kr, 16)
+    f0 = f1 = 0.0
+    for A0 in range(0, v, 16):
+        r, ta = v - A0, min(16, v - A0)
+        dL = A0 + (v - 1 - A0) // 16 * 16
+        w = v - dL
+        reverse = w < 16 and w * ((r + 15) // 16) < r
+        chunks = 0
+        for d0 in range(A0, v, 16):
+            if reverse and d0 == dL:
+                break
+            packed = (not plain_diag) and v >= 16 and d0 + 16 <= v
+            chunks += (d0 if packed else min(d0 + 16, v)) - A0
+        if reverse:
+            chunks += w * ((dL - A0) // 16 + 1)
+        if not plain_diag and v >= 16:
+            chunks += 9 * len([d0 for d0 in range(A0, v, 16) if d0 + 16 <= v])
+        f0 += 2.0 * x * (128 * ((r + 7) // 8)) * (128 * ((chunks + 7) // 8))
+        c1 = min(A0 + 16, v)
+        k0p, k0m = kplus(A0, A0, v), (kminus(A0, A0 + 1, v) - 1 if A0 + 1 < v else Km)
+        k1p, k1m = (kplus(c1, c1, v) if c1 < v else Kp), (kminus(c1, c1 + 1, v) - 1 if c1 + 1 < v else Km)
+        tiles = []  # (use-1 rows +, -, use-2 rows +, -)
+        if rect:
+            nblk, per = (r + 15) // 16, tbg // 16
+            ng = (nblk + per - 1) // per
+            for gi in range(ng):
+                N = 16 * 16 * (nblk // ng + (1 if gi < nblk % ng else 0))
+                tiles.append((N, N, N, N))
+        else:
+            lo, hi = k0p, kplus(A0 + ta - 1, v - 1, v) + 1
+            NT = 16 * tbg
+            ng = (hi - lo + NT - 1) // NT
+            chunk = min(NT, up((hi - lo + ng - 1) // ng, 128))
+            for kp0 in range(lo, hi, chunk):
+                np_ = min(kp0 + chunk, hi) - kp0
+                ms = [kminus(a, b, v) for a in range(A0, A0 + ta) for b in range(a + 1, v) if kp0 <= kplus(a, b, v) < kp0 + np_]
+                nm = (max(ms) + 1 - (min(ms) & ~1)) if ms else 0
+                tiles.append((np_, nm, up(np_, 16), up(nm, 16)))
+        for (n1p, n1m, n2p, n2m) in tiles:
+            f1 += gemm(Mp, n1p, Kp - k0p) + gemm(Mm, n1m, Km - k0m)
+            f1 += gemm(Mp, Kp - (k1p & ~15), n2p) + gemm(Mm, Km - (k1m & ~15), n2m)
+    return f0, f1
+
+
+@pytest.mark.parametrize("name", ["medium", "large", "xl"])
+@pytest.mark.parametrize("form", [{}, {"full_rect_tiles": 1, "full_no_diag_pack": 1}, {"full_no_diag_pack": 1}, {"full_rect_tiles": 1}])
+def test_full_mode_executed_and_useful_flops_recomputed_from_the_tile_grid(name, form):
+    o, v, x = CONFIGS[name]
+    d = P.ppl_plan_dry(o, v, x, debug=form)
+    f0, f1 = full_mode_flops_from_the_grid(o, v, x, tbg=d["full_tbg"], rect=bool(form.get("full_rect_tiles")),
+                                           plain_diag=bool(form.get("full_no_diag_pack")))
+    assert d["flops_step0"] == pytest.approx(f0, rel=1e-12)
+    assert d["flops_step1"] == pytest.approx(f1, rel=1e-12)
+    # useful: the unique (ac|bd) of the 8-fold symmetry, and the whole symmetric S+- applied once (include/ppl.h)
+    P2, Q2, Mp, Mm = v * (v + 1) // 2, v * (v - 1) // 2, o * (o + 1) // 2, o * (o - 1) // 2
+    assert d["flops_useful_step0"] == pytest.approx(2.0 * x * P2 * (P2 + 1) / 2, rel=1e-12)
+    assert d["flops_useful_step1"] == pytest.approx(2.0 * (Mp * P2 * P2 + Mm * Q2 * Q2), rel=1e-12)
+    assert d["flops_useful"] == d["flops_useful_step0"] + d["flops_useful_step1"] <= d["flops_executed"]
+
+
+def test_executed_over_useful_targets():
+    """launched / useful flops of the default mode.  Round 1: 1.064 / 1.059 / 1.255."""
+    ratio = {}
+    for name in ("large", "xl", "medium"):
+        d = P.ppl_plan_dry(*CONFIGS[name])
+        ratio[name] = d["flops_executed"] / d["flops_useful"]
+    assert ratio["xl"] <= 1.03 and ratio["large"] <= 1.045 and ratio["medium"] <= 1.12, ratio
+    old = P.ppl_plan_dry(*CONFIGS["medium"], debug={"full_rect_tiles": 1, "full_no_diag_pack": 1})
+    assert old["flops_executed"] / old["flops_useful"] > ratio["medium"] + 0.08
+
+
 @pytest.mark.parametrize("name", ["small", "medium", "large", "xl"])
 def test_full_mode_accounting(name):
     o, v, x = CONFIGS[name]
@@ -73,27 +161,30 @@ def test_full_mode_accounting(name):
     assert d["full_tbg"] % 16 == 0 and d["n_tiles"] >= d["full_slabs"]
     n0, n1 = 2.0 * x * v ** 4, 2.0 * o * o * v ** 4
     # the 8-fold symmetry bounds the saving: never below 1/8 (step 0) and 1/4 (step 1) of nominal; the excess is the
-    # block granularity (16-wide slabs, 128-wide CTA tiles, zero rows of diagonal blocks) and shrinks with nvirt
-    hi0, hi1 = {"small": (3.5, 1.7), "medium": (1.45, 1.12), "large": (1.15, 1.04), "xl": (1.14, 1.04)}[name]
+    # block granularity (16-wide slabs, 128-wide CTA tiles) and shrinks with nvirt
+    hi0, hi1 = {"small": (3.0, 1.7), "medium": (1.25, 1.08), "large": (1.10, 1.04), "xl": (1.07, 1.03)}[name]
     assert 1.0 <= d["flops_step0"] / (n0 / 8) <= hi0
     assert 1.0 <= d["flops_step1"] / (n1 / 4) <= hi1
-    # per apply: pack [+ pad of L for odd nvirt] + one step 0 per slab + per tile (fold, 2-4 GEMMs, 2 reductions) + unpack
-    lo = 2 + d["full_slabs"] + 4 * d["n_tiles"]
-    assert lo <= d["launches_per_apply"] <= 3 + d["full_slabs"] + 7 * d["n_tiles"]
+    # per apply: pack, diagonal-block pack [+ pad of L for odd nvirt] + one step 0 per slab + per tile (fold, 2-4 GEMMs, 2 reductions) + unpack
+    lo = 3 + d["full_slabs"] + 4 * d["n_tiles"]
+    assert lo <= d["launches_per_apply"] <= 4 + d["full_slabs"] + 7 * d["n_tiles"]
     assert d["full_workspace_bytes"] <= d["workspace_bytes"]
 
 
 def test_plans_recorded_on_the_b200_are_reproduced():
-    """profiles/r01_large_full.md / bench lines of round 1 (B200, 148 SMs): the same plan comes out without the device."""
+    """Bench lines of round 2 (B200, 148 SMs; gpurun_out/c2_bench_*.json): the same plan comes out without the device."""
     large = P.ppl_plan_dry(40, 400, 1600)
     assert (large["ta"], large["full_tbg"], large["n_tiles"], large["full_slabs"], large["splitk"]) == (16, 256, 34, 25, 15)
-    assert large["launches_per_apply"] == 263 and large["workspace_bytes"] == 22777048064
-    assert large["flops_executed"] == 32683249664000.0 and large["flops_nominal"] == 163840000000000.0
+    assert large["launches_per_apply"] == 264 and large["workspace_bytes"] == 22866753536
+    assert large["flops_executed"] == 32103848542208.0 and large["flops_nominal"] == 163840000000000.0
     xl = P.ppl_plan_dry(60, 600, 2400)
-    assert (xl["n_tiles"], xl["full_slabs"], xl["splitk"], xl["workspace_bytes"]) == (66, 38, 9, 66028931072)
-    assert xl["flops_executed"] == 329273179299840.0
+    assert (xl["n_tiles"], xl["full_slabs"], xl["splitk"], xl["workspace_bytes"]) == (66, 38, 15, 66550880768)
+    assert xl["flops_executed"] == 319215647883264.0
     medium = P.ppl_plan_dry(20, 200, 800)
-    assert (medium["full_tbg"], medium["n_tiles"], medium["splitk"]) == (208, 13, 11) and medium["flops_executed"] == 803177799680.0
+    assert (medium["full_tbg"], medium["n_tiles"], medium["splitk"]) == (208, 13, 11) and medium["flops_executed"] == 719121612800.0
+    # the round-1 form of the tiles (debug options) still plans what round 1 recorded (profiles/r01_large_full.md)
+    r1 = P.ppl_plan_dry(40, 400, 1600, debug={"full_rect_tiles": 1, "full_no_diag_pack": 1})
+    assert (r1["n_tiles"], r1["launches_per_apply"]) == (34, 263)
     tiny = P.ppl_plan_dry(5, 20, 60)  # below nvirt = 52: PPL_SYM_PAIR_SA, one tile
     assert (tiny["symmetry"], tiny["n_tiles"], tiny["ta"], tiny["launches_per_apply"]) == (P.PPL_SYM_PAIR_SA, 1, 20, 6)
 
