@@ -375,6 +375,59 @@ def probe_leg():
     print(json.dumps(out))
 
 
+def contract_leg():
+    """--contract: ppl_contract_pair (the generic 'op0,op1->out' entry point) on the paper's two ladder
+    strings at slab sizes of the medium / large configs, with torch.einsum (cuBLAS + permuted copies: the paper's
+    tensordot route on this box) beside it as context."""
+    import torch
+
+    import paper_2603_20912_b200 as P
+
+    torch.cuda.set_device(0)
+    peak = P.ppl_probe_fp64_peak(3, 20.0)
+    out = {"peak": peak, "unit": UNIT, "cases": []}
+    cases = [
+        ("xac,xbd->acbd", (800, 16, 200), (800, 200, 200)),      # step 0, one slab of 16 a's at medium
+        ("abcd,efcd->efab", (16, 200, 200, 200), (20, 20, 200, 200)),  # step 1 on that slab, t2 stored [i,j,c,d]
+        ("abcd,ecfd->efab", (16, 200, 200, 200), (20, 200, 20, 200)),  # the paper's own string: t2 stored [i,c,j,d]
+        ("xac,xbd->acbd", (1600, 4, 400), (1600, 400, 400)),     # step 0, 4 a's at large (output 2 GB)
+        ("abcd,ecfd->efab", (4, 400, 400, 400), (40, 400, 40, 400)),
+        ("ik,kj->ij", (4096, 4096), (4096, 4096)),
+    ]
+    for subs, sa, sb in cases:
+        g = torch.Generator(device="cuda").manual_seed(0)
+        A = torch.randn(sa, dtype=torch.float64, device="cuda", generator=g)
+        B = torch.randn(sb, dtype=torch.float64, device="cuda", generator=g)
+        C = P.ppl_contract_pair(subs, A, B)
+        torch.cuda.synchronize()
+        ref = torch.einsum(subs, A, B)
+        err = float((C - ref).abs().max() / ref.abs().max())
+        ins, _ = subs.split("->")
+        s0, s1 = ins.split(",")
+        ext = dict(zip(s0, sa))
+        ext.update(zip(s1, sb))
+        flops = 2.0
+        for val in ext.values():
+            flops *= val
+        res = {}
+        for name, fn in (("ours", lambda: P.ppl_contract_pair(subs, A, B, C)), ("torch_einsum", lambda: torch.einsum(subs, A, B))):
+            for _ in range(2):
+                fn()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(5):
+                fn()
+            e1.record()
+            torch.cuda.synchronize()
+            res[name] = flops / (e0.elapsed_time(e1) / 5 * 1e-3) * 1e-12
+        out["cases"].append({"subscripts": subs, "dims0": sa, "dims1": sb, "flops": flops, "tflops": res["ours"],
+                             "frac_of_peak": res["ours"] / peak, "torch_einsum_tflops": res["torch_einsum"],
+                             "max_rel_diff_vs_torch": err})
+        del A, B, C, ref
+        torch.cuda.empty_cache()
+    print(json.dumps(out))
+
+
 def run_ours(name, o, v, x, args, steps, warmup, dist, dev, rank, world, peak):
     """One workload through ppl_apply (device-resident), ppl_apply_profiled (roofline), ppl_apply_host (e2e) and the
     oracle sample (cpu_baseline + parity).  Returns the JSON record."""
@@ -402,6 +455,8 @@ def run_ours(name, o, v, x, args, steps, warmup, dist, dev, rank, world, peak):
     if args.symmetry != "default":
         plan.set_symmetry({v_: k_ for k_, v_ in SYM_NAMES.items()}[args.symmetry])
     plan.set_graph({"auto": -1, "off": 0, "on": 1}[args.graph])
+    if args.verify >= 0:
+        plan.set_verify(args.verify)
     info = plan.info()
     stream = torch.cuda.current_stream()
     cfg = workload_config(name, o, v, x)
@@ -480,7 +535,7 @@ def run_ours(name, o, v, x, args, steps, warmup, dist, dev, rank, world, peak):
         "dtype": "f64", "data": "synthetic", "config": cfg,
         "run": {"symmetry": SYM_DESC[info["symmetry"]], "parallelism": "replicas only" if world > 1 else "1 gpu",
                 "plan": {k: info[k] for k in ("ta", "tb", "n_tiles", "ring", "splitk", "vec16", "workspace_bytes")},
-                "graph": args.graph},
+                "graph": args.graph, "verify_inputs": 1 if args.verify < 0 else args.verify},
         "seconds_per_call": sec,
         "tflops_executed": f_exec / sec * 1e-12,
         "tflops_useful": f_use / sec * 1e-12,
@@ -548,12 +603,15 @@ def main():
                     help="default = the plan's own choice (full: 8-fold ERI symmetry + pair symmetry, from nvirt = 52 up)")
     ap.add_argument("--graph", default="auto", choices=["auto", "on", "off"],
                     help="ppl_plan_set_graph: replay one CUDA graph per apply (auto: launch-bound shapes only)")
+    ap.add_argument("--verify", type=int, default=-1, choices=[-1, 0, 1, 2],
+                    help="PPL_OPT_VERIFY_INPUTS (-1 = the library default: 1, a symmetry check at the head of every apply)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=0, help="timed ppl_apply_host calls (0 = --steps)")
     ap.add_argument("--no-secondary", action="store_true", help="with --config xl: skip the 'large' sub-record")
     ap.add_argument("--paper-recipe", type=int, default=0, metavar="STEPS",
                     help="context leg: time STEPS calls of the paper's tensordot recipe (cuBLAS) on the same inputs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--contract", action="store_true", help="only time ppl_contract_pair on the paper's two ladder strings")
     ap.add_argument("--probe", action="store_true", help="only measure the FP64 instruction-stream peaks and print them")
     args = ap.parse_args()
 
@@ -561,6 +619,9 @@ def main():
 
     if args.probe:
         probe_leg()
+        return
+    if args.contract:
+        contract_leg()
         return
     if args.shape:
         o, v, x = (int(t) for t in args.shape.split(","))

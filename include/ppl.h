@@ -190,7 +190,13 @@ ppl_plan_t *ppl_plan_ex(int nocc, int nvirt, int nchol, size_t workspace_bytes, 
  * producer stream is forked and joined with events).
  *   L, t2, R: DEVICE pointers, layouts above, 8-byte aligned (16-byte aligned enables the fast
  *   copy path when nvirt is even; torch allocations are 512-byte aligned).  They must stay valid
- *   until the queued work completes. */
+ *   until the queued work completes.
+ * PRECONDITIONS OF THE DEFAULT MODE: a plan for nvirt >= 52 defaults to PPL_SYM_FULL, which requires the real-orbital
+ *   symmetry L[P,a,c] == L[P,c,a] AND pair-symmetric amplitudes t2[i,j,c,d] == t2[j,i,d,c]; below that
+ *   the default is PPL_SYM_PAIR_SA, which requires the latter.  Both hold for CC amplitudes and real orbitals, neither
+ *   for arbitrary arrays (e.g. the unstructured random arrays of the paper's own benchmark): call
+ *   ppl_plan_set_symmetry(plan, PPL_SYM_NONE) for those.  By default every apply verifies the preconditions on the
+ *   device (PPL_OPT_VERIFY_INPUTS above) and a violation surfaces as PPL_ERR_PRECONDITION. */
 int ppl_apply(ppl_plan_t *plan, const double *L, const double *t2, double *R, void *stream);
 
 /* ppl_apply_ex: ppl_apply with options (storage orders of t2 and R, alpha, beta); opts == NULL
@@ -277,6 +283,25 @@ const char *ppl_error_string(int code);  /* static string, never NULL */
  * was too small for the packed operands.  PPL_ERR_WORKSPACE_TOO_SMALL if the plan holds no buffers for
  * the requested mode.  Re-plans the tile list; must not be called while an apply is in flight. */
 int ppl_plan_set_symmetry(ppl_plan_t *plan, int mode);
+
+/* Plan options.
+ * PPL_OPT_VERIFY_INPUTS: what ppl_apply / ppl_apply_ex do about the preconditions of the plan's symmetry mode
+ * (PPL_SYM_FULL: L[P,a,c] == L[P,c,a] and t2 pair-symmetric; PPL_SYM_PAIR / PPL_SYM_PAIR_SA: t2 pair-symmetric):
+ *   1 (default)  a check kernel is queued at the head of every apply (it reads L and t2 once, coalesced: < 0.1 % of a
+ *                call at `large`); the apply itself is queued regardless.  A violation is reported by the NEXT call on
+ *                the plan -- ppl_apply*, ppl_plan_verify_status or ppl_destroy -- as PPL_ERR_PRECONDITION (R of the
+ *                offending apply is then undefined).  No host synchronisation in the steady state beyond waiting for
+ *                that head-of-apply kernel of the previous call.
+ *   2            synchronous: the check runs and is awaited first; on a violation nothing else is queued and the call
+ *                returns PPL_ERR_PRECONDITION with R untouched.
+ *   0            no check: the caller vouches for the preconditions (result undefined otherwise).
+ * The check is skipped while the caller is capturing `stream` into a CUDA graph, and in PPL_SYM_NONE (no precondition).
+ * ppl_apply_host verifies L only in its streamed form (t2 never sits on the device whole). */
+enum { PPL_OPT_VERIFY_INPUTS = 1 };
+int ppl_plan_set_option(ppl_plan_t *plan, int option, int value);
+/* Waits for the check of the most recent apply (if one is pending) and returns PPL_OK or PPL_ERR_PRECONDITION;
+ * *flags (if non-NULL): bit 0 = L not symmetric, bit 1 = t2 not pair-symmetric.  Clears the pending state. */
+int ppl_plan_verify_status(ppl_plan_t *plan, int *flags);
 
 /* CUDA graph of one apply.  mode 1: ppl_apply / ppl_apply_ex capture the whole apply (all kernels, the forks and
  * joins of the plan's side streams) once into a CUDA graph and replay it with one cudaGraphLaunch on `stream`

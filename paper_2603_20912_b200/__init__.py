@@ -13,6 +13,7 @@ from .binding import (  # noqa: F401
     PPL_ERR_UNSUPPORTED_DEVICE,
     PPL_ERR_WORKSPACE_TOO_SMALL,
     PPL_OK,
+    PPL_OPT_VERIFY_INPUTS,
     PPL_SYM_NONE,
     PPL_LAYOUT_IAJB,
     PPL_LAYOUT_IJAB,

@@ -8,12 +8,12 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(_HERE, "libppl.so")
-SOURCES = ["ppl_api.cu", "ppl_contract.cu"]
+SOURCES = ["ppl_api.cu", "ppl_contract.cu", "ppl_plan.cpp"]
 
 
 def _deps():
     """Every source the library is built from: all of csrc/ plus the public header."""
-    files = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh", ".h"))]
+    files = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh", ".h", ".cpp"))]
     files.append(os.path.join(_HERE, "..", "include", "ppl.h"))
     files.append(os.path.abspath(__file__))
     return files

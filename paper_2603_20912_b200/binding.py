@@ -23,6 +23,7 @@ PPL_SYM_NONE = 0
 PPL_SYM_PAIR = 1
 PPL_SYM_PAIR_SA = 2
 PPL_SYM_FULL = 3
+PPL_OPT_VERIFY_INPUTS = 1
 PPL_LAYOUT_IJAB = 0
 PPL_LAYOUT_IAJB = 1
 LAYOUTS = {"ijab": PPL_LAYOUT_IJAB, "iajb": PPL_LAYOUT_IAJB}
@@ -108,6 +109,8 @@ SYMBOLS = {
     "ppl_error_string": (c_char_p, [c_int]),
     "ppl_plan_set_symmetry": (c_int, [c_void_p, c_int]),
     "ppl_plan_set_graph": (c_int, [c_void_p, c_int]),
+    "ppl_plan_set_option": (c_int, [c_void_p, c_int, c_int]),
+    "ppl_plan_verify_status": (c_int, [c_void_p, POINTER(c_int)]),
     "ppl_plan_info": (c_int, [c_void_p, POINTER(ppl_info_t)]),
     "ppl_plan_dry": (c_int, [c_int, c_int, c_int, c_size_t, c_size_t, c_int, c_int, POINTER(ppl_info_t)]),
     "ppl_plan_dry_ex": (c_int, [c_int, c_int, c_int, c_size_t, c_size_t, c_int, c_int, POINTER(ppl_debug_opts_t), POINTER(ppl_info_t)]),
@@ -257,6 +260,18 @@ class Plan:
     def set_graph(self, mode: int):
         """-1 auto (default), 0 plain launches, 1 replay one CUDA graph per (L, t2, R, opts) key."""
         _check(lib().ppl_plan_set_graph(self._h, int(mode)), "ppl_plan_set_graph")
+
+    def set_verify(self, mode: int):
+        """PPL_OPT_VERIFY_INPUTS: 1 (default) check at the head of every apply, reported by the next call; 2 synchronous; 0 off."""
+        _check(lib().ppl_plan_set_option(self._h, PPL_OPT_VERIFY_INPUTS, int(mode)), "ppl_plan_set_option")
+
+    def verify_status(self) -> int:
+        """Waits for the pending check of the last apply; returns its flags, raises PplError(PPL_ERR_PRECONDITION) on a violation."""
+        flags = c_int(0)
+        rc = lib().ppl_plan_verify_status(self._h, ctypes.byref(flags))
+        if rc != PPL_OK:
+            raise PplError(rc, "ppl_plan_verify_status")
+        return int(flags.value)
 
     def info(self) -> dict:
         out = ppl_info_t()

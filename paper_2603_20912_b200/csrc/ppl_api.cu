@@ -1,12 +1,14 @@
-// ppl_api.cu -- C ABI of libppl (include/ppl.h): planner, W-tile ring, stream orchestration.
-// Everything on the data path runs in the kernels of ppl_kernels.cuh / ppl_kernels_tma.cuh; there
-// is no CPU fallback.
+// ppl_api.cu -- C ABI of libppl (include/ppl.h): device allocation, launches, W-tile ring, stream orchestration, host
+// streaming, probes.  The planner is ppl_plan.cpp (host only).  Everything on the data path runs in the kernels of
+// ppl_kernels*.cuh; there is no CPU fallback.
 #include "../../include/ppl.h"
+#include "ppl_plan.h"
 #include "ppl_kernels.cuh"
 #include "ppl_kernels_tma.cuh"
 #include "ppl_kernels_full.cuh"
 
 #include <atomic>
+#include <initializer_list>
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
@@ -15,16 +17,8 @@
 #include <new>
 #include <vector>
 
-namespace {
+using namespace pplh;
 
-thread_local int g_last_error = PPL_OK;
-
-int fail(int code) {
-    g_last_error = code;
-    return code;
-}
-}  // namespace
-int ppl_fail_code(int code) { return fail(code); }  // for the other translation units of the library (ppl_contract.cu)
 namespace {
 #define PPL_CUDA(expr)                                 \
     do {                                               \
@@ -34,286 +28,13 @@ namespace {
             return fail(PPL_ERR_CUDA);                 \
         }                                              \
     } while (0)
-
-struct SplitChoice {
-    int splitk = 1, k_per_split = ppl::BK;
-    double seconds = 0;
-};
-
-// Row tiling of the M side of step 1.  TMA kernels: 8-row blocks dealt to 2*tiles_m half-tiles of `base` or `base+1`
-// blocks (ppl::MSplit); cp.async kernels: uniform tiles of 128 rows.
-struct MGeom {
-    int tiles_m = 1, base = 0, rem = 0;
-    int ni = 8;         // template instance (TMA box of the A operand: 16*ni rows)
-    double rows = 128;  // average rows computed per CTA tile (cost model)
-};
-
-struct Tile {
-    int a0, ta, b0, tb;
-    int mirror;
-    SplitChoice full;    // step 1 over K = nvirt^2                (PPL_SYM_NONE / PPL_SYM_PAIR)
-    SplitChoice sp, sm;  // step 1 over the packed K+ / K- ranges  (PPL_SYM_PAIR_SA)
-};
-
-// PPL_SYM_FULL: one tile = (a-block A of 16) x (a group of b's), one slab = all tiles of one A
-struct FullTile {
-    int A0, ta;      // a-block
-    int bg0, nb;     // first b of the group, number of b's in it
-    int tbp;         // nb rounded up to a multiple of 16: W-tile rows are a_l*tbp + b_l
-    int k0p, k0m;    // first packed (c<=d) / (c<d) index with c >= A0: start of the use-1 contraction range
-    int k1p, k1m;    // first packed index with c >= A0+16: start of the use-2 output range
-    SplitChoice sp, sm;
-    // memory-tight mode: step 0 runs per tile on the full (b in group, d >= A0) rectangle into a strip of the tile's rows
-    size_t chunk_off = 0;
-    int tiles_n = 0;
-    // range tiles (the default outside the memory-tight form): the W+- rows are a run of the packed pair index of (a <= b),
-    // a in the slab -- no zero rows for a > b and no rounding of the b count, only the holes of the packed layout
-    int range = 0;
-    int kp0 = 0, np = 0, npr = 0;  // plus: first packed index, rows, rows rounded up to 16 (the k-tiles of use 2)
-    int km0 = 0, nm = 0, nmr = 0;  // minus rows of the same pairs
-    int nzm = 0, zrows_m[24] = {};  // minus rows no pair writes (holes, tail): zeroed by the fold
-};
-struct FullSlab {
-    int A0, ta;
-    int tiles_m, tiles_n;  // step-0 CTA tiles: 128 rows (c, a_l), 128 columns (8 chunks of 16 d's)
-    size_t chunk_off;      // first entry of this slab in the chunk table
-    int tile_begin, tile_end;
-    double flops0;
-};
-
-constexpr int MAX_RING = 4;
-constexpr double PEAK_FLOPS = 37.2e12;  // nominal FP64 (148 SM x 64 FMA/clk x 2 x 1.965 GHz); planner cost model only
-constexpr double HBM_BPS = 6.0e12;      // planner cost model only
-constexpr double GRAPH_AUTO_FLOPS = 5.0e9;   // ppl_plan_set_graph(-1): measured -- tiny 47.7 -> 37.9 us, small (1.7e9) 270 -> 231 us with the graph; (10,100,400) (2.8e10) 1.44 -> 1.51 ms, medium 26.1 -> 26.8 ms without
-constexpr double LAUNCH_S = 4e-6;
-
-size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
-
 }  // namespace
-
-struct ppl_plan_s {
-    int o = 0, v = 0, x = 0;
-    int sym = PPL_SYM_PAIR_SA;
-    int sa_ok = 0;        // the workspace holds the packed operands of PPL_SYM_PAIR_SA
-    int T = 0;            // tile edge (ta = tb = T except at the ragged edge)
-    int nblk = 0;
-    int ring = 1;
-    int vec16 = 0;
-    int num_sms = 148;
-    int use_tma = 0;      // 1: persistent TMA/mbarrier kernels; 0: cp.async kernels
-    int64_t vv = 0;       // nvirt^2 = row length of an un-packed W tile / of t2
-    int vp = 0;           // nvirt rounded up to even: the geometry of every PACKED operand (tau+-, W+-, R+-acc) and of the
-    int64_t vvp = 0;      // whole PPL_SYM_FULL path; for odd nvirt the pad index carries exact zeros
-    double *Lpad = nullptr;  // PPL_SYM_FULL with odd nvirt: L copied into [x][vp][vp] (TMA needs 16-byte rows), inside fws
-    // packed geometry (PPL_SYM_PAIR_SA)
-    int Mp = 0, Mm = 0;   // rows (i<=j), (i<j)
-    int Kp = 0, Km = 0;   // extents of the packed column indices of (c<=d), (c<d), holes included
-    int KpT = 0, KmT = 0; // number of pairs (c<=d), (c<d)
-    int64_t ldp = 0, ldm = 0;
-    int bm_full = 128, bm_p = 128, bm_m = 128;  // step-1 CTA tile rows (TMA box: 16*NI)
-    MGeom mg_full, mg_p, mg_m;                  // row tiling of nocc^2 / the packed (i<=j) / (i<j) rows
-    size_t cap = 0;
-    size_t x_bytes = 0, slot_bytes = 0, part_bytes = 0, tau_bytes = 0, ws_bytes = 0;
-    unsigned char *ws = nullptr;
-    double *X = nullptr;                   // SA: step-0 output tile [T*T][vv], folded into a ring slot
-    double *slot[MAX_RING] = {nullptr, nullptr, nullptr, nullptr};  // W tile, or W+ [T*T][ldp] followed by W- [T*T][ldm]
-    double *part = nullptr;
-    double *taup = nullptr, *taum = nullptr;
-    double *tperm = nullptr;               // un-packed modes with PPL_LAYOUT_IAJB input: t2 permuted (lazy)
-    int *flags = nullptr;                  // device word for ppl_check_inputs
-    std::vector<Tile> tiles;
-    cudaStream_t gen = nullptr, host_stream = nullptr;
-    cudaEvent_t ev_in = nullptr, ev_ready[MAX_RING] = {}, ev_free[MAX_RING] = {};
-    double *dL = nullptr, *dT = nullptr, *dR = nullptr;  // ppl_apply_host staging
-    double *hstage[2] = {nullptr, nullptr};              // ppl_apply_host in PPL_SYM_FULL: two chunk buffers for t2 / R
-    int hchunk_rows = 0;                                 // (i,j) rows per chunk
-    cudaStream_t hs2 = nullptr;                          // second chunk stream of ppl_apply_host (the first is `gen`)
-    cudaEvent_t ev_tau = nullptr, ev_done = nullptr;     // tau+- complete / all slabs done
-    double f_step0 = 0, f_step1 = 0;
-    CUtensorMap mapW[MAX_RING], mapWp[MAX_RING], mapWm[MAX_RING], mapTp, mapTm;  // plan-owned operands
-    // ---- PPL_SYM_FULL (own allocation `fws`; shares taup/taum with PPL_SYM_PAIR_SA) ----
-    int full_ok = 0;
-    int full_tight = 0;                        // 1: the strip holds one (slab; b-group) tile, step 0 runs per tile without the b<->d image
-    int tbg = 0;                               // b-group width (multiple of 16)
-    size_t fws_bytes = 0;
-    unsigned char *fws = nullptr;
-    double *fX = nullptr;                      // strip [16*v rows (a_l*v + b)][vv]
-    double *fX2 = nullptr;                     // second strip (when it fits): step 0 of slab k+1 runs on `fs0` while slab k is folded
-    cudaStream_t fs0 = nullptr;                // producer stream of step 0 (two strips only)
-    cudaEvent_t ev_fork = nullptr, ev_s0[2] = {nullptr, nullptr}, ev_xfree[2] = {nullptr, nullptr};
-    int fslots = 1;                            // W+- slots (2 when they fit: the fold of tile k+1 overlaps the GEMMs of tile k)
-    double *fWp[2] = {nullptr, nullptr}, *fWm[2] = {nullptr, nullptr};  // W+- tile [16*tbg][ldp], [16*tbg][ldm]
-    double *fpart = nullptr;
-    double *raccp = nullptr, *raccm = nullptr; // R+- accumulators [Mp][ldp], [Mm][ldm]
-    int2 *fchunks = nullptr;
-    double *Lq = nullptr;                      // packed diagonal 16 x 16 blocks of L: [x][ldq] (ppl_kernels_full.cuh, k_pack_diag)
-    int nfull = 0;                             // full 16-blocks of the (padded) virtual index
-    int64_t ldq = 0;
-    int diag_pack = 0;
-    CUtensorMap mapLq;
-    ppl_debug_opts_t dbg = {};
-    size_t fpart_bytes = 0;
-    size_t fpart_m_off = 0;                    // doubles: the minus partials start here (fixed: + and - run on different streams)
-    std::vector<FullSlab> slabs;
-    std::vector<FullTile> ftiles;
-    double ff_step0 = 0, ff_step1 = 0;
-    cudaStream_t fs[4] = {nullptr, nullptr, nullptr, nullptr};  // side streams of the four step-1 GEMMs of a tile
-    cudaEvent_t ev_fold[2] = {nullptr, nullptr}, evg[2][4] = {};
-    CUtensorMap mapFWp[2], mapFWm[2], mapFWpT[2], mapFWmT[2];  // the W+- tile as the B operand of use 1 (box 16 x 128 rows) / use 2 (box 16 x 16 rows)
-    // ---- CUDA graph of one apply (launch-bound shapes; ppl_plan_set_graph) ----
-    int dry = 0;                               // ppl_plan_dry: geometry only, the plan owns nothing on the device
-    int graph_mode = -1;                       // -1: auto (graph when the executed flops are below GRAPH_AUTO_FLOPS), 0: off, 1: on
-    cudaStream_t gcap = nullptr;               // capture origin (never the caller's stream: the legacy stream cannot capture)
-    cudaGraphExec_t gexec = nullptr;           // the instantiated apply for the key below
-    struct GraphKey {
-        const double *L = nullptr, *t2 = nullptr;
-        double *R = nullptr;
-        ppl_opts_t opts = {0, 0, 0.0, 0.0};
-        int sym = -1;
-    } gkey;
-};
 
 namespace {
 
-// ------------------------------------------------------------------------------------------
-// Planner: the analogue of the paper's memory functions (Table 1) -- but what
-// is being sized is the W-tile ring in HBM, not host->device batches.  For a candidate tile edge
-// T it estimates the time of one apply from CTA-wave counts of both GEMMs (CTA tile 128x128x16 on
-// `sms` SMs), the best split-K per tile shape, and the streaming traffic.
-// ------------------------------------------------------------------------------------------
-
-// TMA kernels: the fewest CTA tiles of at most 16*10 rows, rows dealt in 8-row blocks as evenly as possible
-// (ppl_kernels_tma.cuh, MSplit): padding < 8 rows in all.  nmax: largest template instance to use (debug override).
-// Every warp row gets ni or ni - 1 blocks: the only two cases the kernels are compiled for.
-MGeom m_geom_tma(int M, int nmax) {
-    MGeom g;
-    const int blocks = (std::max(M, 1) + 7) / 8;
-    g.tiles_m = (blocks + 2 * nmax - 1) / (2 * nmax);
-    g.base = blocks / (2 * g.tiles_m);
-    g.rem = blocks % (2 * g.tiles_m);
-    g.ni = g.base + (g.rem > 0 ? 1 : 0);  // 1 .. nmax
-    g.rows = 8.0 * blocks / g.tiles_m;
-    return g;
-}
-MGeom m_geom_plain(int M) {
-    MGeom g;
-    g.tiles_m = (std::max(M, 1) + ppl::BM - 1) / ppl::BM;
-    return g;
-}
-
-SplitChoice choose_split(int M, int N, int64_t K, int sms, const MGeom &mg, size_t part_cap = ~(size_t)0) {
-    SplitChoice best;
-    if (M <= 0 || N <= 0 || K <= 0) return best;
-    const int tiles = mg.tiles_m * ((N + ppl::BN - 1) / ppl::BN);
-    const int nkt = (int)((K + ppl::BK - 1) / ppl::BK);
-    const double tau = 2.0 * mg.rows * ppl::BN * ppl::BK / (PEAK_FLOPS / sms);  // one k-tile on one SM
-    best = SplitChoice{1, nkt * ppl::BK, 1e300};
-    const int smax = std::max(1, std::min(nkt / 8 + 1, 64));
-    for (int s = 1; s <= smax; ++s) {
-        const int kt_per = (nkt + s - 1) / s;
-        const int s_eff = (nkt + kt_per - 1) / kt_per;  // no empty splits
-        if (s_eff != s) continue;
-        if ((size_t)s * M * N * 8 > part_cap && s > 1) continue;
-        const double waves = std::ceil((double)tiles * s / sms);
-        const double t = waves * (kt_per + 6) * tau                      // +6: pipeline fill / epilogue
-                         + (double)(s + 2) * M * N * 8.0 / HBM_BPS;      // partials written + read by the reduce
-        if (t < best.seconds) best = SplitChoice{s, kt_per * ppl::BK, t};
-    }
-    return best;
-}
-
-double step0_seconds(int ta, int tb, int v, int x, int sms) {
-    const int tiles = ((ta * v + ppl::BM - 1) / ppl::BM) * ((tb * v + ppl::BN - 1) / ppl::BN);
-    const int nkt = (x + ppl::BK - 1) / ppl::BK;
-    const double tau = 2.0 * ppl::BM * ppl::BN * ppl::BK / (PEAK_FLOPS / sms);
-    return std::ceil((double)tiles / sms) * (nkt + 6) * tau;
-}
-
-struct Geometry {  // what depends on (o, v) only
-    int64_t vv;
-    int M, Mp, Mm, Kp, Km;
-    int64_t ldp, ldm;
-    MGeom mg_full, mg_p, mg_m;
-};
-
-struct PlanEval {
-    double seconds = 1e300;
-    size_t x_bytes = 0, slot_bytes = 0, part_bytes = 0;
-};
-
-// estimated seconds of one apply with tile edge T in PPL_SYM_PAIR_SA (sa = true) or PPL_SYM_PAIR
-PlanEval evaluate(const Geometry &g, int o, int v, int x, int T, bool sa, int sms) {
-    PlanEval ev;
-    const int nblk = (v + T - 1) / T;
-    const int r = v - (nblk - 1) * T;  // ragged edge
-    double total = 0;
-    size_t part_max = 0;
-    auto count = [&](bool a_edge, bool b_edge) -> int64_t {  // executed tiles (a-block <= b-block) per shape
-        if (a_edge && b_edge) return 1;
-        if (a_edge && !b_edge) return 0;
-        if (!a_edge && b_edge) return nblk - 1;
-        return (int64_t)(nblk - 1) * nblk / 2;
-    };
-    for (int ae = 0; ae < 2; ++ae)
-        for (int be = 0; be < 2; ++be) {
-            const int64_t cnt = count(ae, be);
-            if (cnt == 0) continue;
-            const int ta = ae ? r : T, tb = be ? r : T;
-            const int N = ta * tb;
-            const SplitChoice full = choose_split(g.M, N, g.vv, sms, g.mg_full);
-            size_t part = (size_t)full.splitk * g.M * N * 8;
-            double compute, dram;
-            if (sa) {
-                const SplitChoice sp = choose_split(g.Mp, N, g.Kp, sms, g.mg_p), sm = choose_split(g.Mm, N, g.Km, sms, g.mg_m);
-                const double fold = 2.0 * N * g.vv * 8.0 / HBM_BPS + LAUNCH_S;
-                compute = step0_seconds(ta, tb, v, x, sms) + fold + sp.seconds + sm.seconds;
-                dram = (((double)g.Mp * g.ldp + (double)g.Mm * g.ldm) * 8.0 + 4.0 * N * g.vv * 8.0) / HBM_BPS;
-                part = std::max(part, ((size_t)sp.splitk * g.Mp + (size_t)sm.splitk * g.Mm) * N * 8);
-                total += cnt * (std::max(compute, dram) + 5 * LAUNCH_S);
-            } else {
-                compute = step0_seconds(ta, tb, v, x, sms) + full.seconds;
-                dram = ((double)g.M * g.vv * 8.0 + 2.0 * N * g.vv * 8.0) / HBM_BPS;
-                total += cnt * (std::max(compute, dram) + 3 * LAUNCH_S);
-            }
-            part_max = std::max(part_max, part);
-        }
-    ev.seconds = total;
-    ev.x_bytes = sa ? align256((size_t)T * T * g.vv * 8) : 0;
-    ev.slot_bytes = align256(sa ? (size_t)T * T * (g.ldp + g.ldm) * 8 : (size_t)T * T * g.vv * 8);
-    ev.part_bytes = align256(part_max);
-    return ev;
-}
-
-int build_tiles(ppl_plan_s *p) {
-    p->tiles.clear();
-    p->f_step0 = p->f_step1 = 0;
-    const int T = p->T, v = p->v, M = p->o * p->o;
-    const bool pair = p->sym != PPL_SYM_NONE, sa = p->sym == PPL_SYM_PAIR_SA;
-    for (int ab = 0; ab < p->nblk; ++ab)
-        for (int bb = (pair ? ab : 0); bb < p->nblk; ++bb) {
-            Tile t;
-            t.a0 = ab * T;
-            t.ta = std::min(T, v - t.a0);
-            t.b0 = bb * T;
-            t.tb = std::min(T, v - t.b0);
-            t.mirror = (pair && ab != bb) ? 1 : 0;
-            const int N = t.ta * t.tb;
-            if (sa) {
-                t.sp = choose_split(p->Mp, N, p->Kp, p->num_sms, p->mg_p);
-                t.sm = choose_split(p->Mm, N, p->Km, p->num_sms, p->mg_m);
-                if (((size_t)t.sp.splitk * p->Mp + (size_t)t.sm.splitk * p->Mm) * N * 8 > p->part_bytes)
-                    return PPL_ERR_WORKSPACE_TOO_SMALL;
-                p->f_step1 += 2.0 * N * ((double)p->Mp * p->KpT + (double)p->Mm * p->KmT);
-            } else {
-                t.full = choose_split(M, N, p->vv, p->num_sms, p->mg_full, p->part_bytes);
-                if ((size_t)t.full.splitk * M * N * 8 > p->part_bytes) return PPL_ERR_WORKSPACE_TOO_SMALL;
-                p->f_step1 += 2.0 * M * (double)N * (double)p->vv;
-            }
-            p->tiles.push_back(t);
-            p->f_step0 += 2.0 * p->x * (double)N * (double)p->vv;
-        }
-    return PPL_OK;
-}
+// per-apply verification of the symmetry preconditions (PPL_OPT_VERIFY_INPUTS; defined next to ppl_check_inputs)
+int verify_harvest(ppl_plan_s *p, int *flags_out);
+int verify_begin(ppl_plan_s *p, const double *L, const double *t2, int t2_layout, cudaStream_t stream);
 
 void free_plan(ppl_plan_s *p) {
     if (!p) return;
@@ -364,6 +85,9 @@ void free_plan(ppl_plan_s *p) {
     if (p->ws) cudaFree(p->ws);
     if (p->fws) cudaFree(p->fws);
     if (p->flags) cudaFree(p->flags);
+    if (p->vflags) cudaFree(p->vflags);
+    if (p->vflags_host) cudaFreeHost(p->vflags_host);
+    if (p->ev_verify) cudaEventDestroy(p->ev_verify);
     if (p->tperm) cudaFree(p->tperm);
     if (p->dL) cudaFree(p->dL);
     if (p->dT) cudaFree(p->dT);
@@ -786,229 +510,15 @@ int run_apply(ppl_plan_s *p, const double *L, const double *t2, double *R, const
 // ------------------------------------------------------------------------------------------
 // PPL_SYM_FULL (ppl_kernels_full.cuh): slabs of 16 a's, tiles (A; b-group), chunk table of step 0.
 // ------------------------------------------------------------------------------------------
-// flops of one step-1 launch as the CTA tiles execute it: rows in 8-row blocks (MSplit), columns in tiles of 128, k in tiles of 16
-double gemm_flops_launched(const MGeom &mg, int M, int64_t ncols, int64_t krange) {
-    if (M <= 0 || ncols <= 0 || krange <= 0) return 0;
-    const double rows = 8.0 * ((M + 7) / 8);
-    (void)mg;
-    return 2.0 * rows * (128.0 * ((ncols + 127) / 128)) * (16.0 * ((krange + 15) / 16));
-}
-
-int full_geometry(ppl_plan_s *p, int tbg, size_t part_cap, std::vector<int2> *chunks_out, bool tight = false) {
-    const int v = p->vp, TA = ppl::TA_FULL;
-    p->slabs.clear();
-    p->ftiles.clear();
-    p->ff_step0 = p->ff_step1 = 0;
-    p->fpart_bytes = 0;
-    size_t part_p = 0, part_m = 0;
-    std::vector<int2> chunks;
-    const bool range_tiles = !tight && !p->dbg.full_rect_tiles;
-    const bool diag_pack = !tight && !p->dbg.full_no_diag_pack && v >= 16;
-    p->diag_pack = diag_pack ? 1 : 0;
-    p->nfull = v / 16;
-    p->ldq = (int64_t)std::max(p->nfull, 1) * ppl::DIAG_PACKED;
-    std::vector<unsigned char> mark;
-    for (int A0 = 0; A0 < v; A0 += TA) {
-        FullSlab sl;
-        sl.A0 = A0;
-        sl.ta = std::min(TA, v - A0);
-        sl.tiles_m = ((v - A0) + 7) / 8;  // 8 c's x 16 a_l per 128-row CTA tile
-        sl.chunk_off = chunks.size();
-        // d-block major: the 8 chunks of a CTA tile are 8 consecutive b's of one d-block, so that the b<->d image
-        // X[a,d,c,b] is written as runs of 8 b's (two full 32-byte sectors, merged in L2) instead of lone doubles
-        if (!tight) {
-            // A ragged last d-block [dL, v) of width w < 16 would cost a whole 16-wide chunk for every b >= A0.  It is
-            // covered from the other side instead: the w b's of that block against every d-block from A0 up (chunks with
-            // d-block BELOW the b-block; the epilogue stores their b<->d image like that of any off-diagonal chunk), which
-            // is w * ceil(r / 16) chunks instead of r (nvirt = 200, 600: w = 8, half as many).
-            const int dL = A0 + (v - 1 - A0) / 16 * 16, w = v - dL;
-            const bool reverse = w < 16 && (int64_t)w * ((v - A0 + 15) / 16) < (v - A0);
-            // Diagonal blocks (b-block == d-block, full 16 x 16): only b <= d is needed -- 9 chunks of the packed copy Lq
-            // (k_pack_diag) instead of 16 plain ones.  They go behind the plain chunks so that those keep their
-            // (b even, b + 1) pairing inside the column tiles (16-byte image stores).
-            for (int d0 = A0; d0 < v; d0 += 16) {
-                if (reverse && d0 == dL) break;
-                const bool packed = diag_pack && d0 + 16 <= v;
-                for (int b = A0; b < (packed ? d0 : std::min(d0 + 16, v)); ++b) chunks.push_back(make_int2(b, d0));
-            }
-            if (reverse)
-                for (int d0 = A0; d0 <= dL; d0 += 16)
-                    for (int b = dL; b < v; ++b) chunks.push_back(make_int2(b, d0));
-            if (diag_pack)
-                for (int d0 = A0; d0 + 16 <= v; d0 += 16)
-                    for (int j = 0; j < ppl::DIAG_PACKED / 16; ++j)
-                        chunks.push_back(make_int2(-2 - d0 / 16, d0 / 16 * ppl::DIAG_PACKED + 16 * j));
-            while ((chunks.size() - sl.chunk_off) % 8) chunks.push_back(make_int2(-1, 0));
-        }
-        sl.tiles_n = (int)((chunks.size() - sl.chunk_off) / 8);
-        sl.flops0 = 2.0 * p->x * (128.0 * sl.tiles_m) * (128.0 * sl.tiles_n);
-        p->ff_step0 += sl.flops0;
-        sl.tile_begin = (int)p->ftiles.size();
-        const int c1 = std::min(A0 + TA, v);
-        // range starts are even (TMA alignment): (A0,A0) sits at an even index, and the element before
-        // (A0, A0+1) in the minus triangle is a hole (A0 even)
-        const int k0p = (int)ppl::kplus(A0, A0, v);
-        const int k0m = A0 + 1 < v ? (int)ppl::kminus(A0, A0 + 1, v) - 1 : p->Km;
-        const int k1p = c1 < v ? (int)ppl::kplus(c1, c1, v) : p->Kp;
-        const int k1m = c1 + 1 < v ? (int)ppl::kminus(c1, c1 + 1, v) - 1 : p->Km;
-        auto finish_tile = [&](FullTile &t, int Np, int Nm, int Kup, int Kum) {
-            // Np / Nm: W+- rows contracted by use 1 (its GEMM N); Kup / Kum: W+- rows contracted by use 2 (its GEMM K)
-            t.k0p = k0p;
-            t.k0m = k0m;
-            t.k1p = k1p;
-            t.k1m = k1m;
-            t.sp = choose_split(p->Mp, Np, p->Kp - t.k0p, p->num_sms, p->mg_p, part_cap / 2);
-            t.sm = choose_split(p->Mm, Nm, p->Km - t.k0m, p->num_sms, p->mg_m, part_cap / 2);
-            part_p = std::max(part_p, (size_t)t.sp.splitk * p->Mp * Np);
-            part_m = std::max(part_m, (size_t)t.sm.splitk * p->Mm * std::max(Nm, 0));
-            p->fpart_m_off = (part_p + 31) / 32 * 32;
-            p->fpart_bytes = (p->fpart_m_off + part_m) * 8;
-            // executed flops, as the CTA tiles run them: use 1 (contraction over J >= (A0,A0)) + use 2 (outputs J >= (A0+16,A0+16))
-            p->ff_step1 += gemm_flops_launched(p->mg_p, p->Mp, Np, p->Kp - t.k0p) + gemm_flops_launched(p->mg_m, p->Mm, Nm, p->Km - t.k0m);
-            p->ff_step1 += gemm_flops_launched(p->mg_p, p->Mp, p->Kp - (t.k1p & ~15), Kup) +
-                           gemm_flops_launched(p->mg_m, p->Mm, p->Km - (t.k1m & ~15), Kum);
-        };
-        if (range_tiles) {
-            // the slab's pairs (a <= b), a in the slab, are ONE run of the packed index; it is cut into tiles of at most 16 tbg
-            // rows at multiples of 128 (the column tile of use 1)
-            const int64_t lo = k0p, hi = ppl::kplus(A0 + sl.ta - 1, v - 1, v) + 1, Ls = hi - lo, NT = (int64_t)TA * tbg;
-            const int ng = (int)((Ls + NT - 1) / NT);
-            int64_t chunk = ((Ls + ng - 1) / ng + 127) / 128 * 128;
-            if (chunk > NT) chunk = NT;
-            int64_t prev_last_m = -1;
-            for (int64_t kp0 = lo; kp0 < hi; kp0 += chunk) {
-                FullTile t;
-                t.A0 = A0;
-                t.ta = sl.ta;
-                t.bg0 = A0;
-                t.nb = v - A0;
-                t.tbp = 0;
-                t.range = 1;
-                t.kp0 = (int)kp0;
-                t.np = (int)(std::min(kp0 + chunk, hi) - kp0);
-                t.npr = (t.np + 15) / 16 * 16;
-                // the minus rows of the tile's pairs
-                int64_t first_m = -1, last_m = -1;
-                int a = A0;
-                for (int64_t kap = kp0; kap < kp0 + t.np; ++kap) {
-                    while (a + 1 < A0 + sl.ta && ppl::kplus(a + 1, a + 1, v) <= kap) ++a;
-                    const int b = a + (int)(kap - ppl::kplus(a, a, v));
-                    if (b >= v || b <= a) continue;  // hole / diagonal pair
-                    const int64_t km = ppl::kminus(a, b, v);
-                    if (first_m < 0) first_m = km;
-                    last_m = km;
-                }
-                if (first_m >= 0) {
-                    t.km0 = (int)(first_m & ~(int64_t)1);
-                    if ((int64_t)t.km0 <= prev_last_m) return PPL_ERR_INVALID_ARG;  // never: cuts fall on even indices (kplus / kminus parity = parity of b)
-                    t.nm = (int)(last_m + 1 - t.km0);
-                    t.nmr = (t.nm + 15) / 16 * 16;
-                    prev_last_m = last_m;
-                    mark.assign(t.nmr, 0);
-                    a = A0;
-                    for (int64_t kap = kp0; kap < kp0 + t.np; ++kap) {
-                        while (a + 1 < A0 + sl.ta && ppl::kplus(a + 1, a + 1, v) <= kap) ++a;
-                        const int b = a + (int)(kap - ppl::kplus(a, a, v));
-                        if (b >= v || b <= a) continue;
-                        mark[ppl::kminus(a, b, v) - t.km0] = 1;
-                    }
-                    for (int r = 0; r < t.nmr; ++r)
-                        if (!mark[r]) {
-                            if (t.nzm >= 24) return PPL_ERR_INVALID_ARG;  // never: <= 8 holes (one per two a's) + 15 tail rows
-                            t.zrows_m[t.nzm++] = r;
-                        }
-                }
-                finish_tile(t, t.np, t.nm, t.npr, t.nmr);
-                p->ftiles.push_back(t);
-            }
-        } else {
-            // b-groups: the 16-blocks of [A0, v) dealt into groups of at most tbg/16 blocks, as evenly as possible
-            const int nblk = (v - A0 + 15) / 16, per = tbg / 16, ng = (nblk + per - 1) / per;
-            int blk = 0;
-            for (int gi = 0; gi < ng; ++gi) {
-                const int cnt = nblk / ng + (gi < nblk % ng ? 1 : 0);
-                FullTile t;
-                t.A0 = A0;
-                t.ta = sl.ta;
-                t.bg0 = A0 + 16 * blk;
-                t.nb = std::min(16 * cnt, v - t.bg0);
-                t.tbp = 16 * cnt;
-                blk += cnt;
-                const int N = TA * t.tbp;
-                finish_tile(t, N, N, N, N);
-                if (tight) {  // the full (b, d) rectangle of the group: no image, twice the step-0 flops, a strip of tbp rows per a
-                    t.chunk_off = chunks.size();
-                    for (int d0 = A0; d0 < v; d0 += 16)
-                        for (int b = t.bg0; b < t.bg0 + t.nb; ++b) chunks.push_back(make_int2(b, d0));
-                    while ((chunks.size() - t.chunk_off) % 8) chunks.push_back(make_int2(-1, 0));
-                    t.tiles_n = (int)((chunks.size() - t.chunk_off) / 8);
-                    const double f0 = 2.0 * p->x * (128.0 * sl.tiles_m) * (128.0 * t.tiles_n);
-                    sl.flops0 += f0;
-                    p->ff_step0 += f0;
-                }
-                p->ftiles.push_back(t);
-            }
-        }
-        sl.tile_end = (int)p->ftiles.size();
-        p->slabs.push_back(sl);
-    }
-    if (chunks_out) chunks_out->swap(chunks);
-    return PPL_OK;
-}
-
-// Allocate the PPL_SYM_FULL buffers if they fit into `room` bytes.  Returns PPL_OK and sets full_ok, or leaves it 0.
-int full_setup(ppl_plan_s *p, size_t room, bool dry = false) {
+// Allocate what full_plan sized (device half).  Sets full_ok, or leaves it 0 (the plan then stays without PPL_SYM_FULL).
+int full_allocate(ppl_plan_s *p) {
     p->full_ok = 0;
-    if (!p->use_tma || !p->sa_ok || p->v < 2) return PPL_OK;
-    const int v = p->vp, TA = ppl::TA_FULL;
-    const size_t lpad_bytes = (p->v & 1) ? align256((size_t)p->x * p->vvp * 8) : 0;
-    int tbg = p->dbg.full_tbg >= 16 ? p->dbg.full_tbg / 16 * 16 : 256;  // debug override of the largest tile (rows / 16)
-    tbg = std::min(tbg, (v + 15) / 16 * 16);
-    const size_t racc_bytes = p->tau_bytes;  // same shapes as tau+-
-    std::vector<int2> chunks;
-    const int want_slots = p->dbg.full_slots == 1 ? 1 : 2;
-    const int tbg0 = tbg;
-    size_t x_bytes = 0, lq_bytes = 0;
-    bool two_strips = false, fits = false;
-    // First the slab strip (16 v^3 doubles: step 0 on d-block >= b-block only, 1/8 of nominal).  If it does not fit under
-    // the cap, the memory-tight mode: a strip of one (slab; b-group) tile (16 tbg v^2), step 0 per tile on the group's
-    // full (b, d) rectangle (1/4 of nominal), everything behind the fold unchanged.
-    for (int tight = p->dbg.full_tight == 1 ? 1 : 0; tight <= 1 && !fits; ++tight)
-        for (tbg = tbg0;; tbg = std::max(16, tbg / 2 / 16 * 16)) {
-            x_bytes = align256((size_t)TA * (tight ? tbg : v) * p->vvp * 8);
-            // A second strip pays where slabs are short (medium: 26.19 -> 25.82 ms for 1 GB); at large it buys 0.15 % for
-            // 8.2 GB and is not taken.  In the tight mode it is what lets step 0 of tile k+1 overlap the GEMMs of tile k.
-            const int want_strips = p->dbg.full_strips ? (p->dbg.full_strips == 1 ? 1 : 2) : ((tight || x_bytes <= ((size_t)2 << 30)) ? 2 : 1);
-            const size_t slot_rows = (size_t)TA * tbg + 16;  // + 16: the minus run of a range tile may be a few rows longer than the plus run
-            const size_t slot = align256(slot_rows * p->ldp * 8) + align256(slot_rows * p->ldm * 8);
-            const size_t part_cap = std::max<size_t>((size_t)64 << 20, slot / 8);
-            if (full_geometry(p, tbg, part_cap, &chunks, tight != 0) != PPL_OK) {
-                p->dbg.full_rect_tiles = 1;  // (never taken: the range tiling failed its own invariants)
-                full_geometry(p, tbg, part_cap, &chunks, tight != 0);
-            }
-            const size_t chunk_bytes = align256(chunks.size() * sizeof(int2));
-            lq_bytes = p->diag_pack ? align256((size_t)p->x * p->ldq * 8) : 0;
-            const size_t base = x_bytes + align256(p->fpart_bytes) + racc_bytes + chunk_bytes + lpad_bytes + lq_bytes + 256;
-            int ns = 0;
-            for (int s = want_slots; s >= 1 && !ns; --s)
-                if (base + s * slot <= room) ns = s;
-            if (ns) {
-                p->tbg = tbg;
-                p->fslots = ns;
-                p->full_tight = tight;
-                p->fws_bytes = base + ns * slot;
-                two_strips = want_strips == 2 && ns == want_slots && p->fws_bytes + x_bytes <= room;
-                if (two_strips) p->fws_bytes += x_bytes;
-                fits = true;
-                break;
-            }
-            if (tbg == 16) break;
-        }
-    if (!fits) return PPL_OK;  // the plan stays without PPL_SYM_FULL
-    if (dry) {  // geometry only (ppl_plan_dry): slabs, tiles, splits and byte counts are final at this point
-        p->full_ok = 1;
-        return PPL_OK;
-    }
+    if (!p->full_planned) return PPL_OK;
+    const int TA = ppl::TA_FULL;
+    const size_t x_bytes = p->fx_bytes, lq_bytes = p->lq_bytes, lpad_bytes = p->lpad_bytes;
+    const bool two_strips = p->two_strips;
+    const std::vector<int2> &chunks = p->chunks_host;
+    const size_t racc_bytes = p->tau_bytes;
     if (cudaMalloc(&p->fws, p->fws_bytes) != cudaSuccess) {
         (void)cudaGetLastError();
         p->fws = nullptr;
@@ -1455,124 +965,6 @@ int launch_unpack_full(const ppl_plan_s *p, const ppl_opts_t &opts, double *R, i
 // =============================================================================================
 extern "C" {
 
-int ppl_last_error(void) { return g_last_error; }
-
-const char *ppl_error_string(int code) {
-    switch (code) {
-        case PPL_OK: return "ok";
-        case PPL_ERR_INVALID_ARG: return "invalid argument";
-        case PPL_ERR_WORKSPACE_TOO_SMALL: return "workspace_bytes below the minimum plan";
-        case PPL_ERR_ALLOC: return "allocation failed";
-        case PPL_ERR_CUDA: return "CUDA runtime error";
-        case PPL_ERR_UNSUPPORTED_DEVICE: return "no CUDA device of compute capability 10.x (no fallback path exists)";
-        case PPL_ERR_PRECONDITION: return "input violates a symmetry the plan relies on";
-        default: return "unknown error";
-    }
-}
-
-}  // extern "C"
-
-namespace {
-
-// The host half of ppl_plan: everything that follows from (nocc, nvirt, nchol), the byte budget `cap`, the SM count and
-// the kernel family alone -- packed geometry, row tiling of step 1, tile edge T, ring depth, buffer sizes.  No CUDA call.
-ppl_plan_s *plan_host(int nocc, int nvirt, int nchol, size_t workspace_bytes, size_t cap, int num_sms, bool use_tma,
-                      const ppl_debug_opts_t *dbg, int *rc_out) {
-    *rc_out = PPL_OK;
-    ppl_plan_s *p = new (std::nothrow) ppl_plan_s();
-    if (!p) {
-        *rc_out = PPL_ERR_ALLOC;
-        return nullptr;
-    }
-    if (dbg) p->dbg = *dbg;
-    p->o = nocc;
-    p->v = nvirt;
-    p->x = nchol;
-    p->num_sms = num_sms;
-    p->vec16 = (nvirt % 2 == 0) ? 1 : 0;
-    p->vv = (int64_t)nvirt * nvirt;
-    p->vp = nvirt + (nvirt & 1);
-    p->vvp = (int64_t)p->vp * p->vp;
-    p->cap = workspace_bytes;
-    p->Mp = nocc * (nocc + 1) / 2;
-    p->Mm = nocc * (nocc - 1) / 2;
-    p->KpT = p->vp * (p->vp + 1) / 2;         // packed geometry: nvirt rounded up to even (the pad index carries zeros)
-    p->KmT = p->vp * (p->vp - 1) / 2;
-    p->Kp = (int)ppl::kplus_extent(p->vp);   // extents of the packed index ranges, holes included (ppl_kernels.cuh)
-    p->Km = (int)ppl::kminus_extent(p->vp);
-    p->ldp = ((int64_t)p->Kp + 15) / 16 * 16;  // rows of the packed operands are 128-byte aligned: TMA-legal for any nvirt
-    p->ldm = ((int64_t)std::max(p->Km, 1) + 15) / 16 * 16;
-    p->use_tma = use_tma ? 1 : 0;
-    const int ni_env = (p->dbg.ni_max >= 1 && p->dbg.ni_max <= 10) ? p->dbg.ni_max : 10;  // largest row-tile instance used
-    const bool tma_full = p->use_tma && p->vec16;
-    p->mg_full = tma_full ? m_geom_tma(nocc * nocc, ni_env) : m_geom_plain(nocc * nocc);
-    p->mg_p = p->use_tma ? m_geom_tma(p->Mp, ni_env) : m_geom_plain(p->Mp);
-    p->mg_m = p->use_tma ? m_geom_tma(std::max(p->Mm, 1), ni_env) : m_geom_plain(std::max(p->Mm, 1));
-    p->bm_full = tma_full ? 16 * p->mg_full.ni : ppl::BM;
-    p->bm_p = p->use_tma ? 16 * p->mg_p.ni : ppl::BM;
-    p->bm_m = p->use_tma ? 16 * p->mg_m.ni : ppl::BM;
-    Geometry g{p->vv, nocc * nocc, p->Mp, p->Mm, p->Kp, p->Km, p->ldp, p->ldm, p->mg_full, p->mg_p, p->mg_m};
-    p->tau_bytes = align256((size_t)p->Mp * p->ldp * 8) + align256((size_t)std::max(p->Mm, 1) * p->ldm * 8);
-
-    // choose the tile edge T (and ring depth) that minimises the estimated apply time under the cap:
-    // first with the packed operands of PPL_SYM_PAIR_SA, and if they do not fit, without them
-    const int forced_T = p->dbg.tile_edge > 0 ? std::min(p->dbg.tile_edge, nvirt) : 0;  // debug override
-    double best_t = 1e300;
-    int best_T = 0, best_ring = 1, best_sa = 0;
-    PlanEval best_ev;
-    for (int sa = 1; sa >= 0 && best_T == 0; --sa)
-        for (int T = nvirt; T >= 1; --T) {
-            if (forced_T && T != forced_T) continue;
-            // only edges that tile v evenly or nearly so (ragged edge at least T/2), to keep edge tiles efficient
-            const int nblk = (nvirt + T - 1) / T;
-            const int r = nvirt - (nblk - 1) * T;
-            if (!forced_T && nblk > 1 && 2 * r < T) continue;
-            const PlanEval ev = evaluate(g, nocc, nvirt, nchol, T, sa != 0, p->num_sms);
-            const size_t fixed = ev.x_bytes + ev.part_bytes + (sa ? p->tau_bytes : 0) + 256;
-            int ring = 0;
-            for (int rg = std::min(3, MAX_RING); rg >= 1; --rg)
-                if (rg * ev.slot_bytes + fixed <= cap) {
-                    ring = rg;
-                    break;
-                }
-            if (ring == 0) continue;
-            const int ntiles = nblk * (nblk + 1) / 2;
-            ring = std::min(ring, std::max(1, ntiles));
-            const double t = ev.seconds * (ring >= 2 ? 1.0 : 1.03);
-            if (t < best_t) {
-                best_t = t;
-                best_T = T;
-                best_ring = ring;
-                best_ev = ev;
-                best_sa = sa;
-            }
-        }
-    if (best_T == 0) {
-        free_plan(p);
-        *rc_out = PPL_ERR_WORKSPACE_TOO_SMALL;
-        return nullptr;
-    }
-    p->T = best_T;
-    p->nblk = (nvirt + best_T - 1) / best_T;
-    p->ring = best_ring;
-    p->sa_ok = best_sa;
-    p->x_bytes = best_ev.x_bytes;
-    p->slot_bytes = best_ev.slot_bytes;
-    p->part_bytes = best_ev.part_bytes;
-    p->ws_bytes = p->x_bytes + p->ring * p->slot_bytes + p->part_bytes + (p->sa_ok ? p->tau_bytes : 0);
-    return p;
-}
-
-bool dims_ok(int nocc, int nvirt, int nchol) {
-    return nocc >= 1 && nvirt >= 1 && nchol >= 1 && (int64_t)nvirt * nvirt <= INT32_MAX / 2 && (int64_t)nocc * nocc <= INT32_MAX / 2;
-}
-
-int full_min_v(const ppl_plan_s *p) { return p->dbg.full_min_v > 0 ? p->dbg.full_min_v : 52; }
-
-}  // namespace
-
-extern "C" {
-
 ppl_plan_t *ppl_plan(int nocc, int nvirt, int nchol, size_t workspace_bytes) {
     return ppl_plan_ex(nocc, nvirt, nchol, workspace_bytes, nullptr);
 }
@@ -1608,7 +1000,9 @@ ppl_plan_t *ppl_plan_ex(int nocc, int nvirt, int nchol, size_t workspace_bytes, 
         fail(rc_host);
         return nullptr;
     }
-    if (cudaMalloc(&p->ws, p->ws_bytes) != cudaSuccess || cudaMalloc(&p->flags, sizeof(int)) != cudaSuccess) {
+    if (cudaMalloc(&p->ws, p->ws_bytes) != cudaSuccess || cudaMalloc(&p->flags, sizeof(int)) != cudaSuccess ||
+        cudaMalloc(&p->vflags, sizeof(int)) != cudaSuccess || cudaMallocHost(&p->vflags_host, sizeof(int)) != cudaSuccess ||
+        cudaEventCreateWithFlags(&p->ev_verify, cudaEventDisableTiming) != cudaSuccess) {
         (void)cudaGetLastError();
         free_plan(p);
         fail(PPL_ERR_ALLOC);
@@ -1682,142 +1076,10 @@ ppl_plan_t *ppl_plan_ex(int nocc, int nvirt, int nchol, size_t workspace_bytes, 
     // (below that the extra launches per slab cost more than the flops they save: measured crossover with
     // PPL_SYM_PAIR_SA at nocc = 5..8, nchol = 4 nvirt: 0.157 vs 0.186 ms at nvirt = 48, 0.283 vs 0.274 ms at 53,
     // 0.365 vs 0.328 ms at 64, 1.71 vs 0.97 ms at 96)
-    full_setup(p, cap > p->ws_bytes ? cap - p->ws_bytes : 0);
+    full_plan(p, cap > p->ws_bytes ? cap - p->ws_bytes : 0);
+    full_allocate(p);
     if (p->full_ok && nvirt >= full_min_v(p)) p->sym = PPL_SYM_FULL;
     return p;
-}
-
-// ppl_plan_dry: the planner alone, for a stated device (free bytes, SM count): no CUDA call, nothing allocated.
-int ppl_plan_dry(int nocc, int nvirt, int nchol, size_t workspace_bytes, size_t device_free_bytes, int num_sms, int mode,
-                 ppl_info_t *out) {
-    return ppl_plan_dry_ex(nocc, nvirt, nchol, workspace_bytes, device_free_bytes, num_sms, mode, nullptr, out);
-}
-
-int ppl_plan_dry_ex(int nocc, int nvirt, int nchol, size_t workspace_bytes, size_t device_free_bytes, int num_sms, int mode,
-                    const ppl_debug_opts_t *dbg, ppl_info_t *out) {
-    if (!out || !dims_ok(nocc, nvirt, nchol) || num_sms < 1 || mode < -1 || mode > PPL_SYM_FULL) return fail(PPL_ERR_INVALID_ARG);
-    const size_t auto_cap = (size_t)(0.9 * (double)device_free_bytes);
-    const size_t cap = workspace_bytes ? std::min(workspace_bytes, auto_cap) : auto_cap;
-    int rc = PPL_OK;
-    ppl_plan_s *p = plan_host(nocc, nvirt, nchol, workspace_bytes, cap, num_sms, !(dbg && dbg->cpasync_kernels), dbg, &rc);
-    if (!p) return fail(rc);
-    p->dry = 1;
-    p->sym = p->sa_ok ? PPL_SYM_PAIR_SA : PPL_SYM_PAIR;
-    rc = build_tiles(p);
-    if (rc == PPL_OK) {
-        full_setup(p, cap > p->ws_bytes ? cap - p->ws_bytes : 0, true);
-        if (p->full_ok && nvirt >= full_min_v(p)) p->sym = PPL_SYM_FULL;
-        if (mode >= 0) rc = ppl_plan_set_symmetry(p, mode);
-    }
-    if (rc == PPL_OK) rc = ppl_plan_info(p, out);
-    free_plan(p);
-    return rc == PPL_OK ? PPL_OK : fail(rc);
-}
-
-int ppl_plan_set_symmetry(ppl_plan_t *p, int mode) {
-    if (!p || (mode != PPL_SYM_NONE && mode != PPL_SYM_PAIR && mode != PPL_SYM_PAIR_SA && mode != PPL_SYM_FULL))
-        return fail(PPL_ERR_INVALID_ARG);
-    if (mode == PPL_SYM_PAIR_SA && !p->sa_ok) return fail(PPL_ERR_WORKSPACE_TOO_SMALL);
-    if (mode == PPL_SYM_FULL) {
-        if (!p->full_ok) return fail(PPL_ERR_WORKSPACE_TOO_SMALL);
-        p->sym = mode;  // the slab / tile lists were built by ppl_plan
-        return PPL_OK;
-    }
-    const int old = p->sym;
-    p->sym = mode;
-    const int rc = build_tiles(p);
-    if (rc != PPL_OK) {
-        p->sym = old;
-        build_tiles(p);
-        return fail(rc);
-    }
-    return PPL_OK;
-}
-
-int ppl_plan_info(const ppl_plan_t *p, ppl_info_t *out) {
-    if (!p || !out) return fail(PPL_ERR_INVALID_ARG);
-    memset(out, 0, sizeof(*out));
-    const bool sa = p->sym == PPL_SYM_PAIR_SA;
-    out->nocc = p->o;
-    out->nvirt = p->v;
-    out->nchol = p->x;
-    out->symmetry = p->sym;
-    out->ta = out->tb = p->T;
-    out->n_ablocks = out->n_bblocks = p->nblk;
-    out->n_tiles = (int)p->tiles.size();
-    out->ring = p->ring;
-    out->splitk = p->tiles.empty() ? 0 : (sa ? p->tiles[0].sp.splitk : p->tiles[0].full.splitk);
-    out->vec16 = p->vec16;
-    const bool minus = p->Mm > 0 && p->Km > 0;
-    out->launches_per_apply = sa ? 1 + (minus ? 5 : 4) * (int)p->tiles.size() : 3 * (int)p->tiles.size();
-    out->step1_tile_m = sa ? p->bm_p : p->bm_full;
-    out->workspace_bytes = p->ws_bytes;
-    const double v4 = std::pow((double)p->v, 4);
-    out->flops_nominal = 2.0 * p->x * v4 + 2.0 * p->o * p->o * v4;
-    out->flops_step0 = p->f_step0;
-    out->flops_step1 = p->f_step1;
-    out->flops_executed = p->f_step0 + p->f_step1;
-    out->sa_splitk_plus = p->tiles.empty() ? 0 : p->tiles[0].sp.splitk;
-    out->sa_splitk_minus = p->tiles.empty() ? 0 : p->tiles[0].sm.splitk;
-    out->sa_tile_m_plus = p->bm_p;
-    out->sa_tile_m_minus = p->bm_m;
-    out->sa_rows_plus = p->Mp;
-    out->sa_rows_minus = p->Mm;
-    out->sa_k_plus = p->KpT;
-    out->sa_k_minus = p->KmT;
-    {   // useful flops of the mode (include/ppl.h): exact pair counts, no padding, no zero rows, no overshoot
-        const double v = p->v, P2 = v * (v + 1) / 2, Q2 = v * (v - 1) / 2, M = (double)p->o * p->o;
-        const double Mp = p->Mp, Mm = p->Mm;
-        switch (p->sym) {
-            case PPL_SYM_FULL:
-                out->flops_useful_step0 = 2.0 * p->x * P2 * (P2 + 1) / 2;
-                out->flops_useful_step1 = 2.0 * (Mp * P2 * P2 + Mm * Q2 * Q2);
-                break;
-            case PPL_SYM_PAIR_SA:
-                out->flops_useful_step0 = 2.0 * p->x * v * v * P2;
-                out->flops_useful_step1 = 2.0 * (Mp * P2 + Mm * Q2) * P2;
-                break;
-            case PPL_SYM_PAIR:
-                out->flops_useful_step0 = 2.0 * p->x * v * v * P2;
-                out->flops_useful_step1 = 2.0 * M * v * v * P2;
-                break;
-            default:
-                out->flops_useful_step0 = 2.0 * p->x * v4;
-                out->flops_useful_step1 = 2.0 * M * v4;
-        }
-        out->flops_useful = out->flops_useful_step0 + out->flops_useful_step1;
-    }
-    out->full_available = p->full_ok;
-    out->full_tbg = p->tbg;
-    out->full_slabs = (int)p->slabs.size();
-    out->full_tight = p->full_ok ? p->full_tight : 0;
-    out->full_workspace_bytes = p->fws_bytes;
-    out->workspace_bytes = p->ws_bytes + p->fws_bytes;
-    if (p->sym == PPL_SYM_FULL) {
-        out->ta = ppl::TA_FULL;
-        out->tb = p->tbg;
-        out->n_ablocks = (int)p->slabs.size();
-        out->n_bblocks = p->slabs.empty() ? 0 : p->slabs[0].tile_end - p->slabs[0].tile_begin;
-        out->n_tiles = (int)p->ftiles.size();
-        out->ring = 1;
-        out->splitk = p->ftiles.empty() ? 0 : p->ftiles[0].sp.splitk;
-        // pack, unpack, one step 0 per slab -- per tile in the memory-tight mode -- (+ the L pad copy for odd nvirt)
-        int launches = 2 + (int)(p->full_tight ? p->ftiles.size() : p->slabs.size()) + ((p->v & 1) ? 1 : 0) +
-                       ((p->diag_pack && !p->full_tight) ? 1 : 0);
-        for (const FullTile &t : p->ftiles) {
-            const int Nm = t.range ? t.nm : ppl::TA_FULL * t.tbp;
-            const bool m1 = minus && p->Km - t.k0m > 0 && Nm > 0;
-            launches += 1 + (m1 ? 4 : 2) + (p->Kp - t.k1p > 0 ? 1 : 0) + (minus && p->Km - t.k1m > 0 && Nm > 0 ? 1 : 0);
-        }
-        out->launches_per_apply = launches;
-        out->step1_tile_m = p->bm_p;
-        out->flops_step0 = p->ff_step0;
-        out->flops_step1 = p->ff_step1;
-        out->flops_executed = p->ff_step0 + p->ff_step1;
-        out->sa_splitk_plus = p->ftiles.empty() ? 0 : p->ftiles[0].sp.splitk;
-        out->sa_splitk_minus = p->ftiles.empty() ? 0 : p->ftiles[0].sm.splitk;
-    }
-    return PPL_OK;
 }
 
 int ppl_apply(ppl_plan_t *p, const double *L, const double *t2, double *R, void *stream) {
@@ -1837,12 +1099,6 @@ int apply_direct(ppl_plan_s *p, const double *L, const double *t2, double *R, co
 // symmetry mode, and replayed with one cudaGraphLaunch while the key stays the same (a CCSD iteration
 // calls the ladder on the same buffers).  A new key re-captures (the TMA descriptors of L and t2 are
 // kernel parameters, so the nodes cannot simply be re-pointed).
-bool graph_wanted(const ppl_plan_s *p) {
-    if (p->graph_mode >= 0) return p->graph_mode == 1;
-    const double f = p->sym == PPL_SYM_FULL ? p->ff_step0 + p->ff_step1 : p->f_step0 + p->f_step1;
-    return f < GRAPH_AUTO_FLOPS;
-}
-
 int apply_graph(ppl_plan_s *p, const double *L, const double *t2, double *R, const ppl_opts_t *opts_in, cudaStream_t stream) {
     ppl_opts_t opts;
     bool vec16;
@@ -1888,22 +1144,26 @@ int apply_graph(ppl_plan_s *p, const double *L, const double *t2, double *R, con
 
 int ppl_apply_ex(ppl_plan_t *p, const double *L, const double *t2, double *R, const ppl_opts_t *opts, void *stream_) {
     cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
-    if (p && graph_wanted(p)) {
-        // a caller who is capturing `stream` gets the plain launches recorded into their own graph
-        cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
-        if (cudaStreamIsCapturing(stream, &st) != cudaSuccess) {
-            (void)cudaGetLastError();
-            st = cudaStreamCaptureStatusActive;
+    if (!p || !L || !t2 || !R) return fail(PPL_ERR_INVALID_ARG);
+    // a caller who is capturing `stream` gets the plain launches recorded into their own graph (and no input check:
+    // its result could not be read back during the capture)
+    cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(stream, &st) != cudaSuccess) {
+        (void)cudaGetLastError();
+        st = cudaStreamCaptureStatusActive;
+    }
+    if (st == cudaStreamCaptureStatusNone) {
+        int rc = verify_harvest(p, nullptr);  // what the previous apply's check found
+        if (rc != PPL_OK) return rc;
+        if (p->verify && p->sym != PPL_SYM_NONE) {
+            ppl_opts_t o;
+            if (check_opts(opts, &o) != PPL_OK) return fail(PPL_ERR_INVALID_ARG);
+            rc = verify_begin(p, p->sym == PPL_SYM_FULL ? L : nullptr, t2, o.t2_layout, stream);
+            if (rc != PPL_OK) return rc;
         }
-        if (st == cudaStreamCaptureStatusNone) return apply_graph(p, L, t2, R, opts, stream);
+        if (graph_wanted(p)) return apply_graph(p, L, t2, R, opts, stream);
     }
     return apply_direct(p, L, t2, R, opts, stream);
-}
-
-int ppl_plan_set_graph(ppl_plan_t *p, int mode) {
-    if (!p || mode < -1 || mode > 1) return fail(PPL_ERR_INVALID_ARG);
-    p->graph_mode = mode;
-    return PPL_OK;
 }
 
 int ppl_apply_profiled(ppl_plan_t *p, const double *L, const double *t2, double *R, void *stream_, ppl_times_t *times) {
@@ -2018,7 +1278,7 @@ int ppl_generate_eri(ppl_plan_t *p, const double *L, int a0, int na, double *eri
 // the packed operands, and R+-acc is unpacked chunk by chunk into the staging buffers (R chunk in, result out).
 // Device residency: L + tau+- + R+-acc + the PPL_SYM_FULL workspace -- about half of L + t2 + R + workspace, which
 // is what lets the paper's Table 3 shapes (t2 and R of 39 GB each at N = 800) run on one 180 GB GPU.
-static int apply_host_full(ppl_plan_s *p, const double *Lh, const double *t2h, double *Rh, uint64_t *h2d, uint64_t *d2h) {
+static int apply_host_full_queue(ppl_plan_s *p, const double *Lh, const double *t2h, double *Rh, uint64_t *h2d, uint64_t *d2h) {
     const size_t nL = (size_t)p->x * p->vv * 8;
     const int64_t rows = (int64_t)p->o * p->o;
     const size_t row_bytes = (size_t)p->vv * 8;
@@ -2057,6 +1317,10 @@ static int apply_host_full(ppl_plan_s *p, const double *Lh, const double *t2h, d
     const int64_t nchunks = (rows + p->hchunk_rows - 1) / p->hchunk_rows;
     // phase A: L in on the compute stream; t2 chunks in -> tau+- on the chunk streams, overlapping L and step 0 of slab 0
     PPL_CUDA(cudaMemcpyAsync(p->dL, Lh, nL, cudaMemcpyHostToDevice, cs));
+    if (p->verify) {  // L only: t2 never sits on the device whole (include/ppl.h, PPL_OPT_VERIFY_INPUTS)
+        const int rcv = verify_begin(p, p->dL, nullptr, PPL_LAYOUT_IJAB, cs);
+        if (rcv != PPL_OK) return rcv;
+    }
     PPL_CUDA(cudaMemsetAsync(p->raccp, 0, (size_t)p->Mp * p->ldp * 8, cs));
     if (minus) PPL_CUDA(cudaMemsetAsync(p->raccm, 0, (size_t)p->Mm * p->ldm * 8, cs));
     int k = 0;
@@ -2102,7 +1366,19 @@ static int apply_host_full(ppl_plan_s *p, const double *Lh, const double *t2h, d
     const uint64_t nT = (uint64_t)rows * row_bytes;
     if (h2d) *h2d = (uint64_t)nL + 2 * nT;
     if (d2h) *d2h = nT;
-    return PPL_OK;
+    return verify_harvest(p, nullptr);
+}
+
+// An error half way leaves copies and kernels in flight on three streams that read and write the caller's host buffers:
+// wait for them before the error is returned, so that the caller may free or reuse its buffers.
+static int apply_host_full(ppl_plan_s *p, const double *Lh, const double *t2h, double *Rh, uint64_t *h2d, uint64_t *d2h) {
+    const int rc = apply_host_full_queue(p, Lh, t2h, Rh, h2d, d2h);
+    if (rc != PPL_OK) {
+        for (cudaStream_t st : {p->gen, p->hs2, p->host_stream})
+            if (st && cudaStreamSynchronize(st) != cudaSuccess) (void)cudaGetLastError();
+        p->verify_pending = 0;
+    }
+    return rc;
 }
 
 int ppl_apply_host(ppl_plan_t *p, const double *Lh, const double *t2h, double *Rh, uint64_t *h2d, uint64_t *d2h) {
@@ -2129,6 +1405,7 @@ int ppl_apply_host(ppl_plan_t *p, const double *Lh, const double *t2h, double *R
     PPL_CUDA(cudaMemcpyAsync(p->dT, t2h, nT, cudaMemcpyHostToDevice, s));
     PPL_CUDA(cudaMemcpyAsync(p->dR, Rh, nT, cudaMemcpyHostToDevice, s));
     int rc = ppl_apply(p, p->dL, p->dT, p->dR, s);
+    if (rc != PPL_OK && cudaStreamSynchronize(s) != cudaSuccess) (void)cudaGetLastError();  // the queued H2D copies read the caller's buffers
     if (rc == PPL_OK) {
         cudaError_t e = cudaMemcpyAsync(Rh, p->dR, nT, cudaMemcpyDeviceToHost, s);
         if (e == cudaSuccess) e = cudaStreamSynchronize(s);
@@ -2139,15 +1416,68 @@ int ppl_apply_host(ppl_plan_t *p, const double *Lh, const double *t2h, double *R
     }
     if (h2d) *h2d = (uint64_t)nL + 2 * (uint64_t)nT;
     if (d2h) *d2h = (uint64_t)nT;
+    if (rc == PPL_OK) rc = verify_harvest(p, nullptr);  // the call has synchronised: report a violated precondition at once
     return rc;
 }
+
+}  // extern "C"
+
+namespace {
+
+int launch_check(const ppl_plan_s *p, const double *L, const double *t2, int t2_layout, int *dflags, cudaStream_t stream) {
+    ppl::CheckArgs a;
+    a.L = L;
+    a.t2 = t2;
+    a.o = p->o;
+    a.v = p->v;
+    a.x = p->x;
+    const ppl::RStrides ts = r_strides(p->o, p->v, t2_layout);
+    a.s_i = ts.i;
+    a.s_j = ts.j;
+    a.s_c = ts.a;
+    a.flags = dflags;
+    PPL_CUDA(cudaMemsetAsync(dflags, 0, sizeof(int), stream));
+    ppl::k_check_inputs<<<p->num_sms * 8, 256, 0, stream>>>(a);
+    PPL_CUDA(cudaGetLastError());
+    return PPL_OK;
+}
+
+// result of the pending per-apply verification, if any (waits for that head-of-apply kernel only)
+int verify_harvest(ppl_plan_s *p, int *flags_out) {
+    if (flags_out) *flags_out = 0;
+    if (!p->verify_pending) return PPL_OK;
+    p->verify_pending = 0;
+    if (cudaEventSynchronize(p->ev_verify) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return fail(PPL_ERR_CUDA);
+    }
+    const int h = *p->vflags_host;
+    if (flags_out) *flags_out = h;
+    if ((h & 2) && p->sym != PPL_SYM_NONE) return fail(PPL_ERR_PRECONDITION);
+    if ((h & 1) && p->sym == PPL_SYM_FULL) return fail(PPL_ERR_PRECONDITION);
+    return PPL_OK;
+}
+
+// queue the check of this apply's inputs on `stream` (L == nullptr / t2 == nullptr: not checked)
+int verify_begin(ppl_plan_s *p, const double *L, const double *t2, int t2_layout, cudaStream_t stream) {
+    int rc = launch_check(p, L, t2, t2_layout, p->vflags, stream);
+    if (rc != PPL_OK) return rc;
+    PPL_CUDA(cudaMemcpyAsync(p->vflags_host, p->vflags, sizeof(int), cudaMemcpyDeviceToHost, stream));
+    PPL_CUDA(cudaEventRecord(p->ev_verify, stream));
+    p->verify_pending = 1;
+    if (p->verify == 2) return verify_harvest(p, nullptr);
+    return PPL_OK;
+}
+
+}  // namespace
+
+extern "C" {
 
 int ppl_check_inputs(ppl_plan_t *p, const double *L, const double *t2, void *stream_, int *flags) {
     if (!p || !L || !t2) return fail(PPL_ERR_INVALID_ARG);
     cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
-    PPL_CUDA(cudaMemsetAsync(p->flags, 0, sizeof(int), stream));
-    ppl::k_check_inputs<<<p->num_sms * 8, 256, 0, stream>>>(L, t2, p->o, p->v, p->x, p->flags);
-    PPL_CUDA(cudaGetLastError());
+    const int rc = launch_check(p, L, t2, PPL_LAYOUT_IJAB, p->flags, stream);
+    if (rc != PPL_OK) return rc;
     int h = 0;
     PPL_CUDA(cudaMemcpyAsync(&h, p->flags, sizeof(int), cudaMemcpyDeviceToHost, stream));
     PPL_CUDA(cudaStreamSynchronize(stream));
@@ -2157,10 +1487,16 @@ int ppl_check_inputs(ppl_plan_t *p, const double *L, const double *t2, void *str
     return PPL_OK;
 }
 
+int ppl_plan_verify_status(ppl_plan_t *p, int *flags) {
+    if (!p) return fail(PPL_ERR_INVALID_ARG);
+    return verify_harvest(p, flags);
+}
+
 int ppl_destroy(ppl_plan_t *p) {
     if (!p) return PPL_OK;
+    const int rc = p->dry ? PPL_OK : verify_harvest(p, nullptr);  // a violation found by the last apply's check is not lost
     free_plan(p);
-    return PPL_OK;
+    return rc;
 }
 
 int ppl_probe_fp64_pipe(int kind, double *tflops, int reps, double ms_target) {

@@ -298,13 +298,27 @@ bool pairs_ok(const int64_t *run, int64_t nrun, const int64_t *other, int64_t no
 
 size_t table_bytes(const Parsed &ps) { return (size_t)(2 * ps.M + 2 * ps.N + 2 * ps.K) * sizeof(int64_t); }
 
+// split-K factor: the estimated time of the launch -- whole waves of CTA tiles on `sms` SMs, each (k-tiles + pipeline
+// fill) long, plus writing and re-reading the partials -- minimised over the factors whose partials fit into `room`
 int pick_splitk(const Parsed &ps, int sms, size_t room) {
     const int64_t tiles = ((ps.M + ppl::BM - 1) / ppl::BM) * ((ps.N + ppl::BN - 1) / ppl::BN);
     const int64_t nkt = (ps.K + ppl::BK - 1) / ppl::BK;
-    int64_t s = std::min<int64_t>((2 * sms + tiles - 1) / tiles, nkt / 8);  // about two waves, at least 8 k-tiles per split
-    s = std::max<int64_t>(1, std::min<int64_t>(s, 64));
-    while (s > 1 && (size_t)s * ps.M * ps.N * 8 > room) --s;
-    return (int)s;
+    const double tau = 2.0 * ppl::BM * ppl::BN * ppl::BK / (37.2e12 / sms);  // one k-tile on one SM
+    int best = 1;
+    double best_t = 1e300;
+    const int64_t smax = std::max<int64_t>(1, std::min<int64_t>(nkt / 8, 64));
+    for (int64_t s = 1; s <= smax; ++s) {
+        const int64_t kt_per = (nkt + s - 1) / s;
+        if ((nkt + kt_per - 1) / kt_per != s) continue;  // no empty splits
+        if (s > 1 && (size_t)s * ps.M * ps.N * 8 > room) break;
+        const double waves = (double)((tiles * s + sms - 1) / sms);
+        const double t = waves * (kt_per + 6) * tau + (s > 1 ? (double)(s + 2) * ps.M * ps.N * 8.0 / 6.0e12 + 4e-6 : 0.0);
+        if (t < best_t) {
+            best_t = t;
+            best = (int)s;
+        }
+    }
+    return best;
 }
 
 }  // namespace

@@ -5,11 +5,10 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "ppl_layout.h"
+
 namespace ppl {
 
-constexpr int BM = 128;      // CTA tile rows
-constexpr int BN = 128;      // CTA tile cols
-constexpr int BK = 16;       // k per pipeline stage
 constexpr int STAGES = 4;    // cp.async ring depth
 constexpr int NTHREADS = 256;
 constexpr int WARPS_N = 4;   // 2 (m) x 4 (n) warps, warp tile 64 x 32

@@ -316,24 +316,6 @@ __global__ void __launch_bounds__(256) k_reduce(const ReduceArgs p) {
 //   R+- = tau+- W+-^T ;  R[i,j,a,b] = R+ + R- ;  R[j,i,a,b] = R+ - R-
 // Both packings are the same gather: k_symfold does either (scale 1 for W, 1/2 for tau).
 // ---------------------------------------------------------------------------------------------
-// Packed column index of the pair (c <= d) / (c < d).  Row c of the triangle is placed so that the index of
-// (c,d) has the parity of d (one unused "hole" element every other row; holes are zero in tau+- for good:
-// the buffers are cleared once at plan time and no kernel writes a hole).  This makes every run
-// (c, d0..d0+15) with d0 even start at an even index, i.e. at a 16-byte aligned address: TMA boxes must
-// start 16-byte aligned (an odd FP64 coordinate raises an illegal-instruction error), and PPL_SYM_FULL reads
-// such runs of tau+- as k-tiles.  In the minus triangle the element before (c, c+1), c even, is a hole.
-__host__ __device__ __forceinline__ int64_t kplus(int c, int d, int v) {
-    return (int64_t)c * v - (int64_t)c * (c + 1) / 2 + (c + 1) / 2 + d;
-}
-__host__ __device__ __forceinline__ int64_t kminus(int c, int d, int v) {
-    return (int64_t)c * (2 * v - c - 1) / 2 - c + c / 2 + d;
-}
-__host__ __device__ __forceinline__ int64_t kplus_extent(int v) { return kplus(v - 1, v - 1, v) + 1; }
-__host__ __device__ __forceinline__ int64_t kminus_extent(int v) { return v >= 2 ? kminus(v - 2, v - 1, v) + 1 : 0; }
-// packed row index of the occupied pair (i <= j) / (i < j): dense, no holes
-__host__ __device__ __forceinline__ int64_t rowplus(int i, int j, int o) { return (int64_t)i * o - (int64_t)i * (i - 1) / 2 + (j - i); }
-__host__ __device__ __forceinline__ int64_t rowminus(int i, int j, int o) { return (int64_t)i * (2 * o - i - 1) / 2 + (j - i - 1); }
-
 struct FoldArgs {
     const double *src;   // row r, element (c,d) at src + roff(r) + c*sc + d   (d contiguous)
     int64_t sc;          // stride of c
@@ -546,25 +528,78 @@ __global__ void __launch_bounds__(256) k_permute_t2(const double *src, double *d
 }
 
 // ---------------------------------------------------------------------------------------------
-// debug: input symmetry check.  flags bit 0: L[P,a,c] != L[P,c,a]; bit 1: t2[i,j,c,d] != t2[j,i,d,c]
+// Input symmetry check (the preconditions of the symmetric modes; PAPER.md:66 for L).
+// flags bit 0: L[P,a,c] != L[P,c,a]; bit 1: t2[i,j,c,d] != t2[j,i,d,c].
+// Work items: for L one (P; 32 x 32 block pair ab <= cb), for t2 one (i <= j; block pair (cb, db)).  Each item loads a
+// block and its partner, both along their contiguous index, and compares them through a shared-memory transpose, so
+// every global read is coalesced: the check moves |L| + |t2| bytes once at HBM speed (large: 4 GB, ~0.7 ms).
 // ---------------------------------------------------------------------------------------------
-__global__ void k_check_inputs(const double *L, const double *t2, int o, int v, int x, int *flags) {
-    const int64_t vv = (int64_t)v * v, nL = (int64_t)x * vv, nT = (int64_t)o * o * vv;
+struct CheckArgs {
+    const double *L, *t2;  // either may be null (not checked)
+    int o, v, x;
+    int64_t s_i, s_j, s_c;  // element strides of t2[i][j][c][.] (d contiguous) in the caller's storage order
+    int *flags;
+};
+__global__ void __launch_bounds__(256) k_check_inputs(const CheckArgs p) {
+    __shared__ double sb[32][33];
+    const int nb = (p.v + 31) / 32;
+    const int64_t npair = (int64_t)nb * (nb + 1) / 2, nsq = (int64_t)nb * nb;
+    const int64_t itemsL = p.L ? (int64_t)p.x * npair : 0;
+    const int64_t itemsT = p.t2 ? (int64_t)p.o * (p.o + 1) / 2 * nsq : 0;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     int f = 0;
-    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < nL + nT; idx += (int64_t)gridDim.x * blockDim.x) {
-        if (idx < nL) {
-            const int64_t P = idx / vv, r = idx - P * vv;
-            const int a = (int)(r / v), c = (int)(r - (int64_t)a * v);
-            if (L[idx] != L[P * vv + (int64_t)c * v + a]) f |= 1;
+    for (int64_t item = blockIdx.x; item < itemsL + itemsT; item += gridDim.x) {
+        const double *A, *B;  // block of A at (r0, c0) is compared with the transpose of the block of B at (c0, r0)
+        int64_t lda, ldb;
+        int r0, c0, bit;
+        bool diag;
+        if (item < itemsL) {
+            const int64_t P = item / npair;
+            int rem = (int)(item - P * npair), rb = 0;
+            while (rem >= nb - rb) {
+                rem -= nb - rb;
+                ++rb;
+            }
+            A = B = p.L + P * (int64_t)p.v * p.v;
+            lda = ldb = p.v;
+            r0 = rb * 32;
+            c0 = (rb + rem) * 32;
+            bit = 1;
+            diag = rem == 0;
         } else {
-            const int64_t e = idx - nL;
-            const int64_t ij = e / vv, r = e - ij * vv;
-            const int i = (int)(ij / o), j = (int)(ij - (int64_t)i * o);
-            const int c = (int)(r / v), d = (int)(r - (int64_t)c * v);
-            if (t2[e] != t2[((int64_t)j * o + i) * vv + (int64_t)d * v + c]) f |= 2;
+            const int64_t e = item - itemsL, ij = e / nsq;
+            const int blk = (int)(e - ij * nsq);
+            int i = 0;
+            int64_t rem = ij;
+            while (rem >= p.o - i) {
+                rem -= p.o - i;
+                ++i;
+            }
+            const int j = i + (int)rem;
+            A = p.t2 + i * p.s_i + j * p.s_j;
+            B = p.t2 + j * p.s_i + i * p.s_j;
+            lda = ldb = p.s_c;
+            r0 = (blk / nb) * 32;
+            c0 = (blk % nb) * 32;
+            bit = 2;
+            diag = false;
+        }
+        __syncthreads();  // the previous item's reads of sb are done
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int y = ty + 8 * k, r = c0 + y, c = r0 + tx;  // partner block: rows c0.., columns r0..
+            sb[y][tx] = (r < p.v && c < p.v) ? __ldg(B + (int64_t)r * ldb + c) : 0.0;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int y = ty + 8 * k, r = r0 + y, c = c0 + tx;
+            if (r < p.v && c < p.v && !(diag && c < r)) {
+                if (__ldg(A + (int64_t)r * lda + c) != sb[tx][y]) f |= bit;
+            }
         }
     }
-    if (f) atomicOr(flags, f);
+    if (f) atomicOr(p.flags, f);
 }
 
 // ---------------------------------------------------------------------------------------------

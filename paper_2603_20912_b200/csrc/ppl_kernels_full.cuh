@@ -22,7 +22,6 @@
 
 namespace ppl {
 
-constexpr int TA_FULL = 16;  // a-block edge of PPL_SYM_FULL: one TMA box row of L, one k-tile of use 2
 
 // ---------------------------------------------------------------------------------------------
 // step 0 of one slab.  mapL as in k_step0_tma: {inner = nvirt^2, outer = nchol}, box {16, BK}.
@@ -30,22 +29,6 @@ constexpr int TA_FULL = 16;  // a-block edge of PPL_SYM_FULL: one TMA box row of
 // Column tile tn: 8 boxes, box j <-> chunk 8 tn + j of the slab's chunk table: (b, d0) -> coordinate
 // b*v + d0 (16 d's of L[P][b][.]); b < 0 marks padding.  Chunks of one b start at its own 16-block.
 // ---------------------------------------------------------------------------------------------
-// Diagonal (b-block == d-block) 16 x 16 blocks of L, packed: only the pairs b_l <= d_l are needed there (the rest is their
-// b<->d image), 136 of 256.  k_pack_diag copies them once per apply into Lq[P][blk * 144 + t], t = the row-major index of
-// (b_l <= d_l) in the triangle (row b_l holds 16 - b_l entries; t = 136..143 are zero padding): 9 TMA chunks of 16 columns
-// per block instead of 16.  Chunk-table entry of a packed chunk: x = -2 - blk, y = its inner coordinate in Lq.
-constexpr int DIAG_PACKED = 144, DIAG_PAIRS = 136;
-__host__ __device__ __forceinline__ bool diag_unpack(int t, int &bl, int &dl) {
-    if (t >= DIAG_PAIRS) return false;
-    bl = 0;
-    int off = 0;
-    while (t - off >= 16 - bl) {
-        off += 16 - bl;
-        ++bl;
-    }
-    dl = bl + (t - off);
-    return true;
-}
 __global__ void __launch_bounds__(256) k_pack_diag(const double *__restrict__ L, double *__restrict__ Lq, int x, int v, int nfull,
                                                   int64_t ldq) {
     const int64_t per_p = (int64_t)nfull * DIAG_PACKED, total = (int64_t)x * per_p;

@@ -28,7 +28,7 @@ def gpu_contract(subs, A, B, C0=None, alpha=1.0, beta=0.0, offset=0, workspace_b
 
     Ad, Bd = dev(A), dev(B)
     Cd = None if C0 is None else dev(C0)
-    ws = None if workspace_bytes is None else torch.empty(workspace_bytes + 256, dtype=torch.uint8, device="cuda")
+    ws = None if workspace_bytes is None else torch.empty(workspace_bytes, dtype=torch.uint8, device="cuda")  # 512-byte aligned
     out = P.ppl_contract_pair(subs, Ad, Bd, Cd, alpha=alpha, beta=beta, workspace=ws)
     torch.cuda.synchronize()
     return out.cpu().numpy()
@@ -46,8 +46,9 @@ CASES = [
     ("abcd,ecfd->efab", (6, 7, 20, 22), (5, 20, 5, 22)),
     ("abcd,efcd->efab", (12, 13, 9, 10), (4, 6, 9, 10)),
     ("acbd,efcd->efab", (5, 11, 6, 13), (3, 4, 11, 13)),
-    # a Cholesky factor against an amplitude; summed letter in the middle of op1
-    ("xac,icjd->xajd", (9, 8, 14), (6, 14, 7, 10)),
+    # a Cholesky factor against an amplitude; the summed letter in the middle of op1, five surviving letters
+    ("xac,icjd->xaijd", (9, 8, 14), (6, 14, 7, 10)),
+    ("xac,icjd->ijxad", (9, 8, 14), (6, 14, 7, 10)),
     # plain matrix products in all four storage combinations (unit-stride letter summed or surviving, per operand)
     ("ik,kj->ij", (150, 70), (70, 140)),
     ("ki,kj->ij", (70, 150), (70, 140)),
@@ -75,7 +76,7 @@ def test_parity_with_the_oracle(subs, sa, sb):
     assert relerr(gpu_contract(subs, A, B, offset=1), want) <= TOL
 
 
-@pytest.mark.parametrize("subs,sa,sb", CASES[:8] + CASES[-2:])
+@pytest.mark.parametrize("subs,sa,sb", CASES[:9] + CASES[-2:])
 def test_exact_integers_bit_for_bit(subs, sa, sb):
     A, B = _rand(sa, 3, integer=True), _rand(sb, 4, integer=True)
     want = oracle.contract_pair(subs, A, B)
@@ -132,6 +133,8 @@ def test_workspace_rules_and_malformed_requests():
         gpu_contract("ik,jk->ij", A, B, workspace_bytes=tables - 256)
     assert e.value.code == P.PPL_ERR_WORKSPACE_TOO_SMALL
     Ad, Bd = torch.zeros((3, 3), dtype=torch.float64, device="cuda"), torch.zeros((3, 3), dtype=torch.float64, device="cuda")
+    # not of tensordot type: no '->', a repeated letter, three operands, a batch letter (in all three), a letter summed
+    # inside one operand only
     for bad in ("ab,bc", "aa,ab->b", "ab,bc,cd->ad", "ab,bc->abc", "ab,ab->ab", "ab,cd->ac"):
         with pytest.raises((P.PplError, KeyError, ValueError)):
             P.ppl_contract_pair(bad, Ad, Bd)

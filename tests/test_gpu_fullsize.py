@@ -9,7 +9,9 @@ The full oracle is unaffordable there (large: 164 TFLOP, XL: 1.56 PFLOP on CPU),
        (long double): every entry of R takes part, so a missing, duplicated or mis-mirrored tile
        is caught; bound 1e-11 * max|R| * sum|u_a| sum|w_b|;
   P9   exact small-integer inputs: sampled columns must match bit for bit (medium; large in the default mode).
-Medium can also be compared in full: PPL_FULL_ORACLE=1 (minutes of CPU).
+Medium is compared with the FULL oracle, every entry, in all three modes (about a minute of CPU for the one oracle call;
+PPL_SKIP_FULL_ORACLE=1 skips it).  Every-entry checks at large and XL that need no oracle run (closed forms P3, P4 and
+the tagged L == 1 case) are in tests/test_gpu_fullsize_closed_forms.py.
 """
 import os
 
@@ -97,6 +99,16 @@ def _check_projections(L, t2, Rd, rmax, nrand=2):
         assert np.abs(got - want).max() <= bound, (np.abs(got - want).max(), bound)
 
 
+_FULL_MEDIUM = {}
+
+
+def _medium_full_oracle(L, t2):
+    """oracle.full at medium (3.84 TFLOP of plain loops), once per session."""
+    if "want" not in _FULL_MEDIUM:
+        _FULL_MEDIUM["want"] = oracle.full(L, t2)
+    return _FULL_MEDIUM["want"]
+
+
 @pytest.mark.parametrize("sym", [None, P.PPL_SYM_PAIR_SA, P.PPL_SYM_PAIR])
 def test_medium_sampled_columns_and_projections(sym):
     L, t2, Rd, info = _run("medium", sym=sym)
@@ -106,8 +118,8 @@ def test_medium_sampled_columns_and_projections(sym):
     _check_projections(L, t2, Rd, rmax)
     # pair symmetry of the result (mirror bookkeeping), exact on off-diagonal tiles, to rounding on diagonal ones
     assert float((Rd - Rd.permute(1, 0, 3, 2)).abs().max().item()) <= TOL * rmax
-    if os.environ.get("PPL_FULL_ORACLE") == "1":
-        want = oracle.full(L, t2)
+    if os.environ.get("PPL_SKIP_FULL_ORACLE") != "1":  # full element-wise comparison on configs 0-2
+        want = _medium_full_oracle(L, t2)
         assert np.abs(Rd.cpu().numpy() - want).max() <= TOL * np.abs(want).max()
 
 
@@ -173,5 +185,5 @@ def test_xl_sampled_columns_and_projections():
         pytest.skip("not enough host/device memory for the XL config")
     L, t2, Rd, info = _run("xl")
     rmax = float(Rd.abs().max().item())
-    _check_columns(L, t2, Rd, 40)
+    _check_columns(L, t2, Rd, 256)  # K ~ 256 at XL (about 340 columns with the fixed set and the transposes)
     _check_projections(L, t2, Rd, rmax, nrand=1)

@@ -239,3 +239,30 @@ def test_other_sm_counts_and_bad_arguments(sms):
         P.ppl_plan_dry(5, 20, 60, num_sms=0)
     with pytest.raises(P.PplError):
         P.ppl_plan_dry(5, 20, 60, mode=7)
+
+
+def test_planner_builds_with_gpp_alone_and_agrees_with_the_library(tmp_path):
+    """csrc/ppl_plan.cpp is plain C++: no nvcc, no CUDA call, no link dependency (CUDA headers serve as type definitions
+    only).  Built here with g++ into a library of its own, ppl_plan_dry gives the same answers as the one inside libppl.so."""
+    import ctypes
+    import os
+    import shutil
+    import subprocess
+
+    from paper_2603_20912_b200 import _build
+    from paper_2603_20912_b200.binding import ppl_info_t
+
+    gpp = shutil.which("g++")
+    inc = os.path.join(os.path.dirname(_build.nvcc()), "..", "include")
+    so = str(tmp_path / "libppl_plan_only.so")
+    subprocess.check_call([gpp, "-std=c++17", "-O2", "-shared", "-fPIC", "-I", inc, "-o", so, "ppl_plan.cpp"], cwd=_build.CSRC)
+    assert "libcudart" not in subprocess.check_output(["ldd", so], text=True)
+    lib = ctypes.CDLL(so)
+    lib.ppl_plan_dry.restype = ctypes.c_int
+    lib.ppl_plan_dry.argtypes = [ctypes.c_int] * 3 + [ctypes.c_size_t] * 2 + [ctypes.c_int] * 2 + [ctypes.POINTER(ppl_info_t)]
+    for shape in ((5, 20, 60), (5, 53, 232), (20, 200, 800), (60, 600, 2400)):
+        for cap in (0, 6 << 30):
+            out = ppl_info_t()
+            rc = lib.ppl_plan_dry(*shape, cap, 170 << 30, 148, -1, ctypes.byref(out))
+            assert rc == P.PPL_OK
+            assert out.asdict() == P.ppl_plan_dry(*shape, workspace_bytes=cap)
