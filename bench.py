@@ -498,10 +498,13 @@ def run_ours(name, o, v, x, args, steps, warmup, dist, dev, rank, world, peak):
     prof = plan.apply_profiled(Ld, td, Rd)  # Rd now holds exactly one application of the term
     torch.cuda.synchronize()
     dom = "step0" if prof["step0_ms"] >= prof["step1_ms"] else "step1"
-    dom_flops = info["flops_" + dom] / max(prof["n_" + dom], 1)
+    fused = bool(info.get("small_fused"))
+    # the one-kernel path of launch-bound shapes does both steps in its single launch (timed as "step0")
+    dom_total = info["flops_executed"] if fused else info["flops_" + dom]
+    dom_flops = dom_total / max(prof["n_" + dom], 1)
     dom_ms = prof[dom + "_ms"] / max(prof["n_" + dom], 1)
     achieved = dom_flops / (dom_ms * 1e-3) * 1e-12
-    dom_useful = info["flops_useful_" + dom] / (prof[dom + "_ms"] * 1e-3) * 1e-12
+    dom_useful = (info["flops_useful"] if fused else info["flops_useful_" + dom]) / (prof[dom + "_ms"] * 1e-3) * 1e-12
     traffic = None
     try:
         import csv
@@ -512,7 +515,7 @@ def run_ours(name, o, v, x, args, steps, warmup, dist, dev, rank, world, peak):
     except Exception:
         pass
     roofline = {
-        "bound": "tensor", "kernel": "k_" + dom, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+        "bound": "tensor", "kernel": "k_small_fused" if fused else "k_" + dom, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
         "frac": achieved / peak, "traffic": traffic,
         "achieved_useful": dom_useful, "frac_useful": dom_useful / peak,
         "peak_source": "measured live: ppl_probe_fp64_peak (register-only DMMA m8n8k4 stream; profiles/r02_fp64_peaks.md); "
@@ -521,8 +524,8 @@ def run_ours(name, o, v, x, args, steps, warmup, dist, dev, rank, world, peak):
         "how": "ppl_apply_profiled: one serialised apply after the timed steps, a CUDA event pair around every launch; "
                "achieved = flops of the GEMM extents launched / time, achieved_useful = the symmetry-unique flops of the "
                "same launches / the same time",
-        "step0_tflops": info["flops_step0"] / (prof["step0_ms"] * 1e-3) * 1e-12,
-        "step1_tflops": info["flops_step1"] / (prof["step1_ms"] * 1e-3) * 1e-12,
+        "step0_tflops": info["flops_step0"] / (prof["step0_ms"] * 1e-3) * 1e-12 if prof["step0_ms"] > 0 else None,
+        "step1_tflops": info["flops_step1"] / (prof["step1_ms"] * 1e-3) * 1e-12 if prof["step1_ms"] > 0 else None,
         "share": {"step0": prof["step0_ms"] / prof["total_ms"], "step1": prof["step1_ms"] / prof["total_ms"],
                   "reduce": prof["reduce_ms"] / prof["total_ms"], "fold": prof["fold_ms"] / prof["total_ms"],
                   "pack": prof["pack_ms"] / prof["total_ms"]},
@@ -535,7 +538,7 @@ def run_ours(name, o, v, x, args, steps, warmup, dist, dev, rank, world, peak):
         "dtype": "f64", "data": "synthetic", "config": cfg,
         "run": {"symmetry": SYM_DESC[info["symmetry"]], "parallelism": "replicas only" if world > 1 else "1 gpu",
                 "plan": {k: info[k] for k in ("ta", "tb", "n_tiles", "ring", "splitk", "vec16", "workspace_bytes")},
-                "graph": args.graph, "verify_inputs": 1 if args.verify < 0 else args.verify},
+                "graph": args.graph, "verify_inputs": 1 if args.verify < 0 else args.verify, "small_fused": info.get("small_fused", 0)},
         "seconds_per_call": sec,
         "tflops_executed": f_exec / sec * 1e-12,
         "tflops_useful": f_use / sec * 1e-12,

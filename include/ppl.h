@@ -134,6 +134,10 @@ typedef struct ppl_info_s {
      *   PPL_SYM_PAIR_SA: step 0  2 nchol nvirt^2 P (W rows a <= b only);  step 1  2 (M+ K+ + M- K-) P
      *   PPL_SYM_PAIR:    (2 nchol + 2 nocc^2) nvirt^2 P;   PPL_SYM_NONE: the nominal count. */
     double flops_useful, flops_useful_step0, flops_useful_step1;
+    int32_t small_fused;                     /* 1: ppl_apply runs the one-kernel path of launch-bound shapes (nvirt <= 56, nocc <= 8;
+                                                csrc/ppl_kernels_small.cuh): step 0, step 1 and the accumulate / mirror in one
+                                                launch, W in registers; pair symmetry only (a <= b), whatever the mode allows */
+    int32_t reserved_;
 } ppl_info_t;
 
 /* Per-stage device times of the most recent profiled apply (ppl_apply_profiled), milliseconds. */
@@ -178,7 +182,9 @@ typedef struct ppl_debug_opts_s {
     int32_t debug_sync;       /* 1 = synchronise and report on stderr after every launch */
     int32_t trace;            /* 1 = timeline of one apply on stderr (also: environment variable PPL_TRACE) */
     int32_t host_chunk_mb;    /* ppl_apply_host: staging-buffer size in MiB (0 = 1024) */
-    int32_t reserved[18];     /* must be zero */
+    int32_t no_small_fused;   /* 1 = never take the one-kernel path of launch-bound shapes (nvirt <= 56, nocc <= 8): the tiled
+                                 path of the plan's symmetry mode runs instead (tests of the tiled kernels at small shapes) */
+    int32_t reserved[17];     /* must be zero */
 } ppl_debug_opts_t;
 
 /* ppl_plan with debug options (NULL = defaults). */

@@ -45,6 +45,7 @@ class ppl_info_t(ctypes.Structure):
         ("full_available", c_int32), ("full_tbg", c_int32), ("full_slabs", c_int32), ("full_tight", c_int32),
         ("full_workspace_bytes", c_uint64),
         ("flops_useful", c_double), ("flops_useful_step0", c_double), ("flops_useful_step1", c_double),
+        ("small_fused", c_int32), ("reserved_", c_int32),
     ]
 
     def asdict(self):
@@ -70,10 +71,16 @@ class ppl_debug_opts_t(ctypes.Structure):
     """include/ppl.h ppl_debug_opts_t: planner / orchestration knobs for tests and A/B runs; all zero = the defaults."""
     _fields_ = [(k, c_int32) for k in (
         "tile_edge", "ni_max", "cpasync_kernels", "full_min_v", "full_tbg", "full_slots", "full_strips", "full_tight",
-        "full_rect_tiles", "full_no_diag_pack", "full_serial", "debug_sync", "trace", "host_chunk_mb")] + [("reserved", c_int32 * 18)]
+        "full_rect_tiles", "full_no_diag_pack", "full_serial", "debug_sync", "trace", "host_chunk_mb", "no_small_fused")] + [("reserved", c_int32 * 17)]
+
+
+# Options merged under every Plan(...) / ppl_plan_dry(...) of this process.  Empty in the product; tests/conftest.py sets it so
+# that the -m gpu tests of the TILED kernels keep running them at small shapes (the fused one-kernel path has its own tests).
+DEFAULT_DEBUG: dict = {}
 
 
 def _debug_opts(debug):
+    debug = {**DEFAULT_DEBUG, **(debug or {})}
     if not debug:
         return None
     d = ppl_debug_opts_t()
@@ -177,7 +184,7 @@ class Plan:
 
     def __init__(self, nocc: int, nvirt: int, nchol: int, workspace_bytes: int = 0, debug: dict | None = None):
         """debug: ppl_debug_opts_t fields by name (tests / A-B runs only); None = ppl_plan."""
-        if debug:
+        if debug or DEFAULT_DEBUG:
             h = lib().ppl_plan_ex(int(nocc), int(nvirt), int(nchol), int(workspace_bytes), _debug_opts(debug))
         else:
             h = lib().ppl_plan(int(nocc), int(nvirt), int(nchol), int(workspace_bytes))

@@ -6,6 +6,7 @@
 #include "ppl_kernels.cuh"
 #include "ppl_kernels_tma.cuh"
 #include "ppl_kernels_full.cuh"
+#include "ppl_kernels_small.cuh"
 
 #include <atomic>
 #include <initializer_list>
@@ -114,6 +115,10 @@ int set_kernel_attrs() {
     PPL_CUDA(cudaFuncSetAttribute(ppl::k_step1t_tma<NI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::Step1Cfg<NI>::SMEM));
     PPL_ATTR_NI(1) PPL_ATTR_NI(2) PPL_ATTR_NI(3) PPL_ATTR_NI(4) PPL_ATTR_NI(5) PPL_ATTR_NI(6) PPL_ATTR_NI(7) PPL_ATTR_NI(8) PPL_ATTR_NI(9) PPL_ATTR_NI(10)
 #undef PPL_ATTR_NI
+#define PPL_ATTR_SMALL(NB) \
+    PPL_CUDA(cudaFuncSetAttribute(ppl::k_small_fused<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SmallCfg<NB>::SMEM));
+    PPL_ATTR_SMALL(1) PPL_ATTR_SMALL(2) PPL_ATTR_SMALL(3) PPL_ATTR_SMALL(4) PPL_ATTR_SMALL(5) PPL_ATTR_SMALL(6) PPL_ATTR_SMALL(7)
+#undef PPL_ATTR_SMALL
     if (known) g_attr_set[dev].store(true);
     return PPL_OK;
 }
@@ -167,7 +172,7 @@ int launch_step0(const ppl_plan_s *p, const Tile &t, const double *L, const CUte
         a.tb = t.tb;
         a.W = W;
         a.ldw = p->vv;
-        ppl::k_step0_tma<<<std::min(items, p->num_sms), ppl::TMA_THREADS, ppl::SMEM_TMA, s>>>(*mapL, a);
+        ppl::k_step0_tma<<<std::min(items, p->num_sms), ppl::TMA_THREADS, ppl::SMEM_TMA, s>>>(*mapL, *mapL, a);
     } else {
         ppl::Step0Args a;
         a.A = L + (int64_t)t.a0 * p->v;
@@ -1088,7 +1093,47 @@ int ppl_apply(ppl_plan_t *p, const double *L, const double *t2, double *R, void 
 
 namespace {
 
+// Launch-bound shapes: the whole ladder in one launch (ppl_kernels_small.cuh).  prof: an event pair around it.
+int run_apply_small(ppl_plan_s *p, const double *L, const double *t2, double *R, const ppl_opts_t *opts_in, cudaStream_t stream,
+                    Prof *prof) {
+    bool vec16 = false;
+    int rc = check_ptrs(p, L, t2, R, &vec16);
+    ppl_opts_t opts;
+    if (rc == PPL_OK) rc = check_opts(opts_in, &opts);
+    if (rc != PPL_OK) return fail(rc);
+    static_assert(SMALL_SW_HOST == ppl::SMALL_SW, "planner and kernel disagree on the work item");
+    ppl::SmallArgs a;
+    a.L = L;
+    a.t2 = t2;
+    a.R = R;
+    a.o = p->o;
+    a.v = p->v;
+    a.x = p->x;
+    a.pair = p->sym != PPL_SYM_NONE ? 1 : 0;
+    a.nitems = p->small_items[a.pair];
+    a.alpha = opts.alpha;
+    a.beta = opts.beta;
+    a.ts = r_strides(p->o, p->v, opts.t2_layout);
+    a.rs = r_strides(p->o, p->v, opts.r_layout);
+    const int grid = std::min(a.nitems, 2 * p->num_sms);
+    if (prof && prof->mark(-1, 0, stream) != PPL_OK) return fail(PPL_ERR_CUDA);
+    switch ((p->v + 7) / 8) {
+#define PPL_LAUNCH_SMALL(NB)                                                                                    \
+    case NB:                                                                                                    \
+        ppl::k_small_fused<NB><<<grid, ppl::SMALL_THREADS, ppl::SmallCfg<NB>::SMEM, stream>>>(a);              \
+        break;
+        PPL_LAUNCH_SMALL(1) PPL_LAUNCH_SMALL(2) PPL_LAUNCH_SMALL(3) PPL_LAUNCH_SMALL(4) PPL_LAUNCH_SMALL(5) PPL_LAUNCH_SMALL(6)
+            PPL_LAUNCH_SMALL(7)
+#undef PPL_LAUNCH_SMALL
+        default: return fail(PPL_ERR_INVALID_ARG);
+    }
+    PPL_CUDA(cudaGetLastError());
+    if (prof && prof->mark(K_STEP0, 1, stream) != PPL_OK) return fail(PPL_ERR_CUDA);
+    return PPL_OK;
+}
+
 int apply_direct(ppl_plan_s *p, const double *L, const double *t2, double *R, const ppl_opts_t *opts, cudaStream_t stream) {
+    if (p && p->small_ok) return run_apply_small(p, L, t2, R, opts, stream, nullptr);
     if (p && p->sym == PPL_SYM_FULL) return run_apply_full(p, L, t2, R, opts, stream, nullptr);
     return run_apply(p, L, t2, R, opts, stream, nullptr);
 }
@@ -1171,8 +1216,9 @@ int ppl_apply_profiled(ppl_plan_t *p, const double *L, const double *t2, double 
     cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
     memset(times, 0, sizeof(*times));
     Prof prof;
-    int rc = (p && p->sym == PPL_SYM_FULL) ? run_apply_full(p, L, t2, R, nullptr, stream, &prof)
-                                           : run_apply(p, L, t2, R, nullptr, stream, &prof);
+    int rc = (p && p->small_ok) ? run_apply_small(p, L, t2, R, nullptr, stream, &prof)
+             : (p && p->sym == PPL_SYM_FULL) ? run_apply_full(p, L, t2, R, nullptr, stream, &prof)
+                                             : run_apply(p, L, t2, R, nullptr, stream, &prof);
     const cudaError_t e = cudaStreamSynchronize(stream);
     if (rc == PPL_OK && e == cudaSuccess && prof.ev.size() >= 2) {
         float acc[K_KINDS] = {0, 0, 0, 0, 0};
@@ -1491,6 +1537,55 @@ int ppl_plan_verify_status(ppl_plan_t *p, int *flags) {
     if (!p) return fail(PPL_ERR_INVALID_ARG);
     return verify_harvest(p, flags);
 }
+
+}  // extern "C"
+
+// ---- plain GEMMs on the TMA kernels, for ppl_contract_pair's fast paths (ppl_internal.h) ----
+// C[M][N] (dense) = beta C + alpha A^T B with A[K][M], B[K][N] dense row-major ("k-outer": 'k..m..,k..n..->m..n..'): k_step0_tma
+int ppl_gemm_kouter_tma(const double *A, const double *B, int M, int N, int K, double *C, double alpha, double beta, int sms,
+                        cudaStream_t s) {
+    if (set_kernel_attrs() != PPL_OK) return fail(PPL_ERR_CUDA);
+    CUtensorMap mapA, mapB;
+    if (make_map_2d(&mapA, A, (uint64_t)M, (uint64_t)K, (uint64_t)M * 8, 16, ppl::BK) != PPL_OK ||
+        make_map_2d(&mapB, B, (uint64_t)N, (uint64_t)K, (uint64_t)N * 8, 16, ppl::BK) != PPL_OK)
+        return fail(PPL_ERR_CUDA);
+    ppl::Step0TmaArgs a;
+    a.a0v = a.b0v = 0;
+    a.M = M;
+    a.N = N;
+    a.K = K;
+    a.v = N;  // with tb = 1 and ldw = N^2 the kernel's store address is m N + n (ppl_kernels_tma.cuh)
+    a.tb = 1;
+    a.W = C;
+    a.ldw = (int64_t)N * N;
+    a.alpha = alpha;
+    a.beta = beta;
+    const int64_t items = (int64_t)((M + ppl::BM - 1) / ppl::BM) * ((N + ppl::BN - 1) / ppl::BN);
+    ppl::k_step0_tma<<<(int)std::min<int64_t>(items, sms), ppl::TMA_THREADS, ppl::SMEM_TMA, s>>>(mapA, mapB, a);
+    PPL_CUDA(cudaGetLastError());
+    return PPL_OK;
+}
+
+// part[z][M][N] = sum_{k in split z} A[m][k] B[n][k] with A[M][K], B[N][K] dense row-major ("k-inner"): k_step1_tma.
+// part_bytes: room for the partials; *splitk_out: the split taken (>= 1).  PPL_ERR_WORKSPACE_TOO_SMALL if M N doubles do not fit.
+int ppl_gemm_kinner_tma(const double *A, const double *B, int M, int N, int K, double *part, size_t part_bytes, int *splitk_out,
+                        int sms, cudaStream_t s) {
+    if (set_kernel_attrs() != PPL_OK) return fail(PPL_ERR_CUDA);
+    if ((size_t)M * N * 8 > part_bytes) return fail(PPL_ERR_WORKSPACE_TOO_SMALL);
+    const MGeom mg = m_geom_tma(M, 10);
+    const SplitChoice sc = choose_split(M, N, K, sms, mg, part_bytes);
+    CUtensorMap mapA, mapB;
+    if (make_map_2d(&mapA, A, (uint64_t)K, (uint64_t)M, (uint64_t)K * 8, ppl::BK, (uint32_t)(16 * mg.ni)) != PPL_OK ||
+        make_map_2d(&mapB, B, (uint64_t)K, (uint64_t)N, (uint64_t)K * 8, ppl::BK, ppl::BN) != PPL_OK)
+        return fail(PPL_ERR_CUDA);
+    ppl_plan_s tmp;  // launch_step1 reads the SM count only
+    tmp.num_sms = sms;
+    const int rc = launch_step1(&tmp, &mapA, &mapB, mg, A, K, B, K, M, N, K, sc, part, true, s);
+    if (splitk_out) *splitk_out = sc.splitk;
+    return rc;
+}
+
+extern "C" {
 
 int ppl_destroy(ppl_plan_t *p) {
     if (!p) return PPL_OK;

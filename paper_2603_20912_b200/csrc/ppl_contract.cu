@@ -17,13 +17,12 @@
 // (DMMA m8n8k4) with the accumulators in registers.
 #include "../../include/ppl.h"
 #include "ppl_device.cuh"
+#include "ppl_internal.h"
 
 #include <algorithm>
 #include <cstdint>
 #include <cstring>
 #include <vector>
-
-int ppl_fail_code(int code);  // ppl_api.cu: records the code for ppl_last_error() and returns it
 
 namespace ppl {
 
@@ -296,6 +295,44 @@ bool pairs_ok(const int64_t *run, int64_t nrun, const int64_t *other, int64_t no
     return true;
 }
 
+// offset tables of one request, in the order they sit in the workspace
+struct Tables {
+    std::vector<int64_t> tab;
+    int64_t *Am, *Cm, *Bn, *Cn, *Ak, *Bk;
+};
+void build_tables(const Parsed &ps, Tables *t) {
+    t->tab.resize((size_t)(2 * ps.M + 2 * ps.N + 2 * ps.K));
+    t->Am = t->tab.data();
+    t->Cm = t->Am + ps.M;
+    t->Bn = t->Cm + ps.M;
+    t->Cn = t->Bn + ps.N;
+    t->Ak = t->Cn + ps.N;
+    t->Bk = t->Ak + ps.K;
+    fill_offsets(ps.Ml, ps.op[0], ps.ext, ps.M, t->Am);
+    fill_offsets(ps.Ml, ps.op[2], ps.ext, ps.M, t->Cm);
+    fill_offsets(ps.Nl, ps.op[1], ps.ext, ps.N, t->Bn);
+    fill_offsets(ps.Nl, ps.op[2], ps.ext, ps.N, t->Cn);
+    fill_offsets(ps.Kl, ps.op[0], ps.ext, ps.K, t->Ak);
+    fill_offsets(ps.Kl, ps.op[1], ps.ext, ps.K, t->Bk);
+}
+bool affine(const int64_t *t, int64_t n, int64_t stride) {
+    for (int64_t i = 0; i < n; ++i)
+        if (t[i] != i * stride) return false;
+    return true;
+}
+// Plain matrix pairs that go to the persistent TMA kernels of the ladder (34-35 TFLOP/s):
+//   K_OUTER  A[K][M], B[K][N], C[M][N] all dense in that order (the paper's step 0 'xac,xbd->acbd'): k_step0_tma
+//   K_INNER  A[M][K], B[N][K] dense (its step 1 with t2 stored [e,f,c,d], 'abcd,efcd->efab'): k_step1_tma into split-K
+//            partials, then the table-driven reduction scatters into C in any order
+enum Route { GENERIC = 0, K_OUTER, K_INNER };
+Route classify(const Parsed &ps, const Tables &t) {
+    if (!(ps.M & 1) && !(ps.N & 1) && affine(t.Ak, ps.K, ps.M) && affine(t.Am, ps.M, 1) && affine(t.Bk, ps.K, ps.N) &&
+        affine(t.Bn, ps.N, 1) && affine(t.Cm, ps.M, ps.N) && affine(t.Cn, ps.N, 1))
+        return K_OUTER;
+    if (!(ps.K & 1) && affine(t.Am, ps.M, ps.K) && affine(t.Ak, ps.K, 1) && affine(t.Bn, ps.N, ps.K) && affine(t.Bk, ps.K, 1)) return K_INNER;
+    return GENERIC;
+}
+
 size_t table_bytes(const Parsed &ps) { return (size_t)(2 * ps.M + 2 * ps.N + 2 * ps.K) * sizeof(int64_t); }
 
 // split-K factor: the estimated time of the launch -- whole waves of CTA tiles on `sms` SMs, each (k-tiles + pipeline
@@ -329,8 +366,14 @@ int ppl_contract_pair_workspace(const char *subscripts, const int64_t *dims0, co
     Parsed ps;
     const int rc = parse(subscripts, dims0, dims1, &ps);
     if (rc != PPL_OK || !bytes) return ppl_fail_code(rc != PPL_OK ? rc : PPL_ERR_INVALID_ARG);
+    Tables t;
+    build_tables(ps, &t);
+    const Route route = classify(ps, t);
     const int s = pick_splitk(ps, 148, ~(size_t)0);
-    *bytes = ((table_bytes(ps) + 255) & ~(size_t)255) + (s > 1 ? (size_t)s * ps.M * ps.N * 8 : 0);
+    size_t part = 0;  // K_OUTER writes C directly; K_INNER always goes through partials; GENERIC only when it splits k
+    if (route == K_INNER) part = (size_t)s * ps.M * ps.N * 8;
+    if (route == GENERIC && s > 1) part = (size_t)s * ps.M * ps.N * 8;
+    *bytes = ((table_bytes(ps) + 255) & ~(size_t)255) + part;
     return PPL_OK;
 }
 
@@ -352,14 +395,10 @@ int ppl_contract_pair(const char *subscripts, const int64_t *dims0, const int64_
 
     // offset tables: rows of A / C over the surviving letters of op0, columns of B / C over those of op1, k over the
     // summed letters (in op0's order for both operands)
-    std::vector<int64_t> tab((size_t)(2 * ps.M + 2 * ps.N + 2 * ps.K));
-    int64_t *hAm = tab.data(), *hCm = hAm + ps.M, *hBn = hCm + ps.M, *hCn = hBn + ps.N, *hAk = hCn + ps.N, *hBk = hAk + ps.K;
-    fill_offsets(ps.Ml, ps.op[0], ps.ext, ps.M, hAm);
-    fill_offsets(ps.Ml, ps.op[2], ps.ext, ps.M, hCm);
-    fill_offsets(ps.Nl, ps.op[1], ps.ext, ps.N, hBn);
-    fill_offsets(ps.Nl, ps.op[2], ps.ext, ps.N, hCn);
-    fill_offsets(ps.Kl, ps.op[0], ps.ext, ps.K, hAk);
-    fill_offsets(ps.Kl, ps.op[1], ps.ext, ps.K, hBk);
+    Tables tabs;
+    build_tables(ps, &tabs);
+    std::vector<int64_t> &tab = tabs.tab;
+    int64_t *hAm = tabs.Am, *hBn = tabs.Bn, *hAk = tabs.Ak, *hBk = tabs.Bk;
     // (a pageable source is staged by the runtime before the call returns: `tab` may go out of scope afterwards)
     if (cudaMemcpyAsync(workspace, tab.data(), tab.size() * sizeof(int64_t), cudaMemcpyHostToDevice, stream) != cudaSuccess) {
         (void)cudaGetLastError();
@@ -384,6 +423,23 @@ int ppl_contract_pair(const char *subscripts, const int64_t *dims0, const int64_
     const bool b_kfast = !ps.op[1].empty() && std::find(ps.Kl.begin(), ps.Kl.end(), ps.op[1].back()) != ps.Kl.end();
     a.a_vec = a_kfast ? pairs_ok(hAk, ps.K, hAm, ps.M, A) : pairs_ok(hAm, ps.M, hAk, ps.K, A);
     a.b_vec = b_kfast ? pairs_ok(hBk, ps.K, hBn, ps.N, B) : pairs_ok(hBn, ps.N, hBk, ps.K, B);
+    const bool aligned = (((uintptr_t)A | (uintptr_t)B | (uintptr_t)C) & 15) == 0;
+    const int sms = prop.multiProcessorCount;
+    const Route route = classify(ps, tabs);
+    if (aligned && route == K_OUTER && ps.N * ps.N < ((int64_t)1 << 62))
+        return ppl_gemm_kouter_tma(A, B, (int)ps.M, (int)ps.N, (int)ps.K, C, alpha, beta, sms, stream);
+    if (aligned && route == K_INNER && workspace_bytes - tb >= (size_t)ps.M * ps.N * 8) {
+        a.part = reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(workspace) + tb);
+        a.alpha = alpha;
+        a.beta = beta;
+        a.splitk = 1;
+        rc = ppl_gemm_kinner_tma(A, B, (int)ps.M, (int)ps.N, (int)ps.K, a.part, workspace_bytes - tb, &a.splitk, sms, stream);
+        if (rc != PPL_OK) return rc;
+        const int64_t MN = ps.M * ps.N;
+        ppl::k_contract_reduce<<<(int)std::min<int64_t>((MN + 255) / 256, (int64_t)sms * 8), 256, 0, stream>>>(a);
+        if (cudaGetLastError() != cudaSuccess) return ppl_fail_code(PPL_ERR_CUDA);
+        return PPL_OK;
+    }
     a.splitk = pick_splitk(ps, prop.multiProcessorCount, workspace_bytes - tb);
     const int64_t nkt = (ps.K + ppl::BK - 1) / ppl::BK;
     const int64_t kt_per = (nkt + a.splitk - 1) / a.splitk;

@@ -123,9 +123,14 @@ struct Step0TmaArgs {
     int v, tb;
     double *W;
     int64_t ldw;
+    double alpha = 1.0, beta = 0.0;  // W = beta W + alpha (product); the ladder path overwrites (1, 0)
 };
 
-__global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_tma(const __grid_constant__ CUtensorMap mapL, const Step0TmaArgs p) {
+// mapL / mapB: the row operand and the column operand (the same map twice on the ladder path, where both are L; two
+// different tensors when ppl_contract_pair routes a 'k...m...,k...n...->m...n...' contraction here: with v = N, tb = 1,
+// ldw = N^2 the store address a_l tb ldw + c v + b_l ldw + d is m N + n, a dense row-major C[M][N])
+__global__ void __launch_bounds__(TMA_THREADS, 1)
+    k_step0_tma(const __grid_constant__ CUtensorMap mapL, const __grid_constant__ CUtensorMap mapB, const Step0TmaArgs p) {
     extern __shared__ unsigned char smem_raw[];
     const TmaSmem sm = carve_smem(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -140,6 +145,7 @@ __global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_tma(const __grid_const
         setmaxnreg_dec<PRODUCER_REGS>();
         if (warp == CONSUMER_WARPS && lane == 0) {
             prefetch_tmap(&mapL);
+            prefetch_tmap(&mapB);
             int stage = 0;
             uint32_t phase = 0;
             for (int item = blockIdx.x; item < num_items; item += gridDim.x) {
@@ -153,7 +159,7 @@ __global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_tma(const __grid_const
 #pragma unroll
                     for (int i = 0; i < BM / 16; ++i) tma_load_2d(da + i * BK * 16, &mapL, xa + 16 * i, kt * BK, &sm.full[stage]);
 #pragma unroll
-                    for (int i = 0; i < BN / 16; ++i) tma_load_2d(db + i * BK * 16, &mapL, xb + 16 * i, kt * BK, &sm.full[stage]);
+                    for (int i = 0; i < BN / 16; ++i) tma_load_2d(db + i * BK * 16, &mapB, xb + 16 * i, kt * BK, &sm.full[stage]);
                     if (++stage == TSTAGES) {
                         stage = 0;
                         phase ^= 1;
@@ -216,6 +222,7 @@ __global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_tma(const __grid_const
         //   c0 <-> n = nw + 16j + 2q + f,   c1 <-> n = nw + 16j + 2q + 8 + f
         const int v = p.v;
         const bool pair_ok = (v & 1) == 0;  // n even & v even: (n, n+1) share one b and are 16-byte aligned
+        const bool plain = p.alpha == 1.0 && p.beta == 0.0;
 #pragma unroll
         for (int i = 0; i < 4; ++i)
 #pragma unroll
@@ -231,13 +238,13 @@ __global__ void __launch_bounds__(TMA_THREADS, 1) k_step0_tma(const __grid_const
                         const int n = n0 + wn * WTN + 16 * j + 2 * q + 8 * h;
                         const double v0 = acc[2 * i + e][2 * j][h], v1 = acc[2 * i + e][2 * j + 1][h];
                         const int bl = n / v, d = n - bl * v;
-                        if (pair_ok && n + 1 < p.N) {
+                        if (plain && pair_ok && n + 1 < p.N) {
                             *reinterpret_cast<double2 *>(wrow + (int64_t)bl * p.ldw + d) = make_double2(v0, v1);
                         } else {
-                            if (n < p.N) wrow[(int64_t)bl * p.ldw + d] = v0;
+                            if (n < p.N) r_update(wrow + (int64_t)bl * p.ldw + d, v0, p.alpha, p.beta);
                             if (n + 1 < p.N) {
                                 const int bl1 = (n + 1) / v, d1 = (n + 1) - bl1 * v;
-                                wrow[(int64_t)bl1 * p.ldw + d1] = v1;
+                                r_update(wrow + (int64_t)bl1 * p.ldw + d1, v1, p.alpha, p.beta);
                             }
                         }
                     }

@@ -465,6 +465,24 @@ ppl_plan_s *plan_host(int nocc, int nvirt, int nchol, size_t workspace_bytes, si
                 best_sa = sa;
             }
         }
+    // The one-kernel path (ppl_kernels_small.cuh): nvirt <= 56 (W_ab lives in NB x NB accumulator blocks, NB = ceil(nvirt / 8)
+    // <= 7: 98 of a thread's 255 registers), nocc <= 8 (step 1 runs as FMAs out of those registers) and a launch-bound amount of work.
+    {
+        const int NB = (nvirt + 7) / 8, W8 = 8 * NB, nkt = (nchol + ppl::BK - 1) / ppl::BK;
+        for (int pair = 0; pair < 2; ++pair) {
+            int items = 0;
+            int64_t warps = 0;  // (a, b) columns computed
+            for (int a = 0; a < nvirt; ++a) {
+                const int nb = pair ? nvirt - a : nvirt;
+                items += (nb + SMALL_SW_HOST - 1) / SMALL_SW_HOST;
+                warps += nb;
+            }
+            p->small_items[pair] = items;
+            p->fs_step0[pair] = 2.0 * (ppl::BK * (double)nkt) * W8 * W8 * warps;  // DMMA, padded to 8-blocks and 16 k
+            p->fs_step1[pair] = 2.0 * nocc * nocc * (double)W8 * W8 * warps;       // FMAs out of the accumulators
+        }
+        p->small_ok = !p->dbg.no_small_fused && nvirt <= 56 && nocc <= 8 && p->fs_step0[1] + p->fs_step1[1] < GRAPH_AUTO_FLOPS;
+    }
     if (best_T == 0) {
         delete p;
         *rc_out = PPL_ERR_WORKSPACE_TOO_SMALL;
@@ -489,6 +507,7 @@ int full_min_v(const ppl_plan_s *p) { return p->dbg.full_min_v > 0 ? p->dbg.full
 
 
 bool graph_wanted(const ppl_plan_s *p) {
+    if (p->small_ok) return false;  // one launch: nothing to replay
     if (p->graph_mode >= 0) return p->graph_mode == 1;
     const double f = p->sym == PPL_SYM_FULL ? p->ff_step0 + p->ff_step1 : p->f_step0 + p->f_step1;
     return f < GRAPH_AUTO_FLOPS;
@@ -618,6 +637,7 @@ int ppl_plan_info(const ppl_plan_t *p, ppl_info_t *out) {
         }
         out->flops_useful = out->flops_useful_step0 + out->flops_useful_step1;
     }
+    out->small_fused = p->small_ok;
     out->full_available = p->full_ok;
     out->full_tbg = p->tbg;
     out->full_slabs = (int)p->slabs.size();
@@ -647,6 +667,16 @@ int ppl_plan_info(const ppl_plan_t *p, ppl_info_t *out) {
         out->flops_executed = p->ff_step0 + p->ff_step1;
         out->sa_splitk_plus = p->ftiles.empty() ? 0 : p->ftiles[0].sp.splitk;
         out->sa_splitk_minus = p->ftiles.empty() ? 0 : p->ftiles[0].sm.splitk;
+    }
+    if (p->small_ok) {  // what ppl_apply actually runs: one launch, pair symmetry when the mode allows it
+        const int pr = p->sym != PPL_SYM_NONE ? 1 : 0;
+        out->n_tiles = p->small_items[pr];
+        out->launches_per_apply = 1;
+        out->ring = 1;
+        out->splitk = 1;
+        out->flops_step0 = p->fs_step0[pr];
+        out->flops_step1 = p->fs_step1[pr];
+        out->flops_executed = out->flops_step0 + out->flops_step1;
     }
     return PPL_OK;
 }

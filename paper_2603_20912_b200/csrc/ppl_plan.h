@@ -150,6 +150,10 @@ struct ppl_plan_s {
     cudaEvent_t ev_fold[2] = {nullptr, nullptr}, evg[2][4] = {};
     CUtensorMap mapFWp[2], mapFWm[2], mapFWpT[2], mapFWmT[2];  // the W+- tile as the B operand of use 1 (box 16 x 128 rows) / use 2 (box 16 x 16 rows)
     // ---- CUDA graph of one apply (launch-bound shapes; ppl_plan_set_graph) ----
+    // ---- the one-kernel path of launch-bound shapes (ppl_kernels_small.cuh) ----
+    int small_ok = 0;                          // ppl_apply takes it (whatever the symmetry mode; pair symmetry is used when the mode allows)
+    double fs_step0[2] = {0, 0}, fs_step1[2] = {0, 0};  // its executed flops without / with pair symmetry
+    int small_items[2] = {0, 0};
     int dry = 0;                               // ppl_plan_dry: geometry only, the plan owns nothing on the device
     int graph_mode = -1;                       // -1: auto (graph when the executed flops are below GRAPH_AUTO_FLOPS), 0: off, 1: on
     cudaStream_t gcap = nullptr;               // capture origin (never the caller's stream: the legacy stream cannot capture)
@@ -177,5 +181,6 @@ ppl_plan_s *plan_host(int nocc, int nvirt, int nchol, size_t workspace_bytes, si
 bool dims_ok(int nocc, int nvirt, int nchol);
 int full_min_v(const ppl_plan_s *p);
 bool graph_wanted(const ppl_plan_s *p);
+constexpr int SMALL_SW_HOST = 4;  // b's per work item of the one-kernel path (= ppl::SMALL_SW)
 
 }  // namespace pplh

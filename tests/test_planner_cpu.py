@@ -185,8 +185,15 @@ def test_plans_recorded_on_the_b200_are_reproduced():
     # the round-1 form of the tiles (debug options) still plans what round 1 recorded (profiles/r01_large_full.md)
     r1 = P.ppl_plan_dry(40, 400, 1600, debug={"full_rect_tiles": 1, "full_no_diag_pack": 1})
     assert (r1["n_tiles"], r1["launches_per_apply"]) == (34, 263)
-    tiny = P.ppl_plan_dry(5, 20, 60)  # below nvirt = 52: PPL_SYM_PAIR_SA, one tile
+    tiny = P.ppl_plan_dry(5, 20, 60, debug={"no_small_fused": 1})  # the tiled plan below nvirt = 52: PPL_SYM_PAIR_SA, one tile
     assert (tiny["symmetry"], tiny["n_tiles"], tiny["ta"], tiny["launches_per_apply"]) == (P.PPL_SYM_PAIR_SA, 1, 20, 6)
+    # what the product runs at tiny and small: one fused launch over (a; 4 b's) work items, pair symmetry
+    for shape, items in (((5, 20, 60), sum((20 - a + 3) // 4 for a in range(20))), ((5, 53, 232), sum((53 - a + 3) // 4 for a in range(53)))):
+        d = P.ppl_plan_dry(*shape, debug={"no_small_fused": 0})
+        assert (d["small_fused"], d["launches_per_apply"], d["n_tiles"]) == (1, 1, items)
+        o, v, x = shape
+        w8, pairs, k16 = (v + 7) // 8 * 8, v * (v + 1) // 2, (x + 15) // 16 * 16
+        assert d["flops_step0"] == 2.0 * k16 * w8 * w8 * pairs and d["flops_step1"] == 2.0 * o * o * w8 * w8 * pairs
 
 
 def test_workspace_caps_and_fallbacks():
@@ -265,4 +272,4 @@ def test_planner_builds_with_gpp_alone_and_agrees_with_the_library(tmp_path):
             out = ppl_info_t()
             rc = lib.ppl_plan_dry(*shape, cap, 170 << 30, 148, -1, ctypes.byref(out))
             assert rc == P.PPL_OK
-            assert out.asdict() == P.ppl_plan_dry(*shape, workspace_bytes=cap)
+            assert out.asdict() == P.ppl_plan_dry(*shape, workspace_bytes=cap, debug={"no_small_fused": 0})
