@@ -450,7 +450,7 @@ def run_ours(name, o, v, x, args, steps, warmup, dist, dev, rank, world, peak):
     torch.cuda.synchronize()
 
     t0 = time.perf_counter()
-    plan = P.Plan(o, v, x, int(args.workspace_gb * (1 << 30)))
+    plan = P.Plan(o, v, x, int(args.workspace_gb * (1 << 30)), debug={"no_small_fused": 1} if args.no_small_fused else None)
     plan_s = time.perf_counter() - t0
     if args.symmetry != "default":
         plan.set_symmetry({v_: k_ for k_, v_ in SYM_NAMES.items()}[args.symmetry])
@@ -608,6 +608,8 @@ def main():
                     help="ppl_plan_set_graph: replay one CUDA graph per apply (auto: launch-bound shapes only)")
     ap.add_argument("--verify", type=int, default=-1, choices=[-1, 0, 1, 2],
                     help="PPL_OPT_VERIFY_INPUTS (-1 = the library default: 1, a symmetry check at the head of every apply)")
+    ap.add_argument("--no-small-fused", action="store_true",
+                    help="A/B: send launch-bound shapes (tiny, small) through the tiled path instead of the one fused kernel")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=0, help="timed ppl_apply_host calls (0 = --steps)")
     ap.add_argument("--no-secondary", action="store_true", help="with --config xl: skip the 'large' sub-record")

@@ -41,7 +41,7 @@ void free_plan(ppl_plan_s *p) {
     if (!p) return;
     // applies (plain launches on the caller's stream, or a graph launch) may still be in flight on streams the plan
     // does not own: wait for the device before the workspace goes away
-    const bool owns_device = p->ws || p->fws || p->flags || p->gen || p->gexec;  // not so for ppl_plan_dry or a plan that failed early
+    const bool owns_device = p->ws || p->fws || p->vflags_host || p->gen || p->gexec;  // not so for ppl_plan_dry or a plan that failed early
     if (!p->dry && owns_device && cudaDeviceSynchronize() != cudaSuccess) (void)cudaGetLastError();
     if (p->gen) {
         cudaStreamSynchronize(p->gen);
@@ -85,8 +85,8 @@ void free_plan(ppl_plan_s *p) {
     }
     if (p->ws) cudaFree(p->ws);
     if (p->fws) cudaFree(p->fws);
-    if (p->flags) cudaFree(p->flags);
-    if (p->vflags) cudaFree(p->vflags);
+    if (p->small_Lp) cudaFree(p->small_Lp);
+    if (p->small_tp) cudaFree(p->small_tp);
     if (p->vflags_host) cudaFreeHost(p->vflags_host);
     if (p->ev_verify) cudaEventDestroy(p->ev_verify);
     if (p->tperm) cudaFree(p->tperm);
@@ -779,6 +779,10 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
         a0.rows_per_a = t ? t->tbp : p->vp;
         a0.b_base = t ? t->bg0 : 0;
         a0.image = t ? 0 : 1;
+        {   // row panels of one raster group: about 40 MB of L2 (126 MB, shared with the streamed column panels and the stores)
+            const double panel = 128.0 * p->x * 8.0;
+            a0.group_m = (int)std::max(8.0, std::min((double)a0.tiles_m, std::floor(40e6 / panel)));
+        }
         const int items = a0.tiles_m * a0.tiles_n;
         if (dual && unit_no >= 2) PPL_CUDA(cudaStreamWaitEvent(s0, p->ev_xfree[xi], 0));  // the folds of unit u - 2 have read this strip
         tb("step0", t ? t->bg0 : sl.A0, 0, s0);
@@ -1005,8 +1009,8 @@ ppl_plan_t *ppl_plan_ex(int nocc, int nvirt, int nchol, size_t workspace_bytes, 
         fail(rc_host);
         return nullptr;
     }
-    if (cudaMalloc(&p->ws, p->ws_bytes) != cudaSuccess || cudaMalloc(&p->flags, sizeof(int)) != cudaSuccess ||
-        cudaMalloc(&p->vflags, sizeof(int)) != cudaSuccess || cudaMallocHost(&p->vflags_host, sizeof(int)) != cudaSuccess ||
+    if (cudaMalloc(&p->ws, p->ws_bytes) != cudaSuccess ||
+        cudaHostAlloc(&p->vflags_host, 4 * sizeof(int), cudaHostAllocMapped) != cudaSuccess ||
         cudaEventCreateWithFlags(&p->ev_verify, cudaEventDisableTiming) != cudaSuccess) {
         (void)cudaGetLastError();
         free_plan(p);
@@ -1102,9 +1106,33 @@ int run_apply_small(ppl_plan_s *p, const double *L, const double *t2, double *R,
     if (rc == PPL_OK) rc = check_opts(opts_in, &opts);
     if (rc != PPL_OK) return fail(rc);
     static_assert(SMALL_SW_HOST == ppl::SMALL_SW, "planner and kernel disagree on the work item");
+    if (prof && prof->mark(-1, 0, stream) != PPL_OK) return fail(PPL_ERR_CUDA);
+    // bulk copies want 16-byte aligned rows of even length: otherwise (odd nvirt, t2 stored 'iajb', misaligned buffers) the
+    // operands are first copied into the plan's padded buffers
+    const int vp = p->vp;
+    const bool pack_L = (p->v & 1) || ((uintptr_t)L & 15), pack_t = (p->v & 1) || opts.t2_layout != PPL_LAYOUT_IJAB || ((uintptr_t)t2 & 15);
+    if (pack_L || pack_t) {
+        if (pack_L && !p->small_Lp && cudaMalloc(&p->small_Lp, (size_t)p->x * p->v * vp * 8) != cudaSuccess) {
+            (void)cudaGetLastError();
+            p->small_Lp = nullptr;
+            return fail(PPL_ERR_ALLOC);
+        }
+        if (pack_t && !p->small_tp && cudaMalloc(&p->small_tp, (size_t)p->o * p->o * p->v * vp * 8) != cudaSuccess) {
+            (void)cudaGetLastError();
+            p->small_tp = nullptr;
+            return fail(PPL_ERR_ALLOC);
+        }
+        const int64_t n = (pack_L ? (int64_t)p->x * p->v * vp : 0) + (pack_t ? (int64_t)p->o * p->o * p->v * vp : 0);
+        const int g = (int)std::min<int64_t>((n + 255) / 256, (int64_t)p->num_sms * 8);
+        ppl::k_small_prepack<<<g, 256, 0, stream>>>(pack_L ? L : nullptr, pack_t ? t2 : nullptr, p->small_Lp, p->small_tp, p->o, p->v, p->x,
+                                                  vp, r_strides(p->o, p->v, opts.t2_layout));
+        PPL_CUDA(cudaGetLastError());
+    }
     ppl::SmallArgs a;
-    a.L = L;
-    a.t2 = t2;
+    a.L = pack_L ? p->small_Lp : L;
+    a.ldl = pack_L ? vp : p->v;
+    a.t2 = pack_t ? p->small_tp : t2;
+    a.ldt = pack_t ? vp : p->v;
     a.R = R;
     a.o = p->o;
     a.v = p->v;
@@ -1113,10 +1141,8 @@ int run_apply_small(ppl_plan_s *p, const double *L, const double *t2, double *R,
     a.nitems = p->small_items[a.pair];
     a.alpha = opts.alpha;
     a.beta = opts.beta;
-    a.ts = r_strides(p->o, p->v, opts.t2_layout);
     a.rs = r_strides(p->o, p->v, opts.r_layout);
     const int grid = std::min(a.nitems, 2 * p->num_sms);
-    if (prof && prof->mark(-1, 0, stream) != PPL_OK) return fail(PPL_ERR_CUDA);
     switch ((p->v + 7) / 8) {
 #define PPL_LAUNCH_SMALL(NB)                                                                                    \
     case NB:                                                                                                    \
@@ -1128,7 +1154,7 @@ int run_apply_small(ppl_plan_s *p, const double *L, const double *t2, double *R,
         default: return fail(PPL_ERR_INVALID_ARG);
     }
     PPL_CUDA(cudaGetLastError());
-    if (prof && prof->mark(K_STEP0, 1, stream) != PPL_OK) return fail(PPL_ERR_CUDA);
+    if (prof && prof->mark(K_STEP0, 1 + ((pack_L || pack_t) ? 1 : 0), stream) != PPL_OK) return fail(PPL_ERR_CUDA);
     return PPL_OK;
 }
 
@@ -1470,7 +1496,9 @@ int ppl_apply_host(ppl_plan_t *p, const double *Lh, const double *t2h, double *R
 
 namespace {
 
-int launch_check(const ppl_plan_s *p, const double *L, const double *t2, int t2_layout, int *dflags, cudaStream_t stream) {
+// hflags: two words of the plan's mapped pinned host buffer; cleared here by the host, written by the kernel (no memset, no
+// device-to-host copy: at launch-bound shapes those two operations cost more than the check itself)
+int launch_check(const ppl_plan_s *p, const double *L, const double *t2, int t2_layout, int *hflags, cudaStream_t stream) {
     ppl::CheckArgs a;
     a.L = L;
     a.t2 = t2;
@@ -1481,9 +1509,13 @@ int launch_check(const ppl_plan_s *p, const double *L, const double *t2, int t2_
     a.s_i = ts.i;
     a.s_j = ts.j;
     a.s_c = ts.a;
+    int *dflags = nullptr;
+    PPL_CUDA(cudaHostGetDevicePointer(&dflags, hflags, 0));
     a.flags = dflags;
-    PPL_CUDA(cudaMemsetAsync(dflags, 0, sizeof(int), stream));
-    ppl::k_check_inputs<<<p->num_sms * 8, 256, 0, stream>>>(a);
+    hflags[0] = hflags[1] = 0;
+    const int nb = (p->v + 31) / 32;
+    const int64_t items = (L ? (int64_t)p->x * nb * (nb + 1) / 2 : 0) + (t2 ? (int64_t)p->o * (p->o + 1) / 2 * nb * nb : 0);
+    ppl::k_check_inputs<<<(int)std::max<int64_t>(1, std::min<int64_t>(items, (int64_t)p->num_sms * 8)), 256, 0, stream>>>(a);
     PPL_CUDA(cudaGetLastError());
     return PPL_OK;
 }
@@ -1497,7 +1529,7 @@ int verify_harvest(ppl_plan_s *p, int *flags_out) {
         (void)cudaGetLastError();
         return fail(PPL_ERR_CUDA);
     }
-    const int h = *p->vflags_host;
+    const int h = (p->vflags_host[0] ? 1 : 0) | (p->vflags_host[1] ? 2 : 0);
     if (flags_out) *flags_out = h;
     if ((h & 2) && p->sym != PPL_SYM_NONE) return fail(PPL_ERR_PRECONDITION);
     if ((h & 1) && p->sym == PPL_SYM_FULL) return fail(PPL_ERR_PRECONDITION);
@@ -1506,9 +1538,8 @@ int verify_harvest(ppl_plan_s *p, int *flags_out) {
 
 // queue the check of this apply's inputs on `stream` (L == nullptr / t2 == nullptr: not checked)
 int verify_begin(ppl_plan_s *p, const double *L, const double *t2, int t2_layout, cudaStream_t stream) {
-    int rc = launch_check(p, L, t2, t2_layout, p->vflags, stream);
+    int rc = launch_check(p, L, t2, t2_layout, p->vflags_host, stream);
     if (rc != PPL_OK) return rc;
-    PPL_CUDA(cudaMemcpyAsync(p->vflags_host, p->vflags, sizeof(int), cudaMemcpyDeviceToHost, stream));
     PPL_CUDA(cudaEventRecord(p->ev_verify, stream));
     p->verify_pending = 1;
     if (p->verify == 2) return verify_harvest(p, nullptr);
@@ -1522,11 +1553,10 @@ extern "C" {
 int ppl_check_inputs(ppl_plan_t *p, const double *L, const double *t2, void *stream_, int *flags) {
     if (!p || !L || !t2) return fail(PPL_ERR_INVALID_ARG);
     cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
-    const int rc = launch_check(p, L, t2, PPL_LAYOUT_IJAB, p->flags, stream);
+    const int rc = launch_check(p, L, t2, PPL_LAYOUT_IJAB, p->vflags_host + 2, stream);
     if (rc != PPL_OK) return rc;
-    int h = 0;
-    PPL_CUDA(cudaMemcpyAsync(&h, p->flags, sizeof(int), cudaMemcpyDeviceToHost, stream));
     PPL_CUDA(cudaStreamSynchronize(stream));
+    const int h = (p->vflags_host[2] ? 1 : 0) | (p->vflags_host[3] ? 2 : 0);
     if (flags) *flags = h;
     if ((h & 2) && p->sym != PPL_SYM_NONE) return fail(PPL_ERR_PRECONDITION);
     if ((h & 1) && p->sym == PPL_SYM_FULL) return fail(PPL_ERR_PRECONDITION);

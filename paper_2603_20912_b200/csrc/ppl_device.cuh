@@ -38,11 +38,11 @@ template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
 
 // tile index -> (tm, tn) with grouped rasterisation
-__device__ __forceinline__ void raster(int pid, int tiles_m, int tiles_n, int &tm, int &tn) {
-    const int per_group = GROUP_M * tiles_n;
+__device__ __forceinline__ void raster(int pid, int tiles_m, int tiles_n, int &tm, int &tn, int group_m = GROUP_M) {
+    const int per_group = group_m * tiles_n;
     const int gid = pid / per_group;
-    const int first_m = gid * GROUP_M;
-    const int gsize = min(tiles_m - first_m, GROUP_M);
+    const int first_m = gid * group_m;
+    const int gsize = min(tiles_m - first_m, group_m);
     const int r = pid - gid * per_group;
     tm = first_m + r % gsize;
     tn = r / gsize;

@@ -538,7 +538,9 @@ struct CheckArgs {
     const double *L, *t2;  // either may be null (not checked)
     int o, v, x;
     int64_t s_i, s_j, s_c;  // element strides of t2[i][j][c][.] (d contiguous) in the caller's storage order
-    int *flags;
+    volatile int *flags;    // [2] in MAPPED PINNED HOST memory, cleared by the host before the launch: [0] = 1 if L is not symmetric,
+                            // [1] = 1 if t2 is not pair-symmetric.  Plain stores of the same value (no atomics across PCIe, no
+                            // device-to-host copy behind the kernel): the host reads them once the kernel's event has completed.
 };
 __global__ void __launch_bounds__(256) k_check_inputs(const CheckArgs p) {
     __shared__ double sb[32][33];
@@ -599,7 +601,8 @@ __global__ void __launch_bounds__(256) k_check_inputs(const CheckArgs p) {
             }
         }
     }
-    if (f) atomicOr(p.flags, f);
+    if (f & 1) p.flags[0] = 1;
+    if (f & 2) p.flags[1] = 1;
 }
 
 // ---------------------------------------------------------------------------------------------

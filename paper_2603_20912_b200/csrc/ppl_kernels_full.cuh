@@ -50,6 +50,9 @@ struct Step0SlabArgs {
     double *X;           // strip [(a_l * rows_per_a + b - b_base)][c * v + d], row stride v*v
     int rows_per_a;      // strip rows per a_l: v (the slab's whole strip) or the b-group width (memory-tight mode)
     int b_base;          // first b of the strip: 0, or the b-group's first b
+    int group_m;         // raster: row tiles per group.  A group sweeps all column tiles once, its group_m row panels (128 x
+                         // nchol doubles each) staying in L2: the L rows behind the column tiles are read from DRAM once per
+                         // GROUP, so the planner makes groups as tall as a ~40 MB L2 share allows (large: 24, XL: 16; was 12)
     int image;           // 1: chunks cover d-block >= b-block only and the epilogue stores the b<->d image too (rows of
                          // every b >= A0 must be in the strip); 0: the chunks cover the full (b, d) rectangle of the group
 };
@@ -74,7 +77,7 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
             uint32_t phase = 0;
             for (int item = blockIdx.x; item < num_items; item += gridDim.x) {
                 int tm, tn;
-                raster(item, p.tiles_m, p.tiles_n, tm, tn);
+                raster(item, p.tiles_m, p.tiles_n, tm, tn, p.group_m);
                 int xa[8], xb[8];
                 unsigned packed = 0;  // bit i: chunk i of the column tile comes from the packed diagonal blocks (mapQ)
 #pragma unroll
@@ -113,7 +116,7 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
     uint32_t phase = 0;
     for (int item = blockIdx.x; item < num_items; item += gridDim.x) {
         int tm, tn;
-        raster(item, p.tiles_m, p.tiles_n, tm, tn);
+        raster(item, p.tiles_m, p.tiles_n, tm, tn, p.group_m);
         double acc[8][4][2];
 #pragma unroll
         for (int i = 0; i < 8; ++i)

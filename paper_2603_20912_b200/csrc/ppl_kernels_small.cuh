@@ -5,12 +5,22 @@
 // small to fill 148 SMs (tiny: 27 MFLOP; small: W is 63 MB and the step-1 GEMM has 25 rows).  Here one launch does
 // step 0, step 1 and the accumulate / mirror of SURVEY 8(a), and the v^4 intermediate never leaves the register file:
 //
-//   work item = (a; SW consecutive b's), one warp per b.  The CTA stages L[P][a][:] and L[P][b..b+SW)[:] through a
-//   cp.async ring, each warp forms  W_ab[c][d] = sum_P L[P,a,c] L[P,b,d]  (eq. 5; 'xac,xbd->acbd') with DMMA
-//   m8n8k4 into NB x NB accumulator blocks (NB = ceil(nvirt / 8)), then contracts its W_ab with t2 straight from the
-//   accumulators:  R[i,j,a,b] (+)= sum_cd W_ab[c][d] t2[i,j,c,d]  (eq. 4/6; 'acbd,ecfd->efab') -- nocc^2 dot products of
-//   FP64 FMAs per lane followed by a fixed-order warp reduction -- and lane 0 writes R[i,j,a,b] and, with pair symmetry,
-//   the mirror R[j,i,b,a].  Every R entry is written by exactly one warp: no atomics, bit-reproducible.
+//   work item = (a; SW consecutive b's), one warp per b.  Rows L[P][a][:] and L[P][b .. b+SW)[:] of 16 P's at a time are
+//   brought into a 3-stage shared-memory ring by TMA bulk copies (cp.async.bulk, one per row block, mbarrier complete_tx;
+//   SASS UBLKCP) issued by lane 0 of each warp; each warp forms  W_ab[c][d] = sum_P L[P,a,c] L[P,b,d]  (eq. 5,
+//   PAPER.md:63; 'xac,xbd->acbd') with DMMA m8n8k4 into NB x NB accumulator blocks (NB = ceil(nvirt / 8)), then contracts
+//   its W_ab with t2 straight from the accumulators:  R[i,j,a,b] (+)= sum_cd W_ab[c][d] t2[i,j,c,d]  (eq. 4/6;
+//   'acbd,ecfd->efab') -- nocc^2 dot products of FP64 FMAs per lane against t2 blocks staged through the same shared
+//   memory (one bulk copy per (i,j) block, two blocks at a time, double-buffered, shared by the CTA's warps), followed by
+//   a fixed-order warp reduction -- and lane 0 writes R[i,j,a,b] and, with pair symmetry, the mirror R[j,i,b,a].  Every
+//   R entry is written by exactly one warp: no atomics, bit-reproducible.
+//
+// Bulk copies need 16-byte aligned rows: for odd nvirt (or a t2 stored 'iajb', or misaligned buffers) k_small_prepack
+// first copies L and t2 into plan-owned buffers with rows padded to an even length (one extra launch of a few
+// microseconds).  Earlier forms of this kernel, measured at the small config: element-wise 8-byte cp.async gathers with t2
+// read from global memory in step 1 -- 661 us, 12 of 13 stall samples on the long scoreboard; t2 staged through shared
+// memory -- 342 us, 82 M warp instructions for 4 M DMMAs, i.e. issue-bound on address arithmetic at 1-2 warps per scheduler
+// (the tiled path: 261 us).
 //
 // Symmetry: with pair-symmetric t2 (every mode but PPL_SYM_NONE) only a <= b is computed (half of nominal, both steps);
 // L's own symmetry is not needed and not used.  The S+- packing of the tiled path would save another factor on paper,
@@ -25,23 +35,52 @@ constexpr int SMALL_STAGES = 3;
 constexpr int SMALL_THREADS = 32 * SMALL_SW;
 
 struct SmallArgs {
-    const double *L, *t2;
+    const double *L;     // [x][v][ldl] (ldl even, 16-byte aligned: the caller's L, or the padded copy)
+    const double *t2;    // [o*o][v][ldt] in (i,j) order (ldt even, aligned: the caller's t2, or the padded / re-ordered copy)
     double *R;
     int o, v, x;
+    int ldl, ldt;
     int pair;            // 1: items cover a <= b and the mirror entry is written too; 0: every (a, b)
     int nitems;
     double alpha, beta;
-    RStrides ts, rs;     // element strides of t2[i,j,c,d] and R[i,j,a,b] (either storage order)
+    RStrides rs;         // element strides of R[i,j,a,b] (either storage order)
 };
 
 template <int NB>
 struct SmallCfg {
     static constexpr int W8 = 8 * NB;                      // padded nvirt
     static constexpr int LDA = W8 + 4;                     // [k][c] row stride: 4 mod 8 doubles -> conflict-free LDS.64
-    static constexpr int LDB = SMALL_SW * W8 + 4;          // [k][(b_l, d)]
+    static constexpr int LDB = SMALL_SW * W8 + 4;          // [k][(b_l, d)]: the SW rows of one P are contiguous, ldl apart
     static constexpr int STAGE = BK * (LDA + LDB);         // doubles
-    static constexpr size_t SMEM = (size_t)SMALL_STAGES * STAGE * sizeof(double);
+    static constexpr int RING = SMALL_STAGES * STAGE;
+    static constexpr size_t SMEM = (size_t)RING * sizeof(double) + 64;  // + the mbarriers
 };
+
+// ---- mbarrier / bulk-copy primitives (as in ppl_kernels_tma.cuh; repeated here so that this header stands alone) ----
+__device__ __forceinline__ void sm_mbar_init(uint64_t *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void sm_mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void sm_mbar_wait(uint64_t *bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void sm_bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
 
 // item -> (a, b0): a-major; per a the b's from (pair ? a : 0) in blocks of SW
 __device__ __forceinline__ void small_item(int item, int v, int pair, int &a, int &b0) {
@@ -58,58 +97,49 @@ __device__ __forceinline__ void small_item(int item, int v, int pair, int &a, in
 template <int NB>
 __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArgs p) {
     using Cfg = SmallCfg<NB>;
-    constexpr int W8 = Cfg::W8, LDA = Cfg::LDA, LDB = Cfg::LDB;
+    constexpr int LDA = Cfg::LDA, LDB = Cfg::LDB;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double *sm = reinterpret_cast<double *>(smem_raw);
+    uint64_t *full = reinterpret_cast<uint64_t *>(sm + Cfg::RING);  // [SMALL_STAGES] k-loop stages, then [2] t2 halves
+    uint64_t *tfull = full + SMALL_STAGES;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, q = lane & 3;
-    const int v = p.v, vv = v * v;
+    const int v = p.v, ldl = p.ldl, ldt = p.ldt;
+    const int64_t lstride = (int64_t)v * ldl;              // doubles between L[P] and L[P+1]
     const int nkt = (p.x + BK - 1) / BK;
-    const int rowlen = v * (1 + SMALL_SW);                 // doubles fetched per P: row a, then rows b0 .. b0+SW-1 (contiguous in L)
-    constexpr int MAXR = (W8 * (1 + SMALL_SW) + SMALL_THREADS - 1) / SMALL_THREADS;
 
-    // the padding columns (c, d in [v, 8 NB)) of every stage are never written by a copy: clear them once
-    for (int i = tid; i < SMALL_STAGES * Cfg::STAGE; i += SMALL_THREADS) sm[i] = 0.0;
+    // Everything a fragment may touch beyond what a copy wrote (columns >= ldl of a row, rows of an absent b, the k tail)
+    // must hold FINITE values: it meets exact zeros or is masked out below.  Clear the ring once.
+    for (int i = tid; i < Cfg::RING; i += SMALL_THREADS) sm[i] = 0.0;
+    if (tid == 0) {
+        for (int s = 0; s < SMALL_STAGES; ++s) sm_mbar_init(&full[s], SMALL_SW);
+        sm_mbar_init(&tfull[0], 1);
+        sm_mbar_init(&tfull[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");  // the generic-proxy clears above precede the bulk copies below
     __syncthreads();
+    uint32_t phbits = 0, tphbits = 0;  // phase parity of every barrier, one bit each
 
     for (int item = blockIdx.x; item < p.nitems; item += gridDim.x) {
         int a, b0;
         small_item(item, v, p.pair, a, b0);
         const int nb = min(SMALL_SW, v - b0);              // b's of this item
-        // this thread's elements of one P-row of the stage: source offset inside L[P] and destination inside the stage
-        int srcoff[MAXR], dstoff[MAXR];
-#pragma unroll
-        for (int t = 0; t < MAXR; ++t) {
-            const int r = tid + t * SMALL_THREADS;
-            srcoff[t] = -1;
-            dstoff[t] = 0;
-            if (r < v) {
-                srcoff[t] = a * v + r;
-                dstoff[t] = r;
-            } else if (r < rowlen) {
-                const int s = r - v, bl = s / v, d = s - bl * v;
-                if (bl < nb) {
-                    srcoff[t] = (b0 + bl) * v + d;
-                    dstoff[t] = BK * LDA + bl * W8 + d;
-                } else {
-                    srcoff[t] = -2;                          // a b beyond nvirt: zeros
-                    dstoff[t] = BK * LDA + bl * W8 + d;
-                }
-            }
-        }
+        // stage kt: rows P = 16 kt .. 16 kt + 15 (those below nchol); warp w issues the copies of k = w, w + SW, ...
         auto load_stage = [&](int kt) {
-            double *st = sm + (kt % SMALL_STAGES) * Cfg::STAGE;
-            const double *Lp = p.L + (int64_t)kt * BK * vv;
-#pragma unroll 1  // (a rolled loop with one running pointer: unrolled, ptxas kept dozens of 64-bit addresses live next to the accumulators)
-            for (int k = 0; k < BK; ++k, Lp += vv) {
-                const bool inK = kt * BK + k < p.x;
-#pragma unroll
-                for (int t = 0; t < MAXR; ++t) {
-                    if (srcoff[t] == -1) continue;
-                    const bool ok = inK && srcoff[t] >= 0;
-                    const bool isb = dstoff[t] >= BK * LDA;
-                    cp_async8(st + dstoff[t] + k * (isb ? LDB : LDA), ok ? Lp + srcoff[t] : p.L, ok ? 8 : 0);
-                }
+            if (lane != 0) return;
+            const int s = kt % SMALL_STAGES;
+            double *st = sm + s * Cfg::STAGE;
+            const uint32_t abytes = (uint32_t)ldl * 8, bbytes = (uint32_t)nb * ldl * 8;
+            int rows = 0;
+            for (int k = warp; k < BK; k += SMALL_SW) rows += (kt * BK + k < p.x) ? 1 : 0;
+            sm_mbar_expect_tx(&full[s], rows * (abytes + bbytes));
+            for (int k = warp; k < BK; k += SMALL_SW) {
+                const int P = kt * BK + k;
+                if (P >= p.x) break;
+                const double *Lp = p.L + P * lstride;
+                sm_bulk_g2s(st + k * LDA, Lp + (int64_t)a * ldl, abytes, &full[s]);
+                sm_bulk_g2s(st + BK * LDA + k * LDB, Lp + (int64_t)b0 * ldl, bbytes, &full[s]);
             }
         };
 
@@ -121,25 +151,27 @@ __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArg
 
         __syncthreads();  // the previous item's reads of the ring are done
 #pragma unroll
-        for (int s = 0; s < SMALL_STAGES - 1; ++s) {
+        for (int s = 0; s < SMALL_STAGES - 1; ++s)
             if (s < nkt) load_stage(s);
-            cp_async_commit();
-        }
         for (int kt = 0; kt < nkt; ++kt) {
-            cp_async_wait<SMALL_STAGES - 2>();
-            __syncthreads();
+            const int s = kt % SMALL_STAGES;
+            sm_mbar_wait(&full[s], (phbits >> s) & 1u);
+            phbits ^= 1u << s;
+            __syncthreads();  // every warp has finished stage kt - 1: its slot may be refilled
             if (kt + SMALL_STAGES - 1 < nkt) load_stage(kt + SMALL_STAGES - 1);
-            cp_async_commit();
-            const double *as = sm + (kt % SMALL_STAGES) * Cfg::STAGE + g;
-            const double *bs = as + BK * LDA + warp * W8;
-            if (warp >= nb) continue;  // no b for this warp in a ragged item (it still takes part in the barriers above)
-            constexpr int K4_UNROLL = NB >= 6 ? 2 : BK / 4;  // (unrolled, the fragments of all four k-steps are fetched ahead: 4 x 2 NB doubles)
+            if (warp >= nb) continue;  // no b for this warp in a ragged item (it still takes part in the barriers)
+            const int kvalid = min(BK, p.x - kt * BK);     // the k tail of the last stage holds rows of an older stage: skip them
+            const double *as = sm + s * Cfg::STAGE + g;
+            const double *bs = sm + s * Cfg::STAGE + BK * LDA + warp * ldl + g;
+            constexpr int K4_UNROLL = NB >= 6 ? 2 : BK / 4;  // (unrolled further, the fragments of all four k-steps are fetched ahead)
 #pragma unroll K4_UNROLL
             for (int k4 = 0; k4 < BK / 4; ++k4) {
+                if (k4 * 4 >= kvalid) break;
                 const int kk = k4 * 4 + q;
+                const bool live = kk < kvalid;
                 double af[NB], bf[NB];
 #pragma unroll
-                for (int i = 0; i < NB; ++i) af[i] = as[kk * LDA + 8 * i];
+                for (int i = 0; i < NB; ++i) af[i] = live ? as[kk * LDA + 8 * i] : 0.0;
 #pragma unroll
                 for (int j = 0; j < NB; ++j) bf[j] = bs[kk * LDB + 8 * j];
 #pragma unroll
@@ -148,56 +180,99 @@ __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArg
                     for (int j = 0; j < NB; ++j) dmma(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
             }
         }
-        cp_async_wait<0>();
+        // rows c >= nvirt and columns d >= nvirt of the blocks were fed from beyond the rows (finite, but not W): drop them
+#pragma unroll
+        for (int i = 0; i < NB; ++i)
+#pragma unroll
+            for (int j = 0; j < NB; ++j) {
+                const bool rok = 8 * i + g < v;
+                if (!rok || 8 * j + 2 * q >= v) acc[i][j][0] = 0.0;
+                if (!rok || 8 * j + 2 * q + 1 >= v) acc[i][j][1] = 0.0;
+            }
 
-        // step 1 from the accumulators: block (i, j): c = 8 i + g, d = 8 j + 2 q, + 1.  Rows / columns >= nvirt of W are exact
-        // zeros (zero-padded operands); their t2 addresses are clamped into the array, so they contribute 0 * finite.
+        // ---- step 1 from the accumulators.  W_ab block (i, j) holds c = 8 i + g, d = 8 j + 2 q, + 1.  The (i', j') blocks of t2
+        // ([nvirt][ldt] doubles each, contiguous) come in by one bulk copy each, two per pass, double-buffered, and are read back
+        // as 16-byte pairs (d, d + 1).  Whatever a pair reads beyond a block's rows / columns is finite and meets a zero of W.
+        __syncthreads();  // every warp has left the k loop: the ring is free
         const int b = b0 + warp;
-        if (b < v) {
-            constexpr int U = NB >= 6 ? 2 : 4;  // (i, j) blocks of t2 per pass (register budget: the accumulators stay live)
-            const int oo = p.o * p.o, sa = (int)p.ts.a;
-            for (int ij0 = 0; ij0 < oo; ij0 += U) {
-                double s[U];
-                int64_t tij[U];  // offsets of the (i, j) blocks of t2 (beyond the last one: it is repeated and not stored)
+        const int oo = p.o * p.o;
+        const int tblk = v * ldt;                             // doubles per staged block
+        // blocks per pass: as many as two halves of the ring hold (a fragment pair may read up to 8 NB rows / columns into what
+        // follows its block, which must stay inside the ring): 2 at nvirt = 53, 7 at nvirt = 20 -- fewer, longer passes
+        const int bpp = max(1, min(8, ((Cfg::RING - (8 * NB - 1) * ldt - 8 * NB) / tblk + 1) / 2));
+        const int npass = (oo + bpp - 1) / bpp;
+        auto load_pass = [&](int ps) {                        // blocks bpp ps ... into half (ps & 1)
+            if (tid != 0) return;
+            const int h = ps & 1, n = min(bpp, oo - bpp * ps);
+            sm_mbar_expect_tx(&tfull[h], (uint32_t)n * tblk * 8);
+            for (int u = 0; u < n; ++u)
+                sm_bulk_g2s(sm + (h * bpp + u) * tblk, p.t2 + (int64_t)(bpp * ps + u) * tblk, (uint32_t)tblk * 8, &tfull[h]);
+        };
+        load_pass(0);
+        for (int ps = 0; ps < npass; ++ps) {
+            if (ps + 1 < npass) load_pass(ps + 1);            // (its half was read in pass ps - 1: the barrier below, last iteration)
+            const int h = ps & 1;
+            sm_mbar_wait(&tfull[h], (tphbits >> h) & 1u);
+            tphbits ^= 1u << h;
+            if (b < v) {
+                const int n = min(bpp, oo - bpp * ps);
+                for (int u0 = 0; u0 < n; u0 += 2) {           // two blocks at a time: four independent FMA chains
+                    double s[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+                    const int u1 = min(u0 + 1, n - 1);        // (an odd last block is read twice and stored once)
+                    const double *t0 = sm + (h * bpp + u0) * tblk + g * ldt + 2 * q;
+                    const int du = (u1 - u0) * tblk;
 #pragma unroll
-                for (int u = 0; u < U; ++u) {
-                    const int ij = min(ij0 + u, oo - 1), i_ = ij / p.o, j_ = ij - i_ * p.o;
-                    tij[u] = i_ * p.ts.i + j_ * p.ts.j;
-                    s[u] = 0.0;
-                }
-                // (g, q behind an opaque move: the 2 NB^2 element addresses below are loop-invariant, and hoisted out of this loop
-                // they would sit in registers next to the accumulators -- ptxas spilled them; a few integer ops per load are cheaper)
-                int g2 = g, q2 = q;
-                asm volatile("" : "+r"(g2), "+r"(q2));
+                    for (int i = 0; i < NB; ++i)
 #pragma unroll
-                for (int i = 0; i < NB; ++i) {
-                    const int roff = min(8 * i + g2, v - 1) * sa;
+                        for (int j = 0; j < NB; ++j) {
+                            const double2 ta = *reinterpret_cast<const double2 *>(t0 + 8 * i * ldt + 8 * j);
+                            const double2 tb = *reinterpret_cast<const double2 *>(t0 + du + 8 * i * ldt + 8 * j);
+                            s[0][0] = fma(acc[i][j][0], ta.x, s[0][0]);
+                            s[0][1] = fma(acc[i][j][1], ta.y, s[0][1]);
+                            s[1][0] = fma(acc[i][j][0], tb.x, s[1][0]);
+                            s[1][1] = fma(acc[i][j][1], tb.y, s[1][1]);
+                        }
+                    double r[2] = {s[0][0] + s[0][1], s[1][0] + s[1][1]};
 #pragma unroll
-                    for (int j = 0; j < NB; ++j) {
-                        const double *e0 = p.t2 + (roff + min(8 * j + 2 * q2, v - 1)), *e1 = p.t2 + (roff + min(8 * j + 2 * q2 + 1, v - 1));
+                    for (int u = 0; u < 2; ++u) {
 #pragma unroll
-                        for (int u = 0; u < U; ++u) {
-                            s[u] = fma(acc[i][j][0], __ldg(e0 + tij[u]), s[u]);
-                            s[u] = fma(acc[i][j][1], __ldg(e1 + tij[u]), s[u]);
+                        for (int m = 16; m >= 1; m >>= 1) r[u] += __shfl_xor_sync(0xffffffffu, r[u], m);
+                    }
+                    if (lane == 0) {
+#pragma unroll
+                        for (int u = 0; u < 2; ++u) {
+                            if (u0 + u >= n) break;
+                            const int ij = bpp * ps + u0 + u;
+                            const int i_ = ij / p.o, j_ = ij - i_ * p.o;
+                            r_update(p.R + i_ * p.rs.i + j_ * p.rs.j + a * p.rs.a + b * p.rs.b, r[u], p.alpha, p.beta);
+                            if (p.pair && a != b) r_update(p.R + j_ * p.rs.i + i_ * p.rs.j + b * p.rs.a + a * p.rs.b, r[u], p.alpha, p.beta);
                         }
                     }
                 }
-#pragma unroll
-                for (int u = 0; u < U; ++u) {
-#pragma unroll
-                    for (int m = 16; m >= 1; m >>= 1) s[u] += __shfl_xor_sync(0xffffffffu, s[u], m);
-                }
-                if (lane == 0) {
-#pragma unroll
-                    for (int u = 0; u < U; ++u) {
-                        const int ij = ij0 + u;
-                        if (ij >= oo) break;
-                        const int i_ = ij / p.o, j_ = ij - i_ * p.o;
-                        r_update(p.R + i_ * p.rs.i + j_ * p.rs.j + a * p.rs.a + b * p.rs.b, s[u], p.alpha, p.beta);
-                        if (p.pair && a != b) r_update(p.R + j_ * p.rs.i + i_ * p.rs.j + b * p.rs.a + a * p.rs.b, s[u], p.alpha, p.beta);
-                    }
-                }
             }
+            __syncthreads();  // pass ps has been read: its half may be refilled
+        }
+    }
+}
+
+// Copies of L and t2 with rows of even length ld = nvirt rounded up to even (the pad column is zero) and t2 in (i,j) order,
+// for the bulk copies of k_small_fused: Lp[P][a][ld], tp[i*o+j][c][ld].  Either source may be null (no copy needed).
+__global__ void __launch_bounds__(256) k_small_prepack(const double *__restrict__ L, const double *__restrict__ t2, double *__restrict__ Lp,
+                                                      double *__restrict__ tp, int o, int v, int x, int ld, RStrides ts) {
+    const int64_t nL = L ? (int64_t)x * v * ld : 0, nT = t2 ? (int64_t)o * o * v * ld : 0;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < nL + nT; idx += (int64_t)gridDim.x * blockDim.x) {
+        if (idx < nL) {
+            const int c = (int)(idx % ld);
+            const int64_t row = idx / ld;  // P * v + a
+            Lp[idx] = c < v ? __ldg(L + row * v + c) : 0.0;
+        } else {
+            const int64_t e = idx - nL;
+            const int d = (int)(e % ld);
+            int64_t r = e / ld;
+            const int c = (int)(r % v);
+            r /= v;
+            const int j = (int)(r % o), i = (int)(r / o);
+            tp[e] = d < v ? __ldg(t2 + i * ts.i + j * ts.j + c * ts.a + d) : 0.0;
         }
     }
 }

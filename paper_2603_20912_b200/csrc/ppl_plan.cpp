@@ -671,7 +671,7 @@ int ppl_plan_info(const ppl_plan_t *p, ppl_info_t *out) {
     if (p->small_ok) {  // what ppl_apply actually runs: one launch, pair symmetry when the mode allows it
         const int pr = p->sym != PPL_SYM_NONE ? 1 : 0;
         out->n_tiles = p->small_items[pr];
-        out->launches_per_apply = 1;
+        out->launches_per_apply = 1 + ((p->v & 1) ? 1 : 0);  // + the copy into even-length rows for odd nvirt (also taken for 'iajb' t2 / misaligned buffers)
         out->ring = 1;
         out->splitk = 1;
         out->flops_step0 = p->fs_step0[pr];

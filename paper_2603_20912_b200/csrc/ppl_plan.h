@@ -99,9 +99,8 @@ struct ppl_plan_s {
     double *part = nullptr;
     double *taup = nullptr, *taum = nullptr;
     double *tperm = nullptr;               // un-packed modes with PPL_LAYOUT_IAJB input: t2 permuted (lazy)
-    int *flags = nullptr;                  // device word for ppl_check_inputs
-    int *vflags = nullptr;                 // device word of the per-apply verification (PPL_OPT_VERIFY_INPUTS)
-    int *vflags_host = nullptr;            // its pinned host copy
+    int *vflags_host = nullptr;            // [4] mapped pinned host words written by k_check_inputs: [0..1] the per-apply verification
+                                           // (PPL_OPT_VERIFY_INPUTS), [2..3] ppl_check_inputs
     cudaEvent_t ev_verify = nullptr;
     int verify = 1;                        // PPL_OPT_VERIFY_INPUTS
     int verify_pending = 0;
@@ -154,6 +153,7 @@ struct ppl_plan_s {
     int small_ok = 0;                          // ppl_apply takes it (whatever the symmetry mode; pair symmetry is used when the mode allows)
     double fs_step0[2] = {0, 0}, fs_step1[2] = {0, 0};  // its executed flops without / with pair symmetry
     int small_items[2] = {0, 0};
+    double *small_Lp = nullptr, *small_tp = nullptr;  // copies with even-length rows for its bulk copies (odd nvirt, 'iajb' t2, misaligned buffers)
     int dry = 0;                               // ppl_plan_dry: geometry only, the plan owns nothing on the device
     int graph_mode = -1;                       // -1: auto (graph when the executed flops are below GRAPH_AUTO_FLOPS), 0: off, 1: on
     cudaStream_t gcap = nullptr;               // capture origin (never the caller's stream: the legacy stream cannot capture)

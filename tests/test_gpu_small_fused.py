@@ -30,7 +30,7 @@ def test_fused_path_parity(shape, sym):
     R0 = I.make_t2(o, v, 14, symmetric=False)
     want = oracle.full(L, t2, R0.copy())
     got, info = gpu_ladder(L, t2, R0=R0.copy(), sym=sym, return_info=True, debug=FUSED)
-    assert info["small_fused"] == 1 and info["launches_per_apply"] == 1, info
+    assert info["small_fused"] == 1 and info["launches_per_apply"] == 1 + (v & 1), info  # + the padded copy for odd nvirt
     assert relerr(got, want) <= TOL, info
 
 
@@ -87,7 +87,7 @@ def test_fused_path_zero_t2_repeat_and_which_shapes_take_it():
         prof = plan.apply_profiled(Ld, td, Rd)
         torch.cuda.synchronize()
         assert relerr(Rd.cpu().numpy(), 4.0 * oracle.full(L, t2)) <= TOL
-        assert prof["n_step0"] == 1 and prof["n_step1"] == 0 and prof["total_ms"] > 0
+        assert prof["n_step0"] in (1, 2) and prof["n_step1"] == 0 and prof["total_ms"] > 0
     # the path is for launch-bound shapes only
     assert P.ppl_plan_dry(5, 53, 232, debug=FUSED)["small_fused"] == 1
     assert P.ppl_plan_dry(5, 57, 232, debug=FUSED)["small_fused"] == 0      # nvirt > 56: W_ab no longer fits the accumulators
