@@ -201,8 +201,17 @@ def run_table3(args, o, v, x):
     # before anything else is allocated; the cap leaves room for what ppl_apply_host allocates on first use
     # (L whole + two 1-GiB staging buffers)
     free_b = torch.cuda.mem_get_info()[0]
-    cap = int(free_b * 0.98) - x * v * v * 8 - (3 << 30)
-    plan = P.Plan(o, v, x, cap)
+    unpacked = args.symmetry in ("none", "pair")
+    if unpacked:
+        # the paper's own setting (unstructured random arrays, no symmetry used): nothing assumed of L, and
+        # with `none` nothing of t2.  The plan needs only the W ring and the split-K partials; ppl_apply_host keeps t2
+        # resident and streams L panels / R slabs beside it.
+        cap = 8 << 30
+    else:
+        cap = int(free_b * 0.98) - x * v * v * 8 - (3 << 30)
+    plan = P.Plan(o, v, x, cap, debug={"host_panels": args.host_panels} if unpacked else None)
+    if unpacked:
+        plan.set_symmetry(P.PPL_SYM_NONE if args.symmetry == "none" else P.PPL_SYM_PAIR)
     plan_s = time.perf_counter() - t0
     info = plan.info()
     need = (x * v * v + 2 * o * o * v * v) * 8
@@ -218,8 +227,8 @@ def run_table3(args, o, v, x):
     Lh = torch.empty((x, v, v), dtype=torch.float64, pin_memory=True)
     th = torch.empty((o, o, v, v), dtype=torch.float64, pin_memory=True)
     Rh = torch.zeros((o, o, v, v), dtype=torch.float64, pin_memory=True)
-    I.make_L(v, x, 0, out=Lh.numpy())
-    I.make_t2(o, v, 0, out=th.numpy())
+    I.make_L(v, x, 0, symmetric=not unpacked, out=Lh.numpy())
+    I.make_t2(o, v, 0, symmetric=args.symmetry != "none", out=th.numpy())
     t_gen = time.perf_counter() - t_gen
     sampler = ClockSampler(0)
     for _ in range(max(args.warmup, 0)):
@@ -241,8 +250,13 @@ def run_table3(args, o, v, x):
         "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": False, "scaling": "weak",
         "vs_baseline": (dt / best) if best else None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": args.config, "nocc": o, "nvirt": v, "nchol": x, "seed": 0,
-                   "note": "shape of the paper's Table 3 row (PAPER.md:417-451); operands in pinned HOST memory; "
-                           "symmetric L and pair-symmetric t2 (the paper used unstructured random arrays and no symmetry)",
+                   "note": "shape of the paper's Table 3 row (PAPER.md:417-451); operands in pinned HOST memory; " +
+                           ({"none": "UNSTRUCTURED L and t2 (no symmetry generated, none assumed or used: the paper's own "
+                                     "setting, PAPER.md:385); t2 resident, L whole or in row panels, R in slabs",
+                             "pair": "unstructured L, pair-symmetric t2; t2 and R resident, L whole or in row panels"}.get(
+                                 args.symmetry, "symmetric L and pair-symmetric t2 (the paper used unstructured random "
+                                                "arrays and no symmetry)")),
+                   "host_panels": args.host_panels if unpacked else None,
                    "symmetry": SYM_DESC[info["symmetry"]],
                    "plan": {k: info[k] for k in ("ta", "tb", "n_tiles", "workspace_bytes", "full_tight")}},
         "step_seconds": secs, "plan_seconds": plan_s, "input_gen_seconds": t_gen,
@@ -610,6 +624,8 @@ def main():
                     help="PPL_OPT_VERIFY_INPUTS (-1 = the library default: 1, a symmetry check at the head of every apply)")
     ap.add_argument("--no-small-fused", action="store_true",
                     help="A/B: send launch-bound shapes (tiny, small) through the tiled path instead of the one fused kernel")
+    ap.add_argument("--host-panels", type=int, default=0, choices=[0, 1, 2],
+                    help="table3_* with --symmetry none|pair: 1 = stream L as row panels even if it fits whole, 2 = never")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=0, help="timed ppl_apply_host calls (0 = --steps)")
     ap.add_argument("--no-secondary", action="store_true", help="with --config xl: skip the 'large' sub-record")

@@ -184,7 +184,9 @@ typedef struct ppl_debug_opts_s {
     int32_t host_chunk_mb;    /* ppl_apply_host: staging-buffer size in MiB (0 = 1024) */
     int32_t no_small_fused;   /* 1 = never take the one-kernel path of launch-bound shapes (nvirt <= 56, nocc <= 8): the tiled
                                  path of the plan's symmetry mode runs instead (tests of the tiled kernels at small shapes) */
-    int32_t reserved[17];     /* must be zero */
+    int32_t host_panels;      /* ppl_apply_host, un-packed modes: 1 = stream L as row panels even when L fits on the device whole,
+                                 2 = never (L whole or PPL_ERR_ALLOC); 0 = panels only when L does not fit beside t2 */
+    int32_t reserved[16];     /* must be zero */
 } ppl_debug_opts_t;
 
 /* ppl_plan with debug options (NULL = defaults). */
@@ -261,7 +263,15 @@ int ppl_contract_pair(const char *subscripts, const int64_t *dims0, const int64_
  *     buffers (1 GiB each) and packed chunk by chunk into tau+-, the slabs run on the packed operands, and the result
  *     is unpacked chunk by chunk (R chunk in, R += term, R chunk out), copies of one chunk overlapping the kernels of
  *     the other.  Device residency is about half of L + t2 + R: shapes of the paper's Table 3 fit on one 180 GB GPU.
- *   other modes: L, t2 and R are copied whole, ppl_apply runs, R is copied back (PPL_ERR_ALLOC if they do not fit).
+ *   PPL_SYM_NONE / PPL_SYM_PAIR (nothing assumed of L; PPL_SYM_NONE: nothing of t2 either -- the paper's own benchmark
+ *     arrays), even nvirt: t2 is copied whole and stays resident (every W tile contracts with all of it);
+ *     L never needs to be: when it does not fit beside t2 it is streamed as row panels L[:, A, :] (a 2-D copy of nchol
+ *     rows of |A| nvirt doubles each; the panel of the tile's a-block is kept for a row of tiles, the panel of its b-block
+ *     rides a ring of buffers one tile ahead), and in PPL_SYM_NONE R is never on the device whole either: the slab
+ *     R[:, :, A, :] of one row of tiles travels in before the row's first reduction and out behind its last, the copies
+ *     of row k +- 1 overlapping the GEMMs of row k on streams of their own (in PPL_SYM_PAIR the mirror writes reach
+ *     every slab, so R stays resident).  Device residency: t2 + the W ring + a few panels / slabs.
+ *   PPL_SYM_PAIR_SA, or odd nvirt: L, t2 and R are copied whole, ppl_apply runs, R is copied back (PPL_ERR_ALLOC if they do not fit).
  *   At shapes that fill the device, plan with workspace_bytes = free device bytes - |L| - 3 GiB (what bench.py's
  *   table3_* configs do): the automatic cap of ppl_plan (90 % of the free bytes) leaves no room for L and the staging
  *   buffers, and the call then returns PPL_ERR_ALLOC.  Under such a cap the plan takes the memory-tight form of

@@ -8,7 +8,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(_HERE, "libppl.so")
-SOURCES = ["ppl_api.cu", "ppl_contract.cu", "ppl_plan.cpp"]
+SOURCES = ["ppl_api.cu", "ppl_host.cu", "ppl_contract.cu", "ppl_plan.cpp"]
 
 
 def _deps():

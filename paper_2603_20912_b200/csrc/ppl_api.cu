@@ -3,6 +3,7 @@
 // ppl_kernels*.cuh; there is no CPU fallback.
 #include "../../include/ppl.h"
 #include "ppl_plan.h"
+#include "ppl_launch.h"
 #include "ppl_kernels.cuh"
 #include "ppl_kernels_tma.cuh"
 #include "ppl_kernels_full.cuh"
@@ -95,6 +96,27 @@ void free_plan(ppl_plan_s *p) {
     if (p->dR) cudaFree(p->dR);
     for (int i = 0; i < 2; ++i)
         if (p->hstage[i]) cudaFree(p->hstage[i]);
+    {
+        ppl_plan_s::HostStream &h = p->hsn;
+        for (cudaStream_t st : {h.in, h.out})
+            if (st) {
+                cudaStreamSynchronize(st);
+                cudaStreamDestroy(st);
+            }
+        for (int i = 0; i < 2; ++i) {
+            if (h.pa[i]) cudaFree(h.pa[i]);
+            if (h.rs[i]) cudaFree(h.rs[i]);
+            for (cudaEvent_t e : {h.ev_pa[i], h.ev_pafree[i], h.ev_rsin[i], h.ev_rsdone[i], h.ev_rsfree[i]})
+                if (e) cudaEventDestroy(e);
+        }
+        for (int i = 0; i < MAX_RING; ++i) {
+            if (h.pb[i]) cudaFree(h.pb[i]);
+            for (cudaEvent_t e : {h.ev_pb[i], h.ev_pbfree[i]})
+                if (e) cudaEventDestroy(e);
+        }
+        for (cudaEvent_t e : {h.ev_t2, h.ev_fork})
+            if (e) cudaEventDestroy(e);
+    }
     delete p;
 }
 
@@ -1345,153 +1367,6 @@ int ppl_generate_eri(ppl_plan_t *p, const double *L, int a0, int na, double *eri
     return PPL_OK;
 }
 
-// PPL_SYM_FULL on host operands: the device never holds t2 or R.  t2 is streamed through two staging buffers and
-// packed chunk by chunk into tau+- (rows (i,j) of a chunk are contiguous in the [i][j][c][d] order), the slabs run on
-// the packed operands, and R+-acc is unpacked chunk by chunk into the staging buffers (R chunk in, result out).
-// Device residency: L + tau+- + R+-acc + the PPL_SYM_FULL workspace -- about half of L + t2 + R + workspace, which
-// is what lets the paper's Table 3 shapes (t2 and R of 39 GB each at N = 800) run on one 180 GB GPU.
-static int apply_host_full_queue(ppl_plan_s *p, const double *Lh, const double *t2h, double *Rh, uint64_t *h2d, uint64_t *d2h) {
-    const size_t nL = (size_t)p->x * p->vv * 8;
-    const int64_t rows = (int64_t)p->o * p->o;
-    const size_t row_bytes = (size_t)p->vv * 8;
-    if (!p->dL && cudaMalloc(&p->dL, nL) != cudaSuccess) {
-        (void)cudaGetLastError();
-        p->dL = nullptr;
-        return fail(PPL_ERR_ALLOC);
-    }
-    if (!p->hstage[0]) {
-        const size_t want = p->dbg.host_chunk_mb > 0 ? (size_t)p->dbg.host_chunk_mb << 20 : (size_t)1 << 30;  // debug override of the staging-buffer size
-        p->hchunk_rows = (int)std::max<int64_t>(1, std::min<int64_t>(rows, (int64_t)(want / row_bytes)));
-        for (int i = 0; i < 2; ++i)
-            if (cudaMalloc(&p->hstage[i], (size_t)p->hchunk_rows * row_bytes) != cudaSuccess) {
-                (void)cudaGetLastError();
-                for (int k = 0; k < 2; ++k) {
-                    if (p->hstage[k]) cudaFree(p->hstage[k]);
-                    p->hstage[k] = nullptr;
-                }
-                return fail(PPL_ERR_ALLOC);
-            }
-    }
-    if (!p->hs2) {
-        bool ok = cudaStreamCreateWithFlags(&p->hs2, cudaStreamNonBlocking) == cudaSuccess;
-        ok = ok && cudaEventCreateWithFlags(&p->ev_tau, cudaEventDisableTiming) == cudaSuccess;
-        ok = ok && cudaEventCreateWithFlags(&p->ev_done, cudaEventDisableTiming) == cudaSuccess;
-        if (!ok) {
-            (void)cudaGetLastError();
-            return fail(PPL_ERR_CUDA);
-        }
-    }
-    cudaStream_t cs = p->host_stream;         // L in, all slabs
-    cudaStream_t st[2] = {p->gen, p->hs2};    // chunk k of t2 / R on stream k % 2; each stream owns one staging buffer
-    const bool minus = p->Mm > 0 && p->Km > 0;
-    ppl_opts_t opts;
-    check_opts(nullptr, &opts);
-    const int64_t nchunks = (rows + p->hchunk_rows - 1) / p->hchunk_rows;
-    // phase A: L in on the compute stream; t2 chunks in -> tau+- on the chunk streams, overlapping L and step 0 of slab 0
-    PPL_CUDA(cudaMemcpyAsync(p->dL, Lh, nL, cudaMemcpyHostToDevice, cs));
-    if (p->verify) {  // L only: t2 never sits on the device whole (include/ppl.h, PPL_OPT_VERIFY_INPUTS)
-        const int rcv = verify_begin(p, p->dL, nullptr, PPL_LAYOUT_IJAB, cs);
-        if (rcv != PPL_OK) return rcv;
-    }
-    PPL_CUDA(cudaMemsetAsync(p->raccp, 0, (size_t)p->Mp * p->ldp * 8, cs));
-    if (minus) PPL_CUDA(cudaMemsetAsync(p->raccm, 0, (size_t)p->Mm * p->ldm * 8, cs));
-    int k = 0;
-    for (int64_t r0 = 0; r0 < rows; r0 += p->hchunk_rows, ++k) {
-        const int64_t r1 = std::min<int64_t>(rows, r0 + p->hchunk_rows);
-        cudaStream_t s = st[k & 1];
-        double *buf = p->hstage[k & 1];
-        PPL_CUDA(cudaMemcpyAsync(buf, t2h + r0 * p->vv, (size_t)(r1 - r0) * row_bytes, cudaMemcpyHostToDevice, s));
-        const int rc = launch_pack(p, buf - r0 * p->vv, PPL_LAYOUT_IJAB, 0.5, s, (int)r0, (int)r1);
-        if (rc != PPL_OK) return rc;
-    }
-    PPL_CUDA(cudaEventRecord(p->ev_in, st[1]));
-    PPL_CUDA(cudaStreamWaitEvent(st[0], p->ev_in, 0));
-    PPL_CUDA(cudaEventRecord(p->ev_tau, st[0]));
-    // the first two R chunks travel to the (now free) staging buffers while the slabs run
-    auto r_chunk_in = [&](int64_t kk) -> int {
-        const int64_t r0 = kk * p->hchunk_rows, r1 = std::min<int64_t>(rows, r0 + p->hchunk_rows);
-        PPL_CUDA(cudaMemcpyAsync(p->hstage[kk & 1], Rh + r0 * p->vv, (size_t)(r1 - r0) * row_bytes, cudaMemcpyHostToDevice, st[kk & 1]));
-        return PPL_OK;
-    };
-    int rc = PPL_OK;
-    for (int64_t kk = 0; kk < std::min<int64_t>(2, nchunks); ++kk)
-        if ((rc = r_chunk_in(kk)) != PPL_OK) return rc;
-    // phase B: all slabs on the packed operands
-    rc = run_apply_full(p, p->dL, nullptr, nullptr, nullptr, cs, nullptr, FULL_COMPUTE, p->ev_tau);
-    if (rc != PPL_OK) return rc;
-    PPL_CUDA(cudaEventRecord(p->ev_done, cs));
-    PPL_CUDA(cudaStreamWaitEvent(st[0], p->ev_done, 0));
-    PPL_CUDA(cudaStreamWaitEvent(st[1], p->ev_done, 0));
-    // phase C: R chunk in (the first two are there already), R += term, R chunk out
-    for (int64_t kk = 0; kk < nchunks; ++kk) {
-        const int64_t r0 = kk * p->hchunk_rows, r1 = std::min<int64_t>(rows, r0 + p->hchunk_rows);
-        cudaStream_t s = st[kk & 1];
-        double *buf = p->hstage[kk & 1];
-        const size_t bytes = (size_t)(r1 - r0) * row_bytes;
-        if (kk >= 2 && (rc = r_chunk_in(kk)) != PPL_OK) return rc;
-        if ((rc = launch_unpack_full(p, opts, buf - r0 * p->vv, r0 * p->vv, r1 * p->vv, s)) != PPL_OK) return rc;
-        PPL_CUDA(cudaMemcpyAsync(Rh + r0 * p->vv, buf, bytes, cudaMemcpyDeviceToHost, s));
-    }
-    PPL_CUDA(cudaStreamSynchronize(st[0]));
-    PPL_CUDA(cudaStreamSynchronize(st[1]));
-    PPL_CUDA(cudaStreamSynchronize(cs));
-    const uint64_t nT = (uint64_t)rows * row_bytes;
-    if (h2d) *h2d = (uint64_t)nL + 2 * nT;
-    if (d2h) *d2h = nT;
-    return verify_harvest(p, nullptr);
-}
-
-// An error half way leaves copies and kernels in flight on three streams that read and write the caller's host buffers:
-// wait for them before the error is returned, so that the caller may free or reuse its buffers.
-static int apply_host_full(ppl_plan_s *p, const double *Lh, const double *t2h, double *Rh, uint64_t *h2d, uint64_t *d2h) {
-    const int rc = apply_host_full_queue(p, Lh, t2h, Rh, h2d, d2h);
-    if (rc != PPL_OK) {
-        for (cudaStream_t st : {p->gen, p->hs2, p->host_stream})
-            if (st && cudaStreamSynchronize(st) != cudaSuccess) (void)cudaGetLastError();
-        p->verify_pending = 0;
-    }
-    return rc;
-}
-
-int ppl_apply_host(ppl_plan_t *p, const double *Lh, const double *t2h, double *Rh, uint64_t *h2d, uint64_t *d2h) {
-    if (!p || !Lh || !t2h || !Rh) return fail(PPL_ERR_INVALID_ARG);
-    if (p->sym == PPL_SYM_FULL && p->full_ok && (((uintptr_t)Lh | (uintptr_t)t2h | (uintptr_t)Rh) & 7) == 0)
-        return apply_host_full(p, Lh, t2h, Rh, h2d, d2h);
-    const size_t nL = (size_t)p->x * p->v * p->v * 8, nT = (size_t)p->o * p->o * p->v * p->v * 8;
-    if (!p->dL && cudaMalloc(&p->dL, nL) != cudaSuccess) {
-        (void)cudaGetLastError();
-        p->dL = nullptr;
-        return fail(PPL_ERR_ALLOC);
-    }
-    if (!p->dT) {
-        if (cudaMalloc(&p->dT, nT) != cudaSuccess || cudaMalloc(&p->dR, nT) != cudaSuccess) {
-            (void)cudaGetLastError();
-            if (p->dT) cudaFree(p->dT);
-            if (p->dR) cudaFree(p->dR);
-            p->dT = p->dR = nullptr;
-            return fail(PPL_ERR_ALLOC);
-        }
-    }
-    cudaStream_t s = p->host_stream;
-    PPL_CUDA(cudaMemcpyAsync(p->dL, Lh, nL, cudaMemcpyHostToDevice, s));
-    PPL_CUDA(cudaMemcpyAsync(p->dT, t2h, nT, cudaMemcpyHostToDevice, s));
-    PPL_CUDA(cudaMemcpyAsync(p->dR, Rh, nT, cudaMemcpyHostToDevice, s));
-    int rc = ppl_apply(p, p->dL, p->dT, p->dR, s);
-    if (rc != PPL_OK && cudaStreamSynchronize(s) != cudaSuccess) (void)cudaGetLastError();  // the queued H2D copies read the caller's buffers
-    if (rc == PPL_OK) {
-        cudaError_t e = cudaMemcpyAsync(Rh, p->dR, nT, cudaMemcpyDeviceToHost, s);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-        if (e != cudaSuccess) {
-            (void)cudaGetLastError();
-            rc = fail(PPL_ERR_CUDA);
-        }
-    }
-    if (h2d) *h2d = (uint64_t)nL + 2 * (uint64_t)nT;
-    if (d2h) *d2h = (uint64_t)nT;
-    if (rc == PPL_OK) rc = verify_harvest(p, nullptr);  // the call has synchronised: report a violated precondition at once
-    return rc;
-}
-
 }  // extern "C"
 
 namespace {
@@ -1569,6 +1444,88 @@ int ppl_plan_verify_status(ppl_plan_t *p, int *flags) {
 }
 
 }  // extern "C"
+
+// ---- what ppl_host.cu calls (ppl_launch.h) ----
+namespace pplapi {
+
+int map_2d(CUtensorMap *map, const void *base, uint64_t inner, uint64_t outer, uint64_t row_bytes, uint32_t box_inner,
+           uint32_t box_outer) {
+    return make_map_2d(map, base, inner, outer, row_bytes, box_inner, box_outer);
+}
+
+int step0_tile(const ppl_plan_s *p, const Tile &t, const CUtensorMap *mapA, int a0v, const CUtensorMap *mapB, int b0v, double *W,
+               cudaStream_t s) {
+    ppl::Step0TmaArgs a;
+    a.a0v = a0v;
+    a.b0v = b0v;
+    a.M = t.ta * p->v;
+    a.N = t.tb * p->v;
+    a.K = p->x;
+    a.v = p->v;
+    a.tb = t.tb;
+    a.W = W;
+    a.ldw = p->vv;
+    const int items = ((a.M + ppl::BM - 1) / ppl::BM) * ((a.N + ppl::BN - 1) / ppl::BN);
+    ppl::k_step0_tma<<<std::min(items, p->num_sms), ppl::TMA_THREADS, ppl::SMEM_TMA, s>>>(*mapA, *mapB, a);
+    PPL_CUDA(cudaGetLastError());
+    return PPL_OK;
+}
+
+uint32_t step1_box_rows(const ppl_plan_s *p) { return (uint32_t)p->bm_full; }
+
+int step1_tile(const ppl_plan_s *p, const CUtensorMap *mapT, const double *t2, int slot, const Tile &t, cudaStream_t s) {
+    return launch_step1(p, mapT, &p->mapW[slot], p->mg_full, t2, p->vv, p->slot[slot], p->vv, p->o * p->o, t.ta * t.tb, p->vv, t.full,
+                        p->part, true, s);
+}
+
+int reduce_tile(const ppl_plan_s *p, const Tile &t, double *R, int64_t si, int64_t sj, int64_t sa, int64_t sb, double alpha,
+                double beta, cudaStream_t s) {
+    ppl::ReduceArgs a;
+    a.part = p->part;
+    a.splitk = t.full.splitk;
+    a.M = p->o * p->o;
+    a.N = t.ta * t.tb;
+    a.o = p->o;
+    a.v = p->v;
+    a.tb = t.tb;
+    a.a0 = t.a0;
+    a.b0 = t.b0;
+    a.n_off = 0;
+    a.mirror = t.mirror;
+    a.alpha = alpha;
+    a.beta = beta;
+    a.rs.i = si;
+    a.rs.j = sj;
+    a.rs.a = sa;
+    a.rs.b = sb;
+    a.R = R;
+    const int64_t MN = (int64_t)a.M * a.N;
+    const int grid = (int)std::min<int64_t>((MN + 255) / 256, (int64_t)p->num_sms * 8);
+    ppl::k_reduce<<<grid, 256, 0, s>>>(a);
+    PPL_CUDA(cudaGetLastError());
+    return PPL_OK;
+}
+
+int pack_rows(const ppl_plan_s *p, const double *t2, double diag, cudaStream_t s, int row0, int row1) {
+    return launch_pack(p, t2, PPL_LAYOUT_IJAB, diag, s, row0, row1);
+}
+
+int unpack_range(const ppl_plan_s *p, double *R, int64_t idx0, int64_t idx1, cudaStream_t s) {
+    ppl_opts_t opts;
+    check_opts(nullptr, &opts);
+    return launch_unpack_full(p, opts, R, idx0, idx1, s);
+}
+
+int full_compute(ppl_plan_s *p, const double *L, cudaStream_t s, cudaEvent_t tau_ready) {
+    return run_apply_full(p, L, nullptr, nullptr, nullptr, s, nullptr, FULL_COMPUTE, tau_ready);
+}
+
+int verify_begin(ppl_plan_s *p, const double *L, const double *t2, int t2_layout, cudaStream_t stream) {
+    return ::verify_begin(p, L, t2, t2_layout, stream);
+}
+int verify_harvest(ppl_plan_s *p, int *flags_out) { return ::verify_harvest(p, flags_out); }
+
+}  // namespace pplapi
 
 // ---- plain GEMMs on the TMA kernels, for ppl_contract_pair's fast paths (ppl_internal.h) ----
 // C[M][N] (dense) = beta C + alpha A^T B with A[K][M], B[K][N] dense row-major ("k-outer": 'k..m..,k..n..->m..n..'): k_step0_tma

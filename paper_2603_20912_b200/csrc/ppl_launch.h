@@ -1,0 +1,33 @@
+// ppl_launch.h -- internal: what ppl_host.cu (host-resident operands) needs from ppl_api.cu, where the kernels are
+// instantiated: single launches of the hot-path kernels, the slab loop of PPL_SYM_FULL, the precondition check.
+#pragma once
+#include "ppl_plan.h"
+
+namespace pplapi {
+
+// 2-D FP64 tensor map {inner (contiguous), outer}, row stride row_bytes, box {box_inner, box_outer}, SWIZZLE_128B, zero fill
+int map_2d(CUtensorMap *map, const void *base, uint64_t inner, uint64_t outer, uint64_t row_bytes, uint32_t box_inner,
+           uint32_t box_outer);
+
+// step 0 of one W tile with the row and the column operand given as two tensor maps {inner = columns, outer = nchol} and
+// the first column of the tile's a-block / b-block inside each (the whole L: a0 * nvirt; a row panel of its own: 0)
+int step0_tile(const ppl_plan_s *p, const pplh::Tile &t, const CUtensorMap *mapA, int a0v, const CUtensorMap *mapB, int b0v, double *W,
+               cudaStream_t s);
+// step 1 of one W tile of the un-packed modes out of ring slot `slot` into the plan's split-K partials; mapT: t2 as
+// {inner = nvirt^2, outer = nocc^2}, box {BK, step1_tile_m}
+int step1_tile(const ppl_plan_s *p, const CUtensorMap *mapT, const double *t2, int slot, const pplh::Tile &t, cudaStream_t s);
+// fixed-order sum of the partials into R[i,j,a,b] (+ the mirror if the tile has one); R = address of element (0,0,0,0)
+// with element strides (si, sj, sa, sb): the caller's array, or a slab buffer that holds only the tile's a-block
+int reduce_tile(const ppl_plan_s *p, const pplh::Tile &t, double *R, int64_t si, int64_t sj, int64_t sa, int64_t sb, double alpha,
+                double beta, cudaStream_t s);
+uint32_t step1_box_rows(const ppl_plan_s *p);  // TMA box rows of the t2 map of step1_tile
+
+// PPL_SYM_FULL pieces (ppl_apply_host packs and unpacks chunk by chunk)
+int pack_rows(const ppl_plan_s *p, const double *t2, double diag, cudaStream_t s, int row0, int row1);
+int unpack_range(const ppl_plan_s *p, double *R, int64_t idx0, int64_t idx1, cudaStream_t s);
+int full_compute(ppl_plan_s *p, const double *L, cudaStream_t s, cudaEvent_t tau_ready);  // all slabs on the packed operands
+
+int verify_begin(ppl_plan_s *p, const double *L, const double *t2, int t2_layout, cudaStream_t stream);
+int verify_harvest(ppl_plan_s *p, int *flags_out);
+
+}  // namespace pplapi

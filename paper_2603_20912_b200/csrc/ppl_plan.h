@@ -112,6 +112,18 @@ struct ppl_plan_s {
     int hchunk_rows = 0;                                 // (i,j) rows per chunk
     cudaStream_t hs2 = nullptr;                          // second chunk stream of ppl_apply_host (the first is `gen`)
     cudaEvent_t ev_tau = nullptr, ev_done = nullptr;     // tau+- complete / all slabs done
+    // ppl_apply_host in the un-packed modes (ppl_host.cu): L row panels, R slabs, their streams and events
+    struct HostStream {
+        double *pa[2] = {nullptr, nullptr};              // panel L[:, A, :] of the current / next row of tiles: [x][ta * v]
+        double *pb[pplh::MAX_RING] = {};                 // panels L[:, B, :], one per W slot
+        double *rs[2] = {nullptr, nullptr};              // R slab [o*o][ta * v] of the current / next row (PPL_SYM_NONE)
+        size_t panel_bytes = 0, slab_bytes = 0;
+        int npb = 0;
+        cudaStream_t in = nullptr, out = nullptr;        // H2D copies / D2H copies
+        cudaEvent_t ev_pa[2] = {}, ev_pafree[2] = {}, ev_pb[pplh::MAX_RING] = {}, ev_pbfree[pplh::MAX_RING] = {};
+        cudaEvent_t ev_rsin[2] = {}, ev_rsdone[2] = {}, ev_rsfree[2] = {}, ev_t2 = nullptr, ev_fork = nullptr;
+        bool events = false;
+    } hsn;
     double f_step0 = 0, f_step1 = 0;
     CUtensorMap mapW[pplh::MAX_RING], mapWp[pplh::MAX_RING], mapWm[pplh::MAX_RING], mapTp, mapTm;  // plan-owned operands
     // ---- PPL_SYM_FULL (own allocation `fws`; shares taup/taum with PPL_SYM_PAIR_SA) ----
