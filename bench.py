@@ -464,7 +464,11 @@ def run_ours(name, o, v, x, args, steps, warmup, dist, dev, rank, world, peak):
     torch.cuda.synchronize()
 
     t0 = time.perf_counter()
-    plan = P.Plan(o, v, x, int(args.workspace_gb * (1 << 30)), debug={"no_small_fused": 1} if args.no_small_fused else None)
+    debug = {"no_small_fused": 1} if args.no_small_fused else {}
+    for kv in (args.debug.split(",") if args.debug else []):  # A/B runs: ppl_debug_opts_t fields by name
+        k_, v_ = kv.split("=")
+        debug[k_] = int(v_)
+    plan = P.Plan(o, v, x, int(args.workspace_gb * (1 << 30)), debug=debug or None)
     plan_s = time.perf_counter() - t0
     if args.symmetry != "default":
         plan.set_symmetry({v_: k_ for k_, v_ in SYM_NAMES.items()}[args.symmetry])
@@ -626,6 +630,7 @@ def main():
                     help="A/B: send launch-bound shapes (tiny, small) through the tiled path instead of the one fused kernel")
     ap.add_argument("--host-panels", type=int, default=0, choices=[0, 1, 2],
                     help="table3_* with --symmetry none|pair: 1 = stream L as row panels even if it fits whole, 2 = never")
+    ap.add_argument("--debug", default="", help="ppl_debug_opts_t fields for A/B runs, e.g. full_group_m=12,full_hints=5")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=0, help="timed ppl_apply_host calls (0 = --steps)")
     ap.add_argument("--no-secondary", action="store_true", help="with --config xl: skip the 'large' sub-record")

@@ -71,7 +71,7 @@ class ppl_debug_opts_t(ctypes.Structure):
     """include/ppl.h ppl_debug_opts_t: planner / orchestration knobs for tests and A/B runs; all zero = the defaults."""
     _fields_ = [(k, c_int32) for k in (
         "tile_edge", "ni_max", "cpasync_kernels", "full_min_v", "full_tbg", "full_slots", "full_strips", "full_tight",
-        "full_rect_tiles", "full_no_diag_pack", "full_serial", "debug_sync", "trace", "host_chunk_mb", "no_small_fused", "host_panels")] + [("reserved", c_int32 * 16)]
+        "full_rect_tiles", "full_no_diag_pack", "full_serial", "debug_sync", "trace", "host_chunk_mb", "no_small_fused", "host_panels", "full_group_m", "full_hints")] + [("reserved", c_int32 * 14)]
 
 
 # Options merged under every Plan(...) / ppl_plan_dry(...) of this process.  Empty in the product; tests/conftest.py sets it so

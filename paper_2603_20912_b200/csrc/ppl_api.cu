@@ -165,7 +165,7 @@ EncodeTiledFn get_encode() {
 // 2-D FP64 tensor {inner (contiguous), outer} with row stride `row_bytes`, box {box_inner, box_outer}, 128B swizzle;
 // out-of-bounds elements of a box are filled with zeros (tile edges, k tails)
 int make_map_2d(CUtensorMap *map, const void *base, uint64_t inner, uint64_t outer, uint64_t row_bytes, uint32_t box_inner,
-                uint32_t box_outer) {
+                uint32_t box_outer, bool promo128 = false) {
     EncodeTiledFn enc = get_encode();
     if (!enc || inner == 0 || outer == 0) return PPL_ERR_CUDA;
     const cuuint64_t gdim[2] = {inner, outer};
@@ -173,7 +173,8 @@ int make_map_2d(CUtensorMap *map, const void *base, uint64_t inner, uint64_t out
     const cuuint32_t box[2] = {box_inner, box_outer};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void *>(base), gdim, gstride, box, estr,
-                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                           promo128 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B : CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS ? PPL_OK : PPL_ERR_CUDA;
 }
@@ -739,7 +740,8 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
         L = p->Lpad;
     }
     CUtensorMap mapL;
-    if (make_map_2d(&mapL, L, (uint64_t)p->vvp, (uint64_t)p->x, (uint64_t)p->vvp * 8, 16, ppl::BK) != PPL_OK) return fail(PPL_ERR_CUDA);
+    if (make_map_2d(&mapL, L, (uint64_t)p->vvp, (uint64_t)p->x, (uint64_t)p->vvp * 8, 16, ppl::BK, (p->dbg.full_hints & 8) != 0) != PPL_OK)
+        return fail(PPL_ERR_CUDA);
     if (p->Lq && p->diag_pack && !p->full_tight) {  // the diagonal 16 x 16 blocks of L, pairs b <= d only (|L| / (nvirt / 16) bytes)
         const int64_t total = (int64_t)p->x * p->nfull * ppl::DIAG_PACKED;
         const int grid = (int)std::min<int64_t>((total + 255) / 256, (int64_t)p->num_sms * 8);
@@ -804,7 +806,9 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
         {   // row panels of one raster group: about 40 MB of L2 (126 MB, shared with the streamed column panels and the stores)
             const double panel = 128.0 * p->x * 8.0;
             a0.group_m = (int)std::max(8.0, std::min((double)a0.tiles_m, std::floor(40e6 / panel)));
+            if (p->dbg.full_group_m > 0) a0.group_m = p->dbg.full_group_m;
         }
+        a0.hints = p->dbg.full_hints & 7;
         const int items = a0.tiles_m * a0.tiles_n;
         if (dual && unit_no >= 2) PPL_CUDA(cudaStreamWaitEvent(s0, p->ev_xfree[xi], 0));  // the folds of unit u - 2 have read this strip
         tb("step0", t ? t->bg0 : sl.A0, 0, s0);

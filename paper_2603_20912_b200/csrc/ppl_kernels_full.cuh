@@ -53,6 +53,7 @@ struct Step0SlabArgs {
     int group_m;         // raster: row tiles per group.  A group sweeps all column tiles once, its group_m row panels (128 x
                          // nchol doubles each) staying in L2: the L rows behind the column tiles are read from DRAM once per
                          // GROUP, so the planner makes groups as tall as a ~40 MB L2 share allows (large: 24, XL: 16; was 12)
+    int hints;           // L2 policy bits (ppl_debug_opts_t.full_hints): 1 evict_last row panels, 2 evict_first column panels, 4 streaming stores
     int image;           // 1: chunks cover d-block >= b-block only and the epilogue stores the b<->d image too (rows of
                          // every b >= A0 must be in the strip); 0: the chunks cover the full (b, d) rectangle of the group
 };
@@ -88,15 +89,16 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
                     xb[i] = ch.x >= 0 ? ch.x * v + ch.y : (ch.x == -1 ? vv : ch.y);
                     packed |= (ch.x <= -2 ? 1u : 0u) << i;
                 }
+                const uint64_t pol_a = (p.hints & 1) ? L2_EVICT_LAST : L2_EVICT_NORMAL, pol_b = (p.hints & 2) ? L2_EVICT_FIRST : L2_EVICT_NORMAL;
                 for (int kt = 0; kt < nkt; ++kt) {
                     mbar_wait(&sm.empty[stage], phase ^ 1);
                     mbar_expect_tx(&sm.full[stage], STAGE_BYTES);
                     double *da = sm.a + (size_t)stage * BM * BK, *db = sm.b + (size_t)stage * BN * BK;
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) tma_load_2d(da + i * BK * 16, &mapL, xa[i], kt * BK, &sm.full[stage]);
+                    for (int i = 0; i < 8; ++i) tma_load_2d_hint(da + i * BK * 16, &mapL, xa[i], kt * BK, &sm.full[stage], pol_a);
 #pragma unroll
                     for (int i = 0; i < 8; ++i)
-                        tma_load_2d(db + i * BK * 16, ((packed >> i) & 1) ? &mapQ : &mapL, xb[i], kt * BK, &sm.full[stage]);
+                        tma_load_2d_hint(db + i * BK * 16, ((packed >> i) & 1) ? &mapQ : &mapL, xb[i], kt * BK, &sm.full[stage], pol_b);
                     if (++stage == TSTAGES) {
                         stage = 0;
                         phase ^= 1;
@@ -194,7 +196,10 @@ __global__ void __launch_bounds__(TMA_THREADS, 1)
                         const int d = d0 + 2 * q + 8 * h;
                         const double v0 = acc[2 * i + e][2 * j][h], v1 = acc[2 * i + e][2 * j + 1][h];
                         if (d + 1 < v) {  // v even (TMA path), d even: 16-byte aligned
-                            *reinterpret_cast<double2 *>(xa + (int64_t)b * vv + d) = make_double2(v0, v1);
+                            if (p.hints & 4)
+                                __stcs(reinterpret_cast<double2 *>(xa + (int64_t)b * vv + d), make_double2(v0, v1));
+                            else
+                                *reinterpret_cast<double2 *>(xa + (int64_t)b * vv + d) = make_double2(v0, v1);
                             if (offdiag && !pair) {
                                 xa[(int64_t)d * vv + b] = v0;
                                 xa[(int64_t)(d + 1) * vv + b] = v1;

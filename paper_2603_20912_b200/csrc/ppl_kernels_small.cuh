@@ -33,6 +33,7 @@ namespace ppl {
 constexpr int SMALL_SW = 4;        // warps (= b's) per CTA
 constexpr int SMALL_STAGES = 3;
 constexpr int SMALL_THREADS = 32 * SMALL_SW;
+constexpr int SMALL_MAX_OO = 64;   // nocc <= 8
 
 struct SmallArgs {
     const double *L;     // [x][v][ldl] (ldl even, 16-byte aligned: the caller's L, or the padded copy)
@@ -53,7 +54,9 @@ struct SmallCfg {
     static constexpr int LDB = SMALL_SW * W8 + 4;          // [k][(b_l, d)]: the SW rows of one P are contiguous, ldl apart
     static constexpr int STAGE = BK * (LDA + LDB);         // doubles
     static constexpr int RING = SMALL_STAGES * STAGE;
-    static constexpr size_t SMEM = (size_t)RING * sizeof(double) + 64;  // + the mbarriers
+    static constexpr int LDT = W8 + ((NB & 1) ? 0 : 8);    // row stride of a staged t2 block: 8 (mod 16) doubles (see step 1)
+    static constexpr size_t SMEM = (size_t)RING * sizeof(double) + 64 + (size_t)SMALL_SW * SMALL_MAX_OO * sizeof(double);  // + mbarriers + results
+    __device__ static double *results(double *sm) { return sm + RING + 8; }  // behind the ring and the 5 mbarriers
 };
 
 // ---- mbarrier / bulk-copy primitives (as in ppl_kernels_tma.cuh; repeated here so that this header stands alone) ----
@@ -191,24 +194,32 @@ __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArg
             }
 
         // ---- step 1 from the accumulators.  W_ab block (i, j) holds c = 8 i + g, d = 8 j + 2 q, + 1.  The (i', j') blocks of t2
-        // ([nvirt][ldt] doubles each, contiguous) come in by one bulk copy each, two per pass, double-buffered, and are read back
-        // as 16-byte pairs (d, d + 1).  Whatever a pair reads beyond a block's rows / columns is finite and meets a zero of W.
+        // come in row by row (one bulk copy per row of ldt doubles, issued by the lanes of warp 0) into rows of LDT doubles --
+        // LDT = 8 (mod 16), so that the 16-byte pairs (d, d + 1) a quarter warp reads (two consecutive g's, q = 0..3) fall into
+        // eight different bank groups: ncu showed step 1 bound by shared-memory wavefronts, half of them bank conflicts, with
+        // rows at the natural stride.  Several blocks per pass, double-buffered.  Whatever a pair reads beyond a block's rows /
+        // columns is finite and meets a zero of W.
         __syncthreads();  // every warp has left the k loop: the ring is free
         const int b = b0 + warp;
         const int oo = p.o * p.o;
-        const int tblk = v * ldt;                             // doubles per staged block
+        constexpr int LDT = Cfg::LDT;
+        const int tblk = v * LDT;                             // doubles per staged block
         // blocks per pass: as many as two halves of the ring hold (a fragment pair may read up to 8 NB rows / columns into what
-        // follows its block, which must stay inside the ring): 2 at nvirt = 53, 7 at nvirt = 20 -- fewer, longer passes
-        const int bpp = max(1, min(8, ((Cfg::RING - (8 * NB - 1) * ldt - 8 * NB) / tblk + 1) / 2));
+        // follows its block, which must stay inside the ring)
+        const int bpp = max(1, min(8, ((Cfg::RING - (8 * NB - 1) * LDT - 8 * NB) / tblk + 1) / 2));
         const int npass = (oo + bpp - 1) / bpp;
         auto load_pass = [&](int ps) {                        // blocks bpp ps ... into half (ps & 1)
-            if (tid != 0) return;
+            if (warp != 0) return;
             const int h = ps & 1, n = min(bpp, oo - bpp * ps);
-            sm_mbar_expect_tx(&tfull[h], (uint32_t)n * tblk * 8);
-            for (int u = 0; u < n; ++u)
-                sm_bulk_g2s(sm + (h * bpp + u) * tblk, p.t2 + (int64_t)(bpp * ps + u) * tblk, (uint32_t)tblk * 8, &tfull[h]);
+            if (lane == 0) sm_mbar_expect_tx(&tfull[h], (uint32_t)n * v * ldt * 8);
+            __syncwarp();
+            for (int r = lane; r < n * v; r += 32) {
+                const int u = r / v, c = r - u * v;
+                sm_bulk_g2s(sm + (h * bpp + u) * tblk + c * LDT, p.t2 + ((int64_t)(bpp * ps + u) * v + c) * ldt, (uint32_t)ldt * 8, &tfull[h]);
+            }
         };
         load_pass(0);
+        double *res = Cfg::results(sm) + warp * SMALL_MAX_OO;  // this warp's nocc^2 results
         for (int ps = 0; ps < npass; ++ps) {
             if (ps + 1 < npass) load_pass(ps + 1);            // (its half was read in pass ps - 1: the barrier below, last iteration)
             const int h = ps & 1;
@@ -219,14 +230,14 @@ __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArg
                 for (int u0 = 0; u0 < n; u0 += 2) {           // two blocks at a time: four independent FMA chains
                     double s[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
                     const int u1 = min(u0 + 1, n - 1);        // (an odd last block is read twice and stored once)
-                    const double *t0 = sm + (h * bpp + u0) * tblk + g * ldt + 2 * q;
+                    const double *t0 = sm + (h * bpp + u0) * tblk + g * LDT + 2 * q;
                     const int du = (u1 - u0) * tblk;
 #pragma unroll
                     for (int i = 0; i < NB; ++i)
 #pragma unroll
                         for (int j = 0; j < NB; ++j) {
-                            const double2 ta = *reinterpret_cast<const double2 *>(t0 + 8 * i * ldt + 8 * j);
-                            const double2 tb = *reinterpret_cast<const double2 *>(t0 + du + 8 * i * ldt + 8 * j);
+                            const double2 ta = *reinterpret_cast<const double2 *>(t0 + 8 * i * LDT + 8 * j);
+                            const double2 tb = *reinterpret_cast<const double2 *>(t0 + du + 8 * i * LDT + 8 * j);
                             s[0][0] = fma(acc[i][j][0], ta.x, s[0][0]);
                             s[0][1] = fma(acc[i][j][1], ta.y, s[0][1]);
                             s[1][0] = fma(acc[i][j][0], tb.x, s[1][0]);
@@ -238,19 +249,21 @@ __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArg
 #pragma unroll
                         for (int m = 16; m >= 1; m >>= 1) r[u] += __shfl_xor_sync(0xffffffffu, r[u], m);
                     }
-                    if (lane == 0) {
-#pragma unroll
-                        for (int u = 0; u < 2; ++u) {
-                            if (u0 + u >= n) break;
-                            const int ij = bpp * ps + u0 + u;
-                            const int i_ = ij / p.o, j_ = ij - i_ * p.o;
-                            r_update(p.R + i_ * p.rs.i + j_ * p.rs.j + a * p.rs.a + b * p.rs.b, r[u], p.alpha, p.beta);
-                            if (p.pair && a != b) r_update(p.R + j_ * p.rs.i + i_ * p.rs.j + b * p.rs.a + a * p.rs.b, r[u], p.alpha, p.beta);
-                        }
-                    }
+                    if (lane < 2 && u0 + lane < n) res[bpp * ps + u0 + lane] = lane ? r[1] : r[0];
                 }
             }
             __syncthreads();  // pass ps has been read: its half may be refilled
+        }
+        // R[i,j,a,b] (and the mirror): one (i,j) per lane, so that the read-modify-writes of a warp are in flight together
+        // (one result at a time from lane 0, each behind its own global load, was 40 % of the stall samples at tiny)
+        if (b < v) {
+            __syncwarp();
+            for (int ij = lane; ij < oo; ij += 32) {
+                const int i_ = ij / p.o, j_ = ij - i_ * p.o;
+                const double val = res[ij];
+                r_update(p.R + i_ * p.rs.i + j_ * p.rs.j + a * p.rs.a + b * p.rs.b, val, p.alpha, p.beta);
+                if (p.pair && a != b) r_update(p.R + j_ * p.rs.i + i_ * p.rs.j + b * p.rs.a + a * p.rs.b, val, p.alpha, p.beta);
+            }
         }
     }
 }
