@@ -186,10 +186,10 @@ typedef struct ppl_debug_opts_s {
                                  path of the plan's symmetry mode runs instead (tests of the tiled kernels at small shapes) */
     int32_t host_panels;      /* ppl_apply_host, un-packed modes: 1 = stream L as row panels even when L fits on the device whole,
                                  2 = never (L whole or PPL_ERR_ALLOC); 0 = panels only when L does not fit beside t2 */
-    int32_t full_group_m;     /* PPL_SYM_FULL, step 0: row tiles per raster group (0 = the planner's choice) */
-    int32_t full_hints;       /* PPL_SYM_FULL, step 0: L2 policy experiments, a bit mask: 1 = evict_last on the row-panel loads,
-                                 2 = evict_first on the column-panel loads, 4 = streaming (evict-first) stores of the strip,
-                                 8 = 128-byte instead of 256-byte L2 promotion of the TMA loads of L */
+    int32_t full_group_m;     /* PPL_SYM_FULL, step 0: row tiles per raster group (0 = 12) */
+    int32_t full_hints;       /* PPL_SYM_FULL, step 0: L2 policy, a bit mask: 1 = evict_last on the row-panel loads, 2 = evict_first
+                                 on the column-panel loads, 4 = streaming (evict-first) stores of the strip, 8 = 128-byte instead
+                                 of 256-byte L2 promotion of the TMA loads of L; 0 = the default (1 + 4 + 8), -1 = none */
     int32_t reserved[14];     /* must be zero */
 } ppl_debug_opts_t;
 

@@ -89,6 +89,7 @@ void free_plan(ppl_plan_s *p) {
     if (p->small_Lp) cudaFree(p->small_Lp);
     if (p->small_tp) cudaFree(p->small_tp);
     if (p->vflags_host) cudaFreeHost(p->vflags_host);
+    if (p->vdone_dev) cudaFree(p->vdone_dev);
     if (p->ev_verify) cudaEventDestroy(p->ev_verify);
     if (p->tperm) cudaFree(p->tperm);
     if (p->dL) cudaFree(p->dL);
@@ -138,7 +139,7 @@ int set_kernel_attrs() {
     PPL_ATTR_NI(1) PPL_ATTR_NI(2) PPL_ATTR_NI(3) PPL_ATTR_NI(4) PPL_ATTR_NI(5) PPL_ATTR_NI(6) PPL_ATTR_NI(7) PPL_ATTR_NI(8) PPL_ATTR_NI(9) PPL_ATTR_NI(10)
 #undef PPL_ATTR_NI
 #define PPL_ATTR_SMALL(NB) \
-    PPL_CUDA(cudaFuncSetAttribute(ppl::k_small_fused<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SmallCfg<NB>::SMEM));
+    PPL_CUDA(cudaFuncSetAttribute(ppl::k_small_fused<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     PPL_ATTR_SMALL(1) PPL_ATTR_SMALL(2) PPL_ATTR_SMALL(3) PPL_ATTR_SMALL(4) PPL_ATTR_SMALL(5) PPL_ATTR_SMALL(6) PPL_ATTR_SMALL(7)
 #undef PPL_ATTR_SMALL
     if (known) g_attr_set[dev].store(true);
@@ -691,6 +692,9 @@ int launch_reduce_acc(const ppl_plan_s *p, const FullTile &t, const double *part
     return PPL_OK;
 }
 
+// L2 policy bits of step 0 (ppl_debug_opts_t.full_hints: 0 = the default 1 + 4 + 8, -1 = none)
+inline int step0_hints(const ppl_plan_s *p) { return p->dbg.full_hints == 0 ? 13 : (p->dbg.full_hints < 0 ? 0 : p->dbg.full_hints); }
+
 // The whole path in PPL_SYM_FULL: everything on the caller's stream (every kernel fills the GPU; the
 // strip is single-buffered), prof as in run_apply.
 enum { FULL_PACK = 1, FULL_COMPUTE = 2, FULL_UNPACK = 4, FULL_ALL = 7 };
@@ -740,7 +744,7 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
         L = p->Lpad;
     }
     CUtensorMap mapL;
-    if (make_map_2d(&mapL, L, (uint64_t)p->vvp, (uint64_t)p->x, (uint64_t)p->vvp * 8, 16, ppl::BK, (p->dbg.full_hints & 8) != 0) != PPL_OK)
+    if (make_map_2d(&mapL, L, (uint64_t)p->vvp, (uint64_t)p->x, (uint64_t)p->vvp * 8, 16, ppl::BK, (step0_hints(p) & 8) != 0) != PPL_OK)
         return fail(PPL_ERR_CUDA);
     if (p->Lq && p->diag_pack && !p->full_tight) {  // the diagonal 16 x 16 blocks of L, pairs b <= d only (|L| / (nvirt / 16) bytes)
         const int64_t total = (int64_t)p->x * p->nfull * ppl::DIAG_PACKED;
@@ -803,12 +807,13 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
         a0.rows_per_a = t ? t->tbp : p->vp;
         a0.b_base = t ? t->bg0 : 0;
         a0.image = t ? 0 : 1;
-        {   // row panels of one raster group: about 40 MB of L2 (126 MB, shared with the streamed column panels and the stores)
-            const double panel = 128.0 * p->x * 8.0;
-            a0.group_m = (int)std::max(8.0, std::min((double)a0.tiles_m, std::floor(40e6 / panel)));
-            if (p->dbg.full_group_m > 0) a0.group_m = p->dbg.full_group_m;
-        }
-        a0.hints = p->dbg.full_hints & 7;
+        // Raster and L2 policy of step 0, from ncu's DRAM bytes of one slab (profiles/r02_step0_l2.md): the 148 persistent CTAs
+        // drift apart, so a panel is shared only while it survives in L2.  Groups of 12 row tiles (a wave covers ~12 x 12 tiles:
+        // the fewest panels per wave), 128-byte instead of 256-byte L2 promotion of the TMA loads (a box row is 128 bytes: the
+        // promoted other half belongs to a column tile that runs much later), evict_last on the row panels and streaming
+        // stores of the strip: 204 -> 82 GB read per slab at XL, 7.5 -> 3.5 GB at large, same kernel time (DMMA-bound).
+        a0.group_m = p->dbg.full_group_m > 0 ? p->dbg.full_group_m : ppl::GROUP_M;
+        a0.hints = step0_hints(p) & 7;
         const int items = a0.tiles_m * a0.tiles_n;
         if (dual && unit_no >= 2) PPL_CUDA(cudaStreamWaitEvent(s0, p->ev_xfree[xi], 0));  // the folds of unit u - 2 have read this strip
         tb("step0", t ? t->bg0 : sl.A0, 0, s0);
@@ -1036,7 +1041,8 @@ ppl_plan_t *ppl_plan_ex(int nocc, int nvirt, int nchol, size_t workspace_bytes, 
         return nullptr;
     }
     if (cudaMalloc(&p->ws, p->ws_bytes) != cudaSuccess ||
-        cudaHostAlloc(&p->vflags_host, 4 * sizeof(int), cudaHostAllocMapped) != cudaSuccess ||
+        cudaHostAlloc(&p->vflags_host, 8 * sizeof(int), cudaHostAllocMapped) != cudaSuccess ||
+        cudaMalloc(&p->vdone_dev, sizeof(int)) != cudaSuccess || cudaMemset(p->vdone_dev, 0, sizeof(int)) != cudaSuccess ||
         cudaEventCreateWithFlags(&p->ev_verify, cudaEventDisableTiming) != cudaSuccess) {
         (void)cudaGetLastError();
         free_plan(p);
@@ -1125,7 +1131,7 @@ namespace {
 
 // Launch-bound shapes: the whole ladder in one launch (ppl_kernels_small.cuh).  prof: an event pair around it.
 int run_apply_small(ppl_plan_s *p, const double *L, const double *t2, double *R, const ppl_opts_t *opts_in, cudaStream_t stream,
-                    Prof *prof) {
+                    Prof *prof, bool fused_check = false) {
     bool vec16 = false;
     int rc = check_ptrs(p, L, t2, R, &vec16);
     ppl_opts_t opts;
@@ -1135,7 +1141,7 @@ int run_apply_small(ppl_plan_s *p, const double *L, const double *t2, double *R,
     if (prof && prof->mark(-1, 0, stream) != PPL_OK) return fail(PPL_ERR_CUDA);
     // bulk copies want 16-byte aligned rows of even length: otherwise (odd nvirt, t2 stored 'iajb', misaligned buffers) the
     // operands are first copied into the plan's padded buffers
-    const int vp = p->vp;
+    const int vp = p->vp, nb8 = (p->v + 7) / 8, ldt_pack = 8 * nb8 + ((nb8 & 1) ? 0 : 8);  // = ppl::SmallCfg<NB>::LDT
     const bool pack_L = (p->v & 1) || ((uintptr_t)L & 15), pack_t = (p->v & 1) || opts.t2_layout != PPL_LAYOUT_IJAB || ((uintptr_t)t2 & 15);
     if (pack_L || pack_t) {
         if (pack_L && !p->small_Lp && cudaMalloc(&p->small_Lp, (size_t)p->x * p->v * vp * 8) != cudaSuccess) {
@@ -1143,22 +1149,22 @@ int run_apply_small(ppl_plan_s *p, const double *L, const double *t2, double *R,
             p->small_Lp = nullptr;
             return fail(PPL_ERR_ALLOC);
         }
-        if (pack_t && !p->small_tp && cudaMalloc(&p->small_tp, (size_t)p->o * p->o * p->v * vp * 8) != cudaSuccess) {
+        if (pack_t && !p->small_tp && cudaMalloc(&p->small_tp, (size_t)p->o * p->o * p->v * ldt_pack * 8) != cudaSuccess) {
             (void)cudaGetLastError();
             p->small_tp = nullptr;
             return fail(PPL_ERR_ALLOC);
         }
-        const int64_t n = (pack_L ? (int64_t)p->x * p->v * vp : 0) + (pack_t ? (int64_t)p->o * p->o * p->v * vp : 0);
+        const int64_t n = (pack_L ? (int64_t)p->x * p->v * vp : 0) + (pack_t ? (int64_t)p->o * p->o * p->v * ldt_pack : 0);
         const int g = (int)std::min<int64_t>((n + 255) / 256, (int64_t)p->num_sms * 8);
         ppl::k_small_prepack<<<g, 256, 0, stream>>>(pack_L ? L : nullptr, pack_t ? t2 : nullptr, p->small_Lp, p->small_tp, p->o, p->v, p->x,
-                                                  vp, r_strides(p->o, p->v, opts.t2_layout));
+                                                  vp, ldt_pack, r_strides(p->o, p->v, opts.t2_layout));
         PPL_CUDA(cudaGetLastError());
     }
     ppl::SmallArgs a;
     a.L = pack_L ? p->small_Lp : L;
     a.ldl = pack_L ? vp : p->v;
     a.t2 = pack_t ? p->small_tp : t2;
-    a.ldt = pack_t ? vp : p->v;
+    a.ldt = pack_t ? ldt_pack : p->v;
     a.R = R;
     a.o = p->o;
     a.v = p->v;
@@ -1168,11 +1174,43 @@ int run_apply_small(ppl_plan_s *p, const double *L, const double *t2, double *R,
     a.alpha = opts.alpha;
     a.beta = opts.beta;
     a.rs = r_strides(p->o, p->v, opts.r_layout);
-    const int grid = std::min(a.nitems, 2 * p->num_sms);
+    a.chk.L = a.chk.t2 = nullptr;
+    a.chk.flags = nullptr;
+    a.ncheck = 0;
+    a.seq = 0;
+    a.done = p->vdone_dev;
+    if (fused_check) {  // PPL_OPT_VERIFY_INPUTS = 1: the caller's arrays, scanned by the first CTAs of the same launch
+        a.chk.L = p->sym == PPL_SYM_FULL ? L : nullptr;
+        a.chk.t2 = t2;
+        a.chk.o = p->o;
+        a.chk.v = p->v;
+        a.chk.x = p->x;
+        const ppl::RStrides ts = r_strides(p->o, p->v, opts.t2_layout);
+        a.chk.s_i = ts.i;
+        a.chk.s_j = ts.j;
+        a.chk.s_c = ts.a;
+        int *dflags = nullptr;
+        PPL_CUDA(cudaHostGetDevicePointer(&dflags, p->vflags_host, 0));
+        a.chk.flags = dflags;
+        const int nb = (p->v + 31) / 32;
+        const int64_t items = (a.chk.L ? (int64_t)p->x * nb * (nb + 1) / 2 : 0) + (int64_t)p->o * (p->o + 1) / 2 * nb * nb;
+        a.ncheck = (int)std::max<int64_t>(1, std::min<int64_t>(16, items / 4));
+        a.seq = ++p->vseq;
+        p->vflags_host[0] = p->vflags_host[1] = 0;
+    }
+    const int grid = std::min(a.nitems, 2 * p->num_sms) + a.ncheck;
+    // all of t2 staged once per CTA when every CTA has one work item and the region fits beside the ring (tiny: 80 KB)
+    const size_t t2_region = ((size_t)p->o * p->o * p->v * a.ldt + (size_t)8 * nb8 * a.ldt + 8 * nb8) * 8;
+    size_t smem_extra = 0;
+    a.t2_resident = 0;
+    if (a.nitems + a.ncheck <= p->num_sms && t2_region <= (size_t)96 * 1024 && t2_region < ((size_t)1 << 20)) {
+        a.t2_resident = 1;
+        smem_extra = t2_region;
+    }
     switch ((p->v + 7) / 8) {
 #define PPL_LAUNCH_SMALL(NB)                                                                                    \
     case NB:                                                                                                    \
-        ppl::k_small_fused<NB><<<grid, ppl::SMALL_THREADS, ppl::SmallCfg<NB>::SMEM, stream>>>(a);              \
+        ppl::k_small_fused<NB><<<grid, ppl::SMALL_THREADS, ppl::SmallCfg<NB>::SMEM + smem_extra, stream>>>(a); \
         break;
         PPL_LAUNCH_SMALL(1) PPL_LAUNCH_SMALL(2) PPL_LAUNCH_SMALL(3) PPL_LAUNCH_SMALL(4) PPL_LAUNCH_SMALL(5) PPL_LAUNCH_SMALL(6)
             PPL_LAUNCH_SMALL(7)
@@ -1180,6 +1218,10 @@ int run_apply_small(ppl_plan_s *p, const double *L, const double *t2, double *R,
         default: return fail(PPL_ERR_INVALID_ARG);
     }
     PPL_CUDA(cudaGetLastError());
+    if (fused_check) {
+        p->verify_pending = 2;
+        p->vstream = stream;
+    }
     if (prof && prof->mark(K_STEP0, 1 + ((pack_L || pack_t) ? 1 : 0), stream) != PPL_OK) return fail(PPL_ERR_CUDA);
     return PPL_OK;
 }
@@ -1253,6 +1295,8 @@ int ppl_apply_ex(ppl_plan_t *p, const double *L, const double *t2, double *R, co
         int rc = verify_harvest(p, nullptr);  // what the previous apply's check found
         if (rc != PPL_OK) return rc;
         if (p->verify && p->sym != PPL_SYM_NONE) {
+            // launch-bound shapes: the check rides in the apply's one launch (its first CTAs) instead of a launch of its own
+            if (p->verify == 1 && p->small_ok) return run_apply_small(p, L, t2, R, opts, stream, nullptr, true);
             ppl_opts_t o;
             if (check_opts(opts, &o) != PPL_OK) return fail(PPL_ERR_INVALID_ARG);
             rc = verify_begin(p, p->sym == PPL_SYM_FULL ? L : nullptr, t2, o.t2_layout, stream);
@@ -1403,8 +1447,24 @@ int launch_check(const ppl_plan_s *p, const double *L, const double *t2, int t2_
 int verify_harvest(ppl_plan_s *p, int *flags_out) {
     if (flags_out) *flags_out = 0;
     if (!p->verify_pending) return PPL_OK;
+    const int kind = p->verify_pending;
     p->verify_pending = 0;
-    if (cudaEventSynchronize(p->ev_verify) != cudaSuccess) {
+    if (kind == 2) {
+        // the check CTAs of k_small_fused: the last of them stores the apply's sequence number into mapped host memory.  They are
+        // the first CTAs of the grid and take a few microseconds, so in the steady state the word is there already.  Should
+        // the launch have failed it never arrives: every so often ask the stream, and stop once it has drained.
+        volatile int *seqw = p->vflags_host + 4;
+        for (unsigned spin = 1; *seqw != p->vseq; ++spin) {
+            if ((spin & 0x3ff) == 0) {
+                const cudaError_t e = cudaStreamQuery(p->vstream);
+                if (e == cudaErrorNotReady) continue;
+                if (e != cudaSuccess || *seqw != p->vseq) {
+                    (void)cudaGetLastError();
+                    return fail(PPL_ERR_CUDA);
+                }
+            }
+        }
+    } else if (cudaEventSynchronize(p->ev_verify) != cudaSuccess) {
         (void)cudaGetLastError();
         return fail(PPL_ERR_CUDA);
     }

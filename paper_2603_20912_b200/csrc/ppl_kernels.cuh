@@ -542,15 +542,17 @@ struct CheckArgs {
                             // [1] = 1 if t2 is not pair-symmetric.  Plain stores of the same value (no atomics across PCIe, no
                             // device-to-host copy behind the kernel): the host reads them once the kernel's event has completed.
 };
-__global__ void __launch_bounds__(256) k_check_inputs(const CheckArgs p) {
-    __shared__ double sb[32][33];
+// The scan of block `bid` of `nblocks` (any block size that is a multiple of 32; sb: 32 x 33 doubles of shared memory); returns the
+// flag bits this thread found.  Shared by k_check_inputs and by the one-kernel path of launch-bound shapes, whose first few
+// CTAs run it (ppl_kernels_small.cuh).
+__device__ __forceinline__ int check_inputs_scan(const CheckArgs &p, double (*sb)[33], int bid, int nblocks) {
     const int nb = (p.v + 31) / 32;
     const int64_t npair = (int64_t)nb * (nb + 1) / 2, nsq = (int64_t)nb * nb;
     const int64_t itemsL = p.L ? (int64_t)p.x * npair : 0;
     const int64_t itemsT = p.t2 ? (int64_t)p.o * (p.o + 1) / 2 * nsq : 0;
-    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5, nty = blockDim.x >> 5;
     int f = 0;
-    for (int64_t item = blockIdx.x; item < itemsL + itemsT; item += gridDim.x) {
+    for (int64_t item = bid; item < itemsL + itemsT; item += nblocks) {
         const double *A, *B;  // block of A at (r0, c0) is compared with the transpose of the block of B at (c0, r0)
         int64_t lda, ldb;
         int r0, c0, bit;
@@ -587,20 +589,23 @@ __global__ void __launch_bounds__(256) k_check_inputs(const CheckArgs p) {
             diag = false;
         }
         __syncthreads();  // the previous item's reads of sb are done
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const int y = ty + 8 * k, r = c0 + y, c = r0 + tx;  // partner block: rows c0.., columns r0..
+        for (int y = ty; y < 32; y += nty) {
+            const int r = c0 + y, c = r0 + tx;  // partner block: rows c0.., columns r0..
             sb[y][tx] = (r < p.v && c < p.v) ? __ldg(B + (int64_t)r * ldb + c) : 0.0;
         }
         __syncthreads();
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const int y = ty + 8 * k, r = r0 + y, c = c0 + tx;
+        for (int y = ty; y < 32; y += nty) {
+            const int r = r0 + y, c = c0 + tx;
             if (r < p.v && c < p.v && !(diag && c < r)) {
                 if (__ldg(A + (int64_t)r * lda + c) != sb[tx][y]) f |= bit;
             }
         }
     }
+    return f;
+}
+__global__ void __launch_bounds__(256) k_check_inputs(const CheckArgs p) {
+    __shared__ double sb[32][33];
+    const int f = check_inputs_scan(p, sb, blockIdx.x, gridDim.x);
     if (f & 1) p.flags[0] = 1;
     if (f & 2) p.flags[1] = 1;
 }

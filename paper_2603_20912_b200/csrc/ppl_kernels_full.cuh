@@ -50,9 +50,8 @@ struct Step0SlabArgs {
     double *X;           // strip [(a_l * rows_per_a + b - b_base)][c * v + d], row stride v*v
     int rows_per_a;      // strip rows per a_l: v (the slab's whole strip) or the b-group width (memory-tight mode)
     int b_base;          // first b of the strip: 0, or the b-group's first b
-    int group_m;         // raster: row tiles per group.  A group sweeps all column tiles once, its group_m row panels (128 x
-                         // nchol doubles each) staying in L2: the L rows behind the column tiles are read from DRAM once per
-                         // GROUP, so the planner makes groups as tall as a ~40 MB L2 share allows (large: 24, XL: 16; was 12)
+    int group_m;         // raster: row tiles per group (12: a wave of 148 CTAs covers ~12 x 12 tiles, the fewest operand panels per
+                         // wave; taller groups read MORE from DRAM -- measured, profiles/r02_step0_l2.md)
     int hints;           // L2 policy bits (ppl_debug_opts_t.full_hints): 1 evict_last row panels, 2 evict_first column panels, 4 streaming stores
     int image;           // 1: chunks cover d-block >= b-block only and the epilogue stores the b<->d image too (rows of
                          // every b >= A0 must be in the strip); 0: the chunks cover the full (b, d) rectangle of the group

@@ -26,7 +26,7 @@
 // L's own symmetry is not needed and not used.  The S+- packing of the tiled path would save another factor on paper,
 // but its fold / two-use bookkeeping is exactly the chain of small launches this kernel exists to avoid.
 #pragma once
-#include "ppl_device.cuh"
+#include "ppl_kernels.cuh"
 
 namespace ppl {
 
@@ -45,6 +45,19 @@ struct SmallArgs {
     int nitems;
     double alpha, beta;
     RStrides rs;         // element strides of R[i,j,a,b] (either storage order)
+    // PPL_OPT_VERIFY_INPUTS = 1 without a launch of its own: the first `ncheck` CTAs scan the inputs for the symmetry the plan's
+    // mode relies on (check_inputs_scan) instead of taking work items; flags and, from the last of them to finish, the
+    // sequence number `seq` go to mapped pinned host memory (chk.flags[0..1], chk.flags[4]), where the next call on the plan
+    // reads them.  The work items run on the other CTAs meanwhile.
+    CheckArgs chk;
+    int ncheck;
+    int seq;
+    int *done;           // device counter of finished check CTAs (zero between launches)
+    // 1: all of t2 (nocc^2 blocks of nvirt x ldt doubles) is staged ONCE per CTA into a region of its own behind the ring, by
+    // bulk copies issued before the k loop: step 1 then waits for nothing and makes one pass.  The host sets it when every
+    // CTA has a single work item and the region fits (the tiny config: 80 KB) -- there the 4-5 dependent copy latencies of
+    // the passes were a third of the kernel.
+    int t2_resident;
 };
 
 template <int NB>
@@ -54,7 +67,7 @@ struct SmallCfg {
     static constexpr int LDB = SMALL_SW * W8 + 4;          // [k][(b_l, d)]: the SW rows of one P are contiguous, ldl apart
     static constexpr int STAGE = BK * (LDA + LDB);         // doubles
     static constexpr int RING = SMALL_STAGES * STAGE;
-    static constexpr int LDT = W8 + ((NB & 1) ? 0 : 8);    // row stride of a staged t2 block: 8 (mod 16) doubles (see step 1)
+    static constexpr int LDT = W8 + ((NB & 1) ? 0 : 8);    // row stride of the padded copy of t2: 8 (mod 16) doubles (see step 1)
     static constexpr size_t SMEM = (size_t)RING * sizeof(double) + 64 + (size_t)SMALL_SW * SMALL_MAX_OO * sizeof(double);  // + mbarriers + results
     __device__ static double *results(double *sm) { return sm + RING + 8; }  // behind the ring and the 5 mbarriers
 };
@@ -104,8 +117,21 @@ __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArg
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double *sm = reinterpret_cast<double *>(smem_raw);
     uint64_t *full = reinterpret_cast<uint64_t *>(sm + Cfg::RING);  // [SMALL_STAGES] k-loop stages, then [2] t2 halves
-    uint64_t *tfull = full + SMALL_STAGES;
+    uint64_t *tfull = full + SMALL_STAGES;                          // [2], then [1]: all of t2 (t2_resident)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if ((int)blockIdx.x < p.ncheck) {  // a check CTA (see SmallArgs)
+        const int f = check_inputs_scan(p.chk, reinterpret_cast<double(*)[33]>(sm), blockIdx.x, p.ncheck);
+        if (f & 1) p.chk.flags[0] = 1;
+        if (f & 2) p.chk.flags[1] = 1;
+        __threadfence_system();  // the flags are on their way before this CTA counts as done
+        __syncthreads();
+        if (tid == 0 && atomicAdd(p.done, 1) == p.ncheck - 1) {
+            *p.done = 0;
+            __threadfence_system();
+            p.chk.flags[4] = p.seq;
+        }
+        return;
+    }
     const int g = lane >> 2, q = lane & 3;
     const int v = p.v, ldl = p.ldl, ldt = p.ldt;
     const int64_t lstride = (int64_t)v * ldl;              // doubles between L[P] and L[P+1]
@@ -118,13 +144,24 @@ __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArg
         for (int s = 0; s < SMALL_STAGES; ++s) sm_mbar_init(&full[s], SMALL_SW);
         sm_mbar_init(&tfull[0], 1);
         sm_mbar_init(&tfull[1], 1);
+        sm_mbar_init(&tfull[2], 1);
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
     asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");  // the generic-proxy clears above precede the bulk copies below
     __syncthreads();
     uint32_t phbits = 0, tphbits = 0;  // phase parity of every barrier, one bit each
+    double *tres = Cfg::results(sm) + SMALL_SW * SMALL_MAX_OO;  // t2_resident: nocc^2 blocks, then a cleared pad (reads past the last block)
+    bool t2_here = false;
+    if (p.t2_resident) {
+        const int oo_ = p.o * p.o, tblk_ = v * ldt;
+        for (int i = tid; i < 8 * NB * ldt + 8 * NB; i += SMALL_THREADS) tres[oo_ * tblk_ + i] = 0.0;
+        if (tid == 0) {
+            sm_mbar_expect_tx(&tfull[2], (uint32_t)oo_ * tblk_ * 8);
+            for (int u = 0; u < oo_; ++u) sm_bulk_g2s(tres + u * tblk_, p.t2 + (int64_t)u * tblk_, (uint32_t)tblk_ * 8, &tfull[2]);
+        }
+    }
 
-    for (int item = blockIdx.x; item < p.nitems; item += gridDim.x) {
+    for (int item = blockIdx.x - p.ncheck; item < p.nitems; item += gridDim.x - p.ncheck) {
         int a, b0;
         small_item(item, v, p.pair, a, b0);
         const int nb = min(SMALL_SW, v - b0);              // b's of this item
@@ -194,43 +231,48 @@ __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArg
             }
 
         // ---- step 1 from the accumulators.  W_ab block (i, j) holds c = 8 i + g, d = 8 j + 2 q, + 1.  The (i', j') blocks of t2
-        // come in row by row (one bulk copy per row of ldt doubles, issued by the lanes of warp 0) into rows of LDT doubles --
-        // LDT = 8 (mod 16), so that the 16-byte pairs (d, d + 1) a quarter warp reads (two consecutive g's, q = 0..3) fall into
-        // eight different bank groups: ncu showed step 1 bound by shared-memory wavefronts, half of them bank conflicts, with
-        // rows at the natural stride.  Several blocks per pass, double-buffered.  Whatever a pair reads beyond a block's rows /
-        // columns is finite and meets a zero of W.
+        // ([nvirt][ldt] doubles each, contiguous) come in by one bulk copy each, several per pass, double-buffered, and are
+        // read back as 16-byte pairs (d, d + 1).  With ldt = 8 (mod 16) -- what the padded copy of k_small_prepack has, and an
+        // un-padded t2 with nvirt = 8 (mod 16) -- the pairs a quarter warp reads (two consecutive g's, q = 0..3) fall into eight
+        // different bank groups; at other strides some of them collide (ncu, nvirt = 53 at stride 54: half of the step's
+        // shared-memory wavefronts).  Whatever a pair reads beyond a block's rows / columns is finite and meets a zero of W.
         __syncthreads();  // every warp has left the k loop: the ring is free
         const int b = b0 + warp;
         const int oo = p.o * p.o;
-        constexpr int LDT = Cfg::LDT;
-        const int tblk = v * LDT;                             // doubles per staged block
+        const int LDT = ldt;
+        const int tblk = v * ldt;                             // doubles per staged block
         // blocks per pass: as many as two halves of the ring hold (a fragment pair may read up to 8 NB rows / columns into what
         // follows its block, which must stay inside the ring)
-        const int bpp = max(1, min(8, ((Cfg::RING - (8 * NB - 1) * LDT - 8 * NB) / tblk + 1) / 2));
+        const bool resident = p.t2_resident != 0;
+        const int bpp = resident ? oo : max(1, min(8, ((Cfg::RING - (8 * NB - 1) * ldt - 8 * NB) / tblk + 1) / 2));
         const int npass = (oo + bpp - 1) / bpp;
+        if (resident && !t2_here) {
+            sm_mbar_wait(&tfull[2], 0);
+            t2_here = true;
+        }
         auto load_pass = [&](int ps) {                        // blocks bpp ps ... into half (ps & 1)
-            if (warp != 0) return;
+            if (tid != 0) return;
             const int h = ps & 1, n = min(bpp, oo - bpp * ps);
-            if (lane == 0) sm_mbar_expect_tx(&tfull[h], (uint32_t)n * v * ldt * 8);
-            __syncwarp();
-            for (int r = lane; r < n * v; r += 32) {
-                const int u = r / v, c = r - u * v;
-                sm_bulk_g2s(sm + (h * bpp + u) * tblk + c * LDT, p.t2 + ((int64_t)(bpp * ps + u) * v + c) * ldt, (uint32_t)ldt * 8, &tfull[h]);
-            }
+            sm_mbar_expect_tx(&tfull[h], (uint32_t)n * tblk * 8);
+            for (int u = 0; u < n; ++u)
+                sm_bulk_g2s(sm + (h * bpp + u) * tblk, p.t2 + (int64_t)(bpp * ps + u) * tblk, (uint32_t)tblk * 8, &tfull[h]);
         };
-        load_pass(0);
+        if (!resident) load_pass(0);
         double *res = Cfg::results(sm) + warp * SMALL_MAX_OO;  // this warp's nocc^2 results
         for (int ps = 0; ps < npass; ++ps) {
-            if (ps + 1 < npass) load_pass(ps + 1);            // (its half was read in pass ps - 1: the barrier below, last iteration)
             const int h = ps & 1;
-            sm_mbar_wait(&tfull[h], (tphbits >> h) & 1u);
-            tphbits ^= 1u << h;
+            if (!resident) {
+                if (ps + 1 < npass) load_pass(ps + 1);        // (its half was read in pass ps - 1: the barrier below, last iteration)
+                sm_mbar_wait(&tfull[h], (tphbits >> h) & 1u);
+                tphbits ^= 1u << h;
+            }
+            const double *tbase = resident ? tres : sm + h * bpp * tblk;
             if (b < v) {
                 const int n = min(bpp, oo - bpp * ps);
                 for (int u0 = 0; u0 < n; u0 += 2) {           // two blocks at a time: four independent FMA chains
                     double s[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
                     const int u1 = min(u0 + 1, n - 1);        // (an odd last block is read twice and stored once)
-                    const double *t0 = sm + (h * bpp + u0) * tblk + g * LDT + 2 * q;
+                    const double *t0 = tbase + u0 * tblk + g * LDT + 2 * q;
                     const int du = (u1 - u0) * tblk;
 #pragma unroll
                     for (int i = 0; i < NB; ++i)
@@ -252,7 +294,7 @@ __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArg
                     if (lane < 2 && u0 + lane < n) res[bpp * ps + u0 + lane] = lane ? r[1] : r[0];
                 }
             }
-            __syncthreads();  // pass ps has been read: its half may be refilled
+            if (!resident) __syncthreads();  // pass ps has been read: its half may be refilled
         }
         // R[i,j,a,b] (and the mirror): one (i,j) per lane, so that the read-modify-writes of a warp are in flight together
         // (one result at a time from lane 0, each behind its own global load, was 40 % of the stall samples at tiny)
@@ -268,11 +310,11 @@ __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArg
     }
 }
 
-// Copies of L and t2 with rows of even length ld = nvirt rounded up to even (the pad column is zero) and t2 in (i,j) order,
-// for the bulk copies of k_small_fused: Lp[P][a][ld], tp[i*o+j][c][ld].  Either source may be null (no copy needed).
+// Copies of L and t2 with padded rows (the pad columns are zero) and t2 in (i,j) order, for the bulk copies of k_small_fused:
+// Lp[P][a][ld] (ld = nvirt rounded up to even), tp[i*o+j][c][ldt] (ldt = SmallCfg::LDT: conflict-free reads in step 1).  Either source may be null (no copy needed).
 __global__ void __launch_bounds__(256) k_small_prepack(const double *__restrict__ L, const double *__restrict__ t2, double *__restrict__ Lp,
-                                                      double *__restrict__ tp, int o, int v, int x, int ld, RStrides ts) {
-    const int64_t nL = L ? (int64_t)x * v * ld : 0, nT = t2 ? (int64_t)o * o * v * ld : 0;
+                                                      double *__restrict__ tp, int o, int v, int x, int ld, int ldt, RStrides ts) {
+    const int64_t nL = L ? (int64_t)x * v * ld : 0, nT = t2 ? (int64_t)o * o * v * ldt : 0;
     for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < nL + nT; idx += (int64_t)gridDim.x * blockDim.x) {
         if (idx < nL) {
             const int c = (int)(idx % ld);
@@ -280,8 +322,8 @@ __global__ void __launch_bounds__(256) k_small_prepack(const double *__restrict_
             Lp[idx] = c < v ? __ldg(L + row * v + c) : 0.0;
         } else {
             const int64_t e = idx - nL;
-            const int d = (int)(e % ld);
-            int64_t r = e / ld;
+            const int d = (int)(e % ldt);
+            int64_t r = e / ldt;
             const int c = (int)(r % v);
             r /= v;
             const int j = (int)(r % o), i = (int)(r / o);

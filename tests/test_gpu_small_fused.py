@@ -94,3 +94,43 @@ def test_fused_path_zero_t2_repeat_and_which_shapes_take_it():
     assert P.ppl_plan_dry(9, 40, 100, debug=FUSED)["small_fused"] == 0      # nocc > 8
     assert P.ppl_plan_dry(5, 53, 4000, debug=FUSED)["small_fused"] == 0     # not launch-bound any more
     assert P.ppl_plan_dry(5, 53, 232, debug={"no_small_fused": 1})["small_fused"] == 0
+
+
+@pytest.mark.parametrize("shape", [(5, 20, 60), (5, 53, 232), (3, 41, 31), (1, 5, 1)])
+def test_fused_path_checks_its_inputs_inside_the_same_launch(shape):
+    """PPL_OPT_VERIFY_INPUTS = 1 on the one-kernel path: the first CTAs of the launch scan the inputs; a violation is reported
+    by the next call on the plan, a clean apply by none -- over many back-to-back applies (the sequence word), and again
+    after the mode no longer relies on the violated symmetry."""
+    import torch
+
+    o, v, x = shape
+    L = I.make_L(v, x, 23, symmetric=True)
+    t2 = I.make_t2(o, v, 23, symmetric=True)
+    Ld, td = torch.from_numpy(L).cuda(), torch.from_numpy(t2).cuda()
+    bad_t = torch.from_numpy(I.make_t2(o, v, 24, symmetric=False)).cuda()
+    bad_L = torch.from_numpy(I.make_L(v, x, 24, symmetric=False)).cuda()
+    with P.Plan(o, v, x, debug=FUSED) as plan:
+        info = plan.info()
+        assert info["small_fused"] == 1
+        Rd = torch.zeros((o, o, v, v), dtype=torch.float64, device="cuda")
+        for _ in range(20):
+            plan.apply(Ld, td, Rd)
+        assert plan.verify_status() == 0
+        torch.cuda.synchronize()
+        assert relerr(Rd.cpu().numpy(), 20.0 * oracle.full(L, t2)) <= TOL
+        if o > 1 or v > 1:  # (a 1 x 1 x 1 x 1 t2 is pair-symmetric whatever it holds)
+            plan.apply(Ld, bad_t, Rd)
+            with pytest.raises(P.PplError) as e:
+                plan.apply(Ld, td, Rd)           # the NEXT call reports it (and queues nothing)
+            assert e.value.code == P.PPL_ERR_PRECONDITION
+            plan.apply(Ld, td, Rd)               # cleared: a clean apply goes through again
+            assert plan.verify_status() == 0
+        if info["symmetry"] == P.PPL_SYM_FULL and v > 1:  # the default mode from nvirt = 52 also relies on L[P,a,c] = L[P,c,a]
+            plan.apply(bad_L, td, Rd)
+            with pytest.raises(P.PplError) as e:
+                plan.verify_status()
+            assert e.value.code == P.PPL_ERR_PRECONDITION
+        plan.set_symmetry(P.PPL_SYM_NONE)        # nothing assumed: nothing checked, nothing reported
+        plan.apply(bad_L, bad_t, Rd)
+        assert plan.verify_status() == 0
+        torch.cuda.synchronize()
