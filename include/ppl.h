@@ -316,6 +316,9 @@ int ppl_plan_set_symmetry(ppl_plan_t *plan, int mode);
  *                returns PPL_ERR_PRECONDITION with R untouched.
  *   0            no check: the caller vouches for the preconditions (result undefined otherwise).
  * The check is skipped while the caller is capturing `stream` into a CUDA graph, and in PPL_SYM_NONE (no precondition).
+ * On the one-kernel path of launch-bound shapes (ppl_info_t.small_fused) mode 1 costs no launch of its own -- the first CTAs
+ * of the apply's single launch scan t2 -- and L is not verified there: that path does not use the symmetry of L, its result
+ * is right for any L (mode 2 and ppl_check_inputs verify both arrays as everywhere else).
  * ppl_apply_host verifies L only in its streamed form (t2 never sits on the device whole). */
 enum { PPL_OPT_VERIFY_INPUTS = 1 };
 int ppl_plan_set_option(ppl_plan_t *plan, int option, int value);

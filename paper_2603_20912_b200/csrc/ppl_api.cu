@@ -1179,8 +1179,10 @@ int run_apply_small(ppl_plan_s *p, const double *L, const double *t2, double *R,
     a.ncheck = 0;
     a.seq = 0;
     a.done = p->vdone_dev;
-    if (fused_check) {  // PPL_OPT_VERIFY_INPUTS = 1: the caller's arrays, scanned by the first CTAs of the same launch
-        a.chk.L = p->sym == PPL_SYM_FULL ? L : nullptr;
+    if (fused_check) {  // PPL_OPT_VERIFY_INPUTS = 1: the caller's t2, scanned by the first CTAs of the same launch.  Not L: this
+                        // path never uses L[P,a,c] = L[P,c,a] (its result is right for any L), and scanning L -- 92 % of the
+                        // check's bytes at `small` -- kept the check CTAs busy for the whole length of the kernel (ncu)
+        a.chk.L = nullptr;
         a.chk.t2 = t2;
         a.chk.o = p->o;
         a.chk.v = p->v;
@@ -1194,11 +1196,13 @@ int run_apply_small(ppl_plan_s *p, const double *L, const double *t2, double *R,
         a.chk.flags = dflags;
         const int nb = (p->v + 31) / 32;
         const int64_t items = (a.chk.L ? (int64_t)p->x * nb * (nb + 1) / 2 : 0) + (int64_t)p->o * (p->o + 1) / 2 * nb * nb;
-        a.ncheck = (int)std::max<int64_t>(1, std::min<int64_t>(16, items / 4));
+        a.ncheck = (int)std::max<int64_t>(1, std::min<int64_t>(32, items / 4));
         a.seq = ++p->vseq;
         p->vflags_host[0] = p->vflags_host[1] = 0;
     }
-    const int grid = std::min(a.nitems, 2 * p->num_sms) + a.ncheck;
+    // every CTA of the grid is resident from the start (two per SM): a work-item CTA that had to wait for a check CTA's slot
+    // would start its items late and end the kernel late (ncu: a check CTA scans its share of L for ~100 us at `small`)
+    const int grid = std::min(a.nitems, 2 * p->num_sms - a.ncheck) + a.ncheck;
     // all of t2 staged once per CTA when every CTA has one work item and the region fits beside the ring (tiny: 80 KB)
     const size_t t2_region = ((size_t)p->o * p->o * p->v * a.ldt + (size_t)8 * nb8 * a.ldt + 8 * nb8) * 8;
     size_t smem_extra = 0;

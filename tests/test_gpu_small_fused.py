@@ -23,9 +23,7 @@ SHAPES = [(1, 1, 1), (2, 1, 3), (1, 5, 1), (3, 7, 5), (2, 8, 16), (5, 9, 17), (4
 def test_fused_path_parity(shape, sym):
     o, v, x = shape
     symmetric = sym != P.PPL_SYM_NONE
-    L = I.make_L(v, x, 13, symmetric=False)          # the fused path never uses L's symmetry ...
-    if sym is None and v >= 52:
-        L = I.make_L(v, x, 13, symmetric=True)        # ... but the default mode from nvirt = 52 (PPL_SYM_FULL) verifies it
+    L = I.make_L(v, x, 13, symmetric=False)          # the fused path never uses L's symmetry, in any mode
     t2 = I.make_t2(o, v, 13, symmetric=symmetric)
     R0 = I.make_t2(o, v, 14, symmetric=False)
     want = oracle.full(L, t2, R0.copy())
@@ -125,11 +123,18 @@ def test_fused_path_checks_its_inputs_inside_the_same_launch(shape):
             assert e.value.code == P.PPL_ERR_PRECONDITION
             plan.apply(Ld, td, Rd)               # cleared: a clean apply goes through again
             assert plan.verify_status() == 0
-        if info["symmetry"] == P.PPL_SYM_FULL and v > 1:  # the default mode from nvirt = 52 also relies on L[P,a,c] = L[P,c,a]
-            plan.apply(bad_L, td, Rd)
+        # L is not verified on this path (it does not use L[P,a,c] = L[P,c,a]: the result is right for any L) ...
+        Rd.zero_()
+        plan.apply(bad_L, td, Rd)
+        assert plan.verify_status() == 0
+        torch.cuda.synchronize()
+        assert relerr(Rd.cpu().numpy(), oracle.full(bad_L.cpu().numpy(), t2)) <= TOL
+        if info["symmetry"] == P.PPL_SYM_FULL and v > 1:  # ... except by the synchronous mode, which checks what the mode names
+            plan.set_verify(2)
             with pytest.raises(P.PplError) as e:
-                plan.verify_status()
+                plan.apply(bad_L, td, Rd)
             assert e.value.code == P.PPL_ERR_PRECONDITION
+            plan.set_verify(1)
         plan.set_symmetry(P.PPL_SYM_NONE)        # nothing assumed: nothing checked, nothing reported
         plan.apply(bad_L, bad_t, Rd)
         assert plan.verify_status() == 0
