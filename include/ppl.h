@@ -318,7 +318,10 @@ int ppl_plan_set_symmetry(ppl_plan_t *plan, int mode);
  * The check is skipped while the caller is capturing `stream` into a CUDA graph, and in PPL_SYM_NONE (no precondition).
  * On the one-kernel path of launch-bound shapes (ppl_info_t.small_fused) mode 1 costs no launch of its own -- the first CTAs
  * of the apply's single launch scan t2 -- and L is not verified there: that path does not use the symmetry of L, its result
- * is right for any L (mode 2 and ppl_check_inputs verify both arrays as everywhere else).
+ * is right for any L (mode 2 and ppl_check_inputs verify both arrays as everywhere else).  There the next call reports a
+ * violation if the check has finished by then, and otherwise the call after it does: a call never waits for the check of the
+ * apply queued just before it (that would serialise host and device at shapes where an apply takes 20 us);
+ * ppl_plan_verify_status and ppl_destroy wait for everything outstanding.
  * ppl_apply_host verifies L only in its streamed form (t2 never sits on the device whole). */
 enum { PPL_OPT_VERIFY_INPUTS = 1 };
 int ppl_plan_set_option(ppl_plan_t *plan, int option, int value);

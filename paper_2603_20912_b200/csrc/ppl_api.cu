@@ -35,7 +35,7 @@ namespace {
 namespace {
 
 // per-apply verification of the symmetry preconditions (PPL_OPT_VERIFY_INPUTS; defined next to ppl_check_inputs)
-int verify_harvest(ppl_plan_s *p, int *flags_out);
+int verify_harvest(ppl_plan_s *p, int *flags_out, bool wait_all = true);
 int verify_begin(ppl_plan_s *p, const double *L, const double *t2, int t2_layout, cudaStream_t stream);
 
 void free_plan(ppl_plan_s *p) {
@@ -1041,8 +1041,8 @@ ppl_plan_t *ppl_plan_ex(int nocc, int nvirt, int nchol, size_t workspace_bytes, 
         return nullptr;
     }
     if (cudaMalloc(&p->ws, p->ws_bytes) != cudaSuccess ||
-        cudaHostAlloc(&p->vflags_host, 8 * sizeof(int), cudaHostAllocMapped) != cudaSuccess ||
-        cudaMalloc(&p->vdone_dev, sizeof(int)) != cudaSuccess || cudaMemset(p->vdone_dev, 0, sizeof(int)) != cudaSuccess ||
+        cudaHostAlloc(&p->vflags_host, 32 * sizeof(int), cudaHostAllocMapped) != cudaSuccess ||
+        cudaMalloc(&p->vdone_dev, 2 * sizeof(int)) != cudaSuccess || cudaMemset(p->vdone_dev, 0, 2 * sizeof(int)) != cudaSuccess ||
         cudaEventCreateWithFlags(&p->ev_verify, cudaEventDisableTiming) != cudaSuccess) {
         (void)cudaGetLastError();
         free_plan(p);
@@ -1191,14 +1191,16 @@ int run_apply_small(ppl_plan_s *p, const double *L, const double *t2, double *R,
         a.chk.s_i = ts.i;
         a.chk.s_j = ts.j;
         a.chk.s_c = ts.a;
+        a.seq = ++p->vseq;
+        const int slot = a.seq & 1;  // free: the caller has harvested everything but the newest outstanding check
         int *dflags = nullptr;
         PPL_CUDA(cudaHostGetDevicePointer(&dflags, p->vflags_host, 0));
-        a.chk.flags = dflags;
+        a.chk.flags = dflags + 8 + 8 * slot;
+        a.done = p->vdone_dev + slot;
+        p->vflags_host[8 + 8 * slot] = p->vflags_host[8 + 8 * slot + 1] = 0;
         const int nb = (p->v + 31) / 32;
         const int64_t items = (a.chk.L ? (int64_t)p->x * nb * (nb + 1) / 2 : 0) + (int64_t)p->o * (p->o + 1) / 2 * nb * nb;
         a.ncheck = (int)std::max<int64_t>(1, std::min<int64_t>(32, items / 4));
-        a.seq = ++p->vseq;
-        p->vflags_host[0] = p->vflags_host[1] = 0;
     }
     // every CTA of the grid is resident from the start (two per SM): a work-item CTA that had to wait for a check CTA's slot
     // would start its items late and end the kernel late (ncu: a check CTA scans its share of L for ~100 us at `small`)
@@ -1223,7 +1225,7 @@ int run_apply_small(ppl_plan_s *p, const double *L, const double *t2, double *R,
     }
     PPL_CUDA(cudaGetLastError());
     if (fused_check) {
-        p->verify_pending = 2;
+        if (p->vq_n < 2) p->vq_seq[p->vq_n++] = a.seq;
         p->vstream = stream;
     }
     if (prof && prof->mark(K_STEP0, 1 + ((pack_L || pack_t) ? 1 : 0), stream) != PPL_OK) return fail(PPL_ERR_CUDA);
@@ -1296,7 +1298,7 @@ int ppl_apply_ex(ppl_plan_t *p, const double *L, const double *t2, double *R, co
         st = cudaStreamCaptureStatusActive;
     }
     if (st == cudaStreamCaptureStatusNone) {
-        int rc = verify_harvest(p, nullptr);  // what the previous apply's check found
+        int rc = verify_harvest(p, nullptr, false);  // what the previous apply's check found
         if (rc != PPL_OK) return rc;
         if (p->verify && p->sym != PPL_SYM_NONE) {
             // launch-bound shapes: the check rides in the apply's one launch (its first CTAs) instead of a launch of its own
@@ -1447,32 +1449,47 @@ int launch_check(const ppl_plan_s *p, const double *L, const double *t2, int t2_
     return PPL_OK;
 }
 
-// result of the pending per-apply verification, if any (waits for that head-of-apply kernel only)
-int verify_harvest(ppl_plan_s *p, int *flags_out) {
+// Result of the outstanding per-apply verifications.  A k_check_inputs launch (the tiled paths): waits for that head-of-apply
+// kernel only.  The check CTAs of k_small_fused (launch-bound shapes): the last of them stores the apply's sequence number into
+// mapped host memory; wait_all = false (the head of the next apply) does not wait for the NEWEST of them -- that apply may
+// still be running, and waiting would serialise the host with the device (tiny: 25 instead of 18 us per back-to-back apply)
+// -- but reads it if it is there, and waits for an older one; so a violation is reported by the next call or the one after.
+// Should a launch have died its number never arrives: every so often ask the stream, and stop once it has drained.
+int verify_harvest(ppl_plan_s *p, int *flags_out, bool wait_all) {
     if (flags_out) *flags_out = 0;
-    if (!p->verify_pending) return PPL_OK;
-    const int kind = p->verify_pending;
-    p->verify_pending = 0;
-    if (kind == 2) {
-        // the check CTAs of k_small_fused: the last of them stores the apply's sequence number into mapped host memory.  They are
-        // the first CTAs of the grid and take a few microseconds, so in the steady state the word is there already.  Should
-        // the launch have failed it never arrives: every so often ask the stream, and stop once it has drained.
-        volatile int *seqw = p->vflags_host + 4;
-        for (unsigned spin = 1; *seqw != p->vseq; ++spin) {
+    int h = 0;
+    bool any = false;
+    if (p->verify_pending) {
+        p->verify_pending = 0;
+        if (cudaEventSynchronize(p->ev_verify) != cudaSuccess) {
+            (void)cudaGetLastError();
+            return fail(PPL_ERR_CUDA);
+        }
+        h |= (p->vflags_host[0] ? 1 : 0) | (p->vflags_host[1] ? 2 : 0);
+        any = true;
+    }
+    while (p->vq_n > 0) {
+        const int seq = p->vq_seq[0], slot = seq & 1;
+        volatile int *w = p->vflags_host + 8 + 8 * slot;
+        const bool must = wait_all || p->vq_n > 1;
+        if (!must && w[4] != seq) break;
+        for (unsigned spin = 1; w[4] != seq; ++spin) {
             if ((spin & 0x3ff) == 0) {
                 const cudaError_t e = cudaStreamQuery(p->vstream);
                 if (e == cudaErrorNotReady) continue;
-                if (e != cudaSuccess || *seqw != p->vseq) {
+                if (e != cudaSuccess || w[4] != seq) {
                     (void)cudaGetLastError();
+                    p->vq_n = 0;
                     return fail(PPL_ERR_CUDA);
                 }
             }
         }
-    } else if (cudaEventSynchronize(p->ev_verify) != cudaSuccess) {
-        (void)cudaGetLastError();
-        return fail(PPL_ERR_CUDA);
+        h |= (w[0] ? 1 : 0) | (w[1] ? 2 : 0);
+        any = true;
+        p->vq_seq[0] = p->vq_seq[1];
+        --p->vq_n;
     }
-    const int h = (p->vflags_host[0] ? 1 : 0) | (p->vflags_host[1] ? 2 : 0);
+    if (!any) return PPL_OK;
     if (flags_out) *flags_out = h;
     if ((h & 2) && p->sym != PPL_SYM_NONE) return fail(PPL_ERR_PRECONDITION);
     if ((h & 1) && p->sym == PPL_SYM_FULL) return fail(PPL_ERR_PRECONDITION);
@@ -1591,7 +1608,7 @@ int full_compute(ppl_plan_s *p, const double *L, cudaStream_t s, cudaEvent_t tau
 int verify_begin(ppl_plan_s *p, const double *L, const double *t2, int t2_layout, cudaStream_t stream) {
     return ::verify_begin(p, L, t2, t2_layout, stream);
 }
-int verify_harvest(ppl_plan_s *p, int *flags_out) { return ::verify_harvest(p, flags_out); }
+int verify_harvest(ppl_plan_s *p, int *flags_out) { return ::verify_harvest(p, flags_out, true); }
 
 }  // namespace pplapi
 

@@ -351,6 +351,7 @@ static int apply_host_tiles(ppl_plan_s *p, const double *Lh, const double *t2h, 
         for (cudaStream_t st : {p->hsn.in, p->gen, p->host_stream, p->hsn.out})
             if (st && cudaStreamSynchronize(st) != cudaSuccess) (void)cudaGetLastError();
         p->verify_pending = 0;
+        p->vq_n = 0;
         if (rc == PPL_ERR_ALLOC) {  // leave nothing half-allocated behind: a later call may take another route
             for (int i = 0; i < 2; ++i) {
                 dev_free(&p->hsn.pa[i]);

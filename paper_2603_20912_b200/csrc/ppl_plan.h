@@ -99,14 +99,17 @@ struct ppl_plan_s {
     double *part = nullptr;
     double *taup = nullptr, *taum = nullptr;
     double *tperm = nullptr;               // un-packed modes with PPL_LAYOUT_IAJB input: t2 permuted (lazy)
-    int *vflags_host = nullptr;            // [8] mapped pinned host words written by k_check_inputs: [0..1] the per-apply verification
+    int *vflags_host = nullptr;            // [32] mapped pinned host words written by k_check_inputs: [0..1] the per-apply verification
                                            // (PPL_OPT_VERIFY_INPUTS), [2..3] ppl_check_inputs
     cudaEvent_t ev_verify = nullptr;
     int verify = 1;                        // PPL_OPT_VERIFY_INPUTS
-    int verify_pending = 0;                // 1: a k_check_inputs launch (ev_verify follows it); 2: the check CTAs of k_small_fused
-    int *vdone_dev = nullptr;              // device counter of the check CTAs
-    int vseq = 0;                          // sequence number of the last fused check (arrives in vflags_host[4])
-    cudaStream_t vstream = nullptr;        // the stream it was launched on
+    int verify_pending = 0;                // 1: a k_check_inputs launch is outstanding (ev_verify follows it)
+    // the check CTAs of k_small_fused (launch-bound shapes): up to two applies outstanding, oldest first.  Apply number `seq`
+    // uses slot seq & 1: flags in vflags_host[8 + 8 slot + 0..1], its sequence number arrives in vflags_host[8 + 8 slot + 4]
+    int *vdone_dev = nullptr;              // [2] device counters of finished check CTAs, one per slot
+    int vseq = 0;                          // sequence number of the last fused check
+    int vq_seq[2] = {0, 0}, vq_n = 0;      // outstanding sequence numbers
+    cudaStream_t vstream = nullptr;        // the stream the last one was launched on
     std::vector<pplh::Tile> tiles;
     cudaStream_t gen = nullptr, host_stream = nullptr;
     cudaEvent_t ev_in = nullptr, ev_ready[pplh::MAX_RING] = {}, ev_free[pplh::MAX_RING] = {};

@@ -118,11 +118,18 @@ def test_fused_path_checks_its_inputs_inside_the_same_launch(shape):
         assert relerr(Rd.cpu().numpy(), 20.0 * oracle.full(L, t2)) <= TOL
         if o > 1 or v > 1:  # (a 1 x 1 x 1 x 1 t2 is pair-symmetric whatever it holds)
             plan.apply(Ld, bad_t, Rd)
-            with pytest.raises(P.PplError) as e:
-                plan.apply(Ld, td, Rd)           # the NEXT call reports it (and queues nothing)
+            with pytest.raises(P.PplError) as e:  # the next call reports it if the check has finished by then, else the one
+                plan.apply(Ld, td, Rd)            # after: a call never waits for the check of the apply just before it
+                plan.apply(Ld, td, Rd)
             assert e.value.code == P.PPL_ERR_PRECONDITION
+            plan.verify_status()                 # (drains a clean check the first of the two calls may have queued)
             plan.apply(Ld, td, Rd)               # cleared: a clean apply goes through again
             assert plan.verify_status() == 0
+            plan.apply(Ld, bad_t, Rd)            # and a device that has finished reports at the very next call
+            torch.cuda.synchronize()
+            with pytest.raises(P.PplError) as e:
+                plan.apply(Ld, td, Rd)
+            assert e.value.code == P.PPL_ERR_PRECONDITION
         # L is not verified on this path (it does not use L[P,a,c] = L[P,c,a]: the result is right for any L) ...
         Rd.zero_()
         plan.apply(bad_L, td, Rd)
