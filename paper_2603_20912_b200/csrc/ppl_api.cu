@@ -1209,14 +1209,18 @@ int run_apply_small(ppl_plan_s *p, const double *L, const double *t2, double *R,
     const size_t t2_region = ((size_t)p->o * p->o * p->v * a.ldt + (size_t)8 * nb8 * a.ldt + 8 * nb8) * 8;
     size_t smem_extra = 0;
     a.t2_resident = 0;
-    if (a.nitems + a.ncheck <= p->num_sms && t2_region <= (size_t)96 * 1024 && t2_region < ((size_t)1 << 20)) {
+    a.nstages = ppl::SMALL_STAGES;
+    const bool one_item = a.nitems + a.ncheck <= p->num_sms;  // one CTA per SM is enough: shared memory to spare
+    if (one_item && t2_region <= (size_t)96 * 1024 && t2_region < ((size_t)1 << 20)) {
         a.t2_resident = 1;
         smem_extra = t2_region;
     }
+    if (one_item) a.nstages = std::max(ppl::SMALL_STAGES, std::min(ppl::SMALL_MAX_STAGES, (p->x + ppl::BK - 1) / ppl::BK + 1));
     switch ((p->v + 7) / 8) {
 #define PPL_LAUNCH_SMALL(NB)                                                                                    \
     case NB:                                                                                                    \
-        ppl::k_small_fused<NB><<<grid, ppl::SMALL_THREADS, ppl::SmallCfg<NB>::SMEM + smem_extra, stream>>>(a); \
+        while (a.nstages > ppl::SMALL_STAGES && ppl::SmallCfg<NB>::smem(a.nstages) + smem_extra > (size_t)200 * 1024) --a.nstages; \
+        ppl::k_small_fused<NB><<<grid, ppl::SMALL_THREADS, ppl::SmallCfg<NB>::smem(a.nstages) + smem_extra, stream>>>(a); \
         break;
         PPL_LAUNCH_SMALL(1) PPL_LAUNCH_SMALL(2) PPL_LAUNCH_SMALL(3) PPL_LAUNCH_SMALL(4) PPL_LAUNCH_SMALL(5) PPL_LAUNCH_SMALL(6)
             PPL_LAUNCH_SMALL(7)

@@ -34,6 +34,7 @@ constexpr int SMALL_SW = 4;        // warps (= b's) per CTA
 constexpr int SMALL_STAGES = 3;
 constexpr int SMALL_THREADS = 32 * SMALL_SW;
 constexpr int SMALL_MAX_OO = 64;   // nocc <= 8
+constexpr int SMALL_MAX_STAGES = 8;
 
 struct SmallArgs {
     const double *L;     // [x][v][ldl] (ldl even, 16-byte aligned: the caller's L, or the padded copy)
@@ -58,6 +59,8 @@ struct SmallArgs {
     // CTA has a single work item and the region fits (the tiny config: 80 KB) -- there the 4-5 dependent copy latencies of
     // the passes were a third of the kernel.
     int t2_resident;
+    int nstages;         // k-loop ring depth: SMALL_STAGES, or nchol / 16 + 1 (<= SMALL_MAX_STAGES) where a CTA has one item and the
+                         // shared memory to spare: every row of L the item needs is then in flight at once (tiny: one copy latency, not two)
 };
 
 template <int NB>
@@ -66,10 +69,13 @@ struct SmallCfg {
     static constexpr int LDA = W8 + 4;                     // [k][c] row stride: 4 mod 8 doubles -> conflict-free LDS.64
     static constexpr int LDB = SMALL_SW * W8 + 4;          // [k][(b_l, d)]: the SW rows of one P are contiguous, ldl apart
     static constexpr int STAGE = BK * (LDA + LDB);         // doubles
-    static constexpr int RING = SMALL_STAGES * STAGE;
+    static constexpr int RING = SMALL_STAGES * STAGE;      // the default ring (the host may ask for up to SMALL_MAX_STAGES stages)
     static constexpr int LDT = W8 + ((NB & 1) ? 0 : 8);    // row stride of the padded copy of t2: 8 (mod 16) doubles (see step 1)
-    static constexpr size_t SMEM = (size_t)RING * sizeof(double) + 64 + (size_t)SMALL_SW * SMALL_MAX_OO * sizeof(double);  // + mbarriers + results
-    __device__ static double *results(double *sm) { return sm + RING + 8; }  // behind the ring and the 5 mbarriers
+    // ring, then 16 doubles for the mbarriers (<= SMALL_MAX_STAGES + 3), then the warps' results
+    __host__ __device__ static constexpr size_t smem(int nstages) {
+        return ((size_t)nstages * STAGE + 16 + (size_t)SMALL_SW * SMALL_MAX_OO) * sizeof(double);
+    }
+    static constexpr size_t SMEM = smem(SMALL_STAGES);
 };
 
 // ---- mbarrier / bulk-copy primitives (as in ppl_kernels_tma.cuh; repeated here so that this header stands alone) ----
@@ -116,8 +122,10 @@ __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArg
     constexpr int LDA = Cfg::LDA, LDB = Cfg::LDB;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double *sm = reinterpret_cast<double *>(smem_raw);
-    uint64_t *full = reinterpret_cast<uint64_t *>(sm + Cfg::RING);  // [SMALL_STAGES] k-loop stages, then [2] t2 halves
-    uint64_t *tfull = full + SMALL_STAGES;                          // [2], then [1]: all of t2 (t2_resident)
+    const int nst = p.nstages, RING = nst * Cfg::STAGE;
+    uint64_t *full = reinterpret_cast<uint64_t *>(sm + RING);  // [nst] k-loop stages, then [2] t2 halves, then [1]: all of t2 (t2_resident)
+    uint64_t *tfull = full + nst;
+    double *results = sm + RING + 16;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if ((int)blockIdx.x < p.ncheck) {  // a check CTA (see SmallArgs)
         const int f = check_inputs_scan(p.chk, reinterpret_cast<double(*)[33]>(sm), blockIdx.x, p.ncheck);
@@ -139,9 +147,9 @@ __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArg
 
     // Everything a fragment may touch beyond what a copy wrote (columns >= ldl of a row, rows of an absent b, the k tail)
     // must hold FINITE values: it meets exact zeros or is masked out below.  Clear the ring once.
-    for (int i = tid; i < Cfg::RING; i += SMALL_THREADS) sm[i] = 0.0;
+    for (int i = tid; i < RING; i += SMALL_THREADS) sm[i] = 0.0;
     if (tid == 0) {
-        for (int s = 0; s < SMALL_STAGES; ++s) sm_mbar_init(&full[s], SMALL_SW);
+        for (int s = 0; s < nst; ++s) sm_mbar_init(&full[s], SMALL_SW);
         sm_mbar_init(&tfull[0], 1);
         sm_mbar_init(&tfull[1], 1);
         sm_mbar_init(&tfull[2], 1);
@@ -150,7 +158,7 @@ __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArg
     asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");  // the generic-proxy clears above precede the bulk copies below
     __syncthreads();
     uint32_t phbits = 0, tphbits = 0;  // phase parity of every barrier, one bit each
-    double *tres = Cfg::results(sm) + SMALL_SW * SMALL_MAX_OO;  // t2_resident: nocc^2 blocks, then a cleared pad (reads past the last block)
+    double *tres = results + SMALL_SW * SMALL_MAX_OO;  // t2_resident: nocc^2 blocks, then a cleared pad (reads past the last block)
     bool t2_here = false;
     if (p.t2_resident) {
         const int oo_ = p.o * p.o, tblk_ = v * ldt;
@@ -168,7 +176,7 @@ __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArg
         // stage kt: rows P = 16 kt .. 16 kt + 15 (those below nchol); warp w issues the copies of k = w, w + SW, ...
         auto load_stage = [&](int kt) {
             if (lane != 0) return;
-            const int s = kt % SMALL_STAGES;
+            const int s = kt % nst;
             double *st = sm + s * Cfg::STAGE;
             const uint32_t abytes = (uint32_t)ldl * 8, bbytes = (uint32_t)nb * ldl * 8;
             int rows = 0;
@@ -183,6 +191,22 @@ __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArg
             }
         };
 
+        // small accumulator files have registers to spare: the old R values this warp will update are fetched now, so that their
+        // (cold) global-memory latency runs under the k loop instead of behind step 1
+        constexpr int PREFETCH_R_MAX_NB = 4;
+        double rold[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+        if (NB <= PREFETCH_R_MAX_NB && p.beta != 0.0 && b0 + warp < v) {
+            const int b_ = b0 + warp;
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                const int ij = lane + 32 * t;
+                if (ij >= p.o * p.o) break;
+                const int i_ = ij / p.o, j_ = ij - i_ * p.o;
+                rold[t][0] = p.R[i_ * p.rs.i + j_ * p.rs.j + a * p.rs.a + b_ * p.rs.b];
+                if (p.pair && a != b_) rold[t][1] = p.R[j_ * p.rs.i + i_ * p.rs.j + b_ * p.rs.a + a * p.rs.b];
+            }
+        }
+
         double acc[NB][NB][2];
 #pragma unroll
         for (int i = 0; i < NB; ++i)
@@ -190,15 +214,14 @@ __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArg
             for (int j = 0; j < NB; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
         __syncthreads();  // the previous item's reads of the ring are done
-#pragma unroll
-        for (int s = 0; s < SMALL_STAGES - 1; ++s)
+        for (int s = 0; s < nst - 1; ++s)
             if (s < nkt) load_stage(s);
         for (int kt = 0; kt < nkt; ++kt) {
-            const int s = kt % SMALL_STAGES;
+            const int s = kt % nst;
             sm_mbar_wait(&full[s], (phbits >> s) & 1u);
             phbits ^= 1u << s;
             __syncthreads();  // every warp has finished stage kt - 1: its slot may be refilled
-            if (kt + SMALL_STAGES - 1 < nkt) load_stage(kt + SMALL_STAGES - 1);
+            if (kt + nst - 1 < nkt) load_stage(kt + nst - 1);
             if (warp >= nb) continue;  // no b for this warp in a ragged item (it still takes part in the barriers)
             const int kvalid = min(BK, p.x - kt * BK);     // the k tail of the last stage holds rows of an older stage: skip them
             const double *as = sm + s * Cfg::STAGE + g;
@@ -244,7 +267,7 @@ __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArg
         // blocks per pass: as many as two halves of the ring hold (a fragment pair may read up to 8 NB rows / columns into what
         // follows its block, which must stay inside the ring)
         const bool resident = p.t2_resident != 0;
-        const int bpp = resident ? oo : max(1, min(8, ((Cfg::RING - (8 * NB - 1) * ldt - 8 * NB) / tblk + 1) / 2));
+        const int bpp = resident ? oo : max(1, min(8, ((RING - (8 * NB - 1) * ldt - 8 * NB) / tblk + 1) / 2));
         const int npass = (oo + bpp - 1) / bpp;
         if (resident && !t2_here) {
             sm_mbar_wait(&tfull[2], 0);
@@ -258,7 +281,7 @@ __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArg
                 sm_bulk_g2s(sm + (h * bpp + u) * tblk, p.t2 + (int64_t)(bpp * ps + u) * tblk, (uint32_t)tblk * 8, &tfull[h]);
         };
         if (!resident) load_pass(0);
-        double *res = Cfg::results(sm) + warp * SMALL_MAX_OO;  // this warp's nocc^2 results
+        double *res = results + warp * SMALL_MAX_OO;  // this warp's nocc^2 results
         for (int ps = 0; ps < npass; ++ps) {
             const int h = ps & 1;
             if (!resident) {
@@ -300,11 +323,21 @@ __global__ void __launch_bounds__(SMALL_THREADS, 2) k_small_fused(const SmallArg
         // (one result at a time from lane 0, each behind its own global load, was 40 % of the stall samples at tiny)
         if (b < v) {
             __syncwarp();
-            for (int ij = lane; ij < oo; ij += 32) {
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                const int ij = lane + 32 * t;
+                if (ij >= oo) break;
                 const int i_ = ij / p.o, j_ = ij - i_ * p.o;
                 const double val = res[ij];
-                r_update(p.R + i_ * p.rs.i + j_ * p.rs.j + a * p.rs.a + b * p.rs.b, val, p.alpha, p.beta);
-                if (p.pair && a != b) r_update(p.R + j_ * p.rs.i + i_ * p.rs.j + b * p.rs.a + a * p.rs.b, val, p.alpha, p.beta);
+                double *rd = p.R + i_ * p.rs.i + j_ * p.rs.j + a * p.rs.a + b * p.rs.b;
+                double *rm = p.R + j_ * p.rs.i + i_ * p.rs.j + b * p.rs.a + a * p.rs.b;
+                if (NB <= PREFETCH_R_MAX_NB) {  // the old values were fetched before the k loop
+                    *rd = (p.beta == 0.0) ? p.alpha * val : p.beta * rold[t][0] + p.alpha * val;
+                    if (p.pair && a != b) *rm = (p.beta == 0.0) ? p.alpha * val : p.beta * rold[t][1] + p.alpha * val;
+                } else {
+                    r_update(rd, val, p.alpha, p.beta);
+                    if (p.pair && a != b) r_update(rm, val, p.alpha, p.beta);
+                }
             }
         }
     }
