@@ -264,9 +264,9 @@ int ppl_contract_pair(const char *subscripts, const int64_t *dims0, const int64_
  * host memory).  Synchronises before returning.  Device buffers are
  * allocated on first use and kept by the plan (they are not counted against workspace_bytes).
  *   PPL_SYM_FULL: L is copied whole; t2 and R never sit on the device whole -- t2 is streamed through two staging
- *     buffers (1 GiB each) and packed chunk by chunk into tau+-, the slabs run on the packed operands, and the result
- *     is unpacked chunk by chunk (R chunk in, R += term, R chunk out), copies of one chunk overlapping the kernels of
- *     the other.  Device residency is about half of L + t2 + R: shapes of the paper's Table 3 fit on one 180 GB GPU.
+ *     buffers (1 GiB each) and packed chunk by chunk into tau+-, the slabs run on the packed operands, and R leaves
+ *     slab by slab while they run: behind every slab of 16 a's, R[:, :, slab, :] travels in (a 2-D copy), takes the
+ *     term, and travels out, beside the GEMMs of the following slabs.  Device residency is about half of L + t2 + R: shapes of the paper's Table 3 fit on one 180 GB GPU.
  *   PPL_SYM_NONE / PPL_SYM_PAIR (nothing assumed of L; PPL_SYM_NONE: nothing of t2 either -- the paper's own benchmark
  *     arrays), even nvirt: t2 is copied whole and stays resident (every W tile contracts with all of it);
  *     L never needs to be: when it does not fit beside t2 it is streamed as row panels L[:, A, :] (a 2-D copy of nchol

@@ -698,14 +698,15 @@ inline int step0_hints(const ppl_plan_s *p) { return p->dbg.full_hints == 0 ? 13
 // The whole path in PPL_SYM_FULL: everything on the caller's stream (every kernel fills the GPU; the
 // strip is single-buffered), prof as in run_apply.
 enum { FULL_PACK = 1, FULL_COMPUTE = 2, FULL_UNPACK = 4, FULL_ALL = 7 };
-int launch_unpack_full(const ppl_plan_s *p, const ppl_opts_t &opts, double *R, int64_t idx0, int64_t idx1, cudaStream_t stream);
+int launch_unpack_full(const ppl_plan_s *p, const ppl_opts_t &opts, double *R, int64_t idx0, int64_t idx1, cudaStream_t stream,
+                       int a0 = 0, int na = -1, const ppl::RStrides *rs = nullptr);
 
 // phases: FULL_PACK (t2 -> tau+-, clear R+-acc), FULL_COMPUTE (all slabs), FULL_UNPACK (R+-acc -> R).  ppl_apply runs all
 // three; ppl_apply_host packs and unpacks chunk by chunk itself and calls this with FULL_COMPUTE only (t2, R unused).
 // tau_ready (ppl_apply_host): tau+- are being packed on other streams; step 0 of the first slab needs only L and starts at
 // once, the event is waited for behind it.
 int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, const ppl_opts_t *opts_in, cudaStream_t stream,
-                   Prof *prof, int phases = FULL_ALL, cudaEvent_t tau_ready = nullptr) {
+                   Prof *prof, int phases = FULL_ALL, cudaEvent_t tau_ready = nullptr, const pplapi::SlabHook *hook = nullptr) {
     bool vec16 = false;
     int rc = check_ptrs(p, L, (phases & FULL_PACK) ? t2 : L, (phases & FULL_UNPACK) ? R : L, &vec16);
     ppl_opts_t opts;
@@ -949,6 +950,9 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
             ++tile_no;
         }
         if (!tight && (rc = unit_done()) != PPL_OK) return rc;
+        // the R+-acc columns (a, b >= a) of this slab's a's are final once its last reductions have run: they were the last
+        // writers (use 2 of every earlier slab is ordered before them), later slabs add to later columns only
+        if (hook && (rc = hook->fn(hook->ctx, sl.A0, sl.ta, conc ? p->fs[0] : stream, conc ? p->fs[1] : stream)) != PPL_OK) return rc;
     }
     if (conc)  // join: the side streams run in order, so the events of the last min(tiles, slots) tiles cover all work
         for (int s = 0; s < std::min(tile_no, p->fslots); ++s)
@@ -979,7 +983,9 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
 }
 
 // R[idx] = beta R + alpha (R+ +- R-) for the flattened (i,j,a,b) indices [idx0, idx1); R is the address of element (0,0,0,0)
-int launch_unpack_full(const ppl_plan_s *p, const ppl_opts_t &opts, double *R, int64_t idx0, int64_t idx1, cudaStream_t stream) {
+// na < 0: all a's, R in the caller's layout; else the a's [a0, a0 + na) with R addressed through *rs (a slab buffer)
+int launch_unpack_full(const ppl_plan_s *p, const ppl_opts_t &opts, double *R, int64_t idx0, int64_t idx1, cudaStream_t stream, int a0,
+                       int na, const ppl::RStrides *rs) {
     ppl::UnpackArgs u;
     u.rp = p->raccp;
     u.rm = p->raccm;
@@ -990,10 +996,12 @@ int launch_unpack_full(const ppl_plan_s *p, const ppl_opts_t &opts, double *R, i
     u.vk = p->vp;
     u.alpha = opts.alpha;
     u.beta = opts.beta;
-    u.rs = r_strides(p->o, p->v, opts.r_layout);
+    u.rs = rs ? *rs : r_strides(p->o, p->v, opts.r_layout);
     u.R = R;
     u.idx0 = idx0;
     u.idx1 = idx1;
+    u.a0 = na < 0 ? 0 : a0;
+    u.na = na < 0 ? p->v : na;
     const int64_t blocks = (idx1 - idx0 + 255) / 256;
     ppl::k_unpack_full<<<(int)std::min<int64_t>(std::max<int64_t>(blocks, 1), (int64_t)p->num_sms * 8), 256, 0, stream>>>(u);
     PPL_CUDA(cudaGetLastError());
@@ -1605,8 +1613,19 @@ int unpack_range(const ppl_plan_s *p, double *R, int64_t idx0, int64_t idx1, cud
     return launch_unpack_full(p, opts, R, idx0, idx1, s);
 }
 
-int full_compute(ppl_plan_s *p, const double *L, cudaStream_t s, cudaEvent_t tau_ready) {
-    return run_apply_full(p, L, nullptr, nullptr, nullptr, s, nullptr, FULL_COMPUTE, tau_ready);
+int full_compute(ppl_plan_s *p, const double *L, cudaStream_t s, cudaEvent_t tau_ready, const SlabHook *hook) {
+    return run_apply_full(p, L, nullptr, nullptr, nullptr, s, nullptr, FULL_COMPUTE, tau_ready, hook);
+}
+
+int unpack_slab(const ppl_plan_s *p, double *slab, int a0, int na, cudaStream_t s) {
+    ppl_opts_t opts;
+    check_opts(nullptr, &opts);
+    ppl::RStrides rs;  // the slab buffer holds R[i][j][a - a0][b], dense
+    rs.i = (int64_t)p->o * na * p->v;
+    rs.j = (int64_t)na * p->v;
+    rs.a = p->v;
+    rs.b = 1;
+    return launch_unpack_full(p, opts, slab - (int64_t)a0 * p->v, 0, (int64_t)p->o * p->o * na * p->v, s, a0, na, &rs);
 }
 
 int verify_begin(ppl_plan_s *p, const double *L, const double *t2, int t2_layout, cudaStream_t stream) {

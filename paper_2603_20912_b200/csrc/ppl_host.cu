@@ -38,11 +38,46 @@ void dev_free(double **ptr) {
 }
 }  // namespace
 
+static int host_events(ppl_plan_s *p);
+
 // PPL_SYM_FULL on host operands: the device never holds t2 or R.  t2 is streamed through two staging buffers and
 // packed chunk by chunk into tau+- (rows (i,j) of a chunk are contiguous in the [i][j][c][d] order), the slabs run on
-// the packed operands, and R+-acc is unpacked chunk by chunk into the staging buffers (R chunk in, result out).
+// the packed operands, and R leaves slab by slab WHILE they run: the rows a of R[i,j,a,b] that belong to a slab of the loop
+// are final as soon as that slab's reductions are (k_unpack_full on the a-range: slab R[:, :, A, :] in by a 2-D copy,
+// R += term, slab out), so that at the end only the last, smallest slab is still to travel.
 // Device residency: L + tau+- + R+-acc + the PPL_SYM_FULL workspace -- about half of L + t2 + R + workspace, which
 // is what lets the paper's Table 3 shapes (t2 and R of 39 GB each at N = 800) run on one 180 GB GPU.
+struct FullHostCtx {
+    ppl_plan_s *p;
+    double *Rh;
+    cudaStream_t st[2];
+    int k;
+};
+// called behind the launches of every slab (ppl_launch.h, SlabHook): the R+-acc columns of the a's [a0, a0 + ta) are final
+// once the work queued so far on s_plus / s_minus has run
+static int full_slab_hook(void *ctx_, int a0, int ta, cudaStream_t s_plus, cudaStream_t s_minus) {
+    FullHostCtx &c = *static_cast<FullHostCtx *>(ctx_);
+    ppl_plan_s *p = c.p;
+    ppl_plan_s::HostStream &h = p->hsn;
+    const int na = std::min(ta, p->v - a0);  // (odd nvirt: the pad index of the packed geometry is no row of R)
+    if (na <= 0) return PPL_OK;
+    const int slot = c.k & 1;
+    cudaStream_t s = c.st[slot];
+    ++c.k;
+    const size_t w = (size_t)na * p->v * 8, pitch = (size_t)p->vv * 8, rows = (size_t)p->o * p->o;
+    PPL_CUDA(cudaMemcpy2DAsync(h.rs[slot], w, c.Rh + (size_t)a0 * p->v, pitch, w, rows, cudaMemcpyHostToDevice, s));
+    PPL_CUDA(cudaEventRecord(h.ev_rsdone[slot], s_plus));
+    PPL_CUDA(cudaStreamWaitEvent(s, h.ev_rsdone[slot], 0));
+    if (s_minus != s_plus) {
+        PPL_CUDA(cudaEventRecord(h.ev_rsin[slot], s_minus));
+        PPL_CUDA(cudaStreamWaitEvent(s, h.ev_rsin[slot], 0));
+    }
+    const int rc = pplapi::unpack_slab(p, h.rs[slot], a0, na, s);
+    if (rc != PPL_OK) return rc;
+    PPL_CUDA(cudaMemcpy2DAsync(c.Rh + (size_t)a0 * p->v, pitch, h.rs[slot], w, w, rows, cudaMemcpyDeviceToHost, s));
+    return PPL_OK;
+}
+
 static int apply_host_full_queue(ppl_plan_s *p, const double *Lh, const double *t2h, double *Rh, uint64_t *h2d, uint64_t *d2h) {
     const size_t nL = (size_t)p->x * p->vv * 8;
     const int64_t rows = (int64_t)p->o * p->o;
@@ -74,10 +109,24 @@ static int apply_host_full_queue(ppl_plan_s *p, const double *Lh, const double *
             return fail(PPL_ERR_CUDA);
         }
     }
+    {
+        int rce = host_events(p);
+        if (rce != PPL_OK) return rce;
+        ppl_plan_s::HostStream &h = p->hsn;
+        const size_t slab = (size_t)rows * ppl::TA_FULL * p->v * 8;  // R[:, :, 16 a's, :]
+        if (h.slab_bytes < slab) {
+            for (int i = 0; i < 2; ++i) dev_free(&h.rs[i]);
+            h.slab_bytes = slab;
+        }
+        if (!dev_alloc(&h.rs[0], h.slab_bytes) || !dev_alloc(&h.rs[1], h.slab_bytes)) {
+            for (int i = 0; i < 2; ++i) dev_free(&h.rs[i]);
+            h.slab_bytes = 0;
+            return fail(PPL_ERR_ALLOC);
+        }
+    }
     cudaStream_t cs = p->host_stream;         // L in, all slabs
-    cudaStream_t st[2] = {p->gen, p->hs2};    // chunk k of t2 / R on stream k % 2; each stream owns one staging buffer
+    cudaStream_t st[2] = {p->gen, p->hs2};    // chunk k of t2, then slab k of R, on stream k % 2; each stream owns one buffer of each kind
     const bool minus = p->Mm > 0 && p->Km > 0;
-    const int64_t nchunks = (rows + p->hchunk_rows - 1) / p->hchunk_rows;
     // phase A: L in on the compute stream; t2 chunks in -> tau+- on the chunk streams, overlapping L and step 0 of slab 0
     PPL_CUDA(cudaMemcpyAsync(p->dL, Lh, nL, cudaMemcpyHostToDevice, cs));
     if (p->verify) {  // L only: t2 never sits on the device whole (include/ppl.h, PPL_OPT_VERIFY_INPUTS)
@@ -98,31 +147,12 @@ static int apply_host_full_queue(ppl_plan_s *p, const double *Lh, const double *
     PPL_CUDA(cudaEventRecord(p->ev_in, st[1]));
     PPL_CUDA(cudaStreamWaitEvent(st[0], p->ev_in, 0));
     PPL_CUDA(cudaEventRecord(p->ev_tau, st[0]));
-    // the first two R chunks travel to the (now free) staging buffers while the slabs run
-    auto r_chunk_in = [&](int64_t kk) -> int {
-        const int64_t r0 = kk * p->hchunk_rows, r1 = std::min<int64_t>(rows, r0 + p->hchunk_rows);
-        PPL_CUDA(cudaMemcpyAsync(p->hstage[kk & 1], Rh + r0 * p->vv, (size_t)(r1 - r0) * row_bytes, cudaMemcpyHostToDevice, st[kk & 1]));
-        return PPL_OK;
-    };
-    int rc = PPL_OK;
-    for (int64_t kk = 0; kk < std::min<int64_t>(2, nchunks); ++kk)
-        if ((rc = r_chunk_in(kk)) != PPL_OK) return rc;
-    // phase B: all slabs on the packed operands
-    rc = pplapi::full_compute(p, p->dL, cs, p->ev_tau);
+    // phase B: all slabs on the packed operands; behind every slab its rows of R travel in, take the term and travel out
+    // (slab k on chunk stream k & 1, which owns slab buffer k & 1: in order, so a buffer is refilled behind its D2H copy)
+    FullHostCtx ctx{p, Rh, {st[0], st[1]}, 0};
+    const pplapi::SlabHook hook{full_slab_hook, &ctx};
+    int rc = pplapi::full_compute(p, p->dL, cs, p->ev_tau, &hook);
     if (rc != PPL_OK) return rc;
-    PPL_CUDA(cudaEventRecord(p->ev_done, cs));
-    PPL_CUDA(cudaStreamWaitEvent(st[0], p->ev_done, 0));
-    PPL_CUDA(cudaStreamWaitEvent(st[1], p->ev_done, 0));
-    // phase C: R chunk in (the first two are there already), R += term, R chunk out
-    for (int64_t kk = 0; kk < nchunks; ++kk) {
-        const int64_t r0 = kk * p->hchunk_rows, r1 = std::min<int64_t>(rows, r0 + p->hchunk_rows);
-        cudaStream_t s = st[kk & 1];
-        double *buf = p->hstage[kk & 1];
-        const size_t bytes = (size_t)(r1 - r0) * row_bytes;
-        if (kk >= 2 && (rc = r_chunk_in(kk)) != PPL_OK) return rc;
-        if ((rc = pplapi::unpack_range(p, buf - r0 * p->vv, r0 * p->vv, r1 * p->vv, s)) != PPL_OK) return rc;
-        PPL_CUDA(cudaMemcpyAsync(Rh + r0 * p->vv, buf, bytes, cudaMemcpyDeviceToHost, s));
-    }
     PPL_CUDA(cudaStreamSynchronize(st[0]));
     PPL_CUDA(cudaStreamSynchronize(st[1]));
     PPL_CUDA(cudaStreamSynchronize(cs));
@@ -161,9 +191,8 @@ static int apply_host_full(ppl_plan_s *p, const double *Lh, const double *t2h, d
 // Streams: `in` all H2D copies in program order; `gen` step 0 (the plan's producer stream); `cs` step 1 + reduction;
 // `out` the D2H copies.  Events guard every buffer in both directions (filled -> may be read, read -> may be refilled).
 // ------------------------------------------------------------------------------------------------------------------
-static int host_tiles_setup(ppl_plan_s *p, bool panels, bool slabs) {
+static int host_events(ppl_plan_s *p) {
     ppl_plan_s::HostStream &h = p->hsn;
-    const size_t nT = (size_t)p->o * p->o * p->vv * 8, nL = (size_t)p->x * p->vv * 8;
     if (!h.events) {
         bool ok = cudaStreamCreateWithFlags(&h.in, cudaStreamNonBlocking) == cudaSuccess;
         ok = ok && cudaStreamCreateWithFlags(&h.out, cudaStreamNonBlocking) == cudaSuccess;
@@ -187,11 +216,24 @@ static int host_tiles_setup(ppl_plan_s *p, bool panels, bool slabs) {
         }
         h.events = true;
     }
+    return PPL_OK;
+}
+
+static int host_tiles_setup(ppl_plan_s *p, bool panels, bool slabs) {
+    ppl_plan_s::HostStream &h = p->hsn;
+    const size_t nT = (size_t)p->o * p->o * p->vv * 8, nL = (size_t)p->x * p->vv * 8;
+    int rc = host_events(p);
+    if (rc != PPL_OK) return rc;
     bool ok = dev_alloc(&p->dT, nT);
     if (ok && !slabs) ok = dev_alloc(&p->dR, nT);
     if (ok && slabs) {
-        h.slab_bytes = (size_t)p->o * p->o * p->T * p->v * 8;
+        const size_t slab = (size_t)p->o * p->o * p->T * p->v * 8;
+        if (h.slab_bytes < slab) {  // (the PPL_SYM_FULL route sizes the same two buffers for its own slabs)
+            for (int i = 0; i < 2; ++i) dev_free(&h.rs[i]);
+            h.slab_bytes = slab;
+        }
         for (int i = 0; i < 2 && ok; ++i) ok = dev_alloc(&h.rs[i], h.slab_bytes);
+        if (!ok) h.slab_bytes = 0;
     }
     if (ok && panels) {
         h.panel_bytes = (size_t)p->x * p->T * p->v * 8;
@@ -357,6 +399,7 @@ static int apply_host_tiles(ppl_plan_s *p, const double *Lh, const double *t2h, 
                 dev_free(&p->hsn.pa[i]);
                 dev_free(&p->hsn.rs[i]);
             }
+            p->hsn.slab_bytes = 0;
             for (int i = 0; i < MAX_RING; ++i) dev_free(&p->hsn.pb[i]);
         }
     }

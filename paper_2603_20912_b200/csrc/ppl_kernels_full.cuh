@@ -468,15 +468,17 @@ struct UnpackArgs {
     double alpha, beta;
     RStrides rs;
     double *R;
-    int64_t idx0, idx1;  // range of the flattened (i,j,a,b) index that is written (all: 0, o^2 v^2)
+    int64_t idx0, idx1;  // range of the flattened (i,j,a_l,b) index that is written (all: 0, o^2 na v)
+    int a0, na;          // the a's covered: a = a0 + a_l, a_l < na (all: 0, v).  A slab of a's is complete as soon as its own slab
+                         // of the PPL_SYM_FULL loop is: ppl_apply_host unpacks and ships R[:, :, slab, :] while later slabs run
 };
 
 __global__ void __launch_bounds__(256) k_unpack_full(const UnpackArgs p) {
     for (int64_t idx = p.idx0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < p.idx1; idx += (int64_t)gridDim.x * blockDim.x) {
         const int b = (int)(idx % p.v);
         int64_t r = idx / p.v;
-        const int a = (int)(r % p.v);
-        r /= p.v;
+        const int a = p.a0 + (int)(r % p.na);
+        r /= p.na;
         const int j = (int)(r % p.o), i = (int)(r / p.o);
         const int i1 = min(i, j), j1 = max(i, j), a1 = min(a, b), b1 = max(a, b);
         double val = p.rp[rowplus(i1, j1, p.o) * p.ldp + kplus(a1, b1, p.vk)];

@@ -25,7 +25,15 @@ uint32_t step1_box_rows(const ppl_plan_s *p);  // TMA box rows of the t2 map of 
 // PPL_SYM_FULL pieces (ppl_apply_host packs and unpacks chunk by chunk)
 int pack_rows(const ppl_plan_s *p, const double *t2, double diag, cudaStream_t s, int row0, int row1);
 int unpack_range(const ppl_plan_s *p, double *R, int64_t idx0, int64_t idx1, cudaStream_t s);
-int full_compute(ppl_plan_s *p, const double *L, cudaStream_t s, cudaEvent_t tau_ready);  // all slabs on the packed operands
+// all slabs on the packed operands.  hook (may be null): called behind the launches of every slab with the two streams whose
+// work so far completes the R+-acc columns of that slab's a's [a0, a0 + na)
+struct SlabHook {
+    int (*fn)(void *ctx, int a0, int na, cudaStream_t s_plus, cudaStream_t s_minus);
+    void *ctx;
+};
+int full_compute(ppl_plan_s *p, const double *L, cudaStream_t s, cudaEvent_t tau_ready, const SlabHook *hook);
+// R+-acc -> the slab R[:, :, a0 .. a0 + na, :] held dense in `slab` ([o*o][na][nvirt]); R += term
+int unpack_slab(const ppl_plan_s *p, double *slab, int a0, int na, cudaStream_t s);
 
 int verify_begin(ppl_plan_s *p, const double *L, const double *t2, int t2_layout, cudaStream_t stream);
 int verify_harvest(ppl_plan_s *p, int *flags_out);
