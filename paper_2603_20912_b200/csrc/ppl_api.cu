@@ -1317,8 +1317,21 @@ int ppl_apply_ex(ppl_plan_t *p, const double *L, const double *t2, double *R, co
             if (p->verify == 1 && p->small_ok) return run_apply_small(p, L, t2, R, opts, stream, nullptr, true);
             ppl_opts_t o;
             if (check_opts(opts, &o) != PPL_OK) return fail(PPL_ERR_INVALID_ARG);
-            rc = verify_begin(p, p->sym == PPL_SYM_FULL ? L : nullptr, t2, o.t2_layout, stream);
+            // PPL_SYM_FULL, mode 1: the check (HBM-bound: it reads L and t2 once) runs on the plan's producer stream, which that
+            // mode leaves idle, beside the first slab's step 0 instead of in front of it; `stream` joins it at the end of the
+            // apply, so that nothing queued later can change the inputs under it
+            const bool aside = p->sym == PPL_SYM_FULL && p->verify == 1 && p->gen != nullptr;
+            if (aside) {
+                PPL_CUDA(cudaEventRecord(p->ev_in, stream));
+                PPL_CUDA(cudaStreamWaitEvent(p->gen, p->ev_in, 0));
+            }
+            rc = verify_begin(p, p->sym == PPL_SYM_FULL ? L : nullptr, t2, o.t2_layout, aside ? p->gen : stream);
             if (rc != PPL_OK) return rc;
+            if (aside) {
+                rc = graph_wanted(p) ? apply_graph(p, L, t2, R, opts, stream) : apply_direct(p, L, t2, R, opts, stream);
+                PPL_CUDA(cudaStreamWaitEvent(stream, p->ev_verify, 0));
+                return rc;
+            }
         }
         if (graph_wanted(p)) return apply_graph(p, L, t2, R, opts, stream);
     }
