@@ -208,7 +208,8 @@ def run_table3(args, o, v, x):
         # resident and streams L panels / R slabs beside it.
         cap = 8 << 30
     else:
-        cap = int(free_b * 0.98) - x * v * v * 8 - (3 << 30)
+        # room for what ppl_apply_host allocates on first use: L whole, two 1-GiB staging buffers, two R slabs of 16 a's
+        cap = int(free_b * 0.98) - x * v * v * 8 - (2 << 30) - 2 * o * o * 16 * v * 8 - (1 << 30)
     plan = P.Plan(o, v, x, cap, debug={"host_panels": args.host_panels} if unpacked else None)
     if unpacked:
         plan.set_symmetry(P.PPL_SYM_NONE if args.symmetry == "none" else P.PPL_SYM_PAIR)

@@ -276,7 +276,7 @@ int ppl_contract_pair(const char *subscripts, const int64_t *dims0, const int64_
  *     of row k +- 1 overlapping the GEMMs of row k on streams of their own (in PPL_SYM_PAIR the mirror writes reach
  *     every slab, so R stays resident).  Device residency: t2 + the W ring + a few panels / slabs.
  *   PPL_SYM_PAIR_SA, or odd nvirt: L, t2 and R are copied whole, ppl_apply runs, R is copied back (PPL_ERR_ALLOC if they do not fit).
- *   At shapes that fill the device, plan with workspace_bytes = free device bytes - |L| - 3 GiB (what bench.py's
+ *   At shapes that fill the device, plan with workspace_bytes = free device bytes - |L| - 3 GiB - 2 R slabs of 16 a's (nocc^2 x 16 x nvirt doubles each) (what bench.py's
  *   table3_* configs do): the automatic cap of ppl_plan (90 % of the free bytes) leaves no room for L and the staging
  *   buffers, and the call then returns PPL_ERR_ALLOC.  Under such a cap the plan takes the memory-tight form of
  *   PPL_SYM_FULL (ppl_info_t.full_tight) when the 16 nvirt^3 strip does not fit.

@@ -441,10 +441,13 @@ ppl_plan_s *plan_host(int nocc, int nvirt, int nchol, size_t workspace_bytes, si
     for (int sa = 1; sa >= 0 && best_T == 0; --sa)
         for (int T = nvirt; T >= 1; --T) {
             if (forced_T && T != forced_T) continue;
-            // only edges that tile v evenly or nearly so (ragged edge at least T/2), to keep edge tiles efficient
+            // only edges that tile v evenly or nearly so (ragged edge at least T/4), to keep edge tiles efficient; the cost model
+            // weighs the rest.  (T/2 until round 2: it ruled out T = 16 at nvirt = 900 -- ragged 4 -- and the plan took T = 22, whose
+            // 484-row W tiles pad to 512 in step 1: 571 s instead of 549 s on the Table 3 row N = 1000; medium in the un-packed modes
+            // moved from T = 30 to 32: 68.2 -> 65.8 ms)
             const int nblk = (nvirt + T - 1) / T;
             const int r = nvirt - (nblk - 1) * T;
-            if (!forced_T && nblk > 1 && 2 * r < T) continue;
+            if (!forced_T && nblk > 1 && 4 * r < T) continue;
             const PlanEval ev = evaluate(g, nocc, nvirt, nchol, T, sa != 0, p->num_sms);
             const size_t fixed = ev.x_bytes + ev.part_bytes + (sa ? p->tau_bytes : 0) + 256;
             int ring = 0;
