@@ -273,3 +273,17 @@ def test_planner_builds_with_gpp_alone_and_agrees_with_the_library(tmp_path):
             rc = lib.ppl_plan_dry(*shape, cap, 170 << 30, 148, -1, ctypes.byref(out))
             assert rc == P.PPL_OK
             assert out.asdict() == P.ppl_plan_dry(*shape, workspace_bytes=cap, debug={"no_small_fused": 0})
+
+
+def test_ragged_tile_edges_down_to_a_quarter_are_candidates():
+    """Un-packed modes: an edge whose last block is ragged down to T/4 competes (the cost model counts its tiles); the round-1
+    rule (T/2) kept T = 16 out at nvirt = 900 and cost 4 % on the paper's Table 3 row N = 1000 (measured: 571 -> 549 s)."""
+    d = P.ppl_plan_dry(100, 900, 5000, workspace_bytes=8 << 30, mode=P.PPL_SYM_NONE)
+    assert (d["ta"], d["n_ablocks"], d["n_tiles"]) == (16, 57, 57 * 57)
+    d = P.ppl_plan_dry(20, 200, 800, mode=P.PPL_SYM_PAIR)
+    assert d["ta"] == 32 and d["n_ablocks"] == 7  # ragged last block of 8 = T/4
+    for v in (97, 130, 171, 200, 333):  # and never a last block below T/4
+        d = P.ppl_plan_dry(6, v, 64, mode=P.PPL_SYM_NONE, debug={"no_small_fused": 1})
+        T = d["ta"]
+        nblk = (v + T - 1) // T
+        assert nblk == 1 or 4 * (v - (nblk - 1) * T) >= T, (v, T)
