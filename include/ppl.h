@@ -47,7 +47,8 @@ enum {
     PPL_ERR_ALLOC = 3,               /* cudaMalloc / host allocation failed */
     PPL_ERR_CUDA = 4,                /* a CUDA runtime call or kernel launch failed */
     PPL_ERR_UNSUPPORTED_DEVICE = 5,  /* no CUDA device, or not compute capability 10.x */
-    PPL_ERR_PRECONDITION = 6         /* ppl_check_inputs: a symmetry the plan relies on is violated */
+    PPL_ERR_PRECONDITION = 6,        /* ppl_check_inputs: a symmetry the plan relies on is violated */
+    PPL_ERR_SCRATCH_LIMIT = 7        /* ppl_contract_pair_noalloc: the request needs more than PPL_NOALLOC_SCRATCH_BYTES */
 };
 
 /* Symmetry modes (ppl_plan_set_symmetry). */
@@ -259,6 +260,44 @@ int ppl_apply_dense(ppl_plan_t *plan, const double *eri, int a0, int na, const d
 int ppl_contract_pair_workspace(const char *subscripts, const int64_t *dims0, const int64_t *dims1, size_t *bytes);
 int ppl_contract_pair(const char *subscripts, const int64_t *dims0, const int64_t *dims1, const double *A, const double *B,
                       double *C, double alpha, double beta, void *workspace, size_t workspace_bytes, void *stream);
+
+/* ppl_contract_pair_noalloc: ppl_contract_pair for callers that cannot allocate device memory.
+ *
+ * Who that is: a program that has already handed the whole GPU to its own memory pool (a CC driver that sizes its
+ * tensors to 90 % of VRAM the way the paper does; a framework with a caching allocator that owns what is
+ * left), so that a cudaMalloc for a workspace would fail or push someone else out; code on a path where cudaMalloc /
+ * cudaFree are unwelcome because they synchronise the whole device and take a driver-wide lock; and plug-ins that are
+ * handed device pointers and a stream by their host and have no allocator of their own to ask.  Such callers cannot
+ * satisfy ppl_contract_pair's `workspace` argument.  This entry point does not have one.
+ *
+ * Same operation, same arguments otherwise:  C[out] = beta * C[out] + alpha * sum_{summed letters} A[op0] * B[op1],
+ * A, B, C DEVICE pointers (8-byte aligned, dense row-major in the order of their subscripts; C must not alias A or B;
+ * beta == 0 overwrites without reading C).  It always runs the in-place gather GEMM of the generic recipe (offset
+ * tables, DMMA, fixed-order split-K: bit-reproducible); plain matrix pairs are NOT re-routed to the ladder's TMA
+ * kernels as in ppl_contract_pair.
+ *
+ * Scratch: the offset tables, 16 (M + N + K) bytes (M, N = products of the surviving extents of op0 / op1, K = product
+ * of the summed extents), and the split-K partials live in a fixed array of PPL_NOALLOC_SCRATCH_BYTES that is part of
+ * the library: every GPU on which the library's code is loaded holds those bytes until the process exits, whether or
+ * not this function is ever called again.  Apart from the one-time set-up described below, a call is kernel launches
+ * only: no cudaMalloc, cudaFree, cudaMemcpy or allocating library routine; the tables are computed on the device.
+ *   Limit: a request whose tables alone exceed PPL_NOALLOC_SCRATCH_BYTES is refused with PPL_ERR_SCRATCH_LIMIT and
+ *   nothing is queued (use ppl_contract_pair with a workspace of your own).  Partials take what the tables leave:
+ *   the split-K factor is lowered, down to none, until they fit -- exactly what ppl_contract_pair does when given a
+ *   workspace of PPL_NOALLOC_SCRATCH_BYTES, and with the same results bit for bit on the gather route.
+ *   First call on a device: looks up the array's device address and the SM count and opts the kernels into their
+ *   shared-memory size, with the calling thread's current device; cached afterwards (thread-safe).  Make that first
+ *   call during start-up, before any stream capture begins in the process.
+ *   Sharing: there is ONE array per device and every call uses it.  Nothing in it needs clearing between calls (each
+ *   call rewrites all it reads), but calls whose kernels may overlap on the GPU -- issued on different streams without
+ *   an ordering between them, or from two threads -- race on it and give undefined results.  Calls on one stream, or
+ *   ordered by events, are safe.  The array keeps the last call's tables and partials; do not rely on that.
+ * Asynchronous on `stream` (NULL = the legacy default stream).  Errors: PPL_ERR_INVALID_ARG (malformed request, NULL or
+ * misaligned pointers), PPL_ERR_SCRATCH_LIMIT, PPL_ERR_UNSUPPORTED_DEVICE (no cc 10.x device current),
+ * PPL_ERR_CUDA. */
+#define PPL_NOALLOC_SCRATCH_BYTES (32u << 20) /* 32 MiB, resident per GPU for the life of the process */
+int ppl_contract_pair_noalloc(const char *subscripts, const int64_t *dims0, const int64_t *dims1, const double *A,
+                              const double *B, double *C, double alpha, double beta, void *stream);
 
 /* ppl_apply_host: the same operation on HOST buffers (pageable or pinned), the paper's own setting (operands in
  * host memory).  Synchronises before returning.  Device buffers are

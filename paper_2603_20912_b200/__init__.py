@@ -10,6 +10,8 @@ from .binding import (  # noqa: F401
     PPL_ERR_CUDA,
     PPL_ERR_INVALID_ARG,
     PPL_ERR_PRECONDITION,
+    PPL_ERR_SCRATCH_LIMIT,
+    PPL_NOALLOC_SCRATCH_BYTES,
     PPL_ERR_UNSUPPORTED_DEVICE,
     PPL_ERR_WORKSPACE_TOO_SMALL,
     PPL_OK,
@@ -28,6 +30,7 @@ from .binding import (  # noqa: F401
     library_path,
     ppl_apply,
     ppl_contract_pair,
+    ppl_contract_pair_noalloc,
     ppl_debug_dmma_layout,
     ppl_destroy,
     ppl_last_error,

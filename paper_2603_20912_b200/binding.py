@@ -19,6 +19,8 @@ PPL_ERR_ALLOC = 3
 PPL_ERR_CUDA = 4
 PPL_ERR_UNSUPPORTED_DEVICE = 5
 PPL_ERR_PRECONDITION = 6
+PPL_ERR_SCRATCH_LIMIT = 7
+PPL_NOALLOC_SCRATCH_BYTES = 32 << 20  # include/ppl.h
 PPL_SYM_NONE = 0
 PPL_SYM_PAIR = 1
 PPL_SYM_PAIR_SA = 2
@@ -109,6 +111,8 @@ SYMBOLS = {
     "ppl_contract_pair_workspace": (c_int, [c_char_p, POINTER(ctypes.c_int64), POINTER(ctypes.c_int64), POINTER(c_size_t)]),
     "ppl_contract_pair": (c_int, [c_char_p, POINTER(ctypes.c_int64), POINTER(ctypes.c_int64), c_void_p, c_void_p, c_void_p,
                                   c_double, c_double, c_void_p, c_size_t, c_void_p]),
+    "ppl_contract_pair_noalloc": (c_int, [c_char_p, POINTER(ctypes.c_int64), POINTER(ctypes.c_int64), c_void_p, c_void_p, c_void_p,
+                                          c_double, c_double, c_void_p]),
     "ppl_apply_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, POINTER(c_uint64), POINTER(c_uint64)]),
     "ppl_apply_profiled": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, POINTER(ppl_times_t)]),
     "ppl_destroy": (c_int, [c_void_p]),
@@ -368,6 +372,27 @@ def ppl_contract_pair(subscripts: str, A, B, C=None, alpha: float = 1.0, beta: f
                                    _stream_ptr(stream)), "ppl_contract_pair")
     if hasattr(workspace, "record_stream"):
         workspace.record_stream(stream if stream is not None else torch.cuda.current_stream())
+    return C
+
+
+def ppl_contract_pair_noalloc(subscripts: str, A, B, C, alpha: float = 1.0, beta: float = 0.0, stream=None):
+    """C = beta*C + alpha*einsum(subscripts, A, B) through the entry point that allocates nothing (include/ppl.h).
+
+    For callers that cannot get device memory of their own -- the GPU already belongs to someone's pool, or the call sits
+    where cudaMalloc's device-wide synchronisation is not acceptable.  Accordingly this wrapper allocates nothing either: the
+    caller passes the output C (a contiguous CUDA float64 tensor of the shape `out` spells), and there is no workspace
+    argument -- the library's fixed 32 MiB array (PPL_NOALLOC_SCRATCH_BYTES, one per GPU, shared by all calls) is the scratch.
+    Raises PplError(PPL_ERR_SCRATCH_LIMIT) when the request's offset tables do not fit into it.  Calls that may overlap on
+    the GPU (different streams, no ordering) race on that array; keep them on one stream."""
+    ins, out = subscripts.replace(" ", "").split("->")
+    s0, s1 = ins.split(",")
+    d0 = (ctypes.c_int64 * max(A.dim(), 1))(*A.shape)
+    d1 = (ctypes.c_int64 * max(B.dim(), 1))(*B.shape)
+    ext = dict(zip(s0, A.shape))
+    ext.update(zip(s1, B.shape))
+    shape = tuple(ext[c] for c in out)
+    _check(lib().ppl_contract_pair_noalloc(subscripts.encode(), d0, d1, _dev_ptr(A, "A"), _dev_ptr(B, "B"), _dev_ptr(C, "C", shape),
+                                           float(alpha), float(beta), _stream_ptr(stream)), "ppl_contract_pair_noalloc")
     return C
 
 

@@ -22,6 +22,7 @@
 #include <algorithm>
 #include <cstdint>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 namespace ppl {
@@ -483,3 +484,204 @@ int ppl_contract_pair(const char *subscripts, const int64_t *dims0, const int64_
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// ppl_contract_pair_noalloc: the same contraction for callers that must not allocate device memory (include/ppl.h).
+//
+// Everything the gather GEMM needs beyond A, B and C -- the six offset tables and, when the summed range is split, the
+// split-K partials -- lives in ONE fixed array that is part of the library image.  The driver places it on every
+// device that loads this library's code and keeps it there until the process exits; PPL_NOALLOC_SCRATCH_BYTES is the
+// whole price, paid once, and also the hard limit of what a request may need.
+//
+// In host code the identifier `noalloc_scratch` is only the host-side handle of that array, not something a kernel
+// may dereference: the device address comes from cudaGetSymbolAddress, asked for once per device (with that device
+// current) in noalloc_device() below, and it is that address which the kernels receive.
+//
+// The tables are written by a small kernel from the <= 12 extents and strides of each axis group (kernel parameters:
+// no host table, no upload), so a call is three launches at most and touches no allocator, on the host side of CUDA or
+// on the device.  Every call rewrites every word of the array it later reads (all tables; all M x N entries of every
+// partial), so nothing has to be cleared between calls; what the previous call left there is simply overwritten.
+// All calls on a device share the array: two calls whose kernels can overlap on the GPU (different streams with no
+// dependency between them, or two host threads) race on it.  Calls on one stream are ordered and safe.
+namespace ppl {
+
+static __device__ __align__(256) unsigned char noalloc_scratch[PPL_NOALLOC_SCRATCH_BYTES];
+
+struct NoallocAxes {       // one offset table: the flattened index over n letters, last letter fastest
+    int64_t ext[12], stride[12];
+    int64_t count;         // product of the extents (1 when n == 0)
+    int32_t n, pad_;
+};
+struct NoallocTables {
+    NoallocAxes t[6];      // in workspace order: A rows, C rows, B columns, C columns, A k, B k
+};
+
+__global__ void __launch_bounds__(256) k_noalloc_fill_tables(const NoallocTables f, int64_t *tab) {
+    int64_t total = 0;
+    for (int w = 0; w < 6; ++w) total += f.t[w].count;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+        int64_t r = idx;
+        int w = 0;
+        while (r >= f.t[w].count) r -= f.t[w++].count;
+        const NoallocAxes &ax = f.t[w];
+        int64_t off = 0;
+        for (int k = ax.n - 1; k >= 0; --k) {
+            const int64_t q = r / ax.ext[k];
+            off += (r - q * ax.ext[k]) * ax.stride[k];
+            r = q;
+        }
+        tab[idx] = off;
+    }
+}
+
+}  // namespace ppl
+
+namespace {
+
+struct NoallocDevice {
+    bool ready = false;
+    unsigned char *scratch = nullptr;  // DEVICE address of ppl::noalloc_scratch on this device
+    int sms = 0;
+};
+std::mutex noalloc_mutex;
+NoallocDevice noalloc_dev[64];
+
+// Once per device, with that device current: the device address of the array, the SM count, the kernels' shared-memory
+// opt-in.  Later calls only read the cached entry.
+int noalloc_device(const NoallocDevice **out) {
+    int dev = -1, major = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64 ||
+        cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess || major != 10) {
+        (void)cudaGetLastError();
+        return PPL_ERR_UNSUPPORTED_DEVICE;
+    }
+    std::lock_guard<std::mutex> lock(noalloc_mutex);
+    NoallocDevice &d = noalloc_dev[dev];
+    if (!d.ready) {
+        unsigned char *ptr = nullptr;
+        bool ok = cudaGetSymbolAddress((void **)&ptr, ppl::noalloc_scratch) == cudaSuccess && ptr != nullptr;
+        ok = ok && cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && d.sms > 0;
+        ok = ok && cudaFuncSetAttribute(ppl::k_contract_gather<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
+        ok = ok && cudaFuncSetAttribute(ppl::k_contract_gather<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
+        ok = ok && cudaFuncSetAttribute(ppl::k_contract_gather<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
+        ok = ok && cudaFuncSetAttribute(ppl::k_contract_gather<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
+        if (!ok) {
+            (void)cudaGetLastError();
+            return PPL_ERR_CUDA;
+        }
+        d.scratch = ptr;
+        d.ready = true;
+    }
+    *out = &d;
+    return PPL_OK;
+}
+
+void noalloc_axes(const std::vector<char> &letters, const std::vector<char> &op, const int64_t *ext, ppl::NoallocAxes *ax) {
+    ax->n = (int32_t)letters.size();
+    ax->pad_ = 0;
+    ax->count = 1;
+    for (int k = 0; k < 12; ++k) ax->ext[k] = 1, ax->stride[k] = 0;
+    for (size_t k = 0; k < letters.size(); ++k) {
+        ax->ext[k] = ext[(int)letters[k]];
+        ax->stride[k] = stride_of(op, ext, letters[k]);
+        ax->count *= ax->ext[k];
+    }
+}
+
+// What pairs_ok() decides from the tables, decided from the axes instead: along `run`, are the elements (2i, 2i+1)
+// neighbours in memory at an even element offset, whatever the position along `other`?  Fold the trailing letters of
+// `run` that are contiguous with each other into one; that group must have stride 1 and an even extent, and every
+// other letter with more than one value (of `run` and of `other`) must have an even stride.
+bool noalloc_pairs_ok(const ppl::NoallocAxes &run, const ppl::NoallocAxes &other, const void *base) {
+    if (((uintptr_t)base & 15) != 0 || (run.count & 1)) return false;
+    int k = run.n - 1;
+    while (k >= 0 && run.ext[k] == 1) --k;
+    if (k < 0 || run.stride[k] != 1) return false;
+    int64_t group = run.ext[k];
+    for (--k; k >= 0; --k) {
+        if (run.ext[k] == 1) continue;
+        if (run.stride[k] != group) break;  // not contiguous with the group so far
+        group *= run.ext[k];
+    }
+    if (group & 1) return false;
+    for (; k >= 0; --k)
+        if (run.ext[k] > 1 && (run.stride[k] & 1)) return false;
+    for (int j = 0; j < other.n; ++j)
+        if (other.ext[j] > 1 && (other.stride[j] & 1)) return false;
+    return true;
+}
+
+}  // namespace
+
+extern "C" int ppl_contract_pair_noalloc(const char *subscripts, const int64_t *dims0, const int64_t *dims1, const double *A,
+                                         const double *B, double *C, double alpha, double beta, void *stream_) {
+    Parsed ps;
+    int rc = parse(subscripts, dims0, dims1, &ps);
+    if (rc != PPL_OK) return ppl_fail_code(rc);
+    if (!A || !B || !C || (((uintptr_t)A | (uintptr_t)B | (uintptr_t)C) & 7)) return ppl_fail_code(PPL_ERR_INVALID_ARG);
+    const size_t tb = (table_bytes(ps) + 255) & ~(size_t)255;
+    if (tb > (size_t)PPL_NOALLOC_SCRATCH_BYTES) return ppl_fail_code(PPL_ERR_SCRATCH_LIMIT);
+    const int64_t tiles = ((ps.M + ppl::BM - 1) / ppl::BM) * ((ps.N + ppl::BN - 1) / ppl::BN);
+    if (tiles > INT32_MAX) return ppl_fail_code(PPL_ERR_INVALID_ARG);
+    const NoallocDevice *dev = nullptr;
+    rc = noalloc_device(&dev);
+    if (rc != PPL_OK) return ppl_fail_code(rc);
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+
+    ppl::NoallocTables f;
+    noalloc_axes(ps.Ml, ps.op[0], ps.ext, &f.t[0]);
+    noalloc_axes(ps.Ml, ps.op[2], ps.ext, &f.t[1]);
+    noalloc_axes(ps.Nl, ps.op[1], ps.ext, &f.t[2]);
+    noalloc_axes(ps.Nl, ps.op[2], ps.ext, &f.t[3]);
+    noalloc_axes(ps.Kl, ps.op[0], ps.ext, &f.t[4]);
+    noalloc_axes(ps.Kl, ps.op[1], ps.ext, &f.t[5]);
+    int64_t *tab = reinterpret_cast<int64_t *>(dev->scratch);
+    const int64_t entries = 2 * (ps.M + ps.N + ps.K);
+    ppl::k_noalloc_fill_tables<<<(int)std::min<int64_t>((entries + 255) / 256, (int64_t)dev->sms * 8), 256, 0, stream>>>(f, tab);
+    if (cudaGetLastError() != cudaSuccess) return ppl_fail_code(PPL_ERR_CUDA);
+
+    ppl::ContractArgs a;
+    a.A = A;
+    a.B = B;
+    a.C = C;
+    a.offAm = tab;
+    a.offCm = a.offAm + ps.M;
+    a.offBn = a.offCm + ps.M;
+    a.offCn = a.offBn + ps.N;
+    a.offAk = a.offCn + ps.N;
+    a.offBk = a.offAk + ps.K;
+    a.M = (int)ps.M;
+    a.N = (int)ps.N;
+    a.K = (int)ps.K;
+    const bool a_kfast = !ps.op[0].empty() && std::find(ps.Kl.begin(), ps.Kl.end(), ps.op[0].back()) != ps.Kl.end();
+    const bool b_kfast = !ps.op[1].empty() && std::find(ps.Kl.begin(), ps.Kl.end(), ps.op[1].back()) != ps.Kl.end();
+    a.a_vec = a_kfast ? noalloc_pairs_ok(f.t[4], f.t[0], A) : noalloc_pairs_ok(f.t[0], f.t[4], A);
+    a.b_vec = b_kfast ? noalloc_pairs_ok(f.t[5], f.t[2], B) : noalloc_pairs_ok(f.t[2], f.t[5], B);
+    // split-K as ppl_contract_pair picks it for a workspace of PPL_NOALLOC_SCRATCH_BYTES: the partials take what the
+    // tables leave, and the factor shrinks (down to 1 = no partials at all) when they would not fit
+    a.splitk = pick_splitk(ps, dev->sms, (size_t)PPL_NOALLOC_SCRATCH_BYTES - tb);
+    const int64_t nkt = (ps.K + ppl::BK - 1) / ppl::BK;
+    const int64_t kt_per = (nkt + a.splitk - 1) / a.splitk;
+    a.splitk = (int)((nkt + kt_per - 1) / kt_per);  // no empty splits
+    a.k_per_split = (int)(kt_per * ppl::BK);
+    a.part = a.splitk > 1 ? reinterpret_cast<double *>(dev->scratch + tb) : nullptr;
+    a.alpha = alpha;
+    a.beta = beta;
+
+    const dim3 grid((unsigned)tiles, (unsigned)a.splitk);
+    if (a_kfast && b_kfast)
+        ppl::k_contract_gather<true, true><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
+    else if (a_kfast)
+        ppl::k_contract_gather<true, false><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
+    else if (b_kfast)
+        ppl::k_contract_gather<false, true><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
+    else
+        ppl::k_contract_gather<false, false><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
+    if (cudaGetLastError() != cudaSuccess) return ppl_fail_code(PPL_ERR_CUDA);
+    if (a.splitk > 1) {
+        const int64_t MN = ps.M * ps.N;
+        ppl::k_contract_reduce<<<(int)std::min<int64_t>((MN + 255) / 256, (int64_t)dev->sms * 8), 256, 0, stream>>>(a);
+        if (cudaGetLastError() != cudaSuccess) return ppl_fail_code(PPL_ERR_CUDA);
+    }
+    return PPL_OK;
+}

@@ -535,6 +535,7 @@ const char *ppl_error_string(int code) {
         case PPL_ERR_CUDA: return "CUDA runtime error";
         case PPL_ERR_UNSUPPORTED_DEVICE: return "no CUDA device of compute capability 10.x (no fallback path exists)";
         case PPL_ERR_PRECONDITION: return "input violates a symmetry the plan relies on";
+        case PPL_ERR_SCRATCH_LIMIT: return "request exceeds the built-in scratch of the no-allocation entry point (PPL_NOALLOC_SCRATCH_BYTES)";
         default: return "unknown error";
     }
 }
