@@ -361,7 +361,10 @@ int ppl_plan_set_symmetry(ppl_plan_t *plan, int mode);
  * violation if the check has finished by then, and otherwise the call after it does: a call never waits for the check of the
  * apply queued just before it (that would serialise host and device at shapes where an apply takes 20 us);
  * ppl_plan_verify_status and ppl_destroy wait for everything outstanding.
- * ppl_apply_host verifies L only in its streamed form (t2 never sits on the device whole). */
+ * ppl_apply_host reports a violation from the same call (it synchronises before returning; R is then undefined).  In its
+ * streamed PPL_SYM_FULL form t2 never sits on the device whole: its pair symmetry is verified chunk by chunk instead -- the
+ * rows i >= j of every staged chunk, which the packing never reads, are folded as their mirror images and compared bit for
+ * bit with what the rows (j,i) packed into tau+- (diagonal rows i == j: t2[i,i,c,d] == t2[i,i,d,c] directly). */
 enum { PPL_OPT_VERIFY_INPUTS = 1 };
 int ppl_plan_set_option(ppl_plan_t *plan, int option, int value);
 /* Waits for the check of the most recent apply (if one is pending) and returns PPL_OK or PPL_ERR_PRECONDITION;

@@ -107,7 +107,7 @@ void free_plan(ppl_plan_s *p) {
         for (int i = 0; i < 2; ++i) {
             if (h.pa[i]) cudaFree(h.pa[i]);
             if (h.rs[i]) cudaFree(h.rs[i]);
-            for (cudaEvent_t e : {h.ev_pa[i], h.ev_pafree[i], h.ev_rsin[i], h.ev_rsdone[i], h.ev_rsfree[i]})
+            for (cudaEvent_t e : {h.ev_pa[i], h.ev_pafree[i], h.ev_rsin[i], h.ev_rsdone[i], h.ev_rsfree[i], h.ev_chunk[i]})
                 if (e) cudaEventDestroy(e);
         }
         for (int i = 0; i < MAX_RING; ++i) {
@@ -1618,6 +1618,32 @@ int reduce_tile(const ppl_plan_s *p, const Tile &t, double *R, int64_t si, int64
 
 int pack_rows(const ppl_plan_s *p, const double *t2, double diag, cudaStream_t s, int row0, int row1) {
     return launch_pack(p, t2, PPL_LAYOUT_IJAB, diag, s, row0, row1);
+}
+
+// rows [row0, row1) of t2 (staged; t2 = address of element (0,0,0,0)) against the tau+- rows their mirror images wrote:
+// sets bit 1 of the per-apply verification flags (the words verify_begin cleared), see k_check_t2_rows
+int check_rows(const ppl_plan_s *p, const double *t2, double diag, cudaStream_t s, int row0, int row1) {
+    ppl::CheckRowsArgs a;
+    a.t2 = t2;
+    a.taup = p->taup;
+    a.taum = p->taum;
+    a.ldp = p->ldp;
+    a.ldm = p->ldm;
+    a.row0 = row0;
+    a.row1 = row1;
+    a.o = p->o;
+    a.v = p->v;
+    a.vp = p->vp;
+    a.scale = 0.5;
+    a.diag = diag;
+    int *dflags = nullptr;
+    PPL_CUDA(cudaHostGetDevicePointer(&dflags, p->vflags_host, 0));
+    a.flags = dflags;
+    const int nb = (p->v + 31) / 32;
+    const int64_t items = (int64_t)(row1 - row0) * nb * (nb + 1) / 2;
+    ppl::k_check_t2_rows<<<(int)std::max<int64_t>(1, std::min<int64_t>(items, (int64_t)p->num_sms * 8)), 256, 0, s>>>(a);
+    PPL_CUDA(cudaGetLastError());
+    return PPL_OK;
 }
 
 int unpack_range(const ppl_plan_s *p, double *R, int64_t idx0, int64_t idx1, cudaStream_t s) {

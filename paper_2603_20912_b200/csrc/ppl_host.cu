@@ -129,7 +129,7 @@ static int apply_host_full_queue(ppl_plan_s *p, const double *Lh, const double *
     const bool minus = p->Mm > 0 && p->Km > 0;
     // phase A: L in on the compute stream; t2 chunks in -> tau+- on the chunk streams, overlapping L and step 0 of slab 0
     PPL_CUDA(cudaMemcpyAsync(p->dL, Lh, nL, cudaMemcpyHostToDevice, cs));
-    if (p->verify) {  // L only: t2 never sits on the device whole (include/ppl.h, PPL_OPT_VERIFY_INPUTS)
+    if (p->verify) {  // L here; t2 never sits on the device whole and is verified chunk by chunk below (same flag words)
         const int rcv = pplapi::verify_begin(p, p->dL, nullptr, PPL_LAYOUT_IJAB, cs);
         if (rcv != PPL_OK) return rcv;
     }
@@ -141,8 +141,16 @@ static int apply_host_full_queue(ppl_plan_s *p, const double *Lh, const double *
         cudaStream_t s = st[k & 1];
         double *buf = p->hstage[k & 1];
         PPL_CUDA(cudaMemcpyAsync(buf, t2h + r0 * p->vv, (size_t)(r1 - r0) * row_bytes, cudaMemcpyHostToDevice, s));
-        const int rc = pplapi::pack_rows(p, buf - r0 * p->vv, 0.5, s, (int)r0, (int)r1);
+        int rc = pplapi::pack_rows(p, buf - r0 * p->vv, 0.5, s, (int)r0, (int)r1);
         if (rc != PPL_OK) return rc;
+        if (p->verify) {
+            // pair symmetry of t2: the rows i >= j of the chunk against the tau+- rows their mirror images (j,i) <= (i,j)
+            // wrote -- in this chunk, in chunk k - 2, k - 4, ... (this stream) or in chunk k - 1, k - 3, ... (the other one)
+            PPL_CUDA(cudaEventRecord(p->hsn.ev_chunk[k & 1], s));
+            if (k > 0) PPL_CUDA(cudaStreamWaitEvent(s, p->hsn.ev_chunk[(k - 1) & 1], 0));
+            rc = pplapi::check_rows(p, buf - r0 * p->vv, 0.5, s, (int)r0, (int)r1);
+            if (rc != PPL_OK) return rc;
+        }
     }
     PPL_CUDA(cudaEventRecord(p->ev_in, st[1]));
     PPL_CUDA(cudaStreamWaitEvent(st[0], p->ev_in, 0));
@@ -159,7 +167,10 @@ static int apply_host_full_queue(ppl_plan_s *p, const double *Lh, const double *
     const uint64_t nT = (uint64_t)rows * row_bytes;
     if (h2d) *h2d = (uint64_t)nL + 2 * nT;
     if (d2h) *d2h = nT;
-    return pplapi::verify_harvest(p, nullptr);
+    rc = pplapi::verify_harvest(p, nullptr);
+    // (synchronous mode 2 harvested L's word at the head of the call; the chunk checks have set t2's word since)
+    if (rc == PPL_OK && p->verify && p->vflags_host[1]) rc = fail(PPL_ERR_PRECONDITION);
+    return rc;
 }
 
 // An error half way leaves copies and kernels in flight on three streams that read and write the caller's host buffers:
@@ -203,6 +214,7 @@ static int host_events(ppl_plan_s *p) {
             ev(&h.ev_rsin[i]);
             ev(&h.ev_rsdone[i]);
             ev(&h.ev_rsfree[i]);
+            ev(&h.ev_chunk[i]);
         }
         for (int i = 0; i < MAX_RING; ++i) {
             ev(&h.ev_pb[i]);

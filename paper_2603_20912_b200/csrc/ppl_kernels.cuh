@@ -610,6 +610,72 @@ __global__ void __launch_bounds__(256) k_check_inputs(const CheckArgs p) {
     if (f & 2) p.flags[1] = 1;
 }
 
+// ppl_apply_host in PPL_SYM_FULL: t2 never sits on the device whole, so k_check_inputs cannot compare row (i,j) with row
+// (j,i).  The packing uses the rows i <= j only; this kernel looks at the OTHER rows of a staged chunk, which the path
+// would otherwise never read:
+//   i == j:  t2[i,i,c,d] == t2[i,i,d,c] directly (the antisymmetric part of a diagonal row has no place in tau-);
+//   i >  j:  the row folded as its mirror image must reproduce, bit for bit, what row (j,i) wrote into tau+- earlier
+//            (chunks arrive in ascending (i,j), and (j,i) < (i,j)):
+//                tau+[(j,i)][(c,d)] == scale (x[c,d] + x[d,c]),   tau-[(j,i)][(c,d)] == scale (x[d,c] - x[c,d]),   x = t2[i,j,.,.]
+//            -- the same two operands in the same operations as k_symfold, so a pair-symmetric t2 passes exactly, and a
+//            t2 that passes differs from a pair-symmetric one by at most the rounding of those sums.
+// One item = one such row x one pair (c-block <= d-block) of 32 x 32 blocks, staged through shared memory as in
+// check_inputs_scan so that both the block and its transpose are read coalesced.
+struct CheckRowsArgs {
+    const double *t2;       // address of element (0,0,0,0) of the dense [i][j][c][d] array; only rows [row0, row1) are dereferenced
+    const double *taup, *taum;
+    int64_t ldp, ldm;
+    int row0, row1;         // rows of the flattened (i,j) index held by the staged chunk
+    int o, v, vp;           // v: nvirt of the source; vp: nvirt of the packed geometry (kplus / kminus)
+    double scale, diag;     // the factors the chunk was packed with (k_symfold)
+    volatile int *flags;    // as CheckArgs::flags; only [1] is written here
+};
+__global__ void __launch_bounds__(256) k_check_t2_rows(const CheckRowsArgs p) {
+    __shared__ double sa[32][33], sb[32][33];
+    const int nb = (p.v + 31) / 32;
+    const int64_t npair = (int64_t)nb * (nb + 1) / 2;
+    const int64_t items = (int64_t)(p.row1 - p.row0) * npair;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int64_t vv = (int64_t)p.v * p.v;
+    bool bad = false;
+    for (int64_t item = blockIdx.x; item < items; item += gridDim.x) {
+        const int r = p.row0 + (int)(item / npair);
+        const int i = r / p.o, j = r - i * p.o;
+        if (i < j) continue;  // (uniform over the block) rows the packing itself reads
+        int rem = (int)(item % npair), cb = 0;
+        while (rem >= nb - cb) {
+            rem -= nb - cb;
+            ++cb;
+        }
+        const int c0 = cb * 32, d0 = (cb + rem) * 32;
+        const double *x = p.t2 + (int64_t)r * vv;
+        __syncthreads();  // the previous item's reads of sa / sb are done
+        for (int y = ty; y < 32; y += 8) {
+            const int c = c0 + y, d = d0 + tx;
+            sa[y][tx] = (c < p.v && d < p.v) ? __ldg(x + (int64_t)c * p.v + d) : 0.0;
+            const int c2 = d0 + y, d2 = c0 + tx;
+            sb[y][tx] = (c2 < p.v && d2 < p.v) ? __ldg(x + (int64_t)c2 * p.v + d2) : 0.0;
+        }
+        __syncthreads();
+        const double *tp = p.taup + rowplus(j, i, p.o) * p.ldp;
+        const double *tm = i > j ? p.taum + rowminus(j, i, p.o) * p.ldm : nullptr;
+        for (int y = ty; y < 32; y += 8) {
+            const int c = c0 + y, d = d0 + tx;
+            if (c >= p.v || d >= p.v || d < c) continue;
+            const double xcd = sa[y][tx], xdc = sb[tx][y];
+            if (i == j) {
+                if (xcd != xdc) bad = true;
+            } else if (c == d) {
+                if (tp[kplus(c, d, p.vp)] != p.diag * xcd) bad = true;
+            } else {
+                if (tp[kplus(c, d, p.vp)] != p.scale * (xcd + xdc)) bad = true;
+                if (tm[kminus(c, d, p.vp)] != p.scale * (xdc - xcd)) bad = true;
+            }
+        }
+    }
+    if (bad) p.flags[1] = 1;
+}
+
 // ---------------------------------------------------------------------------------------------
 // FP64 tensor-pipe peak probe (register-only DMMA stream) and a one-warp fragment-layout check
 // ---------------------------------------------------------------------------------------------

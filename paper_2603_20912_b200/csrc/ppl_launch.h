@@ -24,6 +24,8 @@ uint32_t step1_box_rows(const ppl_plan_s *p);  // TMA box rows of the t2 map of 
 
 // PPL_SYM_FULL pieces (ppl_apply_host packs and unpacks chunk by chunk)
 int pack_rows(const ppl_plan_s *p, const double *t2, double diag, cudaStream_t s, int row0, int row1);
+// verification of a staged chunk: its rows i >= j against what the rows i <= j packed (bit 1 of the per-apply flags)
+int check_rows(const ppl_plan_s *p, const double *t2, double diag, cudaStream_t s, int row0, int row1);
 int unpack_range(const ppl_plan_s *p, double *R, int64_t idx0, int64_t idx1, cudaStream_t s);
 // all slabs on the packed operands.  hook (may be null): called behind the launches of every slab with the two streams whose
 // work so far completes the R+-acc columns of that slab's a's [a0, a0 + na)

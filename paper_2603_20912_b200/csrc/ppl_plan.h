@@ -128,6 +128,7 @@ struct ppl_plan_s {
         cudaStream_t in = nullptr, out = nullptr;        // H2D copies / D2H copies
         cudaEvent_t ev_pa[2] = {}, ev_pafree[2] = {}, ev_pb[pplh::MAX_RING] = {}, ev_pbfree[pplh::MAX_RING] = {};
         cudaEvent_t ev_rsin[2] = {}, ev_rsdone[2] = {}, ev_rsfree[2] = {}, ev_t2 = nullptr, ev_fork = nullptr;
+        cudaEvent_t ev_chunk[2] = {};                    // PPL_SYM_FULL: chunk k of t2 is packed (recorded on chunk stream k & 1)
         bool events = false;
     } hsn;
     double f_step0 = 0, f_step1 = 0;

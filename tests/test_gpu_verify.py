@@ -129,3 +129,42 @@ def test_host_entry_point_reports_at_once():
         with pytest.raises(P.PplError) as e:
             plan.apply_host(Ln, t2, R)
         assert e.value.code == P.PPL_ERR_PRECONDITION
+
+
+@pytest.mark.parametrize("shape,chunk_mb", [((6, 96, 6), 1), ((6, 96, 6), 0), ((5, 53, 7), 1), ((4, 130, 5), 1)])
+def test_host_entry_point_checks_t2_chunk_by_chunk_in_the_default_mode(shape, chunk_mb):
+    """ppl_apply_host in PPL_SYM_FULL streams t2 through staging buffers and packs only its rows i <= j, so a
+    t2 that is not pair-symmetric used to give a wrong R with PPL_OK.  Now the rows i >= j of every chunk are compared with
+    what their mirror images packed (k_check_t2_rows); 1 MiB staging buffers put a row and its image into different chunks
+    on different streams."""
+    o, v, x = shape
+    L = I.make_L(v, x, 21, symmetric=True)
+    ts = I.make_t2(o, v, 21, symmetric=True)
+    dbg = {"host_chunk_mb": chunk_mb} if chunk_mb else None
+    with P.Plan(o, v, x, debug=dbg) as plan:
+        assert plan.info()["symmetry"] == P.PPL_SYM_FULL
+        R = np.zeros((o, o, v, v))
+        plan.apply_host(L, ts, R)  # clean inputs pass, and the result is the oracle's
+        assert relerr(R, oracle.full(L, ts)) <= 1e-11
+        # one wrong element: in a row i > j (never read by the packing), in a row i < j, in the antisymmetric part of a
+        # diagonal row, in the last row, on the diagonal c == d of a row i > j
+        for (i, j, c, d) in [(o - 1, 0, 3, v - 2), (0, o - 1, v - 1, 0), (2, 2, 1, v - 1), (o - 1, o - 2, 0, 1), (3, 1, 7, 7)]:
+            t = ts.copy()
+            t[i, j, c, d] += 1e-9
+            with pytest.raises(P.PplError) as e:
+                plan.apply_host(L, t, np.zeros((o, o, v, v)))
+            assert e.value.code == P.PPL_ERR_PRECONDITION, (i, j, c, d)
+        # a fully unstructured t2, in the synchronous mode as well
+        tn = I.make_t2(o, v, 22, symmetric=False)
+        for mode in (1, 2):
+            plan.set_verify(mode)
+            with pytest.raises(P.PplError) as e:
+                plan.apply_host(L, tn, np.zeros((o, o, v, v)))
+            assert e.value.code == P.PPL_ERR_PRECONDITION
+        # the report clears the state; the caller may vouch for its inputs instead
+        plan.set_verify(0)
+        plan.apply_host(L, tn, np.zeros((o, o, v, v)))
+        plan.set_verify(1)
+        R = np.zeros((o, o, v, v))
+        plan.apply_host(L, ts, R)
+        assert relerr(R, oracle.full(L, ts)) <= 1e-11
