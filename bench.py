@@ -6,12 +6,14 @@
 
 A "step" is one ppl_apply: the whole hot path (step 0 W-tile generation, step 1
 (c,d) contraction, reduce/accumulate/mirror, ring/streams) over one seeded synthetic batch shaped
-like BASELINE.json's configs.  Default workload: 'large' (configs[3], one of the two configs the
-north_star target is quoted on; 'xl' is the other: --config xl).
+like BASELINE.json's configs.  Default workload: 'xl' (configs[4], the largest single-GPU config);
+the default line also carries complete sub-records "large", "medium", "small", "tiny" (all five
+configs of BASELINE.json; the launch-bound ones averaged over >= 50 calls).
 
-value  = executed FP64 TFLOP/s (flops of the tiles actually computed / time; pair symmetry halves
-         the nominal 2*nchol*nvirt^4 + 2*nocc^2*nvirt^4, and the line says so), inputs resident
-         in HBM.
+value  = FP64 TFLOP/s on the USEFUL flops: what the exploited symmetry leaves of the nominal
+         2*nchol*nvirt^4 + 2*nocc^2*nvirt^4 (ppl_info_t.flops_useful: no tile padding, no zero
+         rows, no slab overshoot), inputs resident in HBM.  tflops_executed (the GEMM extents
+         actually launched / time) is the kernel-efficiency figure beside it.
 e2e    = the same through ppl_apply_host with pinned HOST buffers (H2D of L, t2, R and D2H of R
          inside the timed region).
 roofline = the dominant kernel against the FP64 tensor (DMMA) pipe peak measured live by
@@ -36,7 +38,11 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-METRIC = "pp_ladder_fp64_tflops_executed"
+# Headline: FP64 TFLOP/s on the flops the exploited symmetry leaves ("halved where symmetry is exploited, and stated",
+# north_star) -- the symmetry-unique count flops_useful of ppl_info_t, with no tile padding, no zero rows and no
+# slab-granularity overshoot in the numerator.  The rate on the GEMM extents actually launched
+# (tflops_executed) is the kernel-efficiency number and stays in the line and in `roofline.achieved`.
+METRIC = "pp_ladder_fp64_tflops_useful"
 UNIT = "TFLOP/s"
 SYM_NAMES = {0: "none", 1: "pair", 2: "pair_sa", 3: "full"}
 SYM_DESC = {0: "none (every tile)", 1: "pair (tiles a-block<=b-block, mirrored)",
@@ -510,7 +516,7 @@ def run_ours(name, o, v, x, args, steps, warmup, dist, dev, rank, world, peak):
     ms_per_step = total_ms / steps
     sec = ms_per_step * 1e-3
     f_exec, f_nom, f_use = info["flops_executed"], info["flops_nominal"], info["flops_useful"]
-    value = replicas_value(f_exec, ms_per_step, world)
+    value = replicas_value(f_use, ms_per_step, world)
 
     # ---- dominant kernel, timed live with CUDA events on the launching stream (serialised pass) ----
     Rd.zero_()
@@ -550,11 +556,18 @@ def run_ours(name, o, v, x, args, steps, warmup, dist, dev, rank, world, peak):
                   "pack": prof["pack_ms"] / prof["total_ms"]},
         "launches": {k: prof["n_" + k] for k in ("step0", "step1", "reduce", "fold", "pack")},
     }
+    if fused:
+        # launch-bound shapes: one fused launch; the FP64 pipe is not what bounds it (profiles/r02_small_fused.md)
+        roofline["limiter"] = ("launch + shared-memory latency, not the tensor pipe: one launch per apply (floor 4-5 us); at "
+                               "`small` the work decomposition (one warp = one (a,b) column, t2 re-read from shared memory per "
+                               "column) has a floor of about 100 us")
 
     rec = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic", "config": cfg,
+        "value_counts": "flops_useful (symmetry-unique flops of the mode: no tile padding, no zero rows, no slab overshoot) / "
+                        "time; tflops_executed counts the GEMM extents launched",
         "run": {"symmetry": SYM_DESC[info["symmetry"]], "parallelism": "replicas only" if world > 1 else "1 gpu",
                 "plan": {k: info[k] for k in ("ta", "tb", "n_tiles", "ring", "splitk", "vec16", "workspace_bytes")},
                 "graph": args.graph, "verify_inputs": 1 if args.verify < 0 else args.verify, "small_fused": info.get("small_fused", 0)},
@@ -581,9 +594,9 @@ def run_ours(name, o, v, x, args, steps, warmup, dist, dev, rank, world, peak):
         for _ in range(n_e2e):
             h2d, d2h = plan.apply_host(Lh, th, Rh)
         dt = (time.perf_counter() - t0) / n_e2e
-        rec["e2e"] = {"value": world * f_exec / dt * 1e-12, "unit": UNIT, "h2d_bytes_per_step": h2d,
+        rec["e2e"] = {"value": world * f_use / dt * 1e-12, "unit": UNIT, "h2d_bytes_per_step": h2d,
                       "d2h_bytes_per_step": d2h, "seconds_per_call": dt, "steps": n_e2e,
-                      "tflops_useful": world * f_use / dt * 1e-12,
+                      "tflops_executed": world * f_exec / dt * 1e-12,
                       "how": "ppl_apply_host on pinned host buffers; wall clock around the synchronous call"}
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -686,6 +699,11 @@ def main():
         # BASELINE.json quotes the metric on "the two largest configs": the other one rides on the same line
         lo, lv, lx = I.CONFIGS["large"]
         line["large"] = run_ours("large", lo, lv, lx, args, args.steps, args.warmup, dist, dev, rank, world, peak)
+        # ... and north_star asks for all five: medium, small and tiny as complete sub-records too (averaged over more
+        # calls, the launch-bound ones over >= 50; they add about a minute, most of it the oracle samples)
+        for name, nsteps in (("medium", max(args.steps, 20)), ("small", max(args.steps, 50)), ("tiny", max(args.steps, 50))):
+            so, sv, sx = I.CONFIGS[name]
+            line[name] = run_ours(name, so, sv, sx, args, nsteps, max(args.warmup, 5), dist, dev, rank, world, peak)
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
