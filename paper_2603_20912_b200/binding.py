@@ -309,7 +309,13 @@ class Plan:
         return self
 
     def __exit__(self, *exc):
-        self.destroy()
+        if exc[0] is None:
+            self.destroy()
+            return
+        try:  # an exception is already on its way out of the with-block: a late PPL_ERR_PRECONDITION must not mask it
+            self.destroy()
+        except PplError:
+            pass
 
     def __del__(self):
         try:

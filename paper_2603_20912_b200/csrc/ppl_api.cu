@@ -91,6 +91,8 @@ void free_plan(ppl_plan_s *p) {
     if (p->vflags_host) cudaFreeHost(p->vflags_host);
     if (p->vdone_dev) cudaFree(p->vdone_dev);
     if (p->ev_verify) cudaEventDestroy(p->ev_verify);
+    for (cudaEvent_t e : {p->ev_vq[0], p->ev_vq[1]})
+        if (e) cudaEventDestroy(e);
     if (p->tperm) cudaFree(p->tperm);
     if (p->dL) cudaFree(p->dL);
     if (p->dT) cudaFree(p->dT);
@@ -365,11 +367,14 @@ int launch_fold(const ppl_plan_s *p, const double *X, int rows, double *Wp, doub
 }
 
 // t2 (either storage order) -> tau+ [Mp][ldp], tau- [Mm][ldm]
-// rows [row0, row1) of the flattened (i,j) index (default: all); t2 is the address of element (0,0,0,0) -- when the
-// amplitudes are packed chunk by chunk (ppl_apply_host) only the rows of the chunk are dereferenced
-int launch_pack(const ppl_plan_s *p, const double *t2, int layout, double diag, cudaStream_t s, int row0 = 0, int row1 = -1) {
+// rows [row0, row1) of the flattened (i,j) index (default: all).  t2 is the address of element (0,0,0,0) and roff_bias 0; when
+// the amplitudes are packed chunk by chunk (ppl_apply_host) t2 is the staged chunk's own base and roff_bias the number of
+// elements the array would have in front of it (row0 * nvirt^2): no pointer outside the chunk is ever formed
+int launch_pack(const ppl_plan_s *p, const double *t2, int layout, double diag, cudaStream_t s, int row0 = 0, int row1 = -1,
+                int64_t roff_bias = 0) {
     ppl::FoldArgs a;
     a.src = t2;
+    a.roff_bias = roff_bias;
     const ppl::RStrides ts = r_strides(p->o, p->v, layout);  // t2[i,j,c,d] has the strides of R[i,j,a,b]
     a.sc = ts.a;
     a.s_row = 0;
@@ -699,7 +704,7 @@ inline int step0_hints(const ppl_plan_s *p) { return p->dbg.full_hints == 0 ? 13
 // strip is single-buffered), prof as in run_apply.
 enum { FULL_PACK = 1, FULL_COMPUTE = 2, FULL_UNPACK = 4, FULL_ALL = 7 };
 int launch_unpack_full(const ppl_plan_s *p, const ppl_opts_t &opts, double *R, int64_t idx0, int64_t idx1, cudaStream_t stream,
-                       int a0 = 0, int na = -1, const ppl::RStrides *rs = nullptr);
+                       int a0 = 0, int na = -1, const ppl::RStrides *rs = nullptr, int64_t r_bias = 0);
 
 // phases: FULL_PACK (t2 -> tau+-, clear R+-acc), FULL_COMPUTE (all slabs), FULL_UNPACK (R+-acc -> R).  ppl_apply runs all
 // three; ppl_apply_host packs and unpacks chunk by chunk itself and calls this with FULL_COMPUTE only (t2, R unused).
@@ -983,9 +988,10 @@ int run_apply_full(ppl_plan_s *p, const double *L, const double *t2, double *R, 
 }
 
 // R[idx] = beta R + alpha (R+ +- R-) for the flattened (i,j,a,b) indices [idx0, idx1); R is the address of element (0,0,0,0)
-// na < 0: all a's, R in the caller's layout; else the a's [a0, a0 + na) with R addressed through *rs (a slab buffer)
+// na < 0: all a's, R in the caller's layout; else the a's [a0, a0 + na) with R addressed through *rs (a slab buffer: R is its
+// own base, r_bias = a0 * rs->a the elements the full array would have in front of it)
 int launch_unpack_full(const ppl_plan_s *p, const ppl_opts_t &opts, double *R, int64_t idx0, int64_t idx1, cudaStream_t stream, int a0,
-                       int na, const ppl::RStrides *rs) {
+                       int na, const ppl::RStrides *rs, int64_t r_bias) {
     ppl::UnpackArgs u;
     u.rp = p->raccp;
     u.rm = p->raccm;
@@ -998,6 +1004,7 @@ int launch_unpack_full(const ppl_plan_s *p, const ppl_opts_t &opts, double *R, i
     u.beta = opts.beta;
     u.rs = rs ? *rs : r_strides(p->o, p->v, opts.r_layout);
     u.R = R;
+    u.r_bias = r_bias;
     u.idx0 = idx0;
     u.idx1 = idx1;
     u.a0 = na < 0 ? 0 : a0;
@@ -1051,7 +1058,9 @@ ppl_plan_t *ppl_plan_ex(int nocc, int nvirt, int nchol, size_t workspace_bytes, 
     if (cudaMalloc(&p->ws, p->ws_bytes) != cudaSuccess ||
         cudaHostAlloc(&p->vflags_host, 32 * sizeof(int), cudaHostAllocMapped) != cudaSuccess ||
         cudaMalloc(&p->vdone_dev, 2 * sizeof(int)) != cudaSuccess || cudaMemset(p->vdone_dev, 0, 2 * sizeof(int)) != cudaSuccess ||
-        cudaEventCreateWithFlags(&p->ev_verify, cudaEventDisableTiming) != cudaSuccess) {
+        cudaEventCreateWithFlags(&p->ev_verify, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&p->ev_vq[0], cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&p->ev_vq[1], cudaEventDisableTiming) != cudaSuccess) {
         (void)cudaGetLastError();
         free_plan(p);
         fail(PPL_ERR_ALLOC);
@@ -1238,7 +1247,7 @@ int run_apply_small(ppl_plan_s *p, const double *L, const double *t2, double *R,
     PPL_CUDA(cudaGetLastError());
     if (fused_check) {
         if (p->vq_n < 2) p->vq_seq[p->vq_n++] = a.seq;
-        p->vstream = stream;
+        PPL_CUDA(cudaEventRecord(p->ev_vq[a.seq & 1], stream));
     }
     if (prof && prof->mark(K_STEP0, 1 + ((pack_L || pack_t) ? 1 : 0), stream) != PPL_OK) return fail(PPL_ERR_CUDA);
     return PPL_OK;
@@ -1479,7 +1488,8 @@ int launch_check(const ppl_plan_s *p, const double *L, const double *t2, int t2_
 // mapped host memory; wait_all = false (the head of the next apply) does not wait for the NEWEST of them -- that apply may
 // still be running, and waiting would serialise the host with the device (tiny: 25 instead of 18 us per back-to-back apply)
 // -- but reads it if it is there, and waits for an older one; so a violation is reported by the next call or the one after.
-// Should a launch have died its number never arrives: every so often ask the stream, and stop once it has drained.
+// Should a launch have died its number never arrives: every so often ask the event recorded behind that launch (on whichever
+// stream the caller gave for it), and stop once it has completed.
 int verify_harvest(ppl_plan_s *p, int *flags_out, bool wait_all) {
     if (flags_out) *flags_out = 0;
     int h = 0;
@@ -1500,7 +1510,7 @@ int verify_harvest(ppl_plan_s *p, int *flags_out, bool wait_all) {
         if (!must && w[4] != seq) break;
         for (unsigned spin = 1; w[4] != seq; ++spin) {
             if ((spin & 0x3ff) == 0) {
-                const cudaError_t e = cudaStreamQuery(p->vstream);
+                const cudaError_t e = cudaEventQuery(p->ev_vq[slot]);  // complete <=> the launch of this check has left the GPU
                 if (e == cudaErrorNotReady) continue;
                 if (e != cudaSuccess || w[4] != seq) {
                     (void)cudaGetLastError();
@@ -1589,7 +1599,7 @@ int step1_tile(const ppl_plan_s *p, const CUtensorMap *mapT, const double *t2, i
 }
 
 int reduce_tile(const ppl_plan_s *p, const Tile &t, double *R, int64_t si, int64_t sj, int64_t sa, int64_t sb, double alpha,
-                double beta, cudaStream_t s) {
+                double beta, cudaStream_t s, int64_t r_bias) {
     ppl::ReduceArgs a;
     a.part = p->part;
     a.splitk = t.full.splitk;
@@ -1609,6 +1619,7 @@ int reduce_tile(const ppl_plan_s *p, const Tile &t, double *R, int64_t si, int64
     a.rs.a = sa;
     a.rs.b = sb;
     a.R = R;
+    a.r_bias = r_bias;
     const int64_t MN = (int64_t)a.M * a.N;
     const int grid = (int)std::min<int64_t>((MN + 255) / 256, (int64_t)p->num_sms * 8);
     ppl::k_reduce<<<grid, 256, 0, s>>>(a);
@@ -1616,15 +1627,15 @@ int reduce_tile(const ppl_plan_s *p, const Tile &t, double *R, int64_t si, int64
     return PPL_OK;
 }
 
-int pack_rows(const ppl_plan_s *p, const double *t2, double diag, cudaStream_t s, int row0, int row1) {
-    return launch_pack(p, t2, PPL_LAYOUT_IJAB, diag, s, row0, row1);
+int pack_rows(const ppl_plan_s *p, const double *chunk, double diag, cudaStream_t s, int row0, int row1) {
+    return launch_pack(p, chunk, PPL_LAYOUT_IJAB, diag, s, row0, row1, (int64_t)row0 * p->vv);
 }
 
-// rows [row0, row1) of t2 (staged; t2 = address of element (0,0,0,0)) against the tau+- rows their mirror images wrote:
+// rows [row0, row1) of t2 (the staged chunk, row row0 first) against the tau+- rows their mirror images wrote:
 // sets bit 1 of the per-apply verification flags (the words verify_begin cleared), see k_check_t2_rows
-int check_rows(const ppl_plan_s *p, const double *t2, double diag, cudaStream_t s, int row0, int row1) {
+int check_rows(const ppl_plan_s *p, const double *chunk, double diag, cudaStream_t s, int row0, int row1) {
     ppl::CheckRowsArgs a;
-    a.t2 = t2;
+    a.t2 = chunk;
     a.taup = p->taup;
     a.taum = p->taum;
     a.ldp = p->ldp;
@@ -1664,7 +1675,7 @@ int unpack_slab(const ppl_plan_s *p, double *slab, int a0, int na, cudaStream_t 
     rs.j = (int64_t)na * p->v;
     rs.a = p->v;
     rs.b = 1;
-    return launch_unpack_full(p, opts, slab - (int64_t)a0 * p->v, 0, (int64_t)p->o * p->o * na * p->v, s, a0, na, &rs);
+    return launch_unpack_full(p, opts, slab, 0, (int64_t)p->o * p->o * na * p->v, s, a0, na, &rs, (int64_t)a0 * rs.a);
 }
 
 int verify_begin(ppl_plan_s *p, const double *L, const double *t2, int t2_layout, cudaStream_t stream) {

@@ -141,14 +141,14 @@ static int apply_host_full_queue(ppl_plan_s *p, const double *Lh, const double *
         cudaStream_t s = st[k & 1];
         double *buf = p->hstage[k & 1];
         PPL_CUDA(cudaMemcpyAsync(buf, t2h + r0 * p->vv, (size_t)(r1 - r0) * row_bytes, cudaMemcpyHostToDevice, s));
-        int rc = pplapi::pack_rows(p, buf - r0 * p->vv, 0.5, s, (int)r0, (int)r1);
+        int rc = pplapi::pack_rows(p, buf, 0.5, s, (int)r0, (int)r1);
         if (rc != PPL_OK) return rc;
         if (p->verify) {
             // pair symmetry of t2: the rows i >= j of the chunk against the tau+- rows their mirror images (j,i) <= (i,j)
             // wrote -- in this chunk, in chunk k - 2, k - 4, ... (this stream) or in chunk k - 1, k - 3, ... (the other one)
             PPL_CUDA(cudaEventRecord(p->hsn.ev_chunk[k & 1], s));
             if (k > 0) PPL_CUDA(cudaStreamWaitEvent(s, p->hsn.ev_chunk[(k - 1) & 1], 0));
-            rc = pplapi::check_rows(p, buf - r0 * p->vv, 0.5, s, (int)r0, (int)r1);
+            rc = pplapi::check_rows(p, buf, 0.5, s, (int)r0, (int)r1);
             if (rc != PPL_OK) return rc;
         }
     }
@@ -361,7 +361,7 @@ static int apply_host_tiles_queue(ppl_plan_s *p, const double *Lh, const double 
             if (first) PPL_CUDA(cudaStreamWaitEvent(cs, h.ev_rsin[ra], 0));
             // the slab holds R[i][j][a - a0][b]: strides (o ta v, ta v, v, 1) from the address element (0,0,0,0) would have
             const int64_t tav = (int64_t)t.ta * v;
-            rc = pplapi::reduce_tile(p, t, h.rs[ra] - (int64_t)t.a0 * v, (int64_t)p->o * tav, tav, v, 1, 1.0, 1.0, cs);
+            rc = pplapi::reduce_tile(p, t, h.rs[ra], (int64_t)p->o * tav, tav, v, 1, 1.0, 1.0, cs, (int64_t)t.a0 * v);
         } else {
             rc = pplapi::reduce_tile(p, t, p->dR, (int64_t)p->o * p->vv, p->vv, v, 1, 1.0, 1.0, cs);
         }

@@ -291,7 +291,9 @@ struct ReduceArgs {
     int mirror;          // 1: also write R[j,i,b,a]
     double alpha, beta;
     RStrides rs;
-    double *R;
+    double *R;           // base of the array the strides address ...
+    int64_t r_bias = 0;  // ... after this many elements are subtracted from the offset: 0 for the caller's R; a slab buffer that
+                         // holds only the a's from a0 on passes its own base and a0 * rs.a (no pointer is formed outside it)
 };
 
 __global__ void __launch_bounds__(256) k_reduce(const ReduceArgs p) {
@@ -303,8 +305,8 @@ __global__ void __launch_bounds__(256) k_reduce(const ReduceArgs p) {
         const int al = n / p.tb, bl = n - al * p.tb;
         const int a = p.a0 + al, b = p.b0 + bl;
         const int i = m / p.o, j = m - i * p.o;
-        r_update(p.R + i * p.rs.i + j * p.rs.j + a * p.rs.a + b * p.rs.b, s, p.alpha, p.beta);
-        if (p.mirror) r_update(p.R + j * p.rs.i + i * p.rs.j + b * p.rs.a + a * p.rs.b, s, p.alpha, p.beta);
+        r_update(p.R + (i * p.rs.i + j * p.rs.j + a * p.rs.a + b * p.rs.b - p.r_bias), s, p.alpha, p.beta);
+        if (p.mirror) r_update(p.R + (j * p.rs.i + i * p.rs.j + b * p.rs.a + a * p.rs.b - p.r_bias), s, p.alpha, p.beta);
     }
 }
 
@@ -320,7 +322,8 @@ struct FoldArgs {
     const double *src;   // row r, element (c,d) at src + roff(r) + c*sc + d   (d contiguous)
     int64_t sc;          // stride of c
     int64_t s_row;       // mode 0: row r at r*s_row;  mode 2: row (a_l, b) at (a_l*v + b)*s_row
-    int64_t s_i, s_j;    // mode 1: row (i,j) at i*s_i + j*s_j
+    int64_t s_i, s_j;    // mode 1: row (i,j) at i*s_i + j*s_j - roff_bias
+    int64_t roff_bias = 0;  // mode 1: elements in front of src that the array would have (a staged chunk of rows passes its own base)
     int mode;            // 0: fold W tile rows (every row has + and -); 1: pack amplitudes, rows (i<=j) of an o x o grid; 3: see below;
                          // 2: PPL_SYM_FULL: rows r = a_l*tbp + b_l of the tile (A; b-group) taken from the slab's strip;
                          //    rows with a > b, b >= v or a_l >= ta are written as zeros; only c >= A0 is touched
@@ -389,7 +392,7 @@ __device__ __forceinline__ FoldRow fold_row(const FoldArgs &p, int r) {
     } else {
         const int i = r / p.o, j = r - i * p.o;
         f.skip = i > j;
-        f.roff = i * p.s_i + j * p.s_j;
+        f.roff = i * p.s_i + j * p.s_j - p.roff_bias;
         f.rowp = (int64_t)i * p.o - (int64_t)i * (i - 1) / 2 + (j - i);
         f.rowm = (i < j) ? (int64_t)i * (2 * p.o - i - 1) / 2 + (j - i - 1) : -1;
     }
@@ -622,7 +625,7 @@ __global__ void __launch_bounds__(256) k_check_inputs(const CheckArgs p) {
 // One item = one such row x one pair (c-block <= d-block) of 32 x 32 blocks, staged through shared memory as in
 // check_inputs_scan so that both the block and its transpose are read coalesced.
 struct CheckRowsArgs {
-    const double *t2;       // address of element (0,0,0,0) of the dense [i][j][c][d] array; only rows [row0, row1) are dereferenced
+    const double *t2;       // the staged chunk: rows [row0, row1) of the dense [i][j][c][d] array, row row0 first
     const double *taup, *taum;
     int64_t ldp, ldm;
     int row0, row1;         // rows of the flattened (i,j) index held by the staged chunk
@@ -648,7 +651,7 @@ __global__ void __launch_bounds__(256) k_check_t2_rows(const CheckRowsArgs p) {
             ++cb;
         }
         const int c0 = cb * 32, d0 = (cb + rem) * 32;
-        const double *x = p.t2 + (int64_t)r * vv;
+        const double *x = p.t2 + (int64_t)(r - p.row0) * vv;
         __syncthreads();  // the previous item's reads of sa / sb are done
         for (int y = ty; y < 32; y += 8) {
             const int c = c0 + y, d = d0 + tx;

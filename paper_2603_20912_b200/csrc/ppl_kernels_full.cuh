@@ -467,7 +467,8 @@ struct UnpackArgs {
     int vk;              // nvirt of the packed geometry (v rounded up to even)
     double alpha, beta;
     RStrides rs;
-    double *R;
+    double *R;           // base of the array the strides address, after r_bias elements are subtracted from the offset
+    int64_t r_bias = 0;  // 0: the caller's R; a slab buffer holding the a's [a0, a0 + na) passes its own base and a0 * rs.a
     int64_t idx0, idx1;  // range of the flattened (i,j,a_l,b) index that is written (all: 0, o^2 na v)
     int a0, na;          // the a's covered: a = a0 + a_l, a_l < na (all: 0, v).  A slab of a's is complete as soon as its own slab
                          // of the PPL_SYM_FULL loop is: ppl_apply_host unpacks and ships R[:, :, slab, :] while later slabs run
@@ -486,7 +487,7 @@ __global__ void __launch_bounds__(256) k_unpack_full(const UnpackArgs p) {
             const double rm = p.rm[rowminus(i1, j1, p.o) * p.ldm + kminus(a1, b1, p.vk)];
             val += ((i > j) == (a > b)) ? rm : -rm;
         }
-        r_update(p.R + i * p.rs.i + j * p.rs.j + a * p.rs.a + b * p.rs.b, val, p.alpha, p.beta);
+        r_update(p.R + (i * p.rs.i + j * p.rs.j + a * p.rs.a + b * p.rs.b - p.r_bias), val, p.alpha, p.beta);
     }
 }
 

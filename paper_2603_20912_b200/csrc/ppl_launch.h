@@ -16,16 +16,18 @@ int step0_tile(const ppl_plan_s *p, const pplh::Tile &t, const CUtensorMap *mapA
 // step 1 of one W tile of the un-packed modes out of ring slot `slot` into the plan's split-K partials; mapT: t2 as
 // {inner = nvirt^2, outer = nocc^2}, box {BK, step1_tile_m}
 int step1_tile(const ppl_plan_s *p, const CUtensorMap *mapT, const double *t2, int slot, const pplh::Tile &t, cudaStream_t s);
-// fixed-order sum of the partials into R[i,j,a,b] (+ the mirror if the tile has one); R = address of element (0,0,0,0)
-// with element strides (si, sj, sa, sb): the caller's array, or a slab buffer that holds only the tile's a-block
+// fixed-order sum of the partials into R[i,j,a,b] (+ the mirror if the tile has one); R with element strides (si, sj, sa, sb)
+// and r_bias = 0: the caller's array from element (0,0,0,0); a slab buffer that holds only the tile's a-block: its own base
+// and r_bias = a0 * sa, the elements the whole array would have in front of it (the kernel subtracts them from the offset)
 int reduce_tile(const ppl_plan_s *p, const pplh::Tile &t, double *R, int64_t si, int64_t sj, int64_t sa, int64_t sb, double alpha,
-                double beta, cudaStream_t s);
+                double beta, cudaStream_t s, int64_t r_bias = 0);
 uint32_t step1_box_rows(const ppl_plan_s *p);  // TMA box rows of the t2 map of step1_tile
 
 // PPL_SYM_FULL pieces (ppl_apply_host packs and unpacks chunk by chunk)
-int pack_rows(const ppl_plan_s *p, const double *t2, double diag, cudaStream_t s, int row0, int row1);
+// chunk: rows [row0, row1) of t2, row row0 first (the staging buffer itself)
+int pack_rows(const ppl_plan_s *p, const double *chunk, double diag, cudaStream_t s, int row0, int row1);
 // verification of a staged chunk: its rows i >= j against what the rows i <= j packed (bit 1 of the per-apply flags)
-int check_rows(const ppl_plan_s *p, const double *t2, double diag, cudaStream_t s, int row0, int row1);
+int check_rows(const ppl_plan_s *p, const double *chunk, double diag, cudaStream_t s, int row0, int row1);
 int unpack_range(const ppl_plan_s *p, double *R, int64_t idx0, int64_t idx1, cudaStream_t s);
 // all slabs on the packed operands.  hook (may be null): called behind the launches of every slab with the two streams whose
 // work so far completes the R+-acc columns of that slab's a's [a0, a0 + na)

@@ -109,7 +109,9 @@ struct ppl_plan_s {
     int *vdone_dev = nullptr;              // [2] device counters of finished check CTAs, one per slot
     int vseq = 0;                          // sequence number of the last fused check
     int vq_seq[2] = {0, 0}, vq_n = 0;      // outstanding sequence numbers
-    cudaStream_t vstream = nullptr;        // the stream the last one was launched on
+    cudaEvent_t ev_vq[2] = {nullptr, nullptr};  // one per slot, recorded right behind the fused launch on ITS stream: what the
+                                           // harvest asks when the sequence number is slow to arrive (the caller's streams are
+                                           // borrowed and may differ between applies or be destroyed; an event stays valid)
     std::vector<pplh::Tile> tiles;
     cudaStream_t gen = nullptr, host_stream = nullptr;
     cudaEvent_t ev_in = nullptr, ev_ready[pplh::MAX_RING] = {}, ev_free[pplh::MAX_RING] = {};

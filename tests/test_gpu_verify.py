@@ -168,3 +168,37 @@ def test_host_entry_point_checks_t2_chunk_by_chunk_in_the_default_mode(shape, ch
         R = np.zeros((o, o, v, v))
         plan.apply_host(L, ts, R)
         assert relerr(R, oracle.full(L, ts)) <= 1e-11
+
+
+def test_with_block_does_not_mask_the_callers_exception_and_checks_survive_their_stream():
+    """(1) Plan.__exit__ used to raise PPL_ERR_PRECONDITION from destroy() over an exception already leaving the
+    with-block; (2) on the one-kernel path the outstanding checks are now followed by events of their own, so a caller may
+    issue applies on different streams and destroy a stream while a check is still outstanding."""
+    import torch
+
+    o, v, x = 5, 20, 60
+    L = I.make_L(v, x, 1, symmetric=True)
+    ts, tn = I.make_t2(o, v, 1, symmetric=True), I.make_t2(o, v, 1, symmetric=False)
+    Ld, tsd, tnd = _dev(L, ts, tn)
+    Rd = torch.zeros((o, o, v, v), dtype=torch.float64, device="cuda")
+    with pytest.raises(KeyError):
+        with P.Plan(o, v, x, debug={"no_small_fused": 0}) as plan:
+            assert plan.info()["small_fused"] == 1
+            plan.apply(Ld, tnd, Rd)  # violation, still unreported when the block is left ...
+            raise KeyError("the caller's own error")  # ... by this exception, which must come out
+    with P.Plan(o, v, x, debug={"no_small_fused": 0}) as plan:
+        s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+        torch.cuda.synchronize()
+        plan.apply(Ld, tsd, Rd, s1)
+        s2.wait_stream(s1)           # one apply of a plan in flight at a time (include/ppl.h, Threading)
+        plan.apply(Ld, tnd, Rd, s2)  # two checks outstanding, on two streams
+        del s1, s2                   # (torch returns them to its pool; an event would survive a destroyed stream as well)
+        with pytest.raises(P.PplError) as e:
+            plan.verify_status()
+        assert e.value.code == P.PPL_ERR_PRECONDITION
+        torch.cuda.synchronize()
+        Rd.zero_()
+        plan.apply(Ld, tsd, Rd)
+        assert plan.verify_status() == 0
+        torch.cuda.synchronize()
+        assert relerr(Rd.cpu().numpy(), oracle.full(L, ts)) <= 1e-11
