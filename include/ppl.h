@@ -27,6 +27,9 @@
  *     compute-capability 10.x device the library refuses (PPL_ERR_UNSUPPORTED_DEVICE).
  *   - Threading: one in-flight ppl_apply per plan (the workspace is shared); distinct plans are
  *     independent.  ppl_last_error() is per thread.
+ *   - Devices: a plan belongs to the CUDA device that was current when ppl_plan ran (its workspace, streams and
+ *     events live there).  Every entry point that takes a plan returns PPL_ERR_INVALID_ARG when the calling
+ *     thread's current device is another one; make the plan's device current first (cudaSetDevice).
  */
 #ifndef PPL_H
 #define PPL_H

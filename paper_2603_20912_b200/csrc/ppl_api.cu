@@ -401,8 +401,20 @@ int launch_pack(const ppl_plan_s *p, const double *t2, int layout, double diag, 
     return PPL_OK;
 }
 
+// The plan's workspace, streams and events belong to the device ppl_plan ran on; a call from a thread whose current device
+// is another one would launch there against this device's memory.
+bool device_ok(const ppl_plan_s *p) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return false;
+    }
+    return dev == p->device;
+}
+
 int check_ptrs(const ppl_plan_s *p, const double *L, const double *t2, const double *R, bool *vec16) {
     if (!p || !L || !t2 || !R) return PPL_ERR_INVALID_ARG;
+    if (!device_ok(p)) return PPL_ERR_INVALID_ARG;
     const uintptr_t all = (uintptr_t)L | (uintptr_t)t2 | (uintptr_t)R;
     if (all & 7) return PPL_ERR_INVALID_ARG;
     *vec16 = p->vec16 && ((all & 15) == 0);
@@ -1051,6 +1063,7 @@ ppl_plan_t *ppl_plan_ex(int nocc, int nvirt, int nchol, size_t workspace_bytes, 
     const bool use_tma = !(dbg && dbg->cpasync_kernels) && get_encode() != nullptr;
     int rc_host = PPL_OK;
     ppl_plan_s *p = plan_host(nocc, nvirt, nchol, workspace_bytes, cap, prop.multiProcessorCount, use_tma, dbg, &rc_host);
+    if (p) p->device = dev;
     if (!p) {
         fail(rc_host);
         return nullptr;
@@ -1310,7 +1323,7 @@ int apply_graph(ppl_plan_s *p, const double *L, const double *t2, double *R, con
 
 int ppl_apply_ex(ppl_plan_t *p, const double *L, const double *t2, double *R, const ppl_opts_t *opts, void *stream_) {
     cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
-    if (!p || !L || !t2 || !R) return fail(PPL_ERR_INVALID_ARG);
+    if (!p || !L || !t2 || !R || !device_ok(p)) return fail(PPL_ERR_INVALID_ARG);
     // a caller who is capturing `stream` gets the plain launches recorded into their own graph (and no input check:
     // its result could not be read back during the capture)
     cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
@@ -1546,7 +1559,7 @@ int verify_begin(ppl_plan_s *p, const double *L, const double *t2, int t2_layout
 extern "C" {
 
 int ppl_check_inputs(ppl_plan_t *p, const double *L, const double *t2, void *stream_, int *flags) {
-    if (!p || !L || !t2) return fail(PPL_ERR_INVALID_ARG);
+    if (!p || !L || !t2 || !device_ok(p)) return fail(PPL_ERR_INVALID_ARG);
     cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
     const int rc = launch_check(p, L, t2, PPL_LAYOUT_IJAB, p->vflags_host + 2, stream);
     if (rc != PPL_OK) return rc;

@@ -421,7 +421,12 @@ static int apply_host_tiles(ppl_plan_s *p, const double *Lh, const double *t2h, 
 extern "C" {
 
 int ppl_apply_host(ppl_plan_t *p, const double *Lh, const double *t2h, double *Rh, uint64_t *h2d, uint64_t *d2h) {
+    int cur = -1;
     if (!p || !Lh || !t2h || !Rh) return fail(PPL_ERR_INVALID_ARG);
+    if (cudaGetDevice(&cur) != cudaSuccess || cur != p->device) {  // the plan's buffers and streams live on its own device
+        (void)cudaGetLastError();
+        return fail(PPL_ERR_INVALID_ARG);
+    }
     const bool aligned = (((uintptr_t)Lh | (uintptr_t)t2h | (uintptr_t)Rh) & 7) == 0;
     if (p->sym == PPL_SYM_FULL && p->full_ok && aligned) return apply_host_full(p, Lh, t2h, Rh, h2d, d2h);
     if ((p->sym == PPL_SYM_NONE || p->sym == PPL_SYM_PAIR) && p->use_tma && p->vec16 && aligned && !p->small_ok)

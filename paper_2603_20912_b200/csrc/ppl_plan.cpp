@@ -74,7 +74,8 @@ SplitChoice choose_split(int M, int N, int64_t K, int sms, const MGeom &mg, size
 }
 
 double step0_seconds(int ta, int tb, int v, int x, int sms) {
-    const int tiles = ((ta * v + ppl::BM - 1) / ppl::BM) * ((tb * v + ppl::BN - 1) / ppl::BN);
+    // (64-bit: with nvirt >= 2431 a whole-range tile edge has more than 2^31 CTA tiles -- found by UBSan, tests/test_planner_sanitizers_cpu.py)
+    const int64_t tiles = (((int64_t)ta * v + ppl::BM - 1) / ppl::BM) * (((int64_t)tb * v + ppl::BN - 1) / ppl::BN);
     const int nkt = (x + ppl::BK - 1) / ppl::BK;
     const double tau = 2.0 * ppl::BM * ppl::BN * ppl::BK / (PEAK_FLOPS / sms);
     return std::ceil((double)tiles / sms) * (nkt + 6) * tau;

@@ -79,6 +79,7 @@ struct ppl_plan_s {
     int ring = 1;
     int vec16 = 0;
     int num_sms = 148;
+    int device = -1;      // the CUDA device ppl_plan ran on: workspace, streams and events live there (-1: ppl_plan_dry)
     int use_tma = 0;      // 1: persistent TMA/mbarrier kernels; 0: cp.async kernels
     int64_t vv = 0;       // nvirt^2 = row length of an un-packed W tile / of t2
     int vp = 0;           // nvirt rounded up to even: the geometry of every PACKED operand (tau+-, W+-, R+-acc) and of the
