@@ -449,6 +449,74 @@ def contract_leg():
     print(json.dumps(out))
 
 
+def entry_points_leg(peak, plain_seconds):
+    """The widened entry points at `large`: seconds and TFLOP/s of ppl_apply_ex in the paper's storage
+    orders ('icjd' -> 'iajb', alpha != 1, beta = 0; the permutation is folded into the pack / unpack kernels),
+    of ppl_generate_eri + ppl_apply_dense on one slab of 16 a's, and of ppl_contract_pair on the ladder's strings."""
+    import torch
+
+    import paper_2603_20912_b200 as P
+    import ppl_inputs as I
+
+    o, v, x = I.CONFIGS["large"]
+    Ld = torch.from_numpy(I.make_L(v, x, 0)).cuda()
+    td = torch.from_numpy(I.make_t2(o, v, 0)).cuda()
+    t_icjd = td.permute(0, 2, 1, 3).contiguous()
+    R_iajb = torch.empty((o, v, o, v), dtype=torch.float64, device="cuda")
+    Rd = torch.zeros((o, o, v, v), dtype=torch.float64, device="cuda")
+
+    def timed(fn, n=3, warm=1):
+        for _ in range(warm):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n * 1e-3
+
+    out = {"workload": "large", "peak": peak, "unit": UNIT}
+    with P.Plan(o, v, x) as plan:
+        info = plan.info()
+        t_ex = timed(lambda: plan.apply_ex(Ld, t_icjd, R_iajb, "iajb", "iajb", alpha=-0.625, beta=0.0))
+        out["apply_ex_iajb_beta0"] = {"seconds_per_call": t_ex, "plain_apply_seconds": plain_seconds,
+                                      "over_plain": t_ex / plain_seconds if plain_seconds else None,
+                                      "tflops_executed": info["flops_executed"] / t_ex * 1e-12,
+                                      "frac_of_peak": info["flops_executed"] / t_ex * 1e-12 / peak}
+        na = 16
+        eri = torch.empty((na, v, v, v), dtype=torch.float64, device="cuda")
+        t_gen = timed(lambda: plan.generate_eri(Ld, 64, na, eri))
+        f_gen = 2.0 * x * na * v ** 3
+        out["generate_eri_16"] = {"seconds_per_call": t_gen, "tflops": f_gen / t_gen * 1e-12, "frac_of_peak": f_gen / t_gen * 1e-12 / peak}
+        t_dense = timed(lambda: plan.apply_dense(eri, 64, td, Rd))
+        f_dense = 2.0 * o * o * na * v ** 3
+        out["apply_dense_16"] = {"seconds_per_call": t_dense, "tflops": f_dense / t_dense * 1e-12,
+                                 "frac_of_peak": f_dense / t_dense * 1e-12 / peak}
+        del eri
+    del Rd, R_iajb, t_icjd
+    torch.cuda.empty_cache()
+    out["contract_pair"] = []
+    for subs, A, B in (("xac,xbd->acbd", Ld[:, 200:204, :].contiguous(), Ld),
+                       ("abcd,ecfd->efab", torch.randn((4, v, v, v), dtype=torch.float64, device="cuda"), td.permute(0, 2, 1, 3).contiguous()),
+                       ("ik,kj->ij", torch.randn((4096, 4096), dtype=torch.float64, device="cuda"),
+                        torch.randn((4096, 4096), dtype=torch.float64, device="cuda"))):
+        C = P.ppl_contract_pair(subs, A, B)
+        ins, _ = subs.split("->")
+        s0, s1 = ins.split(",")
+        ext = dict(zip(s0, A.shape))
+        ext.update(zip(s1, B.shape))
+        flops = 2.0
+        for val in ext.values():
+            flops *= val
+        t = timed(lambda: P.ppl_contract_pair(subs, A, B, C), n=5, warm=2)
+        out["contract_pair"].append({"subscripts": subs, "dims0": list(A.shape), "dims1": list(B.shape), "seconds_per_call": t,
+                                     "tflops": flops / t * 1e-12, "frac_of_peak": flops / t * 1e-12 / peak})
+        del A, B, C
+    torch.cuda.empty_cache()
+    return out
+
+
 def run_ours(name, o, v, x, args, steps, warmup, dist, dev, rank, world, peak):
     """One workload through ppl_apply (device-resident), ppl_apply_profiled (roofline), ppl_apply_host (e2e) and the
     oracle sample (cpu_baseline + parity).  Returns the JSON record."""
@@ -652,6 +720,8 @@ def main():
                     help="context leg: time STEPS calls of the paper's tensordot recipe (cuBLAS) on the same inputs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--contract", action="store_true", help="only time ppl_contract_pair on the paper's two ladder strings")
+    ap.add_argument("--entry-points", action="store_true", help="only the entry_points record (ppl_apply_ex in the paper's layouts, "
+                    "ppl_generate_eri + ppl_apply_dense, ppl_contract_pair) at large")
     ap.add_argument("--probe", action="store_true", help="only measure the FP64 instruction-stream peaks and print them")
     args = ap.parse_args()
 
@@ -662,6 +732,14 @@ def main():
         return
     if args.contract:
         contract_leg()
+        return
+    if args.entry_points:
+        import torch
+
+        import paper_2603_20912_b200 as P
+
+        torch.cuda.set_device(0)
+        print(json.dumps(entry_points_leg(P.ppl_probe_fp64_peak(3, 20.0), None)))
         return
     if args.shape:
         o, v, x = (int(t) for t in args.shape.split(","))
@@ -699,6 +777,8 @@ def main():
         # BASELINE.json quotes the metric on "the two largest configs": the other one rides on the same line
         lo, lv, lx = I.CONFIGS["large"]
         line["large"] = run_ours("large", lo, lv, lx, args, args.steps, args.warmup, dist, dev, rank, world, peak)
+        if rank == 0 and world == 1:
+            line["entry_points"] = entry_points_leg(peak, line["large"]["seconds_per_call"])
         # ... and north_star asks for all five: medium, small and tiny as complete sub-records too (averaged over more
         # calls, the launch-bound ones over >= 50; they add about a minute, most of it the oracle samples)
         for name, nsteps in (("medium", max(args.steps, 20)), ("small", max(args.steps, 50)), ("tiny", max(args.steps, 50))):
