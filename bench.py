@@ -669,7 +669,7 @@ def run_ours(name, o, v, x, args, steps, warmup, dist, dev, rank, world, peak):
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         # ---- the oracle on the host cores, bounded sample; the same sample checks the GPU result ----
-        pairs, cols, dt, cores = oracle_sample(Lh.numpy(), th.numpy(), o, v, x)
+        pairs, cols, dt, cores = oracle_sample(Lh.numpy(), th.numpy(), o, v, x, target_s=getattr(args, "oracle_target_s", 15.0))
         rec["cpu_baseline"] = {
             "value": len(pairs) * col_flops(o, v, x) / dt * 1e-12, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"{len(pairs)} of {v*v} (a,b) columns (oracle.columns), all i,j; {dt:.1f} s",
@@ -720,6 +720,8 @@ def main():
                     help="context leg: time STEPS calls of the paper's tensordot recipe (cuBLAS) on the same inputs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--contract", action="store_true", help="only time ppl_contract_pair on the paper's two ladder strings")
+    ap.add_argument("--sweep", action="store_true", help="molecule-like shapes between medium and large (Table 4 of the paper, "
+                    "PAPER.md:466-507: odd nvirt, nvirt = 8 mod 16, ...): one compact record per shape in one JSON line")
     ap.add_argument("--entry-points", action="store_true", help="only the entry_points record (ppl_apply_ex in the paper's layouts, "
                     "ppl_generate_eri + ppl_apply_dense, ppl_contract_pair) at large")
     ap.add_argument("--probe", action="store_true", help="only measure the FP64 instruction-stream peaks and print them")
@@ -772,6 +774,24 @@ def main():
     dev = torch.device("cuda", local)
     peak = P.ppl_probe_fp64_peak(3, 20.0)
 
+    if args.sweep:
+        # shapes of the medium class, where the paper's molecules live ((H2O)10 / cc-pVDZ is nocc 40, nvirt 190)
+        shapes = [(20, 200, 800), (40, 190, 1150), (40, 191, 1150), (30, 230, 1200), (25, 260, 1300), (40, 264, 1400),
+                  (32, 296, 1500), (48, 312, 1700), (64, 330, 1970), (36, 360, 1800), (40, 400, 1600), (40, 401, 1600),
+                  (50, 450, 2200), (40, 530, 2850)]
+        args.no_e2e, args.oracle_target_s = True, 4.0
+        recs = []
+        for (so, sv, sx) in shapes:
+            r = run_ours(f"sweep_{so}_{sv}_{sx}", so, sv, sx, args, args.steps, args.warmup, dist, dev, rank, world, peak)
+            recs.append({"shape": [so, sv, sx], "seconds_per_call": r["seconds_per_call"], "tflops_executed": r["tflops_executed"],
+                         "tflops_useful": r["tflops_useful"], "frac_executed": r["frac_of_fp64_peak_measured"],
+                         "frac_useful": r["frac_of_fp64_peak_measured_useful"], "executed_over_useful": r["executed_over_useful"],
+                         "share": r["roofline"]["share"], "launches": r["roofline"]["launches"],
+                         "step0_tflops": r["roofline"]["step0_tflops"], "step1_tflops": r["roofline"]["step1_tflops"],
+                         "plan": r["run"]["plan"], "parity": r.get("parity"), "clocks": r["clocks"]})
+        if rank == 0:
+            print(json.dumps({"sweep": recs, "peak": peak, "unit": UNIT, "steps": args.steps, "warmup": args.warmup}))
+        return
     line = run_ours(args.config, o, v, x, args, args.steps, args.warmup, dist, dev, rank, world, peak)
     if args.config == "xl" and not args.no_secondary and not args.shape:
         # BASELINE.json quotes the metric on "the two largest configs": the other one rides on the same line
