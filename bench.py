@@ -158,6 +158,8 @@ def run_reference(args, o, v, x):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": workload_config(args.config, o, v, x),
+        "value_counts": "the oracle's own flops / time: it uses no symmetry, so this is the nominal count per (a,b) column; our arm "
+                        "counts the symmetry-unique flops (1/5 of nominal at xl) -- for seconds per call compare seconds_per_call",
         "seconds_per_call": dt / args.steps / len(pairs) * v * v,
         "seconds_per_call_how": "EXTRAPOLATED: measured seconds per sampled (a,b) column x nvirt^2 columns",
         "cpu_baseline": {"value": tflops, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
